@@ -1,0 +1,132 @@
+/* fem.h — C ABI of the B200-native finite-strain Hill-48 element evaluation + CSR assembly library.
+ *
+ * One call of fem_assemble is one pass of the hot path of the Newton–Raphson FEM loop of
+ * arxiv 2606.17390 ("JAX-FEM-ANISO"): per-quadrature-point logarithmic-strain return mapping
+ * (Alg. C1/C2 :889-982), hex8 element internal force and consistent tangent
+ * (Eq.(35)-(37),(40) :255-296) and assembly into a fixed-pattern global CSR matrix
+ * (Eq.(34),(38) :251-275; Alg. E1 :1037-1049).  Readings of the paper are listed in DESIGN.md.
+ *
+ * Conventions (all calls)
+ *   - units mm / MPa; all floating point is IEEE double; all indices are int32.
+ *   - "dev" = pointer to CUDA device memory of the current device, "host" = ordinary host memory.
+ *   - DOF id = 3*node + component.  Symmetric 2-tensors are 6 tensor components in the order
+ *     (11,22,33,12,23,13) (PAPER.md:779 Eq.(A2), :793-796 Eq.(A4)).
+ *   - hex8 node order of conn[e][0..7]: xi-signs (-,-,-),(+,-,-),(+,+,-),(-,+,-),(-,-,+),(+,-,+),(+,+,+),(-,+,+)
+ *     (trilinear HEX-8); Gauss point q = kx + 2 ky + 4 kz, bit 0 <-> -1/sqrt3, weights 1.
+ *   - every array argument is caller-owned; outputs are caller-allocated and fully overwritten;
+ *     pattern arrays returned by fem_build_csr_pattern are library-owned and live until fem_destroy.
+ *   - every call returns FEM_OK (0) or a negative error code; nothing throws.  There is no CPU fallback:
+ *     without a CUDA device fem_setup returns FEM_ERR_CUDA.
+ */
+#ifndef FEM_B200_H
+#define FEM_B200_H
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define FEM_NPAR 16 /* doubles per material record, see fem_assemble */
+
+enum {
+    FEM_OK = 0,
+    FEM_ERR_NULL = -1,        /* a required pointer is NULL */
+    FEM_ERR_ARG = -2,         /* invalid size / option value */
+    FEM_ERR_QUAD = -3,        /* quad_order != 2 */
+    FEM_ERR_CONN = -4,        /* connectivity index out of [0, n_nodes) */
+    FEM_ERR_INVERTED = -5,    /* det J_ref <= 0 at a Gauss point of some element */
+    FEM_ERR_CUDA = -6,        /* CUDA runtime error (message via fem_last_cuda_error) */
+    FEM_ERR_NO_PATTERN = -7,  /* fem_assemble before fem_build_csr_pattern */
+    FEM_ERR_DEGREE = -8,      /* a node belongs to more than FEM_MAX_NODE_ELEMS elements */
+    FEM_ERR_ALIAS = -9,       /* hist_out aliases hist_in */
+    FEM_ERR_MAT = -10         /* n_mat is neither 1 nor n_elems */
+};
+#define FEM_MAX_NODE_ELEMS 32
+
+typedef struct fem_ctx fem_ctx; /* opaque, owned by the library */
+
+typedef struct {
+    int fbar;          /* 0 = standard element (default); 1 = F-bar, Eq.(31)-(32) PAPER.md:233-245 */
+    int quad_order;    /* must be 2 (2x2x2 Gauss) */
+    double tol;        /* relative step tolerance of the local (return-map) Newton solve; default 1e-10,
+                          the step that meets it is still applied, so the root is at round-off */
+    int kmax;          /* local Newton iteration cap (default 60); a point that hits it is counted, not an error */
+    int jmax;          /* kept for ABI parity with Alg. C2's line search; the scalar solve
+                          uses a bracket instead, so it is unused */
+    double beta, eta;  /* Alg. C2 / App. B constants; unused by the scalar solve */
+    int assembly_mode; /* 0 = element scratch + deterministic node-row gather (only mode) */
+} fem_options;
+
+typedef struct {
+    long long n_plastic;      /* quadrature points that took the plastic branch (f_trial > 0, Eq.(17) :165) */
+    long long n_nonconverged; /* local solves that hit kmax */
+    long long n_detF_nonpos;  /* points with det F <= 0 (computation continues, C stays SPD) */
+    long long n_nonfinite;    /* points whose stress is not finite */
+    int max_local_iters;      /* largest local Newton iteration count */
+    long long iter_hist[64];  /* iter_hist[k] = plastic points that used k iterations (k >= 63 clipped) */
+} fem_stats;
+
+/* Fills *opt with the defaults named above. */
+void fem_default_options(fem_options *opt /*host*/);
+
+/* fem_setup — "fem_setup(coords, hex8 connectivity, quadrature)" of the problem statement.
+ * Copies mesh to library-owned device memory, validates connectivity range and det J_ref > 0 at all 8 Gauss points
+ * of every element (O1: J_ref = sum_I X_I (x) dN_I/dxi, Eq.(28)).
+ *   coords  dev [n_nodes*3]  xyz interleaved          conn  dev [n_elems*8] int32
+ *   opt     host, may be NULL (defaults)
+ * Synchronises the device once.  On error *out is NULL. */
+int fem_setup(fem_ctx **out, long long n_nodes, const double *coords, long long n_elems, const int *conn,
+              const fem_options *opt);
+
+/* fem_build_csr_pattern — sorted, duplicate-free CSR pattern of all element DOF pairs (triplets of PAPER.md:296-298,
+ * Alg. E1 :1039-1049; structural zeros are kept) and the element-to-CSR slot map.
+ *   n_rows = 3*n_nodes, row_ptr dev [n_rows+1], col_idx dev [nnz] ascending within a row,
+ *   elem_slot dev [n_elems*576]: elem_slot[e*576 + a*24 + b] = index into the CSR values of (dof_a, dof_b),
+ *   a,b = 3*local_node + component.  Any out-pointer may be NULL; the 576-wide map is only materialised when
+ *   elem_slot != NULL (fem_assemble uses the compressed per-node-pair form internally).
+ * Built entirely on the device; synchronises once.  Must precede fem_assemble. */
+int fem_build_csr_pattern(fem_ctx *c, long long *n_rows, long long *nnz, const int **row_ptr, const int **col_idx,
+                          const int **elem_slot);
+
+/* fem_assemble — one evaluation of residual R = A R^e (internal force, Eq.(35) :257 without the traction term),
+ * tangent K = A K^e (Eq.(37) :267 / Eq.(40) :294) and updated history (Alg. C1 :916).
+ *   u         dev [n_rows]         nodal displacement
+ *   hist_in   dev [n_elems*8*7]    per Gauss point (eps_p 11,22,33,12,23,13 ; alpha), Eq.(6) :98-102
+ *   mat       dev [n_mat*16]       E, nu, r11, r22, r33, r12, r23, r13, law(0 Voce,1 Swift), h0, h1, h2, q0..q3
+ *                                  Voce (sigma0,Q,b) Eq.(10) :121; Swift (K,eps0,n); r = yield-stress ratios of Eq.(A3) :784;
+ *                                  q = unit quaternion (w,x,y,z) of the material orientation Theta, Eq.(A1) :774
+ *   n_mat     1 (uniform) or n_elems
+ *   residual  dev [n_rows]   csr_vals dev [nnz]   hist_out dev [n_elems*8*7] (must not alias hist_in)
+ *   stats     host, may be NULL; when non-NULL the call synchronises `stream` and copies the counters back
+ *   cuda_stream  a cudaStream_t (NULL = legacy default stream); all work is ordered on it
+ * Sums are taken in a fixed order (ascending element id per entry): two calls with equal inputs give bit-identical output.
+ * Physics trouble (local non-convergence, det F <= 0, non-finite) is counted in stats, never an error return. */
+int fem_assemble(fem_ctx *c, const double *u, const double *hist_in, const double *mat, long long n_mat,
+                 double *residual, double *csr_vals, double *hist_out, fem_stats *stats, void *cuda_stream);
+
+/* Same call with HOST buffers for every array: copies in, assembles, copies out, synchronises (used for end-to-end timing). */
+int fem_assemble_host(fem_ctx *c, const double *u, const double *hist_in, const double *mat, long long n_mat,
+                      double *residual, double *csr_vals, double *hist_out, fem_stats *stats);
+
+/* Device time in milliseconds of the two kernels of the last fem_assemble on this context, measured with CUDA events
+ * on the call's stream: ms[0] = element kernel (S2-S12), ms[1] = gather kernel (S14), ms[2] = material pre-pass.
+ * Synchronises on the recorded events. */
+int fem_last_kernel_ms(fem_ctx *c, double ms[3] /*host*/);
+
+/* Number of kernels launched by one fem_assemble on this context (for bench.py's gpu_launches). */
+int fem_launches_per_assemble(const fem_ctx *c);
+
+/* Dependent-chain-free DFMA throughput probe: runs a register-resident fused-multiply-add kernel for about `ms_target`
+ * milliseconds and returns the achieved FP64 rate in TFLOP/s (FMA = 2 flops) in *tflops.  Roofline denominator only. */
+int fem_probe_fp64_peak(double ms_target, double *tflops /*host*/, void *cuda_stream);
+
+void fem_destroy(fem_ctx *c);
+const char *fem_strerror(int code);
+const char *fem_last_cuda_error(void);
+
+/* Host helper: Lankford r0, r45, r90 -> the paper's yield-stress ratios (r11,r22,r33,r12,r23,r13) of Eq.(A3)-(A5)
+ * (textbook Hill-1948 plane-stress relations, axis 1 = rolling direction, sigma11^y = sigma0; reading D2). */
+int fem_hill_from_lankford(double r0, double r45, double r90, double r_out[6] /*host*/);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,250 @@
+"""ctypes binding with the same names as include/fem.h.  Argument marshalling only."""
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+NPAR = 16
+
+ABI_SYMBOLS = ["fem_default_options", "fem_setup", "fem_build_csr_pattern", "fem_assemble", "fem_assemble_host",
+               "fem_last_kernel_ms", "fem_launches_per_assemble", "fem_probe_fp64_peak", "fem_destroy", "fem_strerror",
+               "fem_last_cuda_error", "fem_hill_from_lankford"]
+
+
+class FemOptions(C.Structure):
+    _fields_ = [("fbar", C.c_int), ("quad_order", C.c_int), ("tol", C.c_double), ("kmax", C.c_int), ("jmax", C.c_int),
+                ("beta", C.c_double), ("eta", C.c_double), ("assembly_mode", C.c_int)]
+
+
+class FemStats(C.Structure):
+    _fields_ = [("n_plastic", C.c_longlong), ("n_nonconverged", C.c_longlong), ("n_detF_nonpos", C.c_longlong),
+                ("n_nonfinite", C.c_longlong), ("max_local_iters", C.c_int), ("iter_hist", C.c_longlong * 64)]
+
+    def as_dict(self):
+        return dict(n_plastic=self.n_plastic, n_nonconverged=self.n_nonconverged, n_detF_nonpos=self.n_detF_nonpos,
+                    n_nonfinite=self.n_nonfinite, max_local_iters=self.max_local_iters, iter_hist=list(self.iter_hist))
+
+
+class FemError(RuntimeError):
+    def __init__(self, code, where):
+        self.code = code
+        msg = lib().fem_strerror(code).decode()
+        if code == -6:
+            msg += ": " + lib().fem_last_cuda_error().decode()
+        super().__init__("%s failed (%d): %s" % (where, code, msg))
+
+
+_lib = None
+
+
+def lib_path():
+    return os.path.join(_HERE, "libfem_b200.so")
+
+
+def lib():
+    """Loads libfem_b200.so (built in-tree by build.py).  Fails loudly when it is missing: no fallback exists."""
+    global _lib
+    if _lib is None:
+        p = lib_path()
+        if not os.path.exists(p):
+            raise FileNotFoundError(p + " not built: run `python -m paper_2606_17390_b200.build` "
+                                    "(or __graft_entry__.build()); there is no CPU fallback")
+        L = C.CDLL(p)
+        vp, ll, dp = C.c_void_p, C.c_longlong, C.POINTER(C.c_double)
+        L.fem_default_options.argtypes = [C.POINTER(FemOptions)]
+        L.fem_default_options.restype = None
+        L.fem_setup.argtypes = [C.POINTER(vp), ll, vp, ll, vp, C.POINTER(FemOptions)]
+        L.fem_build_csr_pattern.argtypes = [vp, C.POINTER(ll), C.POINTER(ll), C.POINTER(vp), C.POINTER(vp), C.POINTER(vp)]
+        L.fem_assemble.argtypes = [vp, vp, vp, vp, ll, vp, vp, vp, C.POINTER(FemStats), vp]
+        L.fem_assemble_host.argtypes = [vp, vp, vp, vp, ll, vp, vp, vp, C.POINTER(FemStats)]
+        L.fem_last_kernel_ms.argtypes = [vp, dp]
+        L.fem_launches_per_assemble.argtypes = [vp]
+        L.fem_probe_fp64_peak.argtypes = [C.c_double, dp, vp]
+        L.fem_destroy.argtypes = [vp]
+        L.fem_destroy.restype = None
+        L.fem_strerror.argtypes = [C.c_int]
+        L.fem_strerror.restype = C.c_char_p
+        L.fem_last_cuda_error.restype = C.c_char_p
+        L.fem_hill_from_lankford.argtypes = [C.c_double] * 3 + [dp]
+        _lib = L
+    return _lib
+
+
+def _check(rc, where):
+    if rc != 0:
+        raise FemError(rc, where)
+
+
+def hill_from_lankford(r0, r45, r90):
+    out = (C.c_double * 6)()
+    _check(lib().fem_hill_from_lankford(float(r0), float(r45), float(r90), out), "fem_hill_from_lankford")
+    return np.array(out[:], dtype=np.float64)
+
+
+def mat_record(E, nu, r, law, h0, h1, h2, quat=(1.0, 0.0, 0.0, 0.0)):
+    """One FEM_NPAR record: E,nu,r11,r22,r33,r12,r23,r13,law(0 Voce,1 Swift),h0,h1,h2,q0..q3."""
+    return np.array([E, nu, *r, law, h0, h1, h2, *quat], dtype=np.float64)
+
+
+def mat_from_desc(desc, n_elems):
+    """Material description (synth.configs matdesc) -> [n_mat,16] records via the library's own Lankford helper."""
+    per_elem = any(np.ndim(v) > 0 for v in desc.values())
+    n = n_elems if per_elem else 1
+    g = {k: np.broadcast_to(np.asarray(v, dtype=np.float64), (n,)) for k, v in desc.items()}
+    out = np.empty((n, NPAR))
+    for e in range(n):
+        r = hill_from_lankford(g["r0"][e], g["r45"][e], g["r90"][e])
+        out[e] = mat_record(g["E"][e], g["nu"][e], r, g["law"][e], g["h0"][e], g["h1"][e], g["h2"][e])
+    return out
+
+
+def _torch():
+    import torch
+    return torch
+
+
+def _stream_ptr():
+    torch = _torch()
+    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def _ptr(t, dtype, numel=None, name="tensor"):
+    torch = _torch()
+    if not isinstance(t, torch.Tensor) or not t.is_cuda:
+        raise TypeError("%s must be a CUDA torch tensor" % name)
+    if t.dtype != dtype or not t.is_contiguous():
+        raise TypeError("%s must be contiguous %s" % (name, dtype))
+    if numel is not None and t.numel() != numel:
+        raise ValueError("%s has %d elements, expected %d" % (name, t.numel(), numel))
+    return C.c_void_p(t.data_ptr())
+
+
+class FemContext:
+    """fem_setup + fem_build_csr_pattern + fem_assemble on torch CUDA tensors (device memory and streams only)."""
+
+    def __init__(self, coords, conn, fbar=0, tol=None, kmax=None):
+        torch = _torch()
+        L = lib()
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2606_17390_b200 needs a CUDA device: there is no CPU fallback")
+        self.n_nodes, self.n_elems = int(coords.shape[0]), int(conn.shape[0])
+        opt = FemOptions()
+        L.fem_default_options(C.byref(opt))
+        opt.fbar = int(fbar)
+        if tol is not None:
+            opt.tol = float(tol)
+        if kmax is not None:
+            opt.kmax = int(kmax)
+        self._h = C.c_void_p()
+        _check(L.fem_setup(C.byref(self._h), self.n_nodes, _ptr(coords, torch.float64, 3 * self.n_nodes, "coords"),
+                           self.n_elems, _ptr(conn, torch.int32, 8 * self.n_elems, "conn"), C.byref(opt)), "fem_setup")
+        self.device = coords.device
+        self.n_rows = 3 * self.n_nodes
+        self.nnz = None
+
+    def build_csr_pattern(self, want_elem_slot=False):
+        """Returns (row_ptr, col_idx, elem_slot or None) as torch tensors (copies of the library-owned arrays)."""
+        torch = _torch()
+        L = lib()
+        nr, nnz = C.c_longlong(), C.c_longlong()
+        rp, ci, es = C.c_void_p(), C.c_void_p(), C.c_void_p()
+        _check(L.fem_build_csr_pattern(self._h, C.byref(nr), C.byref(nnz), C.byref(rp), C.byref(ci),
+                                       C.byref(es) if want_elem_slot else None), "fem_build_csr_pattern")
+        self.n_rows, self.nnz = nr.value, nnz.value
+
+        def copy(ptr, n):
+            out = torch.empty(n, dtype=torch.int32, device=self.device)
+            rc = _cudart().cudaMemcpy(C.c_void_p(out.data_ptr()), ptr, C.c_size_t(4 * n), 3)
+            if rc != 0:
+                raise RuntimeError("cudaMemcpy failed: %d" % rc)
+            return out
+        row_ptr, col_idx = copy(rp, self.n_rows + 1), copy(ci, self.nnz)
+        elem_slot = copy(es, 576 * self.n_elems).view(self.n_elems, 576) if want_elem_slot else None
+        return row_ptr, col_idx, elem_slot
+
+    def assemble(self, u, hist_in, mat, residual=None, csr_vals=None, hist_out=None, want_stats=False):
+        """One fem_assemble call on the current torch stream.  Returns (residual, csr_vals, hist_out, stats|None)."""
+        torch = _torch()
+        if self.nnz is None:
+            raise FemError(-7, "fem_assemble")
+        f64 = torch.float64
+        n_mat = mat.numel() // NPAR
+        if residual is None:
+            residual = torch.empty(self.n_rows, dtype=f64, device=self.device)
+        if csr_vals is None:
+            csr_vals = torch.empty(self.nnz, dtype=f64, device=self.device)
+        if hist_out is None:
+            hist_out = torch.empty(self.n_elems * 56, dtype=f64, device=self.device)
+        st = FemStats() if want_stats else None
+        _check(lib().fem_assemble(self._h, _ptr(u, f64, self.n_rows, "u"), _ptr(hist_in, f64, 56 * self.n_elems, "hist_in"),
+                                  _ptr(mat, f64, None, "mat"), n_mat, _ptr(residual, f64, self.n_rows, "residual"),
+                                  _ptr(csr_vals, f64, self.nnz, "csr_vals"), _ptr(hist_out, f64, 56 * self.n_elems, "hist_out"),
+                                  C.byref(st) if want_stats else None, _stream_ptr()), "fem_assemble")
+        return residual, csr_vals, hist_out, (st.as_dict() if want_stats else None)
+
+    def assemble_host(self, u, hist_in, mat, residual, csr_vals, hist_out, want_stats=False):
+        """fem_assemble_host on HOST buffers (numpy arrays or pinned CPU torch tensors); copies are inside the call."""
+        def hp(a, n, name):
+            if hasattr(a, "data_ptr"):
+                if a.is_cuda or a.dtype != _torch().float64 or not a.is_contiguous() or a.numel() != n:
+                    raise TypeError("%s must be a contiguous float64 host tensor of %d elements" % (name, n))
+                return C.c_void_p(a.data_ptr())
+            if a.dtype != np.float64 or not a.flags["C_CONTIGUOUS"] or a.size != n:
+                raise TypeError("%s must be a contiguous float64 array of %d elements" % (name, n))
+            return C.c_void_p(a.ctypes.data)
+        n_mat = (mat.numel() if hasattr(mat, "numel") else mat.size) // NPAR
+        st = FemStats() if want_stats else None
+        _check(lib().fem_assemble_host(self._h, hp(u, self.n_rows, "u"), hp(hist_in, 56 * self.n_elems, "hist_in"),
+                                       hp(mat, NPAR * n_mat, "mat"), n_mat, hp(residual, self.n_rows, "residual"),
+                                       hp(csr_vals, self.nnz, "csr_vals"), hp(hist_out, 56 * self.n_elems, "hist_out"),
+                                       C.byref(st) if want_stats else None), "fem_assemble_host")
+        return st.as_dict() if want_stats else None
+
+    def last_kernel_ms(self):
+        ms = (C.c_double * 3)()
+        _check(lib().fem_last_kernel_ms(self._h, ms), "fem_last_kernel_ms")
+        return dict(element=ms[0], gather=ms[1], mat_prep=ms[2])
+
+    def launches_per_assemble(self):
+        return int(lib().fem_launches_per_assemble(self._h))
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            lib().fem_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+_crt = None
+
+
+def _cudart():
+    """The CUDA runtime already loaded by torch (used only to copy library-owned pattern arrays into torch tensors)."""
+    global _crt
+    if _crt is None:
+        import glob
+        torch = _torch()
+        cands = glob.glob(os.path.join(os.path.dirname(torch.__file__), "lib", "libcudart*.so*")) + \
+            glob.glob("/usr/local/cuda/lib64/libcudart.so*")
+        for c in cands:
+            try:
+                _crt = C.CDLL(c)
+                break
+            except OSError:
+                continue
+        if _crt is None:
+            raise RuntimeError("libcudart not found")
+        _crt.cudaMemcpy.argtypes = [C.c_void_p, C.c_void_p, C.c_size_t, C.c_int]
+    return _crt
+
+
+def probe_fp64_peak(ms_target=50.0):
+    out = C.c_double()
+    _check(lib().fem_probe_fp64_peak(float(ms_target), C.byref(out), _stream_ptr()), "fem_probe_fp64_peak")
+    return out.value

@@ -1,0 +1,851 @@
+// fem_assemble: the hot path as three kernels on one stream
+//   k_mat_prep  : per material record -> derived record (Lame constants, Hill eigen-system, orientation)
+//   k_element   : 8 threads per element (one per Gauss point), 4 elements per warp.
+//                 phase 1 (per point): shape gradients, F, C = F^T F, spectral decomposition, Hencky strain,
+//                   Hill-48 return map as ONE scalar equation, algorithmic tangent as diagonal + rank-1,
+//                   geometric post-processor in the eigenbasis of C, A^ = dP/dF in mixed axes -> shared memory
+//                 phase 2 (per element node): K^e block rows and R^e from the 8 points' A^, G^ in shared memory
+//                 phase 3: K^e staged in shared memory, written block-major with coalesced 16-byte stores
+//   k_gather    : one warp per node: sums the <= 8 incident element contributions of each 3x3 node-pair block in
+//                 ascending element id (fixed order, no atomics) into the CSR values and the residual.
+// All formulas are derived by hand from PAPER.md (equation numbers at each step); nothing here is shared with oracle/.
+#include "fem_internal.h"
+#include <math.h>
+#include <stdio.h>
+
+#define W23 0.81649658092772603273   // W = sqrt(2/3)
+#define SQRT2 1.41421356237309504880
+#define RSQRT2 0.70710678118654752440
+
+// ------------------------------------------------------------------------------------------------ material pre-pass
+// mat record (fem.h): E,nu,r11,r22,r33,r12,r23,r13,law,h0,h1,h2,q0..q3.
+// Derived record (FEM_MATD doubles):
+//   [0] 2mu  [1] lambda  [2] bulk modulus  [3] law  [4..6] h0,h1,h2
+//   [7..11]  h_k : the five non-zero eigenvalues of the Hill tensor H (Mandel form), Eq.(A2)-(A5) PAPER.md:779-801
+//   [12..14] v1, [15..17] v2 : eigenvectors of the normal 3x3 block of H in the deviatoric plane (unit, sum = 0);
+//            eigenvectors 3..5 are the pure shears 12, 23, 13 with h = p7, p8, p9
+//   [18..26] Theta row-major (columns = material axes in the global frame, Eq.(A1) :774) ; [27] 1 if Theta != I
+// With isotropic elasticity (Eq.(8) :110) E:H = 2mu H, so in this eigenbasis the return map is diagonal.
+__global__ void k_mat_prep(long long n_mat, const double *__restrict__ mat, double *__restrict__ md) {
+    long long m = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (m >= n_mat) return;
+    const double *p = mat + m * FEM_NPAR;
+    double *o = md + m * FEM_MATD;
+    double E = p[0], nu = p[1];
+    double mu2 = E / (1.0 + nu), lam = E * nu / ((1.0 + nu) * (1.0 - 2.0 * nu));
+    o[0] = mu2; o[1] = lam; o[2] = lam + mu2 / 3.0; o[3] = p[8]; o[4] = p[9]; o[5] = p[10]; o[6] = p[11];
+    double p1 = 2.0 / (3.0 * p[2] * p[2]), p2 = 2.0 / (3.0 * p[3] * p[3]), p3 = 2.0 / (3.0 * p[4] * p[4]);
+    double p7 = 1.0 / (p[5] * p[5]), p8 = 1.0 / (p[6] * p[6]), p9 = 1.0 / (p[7] * p[7]);
+    double p4 = 0.5 * (p3 - p1 - p2), p5 = 0.5 * (p1 - p2 - p3), p6 = 0.5 * (p2 - p1 - p3);
+    // normal block N3 = [[p1,p4,p6],[p4,p2,p5],[p6,p5,p3]] has null vector (1,1,1); project on d1=(1,-1,0)/sqrt2, d2=(1,1,-2)/sqrt6
+    const double d1[3] = {RSQRT2, -RSQRT2, 0.0};
+    const double d2[3] = {0.40824829046386301637, 0.40824829046386301637, -0.81649658092772603273};
+    const double N3[3][3] = {{p1, p4, p6}, {p4, p2, p5}, {p6, p5, p3}};
+    double m11 = 0, m22 = 0, m12 = 0;
+    for (int i = 0; i < 3; i++)
+        for (int j = 0; j < 3; j++) {
+            m11 += d1[i] * N3[i][j] * d1[j]; m22 += d2[i] * N3[i][j] * d2[j]; m12 += d1[i] * N3[i][j] * d2[j];
+        }
+    double c = 1.0, s = 0.0, e1 = m11, e2 = m22;
+    if (m12 != 0.0) {
+        double d = m22 - m11, r = sqrt(d * d + 4.0 * m12 * m12);
+        double t = 2.0 * m12 / (d + copysign(r, d));
+        c = 1.0 / sqrt(1.0 + t * t); s = t * c;
+        e1 = m11 - t * m12; e2 = m22 + t * m12;
+    }
+    o[7] = e1; o[8] = e2; o[9] = p7; o[10] = p8; o[11] = p9;
+    for (int i = 0; i < 3; i++) { o[12 + i] = c * d1[i] - s * d2[i]; o[15 + i] = s * d1[i] + c * d2[i]; }
+    double qn = sqrt(p[12] * p[12] + p[13] * p[13] + p[14] * p[14] + p[15] * p[15]);
+    double w = p[12] / qn, x = p[13] / qn, y = p[14] / qn, z = p[15] / qn;
+    o[18] = 1 - 2 * (y * y + z * z); o[19] = 2 * (x * y - w * z);     o[20] = 2 * (x * z + w * y);
+    o[21] = 2 * (x * y + w * z);     o[22] = 1 - 2 * (x * x + z * z); o[23] = 2 * (y * z - w * x);
+    o[24] = 2 * (x * z - w * y);     o[25] = 2 * (y * z + w * x);     o[26] = 1 - 2 * (x * x + y * y);
+    o[27] = (x == 0.0 && y == 0.0 && z == 0.0) ? 0.0 : 1.0;
+    for (int i = 28; i < FEM_MATD; i++) o[i] = 0.0;
+}
+
+// ------------------------------------------------------------------------------------------------ small device helpers
+// One cyclic-Jacobi rotation annihilating a_pq of a symmetric 3x3 (r = third index); V columns p,q updated.
+__device__ __forceinline__ void jacobi_rot(double &app, double &aqq, double &apq, double &arp, double &arq, double &v0p,
+                                           double &v0q, double &v1p, double &v1q, double &v2p, double &v2q) {
+    double d = aqq - app;
+    double r = sqrt(fma(d, d, 4.0 * apq * apq));
+    double t = (apq == 0.0) ? 0.0 : (2.0 * apq) / (d + copysign(r, d));
+    double c = rsqrt(fma(t, t, 1.0)), s = t * c;
+    app = fma(-t, apq, app); aqq = fma(t, apq, aqq); apq = 0.0;
+    double x = arp, y = arq;
+    arp = c * x - s * y; arq = s * x + c * y;
+    x = v0p; y = v0q; v0p = c * x - s * y; v0q = s * x + c * y;
+    x = v1p; y = v1q; v1p = c * x - s * y; v1q = s * x + c * y;
+    x = v2p; y = v2q; v2p = c * x - s * y; v2q = s * x + c * y;
+}
+
+// atanh(w)/w : first divided difference kernel of ln,  ln(b/a) = 2 atanh((b-a)/(b+a)).
+__device__ __forceinline__ double atanhc(double w, double dlog /* = ln b - ln a */) {
+    double w2 = w * w;
+    if (w2 < 0.0225) {  // |w| < 0.15 : series 1 + w^2/3 + w^4/5 + ...  (11 terms, remainder < 1e-19)
+        double s = 1.0 / 21.0;
+        s = fma(s, w2, 1.0 / 19.0); s = fma(s, w2, 1.0 / 17.0); s = fma(s, w2, 1.0 / 15.0); s = fma(s, w2, 1.0 / 13.0);
+        s = fma(s, w2, 1.0 / 11.0); s = fma(s, w2, 1.0 / 9.0);  s = fma(s, w2, 1.0 / 7.0);  s = fma(s, w2, 1.0 / 5.0);
+        s = fma(s, w2, 1.0 / 3.0);  s = fma(s, w2, 1.0);
+        return s;
+    }
+    return 0.5 * dlog / w;
+}
+
+// Second divided difference g[a,b,c] of g = 1/2 ln, with x1<=x2<=x3 not required.
+// Far apart: recursion on the widest gap from first divided differences; close together: Taylor series about the mean,
+// g[a,b,c] = 1/(2 m^2) sum_{n>=2} (-1)^(n+1)/n h_{n-2}(x), x_i = (l_i - m)/m, h_k = complete homogeneous polynomial.
+__device__ __forceinline__ double dd2_series(double la, double lb, double lc) {
+    double m = (la + lb + lc) * (1.0 / 3.0), im = 1.0 / m;
+    double xa = (la - m) * im, xb = (lb - m) * im, xc = (lc - m) * im;
+    // h_k(a), h_k(a,b), h_k(a,b,c) by the recurrences h_k(a,b) = a^k + b h_{k-1}(a,b), h_k(a,b,c) = h_k(a,b) + c h_{k-1}(a,b,c)
+    double pa = 1.0, hab = 1.0, habc = 1.0, s = -0.5;  // n = 2 term: -1/2 * h_0
+    const double coef[10] = {1.0 / 3, -1.0 / 4, 1.0 / 5, -1.0 / 6, 1.0 / 7, -1.0 / 8, 1.0 / 9, -1.0 / 10, 1.0 / 11, -1.0 / 12};
+#pragma unroll
+    for (int k = 0; k < 10; k++) {
+        pa *= xa; hab = fma(xb, hab, pa); habc = fma(xc, habc, hab);
+        s = fma(coef[k], habc, s);
+    }
+    return 0.5 * s * im * im;
+}
+
+// ------------------------------------------------------------------------------------------------ element kernel
+// Voigt pair index of tensor components (11,22,33,12,23,13)
+__device__ constexpr int VG[3][3] = {{0, 3, 5}, {3, 1, 4}, {5, 4, 2}};
+__host__ __device__ constexpr int sidx9(int r, int c) {  // packed upper triangle of a symmetric 9x9
+    return (r <= c) ? (r * 9 - r * (r - 1) / 2 + (c - r)) : (c * 9 - c * (c - 1) / 2 + (r - c));
+}
+
+// shared-memory layout per element, in doubles (stride = 8 mod 16 so that the two elements of a half-warp hit
+// disjoint bank groups; every per-point array is [entry][q] with the 8 Gauss points adjacent)
+#define SM_GG 0     // [24][8]  G^_Ia  = grad N_I in the eigenbasis of C
+#define SM_AA 192   // [45][8]  w * A^_(ia)(kb), packed symmetric
+#define SM_PP 552   // [9][8]   w * P^_ia
+#define SM_KS 0     // [576]    K^e staging, overlays GG/AA/PP after phase 2
+#define SM_XE 624   // [24]
+#define SM_UE 648   // [24]
+#define SM_GQ 672   // [24][8]  (F-bar) g^q_Kk = G_KL F^-1_Lk
+#define SM_YY 864   // [9][8]   (F-bar) w/3 (A^:F^)_ia
+#define SM_GB 936   // [24]     (F-bar) gbar
+#define SM_WQ 960   // [8]      (F-bar) w_q J_q / (Jbar V)
+#define ES_STD 680
+#define ES_FBAR 968
+#define EL_PER_CTA 16
+
+__device__ __forceinline__ void flow_stress(double law, double h0, double h1, double h2, double alpha, double &sf,
+                                            double &dsf) {
+    if (law == 0.0) {  // Voce, Eq.(10) PAPER.md:121 (flow stress part; the sqrt(2/3) is applied by the caller, G2)
+        double ex = exp(-h2 * alpha);
+        sf = fma(h1, 1.0 - ex, h0);
+        dsf = h1 * h2 * ex;
+    } else {           // Swift K (eps0 + alpha)^n (BASELINE.json configs)
+        double b = h1 + alpha;
+        sf = h0 * exp(h2 * log(b));
+        dsf = h2 * sf / b;
+    }
+}
+
+template <int FBAR>
+__global__ void __launch_bounds__(128, 2)
+k_element(long long n_elems, const double *__restrict__ coords, const int *__restrict__ conn,
+          const double *__restrict__ u, const double *__restrict__ hist_in, const double *__restrict__ matd,
+          int mat_stride, double tol, int kmax, double *__restrict__ Ke, double *__restrict__ Re,
+          double *__restrict__ hist_out, unsigned long long *__restrict__ stats) {
+    extern __shared__ __align__(16) double sm[];
+    __shared__ unsigned int s_hist[64];
+    constexpr int ES = FBAR ? ES_FBAR : ES_STD;
+    const int tid = threadIdx.x, lane = tid & 31, q = lane & 7;
+    const int el_cta = tid >> 3;
+    const long long e_raw = (long long)blockIdx.x * EL_PER_CTA + el_cta;
+    const bool valid = e_raw < n_elems;
+    const long long e = valid ? e_raw : n_elems - 1;
+    double *se = sm + el_cta * ES;
+    if (tid < 64) s_hist[tid] = 0;
+    __syncthreads();
+
+    // ---- S2 gather: thread q loads node q of its element
+    {
+        long long nd = conn[e * 8 + q];
+        se[SM_XE + 3 * q + 0] = coords[3 * nd + 0]; se[SM_XE + 3 * q + 1] = coords[3 * nd + 1];
+        se[SM_XE + 3 * q + 2] = coords[3 * nd + 2];
+        se[SM_UE + 3 * q + 0] = u[3 * nd + 0]; se[SM_UE + 3 * q + 1] = u[3 * nd + 1]; se[SM_UE + 3 * q + 2] = u[3 * nd + 2];
+    }
+    __syncwarp();
+
+    // ---- S1 shape gradients at this Gauss point (O1): Jr = sum X_I (x) dN_I/dxi, G_I = dN_I/dxi Jr^-1, w = det Jr
+    const double gp = 0.57735026918962576451;
+    const double xq = (q & 1) ? gp : -gp, yq = (q & 2) ? gp : -gp, zq = (q & 4) ? gp : -gp;
+    const double fxp = 1.0 + xq, fxm = 1.0 - xq, fyp = 1.0 + yq, fym = 1.0 - yq, fzp = 1.0 + zq, fzm = 1.0 - zq;
+    double Jr[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}};
+#pragma unroll
+    for (int I = 0; I < 8; I++) {
+        const bool px = ((I ^ (I >> 1)) & 1), py = (I & 2), pz = (I & 4);
+        const double fx = px ? fxp : fxm, fy = py ? fyp : fym, fz = pz ? fzp : fzm;
+        const double d0 = (px ? 0.125 : -0.125) * fy * fz, d1 = (py ? 0.125 : -0.125) * fx * fz,
+                     d2 = (pz ? 0.125 : -0.125) * fx * fy;
+#pragma unroll
+        for (int i = 0; i < 3; i++) {
+            double X = se[SM_XE + 3 * I + i];
+            Jr[i][0] = fma(X, d0, Jr[i][0]); Jr[i][1] = fma(X, d1, Jr[i][1]); Jr[i][2] = fma(X, d2, Jr[i][2]);
+        }
+    }
+    double Ji[3][3];
+    double wq;
+    {
+        double c00 = Jr[1][1] * Jr[2][2] - Jr[1][2] * Jr[2][1], c01 = Jr[1][2] * Jr[2][0] - Jr[1][0] * Jr[2][2],
+               c02 = Jr[1][0] * Jr[2][1] - Jr[1][1] * Jr[2][0];
+        wq = Jr[0][0] * c00 + Jr[0][1] * c01 + Jr[0][2] * c02;
+        double id = 1.0 / wq;
+        Ji[0][0] = c00 * id; Ji[1][0] = c01 * id; Ji[2][0] = c02 * id;
+        Ji[0][1] = (Jr[0][2] * Jr[2][1] - Jr[0][1] * Jr[2][2]) * id;
+        Ji[1][1] = (Jr[0][0] * Jr[2][2] - Jr[0][2] * Jr[2][0]) * id;
+        Ji[2][1] = (Jr[0][1] * Jr[2][0] - Jr[0][0] * Jr[2][1]) * id;
+        Ji[0][2] = (Jr[0][1] * Jr[1][2] - Jr[0][2] * Jr[1][1]) * id;
+        Ji[1][2] = (Jr[0][2] * Jr[1][0] - Jr[0][0] * Jr[1][2]) * id;
+        Ji[2][2] = (Jr[0][0] * Jr[1][1] - Jr[0][1] * Jr[1][0]) * id;
+    }
+    // ---- S3 kinematics: F = I + sum u_I (x) G_I  (Eq.(3), Eq.(30) :228); G kept in shared memory
+    double F[3][3] = {{1, 0, 0}, {0, 1, 0}, {0, 0, 1}};
+#pragma unroll
+    for (int I = 0; I < 8; I++) {
+        const bool px = ((I ^ (I >> 1)) & 1), py = (I & 2), pz = (I & 4);
+        const double fx = px ? fxp : fxm, fy = py ? fyp : fym, fz = pz ? fzp : fzm;
+        const double d0 = (px ? 0.125 : -0.125) * fy * fz, d1 = (py ? 0.125 : -0.125) * fx * fz,
+                     d2 = (pz ? 0.125 : -0.125) * fx * fy;
+        double G[3];
+#pragma unroll
+        for (int j = 0; j < 3; j++) {
+            G[j] = d0 * Ji[0][j] + d1 * Ji[1][j] + d2 * Ji[2][j];
+            se[SM_GG + (3 * I + j) * 8 + q] = G[j];
+        }
+#pragma unroll
+        for (int i = 0; i < 3; i++) {
+            double ui = se[SM_UE + 3 * I + i];
+            F[i][0] = fma(ui, G[0], F[i][0]); F[i][1] = fma(ui, G[1], F[i][1]); F[i][2] = fma(ui, G[2], F[i][2]);
+        }
+    }
+    double detF = F[0][0] * (F[1][1] * F[2][2] - F[1][2] * F[2][1]) - F[0][1] * (F[1][0] * F[2][2] - F[1][2] * F[2][0]) +
+                  F[0][2] * (F[1][0] * F[2][1] - F[1][1] * F[2][0]);
+    double wgt = wq;  // integration weight of the tangent (w_q, times c_q with F-bar)
+    if (FBAR) {
+        // ---- S4 F-bar (Eq.(31)-(32) PAPER.md:237-243): Jbar = sum w J / sum w ; Fbar = (Jbar/J)^(1/3) F
+        double Fi[3][3];
+        double idt = 1.0 / detF;
+        Fi[0][0] = (F[1][1] * F[2][2] - F[1][2] * F[2][1]) * idt; Fi[0][1] = (F[0][2] * F[2][1] - F[0][1] * F[2][2]) * idt;
+        Fi[0][2] = (F[0][1] * F[1][2] - F[0][2] * F[1][1]) * idt; Fi[1][0] = (F[1][2] * F[2][0] - F[1][0] * F[2][2]) * idt;
+        Fi[1][1] = (F[0][0] * F[2][2] - F[0][2] * F[2][0]) * idt; Fi[1][2] = (F[0][2] * F[1][0] - F[0][0] * F[1][2]) * idt;
+        Fi[2][0] = (F[1][0] * F[2][1] - F[1][1] * F[2][0]) * idt; Fi[2][1] = (F[0][1] * F[2][0] - F[0][0] * F[2][1]) * idt;
+        Fi[2][2] = (F[0][0] * F[1][1] - F[0][1] * F[1][0]) * idt;
+#pragma unroll
+        for (int K = 0; K < 8; K++) {
+            double g0 = se[SM_GG + (3 * K + 0) * 8 + q], g1 = se[SM_GG + (3 * K + 1) * 8 + q], g2 = se[SM_GG + (3 * K + 2) * 8 + q];
+#pragma unroll
+            for (int k = 0; k < 3; k++) se[SM_GQ + (3 * K + k) * 8 + q] = g0 * Fi[0][k] + g1 * Fi[1][k] + g2 * Fi[2][k];
+        }
+        double V = wq, WJ = wq * detF;
+#pragma unroll
+        for (int o = 1; o < 8; o <<= 1) { V += __shfl_xor_sync(0xffffffffu, V, o); WJ += __shfl_xor_sync(0xffffffffu, WJ, o); }
+        double Jbar = WJ / V;
+        double cq = cbrt(Jbar / detF);
+        se[SM_WQ + q] = wq * detF / WJ;
+#pragma unroll
+        for (int i = 0; i < 3; i++)
+#pragma unroll
+            for (int j = 0; j < 3; j++) F[i][j] *= cq;
+        wgt = wq * cq;
+    }
+
+    // ---- S5 C = F^T F and its spectral decomposition by cyclic Jacobi (Eq.(4) :92; backward stable, fixed 5 sweeps)
+    double c00 = F[0][0] * F[0][0] + F[1][0] * F[1][0] + F[2][0] * F[2][0];
+    double c11 = F[0][1] * F[0][1] + F[1][1] * F[1][1] + F[2][1] * F[2][1];
+    double c22 = F[0][2] * F[0][2] + F[1][2] * F[1][2] + F[2][2] * F[2][2];
+    double c01 = F[0][0] * F[0][1] + F[1][0] * F[1][1] + F[2][0] * F[2][1];
+    double c12 = F[0][1] * F[0][2] + F[1][1] * F[1][2] + F[2][1] * F[2][2];
+    double c02 = F[0][0] * F[0][2] + F[1][0] * F[1][2] + F[2][0] * F[2][2];
+    double R[3][3] = {{1, 0, 0}, {0, 1, 0}, {0, 0, 1}};  // columns = eigenvectors n_a
+#pragma unroll 1
+    for (int sweep = 0; sweep < 5; sweep++) {
+        jacobi_rot(c00, c11, c01, c02, c12, R[0][0], R[0][1], R[1][0], R[1][1], R[2][0], R[2][1]);
+        jacobi_rot(c00, c22, c02, c01, c12, R[0][0], R[0][2], R[1][0], R[1][2], R[2][0], R[2][2]);
+        jacobi_rot(c11, c22, c12, c01, c02, R[0][1], R[0][2], R[1][1], R[1][2], R[2][1], R[2][2]);
+    }
+    const double lam[3] = {c00, c11, c22};
+
+    // ---- rotate F and G into the eigenbasis (Lagrangian principal axes): F^_ia = F_iJ R_Ja, G^_Ia = G_IJ R_Ja
+    double Fh[3][3];
+#pragma unroll
+    for (int i = 0; i < 3; i++)
+#pragma unroll
+        for (int a = 0; a < 3; a++) Fh[i][a] = F[i][0] * R[0][a] + F[i][1] * R[1][a] + F[i][2] * R[2][a];
+#pragma unroll
+    for (int I = 0; I < 8; I++) {
+        double g0 = se[SM_GG + (3 * I + 0) * 8 + q], g1 = se[SM_GG + (3 * I + 1) * 8 + q], g2 = se[SM_GG + (3 * I + 2) * 8 + q];
+#pragma unroll
+        for (int a = 0; a < 3; a++) se[SM_GG + (3 * I + a) * 8 + q] = g0 * R[0][a] + g1 * R[1][a] + g2 * R[2][a];
+    }
+
+    // ---- material (derived record), orientation
+    const double *md = matd + (long long)mat_stride * e;
+    const double mu2 = __ldg(md + 0), kb = __ldg(md + 2);
+    const bool rot = __ldg(md + 27) != 0.0;
+    double Rm[3][3];  // eigenvectors of C in the material frame: Rm = Theta^T R
+    double Th[3][3];
+    if (rot) {
+#pragma unroll
+        for (int i = 0; i < 9; i++) Th[i / 3][i % 3] = __ldg(md + 18 + i);
+#pragma unroll
+        for (int i = 0; i < 3; i++)
+#pragma unroll
+            for (int a = 0; a < 3; a++) Rm[i][a] = Th[0][i] * R[0][a] + Th[1][i] * R[1][a] + Th[2][i] * R[2][a];
+    } else {
+#pragma unroll
+        for (int i = 0; i < 3; i++)
+#pragma unroll
+            for (int a = 0; a < 3; a++) { Rm[i][a] = R[i][a]; Th[i][a] = (i == a) ? 1.0 : 0.0; }
+    }
+
+    // ---- S5 Hencky strain eps = sum_a 1/2 ln(lam_a) n_a (x) n_a (Eq.(5) :96 with the 1/2 restored, G1), material frame
+    const double lg[3] = {log(lam[0]), log(lam[1]), log(lam[2])};
+    double ee[6];  // elastic trial strain eps - eps_p_n, tensor components (11,22,33,12,23,13), material frame
+    {
+        const double e0 = 0.5 * lg[0], e1 = 0.5 * lg[1], e2 = 0.5 * lg[2];
+        ee[0] = e0 * Rm[0][0] * Rm[0][0] + e1 * Rm[0][1] * Rm[0][1] + e2 * Rm[0][2] * Rm[0][2];
+        ee[1] = e0 * Rm[1][0] * Rm[1][0] + e1 * Rm[1][1] * Rm[1][1] + e2 * Rm[1][2] * Rm[1][2];
+        ee[2] = e0 * Rm[2][0] * Rm[2][0] + e1 * Rm[2][1] * Rm[2][1] + e2 * Rm[2][2] * Rm[2][2];
+        ee[3] = e0 * Rm[0][0] * Rm[1][0] + e1 * Rm[0][1] * Rm[1][1] + e2 * Rm[0][2] * Rm[1][2];
+        ee[4] = e0 * Rm[1][0] * Rm[2][0] + e1 * Rm[1][1] * Rm[2][1] + e2 * Rm[1][2] * Rm[2][2];
+        ee[5] = e0 * Rm[0][0] * Rm[2][0] + e1 * Rm[0][1] * Rm[2][1] + e2 * Rm[0][2] * Rm[2][2];
+    }
+    // history in (global components) -> material frame
+    const double *hin = hist_in + (e * 8 + q) * 7;
+    double epn[6];
+#pragma unroll
+    for (int i = 0; i < 6; i++) epn[i] = hin[i];
+    const double alphan = hin[6];
+    double epm[6];  // eps_p_n in the material frame
+    if (rot) {
+        const double A[3][3] = {{epn[0], epn[3], epn[5]}, {epn[3], epn[1], epn[4]}, {epn[5], epn[4], epn[2]}};
+        double B[3][3];  // B = A Theta
+#pragma unroll
+        for (int i = 0; i < 3; i++)
+#pragma unroll
+            for (int j = 0; j < 3; j++) B[i][j] = A[i][0] * Th[0][j] + A[i][1] * Th[1][j] + A[i][2] * Th[2][j];
+        epm[0] = Th[0][0] * B[0][0] + Th[1][0] * B[1][0] + Th[2][0] * B[2][0];
+        epm[1] = Th[0][1] * B[0][1] + Th[1][1] * B[1][1] + Th[2][1] * B[2][1];
+        epm[2] = Th[0][2] * B[0][2] + Th[1][2] * B[1][2] + Th[2][2] * B[2][2];
+        epm[3] = Th[0][0] * B[0][1] + Th[1][0] * B[1][1] + Th[2][0] * B[2][1];
+        epm[4] = Th[0][1] * B[0][2] + Th[1][1] * B[1][2] + Th[2][1] * B[2][2];
+        epm[5] = Th[0][0] * B[0][2] + Th[1][0] * B[1][2] + Th[2][0] * B[2][2];
+    } else {
+#pragma unroll
+        for (int i = 0; i < 6; i++) epm[i] = epn[i];
+    }
+#pragma unroll
+    for (int i = 0; i < 6; i++) ee[i] -= epm[i];
+
+    // ---- S6 elastic predictor in the Hill eigenbasis: T_tr = p I + s, s = 2mu dev(ee) = sum_k c_k v_k (Eq.(16) :160)
+    const double tre = ee[0] + ee[1] + ee[2];
+    const double pres = kb * tre;
+    double hk[5], ck[5], v1[3], v2[3];
+#pragma unroll
+    for (int k = 0; k < 5; k++) hk[k] = __ldg(md + 7 + k);
+#pragma unroll
+    for (int i = 0; i < 3; i++) { v1[i] = __ldg(md + 12 + i); v2[i] = __ldg(md + 15 + i); }
+    {
+        const double tm = tre * (1.0 / 3.0);
+        const double s0 = mu2 * (ee[0] - tm), s1 = mu2 * (ee[1] - tm), s2 = mu2 * (ee[2] - tm);
+        ck[0] = v1[0] * s0 + v1[1] * s1 + v1[2] * s2;
+        ck[1] = v2[0] * s0 + v2[1] * s1 + v2[2] * s2;
+        ck[2] = SQRT2 * mu2 * ee[3]; ck[3] = SQRT2 * mu2 * ee[4]; ck[4] = SQRT2 * mu2 * ee[5];
+    }
+    double hc2[5];
+    double phitr2 = 0.0;
+#pragma unroll
+    for (int k = 0; k < 5; k++) { hc2[k] = hk[k] * ck[k] * ck[k]; phitr2 += hc2[k]; }
+    const double phitr = sqrt(phitr2);  // Eq.(11) :127
+    const double law = __ldg(md + 3), hh0 = __ldg(md + 4), hh1 = __ldg(md + 5), hh2 = __ldg(md + 6);
+    double sf, dsf;
+    flow_stress(law, hh0, hh1, hh2, alphan, sf, dsf);
+    const bool plastic = (phitr - W23 * sf) > 0.0;  // f_tr = phi(T_tr) - sqrt(2/3) sigma_flow(alpha_n), Eq.(17) :165 ; tie -> elastic
+
+    // ---- S7 return map: sigma_y(alpha)/phi(x) - 1 = 0 in dgam, x = 2mu dgam / sigma_y
+    double dg = 0.0, xs = 0.0;
+    int iters = 0;
+    bool nonconv = false;
+    if (plastic) {
+        double lo = 0.0, hi = INFINITY;
+        const double atol = 4.0e-16 * phitr / mu2;  // round-off floor of dgam (a strain): eps * |T| / 2mu
+        bool conv = false;
+        for (iters = 1; iters <= kmax; iters++) {
+            const double al = fma(W23, dg, alphan);
+            flow_stress(law, hh0, hh1, hh2, al, sf, dsf);
+            const double sy = W23 * sf, dsy = W23 * dsf;
+            const double isy = 1.0 / sy;
+            const double x = mu2 * dg * isy;
+            double S2 = 0.0, S3 = 0.0;
+#pragma unroll
+            for (int k = 0; k < 5; k++) {
+                const double r = 1.0 / fma(x, hk[k], 1.0);
+                const double t2 = hc2[k] * r * r;
+                S2 += t2; S3 = fma(t2 * r, hk[k], S3);
+            }
+            const double rphi = rsqrt(S2);
+            const double Fv = fma(sy, rphi, -1.0);
+            const double dxd = mu2 * isy * (1.0 - dg * dsy * W23 * isy);
+            const double Fp = dsy * W23 * rphi + sy * S3 * rphi * rphi * rphi * dxd;
+            if (Fv < 0.0) lo = dg; else hi = dg;
+            double dgn = dg - Fv / Fp;
+            if (!(dgn > lo && dgn < hi)) dgn = (hi < INFINITY) ? 0.5 * (lo + hi) : 2.0 * dg + 1e-12;
+            conv = fabs(dgn - dg) <= fma(tol, dgn, atol);
+            dg = dgn;
+            if (conv) break;
+        }
+        nonconv = !conv;
+        if (iters > kmax) iters = kmax;
+    }
+    // state at the solution (elastic: dg = 0)
+    const double alpha1 = fma(W23, dg, alphan);
+    flow_stress(law, hh0, hh1, hh2, alpha1, sf, dsf);
+    double th[5], cn[5];   // theta_k = 2mu/(1+x h_k) ; c'_k = c_k/(1+x h_k)
+    double phi2 = 0.0;
+    xs = mu2 * dg / (W23 * sf);
+#pragma unroll
+    for (int k = 0; k < 5; k++) {
+        const double r = 1.0 / fma(xs, hk[k], 1.0);
+        th[k] = mu2 * r; cn[k] = ck[k] * r; phi2 += hk[k] * cn[k] * cn[k];
+    }
+    // flow direction N = H:T/phi (Eq.(13) :141) in the Hill eigenbasis, m = D^-1 N, beta of C_ep = D^-1 + beta m (x) m
+    double mk[5], beta = 0.0;
+    double nk[5];
+    {
+        const double iphi = plastic ? rsqrt(phi2) : 0.0;
+        double a = 0.0;
+#pragma unroll
+        for (int k = 0; k < 5; k++) { nk[k] = hk[k] * cn[k] * iphi; mk[k] = th[k] * nk[k]; a = fma(mk[k], nk[k], a); }
+        if (plastic) {
+            const double kap = dg * iphi;                 // dgam / phi
+            const double om = 1.0 - kap * a;
+            const double Hp = (2.0 / 3.0) * dsf;          // W dsigma_y/dalpha = (2/3) sigma_flow'
+            const double den = fma(om, Hp, a);
+            beta = (kap * den - 1.0) / (om * den);
+        }
+    }
+    // ---- S10 history out: eps_p += dgam N, alpha += W dgam (Eq.(19)-(20) :176-178), back to global components
+    if (valid) {
+        double *ho = hist_out + (e * 8 + q) * 7;
+        double ep1[6];
+        ep1[0] = epm[0] + dg * (nk[0] * v1[0] + nk[1] * v2[0]);
+        ep1[1] = epm[1] + dg * (nk[0] * v1[1] + nk[1] * v2[1]);
+        ep1[2] = epm[2] + dg * (nk[0] * v1[2] + nk[1] * v2[2]);
+        ep1[3] = epm[3] + dg * nk[2] * RSQRT2; ep1[4] = epm[4] + dg * nk[3] * RSQRT2; ep1[5] = epm[5] + dg * nk[4] * RSQRT2;
+        if (rot && plastic) {
+            const double A[3][3] = {{ep1[0], ep1[3], ep1[5]}, {ep1[3], ep1[1], ep1[4]}, {ep1[5], ep1[4], ep1[2]}};
+            double B[3][3];  // B = A Theta^T ; out = Theta B
+#pragma unroll
+            for (int i = 0; i < 3; i++)
+#pragma unroll
+                for (int j = 0; j < 3; j++) B[i][j] = A[i][0] * Th[j][0] + A[i][1] * Th[j][1] + A[i][2] * Th[j][2];
+            ep1[0] = Th[0][0] * B[0][0] + Th[0][1] * B[1][0] + Th[0][2] * B[2][0];
+            ep1[1] = Th[1][0] * B[0][1] + Th[1][1] * B[1][1] + Th[1][2] * B[2][1];
+            ep1[2] = Th[2][0] * B[0][2] + Th[2][1] * B[1][2] + Th[2][2] * B[2][2];
+            ep1[3] = Th[0][0] * B[0][1] + Th[0][1] * B[1][1] + Th[0][2] * B[2][1];
+            ep1[4] = Th[1][0] * B[0][2] + Th[1][1] * B[1][2] + Th[1][2] * B[2][2];
+            ep1[5] = Th[0][0] * B[0][2] + Th[0][1] * B[1][2] + Th[0][2] * B[2][2];
+        }
+        if (!plastic) {
+#pragma unroll
+            for (int i = 0; i < 6; i++) ep1[i] = epn[i];  // elastic step: history copied unchanged (Eq.(18) :172)
+        }
+#pragma unroll
+        for (int i = 0; i < 6; i++) ho[i] = ep1[i];
+        ho[6] = alpha1;
+    }
+
+    // ---- S8 algorithmic tangent in the eigenbasis of C (App. D :1002-1019 in closed form):
+    //      C_ep = kb I(x)I + sum_k theta_k V^_k (x) V^_k + beta m^ (x) m^ ,  V^_k = Rm^T V_k Rm ; T^ = p I + sum c'_k V^_k
+    double Ch[6][6];   // tensor components, upper triangle used
+    double Tt[6] = {pres, pres, pres, 0.0, 0.0, 0.0}, mh[6] = {0, 0, 0, 0, 0, 0};
+#pragma unroll
+    for (int A = 0; A < 6; A++)
+#pragma unroll
+        for (int B = A; B < 6; B++) Ch[A][B] = (A < 3 && B < 3) ? kb : 0.0;
+#pragma unroll
+    for (int k = 0; k < 5; k++) {
+        double Vh[6];
+        if (k < 2) {
+            const double *v = (k == 0) ? v1 : v2;
+#pragma unroll
+            for (int A = 0; A < 6; A++) {
+                const int a = (A < 3) ? A : (A == 3 ? 0 : (A == 4 ? 1 : 0)), b = (A < 3) ? A : (A == 3 ? 1 : 2);
+                Vh[A] = v[0] * Rm[0][a] * Rm[0][b] + v[1] * Rm[1][a] * Rm[1][b] + v[2] * Rm[2][a] * Rm[2][b];
+            }
+        } else {
+            const int i = (k == 2) ? 0 : (k == 3 ? 1 : 0), j = (k == 2) ? 1 : 2;  // shear 12, 23, 13
+#pragma unroll
+            for (int A = 0; A < 6; A++) {
+                const int a = (A < 3) ? A : (A == 3 ? 0 : (A == 4 ? 1 : 0)), b = (A < 3) ? A : (A == 3 ? 1 : 2);
+                Vh[A] = RSQRT2 * (Rm[i][a] * Rm[j][b] + Rm[j][a] * Rm[i][b]);
+            }
+        }
+#pragma unroll
+        for (int A = 0; A < 6; A++) {
+            Tt[A] = fma(cn[k], Vh[A], Tt[A]);
+            mh[A] = fma(mk[k], Vh[A], mh[A]);
+            const double tv = th[k] * Vh[A];
+#pragma unroll
+            for (int B = A; B < 6; B++) Ch[A][B] = fma(tv, Vh[B], Ch[A][B]);
+        }
+    }
+#pragma unroll
+    for (int A = 0; A < 6; A++) {
+        const double bm = beta * mh[A];
+#pragma unroll
+        for (int B = A; B < 6; B++) Ch[A][B] = fma(bm, mh[B], Ch[A][B]);
+    }
+
+    // ---- S9 geometric post-processor (Eq.(25) :204, analytic route of :288): with g = 1/2 ln,
+    //      S^_ab = 2 g[a,b] T^_ab ;  C_L = P_L^T:C_ep:P_L + T:L_L  in the eigenbasis
+    double d1[6];  // first divided differences g[a,b], Voigt-indexed: (00,11,22,01,12,02)
+    d1[0] = 0.5 / lam[0]; d1[1] = 0.5 / lam[1]; d1[2] = 0.5 / lam[2];
+    {
+        const double s01 = lam[0] + lam[1], s12 = lam[1] + lam[2], s02 = lam[0] + lam[2];
+        d1[3] = atanhc((lam[1] - lam[0]) / s01, lg[1] - lg[0]) / s01;
+        d1[4] = atanhc((lam[2] - lam[1]) / s12, lg[2] - lg[1]) / s12;
+        d1[5] = atanhc((lam[2] - lam[0]) / s02, lg[2] - lg[0]) / s02;
+    }
+    // second divided differences: g000,g111,g222 exact; gaab by recursion or series; g012
+    const double lmean = (lam[0] + lam[1] + lam[2]) * (1.0 / 3.0);
+    const double thr = 0.05 * lmean;
+    double g_aaa[3], g_aab[3][3], g012;
+#pragma unroll
+    for (int a = 0; a < 3; a++) g_aaa[a] = -d1[a] * d1[a];  // -1/(4 lam^2)
+#pragma unroll
+    for (int a = 0; a < 3; a++)
+#pragma unroll
+        for (int b = 0; b < 3; b++) {
+            if (a == b) { g_aab[a][b] = 0.0; continue; }
+            const double gap = lam[a] - lam[b];
+            g_aab[a][b] = (fabs(gap) >= thr) ? (d1[a] - d1[VG[a][b]]) / gap : dd2_series(lam[a], lam[a], lam[b]);
+        }
+    {
+        const double g01 = fabs(lam[0] - lam[1]), g12 = fabs(lam[1] - lam[2]), g02 = fabs(lam[0] - lam[2]);
+        const double gmax = fmax(g01, fmax(g12, g02));
+        if (gmax < thr) g012 = dd2_series(lam[0], lam[1], lam[2]);
+        else if (gmax == g01) g012 = (d1[VG[0][2]] - d1[VG[2][1]]) / (lam[0] - lam[1]);   // (g[0,2]-g[2,1])/(l0-l1)
+        else if (gmax == g12) g012 = (d1[VG[1][0]] - d1[VG[0][2]]) / (lam[1] - lam[2]);   // (g[1,0]-g[0,2])/(l1-l2)
+        else                  g012 = (d1[VG[0][1]] - d1[VG[1][2]]) / (lam[0] - lam[2]);   // (g[0,1]-g[1,2])/(l0-l2)
+    }
+    // C_L^ = 4 g1_A g1_B C^_AB + Gamma_AB (T:L_L), weighted by the integration weight
+    double CL[6][6];
+#pragma unroll
+    for (int A = 0; A < 6; A++)
+#pragma unroll
+        for (int B = A; B < 6; B++) CL[A][B] = 4.0 * d1[A] * d1[B] * Ch[A][B];
+    // Gamma: [aa][aa] = 8 t_aa g_aaa ; [aa][ab] = 4 t_ab g_aab ; [ab][ab] = 2 (t_aa g_aab + t_bb g_abb) ;
+    //        [ab][ac] = 2 t_bc g_abc ; all others 0
+#pragma unroll
+    for (int a = 0; a < 3; a++) CL[a][a] = fma(8.0 * Tt[a], g_aaa[a], CL[a][a]);
+    // shear index 3 = (0,1), 4 = (1,2), 5 = (0,2)
+    CL[0][3] = fma(4.0 * Tt[3], g_aab[0][1], CL[0][3]); CL[1][3] = fma(4.0 * Tt[3], g_aab[1][0], CL[1][3]);
+    CL[1][4] = fma(4.0 * Tt[4], g_aab[1][2], CL[1][4]); CL[2][4] = fma(4.0 * Tt[4], g_aab[2][1], CL[2][4]);
+    CL[0][5] = fma(4.0 * Tt[5], g_aab[0][2], CL[0][5]); CL[2][5] = fma(4.0 * Tt[5], g_aab[2][0], CL[2][5]);
+    CL[3][3] += 2.0 * (Tt[0] * g_aab[0][1] + Tt[1] * g_aab[1][0]);
+    CL[4][4] += 2.0 * (Tt[1] * g_aab[1][2] + Tt[2] * g_aab[2][1]);
+    CL[5][5] += 2.0 * (Tt[0] * g_aab[0][2] + Tt[2] * g_aab[2][0]);
+    CL[3][4] = fma(2.0 * Tt[5], g012, CL[3][4]);   // (01),(12) share 1 -> t_02
+    CL[3][5] = fma(2.0 * Tt[4], g012, CL[3][5]);   // (01),(02) share 0 -> t_12
+    CL[4][5] = fma(2.0 * Tt[3], g012, CL[4][5]);   // (12),(02) share 2 -> t_01
+    double Sh[6];
+#pragma unroll
+    for (int A = 0; A < 6; A++) Sh[A] = 2.0 * d1[A] * Tt[A];
+
+    // ---- stats flags
+    bool nonfinite = false;
+    {
+        double chk = 0.0;
+#pragma unroll
+        for (int A = 0; A < 6; A++) chk += Sh[A];
+        nonfinite = !isfinite(chk);
+    }
+
+    // ---- (F-bar) Y_ia = w/3 (A^:F^)_ia = w/3 [ P^_ia + F^_im C_L^[(ma)][(nn)] lam_n ]   (before weighting)
+    if (FBAR) {
+        double Z[6];
+#pragma unroll
+        for (int A = 0; A < 6; A++) {
+            Z[A] = 0.0;
+#pragma unroll
+            for (int n = 0; n < 3; n++) Z[A] = fma((A <= n) ? CL[A][n] : CL[n][A], lam[n], Z[A]);
+        }
+#pragma unroll
+        for (int i = 0; i < 3; i++)
+#pragma unroll
+            for (int a = 0; a < 3; a++) {
+                double y = 0.0;
+#pragma unroll
+                for (int m = 0; m < 3; m++) y = fma(Fh[i][m], Sh[VG[m][a]] + Z[VG[m][a]], y);
+                se[SM_YY + (3 * i + a) * 8 + q] = wq * (1.0 / 3.0) * y;
+            }
+    }
+
+    // ---- S9/S10 P^ = F^ S^ (Eq.(26) :208) and A^_(ia)(kb) = delta_ik S^_ab + F^_im F^_kn C_L^[(ma)][(nb)] -> shared memory
+#pragma unroll
+    for (int i = 0; i < 3; i++)
+#pragma unroll
+        for (int a = 0; a < 3; a++)
+            se[SM_PP + (3 * i + a) * 8 + q] =
+                wq * (Fh[i][0] * Sh[VG[0][a]] + Fh[i][1] * Sh[VG[1][a]] + Fh[i][2] * Sh[VG[2][a]]);
+#pragma unroll
+    for (int A = 0; A < 6; A++) {
+        Sh[A] *= wgt;
+#pragma unroll
+        for (int B = A; B < 6; B++) CL[A][B] *= wgt;
+    }
+#pragma unroll
+    for (int i = 0; i < 3; i++) {
+        double X[3][6];  // X[a][B] = sum_m F^_im C_L^[(ma)][B]
+#pragma unroll
+        for (int a = 0; a < 3; a++)
+#pragma unroll
+            for (int B = 0; B < 6; B++) {
+                double x = 0.0;
+#pragma unroll
+                for (int m = 0; m < 3; m++) {
+                    const int A = VG[m][a];
+                    x = fma(Fh[i][m], (A <= B) ? CL[A][B] : CL[B][A], x);
+                }
+                X[a][B] = x;
+            }
+#pragma unroll
+        for (int a = 0; a < 3; a++)
+#pragma unroll
+            for (int k = i; k < 3; k++)
+#pragma unroll
+                for (int b = 0; b < 3; b++) {
+                    if (3 * k + b < 3 * i + a) continue;
+                    double v = (k == i) ? Sh[VG[a][b]] : 0.0;
+#pragma unroll
+                    for (int n = 0; n < 3; n++) v = fma(X[a][VG[n][b]], Fh[k][n], v);
+                    se[SM_AA + sidx9(3 * i + a, 3 * k + b) * 8 + q] = v;
+                }
+    }
+    __syncwarp();
+
+    // ---- S11/S12 phase 2: thread t = node I of the element.  K^e_(Ii)(Kk) = sum_q G^_Ia A^_(ia)(kb) G^_Kb (Eq.(37) :267),
+    //      R^e_Ii = sum_q P^_ia G^_Ia (Eq.(35) :257).  Symmetry: thread I owns blocks (I, I+d mod 8), d = 0..4
+    //      (d = 4 only for I < 4) and writes their transposes.
+    const int I = q;
+    double acc[5][9];
+    double racc[3] = {0, 0, 0};
+    double rq[FBAR ? 8 : 1][3];
+#pragma unroll
+    for (int d = 0; d < 5; d++)
+#pragma unroll
+        for (int j = 0; j < 9; j++) acc[d][j] = 0.0;
+#pragma unroll 1
+    for (int qq = 0; qq < 8; qq++) {
+        const double *sq = se + qq;
+        const double gI0 = sq[SM_GG + (3 * I + 0) * 8], gI1 = sq[SM_GG + (3 * I + 1) * 8], gI2 = sq[SM_GG + (3 * I + 2) * 8];
+        double aik[3][9];  // a_{i,(kb)} = sum_a G^_Ia A^_(ia)(kb)
+#pragma unroll
+        for (int i = 0; i < 3; i++)
+#pragma unroll
+            for (int kb = 0; kb < 9; kb++)
+                aik[i][kb] = gI0 * sq[SM_AA + sidx9(3 * i + 0, kb) * 8] + gI1 * sq[SM_AA + sidx9(3 * i + 1, kb) * 8] +
+                             gI2 * sq[SM_AA + sidx9(3 * i + 2, kb) * 8];
+#pragma unroll
+        for (int i = 0; i < 3; i++)
+            racc[i] += sq[SM_PP + (3 * i + 0) * 8] * gI0 + sq[SM_PP + (3 * i + 1) * 8] * gI1 + sq[SM_PP + (3 * i + 2) * 8] * gI2;
+        if (FBAR) {
+#pragma unroll
+            for (int i = 0; i < 3; i++)
+                rq[FBAR ? qq : 0][i] = sq[SM_YY + (3 * i + 0) * 8] * gI0 + sq[SM_YY + (3 * i + 1) * 8] * gI1 +
+                                       sq[SM_YY + (3 * i + 2) * 8] * gI2;
+        }
+#pragma unroll
+        for (int d = 0; d < 5; d++) {
+            if (d == 4 && I >= 4) continue;
+            const int K = (I + d) & 7;
+            const double gK0 = sq[SM_GG + (3 * K + 0) * 8], gK1 = sq[SM_GG + (3 * K + 1) * 8], gK2 = sq[SM_GG + (3 * K + 2) * 8];
+#pragma unroll
+            for (int i = 0; i < 3; i++)
+#pragma unroll
+                for (int k = 0; k < 3; k++)
+                    acc[d][3 * i + k] += aik[i][3 * k + 0] * gK0 + aik[i][3 * k + 1] * gK1 + aik[i][3 * k + 2] * gK2;
+        }
+    }
+    if (FBAR) {  // gbar_Kk = sum_q (w_q J_q / (Jbar V)) g^q_Kk for node K = I
+#pragma unroll
+        for (int k = 0; k < 3; k++) {
+            double s = 0.0;
+#pragma unroll
+            for (int qq = 0; qq < 8; qq++) s = fma(se[SM_WQ + qq], se[SM_GQ + (3 * I + k) * 8 + qq], s);
+            se[SM_GB + 3 * I + k] = s;
+        }
+    }
+    __syncwarp();
+    // ---- phase 3: stage K^e block-major [I][K][i][k] in shared memory (overlays GG/AA/PP)
+#pragma unroll
+    for (int d = 0; d < 5; d++) {
+        if (d == 4 && I >= 4) continue;
+        const int K = (I + d) & 7;
+#pragma unroll
+        for (int i = 0; i < 3; i++)
+#pragma unroll
+            for (int k = 0; k < 3; k++) {
+                se[SM_KS + (I * 8 + K) * 9 + 3 * i + k] = acc[d][3 * i + k];
+                if (d != 0) se[SM_KS + (K * 8 + I) * 9 + 3 * k + i] = acc[d][3 * i + k];
+            }
+    }
+    if (FBAR) {
+        // K^e_(Ii)(Kk) += sum_q w_q/3 r^q_Ii (gbar_Kk - g^q_Kk)   (unsymmetric rank-1 terms)
+        __syncwarp();
+        double rs[3] = {0, 0, 0};
+#pragma unroll
+        for (int qq = 0; qq < 8; qq++)
+#pragma unroll
+            for (int i = 0; i < 3; i++) rs[i] += rq[FBAR ? qq : 0][i];
+#pragma unroll 1
+        for (int K = 0; K < 8; K++)
+#pragma unroll
+            for (int k = 0; k < 3; k++) {
+                const double gb = se[SM_GB + 3 * K + k];
+                double t0 = rs[0] * gb, t1 = rs[1] * gb, t2 = rs[2] * gb;
+#pragma unroll
+                for (int qq = 0; qq < 8; qq++) {
+                    const double g = se[SM_GQ + (3 * K + k) * 8 + qq];
+                    t0 = fma(-rq[FBAR ? qq : 0][0], g, t0); t1 = fma(-rq[FBAR ? qq : 0][1], g, t1);
+                    t2 = fma(-rq[FBAR ? qq : 0][2], g, t2);
+                }
+                se[SM_KS + (I * 8 + K) * 9 + 0 + k] += t0;
+                se[SM_KS + (I * 8 + K) * 9 + 3 + k] += t1;
+                se[SM_KS + (I * 8 + K) * 9 + 6 + k] += t2;
+            }
+    }
+    if (valid) {
+        double *ro = Re + e * 24 + 3 * I;
+        ro[0] = racc[0]; ro[1] = racc[1]; ro[2] = racc[2];
+    }
+    __syncwarp();
+    // coalesced copy-out of the warp's 4 elements (4 x 576 doubles), 16 bytes per lane per step
+    {
+        const int w_el0 = (tid >> 5) * 4;
+        const long long e0 = (long long)blockIdx.x * EL_PER_CTA + w_el0;
+#pragma unroll 4
+        for (int idx = lane; idx < 4 * 288; idx += 32) {
+            const int el = idx / 288, off = idx - el * 288;
+            if (e0 + el < n_elems) {
+                const double2 v = *reinterpret_cast<const double2 *>(sm + (w_el0 + el) * ES + SM_KS + 2 * off);
+                *reinterpret_cast<double2 *>(Ke + (e0 + el) * 576 + 2 * off) = v;
+            }
+        }
+    }
+
+    // ---- stats: warp-aggregated counters, per-CTA iteration histogram
+    {
+        const unsigned mp = __ballot_sync(0xffffffffu, valid && plastic);
+        const unsigned mn = __ballot_sync(0xffffffffu, valid && nonconv);
+        const unsigned mj = __ballot_sync(0xffffffffu, valid && !(detF > 0.0));
+        const unsigned mf = __ballot_sync(0xffffffffu, valid && nonfinite);
+        if (lane == 0) {
+            if (mp) atomicAdd(&stats[0], (unsigned long long)__popc(mp));
+            if (mn) atomicAdd(&stats[1], (unsigned long long)__popc(mn));
+            if (mj) atomicAdd(&stats[2], (unsigned long long)__popc(mj));
+            if (mf) atomicAdd(&stats[3], (unsigned long long)__popc(mf));
+        }
+        if (valid && plastic) atomicAdd(&s_hist[iters < 63 ? iters : 63], 1u);
+        __syncthreads();
+        if (tid < 64 && s_hist[tid]) atomicAdd(&stats[5 + tid], (unsigned long long)s_hist[tid]);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ gather kernel (S14)
+// One warp per node n (3 CSR rows).  Lane <-> neighbour position pos: the 3x3 block (n, nb[pos]) is the sum over the
+// incident elements (ascending id) that contain nb[pos]; elem_pos bytes give the local node K of that neighbour.
+// K = A K^e, R = A R^e (Eq.(34) :253, Eq.(38) :274) with a fixed summation order and no atomics.
+__global__ void __launch_bounds__(256)
+k_gather(long long n_nodes, const int *__restrict__ inc_ptr, const int *__restrict__ inc, const int *__restrict__ nb_ptr,
+         const unsigned char *__restrict__ elem_pos, const double *__restrict__ Ke, const double *__restrict__ Re,
+         double *__restrict__ csr_vals, double *__restrict__ residual) {
+    const long long n = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    if (n >= n_nodes) return;
+    const int b = inc_ptr[n], m = inc_ptr[n + 1] - b;
+    const int o = nb_ptr[n], len = nb_ptr[n + 1] - o;
+    const uint2 *pos8 = reinterpret_cast<const uint2 *>(elem_pos);
+    for (int pos = lane; pos < len; pos += 32) {
+        double acc[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
+        const unsigned pat = (unsigned)pos * 0x01010101u;
+        for (int s = 0; s < m; s++) {
+            const long long t = inc[b + s];  // e*8 + I
+            const uint2 pk = pos8[t];
+            unsigned long long hit = ((unsigned long long)(__vcmpeq4(pk.y, pat) & 0x01010101u) << 32) |
+                                     (unsigned long long)(__vcmpeq4(pk.x, pat) & 0x01010101u);
+            while (hit) {
+                const int K = (__ffsll((long long)hit) - 1) >> 3;
+                hit &= hit - 1;
+                const double *kb = Ke + (t * 8 + K) * 9;
+#pragma unroll
+                for (int j = 0; j < 9; j++) acc[j] += kb[j];
+            }
+        }
+        double *out = csr_vals + 9LL * o + 3 * pos;
+#pragma unroll
+        for (int i = 0; i < 3; i++) {
+            out[(long long)i * 3 * len + 0] = acc[3 * i + 0];
+            out[(long long)i * 3 * len + 1] = acc[3 * i + 1];
+            out[(long long)i * 3 * len + 2] = acc[3 * i + 2];
+        }
+    }
+    if (lane < 3) {
+        double r = 0.0;
+        for (int s = 0; s < m; s++) {
+            const long long t = inc[b + s];
+            r += Re[(t >> 3) * 24 + (t & 7) * 3 + lane];
+        }
+        residual[3 * n + lane] = r;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ launch
+static inline unsigned nblk2(long long n, int bs) { return (unsigned)((n + bs - 1) / bs); }
+
+int fem_launch_assemble(fem_ctx *c, const double *u, const double *hist_in, const double *mat, long long n_mat,
+                        double *residual, double *csr_vals, double *hist_out, cudaStream_t st) {
+    if (n_mat > c->n_matd_cap) {
+        if (c->d_matd) cudaFree(c->d_matd);
+        c->d_matd = nullptr; c->n_matd_cap = 0;
+        FEM_CUDA(cudaMalloc(&c->d_matd, sizeof(double) * FEM_MATD * n_mat));
+        c->n_matd_cap = n_mat;
+    }
+    static bool attr_set = false;
+    if (!attr_set) {
+        FEM_CUDA(cudaFuncSetAttribute(k_element<0>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      (int)(EL_PER_CTA * ES_STD * sizeof(double))));
+        FEM_CUDA(cudaFuncSetAttribute(k_element<1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      (int)(EL_PER_CTA * ES_FBAR * sizeof(double))));
+        attr_set = true;
+    }
+    FEM_CUDA(cudaMemsetAsync(c->d_stats, 0, sizeof(unsigned long long) * 72, st));
+    FEM_CUDA(cudaEventRecord(c->ev[0], st));
+    k_mat_prep<<<nblk2(n_mat, 128), 128, 0, st>>>(n_mat, mat, c->d_matd);
+    FEM_CUDA(cudaEventRecord(c->ev[1], st));
+    const unsigned grid = nblk2(c->n_elems, EL_PER_CTA);
+    const int mstride = (n_mat == 1) ? 0 : FEM_MATD;
+    if (c->opt.fbar)
+        k_element<1><<<grid, 128, EL_PER_CTA * ES_FBAR * sizeof(double), st>>>(
+            c->n_elems, c->d_coords, c->d_conn, u, hist_in, c->d_matd, mstride, c->opt.tol, c->opt.kmax, c->d_Ke, c->d_Re,
+            hist_out, c->d_stats);
+    else
+        k_element<0><<<grid, 128, EL_PER_CTA * ES_STD * sizeof(double), st>>>(
+            c->n_elems, c->d_coords, c->d_conn, u, hist_in, c->d_matd, mstride, c->opt.tol, c->opt.kmax, c->d_Ke, c->d_Re,
+            hist_out, c->d_stats);
+    FEM_CUDA(cudaEventRecord(c->ev[2], st));
+    k_gather<<<nblk2(c->n_nodes * 32, 256), 256, 0, st>>>(c->n_nodes, c->d_inc_ptr, c->d_inc, c->d_nb_ptr, c->d_elem_pos,
+                                                          c->d_Ke, c->d_Re, csr_vals, residual);
+    FEM_CUDA(cudaEventRecord(c->ev[3], st));
+    FEM_CUDA(cudaGetLastError());
+    c->ev_valid = true;
+    return FEM_OK;
+}

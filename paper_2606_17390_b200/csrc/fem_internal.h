@@ -1,0 +1,48 @@
+// Internal declarations shared by the translation units of libfem_b200.so (not part of the C ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "../../include/fem.h"
+
+#define FEM_MATD 32  // doubles per derived material record (see k_mat_prep in fem_assemble.cu)
+
+struct fem_ctx {
+    long long n_nodes = 0, n_elems = 0, n_rows = 0, nnz = 0;
+    fem_options opt;
+    // mesh (library-owned copies)
+    double *d_coords = nullptr;  // [n_nodes*3]
+    int *d_conn = nullptr;       // [n_elems*8]
+    // pattern
+    bool has_pattern = false;
+    int *d_inc_ptr = nullptr;    // [n_nodes+1]   node -> incident (element,local node) list
+    int *d_inc = nullptr;        // [8*n_elems]   e*8+I, ascending within a node
+    int *d_nb_ptr = nullptr;     // [n_nodes+1]   node -> sorted neighbour-node list
+    int *d_nb = nullptr;         // [nnz/9]
+    int *d_row_ptr = nullptr;    // [n_rows+1]
+    int *d_col_idx = nullptr;    // [nnz]
+    unsigned char *d_elem_pos = nullptr;  // [n_elems*64]  pos(conn[e][I], conn[e][K]) = rank of node K in nb list of node I
+    int *d_elem_slot = nullptr;  // [n_elems*576], built on request
+    // assemble workspace
+    double *d_Ke = nullptr;      // [n_elems*576] element tangents, block-major [e][I][K][i][k]
+    double *d_Re = nullptr;      // [n_elems*24]
+    double *d_matd = nullptr;    // [n_mat_cap*FEM_MATD]
+    long long n_matd_cap = 0;
+    unsigned long long *d_stats = nullptr;  // [4 + 1 + 64] counters
+    // host-buffer path
+    double *d_u = nullptr, *d_hin = nullptr, *d_hout = nullptr, *d_mat = nullptr, *d_res = nullptr, *d_vals = nullptr;
+    long long n_mat_host_cap = 0;
+    cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+    bool ev_valid = false;
+};
+
+extern char g_fem_cuda_err[512];
+int fem_cuda_fail(cudaError_t e, const char *where);
+#define FEM_CUDA(call)                                                   \
+    do {                                                                 \
+        cudaError_t _e = (call);                                         \
+        if (_e != cudaSuccess) return fem_cuda_fail(_e, #call);          \
+    } while (0)
+
+// fem_assemble.cu
+int fem_launch_assemble(fem_ctx *c, const double *u, const double *hist_in, const double *mat, long long n_mat,
+                        double *residual, double *csr_vals, double *hist_out, cudaStream_t st);

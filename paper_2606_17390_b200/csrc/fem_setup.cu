@@ -1,0 +1,312 @@
+// fem_setup / fem_build_csr_pattern: mesh validation and the device-side CSR pattern build.
+// Pattern = sorted union of all element DOF pairs (triplets of PAPER.md:296-298, Alg. E1 :1039-1049).  Because every
+// node carries 3 DOFs the pattern is the node-adjacency graph blown up by 3x3: row 3n+i holds columns 3m+k for every
+// neighbour node m (ascending) and k = 0..2.  The whole build runs on the device; integer atomics are used only for
+// counting / unordered filling, and every list is sorted afterwards, so the result is deterministic.
+#include "fem_internal.h"
+#include <cub/device/device_scan.cuh>
+#include <math.h>
+#include <new>
+#include <stdio.h>
+#include <string.h>
+
+char g_fem_cuda_err[512] = "";
+int fem_cuda_fail(cudaError_t e, const char *where) {
+    snprintf(g_fem_cuda_err, sizeof(g_fem_cuda_err), "%s: %s", where, cudaGetErrorString(e));
+    return FEM_ERR_CUDA;
+}
+
+// ------------------------------------------------------------------------------------------------ validation
+// flags[0] |= 1 : connectivity out of range ; flags[0] |= 2 : det J_ref <= 0 at a Gauss point (O1, Eq.(28))
+__global__ void k_validate(long long n_nodes, long long n_elems, const double *__restrict__ coords,
+                           const int *__restrict__ conn, int *flags) {
+    long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (e >= n_elems) return;
+    int nd[8];
+    bool ok = true;
+    for (int a = 0; a < 8; a++) {
+        nd[a] = conn[e * 8 + a];
+        if (nd[a] < 0 || nd[a] >= n_nodes) ok = false;
+    }
+    if (!ok) { atomicOr(flags, 1); return; }
+    double X[8][3];
+    for (int a = 0; a < 8; a++)
+        for (int i = 0; i < 3; i++) X[a][i] = coords[3 * (long long)nd[a] + i];
+    const double g = 0.57735026918962576451;
+    bool inv = false;
+    for (int q = 0; q < 8; q++) {
+        double xi[3] = {(q & 1) ? g : -g, (q & 2) ? g : -g, (q & 4) ? g : -g};
+        double J[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}};
+        for (int a = 0; a < 8; a++) {
+            double sx = ((a ^ (a >> 1)) & 1) ? 1.0 : -1.0, sy = (a & 2) ? 1.0 : -1.0, sz = (a & 4) ? 1.0 : -1.0;
+            double fx = 1 + sx * xi[0], fy = 1 + sy * xi[1], fz = 1 + sz * xi[2];
+            double d[3] = {0.125 * sx * fy * fz, 0.125 * fx * sy * fz, 0.125 * fx * fy * sz};
+            for (int i = 0; i < 3; i++)
+                for (int j = 0; j < 3; j++) J[i][j] += X[a][i] * d[j];
+        }
+        double det = J[0][0] * (J[1][1] * J[2][2] - J[1][2] * J[2][1]) - J[0][1] * (J[1][0] * J[2][2] - J[1][2] * J[2][0]) +
+                     J[0][2] * (J[1][0] * J[2][1] - J[1][1] * J[2][0]);
+        if (!(det > 0.0)) inv = true;
+    }
+    if (inv) atomicOr(flags, 2);
+}
+
+// ------------------------------------------------------------------------------------------------ pattern kernels
+__global__ void k_count_inc(long long n_elems, const int *__restrict__ conn, int *cnt) {
+    long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (t < 8 * n_elems) atomicAdd(&cnt[conn[t]], 1);
+}
+__global__ void k_fill_inc(long long n_elems, const int *__restrict__ conn, const int *__restrict__ inc_ptr, int *cursor,
+                           int *inc) {
+    long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (t >= 8 * n_elems) return;
+    int n = conn[t];
+    int p = atomicAdd(&cursor[n], 1);
+    inc[inc_ptr[n] + p] = (int)t;  // t = e*8 + I
+}
+// sort each node's incident list ascending (=> ascending element id); flag nodes with too many elements
+__global__ void k_sort_inc(long long n_nodes, const int *__restrict__ inc_ptr, int *inc, int *flags) {
+    long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (n >= n_nodes) return;
+    int b = inc_ptr[n], m = inc_ptr[n + 1] - b;
+    if (m > FEM_MAX_NODE_ELEMS) { atomicOr(flags, 4); return; }
+    for (int i = 1; i < m; i++) {
+        int v = inc[b + i], j = i - 1;
+        while (j >= 0 && inc[b + j] > v) { inc[b + j + 1] = inc[b + j]; j--; }
+        inc[b + j + 1] = v;
+    }
+}
+// neighbour nodes of node n = union of the nodes of its incident elements, sorted ascending, unique.
+// pass 0 (nb == nullptr): nnb[n] = count ; pass 1: write the list at nb_ptr[n].
+__global__ void k_neighbours(long long n_nodes, const int *__restrict__ conn, const int *__restrict__ inc_ptr,
+                             const int *__restrict__ inc, int *nnb, const int *__restrict__ nb_ptr, int *nb) {
+    long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (n >= n_nodes) return;
+    int cand[8 * FEM_MAX_NODE_ELEMS];
+    int b = inc_ptr[n], m = inc_ptr[n + 1] - b, k = 0;
+    if (m > FEM_MAX_NODE_ELEMS) m = FEM_MAX_NODE_ELEMS;
+    for (int s = 0; s < m; s++) {
+        long long e = inc[b + s] >> 3;
+        for (int a = 0; a < 8; a++) {
+            int v = conn[e * 8 + a], j = k - 1;  // insertion keeping cand sorted & unique
+            while (j >= 0 && cand[j] > v) j--;
+            if (j >= 0 && cand[j] == v) continue;
+            for (int t = k - 1; t > j; t--) cand[t + 1] = cand[t];
+            cand[j + 1] = v;
+            k++;
+        }
+    }
+    if (nb == nullptr) { nnb[n] = k; return; }
+    int o = nb_ptr[n];
+    for (int j = 0; j < k; j++) nb[o + j] = cand[j];
+}
+__global__ void k_row_ptr(long long n_nodes, const int *__restrict__ nb_ptr, int *row_ptr) {
+    long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (n > n_nodes) return;
+    if (n == n_nodes) { row_ptr[3 * n_nodes] = 9 * nb_ptr[n_nodes]; return; }
+    int o = nb_ptr[n], len = nb_ptr[n + 1] - o;
+    for (int i = 0; i < 3; i++) row_ptr[3 * n + i] = 9 * o + i * 3 * len;
+}
+__global__ void k_col_idx(long long n_nodes, const int *__restrict__ nb_ptr, const int *__restrict__ nb, int *col_idx) {
+    // one thread per neighbour-list entry j (global index); finds its node by binary search on nb_ptr
+    long long j = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    long long total = nb_ptr[n_nodes];
+    if (j >= total) return;
+    long long lo = 0, hi = n_nodes - 1;
+    while (lo < hi) { long long mid = (lo + hi + 1) >> 1; if (nb_ptr[mid] <= j) lo = mid; else hi = mid - 1; }
+    long long n = lo;
+    int o = nb_ptr[n], len = nb_ptr[n + 1] - o, p = (int)(j - o), m = nb[j];
+    for (int i = 0; i < 3; i++) {
+        long long base = 9LL * o + (long long)i * 3 * len + 3 * p;
+        col_idx[base] = 3 * m; col_idx[base + 1] = 3 * m + 1; col_idx[base + 2] = 3 * m + 2;
+    }
+}
+__global__ void k_elem_pos(long long n_elems, const int *__restrict__ conn, const int *__restrict__ nb_ptr,
+                           const int *__restrict__ nb, unsigned char *elem_pos) {
+    long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;  // t = e*8 + I
+    if (t >= 8 * n_elems) return;
+    long long e = t >> 3;
+    int n = conn[t], o = nb_ptr[n], len = nb_ptr[n + 1] - o;
+    for (int K = 0; K < 8; K++) {
+        int m = conn[e * 8 + K], lo = 0, hi = len - 1;
+        while (lo < hi) { int mid = (lo + hi) >> 1; if (nb[o + mid] < m) lo = mid + 1; else hi = mid; }
+        elem_pos[t * 8 + K] = (unsigned char)lo;
+    }
+}
+__global__ void k_elem_slot(long long n_elems, const int *__restrict__ conn, const int *__restrict__ row_ptr,
+                            const unsigned char *__restrict__ elem_pos, int *elem_slot) {
+    long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;  // t = e*24 + a
+    if (t >= 24 * n_elems) return;
+    long long e = t / 24;
+    int a = (int)(t - e * 24), I = a / 3, i = a - 3 * I;
+    int row = 3 * conn[e * 8 + I] + i, rp = row_ptr[row];
+    for (int K = 0; K < 8; K++) {
+        int p = elem_pos[(e * 8 + I) * 8 + K];
+        for (int k = 0; k < 3; k++) elem_slot[e * 576 + a * 24 + 3 * K + k] = rp + 3 * p + k;
+    }
+}
+
+static inline unsigned nblk(long long n, int bs) { return (unsigned)((n + bs - 1) / bs); }
+
+// ------------------------------------------------------------------------------------------------ C ABI: host side
+extern "C" void fem_default_options(fem_options *o) {
+    if (!o) return;
+    o->fbar = 0; o->quad_order = 2; o->tol = 1e-10; o->kmax = 60; o->jmax = 10; o->beta = 1e-4; o->eta = 0.1;
+    o->assembly_mode = 0;
+}
+
+extern "C" const char *fem_strerror(int code) {
+    switch (code) {
+        case FEM_OK: return "ok";
+        case FEM_ERR_NULL: return "null pointer argument";
+        case FEM_ERR_ARG: return "invalid argument";
+        case FEM_ERR_QUAD: return "unsupported quad_order (must be 2)";
+        case FEM_ERR_CONN: return "connectivity index out of range";
+        case FEM_ERR_INVERTED: return "det J_ref <= 0 (inverted element)";
+        case FEM_ERR_CUDA: return "CUDA error";
+        case FEM_ERR_NO_PATTERN: return "CSR pattern not built";
+        case FEM_ERR_DEGREE: return "node belongs to too many elements";
+        case FEM_ERR_ALIAS: return "hist_out aliases hist_in";
+        case FEM_ERR_MAT: return "n_mat must be 1 or n_elems";
+        default: return "unknown error code";
+    }
+}
+extern "C" const char *fem_last_cuda_error(void) { return g_fem_cuda_err; }
+
+extern "C" int fem_hill_from_lankford(double r0, double r45, double r90, double r_out[6]) {
+    if (!r_out) return FEM_ERR_NULL;
+    if (!(r0 > 0) || !(r45 > 0) || !(r90 > 0)) return FEM_ERR_ARG;
+    // Hill-1948 F,G,H,N from Lankford values with sigma11^y = sigma0 (G+H = 1); L = M = 3/2 (isotropic out-of-plane shear)
+    double Gh = 1.0 / (1.0 + r0), Hh = r0 / (1.0 + r0), Fh = Hh / r90, Nh = (r45 + 0.5) * (Fh + Gh);
+    r_out[0] = 1.0 / sqrt(Gh + Hh);
+    r_out[1] = 1.0 / sqrt(Fh + Hh);
+    r_out[2] = 1.0 / sqrt(Fh + Gh);
+    r_out[3] = sqrt(1.5 / Nh);
+    r_out[4] = 1.0;
+    r_out[5] = 1.0;
+    return FEM_OK;
+}
+
+static void ctx_free(fem_ctx *c) {
+    if (!c) return;
+    void *ptrs[] = {c->d_coords, c->d_conn, c->d_inc_ptr, c->d_inc, c->d_nb_ptr, c->d_nb, c->d_row_ptr, c->d_col_idx,
+                    c->d_elem_pos, c->d_elem_slot, c->d_Ke, c->d_Re, c->d_matd, c->d_stats, c->d_u, c->d_hin, c->d_hout,
+                    c->d_mat, c->d_res, c->d_vals};
+    for (void *p : ptrs) if (p) cudaFree(p);
+    for (int i = 0; i < 4; i++) if (c->ev[i]) cudaEventDestroy(c->ev[i]);
+    delete c;
+}
+extern "C" void fem_destroy(fem_ctx *c) { ctx_free(c); }
+
+extern "C" int fem_setup(fem_ctx **out, long long n_nodes, const double *coords, long long n_elems, const int *conn,
+                         const fem_options *opt) {
+    if (!out) return FEM_ERR_NULL;
+    *out = nullptr;
+    if (!coords || !conn) return FEM_ERR_NULL;
+    if (n_nodes <= 0 || n_elems <= 0 || n_nodes > 700000000LL || n_elems > 200000000LL) return FEM_ERR_ARG;
+    fem_options o;
+    fem_default_options(&o);
+    if (opt) o = *opt;
+    if (o.quad_order != 2) return FEM_ERR_QUAD;
+    if ((o.fbar != 0 && o.fbar != 1) || !(o.tol > 0) || o.kmax < 1 || o.assembly_mode != 0) return FEM_ERR_ARG;
+    int ndev = 0;
+    FEM_CUDA(cudaGetDeviceCount(&ndev));
+    if (ndev < 1) { snprintf(g_fem_cuda_err, sizeof(g_fem_cuda_err), "no CUDA device"); return FEM_ERR_CUDA; }
+    fem_ctx *c = new (std::nothrow) fem_ctx;
+    if (!c) return FEM_ERR_ARG;
+    c->n_nodes = n_nodes; c->n_elems = n_elems; c->n_rows = 3 * n_nodes; c->opt = o;
+    int rc = FEM_OK, hflags = 0, *dflags = nullptr;
+    do {
+#define TRY(call) { cudaError_t _e = (call); if (_e != cudaSuccess) { rc = fem_cuda_fail(_e, #call); break; } }
+        TRY(cudaMalloc(&c->d_coords, sizeof(double) * 3 * n_nodes));
+        TRY(cudaMalloc(&c->d_conn, sizeof(int) * 8 * n_elems));
+        TRY(cudaMemcpy(c->d_coords, coords, sizeof(double) * 3 * n_nodes, cudaMemcpyDeviceToDevice));
+        TRY(cudaMemcpy(c->d_conn, conn, sizeof(int) * 8 * n_elems, cudaMemcpyDeviceToDevice));
+        TRY(cudaMalloc(&dflags, sizeof(int)));
+        TRY(cudaMemset(dflags, 0, sizeof(int)));
+        k_validate<<<nblk(n_elems, 128), 128>>>(n_nodes, n_elems, c->d_coords, c->d_conn, dflags);
+        TRY(cudaGetLastError());
+        TRY(cudaMemcpy(&hflags, dflags, sizeof(int), cudaMemcpyDeviceToHost));
+        if (hflags & 1) { rc = FEM_ERR_CONN; break; }
+        if (hflags & 2) { rc = FEM_ERR_INVERTED; break; }
+        TRY(cudaMalloc(&c->d_stats, sizeof(unsigned long long) * 72));
+        for (int i = 0; i < 4; i++) TRY(cudaEventCreate(&c->ev[i]));
+#undef TRY
+    } while (0);
+    if (dflags) cudaFree(dflags);
+    if (rc != FEM_OK) { ctx_free(c); return rc; }
+    *out = c;
+    return FEM_OK;
+}
+
+extern "C" int fem_build_csr_pattern(fem_ctx *c, long long *n_rows, long long *nnz, const int **row_ptr,
+                                     const int **col_idx, const int **elem_slot) {
+    if (!c) return FEM_ERR_NULL;
+    const long long nn = c->n_nodes, ne = c->n_elems;
+    if (!c->has_pattern) {
+        int *cnt = nullptr, *dflags = nullptr;
+        void *tmp = nullptr;
+        size_t tmp_bytes = 0;
+        int rc = FEM_OK;
+        do {
+#define TRY(call) { cudaError_t _e = (call); if (_e != cudaSuccess) { rc = fem_cuda_fail(_e, #call); break; } }
+            TRY(cudaMalloc(&cnt, sizeof(int) * (nn + 1)));
+            TRY(cudaMalloc(&dflags, sizeof(int)));
+            TRY(cudaMemset(dflags, 0, sizeof(int)));
+            TRY(cudaMalloc(&c->d_inc_ptr, sizeof(int) * (nn + 1)));
+            TRY(cudaMalloc(&c->d_inc, sizeof(int) * 8 * ne));
+            TRY(cudaMalloc(&c->d_nb_ptr, sizeof(int) * (nn + 1)));
+            TRY(cub::DeviceScan::ExclusiveSum(nullptr, tmp_bytes, cnt, c->d_inc_ptr, (int)(nn + 1)));
+            TRY(cudaMalloc(&tmp, tmp_bytes));
+            // node -> incident elements
+            TRY(cudaMemset(cnt, 0, sizeof(int) * (nn + 1)));
+            k_count_inc<<<nblk(8 * ne, 256), 256>>>(ne, c->d_conn, cnt);
+            TRY(cub::DeviceScan::ExclusiveSum(tmp, tmp_bytes, cnt, c->d_inc_ptr, (int)(nn + 1)));
+            TRY(cudaMemset(cnt, 0, sizeof(int) * (nn + 1)));
+            k_fill_inc<<<nblk(8 * ne, 256), 256>>>(ne, c->d_conn, c->d_inc_ptr, cnt, c->d_inc);
+            k_sort_inc<<<nblk(nn, 128), 128>>>(nn, c->d_inc_ptr, c->d_inc, dflags);
+            int hflags = 0;
+            TRY(cudaMemcpy(&hflags, dflags, sizeof(int), cudaMemcpyDeviceToHost));
+            if (hflags & 4) { rc = FEM_ERR_DEGREE; break; }
+            // node -> neighbour nodes
+            TRY(cudaMemset(cnt, 0, sizeof(int) * (nn + 1)));
+            k_neighbours<<<nblk(nn, 64), 64>>>(nn, c->d_conn, c->d_inc_ptr, c->d_inc, cnt, nullptr, nullptr);
+            TRY(cub::DeviceScan::ExclusiveSum(tmp, tmp_bytes, cnt, c->d_nb_ptr, (int)(nn + 1)));
+            int nblocks = 0;
+            TRY(cudaMemcpy(&nblocks, c->d_nb_ptr + nn, sizeof(int), cudaMemcpyDeviceToHost));
+            if (9LL * nblocks > 2147483647LL) { rc = FEM_ERR_ARG; break; }  // int32 CSR offsets
+            c->nnz = 9LL * nblocks;
+            TRY(cudaMalloc(&c->d_nb, sizeof(int) * (size_t)nblocks));
+            k_neighbours<<<nblk(nn, 64), 64>>>(nn, c->d_conn, c->d_inc_ptr, c->d_inc, cnt, c->d_nb_ptr, c->d_nb);
+            TRY(cudaMalloc(&c->d_row_ptr, sizeof(int) * (c->n_rows + 1)));
+            TRY(cudaMalloc(&c->d_col_idx, sizeof(int) * (size_t)c->nnz));
+            k_row_ptr<<<nblk(nn + 1, 256), 256>>>(nn, c->d_nb_ptr, c->d_row_ptr);
+            k_col_idx<<<nblk(nblocks, 256), 256>>>(nn, c->d_nb_ptr, c->d_nb, c->d_col_idx);
+            TRY(cudaMalloc(&c->d_elem_pos, (size_t)64 * ne));
+            k_elem_pos<<<nblk(8 * ne, 256), 256>>>(ne, c->d_conn, c->d_nb_ptr, c->d_nb, c->d_elem_pos);
+            TRY(cudaGetLastError());
+            // assemble workspace
+            TRY(cudaMalloc(&c->d_Ke, sizeof(double) * 576 * ne));
+            TRY(cudaMalloc(&c->d_Re, sizeof(double) * 24 * ne));
+            TRY(cudaDeviceSynchronize());
+#undef TRY
+        } while (0);
+        if (cnt) cudaFree(cnt);
+        if (dflags) cudaFree(dflags);
+        if (tmp) cudaFree(tmp);
+        if (rc != FEM_OK) return rc;
+        c->has_pattern = true;
+    }
+    if (elem_slot && !c->d_elem_slot) {
+        FEM_CUDA(cudaMalloc(&c->d_elem_slot, sizeof(int) * 576 * ne));
+        k_elem_slot<<<nblk(24 * ne, 256), 256>>>(ne, c->d_conn, c->d_row_ptr, c->d_elem_pos, c->d_elem_slot);
+        FEM_CUDA(cudaGetLastError());
+        FEM_CUDA(cudaDeviceSynchronize());
+    }
+    if (n_rows) *n_rows = c->n_rows;
+    if (nnz) *nnz = c->nnz;
+    if (row_ptr) *row_ptr = c->d_row_ptr;
+    if (col_idx) *col_idx = c->d_col_idx;
+    if (elem_slot) *elem_slot = c->d_elem_slot;
+    return FEM_OK;
+}
