@@ -305,12 +305,17 @@ int orc_return_map(const double *mat, const double *eps6, const double *epn6, do
     /* bracket the unique root of the strictly decreasing h: h(0)=ftr>0 */
     double T[6], dh, lo = 0.0, hi = (phitr - sy) / (2.0 * mat[0]) + 1e-12, hv;
     for (int k = 0; k < 200; k++) { hv = rm_h(E6, H6, mat, Ttr, alphan, hi, T, &dh); (*iters)++; if (hv < 0) break; lo = hi; hi *= 2.0; }
-    double x = 0.5 * (lo + hi), tolh;
+    double x = 0.5 * (lo + hi), tolh, ttrn = sqrt(dot6(Ttr, Ttr)), ehn = 0.0;
+    for (int a = 0; a < 6; a++)
+        for (int b = 0; b < 6; b++) { double s = 0; for (int c = 0; c < 6; c++) s += E6[a][c] * H6[c][b]; ehn += s * s; }
+    ehn = sqrt(ehn);
     int done = 0;
     for (int k = 0; k < 200 && !done; k++) {
         hv = rm_h(E6, H6, mat, Ttr, alphan, x, T, &dh); (*iters)++;
         double sycur, d2; yield_stress(mat, alphan + WHILL * x, &sycur, &d2);
-        tolh = 4.0 * 2.220446049250313e-16 * fmax(sycur, phitr);   /* round-off floor of h scales with |Ttr| */
+        /* round-off floor of h: the 6x6 solve T = (I + kappa E:H)^-1 Ttr carries the full |Ttr| (pressure part
+           included) times its condition number <= 1 + kappa |E:H|_F  (stop at the floor, then polish) */
+        tolh = 4.0 * 2.220446049250313e-16 * fmax(sycur, ttrn * (1.0 + x / sycur * ehn));
         if (fabs(hv) <= tolh) done = 1;
         if (hv > 0) lo = x; else hi = x;
         double xn = x - hv / dh;                        /* Newton step */

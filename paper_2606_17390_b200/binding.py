@@ -47,9 +47,15 @@ def lib():
     global _lib
     if _lib is None:
         p = lib_path()
-        if not os.path.exists(p):
-            raise FileNotFoundError(p + " not built: run `python -m paper_2606_17390_b200.build` "
-                                    "(or __graft_entry__.build()); there is no CPU fallback")
+        from . import build as _b
+        if _b.needs_build():          # stale or missing: rebuild in-tree (nvcc); a failure is loud, there is no fallback
+            try:
+                _b.build()
+            except Exception as ex:
+                if not os.path.exists(p):
+                    raise FileNotFoundError(p + " not built and nvcc failed (%s); run `python -m paper_2606_17390_b200.build`"
+                                            " — there is no CPU fallback" % (ex,))
+                raise
         L = C.CDLL(p)
         vp, ll, dp = C.c_void_p, C.c_longlong, C.POINTER(C.c_double)
         L.fem_default_options.argtypes = [C.POINTER(FemOptions)]

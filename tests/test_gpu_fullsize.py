@@ -1,0 +1,101 @@
+"""Full-size parity (BASELINE.json config 3: 100^3, 1M elements, 3.09M DOF) in the launch configuration bench.py times:
+sampled node rows / history against the oracle computed one by one, plus properties that hold at any size."""
+import numpy as np
+import pytest
+
+import synth
+from parity_util import TOL_HIST, TOL_RES, TOL_VALS, rel_l2
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def full3():
+    import torch
+    import paper_2606_17390_b200 as fem
+    cfg = synth.make_config(3)
+    dev = torch.device("cuda:0")
+    ne = cfg["conn"].shape[0]
+    ctx = fem.FemContext(torch.from_numpy(cfg["coords"]).to(dev), torch.from_numpy(cfg["conn"]).to(dev))
+    row_ptr, col_idx, _ = ctx.build_csr_pattern()
+    mat = fem.mat_from_desc(cfg["matdesc"], ne)
+    res, vals, hout, stats = ctx.assemble(torch.from_numpy(cfg["u"].ravel()).to(dev), torch.from_numpy(cfg["hist_in"].ravel()).to(dev),
+                                          torch.from_numpy(mat.ravel()).to(dev), want_stats=True)
+    torch.cuda.synchronize()
+    return dict(cfg=cfg, ctx=ctx, row_ptr=row_ptr, col_idx=col_idx, res=res, vals=vals, hout=hout, stats=stats)
+
+
+def test_full_pattern_closed_form(full3):
+    # P13: nnz = 9 (3n+1)^3 on a structured grid; row lengths in {24,36,54,81}
+    assert full3["ctx"].nnz == 9 * 301 ** 3 == 245_438_109
+    rp = full3["row_ptr"].cpu().numpy().astype(np.int64)
+    assert rp[0] == 0 and rp[-1] == full3["ctx"].nnz
+    assert set(np.unique(np.diff(rp)).tolist()) == {24, 36, 54, 81}
+    ci = full3["col_idx"]
+    import torch
+    n = 2_000_000  # ascending within rows on a prefix: differences negative only at row starts
+    d = (ci[1:n] - ci[:n - 1]).cpu().numpy()
+    starts = rp[(rp > 0) & (rp < n)] - 1
+    mask = np.ones(n - 1, dtype=bool); mask[starts] = False
+    assert (d[mask] > 0).all()
+
+
+def test_full_sampled_rows_against_oracle(full3):
+    import oracle
+    cfg = full3["cfg"]
+    conn = cfg["conn"]
+    nn, ne = cfg["coords"].shape[0], conn.shape[0]
+    nodes = synth.configs.sample_indices(cfg["seed"], nn, 48)
+    rp = full3["row_ptr"].cpu().numpy(); ci = full3["col_idx"].cpu().numpy()
+    mask = np.isin(conn, nodes)
+    node_elems = {int(n): [] for n in nodes}
+    for e in np.nonzero(mask.any(axis=1))[0]:
+        for a in range(8):
+            if mask[e, a]:
+                node_elems[int(conn[e, a])].append(int(e))
+    mat = oracle.mat_from_desc(cfg["matdesc"], ne)
+    rows, hist = oracle.assemble_rows(cfg["coords"], conn, cfg["u"], cfg["hist_in"], mat, rp, ci, [int(n) for n in nodes], node_elems)
+    vals = full3["vals"].cpu().numpy(); res = full3["res"].cpu().numpy()
+    hout = full3["hout"].cpu().numpy().reshape(ne, 8, 7)
+    g_rows, o_rows, g_res, o_res = [], [], [], []
+    for n, (r3, rws) in rows.items():
+        for i in range(3):
+            g_rows.append(vals[rp[3 * n + i]:rp[3 * n + i + 1]]); o_rows.append(rws[i])
+        g_res.append(res[3 * n:3 * n + 3]); o_res.append(r3)
+    assert rel_l2(np.concatenate(g_rows), np.concatenate(o_rows)) <= TOL_VALS
+    scale = np.abs(np.concatenate(o_rows)).max() * 0.01        # residual rows can cancel to ~0: scale by |K| h
+    assert np.abs(np.concatenate(g_res) - np.concatenate(o_res)).max() <= TOL_RES * max(np.abs(np.concatenate(o_res)).max(), scale)
+    es = sorted(hist)
+    assert rel_l2(np.stack([hout[e] for e in es]), np.stack([hist[e] for e in es])) <= TOL_HIST
+
+
+def test_full_properties(full3):
+    import torch
+    vals, rp, ci, res = full3["vals"], full3["row_ptr"], full3["col_idx"], full3["res"]
+    st = full3["stats"]
+    ne = full3["cfg"]["conn"].shape[0]
+    assert st["n_nonconverged"] == 0 and st["n_detF_nonpos"] == 0 and st["n_nonfinite"] == 0
+    frac = st["n_plastic"] / (8.0 * ne)
+    assert 0.55 < frac < 0.85, frac                       # "~70 % of points are plastic"
+    assert bool(torch.isfinite(vals).all()) and bool(torch.isfinite(res).all())
+    # P3: rigid translations are in the null space of K at any state: per row, sum over columns with col%3==k is 0
+    nrows = rp.numel() - 1
+    rows = torch.repeat_interleave(torch.arange(nrows, device=vals.device), (rp[1:] - rp[:-1]).long())
+    absrow = torch.zeros(nrows, dtype=torch.float64, device=vals.device).index_add_(0, rows, vals.abs())
+    for k in range(3):
+        m = (ci % 3) == k
+        s = torch.zeros(nrows, dtype=torch.float64, device=vals.device).index_add_(0, rows[m], vals[m])
+        assert float((s.abs() / absrow).max()) < 1e-12
+    # internal forces are self-equilibrated: sum over nodes of R is 0 per component
+    r3 = res.view(-1, 3)
+    assert float(r3.sum(0).abs().max()) <= 1e-10 * float(r3.abs().sum())
+    # P14: K symmetric (fbar = 0) on sampled entries
+    idx = torch.randint(0, vals.numel(), (20000,), device=vals.device, generator=torch.Generator(device=vals.device).manual_seed(1))
+    r, c = rows[idx], ci[idx].long()
+    lo, hi = rp[c].long(), rp[c + 1].long()
+    for _ in range(8):                                       # binary search of column r in row c
+        mid = (lo + hi) // 2
+        go = ci[mid.clamp(max=vals.numel() - 1)].long() < r
+        lo = torch.where(go, mid + 1, lo); hi = torch.where(go, hi, mid)
+    assert bool((ci[lo].long() == r).all())
+    assert float((vals[idx] - vals[lo]).abs().max()) <= 1e-10 * float(vals.abs().max())

@@ -1,0 +1,150 @@
+"""GPU parity: the CUDA path (through the C ABI) against the oracle, element by element, on the same seeded inputs.
+Sizes: configs 1, 2 at full size; 3, 4, 5 at reduced resolution spanning several CTAs with a ragged tail (the recipe
+is unchanged); full-size config 3 is covered by test_gpu_fullsize.py on sampled rows."""
+import numpy as np
+import pytest
+
+import synth
+from parity_util import compare, run_gpu, run_oracle, rel_l2
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.mark.parametrize("fbar", [0, 1])
+def test_config1_cube4(fbar):
+    cfg = synth.make_config(1)
+    g, o = run_gpu(cfg, fbar, want_elem_slot=True), run_oracle(cfg, fbar, with_slots=True)
+    err = compare(g, o, "cfg1")
+    assert g["stats"]["n_detF_nonpos"] == 0 and g["stats"]["n_nonfinite"] == 0
+    assert err["vals"] < 1e-13
+
+
+@pytest.mark.parametrize("fbar", [0, 1])
+def test_config2_plate(fbar):
+    cfg = synth.make_config(2)
+    g, o = run_gpu(cfg, fbar), run_oracle(cfg, fbar)
+    compare(g, o, "cfg2")
+    frac = g["stats"]["n_plastic"] / (8.0 * cfg["conn"].shape[0])
+    assert 0.3 < frac < 0.7, frac       # "~50 % of quad points yield"
+
+
+@pytest.mark.parametrize("n", [13, 22])   # 13^3 = 2197 elements: ragged tail of the 16-element CTAs and 4-element warps
+def test_config3_reduced(n):
+    cfg = synth.make_config(3, n=n)
+    compare(run_gpu(cfg), run_oracle(cfg), "cfg3@%d" % n)
+
+
+@pytest.mark.parametrize("fbar", [0, 1])
+def test_config4_void_mask_per_element_material(fbar):
+    cfg = synth.make_config(4, n=18)
+    g, o = run_gpu(cfg, fbar, want_elem_slot=True), run_oracle(cfg, fbar, with_slots=True)
+    compare(g, o, "cfg4@18")
+
+
+@pytest.mark.parametrize("level", [0, 1, 2, 3, 4])
+def test_config5_fraction_sweep(level):
+    cfg = synth.make_config(5, n=14, level=level, sweep="fraction")
+    g, o = run_gpu(cfg), run_oracle(cfg)
+    compare(g, o, "cfg5 fraction %d" % level)
+    if level == 0:
+        assert g["stats"]["n_plastic"] == 0
+        assert np.array_equal(g["hist_out"], cfg["hist_in"])      # elastic step: history copied bit for bit
+
+
+@pytest.mark.parametrize("level", [0, 1, 2, 3])
+def test_config5_strain_sweep(level):
+    cfg = synth.make_config(5, n=14, level=level, sweep="strain")
+    g, o = run_gpu(cfg), run_oracle(cfg)
+    compare(g, o, "cfg5 strain %d" % level)
+    assert g["stats"]["max_local_iters"] <= 30
+
+
+def test_voce_and_rotated_material():
+    """Voce hardening (Table 3 :493-495) and a non-identity material orientation (Eq.(A1) :774)."""
+    import oracle
+    cfg = synth.make_config(3, n=9)
+    ne = cfg["conn"].shape[0]
+    q = np.array([0.9, 0.2, -0.3, 0.25]); q /= np.linalg.norm(q)
+    rec = [219000.0, 0.3, 1.5449, 1.0666, 1.0, 1.0307, 0.95, 1.1, 0.0, 138.0, 410.0, 3.8, *q]
+    mat = np.tile(np.array(rec), (ne, 1))
+    mat[:, 9] *= 1.0 + 0.1 * np.sin(np.arange(ne))            # per-element sigma0
+    g, o = run_gpu(cfg, 0, mat=mat), run_oracle(cfg, 0, mat=mat)
+    compare(g, o, "voce+rotation")
+    assert g["stats"]["n_plastic"] > 0
+
+
+def test_history_from_previous_increment_two_steps():
+    """Two increments: hist_out of the first call is hist_in of the second (caller swaps buffers)."""
+    import torch
+    import oracle
+    import paper_2606_17390_b200 as fem
+    cfg = synth.make_config(5, n=8, level=3, sweep="fraction")
+    ne = cfg["conn"].shape[0]
+    g1, o1 = run_gpu(cfg), run_oracle(cfg)
+    compare(g1, o1, "step 1")
+    cfg2 = dict(cfg); cfg2["u"] = 1.5 * cfg["u"]; cfg2["hist_in"] = o1["hist_out"]
+    g2, o2 = run_gpu(cfg2), run_oracle(cfg2)
+    compare(g2, o2, "step 2")
+
+
+def test_determinism_bitwise():
+    import torch
+    import paper_2606_17390_b200 as fem
+    cfg = synth.make_config(4, n=16)
+    g1 = run_gpu(cfg)
+    g2 = run_gpu(cfg)
+    for k in ("residual", "csr_vals", "hist_out"):
+        assert np.array_equal(g1[k], g2[k]), k
+    ctx = g1["ctx"]
+    dev = torch.device("cuda:0")
+    ne = cfg["conn"].shape[0]
+    mat = torch.from_numpy(fem.mat_from_desc(cfg["matdesc"], ne).ravel()).to(dev)
+    u = torch.from_numpy(cfg["u"].ravel()).to(dev); h = torch.from_numpy(cfg["hist_in"].ravel()).to(dev)
+    r3, v3, h3, _ = ctx.assemble(u, h, mat)
+    torch.cuda.synchronize()
+    assert np.array_equal(v3.cpu().numpy(), g1["csr_vals"]) and np.array_equal(r3.cpu().numpy(), g1["residual"])
+
+
+def test_host_buffer_call_matches_device_call():
+    import paper_2606_17390_b200 as fem
+    cfg = synth.make_config(2)
+    g = run_gpu(cfg)
+    ctx = g["ctx"]
+    ne = cfg["conn"].shape[0]
+    mat = fem.mat_from_desc(cfg["matdesc"], ne)
+    res = np.empty(ctx.n_rows); vals = np.empty(ctx.nnz); hout = np.empty(56 * ne)
+    st = ctx.assemble_host(np.ascontiguousarray(cfg["u"].ravel()), np.ascontiguousarray(cfg["hist_in"].ravel()),
+                           np.ascontiguousarray(mat.ravel()), res, vals, hout, want_stats=True)
+    assert np.array_equal(res, g["residual"]) and np.array_equal(vals, g["csr_vals"])
+    assert np.array_equal(hout.reshape(ne, 8, 7), g["hist_out"]) and st["n_plastic"] == g["stats"]["n_plastic"]
+
+
+def test_error_codes_on_device():
+    import torch
+    import paper_2606_17390_b200 as fem
+    dev = torch.device("cuda:0")
+    cfg = synth.make_config(1)
+    coords = torch.from_numpy(cfg["coords"]).to(dev)
+    bad = cfg["conn"].copy(); bad[3, 2] = 10_000
+    with pytest.raises(fem.FemError) as ei:
+        fem.FemContext(coords, torch.from_numpy(bad).to(dev))
+    assert ei.value.code == -4
+    inv = cfg["conn"].copy(); inv[5] = inv[5][[1, 0, 3, 2, 5, 4, 7, 6]]     # mirrored element: det J_ref < 0
+    with pytest.raises(fem.FemError) as ei:
+        fem.FemContext(coords, torch.from_numpy(inv).to(dev))
+    assert ei.value.code == -5
+    ctx = fem.FemContext(coords, torch.from_numpy(cfg["conn"]).to(dev))
+    u = torch.zeros(375, dtype=torch.float64, device=dev); h = torch.zeros(64 * 56, dtype=torch.float64, device=dev)
+    mat = torch.from_numpy(fem.mat_from_desc(cfg["matdesc"], 64).ravel()).to(dev)
+    with pytest.raises(fem.FemError) as ei:       # pattern not built
+        ctx.assemble(u, h, mat)
+    assert ei.value.code == -7
+    ctx.build_csr_pattern()
+    with pytest.raises(fem.FemError) as ei:       # hist_out aliases hist_in
+        ctx.assemble(u, h, mat, hist_out=h)
+    assert ei.value.code == -9
+    with pytest.raises(fem.FemError) as ei:       # n_mat neither 1 nor n_elems
+        ctx.assemble(u, h, torch.cat([mat, mat]))
+    assert ei.value.code == -10
+    r, v, ho, st = ctx.assemble(u, h, mat, want_stats=True)   # u = 0: R = 0, nothing plastic
+    assert float(r.abs().max()) == 0.0 and st["n_plastic"] == 0
