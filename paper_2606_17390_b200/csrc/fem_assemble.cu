@@ -68,10 +68,15 @@ __global__ void k_mat_prep(long long n_mat, const double *__restrict__ mat, doub
 // One cyclic-Jacobi rotation annihilating a_pq of a symmetric 3x3 (r = third index); V columns p,q updated.
 __device__ __forceinline__ void jacobi_rot(double &app, double &aqq, double &apq, double &arp, double &arq, double &v0p,
                                            double &v0q, double &v1p, double &v1q, double &v2p, double &v2q) {
-    double d = aqq - app;
-    double r = sqrt(fma(d, d, 4.0 * apq * apq));
-    double t = (apq == 0.0) ? 0.0 : (2.0 * apq) / (d + copysign(r, d));
-    double c = rsqrt(fma(t, t, 1.0)), s = t * c;
+    // cos^2 = (1 + |d|/r)/2 with r = hypot(d, 2 a_pq); sin = sgn(d) a_pq / (r cos); tan = sin / cos.  Two rsqrt, no division.
+    const double d = aqq - app;
+    const double r2 = fma(d, d, 4.0 * apq * apq);
+    const double ir = (r2 > 0.0) ? rsqrt(r2) : 0.0;
+    const double c2 = fma(0.5 * fabs(d), ir, 0.5);
+    const double ic = rsqrt(c2);
+    const double c = c2 * ic;
+    const double s = ((d < 0.0) ? -apq : apq) * ir * ic;   // sgn(d) a_pq / (r c); d = 0 counts as positive
+    const double t = s * ic;
     app = fma(-t, apq, app); aqq = fma(t, apq, aqq); apq = 0.0;
     double x = arp, y = arq;
     arp = c * x - s * y; arq = s * x + c * y;
@@ -117,20 +122,19 @@ __host__ __device__ constexpr int sidx9(int r, int c) {  // packed upper triangl
     return (r <= c) ? (r * 9 - r * (r - 1) / 2 + (c - r)) : (c * 9 - c * (c - 1) / 2 + (r - c));
 }
 
-// shared-memory layout per element, in doubles (stride = 8 mod 16 so that the two elements of a half-warp hit
-// disjoint bank groups; every per-point array is [entry][q] with the 8 Gauss points adjacent)
+// shared-memory layout per element, in doubles (stride = 4 mod 16 so that broadcast reads of the 4 elements of a warp
+// hit 4 disjoint bank groups; every per-point array is [entry][q] with the 8 Gauss points adjacent)
 #define SM_GG 0     // [24][8]  G^_Ia  = grad N_I in the eigenbasis of C
-#define SM_AA 192   // [45][8]  w * A^_(ia)(kb), packed symmetric
-#define SM_PP 552   // [9][8]   w * P^_ia
-#define SM_KS 0     // [576]    K^e staging, overlays GG/AA/PP after phase 2
-#define SM_XE 624   // [24]
-#define SM_UE 648   // [24]
-#define SM_GQ 672   // [24][8]  (F-bar) g^q_Kk = G_KL F^-1_Lk
-#define SM_YY 864   // [9][8]   (F-bar) w/3 (A^:F^)_ia
-#define SM_GB 936   // [24]     (F-bar) gbar
-#define SM_WQ 960   // [8]      (F-bar) w_q J_q / (Jbar V)
-#define ES_STD 680
-#define ES_FBAR 968
+#define SM_AA 192   // 45 entries w * A^_(ia)(kb), packed symmetric: entry s < 44 at (s/2)*16 + 2 q + (s&1), entry 44 at 352 + q
+#define SM_XE 192   // [24] element coordinates   (overlay: dead before AA is written)
+#define SM_UE 216   // [24] element displacements (overlay)
+#define SM_KS 0     // K^e staging (324 packed / 576 full), overlays GG/AA after phase 2
+#define SM_GQ 576   // [24][8]  (F-bar) g^q_Kk = G_KL F^-1_Lk
+#define SM_YY 768   // [9][8]   (F-bar) w/3 (A^:F^)_ia
+#define SM_GB 840   // [24]     (F-bar) gbar
+#define SM_WQ 864   // [8]      (F-bar) w_q J_q / (Jbar V)
+#define ES_STD 564   // >= 552, = 4 mod 16: the 4 elements of a warp start in 4 different bank groups
+#define ES_FBAR 884  // >= 872, = 4 mod 16
 #define EL_PER_CTA 16
 
 __device__ __forceinline__ void flow_stress(double law, double h0, double h1, double h2, double alpha, double &sf,
@@ -147,13 +151,14 @@ __device__ __forceinline__ void flow_stress(double law, double h0, double h1, do
 }
 
 template <int FBAR>
-__global__ void __launch_bounds__(128, 2)
+__global__ void __launch_bounds__(128, FBAR ? 2 : 3)
 k_element(long long n_elems, const double *__restrict__ coords, const int *__restrict__ conn,
           const double *__restrict__ u, const double *__restrict__ hist_in, const double *__restrict__ matd,
           int mat_stride, double tol, int kmax, double *__restrict__ Ke, double *__restrict__ Re,
           double *__restrict__ hist_out, unsigned long long *__restrict__ stats) {
     extern __shared__ __align__(16) double sm[];
     __shared__ unsigned int s_hist[64];
+    __shared__ unsigned int s_done;
     constexpr int ES = FBAR ? ES_FBAR : ES_STD;
     const int tid = threadIdx.x, lane = tid & 31, q = lane & 7;
     const int el_cta = tid >> 3;
@@ -162,6 +167,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
     const long long e = valid ? e_raw : n_elems - 1;
     double *se = sm + el_cta * ES;
     if (tid < 64) s_hist[tid] = 0;
+    if (tid == 64) s_done = 0;
     __syncthreads();
 
     // ---- S2 gather: thread q loads node q of its element
@@ -225,6 +231,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
             F[i][0] = fma(ui, G[0], F[i][0]); F[i][1] = fma(ui, G[1], F[i][1]); F[i][2] = fma(ui, G[2], F[i][2]);
         }
     }
+    __syncwarp();  // XE/UE (overlaying AA) are dead from here on
     double detF = F[0][0] * (F[1][1] * F[2][2] - F[1][2] * F[2][1]) - F[0][1] * (F[1][0] * F[2][2] - F[1][2] * F[2][0]) +
                   F[0][2] * (F[1][0] * F[2][1] - F[1][1] * F[2][0]);
     double wgt = wq;  // integration weight of the tangent (w_q, times c_q with F-bar)
@@ -256,7 +263,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
         wgt = wq * cq;
     }
 
-    // ---- S5 C = F^T F and its spectral decomposition by cyclic Jacobi (Eq.(4) :92; backward stable, fixed 5 sweeps)
+    // ---- S5 C = F^T F and its spectral decomposition by cyclic Jacobi (Eq.(4) :92; backward stable, fixed 4 sweeps)
     double c00 = F[0][0] * F[0][0] + F[1][0] * F[1][0] + F[2][0] * F[2][0];
     double c11 = F[0][1] * F[0][1] + F[1][1] * F[1][1] + F[2][1] * F[2][1];
     double c22 = F[0][2] * F[0][2] + F[1][2] * F[1][2] + F[2][2] * F[2][2];
@@ -265,7 +272,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
     double c02 = F[0][0] * F[0][2] + F[1][0] * F[1][2] + F[2][0] * F[2][2];
     double R[3][3] = {{1, 0, 0}, {0, 1, 0}, {0, 0, 1}};  // columns = eigenvectors n_a
 #pragma unroll 1
-    for (int sweep = 0; sweep < 5; sweep++) {
+    for (int sweep = 0; sweep < 4; sweep++) {
         jacobi_rot(c00, c11, c01, c02, c12, R[0][0], R[0][1], R[1][0], R[1][1], R[2][0], R[2][1]);
         jacobi_rot(c00, c22, c02, c01, c12, R[0][0], R[0][2], R[1][0], R[1][2], R[2][0], R[2][2]);
         jacobi_rot(c11, c22, c12, c01, c02, R[0][1], R[0][2], R[1][1], R[1][2], R[2][1], R[2][2]);
@@ -396,8 +403,10 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
             const double Fp = dsy * W23 * rphi + sy * S3 * rphi * rphi * rphi * dxd;
             if (Fv < 0.0) lo = dg; else hi = dg;
             double dgn = dg - Fv / Fp;
-            if (!(dgn > lo && dgn < hi)) dgn = (hi < INFINITY) ? 0.5 * (lo + hi) : 2.0 * dg + 1e-12;
-            conv = fabs(dgn - dg) <= fma(tol, dgn, atol);
+            if (!(dgn >= lo && dgn <= hi)) dgn = (hi < INFINITY) ? 0.5 * (lo + hi) : 2.0 * dg + 1e-12;
+                        // converged when the step is at the round-off floor, or when the residual is so small that the step just
+            // computed (kept) lands on the root to round-off
+            conv = (fabs(dgn - dg) <= fma(tol, dgn, atol)) || (fabs(Fv) <= 1e-12);
             dg = dgn;
             if (conv) break;
         }
@@ -590,54 +599,91 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
     }
 
     // ---- S9/S10 P^ = F^ S^ (Eq.(26) :208) and A^_(ia)(kb) = delta_ik S^_ab + F^_im F^_kn C_L^[(ma)][(nb)] -> shared memory
+    // ---- S11 element residual R^e_Ii = sum_q w P^_ia G^_Ia (Eq.(35) :257), P^ = F^ S^ (Eq.(26) :208): every thread forms
+    //      its own point's 24 contributions, then a 3-step reduce-scatter butterfly over the 8 lanes of the element
+    //      (fixed order => deterministic) leaves node I = q's three sums in this thread.
+    double rI[3];
+    {
+        double Ph[3][3];
 #pragma unroll
-    for (int i = 0; i < 3; i++)
+        for (int i = 0; i < 3; i++)
 #pragma unroll
-        for (int a = 0; a < 3; a++)
-            se[SM_PP + (3 * i + a) * 8 + q] =
-                wq * (Fh[i][0] * Sh[VG[0][a]] + Fh[i][1] * Sh[VG[1][a]] + Fh[i][2] * Sh[VG[2][a]]);
+            for (int a = 0; a < 3; a++)
+                Ph[i][a] = wq * (Fh[i][0] * Sh[VG[0][a]] + Fh[i][1] * Sh[VG[1][a]] + Fh[i][2] * Sh[VG[2][a]]);
+        double r[24];
+#pragma unroll
+        for (int J = 0; J < 8; J++) {
+            const double g0 = se[SM_GG + (3 * J + 0) * 8 + q], g1 = se[SM_GG + (3 * J + 1) * 8 + q], g2 = se[SM_GG + (3 * J + 2) * 8 + q];
+#pragma unroll
+            for (int i = 0; i < 3; i++) r[3 * J + i] = fma(Ph[i][2], g2, fma(Ph[i][1], g1, Ph[i][0] * g0));
+        }
+        const bool b4 = q & 4, b2 = q & 2, b1 = q & 1;
+        double r12[12], r6[6];
+#pragma unroll
+        for (int j = 0; j < 12; j++) {   // keep nodes 0-3 (bit2 = 0) or 4-7, send the other half
+            const double keep = b4 ? r[12 + j] : r[j], send = b4 ? r[j] : r[12 + j];
+            r12[j] = keep + __shfl_xor_sync(0xffffffffu, send, 4);
+        }
+#pragma unroll
+        for (int j = 0; j < 6; j++) {
+            const double keep = b2 ? r12[6 + j] : r12[j], send = b2 ? r12[j] : r12[6 + j];
+            r6[j] = keep + __shfl_xor_sync(0xffffffffu, send, 2);
+        }
+#pragma unroll
+        for (int j = 0; j < 3; j++) {
+            const double keep = b1 ? r6[3 + j] : r6[j], send = b1 ? r6[j] : r6[3 + j];
+            rI[j] = keep + __shfl_xor_sync(0xffffffffu, send, 1);
+        }
+    }
+    // ---- S9/S10 A^_(ia)(kb) = delta_ik S^_ab + F^_im F^_kn C_L^[(ma)][(nb)] (weighted) -> shared memory, packed symmetric,
+    //      two entries per 16-byte slot so that phase 2 reads them with one broadcast LDS.128
 #pragma unroll
     for (int A = 0; A < 6; A++) {
         Sh[A] *= wgt;
 #pragma unroll
         for (int B = A; B < 6; B++) CL[A][B] *= wgt;
     }
+    {
+        double prev = 0.0;
 #pragma unroll
-    for (int i = 0; i < 3; i++) {
-        double X[3][6];  // X[a][B] = sum_m F^_im C_L^[(ma)][B]
+        for (int i = 0; i < 3; i++) {
+            double X[3][6];  // X[a][B] = sum_m F^_im C_L^[(ma)][B]
 #pragma unroll
-        for (int a = 0; a < 3; a++)
+            for (int a = 0; a < 3; a++)
 #pragma unroll
-            for (int B = 0; B < 6; B++) {
-                double x = 0.0;
+                for (int B = 0; B < 6; B++) {
+                    double x = 0.0;
 #pragma unroll
-                for (int m = 0; m < 3; m++) {
-                    const int A = VG[m][a];
-                    x = fma(Fh[i][m], (A <= B) ? CL[A][B] : CL[B][A], x);
+                    for (int m = 0; m < 3; m++) {
+                        const int A = VG[m][a];
+                        x = fma(Fh[i][m], (A <= B) ? CL[A][B] : CL[B][A], x);
+                    }
+                    X[a][B] = x;
                 }
-                X[a][B] = x;
-            }
 #pragma unroll
-        for (int a = 0; a < 3; a++)
+            for (int a = 0; a < 3; a++)
 #pragma unroll
-            for (int k = i; k < 3; k++)
+                for (int k = i; k < 3; k++)
 #pragma unroll
-                for (int b = 0; b < 3; b++) {
-                    if (3 * k + b < 3 * i + a) continue;
-                    double v = (k == i) ? Sh[VG[a][b]] : 0.0;
+                    for (int b = 0; b < 3; b++) {
+                        if (3 * k + b < 3 * i + a) continue;
+                        double v = (k == i) ? Sh[VG[a][b]] : 0.0;
 #pragma unroll
-                    for (int n = 0; n < 3; n++) v = fma(X[a][VG[n][b]], Fh[k][n], v);
-                    se[SM_AA + sidx9(3 * i + a, 3 * k + b) * 8 + q] = v;
-                }
+                        for (int n = 0; n < 3; n++) v = fma(X[a][VG[n][b]], Fh[k][n], v);
+                        const int sI = sidx9(3 * i + a, 3 * k + b);   // 0..44, visited in increasing order
+                        if (sI == 44) se[SM_AA + 352 + q] = v;
+                        else if (sI & 1) *reinterpret_cast<double2 *>(se + SM_AA + (sI >> 1) * 16 + 2 * q) = make_double2(prev, v);
+                        else prev = v;
+                    }
+        }
     }
     __syncwarp();
 
-    // ---- S11/S12 phase 2: thread t = node I of the element.  K^e_(Ii)(Kk) = sum_q G^_Ia A^_(ia)(kb) G^_Kb (Eq.(37) :267),
-    //      R^e_Ii = sum_q P^_ia G^_Ia (Eq.(35) :257).  Symmetry: thread I owns blocks (I, I+d mod 8), d = 0..4
-    //      (d = 4 only for I < 4) and writes their transposes.
+    // ---- S12 phase 2: thread t = node I of the element.  K^e_(Ii)(Kk) = sum_q G^_Ia A^_(ia)(kb) G^_Kb (Eq.(37) :267).
+    //      Symmetry: thread I owns blocks (I, I+d mod 8), d = 0..4 (d = 4 only for I < 4); the transposes are implied
+    //      (fbar = 0: packed scratch) or written explicitly (fbar = 1: full scratch).
     const int I = q;
     double acc[5][9];
-    double racc[3] = {0, 0, 0};
     double rq[FBAR ? 8 : 1][3];
 #pragma unroll
     for (int d = 0; d < 5; d++)
@@ -646,22 +692,36 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
 #pragma unroll 1
     for (int qq = 0; qq < 8; qq++) {
         const double *sq = se + qq;
-        const double gI0 = sq[SM_GG + (3 * I + 0) * 8], gI1 = sq[SM_GG + (3 * I + 1) * 8], gI2 = sq[SM_GG + (3 * I + 2) * 8];
-        double aik[3][9];  // a_{i,(kb)} = sum_a G^_Ia A^_(ia)(kb)
+        const double gI[3] = {sq[SM_GG + (3 * I + 0) * 8], sq[SM_GG + (3 * I + 1) * 8], sq[SM_GG + (3 * I + 2) * 8]};
+        double aik[3][9];  // a_{i,(kb)} = sum_a G^_Ia A^_(ia)(kb): each stored entry (r,c) feeds a[r/3][c] and a[c/3][r]
 #pragma unroll
         for (int i = 0; i < 3; i++)
 #pragma unroll
-            for (int kb = 0; kb < 9; kb++)
-                aik[i][kb] = gI0 * sq[SM_AA + sidx9(3 * i + 0, kb) * 8] + gI1 * sq[SM_AA + sidx9(3 * i + 1, kb) * 8] +
-                             gI2 * sq[SM_AA + sidx9(3 * i + 2, kb) * 8];
+            for (int kb = 0; kb < 9; kb++) aik[i][kb] = 0.0;
 #pragma unroll
-        for (int i = 0; i < 3; i++)
-            racc[i] += sq[SM_PP + (3 * i + 0) * 8] * gI0 + sq[SM_PP + (3 * i + 1) * 8] * gI1 + sq[SM_PP + (3 * i + 2) * 8] * gI2;
+        for (int pr = 0; pr < 23; pr++) {
+            double2 av;
+            if (pr < 22) av = *reinterpret_cast<const double2 *>(se + SM_AA + pr * 16 + 2 * qq);
+            else { av.x = se[SM_AA + 352 + qq]; av.y = 0.0; }
+#pragma unroll
+            for (int h = 0; h < 2; h++) {
+                const int sI = 2 * pr + h;
+                if (sI > 44) continue;
+                // invert sidx9: row r with r*9 - r(r-1)/2 <= sI
+                int r = 0;
+#pragma unroll
+                for (int rr = 1; rr < 9; rr++) if (rr * 9 - rr * (rr - 1) / 2 <= sI) r = rr;
+                const int c = r + (sI - (r * 9 - r * (r - 1) / 2));
+                const double A = h ? av.y : av.x;
+                aik[r / 3][c] = fma(A, gI[r % 3], aik[r / 3][c]);
+                if (r != c) aik[c / 3][r] = fma(A, gI[c % 3], aik[c / 3][r]);
+            }
+        }
         if (FBAR) {
 #pragma unroll
             for (int i = 0; i < 3; i++)
-                rq[FBAR ? qq : 0][i] = sq[SM_YY + (3 * i + 0) * 8] * gI0 + sq[SM_YY + (3 * i + 1) * 8] * gI1 +
-                                       sq[SM_YY + (3 * i + 2) * 8] * gI2;
+                rq[FBAR ? qq : 0][i] = sq[SM_YY + (3 * i + 0) * 8] * gI[0] + sq[SM_YY + (3 * i + 1) * 8] * gI[1] +
+                                       sq[SM_YY + (3 * i + 2) * 8] * gI[2];
         }
 #pragma unroll
         for (int d = 0; d < 5; d++) {
@@ -672,30 +732,33 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
             for (int i = 0; i < 3; i++)
 #pragma unroll
                 for (int k = 0; k < 3; k++)
-                    acc[d][3 * i + k] += aik[i][3 * k + 0] * gK0 + aik[i][3 * k + 1] * gK1 + aik[i][3 * k + 2] * gK2;
+                    acc[d][3 * i + k] = fma(aik[i][3 * k + 2], gK2, fma(aik[i][3 * k + 1], gK1, fma(aik[i][3 * k + 0], gK0, acc[d][3 * i + k])));
         }
     }
     if (FBAR) {  // gbar_Kk = sum_q (w_q J_q / (Jbar V)) g^q_Kk for node K = I
 #pragma unroll
         for (int k = 0; k < 3; k++) {
-            double s = 0.0;
+            double sgb = 0.0;
 #pragma unroll
-            for (int qq = 0; qq < 8; qq++) s = fma(se[SM_WQ + qq], se[SM_GQ + (3 * I + k) * 8 + qq], s);
-            se[SM_GB + 3 * I + k] = s;
+            for (int qq = 0; qq < 8; qq++) sgb = fma(se[SM_WQ + qq], se[SM_GQ + (3 * I + k) * 8 + qq], sgb);
+            se[SM_GB + 3 * I + k] = sgb;
         }
     }
     __syncwarp();
-    // ---- phase 3: stage K^e block-major [I][K][i][k] in shared memory (overlays GG/AA/PP)
+    // ---- phase 3: stage K^e in shared memory (overlays GG/AA).  fbar = 0: packed symmetric, 36 blocks [p][i][k] with
+    //      p(I,d) = 4 I + d (d < 4), 32 + I (d = 4);  fbar = 1: full block-major [I][K][i][k]
+    constexpr int KSZ = FBAR ? 576 : 324;
 #pragma unroll
     for (int d = 0; d < 5; d++) {
         if (d == 4 && I >= 4) continue;
         const int K = (I + d) & 7;
+        const int pb = FBAR ? (I * 8 + K) : ((d < 4) ? (4 * I + d) : (32 + I));
 #pragma unroll
         for (int i = 0; i < 3; i++)
 #pragma unroll
             for (int k = 0; k < 3; k++) {
-                se[SM_KS + (I * 8 + K) * 9 + 3 * i + k] = acc[d][3 * i + k];
-                if (d != 0) se[SM_KS + (K * 8 + I) * 9 + 3 * k + i] = acc[d][3 * i + k];
+                se[SM_KS + pb * 9 + 3 * i + k] = acc[d][3 * i + k];
+                if (FBAR && d != 0) se[SM_KS + (K * 8 + I) * 9 + 3 * k + i] = acc[d][3 * i + k];
             }
     }
     if (FBAR) {
@@ -725,19 +788,20 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
     }
     if (valid) {
         double *ro = Re + e * 24 + 3 * I;
-        ro[0] = racc[0]; ro[1] = racc[1]; ro[2] = racc[2];
+        ro[0] = rI[0]; ro[1] = rI[1]; ro[2] = rI[2];
     }
     __syncwarp();
-    // coalesced copy-out of the warp's 4 elements (4 x 576 doubles), 16 bytes per lane per step
+    // coalesced copy-out of the warp's 4 elements (4 x KSZ doubles), 16 bytes per lane per step
     {
         const int w_el0 = (tid >> 5) * 4;
         const long long e0 = (long long)blockIdx.x * EL_PER_CTA + w_el0;
-#pragma unroll 4
-        for (int idx = lane; idx < 4 * 288; idx += 32) {
-            const int el = idx / 288, off = idx - el * 288;
+#pragma unroll
+        for (int el = 0; el < 4; el++) {
             if (e0 + el < n_elems) {
-                const double2 v = *reinterpret_cast<const double2 *>(sm + (w_el0 + el) * ES + SM_KS + 2 * off);
-                *reinterpret_cast<double2 *>(Ke + (e0 + el) * 576 + 2 * off) = v;
+                const double2 *src = reinterpret_cast<const double2 *>(sm + (w_el0 + el) * ES + SM_KS);
+                double2 *dst = reinterpret_cast<double2 *>(Ke + (e0 + el) * KSZ);
+#pragma unroll
+                for (int idx = lane; idx < KSZ / 2; idx += 32) dst[idx] = src[idx];
             }
         }
     }
@@ -755,8 +819,17 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
             if (mf) atomicAdd(&stats[3], (unsigned long long)__popc(mf));
         }
         if (valid && plastic) atomicAdd(&s_hist[iters < 63 ? iters : 63], 1u);
-        __syncthreads();
-        if (tid < 64 && s_hist[tid]) atomicAdd(&stats[5 + tid], (unsigned long long)s_hist[tid]);
+        __syncwarp();
+        unsigned done = 0;
+        if (lane == 0) { __threadfence_block(); done = atomicAdd(&s_done, 1u); }
+        done = __shfl_sync(0xffffffffu, done, 0);
+        if (done == (blockDim.x >> 5) - 1) {   // last warp of the CTA: flush (no CTA-wide barrier at the tail)
+            __threadfence_block();
+            for (int b = lane; b < 64; b += 32) {
+                const unsigned v = s_hist[b];
+                if (v) atomicAdd(&stats[5 + b], (unsigned long long)v);
+            }
+        }
     }
 }
 
@@ -764,6 +837,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
 // One warp per node n (3 CSR rows).  Lane <-> neighbour position pos: the 3x3 block (n, nb[pos]) is the sum over the
 // incident elements (ascending id) that contain nb[pos]; elem_pos bytes give the local node K of that neighbour.
 // K = A K^e, R = A R^e (Eq.(34) :253, Eq.(38) :274) with a fixed summation order and no atomics.
+template <int PACKED>
 __global__ void __launch_bounds__(256)
 k_gather(long long n_nodes, const int *__restrict__ inc_ptr, const int *__restrict__ inc, const int *__restrict__ nb_ptr,
          const unsigned char *__restrict__ elem_pos, const double *__restrict__ Ke, const double *__restrict__ Re,
@@ -785,9 +859,28 @@ k_gather(long long n_nodes, const int *__restrict__ inc_ptr, const int *__restri
             while (hit) {
                 const int K = (__ffsll((long long)hit) - 1) >> 3;
                 hit &= hit - 1;
-                const double *kb = Ke + (t * 8 + K) * 9;
+                if (PACKED) {
+                    // packed symmetric scratch: block (I,K) is stored by its owner (I, d = K-I mod 8 in 0..3, or d = 4 and I < 4),
+                    // otherwise it is the transpose of the block owned by K
+                    const int I = (int)(t & 7), d = (K - I) & 7;
+                    const bool direct = (d < 4) || (d == 4 && I < 4);
+                    const int oI = direct ? I : K, od = direct ? d : (8 - d);
+                    const int pb = (od < 4) ? (4 * oI + od) : (32 + oI);
+                    const double *kb = Ke + (t >> 3) * 324 + pb * 9;
+                    if (direct) {
 #pragma unroll
-                for (int j = 0; j < 9; j++) acc[j] += kb[j];
+                        for (int j = 0; j < 9; j++) acc[j] += kb[j];
+                    } else {
+#pragma unroll
+                        for (int i = 0; i < 3; i++)
+#pragma unroll
+                            for (int k = 0; k < 3; k++) acc[3 * i + k] += kb[3 * k + i];
+                    }
+                } else {
+                    const double *kb = Ke + (t * 8 + K) * 9;
+#pragma unroll
+                    for (int j = 0; j < 9; j++) acc[j] += kb[j];
+                }
             }
         }
         double *out = csr_vals + 9LL * o + 3 * pos;
@@ -842,8 +935,12 @@ int fem_launch_assemble(fem_ctx *c, const double *u, const double *hist_in, cons
             c->n_elems, c->d_coords, c->d_conn, u, hist_in, c->d_matd, mstride, c->opt.tol, c->opt.kmax, c->d_Ke, c->d_Re,
             hist_out, c->d_stats);
     FEM_CUDA(cudaEventRecord(c->ev[2], st));
-    k_gather<<<nblk2(c->n_nodes * 32, 256), 256, 0, st>>>(c->n_nodes, c->d_inc_ptr, c->d_inc, c->d_nb_ptr, c->d_elem_pos,
-                                                          c->d_Ke, c->d_Re, csr_vals, residual);
+    if (c->opt.fbar)
+        k_gather<0><<<nblk2(c->n_nodes * 32, 256), 256, 0, st>>>(c->n_nodes, c->d_inc_ptr, c->d_inc, c->d_nb_ptr,
+                                                                 c->d_elem_pos, c->d_Ke, c->d_Re, csr_vals, residual);
+    else
+        k_gather<1><<<nblk2(c->n_nodes * 32, 256), 256, 0, st>>>(c->n_nodes, c->d_inc_ptr, c->d_inc, c->d_nb_ptr,
+                                                                 c->d_elem_pos, c->d_Ke, c->d_Re, csr_vals, residual);
     FEM_CUDA(cudaEventRecord(c->ev[3], st));
     FEM_CUDA(cudaGetLastError());
     c->ev_valid = true;
