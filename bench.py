@@ -103,6 +103,19 @@ class ClockSampler:
         return out
 
 
+def aggregate_over_ranks(ms_local, n_units_per_rank, world, device=None):
+    """max-over-ranks step time and whole-job throughput (units of all ranks / slowest rank's time); weak scaling:
+    every rank processes its own replica, no data-path collective.  Works with any torch.distributed backend."""
+    ms = float(ms_local)
+    if world > 1:
+        import torch
+        import torch.distributed as dist
+        t = torch.tensor([ms], dtype=torch.float64, device=device)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    return ms, world * n_units_per_rank / (ms * 1e-3)
+
+
 def slab_sample(cfg, n, layers):
     """First `layers` z-layers of the n^3 mesh as a self-contained sub-mesh (nodes are lexicographic, so contiguous)."""
     ne, nn = layers * n * n, (layers + 1) * (n + 1) * (n + 1)
@@ -216,12 +229,7 @@ def run_gpu(args):
         for key in kms:
             kms[key] += k[key] / args.steps
     clk = clocks.stop()
-    if world > 1:
-        t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
-    ms_step = ms_total / args.steps
-    value = world * ne / (ms_step * 1e-3)
+    ms_step, value = aggregate_over_ranks(ms_total / args.steps, ne, world, dev)
 
     # ---- end-to-end: host buffers through fem_assemble_host, copies inside the timed region
     e2e_steps = max(1, min(args.steps, 5))
