@@ -265,10 +265,13 @@ def run_gpu(args):
     dom = max(("element", "gather"), key=lambda k: kms[k])
     ach_tf = fl_el * ne / (kms["element"] * 1e-3) / 1e12
     traffic = None
-    tp = os.path.join(ROOT, "profiles", "traffic.json")
+    tp = os.path.join(ROOT, "profiles", "traffic.csv")   # per-launch DRAM bytes from the committed ncu --set full capture
     if os.path.exists(tp):
         try:
-            traffic = json.load(open(tp)).get("k_element_dram_bytes_per_launch")
+            for line in open(tp):
+                c = line.split(",")
+                if c[0] == "k_element":
+                    traffic = float(c[1])
         except Exception:
             traffic = None
     roofline = {"bound": "alu", "kernel": "k_element", "achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s",
