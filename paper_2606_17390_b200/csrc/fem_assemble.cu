@@ -101,7 +101,7 @@ __device__ __forceinline__ double atanhc(double w, double dlog /* = ln b - ln a 
 // Second divided difference g[a,b,c] of g = 1/2 ln, with x1<=x2<=x3 not required.
 // Far apart: recursion on the widest gap from first divided differences; close together: Taylor series about the mean,
 // g[a,b,c] = 1/(2 m^2) sum_{n>=2} (-1)^(n+1)/n h_{n-2}(x), x_i = (l_i - m)/m, h_k = complete homogeneous polynomial.
-__device__ __forceinline__ double dd2_series(double la, double lb, double lc) {
+__device__ __noinline__ double dd2_series(double la, double lb, double lc) {
     double m = (la + lb + lc) * (1.0 / 3.0), im = 1.0 / m;
     double xa = (la - m) * im, xb = (lb - m) * im, xc = (lc - m) * im;
     // h_k(a), h_k(a,b), h_k(a,b,c) by the recurrences h_k(a,b) = a^k + b h_{k-1}(a,b), h_k(a,b,c) = h_k(a,b) + c h_{k-1}(a,b,c)
@@ -150,6 +150,16 @@ __device__ __forceinline__ void flow_stress(double law, double h0, double h1, do
     }
 }
 
+// Keeping the warps of a CTA in the same code region lets them share instruction-cache lines (the kernel is ~94 KB of
+// straight-line SASS); ncu showed instruction fetch as a top stall without it.
+#ifndef PHASE_SYNC_ON
+#define PHASE_SYNC_ON 1
+#endif
+#if PHASE_SYNC_ON
+#define PHASE_SYNC() __syncthreads()
+#else
+#define PHASE_SYNC() ((void)0)
+#endif
 template <int FBAR>
 __global__ void __launch_bounds__(128, FBAR ? 2 : 3)
 k_element(long long n_elems, const double *__restrict__ coords, const int *__restrict__ conn,
@@ -263,6 +273,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
         wgt = wq * cq;
     }
 
+    PHASE_SYNC();
     // ---- S5 C = F^T F and its spectral decomposition by cyclic Jacobi (Eq.(4) :92; backward stable, fixed 4 sweeps)
     double c00 = F[0][0] * F[0][0] + F[1][0] * F[1][0] + F[2][0] * F[2][0];
     double c11 = F[0][1] * F[0][1] + F[1][1] * F[1][1] + F[2][1] * F[2][1];
@@ -279,6 +290,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
     }
     const double lam[3] = {c00, c11, c22};
 
+    PHASE_SYNC();
     // ---- rotate F and G into the eigenbasis (Lagrangian principal axes): F^_ia = F_iJ R_Ja, G^_Ia = G_IJ R_Ja
     double Fh[3][3];
 #pragma unroll
@@ -351,6 +363,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
 #pragma unroll
     for (int i = 0; i < 6; i++) ee[i] -= epm[i];
 
+    PHASE_SYNC();
     // ---- S6 elastic predictor in the Hill eigenbasis: T_tr = p I + s, s = 2mu dev(ee) = sum_k c_k v_k (Eq.(16) :160)
     const double tre = ee[0] + ee[1] + ee[2];
     const double pres = kb * tre;
@@ -372,19 +385,21 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
     for (int k = 0; k < 5; k++) { hc2[k] = hk[k] * ck[k] * ck[k]; phitr2 += hc2[k]; }
     const double phitr = sqrt(phitr2);  // Eq.(11) :127
     const double law = __ldg(md + 3), hh0 = __ldg(md + 4), hh1 = __ldg(md + 5), hh2 = __ldg(md + 6);
-    double sf, dsf;
-    flow_stress(law, hh0, hh1, hh2, alphan, sf, dsf);
-    const bool plastic = (phitr - W23 * sf) > 0.0;  // f_tr = phi(T_tr) - sqrt(2/3) sigma_flow(alpha_n), Eq.(17) :165 ; tie -> elastic
-
-    // ---- S7 return map: sigma_y(alpha)/phi(x) - 1 = 0 in dgam, x = 2mu dgam / sigma_y
-    double dg = 0.0, xs = 0.0;
+    // ---- S6/S7 yield test and return map in ONE loop with a single evaluation site (code size): pass 0 evaluates the
+    //      trial state (dgam = 0): f_tr = phi(T_tr) - sqrt(2/3) sigma_flow(alpha_n) (Eq.(17) :165, tie -> elastic); later
+    //      passes are Newton on F(dgam) = sigma_y(alpha)/phi(x) - 1, x = 2mu dgam / sigma_y;
+    //      the pass after convergence evaluates the state at the solution and leaves the loop.
+    double dg = 0.0, sf = 0.0, dsf = 0.0;
+    double rk[5] = {1.0, 1.0, 1.0, 1.0, 1.0};   // 1/(1 + x h_k)
+    double phi2 = phitr2;
     int iters = 0;
-    bool nonconv = false;
-    if (plastic) {
+    bool plastic = false, nonconv = false;
+    {
         double lo = 0.0, hi = INFINITY;
         const double atol = 4.0e-16 * phitr / mu2;  // round-off floor of dgam (a strain): eps * |T| / 2mu
         bool conv = false;
-        for (iters = 1; iters <= kmax; iters++) {
+#pragma unroll 1
+        for (int pass = 0;; pass++) {
             const double al = fma(W23, dg, alphan);
             flow_stress(law, hh0, hh1, hh2, al, sf, dsf);
             const double sy = W23 * sf, dsy = W23 * dsf;
@@ -395,8 +410,16 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
             for (int k = 0; k < 5; k++) {
                 const double r = 1.0 / fma(x, hk[k], 1.0);
                 const double t2 = hc2[k] * r * r;
+                rk[k] = r;
                 S2 += t2; S3 = fma(t2 * r, hk[k], S3);
             }
+            phi2 = S2;
+            if (pass == 0) {
+                plastic = (phitr - sy) > 0.0;
+                if (!plastic) break;
+            }
+            if (conv || pass > kmax) { nonconv = !conv; break; }
+            iters = pass + 1;
             const double rphi = rsqrt(S2);
             const double Fv = fma(sy, rphi, -1.0);
             const double dxd = mu2 * isy * (1.0 - dg * dsy * W23 * isy);
@@ -404,26 +427,16 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
             if (Fv < 0.0) lo = dg; else hi = dg;
             double dgn = dg - Fv / Fp;
             if (!(dgn >= lo && dgn <= hi)) dgn = (hi < INFINITY) ? 0.5 * (lo + hi) : 2.0 * dg + 1e-12;
-                        // converged when the step is at the round-off floor, or when the residual is so small that the step just
+            // converged when the step is at the round-off floor, or when the residual is so small that the step just
             // computed (kept) lands on the root to round-off
             conv = (fabs(dgn - dg) <= fma(tol, dgn, atol)) || (fabs(Fv) <= 1e-12);
             dg = dgn;
-            if (conv) break;
         }
-        nonconv = !conv;
-        if (iters > kmax) iters = kmax;
     }
-    // state at the solution (elastic: dg = 0)
     const double alpha1 = fma(W23, dg, alphan);
-    flow_stress(law, hh0, hh1, hh2, alpha1, sf, dsf);
     double th[5], cn[5];   // theta_k = 2mu/(1+x h_k) ; c'_k = c_k/(1+x h_k)
-    double phi2 = 0.0;
-    xs = mu2 * dg / (W23 * sf);
 #pragma unroll
-    for (int k = 0; k < 5; k++) {
-        const double r = 1.0 / fma(xs, hk[k], 1.0);
-        th[k] = mu2 * r; cn[k] = ck[k] * r; phi2 += hk[k] * cn[k] * cn[k];
-    }
+    for (int k = 0; k < 5; k++) { th[k] = mu2 * rk[k]; cn[k] = ck[k] * rk[k]; }
     // flow direction N = H:T/phi (Eq.(13) :141) in the Hill eigenbasis, m = D^-1 N, beta of C_ep = D^-1 + beta m (x) m
     double mk[5], beta = 0.0;
     double nk[5];
@@ -440,6 +453,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
             beta = (kap * den - 1.0) / (om * den);
         }
     }
+    PHASE_SYNC();
     // ---- S10 history out: eps_p += dgam N, alpha += W dgam (Eq.(19)-(20) :176-178), back to global components
     if (valid) {
         double *ho = hist_out + (e * 8 + q) * 7;
@@ -471,6 +485,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
         ho[6] = alpha1;
     }
 
+    PHASE_SYNC();
     // ---- S8 algorithmic tangent in the eigenbasis of C (App. D :1002-1019 in closed form):
     //      C_ep = kb I(x)I + sum_k theta_k V^_k (x) V^_k + beta m^ (x) m^ ,  V^_k = Rm^T V_k Rm ; T^ = p I + sum c'_k V^_k
     double Ch[6][6];   // tensor components, upper triangle used
@@ -513,6 +528,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
         for (int B = A; B < 6; B++) Ch[A][B] = fma(bm, mh[B], Ch[A][B]);
     }
 
+    PHASE_SYNC();
     // ---- S9 geometric post-processor (Eq.(25) :204, analytic route of :288): with g = 1/2 ln,
     //      S^_ab = 2 g[a,b] T^_ab ;  C_L = P_L^T:C_ep:P_L + T:L_L  in the eigenbasis
     double d1[6];  // first divided differences g[a,b], Voigt-indexed: (00,11,22,01,12,02)
@@ -599,6 +615,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
     }
 
     // ---- S9/S10 P^ = F^ S^ (Eq.(26) :208) and A^_(ia)(kb) = delta_ik S^_ab + F^_im F^_kn C_L^[(ma)][(nb)] -> shared memory
+    PHASE_SYNC();
     // ---- S11 element residual R^e_Ii = sum_q w P^_ia G^_Ia (Eq.(35) :257), P^ = F^ S^ (Eq.(26) :208): every thread forms
     //      its own point's 24 contributions, then a 3-step reduce-scatter butterfly over the 8 lanes of the element
     //      (fixed order => deterministic) leaves node I = q's three sums in this thread.
@@ -635,6 +652,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
             rI[j] = keep + __shfl_xor_sync(0xffffffffu, send, 1);
         }
     }
+    PHASE_SYNC();
     // ---- S9/S10 A^_(ia)(kb) = delta_ik S^_ab + F^_im F^_kn C_L^[(ma)][(nb)] (weighted) -> shared memory, packed symmetric,
     //      two entries per 16-byte slot so that phase 2 reads them with one broadcast LDS.128
 #pragma unroll
@@ -679,6 +697,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
     }
     __syncwarp();
 
+    PHASE_SYNC();
     // ---- S12 phase 2: thread t = node I of the element.  K^e_(Ii)(Kk) = sum_q G^_Ia A^_(ia)(kb) G^_Kb (Eq.(37) :267).
     //      Symmetry: thread I owns blocks (I, I+d mod 8), d = 0..4 (d = 4 only for I < 4); the transposes are implied
     //      (fbar = 0: packed scratch) or written explicitly (fbar = 1: full scratch).
@@ -745,6 +764,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
         }
     }
     __syncwarp();
+    PHASE_SYNC();
     // ---- phase 3: stage K^e in shared memory (overlays GG/AA).  fbar = 0: packed symmetric, 36 blocks [p][i][k] with
     //      p(I,d) = 4 I + d (d < 4), 32 + I (d = 4);  fbar = 1: full block-major [I][K][i][k]
     constexpr int KSZ = FBAR ? 576 : 324;
