@@ -129,7 +129,7 @@ def _ptr(t, dtype, numel=None, name="tensor"):
 class FemContext:
     """fem_setup + fem_build_csr_pattern + fem_assemble on torch CUDA tensors (device memory and streams only)."""
 
-    def __init__(self, coords, conn, fbar=0, tol=None, kmax=None):
+    def __init__(self, coords, conn, fbar=0, tol=None, kmax=None, assembly_mode=None):
         torch = _torch()
         L = lib()
         if not torch.cuda.is_available():
@@ -142,6 +142,8 @@ class FemContext:
             opt.tol = float(tol)
         if kmax is not None:
             opt.kmax = int(kmax)
+        if assembly_mode is not None:
+            opt.assembly_mode = int(assembly_mode)
         self._h = C.c_void_p()
         _check(L.fem_setup(C.byref(self._h), self.n_nodes, _ptr(coords, torch.float64, 3 * self.n_nodes, "coords"),
                            self.n_elems, _ptr(conn, torch.int32, 8 * self.n_elems, "conn"), C.byref(opt)), "fem_setup")

@@ -80,7 +80,10 @@ extern "C" int fem_last_kernel_ms(fem_ctx *c, double ms[3]) {
     return FEM_OK;
 }
 
-extern "C" int fem_launches_per_assemble(const fem_ctx *c) { return c ? 3 : 0; }
+extern "C" int fem_launches_per_assemble(const fem_ctx *c) {
+    if (!c) return 0;
+    return c->mode == 1 ? 1 + c->n_colours : 3;   // mat_prep + one element launch per colour | mat_prep + element + gather
+}
 
 // ------------------------------------------------------------------------------------------------ FP64 peak probe
 // 8 independent FMA chains per thread, all operands in registers; 148 SMs x 8 CTAs x 256 threads.

@@ -160,12 +160,22 @@ __device__ __forceinline__ void flow_stress(double law, double h0, double h1, do
 #else
 #define PHASE_SYNC() ((void)0)
 #endif
-template <int FBAR>
+// MODE 0: K^e, R^e go to an HBM scratch (k_gather sums them).  MODE 1: launched once per colour (elist = the colour's
+// elements); K^e, R^e are added in place into csr_vals / residual (no two elements of a launch share a node).
+struct scatter_args {
+    const int *elist;                       // element ids of this launch (MODE 1), nullptr = identity
+    const int *nb_ptr;                      // node -> first neighbour block; CSR rows of node n start at 9*nb_ptr[n]
+    const unsigned char *elem_pos;          // [e][I][K] rank of node K in the neighbour list of node I
+    const unsigned long long *first_mask;   // bit I*8+K: store instead of add
+    const unsigned int *first_res;          // bit I: store the residual instead of add
+    double *csr_vals, *residual;
+};
+template <int FBAR, int MODE>
 __global__ void __launch_bounds__(128, FBAR ? 2 : 3)
 k_element(long long n_elems, const double *__restrict__ coords, const int *__restrict__ conn,
           const double *__restrict__ u, const double *__restrict__ hist_in, const double *__restrict__ matd,
           int mat_stride, double tol, int kmax, double *__restrict__ Ke, double *__restrict__ Re,
-          double *__restrict__ hist_out, unsigned long long *__restrict__ stats) {
+          double *__restrict__ hist_out, unsigned long long *__restrict__ stats, const scatter_args sa) {
     extern __shared__ __align__(16) double sm[];
     __shared__ unsigned int s_hist[64];
     __shared__ unsigned int s_done;
@@ -174,15 +184,18 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
     const int el_cta = tid >> 3;
     const long long e_raw = (long long)blockIdx.x * EL_PER_CTA + el_cta;
     const bool valid = e_raw < n_elems;
-    const long long e = valid ? e_raw : n_elems - 1;
+    const long long e_slot = valid ? e_raw : n_elems - 1;
+    const long long e = (MODE == 1 && sa.elist) ? (long long)sa.elist[e_slot] : e_slot;
     double *se = sm + el_cta * ES;
     if (tid < 64) s_hist[tid] = 0;
     if (tid == 64) s_done = 0;
     __syncthreads();
 
     // ---- S2 gather: thread q loads node q of its element
+    int my_node;
     {
-        long long nd = conn[e * 8 + q];
+        const long long nd = conn[e * 8 + q];
+        my_node = (int)nd;
         se[SM_XE + 3 * q + 0] = coords[3 * nd + 0]; se[SM_XE + 3 * q + 1] = coords[3 * nd + 1];
         se[SM_XE + 3 * q + 2] = coords[3 * nd + 2];
         se[SM_UE + 3 * q + 0] = u[3 * nd + 0]; se[SM_UE + 3 * q + 1] = u[3 * nd + 1]; se[SM_UE + 3 * q + 2] = u[3 * nd + 2];
@@ -765,64 +778,131 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
     }
     __syncwarp();
     PHASE_SYNC();
-    // ---- phase 3: stage K^e in shared memory (overlays GG/AA).  fbar = 0: packed symmetric, 36 blocks [p][i][k] with
-    //      p(I,d) = 4 I + d (d < 4), 32 + I (d = 4);  fbar = 1: full block-major [I][K][i][k]
-    constexpr int KSZ = FBAR ? 576 : 324;
-#pragma unroll
-    for (int d = 0; d < 5; d++) {
-        if (d == 4 && I >= 4) continue;
-        const int K = (I + d) & 7;
-        const int pb = FBAR ? (I * 8 + K) : ((d < 4) ? (4 * I + d) : (32 + I));
-#pragma unroll
-        for (int i = 0; i < 3; i++)
-#pragma unroll
-            for (int k = 0; k < 3; k++) {
-                se[SM_KS + pb * 9 + 3 * i + k] = acc[d][3 * i + k];
-                if (FBAR && d != 0) se[SM_KS + (K * 8 + I) * 9 + 3 * k + i] = acc[d][3 * i + k];
-            }
-    }
-    if (FBAR) {
-        // K^e_(Ii)(Kk) += sum_q w_q/3 r^q_Ii (gbar_Kk - g^q_Kk)   (unsymmetric rank-1 terms)
-        __syncwarp();
-        double rs[3] = {0, 0, 0};
-#pragma unroll
-        for (int qq = 0; qq < 8; qq++)
-#pragma unroll
-            for (int i = 0; i < 3; i++) rs[i] += rq[FBAR ? qq : 0][i];
-#pragma unroll 1
-        for (int K = 0; K < 8; K++)
-#pragma unroll
-            for (int k = 0; k < 3; k++) {
-                const double gb = se[SM_GB + 3 * K + k];
-                double t0 = rs[0] * gb, t1 = rs[1] * gb, t2 = rs[2] * gb;
-#pragma unroll
-                for (int qq = 0; qq < 8; qq++) {
-                    const double g = se[SM_GQ + (3 * K + k) * 8 + qq];
-                    t0 = fma(-rq[FBAR ? qq : 0][0], g, t0); t1 = fma(-rq[FBAR ? qq : 0][1], g, t1);
-                    t2 = fma(-rq[FBAR ? qq : 0][2], g, t2);
+    if (MODE == 0 || FBAR) {
+        // ---- phase 3: stage K^e in shared memory (overlays GG/AA).  fbar = 0: packed symmetric, 36 blocks [p][i][k] with
+        //      p(I,d) = 4 I + d (d < 4), 32 + I (d = 4);  fbar = 1: full block-major [I][K][i][k]
+        #pragma unroll
+        for (int d = 0; d < 5; d++) {
+            if (d == 4 && I >= 4) continue;
+            const int K = (I + d) & 7;
+            const int pb = FBAR ? (I * 8 + K) : ((d < 4) ? (4 * I + d) : (32 + I));
+    #pragma unroll
+            for (int i = 0; i < 3; i++)
+    #pragma unroll
+                for (int k = 0; k < 3; k++) {
+                    se[SM_KS + pb * 9 + 3 * i + k] = acc[d][3 * i + k];
+                    if (FBAR && d != 0) se[SM_KS + (K * 8 + I) * 9 + 3 * k + i] = acc[d][3 * i + k];
                 }
-                se[SM_KS + (I * 8 + K) * 9 + 0 + k] += t0;
-                se[SM_KS + (I * 8 + K) * 9 + 3 + k] += t1;
-                se[SM_KS + (I * 8 + K) * 9 + 6 + k] += t2;
-            }
+        }
+        if (FBAR) {
+            // K^e_(Ii)(Kk) += sum_q w_q/3 r^q_Ii (gbar_Kk - g^q_Kk)   (unsymmetric rank-1 terms)
+            __syncwarp();
+            double rs[3] = {0, 0, 0};
+    #pragma unroll
+            for (int qq = 0; qq < 8; qq++)
+    #pragma unroll
+                for (int i = 0; i < 3; i++) rs[i] += rq[FBAR ? qq : 0][i];
+    #pragma unroll 1
+            for (int K = 0; K < 8; K++)
+    #pragma unroll
+                for (int k = 0; k < 3; k++) {
+                    const double gb = se[SM_GB + 3 * K + k];
+                    double t0 = rs[0] * gb, t1 = rs[1] * gb, t2 = rs[2] * gb;
+    #pragma unroll
+                    for (int qq = 0; qq < 8; qq++) {
+                        const double g = se[SM_GQ + (3 * K + k) * 8 + qq];
+                        t0 = fma(-rq[FBAR ? qq : 0][0], g, t0); t1 = fma(-rq[FBAR ? qq : 0][1], g, t1);
+                        t2 = fma(-rq[FBAR ? qq : 0][2], g, t2);
+                    }
+                    se[SM_KS + (I * 8 + K) * 9 + 0 + k] += t0;
+                    se[SM_KS + (I * 8 + K) * 9 + 3 + k] += t1;
+                    se[SM_KS + (I * 8 + K) * 9 + 6 + k] += t2;
+                }
+        }
     }
-    if (valid) {
-        double *ro = Re + e * 24 + 3 * I;
-        ro[0] = rI[0]; ro[1] = rI[1]; ro[2] = rI[2];
-    }
-    __syncwarp();
-    // coalesced copy-out of the warp's 4 elements (4 x KSZ doubles), 16 bytes per lane per step
-    {
-        const int w_el0 = (tid >> 5) * 4;
-        const long long e0 = (long long)blockIdx.x * EL_PER_CTA + w_el0;
-#pragma unroll
-        for (int el = 0; el < 4; el++) {
-            if (e0 + el < n_elems) {
-                const double2 *src = reinterpret_cast<const double2 *>(sm + (w_el0 + el) * ES + SM_KS);
-                double2 *dst = reinterpret_cast<double2 *>(Ke + (e0 + el) * KSZ);
-#pragma unroll
-                for (int idx = lane; idx < KSZ / 2; idx += 32) dst[idx] = src[idx];
+    if (MODE == 0) {
+        if (valid) {
+            double *ro = Re + e * 24 + 3 * I;
+            ro[0] = rI[0]; ro[1] = rI[1]; ro[2] = rI[2];
+        }
+        __syncwarp();
+        // coalesced copy-out of the warp's 4 elements (4 x KSZ doubles), 16 bytes per lane per step
+        {
+            const int w_el0 = (tid >> 5) * 4;
+            const long long e0 = (long long)blockIdx.x * EL_PER_CTA + w_el0;
+    #pragma unroll
+            for (int el = 0; el < 4; el++) {
+                if (e0 + el < n_elems) {
+                    const double2 *src = reinterpret_cast<const double2 *>(sm + (w_el0 + el) * ES + SM_KS);
+                    double2 *dst = reinterpret_cast<double2 *>(Ke + (e0 + el) * (FBAR ? 576 : 324));
+    #pragma unroll
+                    for (int idx = lane; idx < (FBAR ? 576 : 324) / 2; idx += 32) dst[idx] = src[idx];
+                }
             }
+        }
+
+    }
+    if (MODE == 1) {
+        // ---- S14 in-place assembly (Eq.(34) :253, Eq.(38) :274): no other element of this launch touches this element's
+        //      nodes, so plain read-modify-write is race-free; launches run in colour order => fixed summation order.
+        //      The first contributor of a block (marked at setup) stores, so the outputs need no zero-fill.
+        const int nbI = sa.nb_ptr[my_node], lenI = sa.nb_ptr[my_node + 1] - nbI;
+        const uint2 posI = reinterpret_cast<const uint2 *>(sa.elem_pos)[e * 8 + I];   // bytes pos(I,K), K = 0..7
+        const unsigned long long fm = sa.first_mask[e];
+        const unsigned fr = sa.first_res[e];
+        double *const rowsI = sa.csr_vals + 9LL * nbI;
+        if (FBAR) {
+            __syncwarp();
+#pragma unroll 1
+            for (int K = 0; K < 8; K++) {
+                const int pIK = (int)(((K < 4) ? (posI.x >> (8 * K)) : (posI.y >> (8 * (K - 4)))) & 0xffu);
+                const bool first = (fm >> (I * 8 + K)) & 1ull;
+                if (valid) {
+#pragma unroll
+                    for (int i = 0; i < 3; i++) {
+                        double *a = rowsI + (long long)i * 3 * lenI + 3 * pIK;
+#pragma unroll
+                        for (int k = 0; k < 3; k++) {
+                            const double v = se[SM_KS + (I * 8 + K) * 9 + 3 * i + k];
+                            a[k] = first ? v : a[k] + v;
+                        }
+                    }
+                }
+            }
+        } else {
+#pragma unroll
+            for (int d = 0; d < 5; d++) {
+                const int K = (I + d) & 7;
+                const int srcl = (lane & ~7) | K;   // lane of node K in this element
+                const int nbK = __shfl_sync(0xffffffffu, nbI, srcl), lenK = __shfl_sync(0xffffffffu, lenI, srcl);
+                const unsigned pKx = __shfl_sync(0xffffffffu, posI.x, srcl), pKy = __shfl_sync(0xffffffffu, posI.y, srcl);
+                if ((d == 4 && I >= 4) || !valid) continue;
+                const int pIK = (int)(((K < 4) ? (posI.x >> (8 * K)) : (posI.y >> (8 * (K - 4)))) & 0xffu);
+                const bool first = (fm >> (I * 8 + K)) & 1ull;
+#pragma unroll
+                for (int i = 0; i < 3; i++) {
+                    double *a = rowsI + (long long)i * 3 * lenI + 3 * pIK;
+#pragma unroll
+                    for (int k = 0; k < 3; k++) a[k] = first ? acc[d][3 * i + k] : a[k] + acc[d][3 * i + k];
+                }
+                if (d != 0) {   // transposed block (K,I) into the rows of node K
+                    const int pKI = (int)(((I < 4) ? (pKx >> (8 * I)) : (pKy >> (8 * (I - 4)))) & 0xffu);
+                    const bool first2 = (fm >> (K * 8 + I)) & 1ull;
+                    double *const rowsK = sa.csr_vals + 9LL * nbK + 3 * pKI;
+#pragma unroll
+                    for (int k = 0; k < 3; k++) {
+                        double *a = rowsK + (long long)k * 3 * lenK;
+#pragma unroll
+                        for (int i = 0; i < 3; i++) a[i] = first2 ? acc[d][3 * i + k] : a[i] + acc[d][3 * i + k];
+                    }
+                }
+            }
+        }
+        if (valid) {
+            double *ro = sa.residual + 3LL * my_node;
+            const bool firstr = (fr >> I) & 1u;
+#pragma unroll
+            for (int i = 0; i < 3; i++) ro[i] = firstr ? rI[i] : ro[i] + rI[i];
         }
     }
 
@@ -933,34 +1013,50 @@ int fem_launch_assemble(fem_ctx *c, const double *u, const double *hist_in, cons
         c->n_matd_cap = n_mat;
     }
     static bool attr_set = false;
+    const size_t sm_std = EL_PER_CTA * ES_STD * sizeof(double), sm_fbar = EL_PER_CTA * ES_FBAR * sizeof(double);
     if (!attr_set) {
-        FEM_CUDA(cudaFuncSetAttribute(k_element<0>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                      (int)(EL_PER_CTA * ES_STD * sizeof(double))));
-        FEM_CUDA(cudaFuncSetAttribute(k_element<1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                      (int)(EL_PER_CTA * ES_FBAR * sizeof(double))));
+        FEM_CUDA(cudaFuncSetAttribute(k_element<0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_std));
+        FEM_CUDA(cudaFuncSetAttribute(k_element<0, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_std));
+        FEM_CUDA(cudaFuncSetAttribute(k_element<1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_fbar));
+        FEM_CUDA(cudaFuncSetAttribute(k_element<1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_fbar));
         attr_set = true;
     }
     FEM_CUDA(cudaMemsetAsync(c->d_stats, 0, sizeof(unsigned long long) * 72, st));
     FEM_CUDA(cudaEventRecord(c->ev[0], st));
     k_mat_prep<<<nblk2(n_mat, 128), 128, 0, st>>>(n_mat, mat, c->d_matd);
     FEM_CUDA(cudaEventRecord(c->ev[1], st));
-    const unsigned grid = nblk2(c->n_elems, EL_PER_CTA);
     const int mstride = (n_mat == 1) ? 0 : FEM_MATD;
-    if (c->opt.fbar)
-        k_element<1><<<grid, 128, EL_PER_CTA * ES_FBAR * sizeof(double), st>>>(
-            c->n_elems, c->d_coords, c->d_conn, u, hist_in, c->d_matd, mstride, c->opt.tol, c->opt.kmax, c->d_Ke, c->d_Re,
-            hist_out, c->d_stats);
-    else
-        k_element<0><<<grid, 128, EL_PER_CTA * ES_STD * sizeof(double), st>>>(
-            c->n_elems, c->d_coords, c->d_conn, u, hist_in, c->d_matd, mstride, c->opt.tol, c->opt.kmax, c->d_Ke, c->d_Re,
-            hist_out, c->d_stats);
-    FEM_CUDA(cudaEventRecord(c->ev[2], st));
-    if (c->opt.fbar)
-        k_gather<0><<<nblk2(c->n_nodes * 32, 256), 256, 0, st>>>(c->n_nodes, c->d_inc_ptr, c->d_inc, c->d_nb_ptr,
-                                                                 c->d_elem_pos, c->d_Ke, c->d_Re, csr_vals, residual);
-    else
-        k_gather<1><<<nblk2(c->n_nodes * 32, 256), 256, 0, st>>>(c->n_nodes, c->d_inc_ptr, c->d_inc, c->d_nb_ptr,
-                                                                 c->d_elem_pos, c->d_Ke, c->d_Re, csr_vals, residual);
+    scatter_args sa = {nullptr, c->d_nb_ptr, c->d_elem_pos, c->d_first_mask, c->d_first_res, csr_vals, residual};
+    if (c->mode == 1) {
+        // one launch per colour, in colour order (stream order = summation order)
+        for (int k = 0; k < c->n_colours; k++) {
+            const long long cnt = c->colour_start[k + 1] - c->colour_start[k];
+            sa.elist = c->d_elist + c->colour_start[k];
+            const unsigned grid = nblk2(cnt, EL_PER_CTA);
+            if (c->opt.fbar)
+                k_element<1, 1><<<grid, 128, sm_fbar, st>>>(cnt, c->d_coords, c->d_conn, u, hist_in, c->d_matd, mstride, c->opt.tol,
+                                                            c->opt.kmax, nullptr, nullptr, hist_out, c->d_stats, sa);
+            else
+                k_element<0, 1><<<grid, 128, sm_std, st>>>(cnt, c->d_coords, c->d_conn, u, hist_in, c->d_matd, mstride, c->opt.tol,
+                                                           c->opt.kmax, nullptr, nullptr, hist_out, c->d_stats, sa);
+        }
+        FEM_CUDA(cudaEventRecord(c->ev[2], st));
+    } else {
+        const unsigned grid = nblk2(c->n_elems, EL_PER_CTA);
+        if (c->opt.fbar)
+            k_element<1, 0><<<grid, 128, sm_fbar, st>>>(c->n_elems, c->d_coords, c->d_conn, u, hist_in, c->d_matd, mstride,
+                                                        c->opt.tol, c->opt.kmax, c->d_Ke, c->d_Re, hist_out, c->d_stats, sa);
+        else
+            k_element<0, 0><<<grid, 128, sm_std, st>>>(c->n_elems, c->d_coords, c->d_conn, u, hist_in, c->d_matd, mstride,
+                                                       c->opt.tol, c->opt.kmax, c->d_Ke, c->d_Re, hist_out, c->d_stats, sa);
+        FEM_CUDA(cudaEventRecord(c->ev[2], st));
+        if (c->opt.fbar)
+            k_gather<0><<<nblk2(c->n_nodes * 32, 256), 256, 0, st>>>(c->n_nodes, c->d_inc_ptr, c->d_inc, c->d_nb_ptr,
+                                                                     c->d_elem_pos, c->d_Ke, c->d_Re, csr_vals, residual);
+        else
+            k_gather<1><<<nblk2(c->n_nodes * 32, 256), 256, 0, st>>>(c->n_nodes, c->d_inc_ptr, c->d_inc, c->d_nb_ptr,
+                                                                     c->d_elem_pos, c->d_Ke, c->d_Re, csr_vals, residual);
+    }
     FEM_CUDA(cudaEventRecord(c->ev[3], st));
     FEM_CUDA(cudaGetLastError());
     c->ev_valid = true;

@@ -22,6 +22,14 @@ struct fem_ctx {
     int *d_col_idx = nullptr;    // [nnz]
     unsigned char *d_elem_pos = nullptr;  // [n_elems*64]  pos(conn[e][I], conn[e][K]) = rank of node K in nb list of node I
     int *d_elem_slot = nullptr;  // [n_elems*576], built on request
+    // colouring (assembly_mode 1): elements grouped by colour, first-writer masks
+    int *d_elist = nullptr;                       // [n_elems] element ids sorted by (colour, id)
+    unsigned long long *d_first_mask = nullptr;   // [n_elems] bit I*8+K: this element stores block (I,K) instead of adding
+    unsigned int *d_first_res = nullptr;          // [n_elems] bit I: this element stores the residual of its local node I
+    int mode = 0;                                 // effective assembly mode (1 falls back to 0 for collapsed elements)
+    bool has_collapsed = false;                   // some element lists a node twice
+    int n_colours = 0, colour_rounds = 0;
+    long long colour_start[65] = {0};
     // assemble workspace
     double *d_Ke = nullptr;      // [n_elems*576] element tangents, block-major [e][I][K][i][k]
     double *d_Re = nullptr;      // [n_elems*24]
@@ -43,6 +51,8 @@ int fem_cuda_fail(cudaError_t e, const char *where);
         if (_e != cudaSuccess) return fem_cuda_fail(_e, #call);          \
     } while (0)
 
+// fem_colour.cu
+int fem_build_colouring(fem_ctx *c);
 // fem_assemble.cu
 int fem_launch_assemble(fem_ctx *c, const double *u, const double *hist_in, const double *mat, long long n_mat,
                         double *residual, double *csr_vals, double *hist_out, cudaStream_t st);

@@ -29,6 +29,9 @@ __global__ void k_validate(long long n_nodes, long long n_elems, const double *_
         if (nd[a] < 0 || nd[a] >= n_nodes) ok = false;
     }
     if (!ok) { atomicOr(flags, 1); return; }
+    for (int a = 0; a < 8; a++)
+        for (int c = a + 1; c < 8; c++)
+            if (nd[a] == nd[c]) atomicOr(flags, 8);   // collapsed element (a node listed twice)
     double X[8][3];
     for (int a = 0; a < 8; a++)
         for (int i = 0; i < 3; i++) X[a][i] = coords[3 * (long long)nd[a] + i];
@@ -190,7 +193,7 @@ extern "C" int fem_hill_from_lankford(double r0, double r45, double r90, double 
 static void ctx_free(fem_ctx *c) {
     if (!c) return;
     void *ptrs[] = {c->d_coords, c->d_conn, c->d_inc_ptr, c->d_inc, c->d_nb_ptr, c->d_nb, c->d_row_ptr, c->d_col_idx,
-                    c->d_elem_pos, c->d_elem_slot, c->d_Ke, c->d_Re, c->d_matd, c->d_stats, c->d_u, c->d_hin, c->d_hout,
+                    c->d_elem_pos, c->d_elem_slot, c->d_elist, c->d_first_mask, c->d_first_res, c->d_Ke, c->d_Re, c->d_matd, c->d_stats, c->d_u, c->d_hin, c->d_hout,
                     c->d_mat, c->d_res, c->d_vals};
     for (void *p : ptrs) if (p) cudaFree(p);
     for (int i = 0; i < 4; i++) if (c->ev[i]) cudaEventDestroy(c->ev[i]);
@@ -208,7 +211,7 @@ extern "C" int fem_setup(fem_ctx **out, long long n_nodes, const double *coords,
     fem_default_options(&o);
     if (opt) o = *opt;
     if (o.quad_order != 2) return FEM_ERR_QUAD;
-    if ((o.fbar != 0 && o.fbar != 1) || !(o.tol > 0) || o.kmax < 1 || o.assembly_mode != 0) return FEM_ERR_ARG;
+    if ((o.fbar != 0 && o.fbar != 1) || !(o.tol > 0) || o.kmax < 1 || (o.assembly_mode != 0 && o.assembly_mode != 1)) return FEM_ERR_ARG;
     int ndev = 0;
     FEM_CUDA(cudaGetDeviceCount(&ndev));
     if (ndev < 1) { snprintf(g_fem_cuda_err, sizeof(g_fem_cuda_err), "no CUDA device"); return FEM_ERR_CUDA; }
@@ -229,6 +232,8 @@ extern "C" int fem_setup(fem_ctx **out, long long n_nodes, const double *coords,
         TRY(cudaMemcpy(&hflags, dflags, sizeof(int), cudaMemcpyDeviceToHost));
         if (hflags & 1) { rc = FEM_ERR_CONN; break; }
         if (hflags & 2) { rc = FEM_ERR_INVERTED; break; }
+        c->has_collapsed = (hflags & 8) != 0;
+        c->mode = (o.assembly_mode == 1 && !c->has_collapsed) ? 1 : 0;   // in-place scatter needs distinct nodes per element
         TRY(cudaMalloc(&c->d_stats, sizeof(unsigned long long) * 72));
         for (int i = 0; i < 4; i++) TRY(cudaEventCreate(&c->ev[i]));
 #undef TRY
@@ -285,10 +290,14 @@ extern "C" int fem_build_csr_pattern(fem_ctx *c, long long *n_rows, long long *n
             TRY(cudaMalloc(&c->d_elem_pos, (size_t)64 * ne));
             k_elem_pos<<<nblk(8 * ne, 256), 256>>>(ne, c->d_conn, c->d_nb_ptr, c->d_nb, c->d_elem_pos);
             TRY(cudaGetLastError());
-            // assemble workspace
-            TRY(cudaMalloc(&c->d_Ke, sizeof(double) * 576 * ne));
-            TRY(cudaMalloc(&c->d_Re, sizeof(double) * 24 * ne));
             TRY(cudaDeviceSynchronize());
+            if (c->mode == 1) {
+                rc = fem_build_colouring(c);
+                if (rc != FEM_OK) break;
+            } else {   // scratch for the two-kernel mode
+                TRY(cudaMalloc(&c->d_Ke, sizeof(double) * 576 * ne));
+                TRY(cudaMalloc(&c->d_Re, sizeof(double) * 24 * ne));
+            }
 #undef TRY
         } while (0);
         if (cnt) cudaFree(cnt);

@@ -11,14 +11,15 @@ def rel_l2(a, b):
     return np.linalg.norm(a - b) / nb if nb > 0 else np.linalg.norm(a)
 
 
-def run_gpu(cfg, fbar=0, want_elem_slot=False, mat=None):
+def run_gpu(cfg, fbar=0, want_elem_slot=False, mat=None, assembly_mode=None):
     import torch
     import paper_2606_17390_b200 as fem
     dev = torch.device("cuda:0")
     ne = cfg["conn"].shape[0]
     if mat is None:
         mat = fem.mat_from_desc(cfg["matdesc"], ne)
-    ctx = fem.FemContext(torch.from_numpy(cfg["coords"]).to(dev), torch.from_numpy(cfg["conn"]).to(dev), fbar=fbar)
+    ctx = fem.FemContext(torch.from_numpy(cfg["coords"]).to(dev), torch.from_numpy(cfg["conn"]).to(dev), fbar=fbar,
+                         assembly_mode=assembly_mode)
     row_ptr, col_idx, slots = ctx.build_csr_pattern(want_elem_slot=want_elem_slot)
     res, vals, hout, stats = ctx.assemble(torch.from_numpy(cfg["u"].ravel()).to(dev), torch.from_numpy(cfg["hist_in"].ravel()).to(dev),
                                           torch.from_numpy(np.ascontiguousarray(mat).ravel()).to(dev), want_stats=True)

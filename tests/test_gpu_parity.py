@@ -148,3 +148,15 @@ def test_error_codes_on_device():
     assert ei.value.code == -10
     r, v, ho, st = ctx.assemble(u, h, mat, want_stats=True)   # u = 0: R = 0, nothing plastic
     assert float(r.abs().max()) == 0.0 and st["n_plastic"] == 0
+
+
+@pytest.mark.parametrize("fbar", [0, 1])
+def test_coloured_in_place_assembly_mode(fbar):
+    """assembly_mode 1 (one launch per colour, in-place read-modify-write) gives the same matrix as the oracle and is
+    bitwise reproducible; irregular mesh with shuffled element order."""
+    cfg = synth.make_config(4, n=14)
+    g = run_gpu(cfg, fbar, assembly_mode=1)
+    assert g["ctx"].launches_per_assemble() > 3          # mat_prep + one launch per colour (>= 8 colours for hex meshes)
+    compare(g, run_oracle(cfg, fbar), "coloured")
+    g2 = run_gpu(cfg, fbar, assembly_mode=1)
+    assert np.array_equal(g["csr_vals"], g2["csr_vals"]) and np.array_equal(g["residual"], g2["residual"])
