@@ -65,15 +65,35 @@ __global__ void k_mat_prep(long long n_mat, const double *__restrict__ mat, doub
 }
 
 // ------------------------------------------------------------------------------------------------ small device helpers
+// Branch-free reciprocal and reciprocal square root: the hardware approximation (relative error 2^-23) refined by two
+// Newton steps (2^-46, 2^-92 -> ~1 ulp).  No special-case paths: callers guarantee normal, positive (rsqrt) arguments.
+__device__ __forceinline__ double frcp(double x) {
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+    double e = fma(-x, r, 1.0);
+    r = fma(r, e, r);
+    e = fma(-x, r, 1.0);
+    return fma(r, e, r);
+}
+__device__ __forceinline__ double frsqrt(double x) {
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    const double h = 0.5 * x;
+    double e = fma(-h * y, y, 0.5);
+    y = fma(y, e, y);
+    e = fma(-h * y, y, 0.5);
+    return fma(y, e, y);
+}
+
 // One cyclic-Jacobi rotation annihilating a_pq of a symmetric 3x3 (r = third index); V columns p,q updated.
 __device__ __forceinline__ void jacobi_rot(double &app, double &aqq, double &apq, double &arp, double &arq, double &v0p,
                                            double &v0q, double &v1p, double &v1q, double &v2p, double &v2q) {
     // cos^2 = (1 + |d|/r)/2 with r = hypot(d, 2 a_pq); sin = sgn(d) a_pq / (r cos); tan = sin / cos.  Two rsqrt, no division.
     const double d = aqq - app;
     const double r2 = fma(d, d, 4.0 * apq * apq);
-    const double ir = (r2 > 0.0) ? rsqrt(r2) : 0.0;
+    const double ir = (r2 > 1e-280) ? frsqrt(r2) : 0.0;
     const double c2 = fma(0.5 * fabs(d), ir, 0.5);
-    const double ic = rsqrt(c2);
+    const double ic = frsqrt(c2);
     const double c = c2 * ic;
     const double s = ((d < 0.0) ? -apq : apq) * ir * ic;   // sgn(d) a_pq / (r c); d = 0 counts as positive
     const double t = s * ic;
@@ -104,7 +124,7 @@ __device__ __forceinline__ double atanhc(double w, double dlog /* = ln b - ln a 
 // Farther apart the recursion on the widest gap is used (error 4 eps l/gap <= 1e-11 of g2, which enters C_L with
 // weight |T|/|C_ep| ~ 1e-2).
 __device__ __forceinline__ double dd2_series(double la, double lb, double lc) {
-    const double m = (la + lb + lc) * (1.0 / 3.0), im = 1.0 / m;
+    const double m = (la + lb + lc) * (1.0 / 3.0), im = frcp(m);
     const double xa = (la - m) * im, xb = (lb - m) * im, xc = (lc - m) * im;
     const double h1 = xa + xb + xc;                                   // = 0 up to rounding
     const double h2 = xa * xa + xb * xb + xc * xc + xa * xb + xb * xc + xa * xc;
@@ -142,7 +162,7 @@ __device__ __forceinline__ void flow_stress(double law, double h0, double h1, do
     } else {           // Swift K (eps0 + alpha)^n (BASELINE.json configs)
         double b = h1 + alpha;
         sf = h0 * exp(h2 * log(b));
-        dsf = h2 * sf / b;
+        dsf = h2 * sf * frcp(b);
     }
 }
 
@@ -221,7 +241,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
         double c00 = Jr[1][1] * Jr[2][2] - Jr[1][2] * Jr[2][1], c01 = Jr[1][2] * Jr[2][0] - Jr[1][0] * Jr[2][2],
                c02 = Jr[1][0] * Jr[2][1] - Jr[1][1] * Jr[2][0];
         wq = Jr[0][0] * c00 + Jr[0][1] * c01 + Jr[0][2] * c02;
-        double id = 1.0 / wq;
+        double id = frcp(wq);
         Ji[0][0] = c00 * id; Ji[1][0] = c01 * id; Ji[2][0] = c02 * id;
         Ji[0][1] = (Jr[0][2] * Jr[2][1] - Jr[0][1] * Jr[2][2]) * id;
         Ji[1][1] = (Jr[0][0] * Jr[2][2] - Jr[0][2] * Jr[2][0]) * id;
@@ -413,14 +433,14 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
             const double al = fma(W23, dg, alphan);
             flow_stress(law, hh0, hh1, hh2, al, sf, dsf);
             const double sy = W23 * sf, dsy = W23 * dsf;
-            const double isy = 1.0 / sy;
+            const double isy = frcp(sy);
             const double x = mu2 * dg * isy;
             double S2 = 0.0, S3 = 0.0;
             {   // r_k = 1/(1 + x h_k) for the five k from ONE reciprocal of the product (prefix/suffix products)
                 const double d0 = fma(x, hk[0], 1.0), d1_ = fma(x, hk[1], 1.0), d2 = fma(x, hk[2], 1.0), d3 = fma(x, hk[3], 1.0),
                              d4 = fma(x, hk[4], 1.0);
                 const double p01 = d0 * d1_, p34 = d3 * d4, p012 = p01 * d2, p234 = d2 * p34;
-                const double ip = 1.0 / (p012 * p34);
+                const double ip = frcp(p012 * p34);
                 rk[0] = ip * (d1_ * p234); rk[1] = ip * (d0 * p234); rk[2] = ip * (p01 * p34);
                 rk[3] = ip * (p012 * d4);  rk[4] = ip * (p012 * d3);
             }
@@ -436,12 +456,12 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
             }
             if (conv || pass > kmax) { nonconv = !conv; break; }
             iters = pass + 1;
-            const double rphi = rsqrt(S2);
+            const double rphi = frsqrt(S2);
             const double Fv = fma(sy, rphi, -1.0);
             const double dxd = mu2 * isy * (1.0 - dg * dsy * W23 * isy);
             const double Fp = dsy * W23 * rphi + sy * S3 * rphi * rphi * rphi * dxd;
             if (Fv < 0.0) lo = dg; else hi = dg;
-            double dgn = dg - Fv / Fp;
+            double dgn = dg - Fv * frcp(Fp);
             if (!(dgn >= lo && dgn <= hi)) dgn = (hi < INFINITY) ? 0.5 * (lo + hi) : 2.0 * dg + 1e-12;
             // converged when the step is at the round-off floor, or when the residual is so small that the step just
             // computed (kept) lands on the root to round-off
@@ -462,7 +482,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
     double mk[5], beta = 0.0;
     double nk[5];
     {
-        const double iphi = plastic ? rsqrt(phi2) : 0.0;
+        const double iphi = plastic ? frsqrt(phi2) : 0.0;
         double a = 0.0;
 #pragma unroll
         for (int k = 0; k < 5; k++) { nk[k] = hk[k] * cn[k] * iphi; mk[k] = th[k] * nk[k]; a = fma(mk[k], nk[k], a); }
@@ -553,12 +573,13 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
     // ---- S9 geometric post-processor (Eq.(25) :204, analytic route of :288): with g = 1/2 ln,
     //      S^_ab = 2 g[a,b] T^_ab ;  C_L = P_L^T:C_ep:P_L + T:L_L  in the eigenbasis
     double d1[6];  // first divided differences g[a,b], Voigt-indexed: (00,11,22,01,12,02)
-    d1[0] = 0.5 / lam[0]; d1[1] = 0.5 / lam[1]; d1[2] = 0.5 / lam[2];
+    d1[0] = 0.5 * frcp(lam[0]); d1[1] = 0.5 * frcp(lam[1]); d1[2] = 0.5 * frcp(lam[2]);
     {
         const double s01 = lam[0] + lam[1], s12 = lam[1] + lam[2], s02 = lam[0] + lam[2];
-        d1[3] = atanhc((lam[1] - lam[0]) / s01, lg[1] - lg[0]) / s01;
-        d1[4] = atanhc((lam[2] - lam[1]) / s12, lg[2] - lg[1]) / s12;
-        d1[5] = atanhc((lam[2] - lam[0]) / s02, lg[2] - lg[0]) / s02;
+        const double i01 = frcp(s01), i12 = frcp(s12), i02 = frcp(s02);
+        d1[3] = atanhc((lam[1] - lam[0]) * i01, lg[1] - lg[0]) * i01;
+        d1[4] = atanhc((lam[2] - lam[1]) * i12, lg[2] - lg[1]) * i12;
+        d1[5] = atanhc((lam[2] - lam[0]) * i02, lg[2] - lg[0]) * i02;
     }
     // second divided differences: g000,g111,g222 exact; gaab by recursion or series; g012
     const double lmean = (lam[0] + lam[1] + lam[2]) * (1.0 / 3.0);
