@@ -115,7 +115,7 @@ __device__ __forceinline__ double atanhc(double w, double dlog /* = ln b - ln a 
         s = fma(s, w2, 1.0 / 3.0);  s = fma(s, w2, 1.0);
         return s;
     }
-    return 0.5 * dlog / w;
+    return 0.5 * dlog * frcp(w);
 }
 
 // Second divided difference g[a,b,c] of g = 1/2 ln for three eigenvalues within 1e-4 (relative) of each other:
@@ -277,7 +277,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
     if (FBAR) {
         // ---- S4 F-bar (Eq.(31)-(32) PAPER.md:237-243): Jbar = sum w J / sum w ; Fbar = (Jbar/J)^(1/3) F
         double Fi[3][3];
-        double idt = 1.0 / detF;
+        double idt = frcp(detF);
         Fi[0][0] = (F[1][1] * F[2][2] - F[1][2] * F[2][1]) * idt; Fi[0][1] = (F[0][2] * F[2][1] - F[0][1] * F[2][2]) * idt;
         Fi[0][2] = (F[0][1] * F[1][2] - F[0][2] * F[1][1]) * idt; Fi[1][0] = (F[1][2] * F[2][0] - F[1][0] * F[2][2]) * idt;
         Fi[1][1] = (F[0][0] * F[2][2] - F[0][2] * F[2][0]) * idt; Fi[1][2] = (F[0][2] * F[1][0] - F[0][0] * F[1][2]) * idt;
@@ -354,7 +354,12 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
     }
 
     // ---- S5 Hencky strain eps = sum_a 1/2 ln(lam_a) n_a (x) n_a (Eq.(5) :96 with the 1/2 restored, G1), material frame
-    const double lg[3] = {log(lam[0]), log(lam[1]), log(lam[2])};
+    double lg[3];   // ln(lam_a): for stretches within ~15 % of 1, ln l = 2 w atanh(w)/w with w = (l-1)/(l+1) (same series as atanhc)
+#pragma unroll
+    for (int a = 0; a < 3; a++) {
+        const double w = (lam[a] - 1.0) * frcp(lam[a] + 1.0);
+        lg[a] = (w * w < 0.0225) ? 2.0 * w * atanhc(w, 0.0) : log(lam[a]);
+    }
     double ee[6];  // elastic trial strain eps - eps_p_n, tensor components (11,22,33,12,23,13), material frame
     {
         const double e0 = 0.5 * lg[0], e1 = 0.5 * lg[1], e2 = 0.5 * lg[2];
@@ -491,7 +496,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
             const double om = 1.0 - kap * a;
             const double Hp = (2.0 / 3.0) * dsf;          // W dsigma_y/dalpha = (2/3) sigma_flow'
             const double den = fma(om, Hp, a);
-            beta = (kap * den - 1.0) / (om * den);
+            beta = (kap * den - 1.0) * frcp(om * den);
         }
     }
     PHASE_SYNC();
@@ -593,15 +598,15 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
         for (int b = 0; b < 3; b++) {
             if (a == b) { g_aab[a][b] = 0.0; continue; }
             const double gap = lam[a] - lam[b];
-            g_aab[a][b] = (fabs(gap) >= thr) ? (d1[a] - d1[VG[a][b]]) / gap : dd2_series(lam[a], lam[a], lam[b]);
+            g_aab[a][b] = (fabs(gap) >= thr) ? (d1[a] - d1[VG[a][b]]) * frcp(gap) : dd2_series(lam[a], lam[a], lam[b]);
         }
     {
         const double g01 = fabs(lam[0] - lam[1]), g12 = fabs(lam[1] - lam[2]), g02 = fabs(lam[0] - lam[2]);
         const double gmax = fmax(g01, fmax(g12, g02));
         if (gmax < thr) g012 = dd2_series(lam[0], lam[1], lam[2]);
-        else if (gmax == g01) g012 = (d1[VG[0][2]] - d1[VG[2][1]]) / (lam[0] - lam[1]);   // (g[0,2]-g[2,1])/(l0-l1)
-        else if (gmax == g12) g012 = (d1[VG[1][0]] - d1[VG[0][2]]) / (lam[1] - lam[2]);   // (g[1,0]-g[0,2])/(l1-l2)
-        else                  g012 = (d1[VG[0][1]] - d1[VG[1][2]]) / (lam[0] - lam[2]);   // (g[0,1]-g[1,2])/(l0-l2)
+        else if (gmax == g01) g012 = (d1[VG[0][2]] - d1[VG[2][1]]) * frcp(lam[0] - lam[1]);   // (g[0,2]-g[2,1])/(l0-l1)
+        else if (gmax == g12) g012 = (d1[VG[1][0]] - d1[VG[0][2]]) * frcp(lam[1] - lam[2]);   // (g[1,0]-g[0,2])/(l1-l2)
+        else                  g012 = (d1[VG[0][1]] - d1[VG[1][2]]) * frcp(lam[0] - lam[2]);   // (g[0,1]-g[1,2])/(l0-l2)
     }
     // C_L^ = 4 g1_A g1_B C^_AB + Gamma_AB (T:L_L), weighted by the integration weight
     double CL[6][6];
