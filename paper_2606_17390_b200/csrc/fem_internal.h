@@ -22,6 +22,7 @@ struct fem_ctx {
     int *d_col_idx = nullptr;    // [nnz]
     unsigned char *d_elem_pos = nullptr;  // [n_elems*64]  pos(conn[e][I], conn[e][K]) = rank of node K in nb list of node I
     int *d_elem_slot = nullptr;  // [n_elems*576], built on request
+    unsigned int *d_kvec = nullptr;  // [nnz/9] per node-pair block: nibble s = local node K of the column node in incident entry s (0xF none); null if some node has > 8 elements
     // colouring (assembly_mode 1): elements grouped by colour, first-writer masks
     int *d_elist = nullptr;                       // [n_elems] element ids sorted by (colour, id)
     unsigned long long *d_first_mask = nullptr;   // [n_elems] bit I*8+K: this element stores block (I,K) instead of adding

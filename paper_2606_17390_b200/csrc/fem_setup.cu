@@ -149,6 +149,23 @@ __global__ void k_elem_slot(long long n_elems, const int *__restrict__ conn, con
     }
 }
 
+// kvec for the fast gather; flags |= 16 if some node has more than 8 incident elements
+__global__ void k_kvec(long long n_nodes, const int *__restrict__ inc_ptr, const int *__restrict__ inc,
+                       const int *__restrict__ nb_ptr, const unsigned char *__restrict__ elem_pos, unsigned int *kvec, int *flags) {
+    long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (n >= n_nodes) return;
+    const int b = inc_ptr[n], m = inc_ptr[n + 1] - b, o = nb_ptr[n], len = nb_ptr[n + 1] - o;
+    if (m > 8) { atomicOr(flags, 16); return; }
+    for (int p = 0; p < len; p++) kvec[o + p] = 0xffffffffu;
+    for (int s = 0; s < m; s++) {
+        const long long t = inc[b + s];
+        for (int K = 0; K < 8; K++) {
+            const int p = elem_pos[t * 8 + K];
+            kvec[o + p] = (kvec[o + p] & ~(15u << (4 * s))) | ((unsigned)K << (4 * s));
+        }
+    }
+}
+
 static inline unsigned nblk(long long n, int bs) { return (unsigned)((n + bs - 1) / bs); }
 
 // ------------------------------------------------------------------------------------------------ C ABI: host side
@@ -193,7 +210,7 @@ extern "C" int fem_hill_from_lankford(double r0, double r45, double r90, double 
 static void ctx_free(fem_ctx *c) {
     if (!c) return;
     void *ptrs[] = {c->d_coords, c->d_conn, c->d_inc_ptr, c->d_inc, c->d_nb_ptr, c->d_nb, c->d_row_ptr, c->d_col_idx,
-                    c->d_elem_pos, c->d_elem_slot, c->d_elist, c->d_first_mask, c->d_first_res, c->d_Ke, c->d_Re, c->d_matd, c->d_stats, c->d_u, c->d_hin, c->d_hout,
+                    c->d_elem_pos, c->d_elem_slot, c->d_kvec, c->d_elist, c->d_first_mask, c->d_first_res, c->d_Ke, c->d_Re, c->d_matd, c->d_stats, c->d_u, c->d_hin, c->d_hout,
                     c->d_mat, c->d_res, c->d_vals};
     for (void *p : ptrs) if (p) cudaFree(p);
     for (int i = 0; i < 4; i++) if (c->ev[i]) cudaEventDestroy(c->ev[i]);
@@ -290,6 +307,14 @@ extern "C" int fem_build_csr_pattern(fem_ctx *c, long long *n_rows, long long *n
             TRY(cudaMalloc(&c->d_elem_pos, (size_t)64 * ne));
             k_elem_pos<<<nblk(8 * ne, 256), 256>>>(ne, c->d_conn, c->d_nb_ptr, c->d_nb, c->d_elem_pos);
             TRY(cudaGetLastError());
+            if (!c->has_collapsed) {
+                TRY(cudaMalloc(&c->d_kvec, sizeof(unsigned int) * (size_t)nblocks));
+                TRY(cudaMemset(dflags, 0, sizeof(int)));
+                k_kvec<<<nblk(nn, 128), 128>>>(nn, c->d_inc_ptr, c->d_inc, c->d_nb_ptr, c->d_elem_pos, c->d_kvec, dflags);
+                int kf = 0;
+                TRY(cudaMemcpy(&kf, dflags, sizeof(int), cudaMemcpyDeviceToHost));
+                if (kf & 16) { cudaFree(c->d_kvec); c->d_kvec = nullptr; }   // general gather kernel instead
+            }
             TRY(cudaDeviceSynchronize());
             if (c->mode == 1) {
                 rc = fem_build_colouring(c);
