@@ -207,6 +207,15 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
     if (tid == 64) s_done = 0;
     __syncthreads();
 
+    // history loads are issued first: their latency overlaps the geometry and the Jacobi sweeps
+    double epn[6];
+    double alphan;
+    {
+        const double *hin = hist_in + (e * 8 + q) * 7;
+#pragma unroll
+        for (int i = 0; i < 6; i++) epn[i] = __ldg(hin + i);
+        alphan = __ldg(hin + 6);
+    }
     // ---- S2 gather: thread q loads node q of its element
     int my_node;
     {
@@ -371,11 +380,6 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
         ee[5] = e0 * Rm[0][0] * Rm[2][0] + e1 * Rm[0][1] * Rm[2][1] + e2 * Rm[0][2] * Rm[2][2];
     }
     // history in (global components) -> material frame
-    const double *hin = hist_in + (e * 8 + q) * 7;
-    double epn[6];
-#pragma unroll
-    for (int i = 0; i < 6; i++) epn[i] = hin[i];
-    const double alphan = hin[6];
     double epm[6];  // eps_p_n in the material frame
     if (rot) {
         const double A[3][3] = {{epn[0], epn[3], epn[5]}, {epn[3], epn[1], epn[4]}, {epn[5], epn[4], epn[2]}};
