@@ -101,7 +101,8 @@ int fem_build_csr_pattern(fem_ctx *c, long long *n_rows, long long *nnz, const i
  *   residual  dev [n_rows]   csr_vals dev [nnz]   hist_out dev [n_elems*8*7] (must not alias hist_in)
  *   stats     host, may be NULL; when non-NULL the call synchronises `stream` and copies the counters back
  *   cuda_stream  a cudaStream_t (NULL = legacy default stream); all work is ordered on it
- * Sums are taken in a fixed order (ascending element id per entry): two calls with equal inputs give bit-identical output.
+ * Sums are taken in a fixed order (mode 0: ascending element id per entry; mode 1: colour order): two calls with equal
+ * inputs give bit-identical output.
  * Physics trouble (local non-convergence, det F <= 0, non-finite) is counted in stats, never an error return. */
 int fem_assemble(fem_ctx *c, const double *u, const double *hist_in, const double *mat, long long n_mat,
                  double *residual, double *csr_vals, double *hist_out, fem_stats *stats, void *cuda_stream);

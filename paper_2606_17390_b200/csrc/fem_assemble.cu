@@ -151,7 +151,12 @@ __host__ __device__ constexpr int sidx9(int r, int c) {  // packed upper triangl
 #define SM_WQ 864   // [8]      (F-bar) w_q J_q / (Jbar V)
 #define ES_STD 564   // >= 552, = 4 mod 16: the 4 elements of a warp start in 4 different bank groups
 #define ES_FBAR 884  // >= 872, = 4 mod 16
+#ifndef EL_PER_CTA
 #define EL_PER_CTA 16
+#endif
+#define CTA_THREADS (8 * EL_PER_CTA)
+#define CTAS_STD (384 / CTA_THREADS)   // 12 warps per SM: limited by 168 registers and ~4.5 KB shared memory per element
+#define CTAS_FBAR (256 / CTA_THREADS)
 
 __device__ __forceinline__ void flow_stress(double law, double h0, double h1, double h2, double alpha, double &sf,
                                             double &dsf) {
@@ -168,14 +173,10 @@ __device__ __forceinline__ void flow_stress(double law, double h0, double h1, do
 
 // Keeping the warps of a CTA in the same code region lets them share instruction-cache lines (the kernel is ~94 KB of
 // straight-line SASS); ncu showed instruction fetch as a top stall without it.
-#ifndef PHASE_SYNC_ON
-#define PHASE_SYNC_ON 1
+#ifndef PS_MASK
+#define PS_MASK 0x094   // measured best subset of the ten phase boundaries (sweep in DESIGN.md): before the return map, the tangent, phase 2
 #endif
-#if PHASE_SYNC_ON
-#define PHASE_SYNC() __syncthreads()
-#else
-#define PHASE_SYNC() ((void)0)
-#endif
+#define PHASE_SYNC_N(n) do { if ((PS_MASK >> (n)) & 1) __syncthreads(); } while (0)
 // MODE 0: K^e, R^e go to an HBM scratch (k_gather sums them).  MODE 1: launched once per colour (elist = the colour's
 // elements); K^e, R^e are added in place into csr_vals / residual (no two elements of a launch share a node).
 struct scatter_args {
@@ -187,7 +188,7 @@ struct scatter_args {
     double *csr_vals, *residual;
 };
 template <int FBAR, int MODE>
-__global__ void __launch_bounds__(128, FBAR ? 2 : 3)
+__global__ void __launch_bounds__(CTA_THREADS, FBAR ? CTAS_FBAR : CTAS_STD)
 k_element(long long n_elems, const double *__restrict__ coords, const int *__restrict__ conn,
           const double *__restrict__ u, const double *__restrict__ hist_in, const double *__restrict__ matd,
           int mat_stride, double tol, int kmax, double *__restrict__ Ke, double *__restrict__ Re,
@@ -203,8 +204,8 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
     const long long e_slot = valid ? e_raw : n_elems - 1;
     const long long e = (MODE == 1 && sa.elist) ? (long long)sa.elist[e_slot] : e_slot;
     double *se = sm + el_cta * ES;
-    if (tid < 64) s_hist[tid] = 0;
-    if (tid == 64) s_done = 0;
+    for (int j = tid; j < 64; j += CTA_THREADS) s_hist[j] = 0;
+    if (tid == 0) s_done = 0;
     __syncthreads();
 
     // history loads are issued first: their latency overlaps the geometry and the Jacobi sweeps
@@ -311,7 +312,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
         wgt = wq * cq;
     }
 
-    PHASE_SYNC();
+    PHASE_SYNC_N(0);
     // ---- S5 C = F^T F and its spectral decomposition by cyclic Jacobi (Eq.(4) :92; backward stable, fixed 4 sweeps)
     double c00 = F[0][0] * F[0][0] + F[1][0] * F[1][0] + F[2][0] * F[2][0];
     double c11 = F[0][1] * F[0][1] + F[1][1] * F[1][1] + F[2][1] * F[2][1];
@@ -328,7 +329,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
     }
     const double lam[3] = {c00, c11, c22};
 
-    PHASE_SYNC();
+    PHASE_SYNC_N(1);
     // ---- rotate F and G into the eigenbasis (Lagrangian principal axes): F^_ia = F_iJ R_Ja, G^_Ia = G_IJ R_Ja
     double Fh[3][3];
 #pragma unroll
@@ -401,7 +402,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
 #pragma unroll
     for (int i = 0; i < 6; i++) ee[i] -= epm[i];
 
-    PHASE_SYNC();
+    PHASE_SYNC_N(2);
     // ---- S6 elastic predictor in the Hill eigenbasis: T_tr = p I + s, s = 2mu dev(ee) = sum_k c_k v_k (Eq.(16) :160)
     const double tre = ee[0] + ee[1] + ee[2];
     const double pres = kb * tre;
@@ -503,7 +504,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
             beta = (kap * den - 1.0) * frcp(om * den);
         }
     }
-    PHASE_SYNC();
+    PHASE_SYNC_N(3);
     // ---- S10 history out: eps_p += dgam N, alpha += W dgam (Eq.(19)-(20) :176-178), back to global components
     if (valid) {
         double *ho = hist_out + (e * 8 + q) * 7;
@@ -535,7 +536,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
         ho[6] = alpha1;
     }
 
-    PHASE_SYNC();
+    PHASE_SYNC_N(4);
     // ---- S8 algorithmic tangent in the eigenbasis of C (App. D :1002-1019 in closed form):
     //      C_ep = kb I(x)I + sum_k theta_k V^_k (x) V^_k + beta m^ (x) m^ ,  V^_k = Rm^T V_k Rm ; T^ = p I + sum c'_k V^_k
     double Ch[6][6];   // tensor components, upper triangle used
@@ -578,7 +579,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
         for (int B = A; B < 6; B++) Ch[A][B] = fma(bm, mh[B], Ch[A][B]);
     }
 
-    PHASE_SYNC();
+    PHASE_SYNC_N(5);
     // ---- S9 geometric post-processor (Eq.(25) :204, analytic route of :288): with g = 1/2 ln,
     //      S^_ab = 2 g[a,b] T^_ab ;  C_L = P_L^T:C_ep:P_L + T:L_L  in the eigenbasis
     double d1[6];  // first divided differences g[a,b], Voigt-indexed: (00,11,22,01,12,02)
@@ -666,7 +667,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
     }
 
     // ---- S9/S10 P^ = F^ S^ (Eq.(26) :208) and A^_(ia)(kb) = delta_ik S^_ab + F^_im F^_kn C_L^[(ma)][(nb)] -> shared memory
-    PHASE_SYNC();
+    PHASE_SYNC_N(6);
     // ---- S11 element residual R^e_Ii = sum_q w P^_ia G^_Ia (Eq.(35) :257), P^ = F^ S^ (Eq.(26) :208): every thread forms
     //      its own point's 24 contributions, then a 3-step reduce-scatter butterfly over the 8 lanes of the element
     //      (fixed order => deterministic) leaves node I = q's three sums in this thread.
@@ -703,7 +704,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
             rI[j] = keep + __shfl_xor_sync(0xffffffffu, send, 1);
         }
     }
-    PHASE_SYNC();
+    PHASE_SYNC_N(7);
     // ---- S9/S10 A^_(ia)(kb) = delta_ik S^_ab + F^_im F^_kn C_L^[(ma)][(nb)] (weighted) -> shared memory, packed symmetric,
     //      two entries per 16-byte slot so that phase 2 reads them with one broadcast LDS.128
 #pragma unroll
@@ -748,7 +749,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
     }
     __syncwarp();
 
-    PHASE_SYNC();
+    PHASE_SYNC_N(8);
     // ---- S12 phase 2: thread t = node I of the element.  K^e_(Ii)(Kk) = sum_q G^_Ia A^_(ia)(kb) G^_Kb (Eq.(37) :267).
     //      Symmetry: thread I owns blocks (I, I+d mod 8), d = 0..4 (d = 4 only for I < 4); the transposes are implied
     //      (fbar = 0: packed scratch) or written explicitly (fbar = 1: full scratch).
@@ -815,7 +816,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
         }
     }
     __syncwarp();
-    PHASE_SYNC();
+    PHASE_SYNC_N(9);
     if (MODE == 0 || FBAR) {
         // ---- phase 3: stage K^e in shared memory (overlays GG/AA).  fbar = 0: packed symmetric, 36 blocks [p][i][k] with
         //      p(I,d) = 4 I + d (d < 4), 32 + I (d = 4);  fbar = 1: full block-major [I][K][i][k]
@@ -1145,20 +1146,20 @@ int fem_launch_assemble(fem_ctx *c, const double *u, const double *hist_in, cons
             sa.elist = c->d_elist + c->colour_start[k];
             const unsigned grid = nblk2(cnt, EL_PER_CTA);
             if (c->opt.fbar)
-                k_element<1, 1><<<grid, 128, sm_fbar, st>>>(cnt, c->d_coords, c->d_conn, u, hist_in, c->d_matd, mstride, c->opt.tol,
+                k_element<1, 1><<<grid, CTA_THREADS, sm_fbar, st>>>(cnt, c->d_coords, c->d_conn, u, hist_in, c->d_matd, mstride, c->opt.tol,
                                                             c->opt.kmax, nullptr, nullptr, hist_out, c->d_stats, sa);
             else
-                k_element<0, 1><<<grid, 128, sm_std, st>>>(cnt, c->d_coords, c->d_conn, u, hist_in, c->d_matd, mstride, c->opt.tol,
+                k_element<0, 1><<<grid, CTA_THREADS, sm_std, st>>>(cnt, c->d_coords, c->d_conn, u, hist_in, c->d_matd, mstride, c->opt.tol,
                                                            c->opt.kmax, nullptr, nullptr, hist_out, c->d_stats, sa);
         }
         FEM_CUDA(cudaEventRecord(c->ev[2], st));
     } else {
         const unsigned grid = nblk2(c->n_elems, EL_PER_CTA);
         if (c->opt.fbar)
-            k_element<1, 0><<<grid, 128, sm_fbar, st>>>(c->n_elems, c->d_coords, c->d_conn, u, hist_in, c->d_matd, mstride,
+            k_element<1, 0><<<grid, CTA_THREADS, sm_fbar, st>>>(c->n_elems, c->d_coords, c->d_conn, u, hist_in, c->d_matd, mstride,
                                                         c->opt.tol, c->opt.kmax, c->d_Ke, c->d_Re, hist_out, c->d_stats, sa);
         else
-            k_element<0, 0><<<grid, 128, sm_std, st>>>(c->n_elems, c->d_coords, c->d_conn, u, hist_in, c->d_matd, mstride,
+            k_element<0, 0><<<grid, CTA_THREADS, sm_std, st>>>(c->n_elems, c->d_coords, c->d_conn, u, hist_in, c->d_matd, mstride,
                                                        c->opt.tol, c->opt.kmax, c->d_Ke, c->d_Re, hist_out, c->d_stats, sa);
         FEM_CUDA(cudaEventRecord(c->ev[2], st));
         const unsigned gg = nblk2(c->n_nodes * 32, 256);
