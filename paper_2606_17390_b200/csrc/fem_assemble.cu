@@ -140,16 +140,18 @@ __host__ __device__ constexpr int sidx9(int r, int c) {  // packed upper triangl
 
 // shared-memory layout per element, in doubles (stride = 4 mod 16 so that broadcast reads of the 4 elements of a warp
 // hit 4 disjoint bank groups; every per-point array is [entry][q] with the 8 Gauss points adjacent)
-#define SM_GG 0     // [24][8]  G^_Ia  = grad N_I in the eigenbasis of C
-#define SM_AA 192   // 45 entries w * A^_(ia)(kb), packed symmetric: entry s < 44 at (s/2)*16 + 2 q + (s&1), entry 44 at 352 + q
-#define SM_XE 192   // [24] element coordinates   (overlay: dead before AA is written)
-#define SM_UE 216   // [24] element displacements (overlay)
+#define SM_GG 0     // G^_Ia = grad N_I in the eigenbasis of C at GGX(I,a) + q: node stride 25 (odd) so that both the per-point
+                    // accesses (lanes = q) and the per-node reads of phase 2 (lanes = I) are bank-conflict free
+#define GGX(I, a) (SM_GG + (I) * 25 + (a) * 8)
+#define SM_AA 200   // 45 entries w * A^_(ia)(kb), packed symmetric: entry s < 44 at (s/2)*16 + 2 q + (s&1), entry 44 at 352 + q
+#define SM_XE 200   // [24] element coordinates   (overlay: dead before AA is written)
+#define SM_UE 224   // [24] element displacements (overlay)
 #define SM_KS 0     // K^e staging (324 packed / 576 full), overlays GG/AA after phase 2
 #define SM_GQ 576   // [24][8]  (F-bar) g^q_Kk = G_KL F^-1_Lk
 #define SM_YY 768   // [9][8]   (F-bar) w/3 (A^:F^)_ia
 #define SM_GB 840   // [24]     (F-bar) gbar
 #define SM_WQ 864   // [8]      (F-bar) w_q J_q / (Jbar V)
-#define ES_STD 564   // >= 552, = 4 mod 16: the 4 elements of a warp start in 4 different bank groups
+#define ES_STD 564   // >= 560, = 4 mod 16: the 4 elements of a warp start in 4 different bank groups
 #define ES_FBAR 884  // >= 872, = 4 mod 16
 #ifndef EL_PER_CTA
 #define EL_PER_CTA 16
@@ -272,7 +274,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
 #pragma unroll
         for (int j = 0; j < 3; j++) {
             G[j] = d0 * Ji[0][j] + d1 * Ji[1][j] + d2 * Ji[2][j];
-            se[SM_GG + (3 * I + j) * 8 + q] = G[j];
+            se[GGX(I, j) + q] = G[j];
         }
 #pragma unroll
         for (int i = 0; i < 3; i++) {
@@ -295,7 +297,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
         Fi[2][2] = (F[0][0] * F[1][1] - F[0][1] * F[1][0]) * idt;
 #pragma unroll
         for (int K = 0; K < 8; K++) {
-            double g0 = se[SM_GG + (3 * K + 0) * 8 + q], g1 = se[SM_GG + (3 * K + 1) * 8 + q], g2 = se[SM_GG + (3 * K + 2) * 8 + q];
+            double g0 = se[GGX(K, 0) + q], g1 = se[GGX(K, 1) + q], g2 = se[GGX(K, 2) + q];
 #pragma unroll
             for (int k = 0; k < 3; k++) se[SM_GQ + (3 * K + k) * 8 + q] = g0 * Fi[0][k] + g1 * Fi[1][k] + g2 * Fi[2][k];
         }
@@ -338,9 +340,9 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
         for (int a = 0; a < 3; a++) Fh[i][a] = F[i][0] * R[0][a] + F[i][1] * R[1][a] + F[i][2] * R[2][a];
 #pragma unroll
     for (int I = 0; I < 8; I++) {
-        double g0 = se[SM_GG + (3 * I + 0) * 8 + q], g1 = se[SM_GG + (3 * I + 1) * 8 + q], g2 = se[SM_GG + (3 * I + 2) * 8 + q];
+        double g0 = se[GGX(I, 0) + q], g1 = se[GGX(I, 1) + q], g2 = se[GGX(I, 2) + q];
 #pragma unroll
-        for (int a = 0; a < 3; a++) se[SM_GG + (3 * I + a) * 8 + q] = g0 * R[0][a] + g1 * R[1][a] + g2 * R[2][a];
+        for (int a = 0; a < 3; a++) se[GGX(I, a) + q] = g0 * R[0][a] + g1 * R[1][a] + g2 * R[2][a];
     }
 
     // ---- material (derived record), orientation
@@ -682,7 +684,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
         double r[24];
 #pragma unroll
         for (int J = 0; J < 8; J++) {
-            const double g0 = se[SM_GG + (3 * J + 0) * 8 + q], g1 = se[SM_GG + (3 * J + 1) * 8 + q], g2 = se[SM_GG + (3 * J + 2) * 8 + q];
+            const double g0 = se[GGX(J, 0) + q], g1 = se[GGX(J, 1) + q], g2 = se[GGX(J, 2) + q];
 #pragma unroll
             for (int i = 0; i < 3; i++) r[3 * J + i] = fma(Ph[i][2], g2, fma(Ph[i][1], g1, Ph[i][0] * g0));
         }
@@ -763,7 +765,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
 #pragma unroll 1
     for (int qq = 0; qq < 8; qq++) {
         const double *sq = se + qq;
-        const double gI[3] = {sq[SM_GG + (3 * I + 0) * 8], sq[SM_GG + (3 * I + 1) * 8], sq[SM_GG + (3 * I + 2) * 8]};
+        const double gI[3] = {sq[GGX(I, 0)], sq[GGX(I, 1)], sq[GGX(I, 2)]};
         double aik[3][9];  // a_{i,(kb)} = sum_a G^_Ia A^_(ia)(kb): each stored entry (r,c) feeds a[r/3][c] and a[c/3][r]
 #pragma unroll
         for (int i = 0; i < 3; i++)
@@ -798,7 +800,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
         for (int d = 0; d < 5; d++) {
             if (d == 4 && I >= 4) continue;
             const int K = (I + d) & 7;
-            const double gK0 = sq[SM_GG + (3 * K + 0) * 8], gK1 = sq[SM_GG + (3 * K + 1) * 8], gK2 = sq[SM_GG + (3 * K + 2) * 8];
+            const double gK0 = sq[GGX(K, 0)], gK1 = sq[GGX(K, 1)], gK2 = sq[GGX(K, 2)];
 #pragma unroll
             for (int i = 0; i < 3; i++)
 #pragma unroll
