@@ -820,7 +820,8 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
     __syncwarp();
     PHASE_SYNC_N(9);
     if (MODE == 0 || FBAR) {
-        // ---- phase 3: stage K^e in shared memory (overlays GG/AA).  fbar = 0: packed symmetric, 36 blocks [p][i][k] with
+        // ---- phase 3: stage K^e in shared memory (overlays GG/AA).  fbar = 0: packed symmetric, component-major [3i+k][p]
+    //      (the 8 lanes of a gather warp that read one element then touch 3 cache lines per load instead of 8), 36 blocks with
         //      p(I,d) = 4 I + d (d < 4), 32 + I (d = 4);  fbar = 1: full block-major [I][K][i][k]
         #pragma unroll
         for (int d = 0; d < 5; d++) {
@@ -831,7 +832,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
             for (int i = 0; i < 3; i++)
     #pragma unroll
                 for (int k = 0; k < 3; k++) {
-                    se[SM_KS + pb * 9 + 3 * i + k] = acc[d][3 * i + k];
+                    se[SM_KS + (FBAR ? pb * 9 + 3 * i + k : (3 * i + k) * 36 + pb)] = acc[d][3 * i + k];
                     if (FBAR && d != 0) se[SM_KS + (K * 8 + I) * 9 + 3 * k + i] = acc[d][3 * i + k];
                 }
         }
@@ -1007,15 +1008,15 @@ k_gather(long long n_nodes, const int *__restrict__ inc_ptr, const int *__restri
                     const bool direct = (d < 4) || (d == 4 && I < 4);
                     const int oI = direct ? I : K, od = direct ? d : (8 - d);
                     const int pb = (od < 4) ? (4 * oI + od) : (32 + oI);
-                    const double *kb = Ke + (t >> 3) * 324 + pb * 9;
+                    const double *kb = Ke + (t >> 3) * 324 + pb;   // component-major record: [c][36 blocks]
                     if (direct) {
 #pragma unroll
-                        for (int j = 0; j < 9; j++) acc[j] += kb[j];
+                        for (int j = 0; j < 9; j++) acc[j] += kb[j * 36];
                     } else {
 #pragma unroll
                         for (int i = 0; i < 3; i++)
 #pragma unroll
-                            for (int k = 0; k < 3; k++) acc[3 * i + k] += kb[3 * k + i];
+                            for (int k = 0; k < 3; k++) acc[3 * i + k] += kb[(3 * k + i) * 36];
                     }
                 } else {
                     const double *kb = Ke + (t * 8 + K) * 9;
@@ -1058,7 +1059,7 @@ k_gather_fast(long long n_nodes, const int *__restrict__ inc_ptr, const int *__r
         if (PACKED) {
             const bool direct = (d < 4) || (d == 4 && I < 4);
             const int oI = direct ? I : K, od = direct ? d : (8 - d);
-            off = ((od < 4) ? (4 * oI + od) : (32 + oI)) * 9; tr = direct ? 0u : 1u;
+            off = (od < 4) ? (4 * oI + od) : (32 + oI); tr = direct ? 0u : 1u;   // component-major record [c][36]
         } else off = (I * 8 + K) * 9;
         s_off[threadIdx.x] = (unsigned short)(off | (tr << 15));
     }
@@ -1084,7 +1085,7 @@ k_gather_fast(long long n_nodes, const int *__restrict__ inc_ptr, const int *__r
                     const double *kb = Ke + (long long)(t >> 3) * ESZ + (ent & 0x7fffu);
                     double v[9];
 #pragma unroll
-                    for (int j = 0; j < 9; j++) v[j] = kb[j];
+                    for (int j = 0; j < 9; j++) v[j] = kb[j * (PACKED ? 36 : 1)];
                     if (ent >> 15) {
                         acc[0] += v[0]; acc[1] += v[3]; acc[2] += v[6]; acc[3] += v[1]; acc[4] += v[4]; acc[5] += v[7];
                         acc[6] += v[2]; acc[7] += v[5]; acc[8] += v[8];
