@@ -160,3 +160,57 @@ def test_coloured_in_place_assembly_mode(fbar):
     compare(g, run_oracle(cfg, fbar), "coloured")
     g2 = run_gpu(cfg, fbar, assembly_mode=1)
     assert np.array_equal(g["csr_vals"], g2["csr_vals"]) and np.array_equal(g["residual"], g2["residual"])
+
+
+def _pinwheel_mesh(nsec=12, layers=2):
+    """nsec hexes around the z-axis share the axis edge: axis nodes belong to nsec (> 8) elements per layer pair, which
+    disables the fast gather table and exercises the general gather kernel."""
+    nodes, idx = [], {}
+
+    def nid(key, xyz):
+        if key not in idx:
+            idx[key] = len(nodes); nodes.append(xyz)
+        return idx[key]
+    conn = []
+    for L in range(layers):
+        for j in range(nsec):
+            t0, t1 = 2 * np.pi * j / nsec, 2 * np.pi * (j + 1) / nsec
+            tm = 0.5 * (t0 + t1)
+            quad = [("a",), ("p", j % nsec), ("q", j), ("p", (j + 1) % nsec)]
+            xy = [(0.0, 0.0), (np.cos(t0), np.sin(t0)), (1.5 * np.cos(tm), 1.5 * np.sin(tm)), (np.cos(t1), np.sin(t1))]
+            el = []
+            for z in (L, L + 1):
+                for key, (x, y) in zip(quad, xy):
+                    el.append(nid(key + (z,), (x, y, 0.7 * z)))
+            conn.append(el)
+    return np.array(nodes, dtype=np.float64), np.array(conn, dtype=np.int32)
+
+
+def _mini_cfg(coords, conn, seed=5, amp=0.03):
+    rng = np.random.default_rng(seed)
+    A = rng.normal(size=(3, 3)); A *= amp / np.linalg.norm(A)
+    u = coords @ A.T + 2e-3 * rng.normal(size=coords.shape)
+    return dict(coords=coords, conn=conn, u=u, hist_in=np.zeros((conn.shape[0], 8, 7)), matdesc=dict(synth.configs.SWIFT))
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+def test_high_valence_mesh_uses_general_gather(mode):
+    coords, conn = _pinwheel_mesh()
+    cfg = _mini_cfg(coords, conn)
+    g = run_gpu(cfg, 0, want_elem_slot=True, assembly_mode=mode)
+    compare(g, run_oracle(cfg, 0, with_slots=True), "pinwheel")
+    assert g["stats"]["n_plastic"] > 0
+
+
+def test_collapsed_hex_wedge_elements():
+    """A wedge written as a hex with two node pairs repeated (collapsed element): the same node appears twice in an
+    element, so several local (I,K) pairs map to one CSR block; assembly must add them all (mode falls back to 0)."""
+    base = np.array([[0, 0, 0], [1, 0, 0], [0, 1, 0], [1, 1, 0.0]])
+    coords = np.vstack([np.c_[base[:, :2], np.full(4, z)] for z in (0.0, 0.8, 1.7)])
+    def wedge(a, b, c, off):   # triangle a,b,c extruded: hex nodes a,b,c,c / top
+        return [a + off, b + off, c + off, c + off, a + off + 4, b + off + 4, c + off + 4, c + off + 4]
+    conn = np.array([wedge(0, 1, 2, 0), wedge(1, 3, 2, 0), wedge(0, 1, 2, 4), wedge(1, 3, 2, 4)], dtype=np.int32)
+    cfg = _mini_cfg(coords, conn, seed=9)
+    g = run_gpu(cfg, 0, want_elem_slot=True, assembly_mode=1)     # asks for mode 1, library must fall back to the gather mode
+    assert g["ctx"].launches_per_assemble() == 3
+    compare(g, run_oracle(cfg, 0, with_slots=True), "wedge")
