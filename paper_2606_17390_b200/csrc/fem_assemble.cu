@@ -146,12 +146,15 @@ __host__ __device__ constexpr int sidx9(int r, int c) {  // packed upper triangl
 #define SM_AA 200   // 45 entries w * A^_(ia)(kb), packed symmetric: entry s < 44 at (s/2)*16 + 2 q + (s&1), entry 44 at 352 + q
 #define SM_XE 200   // [24] element coordinates   (overlay: dead before AA is written)
 #define SM_UE 224   // [24] element displacements (overlay)
-#define SM_KS 0     // K^e staging (324 packed / 576 full), overlays GG/AA after phase 2
+#define SM_KS 0     // K^e staging, 8 block-row records of 72 doubles (scratch record layout), overlays GG/AA after phase 2
+// component c of block (I,K) inside block row I: pairs of components interleaved by K so that the gather kernel reads
+// (c, c+1) of one block with one 16-byte load and its 8 lanes of an incident element touch 128 contiguous bytes
+#define KSX(I, K, c) (SM_KS + (I) * 72 + (((c) < 8) ? (((c) >> 1) * 16 + (K) * 2 + ((c) & 1)) : (64 + (K))))
 #define SM_GQ 576   // [24][8]  (F-bar) g^q_Kk = G_KL F^-1_Lk
 #define SM_YY 768   // [9][8]   (F-bar) w/3 (A^:F^)_ia
 #define SM_GB 840   // [24]     (F-bar) gbar
 #define SM_WQ 864   // [8]      (F-bar) w_q J_q / (Jbar V)
-#define ES_STD 564   // >= 560, = 4 mod 16: the 4 elements of a warp start in 4 different bank groups
+#define ES_STD 580   // >= 576, = 4 mod 16: the 4 elements of a warp start in 4 different bank groups
 #define ES_FBAR 884  // >= 872, = 4 mod 16
 #ifndef EL_PER_CTA
 #define EL_PER_CTA 16
@@ -183,6 +186,7 @@ __device__ __forceinline__ void flow_stress(double law, double h0, double h1, do
 // elements); K^e, R^e are added in place into csr_vals / residual (no two elements of a launch share a node).
 struct scatter_args {
     const int *elist;                       // element ids of this launch (MODE 1), nullptr = identity
+    const int *eslot;                       // (MODE 0) [e*8+I] -> scratch record of block row I (node-sorted incidence index)
     const int *nb_ptr;                      // node -> first neighbour block; CSR rows of node n start at 9*nb_ptr[n]
     const unsigned char *elem_pos;          // [e][I][K] rank of node K in the neighbour list of node I
     const unsigned long long *first_mask;   // bit I*8+K: store instead of add
@@ -220,7 +224,8 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
         alphan = __ldg(hin + 6);
     }
     // ---- S2 gather: thread q loads node q of its element
-    int my_node;
+    int my_node, my_slot = 0;
+    if (MODE == 0) my_slot = __ldg(sa.eslot + e * 8 + q);
     {
         const long long nd = conn[e * 8 + q];
         my_node = (int)nd;
@@ -752,63 +757,27 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
     __syncwarp();
 
     PHASE_SYNC_N(8);
-    // ---- S12 phase 2: thread t = node I of the element.  K^e_(Ii)(Kk) = sum_q G^_Ia A^_(ia)(kb) G^_Kb (Eq.(37) :267).
-    //      Symmetry: thread I owns blocks (I, I+d mod 8), d = 0..4 (d = 4 only for I < 4); the transposes are implied
-    //      (fbar = 0: packed scratch) or written explicitly (fbar = 1: full scratch).
+    // ---- S12 phase 2: K^e_(Ii)(Kk) = sum_q G^_Ia A^_(ia)(kb) G^_Kb (Eq.(37) :267) on the FP64 tensor-core path.
+    //      For each component pair (i,k), i <= k, the 8x8 node matrix K^{ik}[I][K] = sum_{(q,a)} G^q_Ia H^{ik}_{(q,a),K} with
+    //      H^{ik}_{(q,a),K} = sum_b A^q_(ia)(kb) G^q_Kb is an 8 x 24 x 8 product: six mma.m8n8k4.f64 steps over (a, q-half).
+    //      The whole warp works on one element at a time; lane (gid = lane/4, tig = lane%4) holds G^q_{gid,a}, q = 4h + tig,
+    //      which is both its A fragment (row I = gid) and the factor of its B fragment (column K = gid), and forms
+    //      its B element H with three FMAs.  K^{ki} = (K^{ik})^T gives the remaining pairs.  DMMA runs at the DFMA rate on
+    //      sm_100a, but one issue keeps the pipe busy for 16 cycles, so the contraction no longer stalls on
+    //      dependent-issue latency, and the accumulators shrink from 45 to 12 doubles per thread.
     const int I = q;
-    double acc[5][9];
     double rq[FBAR ? 8 : 1][3];
+    if (FBAR) {
 #pragma unroll
-    for (int d = 0; d < 5; d++)
-#pragma unroll
-        for (int j = 0; j < 9; j++) acc[d][j] = 0.0;
-#pragma unroll 1
-    for (int qq = 0; qq < 8; qq++) {
-        const double *sq = se + qq;
-        const double gI[3] = {sq[GGX(I, 0)], sq[GGX(I, 1)], sq[GGX(I, 2)]};
-        double aik[3][9];  // a_{i,(kb)} = sum_a G^_Ia A^_(ia)(kb): each stored entry (r,c) feeds a[r/3][c] and a[c/3][r]
-#pragma unroll
-        for (int i = 0; i < 3; i++)
-#pragma unroll
-            for (int kb = 0; kb < 9; kb++) aik[i][kb] = 0.0;
-#pragma unroll
-        for (int pr = 0; pr < 23; pr++) {
-            double2 av;
-            if (pr < 22) av = *reinterpret_cast<const double2 *>(se + SM_AA + pr * 16 + 2 * qq);
-            else { av.x = se[SM_AA + 352 + qq]; av.y = 0.0; }
-#pragma unroll
-            for (int h = 0; h < 2; h++) {
-                const int sI = 2 * pr + h;
-                if (sI > 44) continue;
-                // invert sidx9: row r with r*9 - r(r-1)/2 <= sI
-                int r = 0;
-#pragma unroll
-                for (int rr = 1; rr < 9; rr++) if (rr * 9 - rr * (rr - 1) / 2 <= sI) r = rr;
-                const int c = r + (sI - (r * 9 - r * (r - 1) / 2));
-                const double A = h ? av.y : av.x;
-                aik[r / 3][c] = fma(A, gI[r % 3], aik[r / 3][c]);
-                if (r != c) aik[c / 3][r] = fma(A, gI[c % 3], aik[c / 3][r]);
-            }
-        }
-        if (FBAR) {
+        for (int qq = 0; qq < 8; qq++) {
+            const double *sq = se + qq;
+            const double gI[3] = {sq[GGX(I, 0)], sq[GGX(I, 1)], sq[GGX(I, 2)]};
 #pragma unroll
             for (int i = 0; i < 3; i++)
                 rq[FBAR ? qq : 0][i] = sq[SM_YY + (3 * i + 0) * 8] * gI[0] + sq[SM_YY + (3 * i + 1) * 8] * gI[1] +
                                        sq[SM_YY + (3 * i + 2) * 8] * gI[2];
         }
-#pragma unroll
-        for (int d = 0; d < 5; d++) {
-            if (d == 4 && I >= 4) continue;
-            const int K = (I + d) & 7;
-            const double gK0 = sq[GGX(K, 0)], gK1 = sq[GGX(K, 1)], gK2 = sq[GGX(K, 2)];
-#pragma unroll
-            for (int i = 0; i < 3; i++)
-#pragma unroll
-                for (int k = 0; k < 3; k++)
-                    acc[d][3 * i + k] = fma(aik[i][3 * k + 2], gK2, fma(aik[i][3 * k + 1], gK1, fma(aik[i][3 * k + 0], gK0, acc[d][3 * i + k])));
-        }
-    }
-    if (FBAR) {  // gbar_Kk = sum_q (w_q J_q / (Jbar V)) g^q_Kk for node K = I
+        // gbar_Kk = sum_q (w_q J_q / (Jbar V)) g^q_Kk for node K = I
 #pragma unroll
         for (int k = 0; k < 3; k++) {
             double sgb = 0.0;
@@ -816,73 +785,111 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
             for (int qq = 0; qq < 8; qq++) sgb = fma(se[SM_WQ + qq], se[SM_GQ + (3 * I + k) * 8 + qq], sgb);
             se[SM_GB + 3 * I + k] = sgb;
         }
+        __syncwarp();
     }
-    __syncwarp();
+    {
+        const int gid = lane >> 2, tig = lane & 3;
+        double *const sw = sm + (tid >> 5) * 4 * ES;   // the warp's four elements
+#pragma unroll 1
+        for (int el = 0; el < 4; el++) {
+            double *const sx = sw + el * ES;
+            double g[2][3];
+#pragma unroll
+            for (int h = 0; h < 2; h++)
+#pragma unroll
+                for (int a_ = 0; a_ < 3; a_++) g[h][a_] = sx[GGX(gid, a_) + 4 * h + tig];
+            double C[6][2];
+#pragma unroll
+            for (int p = 0; p < 6; p++) C[p][0] = C[p][1] = 0.0;
+            const double *const sa_ = sx + SM_AA + 2 * tig;
+#pragma unroll
+            for (int a_ = 0; a_ < 3; a_++)
+#pragma unroll
+                for (int h = 0; h < 2; h++) {
+                    int p = 0;
+#pragma unroll
+                    for (int i = 0; i < 3; i++)
+#pragma unroll
+                        for (int k = i; k < 3; k++, p++) {
+                            double hv = 0.0;
+#pragma unroll
+                            for (int b_ = 0; b_ < 3; b_++) {
+                                const int sI = sidx9(3 * i + a_, 3 * k + b_);
+                                const double av = (sI == 44) ? sx[SM_AA + 352 + 4 * h + tig] : sa_[(sI >> 1) * 16 + 8 * h + (sI & 1)];
+                                hv = (b_ == 0) ? av * g[h][0] : fma(av, g[h][b_], hv);
+                            }
+                            asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                                         : "+d"(C[p][0]), "+d"(C[p][1]) : "d"(g[h][a_]), "d"(hv));
+                        }
+                }
+            __syncwarp();   // every lane has read this element's G^ and A^: the staging below overlays them
+            // ---- phase 3: stage the full K^e (8 block-row records [I][72], scratch record layout); lane holds
+            //      K^{ik}[gid][2 tig + j] = component (i,k) of block (gid, 2 tig + j) = component (k,i) of the transposed block
+            {
+                int p = 0;
+#pragma unroll
+                for (int i = 0; i < 3; i++)
+#pragma unroll
+                    for (int k = i; k < 3; k++, p++)
+#pragma unroll
+                        for (int j = 0; j < 2; j++) {
+                            const int K = 2 * tig + j;
+                            sx[KSX(gid, K, 3 * i + k)] = C[p][j];
+                            if (i != k) sx[KSX(K, gid, 3 * k + i)] = C[p][j];
+                        }
+            }
+        }
+        __syncwarp();
+    }
     PHASE_SYNC_N(9);
-    if (MODE == 0 || FBAR) {
-        // ---- phase 3: stage K^e in shared memory (overlays GG/AA).  fbar = 0: packed symmetric, component-major [3i+k][p]
-    //      (the 8 lanes of a gather warp that read one element then touch 3 cache lines per load instead of 8), 36 blocks with
-        //      p(I,d) = 4 I + d (d < 4), 32 + I (d = 4);  fbar = 1: full block-major [I][K][i][k]
-        #pragma unroll
-        for (int d = 0; d < 5; d++) {
-            if (d == 4 && I >= 4) continue;
-            const int K = (I + d) & 7;
-            const int pb = FBAR ? (I * 8 + K) : ((d < 4) ? (4 * I + d) : (32 + I));
-    #pragma unroll
-            for (int i = 0; i < 3; i++)
-    #pragma unroll
-                for (int k = 0; k < 3; k++) {
-                    se[SM_KS + (FBAR ? pb * 9 + 3 * i + k : (3 * i + k) * 36 + pb)] = acc[d][3 * i + k];
-                    if (FBAR && d != 0) se[SM_KS + (K * 8 + I) * 9 + 3 * k + i] = acc[d][3 * i + k];
+    if (FBAR) {
+        // K^e_(Ii)(Kk) += sum_q w_q/3 r^q_Ii (gbar_Kk - g^q_Kk)   (unsymmetric rank-1 terms)
+        double rs[3] = {0, 0, 0};
+#pragma unroll
+        for (int qq = 0; qq < 8; qq++)
+#pragma unroll
+            for (int i = 0; i < 3; i++) rs[i] += rq[FBAR ? qq : 0][i];
+#pragma unroll 1
+        for (int K = 0; K < 8; K++)
+#pragma unroll
+            for (int k = 0; k < 3; k++) {
+                const double gb = se[SM_GB + 3 * K + k];
+                double t0 = rs[0] * gb, t1 = rs[1] * gb, t2 = rs[2] * gb;
+#pragma unroll
+                for (int qq = 0; qq < 8; qq++) {
+                    const double g = se[SM_GQ + (3 * K + k) * 8 + qq];
+                    t0 = fma(-rq[FBAR ? qq : 0][0], g, t0); t1 = fma(-rq[FBAR ? qq : 0][1], g, t1);
+                    t2 = fma(-rq[FBAR ? qq : 0][2], g, t2);
                 }
-        }
-        if (FBAR) {
-            // K^e_(Ii)(Kk) += sum_q w_q/3 r^q_Ii (gbar_Kk - g^q_Kk)   (unsymmetric rank-1 terms)
-            __syncwarp();
-            double rs[3] = {0, 0, 0};
-    #pragma unroll
-            for (int qq = 0; qq < 8; qq++)
-    #pragma unroll
-                for (int i = 0; i < 3; i++) rs[i] += rq[FBAR ? qq : 0][i];
-    #pragma unroll 1
-            for (int K = 0; K < 8; K++)
-    #pragma unroll
-                for (int k = 0; k < 3; k++) {
-                    const double gb = se[SM_GB + 3 * K + k];
-                    double t0 = rs[0] * gb, t1 = rs[1] * gb, t2 = rs[2] * gb;
-    #pragma unroll
-                    for (int qq = 0; qq < 8; qq++) {
-                        const double g = se[SM_GQ + (3 * K + k) * 8 + qq];
-                        t0 = fma(-rq[FBAR ? qq : 0][0], g, t0); t1 = fma(-rq[FBAR ? qq : 0][1], g, t1);
-                        t2 = fma(-rq[FBAR ? qq : 0][2], g, t2);
-                    }
-                    se[SM_KS + (I * 8 + K) * 9 + 0 + k] += t0;
-                    se[SM_KS + (I * 8 + K) * 9 + 3 + k] += t1;
-                    se[SM_KS + (I * 8 + K) * 9 + 6 + k] += t2;
-                }
-        }
+                se[KSX(I, K, 0 + k)] += t0;
+                se[KSX(I, K, 3 + k)] += t1;
+                se[KSX(I, K, 6 + k)] += t2;
+            }
     }
     if (MODE == 0) {
+        // destination-major scratch: block row I of K^e and R^e_I go to the record of incidence entry (e,I) in the node-sorted
+        // list, so that the gather kernel reads every node's contributions as one contiguous run
         if (valid) {
-            double *ro = Re + e * 24 + 3 * I;
+            double *ro = Re + (long long)my_slot * 3;
             ro[0] = rI[0]; ro[1] = rI[1]; ro[2] = rI[2];
         }
         __syncwarp();
-        // coalesced copy-out of the warp's 4 elements (4 x KSZ doubles), 16 bytes per lane per step
+        // copy-out of the warp's 4 elements x 8 records of 576 bytes, 16 bytes per lane per step (9 steps per element)
         {
             const int w_el0 = (tid >> 5) * 4;
             const long long e0 = (long long)blockIdx.x * EL_PER_CTA + w_el0;
-    #pragma unroll
+#pragma unroll
             for (int el = 0; el < 4; el++) {
-                if (e0 + el < n_elems) {
-                    const double2 *src = reinterpret_cast<const double2 *>(sm + (w_el0 + el) * ES + SM_KS);
-                    double2 *dst = reinterpret_cast<double2 *>(Ke + (e0 + el) * (FBAR ? 576 : 324));
-    #pragma unroll
-                    for (int idx = lane; idx < (FBAR ? 576 : 324) / 2; idx += 32) dst[idx] = src[idx];
+                const double2 *src = reinterpret_cast<const double2 *>(sm + (w_el0 + el) * ES + SM_KS);
+                const bool el_ok = e0 + el < n_elems;
+#pragma unroll
+                for (int it = 0; it < 9; it++) {
+                    const int g = it * 32 + lane, rec = g / 36, off = g - rec * 36;
+                    const int slot = __shfl_sync(0xffffffffu, my_slot, el * 8 + rec);
+                    if (el_ok) reinterpret_cast<double2 *>(Ke + (long long)slot * 72)[off] = src[g];
                 }
             }
         }
-
     }
     if (MODE == 1) {
         // ---- S14 in-place assembly (Eq.(34) :253, Eq.(38) :274): no other element of this launch touches this element's
@@ -893,7 +900,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
         const unsigned long long fm = sa.first_mask[e];
         const unsigned fr = sa.first_res[e];
         double *const rowsI = sa.csr_vals + 9LL * nbI;
-        if (FBAR) {
+        {
             __syncwarp();
 #pragma unroll 1
             for (int K = 0; K < 8; K++) {
@@ -905,37 +912,9 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
                         double *a = rowsI + (long long)i * 3 * lenI + 3 * pIK;
 #pragma unroll
                         for (int k = 0; k < 3; k++) {
-                            const double v = se[SM_KS + (I * 8 + K) * 9 + 3 * i + k];
+                            const double v = se[KSX(I, K, 3 * i + k)];
                             a[k] = first ? v : a[k] + v;
                         }
-                    }
-                }
-            }
-        } else {
-#pragma unroll
-            for (int d = 0; d < 5; d++) {
-                const int K = (I + d) & 7;
-                const int srcl = (lane & ~7) | K;   // lane of node K in this element
-                const int nbK = __shfl_sync(0xffffffffu, nbI, srcl), lenK = __shfl_sync(0xffffffffu, lenI, srcl);
-                const unsigned pKx = __shfl_sync(0xffffffffu, posI.x, srcl), pKy = __shfl_sync(0xffffffffu, posI.y, srcl);
-                if ((d == 4 && I >= 4) || !valid) continue;
-                const int pIK = (int)(((K < 4) ? (posI.x >> (8 * K)) : (posI.y >> (8 * (K - 4)))) & 0xffu);
-                const bool first = (fm >> (I * 8 + K)) & 1ull;
-#pragma unroll
-                for (int i = 0; i < 3; i++) {
-                    double *a = rowsI + (long long)i * 3 * lenI + 3 * pIK;
-#pragma unroll
-                    for (int k = 0; k < 3; k++) a[k] = first ? acc[d][3 * i + k] : a[k] + acc[d][3 * i + k];
-                }
-                if (d != 0) {   // transposed block (K,I) into the rows of node K
-                    const int pKI = (int)(((I < 4) ? (pKx >> (8 * I)) : (pKy >> (8 * (I - 4)))) & 0xffu);
-                    const bool first2 = (fm >> (K * 8 + I)) & 1ull;
-                    double *const rowsK = sa.csr_vals + 9LL * nbK + 3 * pKI;
-#pragma unroll
-                    for (int k = 0; k < 3; k++) {
-                        double *a = rowsK + (long long)k * 3 * lenK;
-#pragma unroll
-                        for (int i = 0; i < 3; i++) a[i] = first2 ? acc[d][3 * i + k] : a[i] + acc[d][3 * i + k];
                     }
                 }
             }
@@ -975,11 +954,14 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
     }
 }
 
-// ------------------------------------------------------------------------------------------------ gather kernel (S14)
-// One warp per node n (3 CSR rows).  Lane <-> neighbour position pos: the 3x3 block (n, nb[pos]) is the sum over the
-// incident elements (ascending id) that contain nb[pos]; elem_pos bytes give the local node K of that neighbour.
+// ------------------------------------------------------------------------------------------------ gather kernels (S14)
 // K = A K^e, R = A R^e (Eq.(34) :253, Eq.(38) :274) with a fixed summation order and no atomics.
-template <int PACKED>
+// The scratch is destination-major: node n's contributions are the records inc_ptr[n] .. inc_ptr[n+1]-1 (72 doubles each:
+// block row I of K^e of incident entry s = (e,I), ascending element id), one contiguous run.
+__device__ __forceinline__ int ksoff(int K, int c) { return (c < 8) ? ((c >> 1) * 16 + K * 2 + (c & 1)) : (64 + K); }
+
+// General kernel (a node with more than 8 incident elements, or collapsed elements): one warp per node, lane <-> neighbour
+// position pos; the elem_pos bytes of each incident entry give the local nodes K whose column node sits at pos.
 __global__ void __launch_bounds__(256)
 k_gather(long long n_nodes, const int *__restrict__ inc_ptr, const int *__restrict__ inc, const int *__restrict__ nb_ptr,
          const unsigned char *__restrict__ elem_pos, const double *__restrict__ Ke, const double *__restrict__ Re,
@@ -994,35 +976,15 @@ k_gather(long long n_nodes, const int *__restrict__ inc_ptr, const int *__restri
         double acc[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
         const unsigned pat = (unsigned)pos * 0x01010101u;
         for (int s = 0; s < m; s++) {
-            const long long t = inc[b + s];  // e*8 + I
-            const uint2 pk = pos8[t];
+            const uint2 pk = pos8[inc[b + s]];
             unsigned long long hit = ((unsigned long long)(__vcmpeq4(pk.y, pat) & 0x01010101u) << 32) |
                                      (unsigned long long)(__vcmpeq4(pk.x, pat) & 0x01010101u);
+            const double *rec = Ke + (long long)(b + s) * 72;
             while (hit) {
                 const int K = (__ffsll((long long)hit) - 1) >> 3;
                 hit &= hit - 1;
-                if (PACKED) {
-                    // packed symmetric scratch: block (I,K) is stored by its owner (I, d = K-I mod 8 in 0..3, or d = 4 and I < 4),
-                    // otherwise it is the transpose of the block owned by K
-                    const int I = (int)(t & 7), d = (K - I) & 7;
-                    const bool direct = (d < 4) || (d == 4 && I < 4);
-                    const int oI = direct ? I : K, od = direct ? d : (8 - d);
-                    const int pb = (od < 4) ? (4 * oI + od) : (32 + oI);
-                    const double *kb = Ke + (t >> 3) * 324 + pb;   // component-major record: [c][36 blocks]
-                    if (direct) {
 #pragma unroll
-                        for (int j = 0; j < 9; j++) acc[j] += kb[j * 36];
-                    } else {
-#pragma unroll
-                        for (int i = 0; i < 3; i++)
-#pragma unroll
-                            for (int k = 0; k < 3; k++) acc[3 * i + k] += kb[(3 * k + i) * 36];
-                    }
-                } else {
-                    const double *kb = Ke + (t * 8 + K) * 9;
-#pragma unroll
-                    for (int j = 0; j < 9; j++) acc[j] += kb[j];
-                }
+                for (int j = 0; j < 9; j++) acc[j] += rec[ksoff(K, j)];
             }
         }
         double *out = csr_vals + 9LL * o + 3 * pos;
@@ -1035,42 +997,43 @@ k_gather(long long n_nodes, const int *__restrict__ inc_ptr, const int *__restri
     }
     if (lane < 3) {
         double r = 0.0;
-        for (int s = 0; s < m; s++) {
-            const long long t = inc[b + s];
-            r += Re[(t >> 3) * 24 + (t & 7) * 3 + lane];
-        }
+        for (int s = 0; s < m; s++) r += Re[(long long)(b + s) * 3 + lane];
         residual[3 * n + lane] = r;
     }
 }
 
 // Fast gather for meshes where every node has <= 8 incident elements and no element lists a node twice (all hex meshes
-// of the configs).  kvec[block] (built at setup) holds, for each incident entry s of the block's row node, the local
-// node K of the block's column node in that element (nibble s; 0xF = element does not contain it), so a lane (= neighbour
-// position) needs no search: per incident element it either skips or reads one 3x3 block.  Same fixed order, no atomics.
-template <int PACKED>
-__global__ void __launch_bounds__(256)
-k_gather_fast(long long n_nodes, const int *__restrict__ inc_ptr, const int *__restrict__ inc, const int *__restrict__ nb_ptr,
+// of the configs).  The warp copies the node's run of records (<= 4608 bytes) into shared memory with coalesced 16-byte
+// loads; kvec[block] (built at setup) holds, for each incident entry s, the local node K of the block's column node
+// (nibble s; 0xF = that element does not contain it), so lane = neighbour position adds <= 8 blocks in ascending s with
+// four 16-byte and one 8-byte conflict-free shared loads per block.
+#define GW 8   // warps (nodes) per CTA
+#ifndef GMINB
+#define GMINB 5
+#endif
+__global__ void __launch_bounds__(GW * 32, GMINB)
+k_gather_fast(long long n_nodes, const int *__restrict__ inc_ptr, const int *__restrict__ nb_ptr,
               const unsigned int *__restrict__ kvec, const double *__restrict__ Ke, const double *__restrict__ Re,
               double *__restrict__ csr_vals, double *__restrict__ residual) {
-    __shared__ unsigned short s_off[64];   // [I*8+K]: offset of block (I,K) in the element record | transposed << 15
-    if (threadIdx.x < 64) {
-        const int I = threadIdx.x >> 3, K = threadIdx.x & 7, d = (K - I) & 7;
-        unsigned off, tr = 0;
-        if (PACKED) {
-            const bool direct = (d < 4) || (d == 4 && I < 4);
-            const int oI = direct ? I : K, od = direct ? d : (8 - d);
-            off = (od < 4) ? (4 * oI + od) : (32 + oI); tr = direct ? 0u : 1u;   // component-major record [c][36]
-        } else off = (I * 8 + K) * 9;
-        s_off[threadIdx.x] = (unsigned short)(off | (tr << 15));
-    }
-    __syncthreads();
-    const long long n = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-    const int lane = threadIdx.x & 31;
+    __shared__ __align__(16) double buf[GW][576];
+    const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const long long n = (long long)blockIdx.x * GW + w;
     if (n >= n_nodes) return;
     const int b = inc_ptr[n], m = inc_ptr[n + 1] - b;
     const int o = nb_ptr[n], len = nb_ptr[n + 1] - o;
-    const int t_l = (lane < m) ? inc[b + lane] : 0;
-    constexpr int ESZ = PACKED ? 324 : 576;
+    {
+        const double2 *src = reinterpret_cast<const double2 *>(Ke + (long long)b * 72);
+        double2 *dst = reinterpret_cast<double2 *>(buf[w]);
+        const int lim = m * 36;
+        double2 t[9];
+#pragma unroll
+        for (int it = 0; it < 9; it++) if (it * 32 + lane < lim) t[it] = src[it * 32 + lane];
+#pragma unroll
+        for (int it = 0; it < 9; it++) if (it * 32 + lane < lim) dst[it * 32 + lane] = t[it];
+    }
+    double rv = 0.0;
+    if (lane < 3 * m) rv = Re[(long long)b * 3 + lane];
+    __syncwarp();
     for (int pos0 = 0; pos0 < len; pos0 += 32) {
         const int pos = pos0 + lane;
         const unsigned kv = (pos < len) ? kvec[o + pos] : 0xffffffffu;
@@ -1078,21 +1041,14 @@ k_gather_fast(long long n_nodes, const int *__restrict__ inc_ptr, const int *__r
 #pragma unroll
         for (int s = 0; s < 8; s++) {
             if (s < m) {   // warp-uniform
-                const int t = __shfl_sync(0xffffffffu, t_l, s);
                 const unsigned K = (kv >> (4 * s)) & 15u;
                 if (K != 15u) {
-                    const unsigned ent = s_off[(t & 7) * 8 + K];
-                    const double *kb = Ke + (long long)(t >> 3) * ESZ + (ent & 0x7fffu);
-                    double v[9];
-#pragma unroll
-                    for (int j = 0; j < 9; j++) v[j] = kb[j * (PACKED ? 36 : 1)];
-                    if (ent >> 15) {
-                        acc[0] += v[0]; acc[1] += v[3]; acc[2] += v[6]; acc[3] += v[1]; acc[4] += v[4]; acc[5] += v[7];
-                        acc[6] += v[2]; acc[7] += v[5]; acc[8] += v[8];
-                    } else {
-#pragma unroll
-                        for (int j = 0; j < 9; j++) acc[j] += v[j];
-                    }
+                    const double *rec = buf[w] + s * 72 + 2 * K;
+                    const double2 p0 = *reinterpret_cast<const double2 *>(rec), p1 = *reinterpret_cast<const double2 *>(rec + 16),
+                                  p2 = *reinterpret_cast<const double2 *>(rec + 32), p3 = *reinterpret_cast<const double2 *>(rec + 48);
+                    const double p4 = buf[w][s * 72 + 64 + K];
+                    acc[0] += p0.x; acc[1] += p0.y; acc[2] += p1.x; acc[3] += p1.y; acc[4] += p2.x; acc[5] += p2.y;
+                    acc[6] += p3.x; acc[7] += p3.y; acc[8] += p4;
                 }
             }
         }
@@ -1106,12 +1062,9 @@ k_gather_fast(long long n_nodes, const int *__restrict__ inc_ptr, const int *__r
             }
         }
     }
-    {   // residual: lane l = 3 s + i loads R^e of incident entry s, component i; lanes 0..2 add in ascending s
-        const int s = lane / 3, i = lane - 3 * s;
-        const int t = __shfl_sync(0xffffffffu, t_l, s & 31);
-        double v = 0.0, r = 0.0;
-        if (lane < 24 && s < m) v = Re[(long long)(t >> 3) * 24 + (t & 7) * 3 + i];
-        for (int j = 0; j < m; j++) r += __shfl_sync(0xffffffffu, v, (3 * j + lane) & 31);
+    {   // residual: lane 3 s + i holds R^e component i of incident entry s; lanes 0..2 add in ascending s
+        double r = 0.0;
+        for (int j = 0; j < m; j++) r += __shfl_sync(0xffffffffu, rv, (3 * j + lane) & 31);
         if (lane < 3) residual[3 * n + lane] = r;
     }
 }
@@ -1141,7 +1094,7 @@ int fem_launch_assemble(fem_ctx *c, const double *u, const double *hist_in, cons
     k_mat_prep<<<nblk2(n_mat, 128), 128, 0, st>>>(n_mat, mat, c->d_matd);
     FEM_CUDA(cudaEventRecord(c->ev[1], st));
     const int mstride = (n_mat == 1) ? 0 : FEM_MATD;
-    scatter_args sa = {nullptr, c->d_nb_ptr, c->d_elem_pos, c->d_first_mask, c->d_first_res, csr_vals, residual};
+    scatter_args sa = {nullptr, c->d_eslot, c->d_nb_ptr, c->d_elem_pos, c->d_first_mask, c->d_first_res, csr_vals, residual};
     if (c->mode == 1) {
         // one launch per colour, in colour order (stream order = summation order)
         for (int k = 0; k < c->n_colours; k++) {
@@ -1165,20 +1118,12 @@ int fem_launch_assemble(fem_ctx *c, const double *u, const double *hist_in, cons
             k_element<0, 0><<<grid, CTA_THREADS, sm_std, st>>>(c->n_elems, c->d_coords, c->d_conn, u, hist_in, c->d_matd, mstride,
                                                        c->opt.tol, c->opt.kmax, c->d_Ke, c->d_Re, hist_out, c->d_stats, sa);
         FEM_CUDA(cudaEventRecord(c->ev[2], st));
-        const unsigned gg = nblk2(c->n_nodes * 32, 256);
-        if (c->d_kvec) {   // every node has <= 8 incident elements, no collapsed element
-            if (c->opt.fbar)
-                k_gather_fast<0><<<gg, 256, 0, st>>>(c->n_nodes, c->d_inc_ptr, c->d_inc, c->d_nb_ptr, c->d_kvec, c->d_Ke, c->d_Re,
-                                                     csr_vals, residual);
-            else
-                k_gather_fast<1><<<gg, 256, 0, st>>>(c->n_nodes, c->d_inc_ptr, c->d_inc, c->d_nb_ptr, c->d_kvec, c->d_Ke, c->d_Re,
-                                                     csr_vals, residual);
-        } else if (c->opt.fbar)
-            k_gather<0><<<gg, 256, 0, st>>>(c->n_nodes, c->d_inc_ptr, c->d_inc, c->d_nb_ptr, c->d_elem_pos, c->d_Ke, c->d_Re,
-                                            csr_vals, residual);
+        if (c->d_kvec)   // every node has <= 8 incident elements, no collapsed element
+            k_gather_fast<<<nblk2(c->n_nodes, GW), GW * 32, 0, st>>>(c->n_nodes, c->d_inc_ptr, c->d_nb_ptr, c->d_kvec, c->d_Ke, c->d_Re,
+                                                                  csr_vals, residual);
         else
-            k_gather<1><<<gg, 256, 0, st>>>(c->n_nodes, c->d_inc_ptr, c->d_inc, c->d_nb_ptr, c->d_elem_pos, c->d_Ke, c->d_Re,
-                                            csr_vals, residual);
+            k_gather<<<nblk2(c->n_nodes * 32, 256), 256, 0, st>>>(c->n_nodes, c->d_inc_ptr, c->d_inc, c->d_nb_ptr, c->d_elem_pos, c->d_Ke,
+                                                                 c->d_Re, csr_vals, residual);
     }
     FEM_CUDA(cudaEventRecord(c->ev[3], st));
     FEM_CUDA(cudaGetLastError());

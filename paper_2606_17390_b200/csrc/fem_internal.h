@@ -16,6 +16,7 @@ struct fem_ctx {
     bool has_pattern = false;
     int *d_inc_ptr = nullptr;    // [n_nodes+1]   node -> incident (element,local node) list
     int *d_inc = nullptr;        // [8*n_elems]   e*8+I, ascending within a node
+    int *d_eslot = nullptr;      // [8*n_elems]   inverse of d_inc: index j of (e,I) in the node-sorted incidence list
     int *d_nb_ptr = nullptr;     // [n_nodes+1]   node -> sorted neighbour-node list
     int *d_nb = nullptr;         // [nnz/9]
     int *d_row_ptr = nullptr;    // [n_rows+1]
@@ -32,8 +33,9 @@ struct fem_ctx {
     int n_colours = 0, colour_rounds = 0;
     long long colour_start[65] = {0};
     // assemble workspace
-    double *d_Ke = nullptr;      // [n_elems*576] element tangents, block-major [e][I][K][i][k]
-    double *d_Re = nullptr;      // [n_elems*24]
+    double *d_Ke = nullptr;      // [8*n_elems][72] destination-major scratch: record j = block row I of K^e of incidence entry j
+                                 //   (node-sorted), component c of block (I,K) at (c>>1)*16 + 2K + (c&1) for c < 8, 64 + K for c = 8
+    double *d_Re = nullptr;      // [8*n_elems][3]  R^e_I of incidence entry j
     double *d_matd = nullptr;    // [n_mat_cap*FEM_MATD]
     long long n_matd_cap = 0;
     unsigned long long *d_stats = nullptr;  // [4 + 1 + 64] counters

@@ -149,6 +149,12 @@ __global__ void k_elem_slot(long long n_elems, const int *__restrict__ conn, con
     }
 }
 
+// inverse of the node-sorted incidence list: eslot[e*8+I] = j with inc[j] = e*8+I
+__global__ void k_eslot(long long n_elems, const int *__restrict__ inc, int *eslot) {
+    long long j = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (j < 8 * n_elems) eslot[inc[j]] = (int)j;
+}
+
 // kvec for the fast gather; flags |= 16 if some node has more than 8 incident elements
 __global__ void k_kvec(long long n_nodes, const int *__restrict__ inc_ptr, const int *__restrict__ inc,
                        const int *__restrict__ nb_ptr, const unsigned char *__restrict__ elem_pos, unsigned int *kvec, int *flags) {
@@ -210,7 +216,7 @@ extern "C" int fem_hill_from_lankford(double r0, double r45, double r90, double 
 static void ctx_free(fem_ctx *c) {
     if (!c) return;
     void *ptrs[] = {c->d_coords, c->d_conn, c->d_inc_ptr, c->d_inc, c->d_nb_ptr, c->d_nb, c->d_row_ptr, c->d_col_idx,
-                    c->d_elem_pos, c->d_elem_slot, c->d_kvec, c->d_elist, c->d_first_mask, c->d_first_res, c->d_Ke, c->d_Re, c->d_matd, c->d_stats, c->d_u, c->d_hin, c->d_hout,
+                    c->d_eslot, c->d_elem_pos, c->d_elem_slot, c->d_kvec, c->d_elist, c->d_first_mask, c->d_first_res, c->d_Ke, c->d_Re, c->d_matd, c->d_stats, c->d_u, c->d_hin, c->d_hout,
                     c->d_mat, c->d_res, c->d_vals};
     for (void *p : ptrs) if (p) cudaFree(p);
     for (int i = 0; i < 4; i++) if (c->ev[i]) cudaEventDestroy(c->ev[i]);
@@ -319,9 +325,13 @@ extern "C" int fem_build_csr_pattern(fem_ctx *c, long long *n_rows, long long *n
             if (c->mode == 1) {
                 rc = fem_build_colouring(c);
                 if (rc != FEM_OK) break;
-            } else {   // scratch for the two-kernel mode
+            } else {   // scratch for the two-kernel mode (destination-major: one 72-double record per incidence entry)
+                TRY(cudaMalloc(&c->d_eslot, sizeof(int) * 8 * ne));
+                k_eslot<<<nblk(8 * ne, 256), 256>>>(ne, c->d_inc, c->d_eslot);
+                TRY(cudaGetLastError());
                 TRY(cudaMalloc(&c->d_Ke, sizeof(double) * 576 * ne));
                 TRY(cudaMalloc(&c->d_Re, sizeof(double) * 24 * ne));
+                TRY(cudaDeviceSynchronize());
             }
 #undef TRY
         } while (0);
