@@ -184,7 +184,7 @@ def run_gpu(args):
     ne, nn = cfg["conn"].shape[0], cfg["coords"].shape[0]
     mat_np = fem.mat_from_desc(cfg["matdesc"], ne)
     t0 = time.perf_counter()
-    ctx = fem.FemContext(torch.from_numpy(cfg["coords"]).to(dev), torch.from_numpy(cfg["conn"]).to(dev), fbar=args.fbar)
+    ctx = fem.FemContext(torch.from_numpy(cfg["coords"]).to(dev), torch.from_numpy(cfg["conn"]).to(dev), fbar=args.fbar, assembly_mode=args.mode)
     torch.cuda.synchronize()
     t_setup = time.perf_counter() - t0
     t0 = time.perf_counter()
@@ -326,6 +326,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--n", type=int, default=100, help="mesh resolution (100 = BASELINE.json config 3)")
     ap.add_argument("--fbar", type=int, default=0)
+    ap.add_argument("--mode", type=int, default=None, help="fem_options.assembly_mode (default: the library's default)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     args = ap.parse_args()
     if args.impl == "reference":

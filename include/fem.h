@@ -52,11 +52,17 @@ typedef struct {
     int jmax;          /* kept for ABI parity with Alg. C2's line search; the scalar solve
                           uses a bracket instead, so it is unused */
     double beta, eta;  /* Alg. C2 / App. B constants; unused by the scalar solve */
-    int assembly_mode; /* 0 (default) = element scratch + deterministic node-row gather kernel;
+    int assembly_mode; /* 0 (default) = element kernel writes K^e, R^e to a destination-major scratch, a node-row gather kernel
+                          sums them in ascending element id (deterministic, no atomics);
                           1 = coloured in-place assembly: elements are coloured at pattern-build time so that no two elements
                           of a colour share a node; one element-kernel launch per colour adds K^e, R^e into the outputs with
-                          plain read-modify-write in colour order (deterministic, no atomics, no scratch).  Measured 2.3x
-                          slower than mode 0 at config 3, kept as a tested option. */
+                          plain read-modify-write in colour order (deterministic, no atomics, no scratch);
+                          2 = fused: same scratch and summation order as mode 0, but the element CTAs count every node's
+                          missing contributions down and queue completed nodes, and gather CTAs interleaved in the same
+                          launch (plus a drain kernel) assemble them while other elements are still being evaluated.
+                          Modes 1 and 2 are measured slower than mode 0 at config 3 and are kept as
+                          tested options; they fall back to mode 0 for meshes with collapsed elements (1, 2) or a node with
+                          more than 8 elements (2). */
 } fem_options;
 
 typedef struct {

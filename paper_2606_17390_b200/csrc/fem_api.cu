@@ -82,7 +82,7 @@ extern "C" int fem_last_kernel_ms(fem_ctx *c, double ms[3]) {
 
 extern "C" int fem_launches_per_assemble(const fem_ctx *c) {
     if (!c) return 0;
-    return c->mode == 1 ? 1 + c->n_colours : 3;   // mat_prep + one element launch per colour | mat_prep + element + gather
+    return c->mode == 1 ? 1 + c->n_colours : 3;   // mat_prep + one element launch per colour | mat_prep + element (+ fused gather) + gather / drain
 }
 
 // ------------------------------------------------------------------------------------------------ FP64 peak probe

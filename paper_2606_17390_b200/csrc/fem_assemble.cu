@@ -176,6 +176,113 @@ __device__ __forceinline__ void flow_stress(double law, double h0, double h1, do
     }
 }
 
+// ------------------------------------------------------------------------------------------------ node gather (S14), shared
+// by the stand-alone gather kernels and by the gather CTAs of the fused mode.
+// The scratch is destination-major: node n's contributions are the records inc_ptr[n] .. inc_ptr[n+1]-1 (72 doubles each:
+// block row I of K^e of incident entry s = (e,I), ascending element id), one contiguous run.
+__device__ __forceinline__ int ksoff(int K, int c) { return (c < 8) ? ((c >> 1) * 16 + K * 2 + (c & 1)) : (64 + K); }
+__device__ __forceinline__ void cp_async16(void *smem_dst, const void *gsrc) {
+    const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sa), "l"(gsrc) : "memory");
+}
+// K = A K^e, R = A R^e (Eq.(34) :253, Eq.(38) :274) for one node whose run of records sits in shared memory (buf).
+// kvec[block] (built at setup) holds, for each incident entry s, the local node K of the block's column node (nibble s;
+// 0xF = that element does not contain it), so lane = neighbour position adds <= 8 blocks in ascending s (fixed order, no
+// atomics) with four 16-byte and one 8-byte conflict-free shared loads per block.
+__device__ __forceinline__ void gather_reduce_write(long long n, int b, int m, const double *buf, int lane,
+                                                    const int *__restrict__ nb_ptr, const unsigned int *__restrict__ kvec,
+                                                    const double *Re, double *__restrict__ csr_vals, double *__restrict__ residual) {
+    const int o = nb_ptr[n], len = nb_ptr[n + 1] - o;
+    double rv = 0.0;
+    if (lane < 3 * m) rv = __ldcg(Re + (long long)b * 3 + lane);
+    for (int pos0 = 0; pos0 < len; pos0 += 32) {
+        const int pos = pos0 + lane;
+        const unsigned kv = (pos < len) ? kvec[o + pos] : 0xffffffffu;
+        double acc[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
+#pragma unroll
+        for (int s = 0; s < 8; s++) {
+            if (s < m) {   // warp-uniform
+                const unsigned K = (kv >> (4 * s)) & 15u;
+                if (K != 15u) {
+                    const double *rec = buf + s * 72 + 2 * K;
+                    const double2 p0 = *reinterpret_cast<const double2 *>(rec), p1 = *reinterpret_cast<const double2 *>(rec + 16),
+                                  p2 = *reinterpret_cast<const double2 *>(rec + 32), p3 = *reinterpret_cast<const double2 *>(rec + 48);
+                    const double p4 = buf[s * 72 + 64 + K];
+                    acc[0] += p0.x; acc[1] += p0.y; acc[2] += p1.x; acc[3] += p1.y; acc[4] += p2.x; acc[5] += p2.y;
+                    acc[6] += p3.x; acc[7] += p3.y; acc[8] += p4;
+                }
+            }
+        }
+        if (pos < len) {
+            double *out = csr_vals + 9LL * o + 3 * pos;
+#pragma unroll
+            for (int i = 0; i < 3; i++) {
+                out[(long long)i * 3 * len + 0] = acc[3 * i + 0];
+                out[(long long)i * 3 * len + 1] = acc[3 * i + 1];
+                out[(long long)i * 3 * len + 2] = acc[3 * i + 2];
+            }
+        }
+    }
+    {   // residual: lane 3 s + i holds R^e component i of incident entry s; lanes 0..2 add in ascending s
+        double r = 0.0;
+        for (int j = 0; j < m; j++) r += __shfl_sync(0xffffffffu, rv, (3 * j + lane) & 31);
+        if (lane < 3) residual[3 * n + lane] = r;
+    }
+}
+// One warp gathers up to 4 nodes (lane j < cnt holds node id nd): asynchronous 16-byte copies of the four runs into the
+// warp's shared-memory buffer (4 x 576 doubles) are all in flight before the first reduction starts.
+__device__ __forceinline__ void gather_warp_nodes(int nd, int cnt, double *wbuf, int lane, const int *__restrict__ inc_ptr,
+                                                  const int *__restrict__ nb_ptr, const unsigned int *__restrict__ kvec,
+                                                  const double *Ke, const double *Re, double *__restrict__ csr_vals,
+                                                  double *__restrict__ residual) {
+    int b = 0, m = 0;
+    if (lane < cnt) { b = inc_ptr[nd]; m = inc_ptr[nd + 1] - b; }
+#pragma unroll
+    for (int j = 0; j < 4; j++) {
+        const int bj = __shfl_sync(0xffffffffu, b, j), lim = 36 * __shfl_sync(0xffffffffu, m, j);
+        const double *src = Ke + (long long)bj * 72;
+#pragma unroll
+        for (int it = 0; it < 9; it++) {
+            const int idx = it * 32 + lane;
+            if (idx < lim) cp_async16(wbuf + j * 576 + 2 * idx, src + 2 * idx);
+        }
+    }
+    asm volatile("cp.async.commit_group;" ::: "memory");
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
+    __syncwarp();
+#pragma unroll 1
+    for (int j = 0; j < cnt; j++)
+        gather_reduce_write(__shfl_sync(0xffffffffu, nd, j), __shfl_sync(0xffffffffu, b, j), __shfl_sync(0xffffffffu, m, j),
+                            wbuf + j * 576, lane, nb_ptr, kvec, Re, csr_vals, residual);
+    __syncwarp();
+}
+// Claims up to `want` completed nodes of the queue: returns the count and the first queue index in h.  Entries below the
+// tail have a ticket; their node id may still be on its way (the reader spins on -1).
+__device__ __forceinline__ unsigned queue_claim(unsigned int *qctl, unsigned want, unsigned &h) {
+    volatile unsigned int *q = qctl;
+    for (;;) {
+        h = q[1];
+        const unsigned t = q[0];
+        if (t <= h) return 0u;
+        const unsigned n = min(want, t - h);
+        if (atomicCAS(&qctl[1], h, h + n) == h) return n;
+    }
+}
+__device__ __forceinline__ int queue_read(const int *queue, unsigned idx) {
+    volatile const int *qp = queue + idx;
+    int v;
+    while ((v = *qp) < 0) { }
+    return v;
+}
+#ifndef GATHER_EVERY
+#define GATHER_EVERY 8
+#endif
+// GATHER_EVERY:   // fused mode: one gather CTA after every 8 element CTAs
+#ifndef GATHER_POP
+#define GATHER_POP 160
+#endif
+// GATHER_POP:   // nodes a gather CTA claims at most (8 element CTAs complete ~132 nodes)
+
 // Keeping the warps of a CTA in the same code region lets them share instruction-cache lines (the kernel is ~94 KB of
 // straight-line SASS); ncu showed instruction fetch as a top stall without it.
 #ifndef PS_MASK
@@ -192,6 +299,12 @@ struct scatter_args {
     const unsigned long long *first_mask;   // bit I*8+K: store instead of add
     const unsigned int *first_res;          // bit I: store the residual instead of add
     double *csr_vals, *residual;
+    // MODE 2 (fused): countdown of missing contributions per node, queue of completed nodes, gather tables
+    int *cnt;
+    int *queue;
+    unsigned int *qctl;                     // [0] tail, [1] head
+    const int *inc_ptr;
+    const unsigned int *kvec;
 };
 template <int FBAR, int MODE>
 __global__ void __launch_bounds__(CTA_THREADS, FBAR ? CTAS_FBAR : CTAS_STD)
@@ -205,7 +318,29 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
     constexpr int ES = FBAR ? ES_FBAR : ES_STD;
     const int tid = threadIdx.x, lane = tid & 31, q = lane & 7;
     const int el_cta = tid >> 3;
-    const long long e_raw = (long long)blockIdx.x * EL_PER_CTA + el_cta;
+    long long chunk = blockIdx.x;
+    if (MODE == 2) {
+        // fused mode: every (GATHER_EVERY+1)-th CTA is a gather CTA: it claims nodes whose contributions are complete (queue
+        // filled by the element CTAs below) and assembles their CSR rows; it never waits for a node that is not in the queue
+        const unsigned bx = blockIdx.x, grp = bx / (GATHER_EVERY + 1);
+        if (bx - grp * (GATHER_EVERY + 1) == GATHER_EVERY) {
+            __shared__ unsigned s_qh, s_qn;
+            if (tid == 0) { unsigned h; s_qn = queue_claim(sa.qctl, GATHER_POP, h); s_qh = h; }
+            __syncthreads();
+            const unsigned qh = s_qh, qn = s_qn;
+            double *wbuf = sm + (tid >> 5) * 4 * (FBAR ? ES_FBAR : ES_STD);
+            for (unsigned base = 4u * (tid >> 5); base < qn; base += 4u * (CTA_THREADS / 32)) {
+                const int cnt = (int)min(4u, qn - base);
+                int nd = 0;
+                if (lane < cnt) nd = queue_read(sa.queue, qh + base + lane);
+                __threadfence();
+                gather_warp_nodes(nd, cnt, wbuf, lane, sa.inc_ptr, sa.nb_ptr, sa.kvec, Ke, Re, sa.csr_vals, sa.residual);
+            }
+            return;
+        }
+        chunk = bx - grp;
+    }
+    const long long e_raw = chunk * EL_PER_CTA + el_cta;
     const bool valid = e_raw < n_elems;
     const long long e_slot = valid ? e_raw : n_elems - 1;
     const long long e = (MODE == 1 && sa.elist) ? (long long)sa.elist[e_slot] : e_slot;
@@ -225,7 +360,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
     }
     // ---- S2 gather: thread q loads node q of its element
     int my_node, my_slot = 0;
-    if (MODE == 0) my_slot = __ldg(sa.eslot + e * 8 + q);
+    if (MODE != 1) my_slot = __ldg(sa.eslot + e * 8 + q);
     {
         const long long nd = conn[e * 8 + q];
         my_node = (int)nd;
@@ -866,7 +1001,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
                 se[KSX(I, K, 6 + k)] += t2;
             }
     }
-    if (MODE == 0) {
+    if (MODE != 1) {
         // destination-major scratch: block row I of K^e and R^e_I go to the record of incidence entry (e,I) in the node-sorted
         // list, so that the gather kernel reads every node's contributions as one contiguous run
         if (valid) {
@@ -877,7 +1012,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
         // copy-out of the warp's 4 elements x 8 records of 576 bytes, 16 bytes per lane per step (9 steps per element)
         {
             const int w_el0 = (tid >> 5) * 4;
-            const long long e0 = (long long)blockIdx.x * EL_PER_CTA + w_el0;
+            const long long e0 = chunk * EL_PER_CTA + w_el0;
 #pragma unroll
             for (int el = 0; el < 4; el++) {
                 const double2 *src = reinterpret_cast<const double2 *>(sm + (w_el0 + el) * ES + SM_KS);
@@ -887,6 +1022,25 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
                     const int g = it * 32 + lane, rec = g / 36, off = g - rec * 36;
                     const int slot = __shfl_sync(0xffffffffu, my_slot, el * 8 + rec);
                     if (el_ok) reinterpret_cast<double2 *>(Ke + (long long)slot * 72)[off] = src[g];
+                }
+            }
+        }
+        if (MODE == 2) {
+            // publish: the records above become visible (fence), then each (element, node) counts its node down; whoever
+            // brings a node to zero queues it for the gather CTAs (one ticket request per warp)
+            __threadfence();
+            __syncwarp();
+            __threadfence();
+            const bool last = valid && (atomicSub(&sa.cnt[my_node], 1) == 1);
+            const unsigned mk = __ballot_sync(0xffffffffu, last);
+            if (mk) {
+                const int leader = __ffs(mk) - 1;
+                unsigned base = 0;
+                if (lane == leader) base = atomicAdd(&sa.qctl[0], (unsigned)__popc(mk));
+                base = __shfl_sync(0xffffffffu, base, leader);
+                if (last) {
+                    __threadfence();
+                    *reinterpret_cast<volatile int *>(sa.queue + base + __popc(mk & ((1u << lane) - 1u))) = my_node;
                 }
             }
         }
@@ -955,11 +1109,6 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
 }
 
 // ------------------------------------------------------------------------------------------------ gather kernels (S14)
-// K = A K^e, R = A R^e (Eq.(34) :253, Eq.(38) :274) with a fixed summation order and no atomics.
-// The scratch is destination-major: node n's contributions are the records inc_ptr[n] .. inc_ptr[n+1]-1 (72 doubles each:
-// block row I of K^e of incident entry s = (e,I), ascending element id), one contiguous run.
-__device__ __forceinline__ int ksoff(int K, int c) { return (c < 8) ? ((c >> 1) * 16 + K * 2 + (c & 1)) : (64 + K); }
-
 // General kernel (a node with more than 8 incident elements, or collapsed elements): one warp per node, lane <-> neighbour
 // position pos; the elem_pos bytes of each incident entry give the local nodes K whose column node sits at pos.
 __global__ void __launch_bounds__(256)
@@ -1003,10 +1152,8 @@ k_gather(long long n_nodes, const int *__restrict__ inc_ptr, const int *__restri
 }
 
 // Fast gather for meshes where every node has <= 8 incident elements and no element lists a node twice (all hex meshes
-// of the configs).  The warp copies the node's run of records (<= 4608 bytes) into shared memory with coalesced 16-byte
-// loads; kvec[block] (built at setup) holds, for each incident entry s, the local node K of the block's column node
-// (nibble s; 0xF = that element does not contain it), so lane = neighbour position adds <= 8 blocks in ascending s with
-// four 16-byte and one 8-byte conflict-free shared loads per block.
+// of the configs): one warp per node copies the node's run of records (<= 4608 bytes) into shared memory with coalesced
+// 16-byte loads and reduces it with gather_reduce_write.
 #define GW 8   // warps (nodes) per CTA
 #ifndef GMINB
 #define GMINB 5
@@ -1020,7 +1167,6 @@ k_gather_fast(long long n_nodes, const int *__restrict__ inc_ptr, const int *__r
     const long long n = (long long)blockIdx.x * GW + w;
     if (n >= n_nodes) return;
     const int b = inc_ptr[n], m = inc_ptr[n + 1] - b;
-    const int o = nb_ptr[n], len = nb_ptr[n + 1] - o;
     {
         const double2 *src = reinterpret_cast<const double2 *>(Ke + (long long)b * 72);
         double2 *dst = reinterpret_cast<double2 *>(buf[w]);
@@ -1031,41 +1177,31 @@ k_gather_fast(long long n_nodes, const int *__restrict__ inc_ptr, const int *__r
 #pragma unroll
         for (int it = 0; it < 9; it++) if (it * 32 + lane < lim) dst[it * 32 + lane] = t[it];
     }
-    double rv = 0.0;
-    if (lane < 3 * m) rv = Re[(long long)b * 3 + lane];
     __syncwarp();
-    for (int pos0 = 0; pos0 < len; pos0 += 32) {
-        const int pos = pos0 + lane;
-        const unsigned kv = (pos < len) ? kvec[o + pos] : 0xffffffffu;
-        double acc[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
-#pragma unroll
-        for (int s = 0; s < 8; s++) {
-            if (s < m) {   // warp-uniform
-                const unsigned K = (kv >> (4 * s)) & 15u;
-                if (K != 15u) {
-                    const double *rec = buf[w] + s * 72 + 2 * K;
-                    const double2 p0 = *reinterpret_cast<const double2 *>(rec), p1 = *reinterpret_cast<const double2 *>(rec + 16),
-                                  p2 = *reinterpret_cast<const double2 *>(rec + 32), p3 = *reinterpret_cast<const double2 *>(rec + 48);
-                    const double p4 = buf[w][s * 72 + 64 + K];
-                    acc[0] += p0.x; acc[1] += p0.y; acc[2] += p1.x; acc[3] += p1.y; acc[4] += p2.x; acc[5] += p2.y;
-                    acc[6] += p3.x; acc[7] += p3.y; acc[8] += p4;
-                }
-            }
-        }
-        if (pos < len) {
-            double *out = csr_vals + 9LL * o + 3 * pos;
-#pragma unroll
-            for (int i = 0; i < 3; i++) {
-                out[(long long)i * 3 * len + 0] = acc[3 * i + 0];
-                out[(long long)i * 3 * len + 1] = acc[3 * i + 1];
-                out[(long long)i * 3 * len + 2] = acc[3 * i + 2];
-            }
-        }
-    }
-    {   // residual: lane 3 s + i holds R^e component i of incident entry s; lanes 0..2 add in ascending s
-        double r = 0.0;
-        for (int j = 0; j < m; j++) r += __shfl_sync(0xffffffffu, rv, (3 * j + lane) & 31);
-        if (lane < 3) residual[3 * n + lane] = r;
+    gather_reduce_write(n, b, m, buf[w], lane, nb_ptr, kvec, Re, csr_vals, residual);
+}
+
+// Fused mode, after the element kernel: persistent CTAs drain what is left in the queue of completed nodes (every node is
+// in it by now).  4 warps x 4 nodes per batch.
+__global__ void __launch_bounds__(128)
+k_gather_drain(unsigned int n_nodes, const int *__restrict__ queue, unsigned int *qctl, const int *__restrict__ inc_ptr,
+               const int *__restrict__ nb_ptr, const unsigned int *__restrict__ kvec, const double *__restrict__ Ke,
+               const double *__restrict__ Re, double *__restrict__ csr_vals, double *__restrict__ residual) {
+    extern __shared__ __align__(16) double dbuf[];
+    __shared__ unsigned s_h;
+    const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    for (;;) {
+        if (threadIdx.x == 0) s_h = atomicAdd(&qctl[1], 16u);
+        __syncthreads();
+        const unsigned h = s_h;
+        __syncthreads();
+        if (h >= n_nodes) return;
+        const unsigned base = h + 4u * w;
+        if (base >= n_nodes) continue;
+        const int cnt = (int)min(4u, n_nodes - base);
+        int nd = 0;
+        if (lane < cnt) nd = queue[base + lane];
+        gather_warp_nodes(nd, cnt, dbuf + w * 2304, lane, inc_ptr, nb_ptr, kvec, Ke, Re, csr_vals, residual);
     }
 }
 
@@ -1094,7 +1230,36 @@ int fem_launch_assemble(fem_ctx *c, const double *u, const double *hist_in, cons
     k_mat_prep<<<nblk2(n_mat, 128), 128, 0, st>>>(n_mat, mat, c->d_matd);
     FEM_CUDA(cudaEventRecord(c->ev[1], st));
     const int mstride = (n_mat == 1) ? 0 : FEM_MATD;
-    scatter_args sa = {nullptr, c->d_eslot, c->d_nb_ptr, c->d_elem_pos, c->d_first_mask, c->d_first_res, csr_vals, residual};
+    scatter_args sa = {nullptr, c->d_eslot, c->d_nb_ptr, c->d_elem_pos, c->d_first_mask, c->d_first_res, csr_vals, residual,
+                       c->d_cnt, c->d_queue, c->d_qctl, c->d_inc_ptr, c->d_kvec};
+    if (c->mode == 2) {
+        // fused mode: element CTAs count the nodes down and queue completed ones; interleaved gather CTAs and the drain
+        // kernel assemble them.  Per call: reset the countdown, the queue (nodes without elements are pre-queued) and its counters.
+        static bool attr2 = false;
+        if (!attr2) {
+            FEM_CUDA(cudaFuncSetAttribute(k_element<0, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_std));
+            FEM_CUDA(cudaFuncSetAttribute(k_element<1, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_fbar));
+            FEM_CUDA(cudaFuncSetAttribute(k_gather_drain, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * 2304 * 8));
+            attr2 = true;
+        }
+        FEM_CUDA(cudaMemcpyAsync(c->d_cnt, c->d_cnt_init, sizeof(int) * c->n_nodes, cudaMemcpyDeviceToDevice, st));
+        FEM_CUDA(cudaMemcpyAsync(c->d_queue, c->d_queue_init, sizeof(int) * c->n_nodes, cudaMemcpyDeviceToDevice, st));
+        FEM_CUDA(cudaMemcpyAsync(c->d_qctl, c->d_qctl + 2, sizeof(unsigned int) * 2, cudaMemcpyDeviceToDevice, st));   // tail = isolated nodes, head = 0
+        const long long nE = (c->n_elems + EL_PER_CTA - 1) / EL_PER_CTA;
+        const unsigned grid = (unsigned)(nE + (nE + GATHER_EVERY - 1) / GATHER_EVERY);   // element CTAs + one gather CTA per GATHER_EVERY
+        if (c->opt.fbar)
+            k_element<1, 2><<<grid, CTA_THREADS, sm_fbar, st>>>(c->n_elems, c->d_coords, c->d_conn, u, hist_in, c->d_matd, mstride,
+                                                        c->opt.tol, c->opt.kmax, c->d_Ke, c->d_Re, hist_out, c->d_stats, sa);
+        else
+            k_element<0, 2><<<grid, CTA_THREADS, sm_std, st>>>(c->n_elems, c->d_coords, c->d_conn, u, hist_in, c->d_matd, mstride,
+                                                       c->opt.tol, c->opt.kmax, c->d_Ke, c->d_Re, hist_out, c->d_stats, sa);
+        FEM_CUDA(cudaEventRecord(c->ev[2], st));
+        int dev = 0, nsm = 148;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+        k_gather_drain<<<3 * nsm, 128, 4 * 2304 * 8, st>>>((unsigned)c->n_nodes, c->d_queue, c->d_qctl, c->d_inc_ptr, c->d_nb_ptr, c->d_kvec,
+                                                        c->d_Ke, c->d_Re, csr_vals, residual);
+    } else
     if (c->mode == 1) {
         // one launch per colour, in colour order (stream order = summation order)
         for (int k = 0; k < c->n_colours; k++) {

@@ -28,7 +28,14 @@ struct fem_ctx {
     int *d_elist = nullptr;                       // [n_elems] element ids sorted by (colour, id)
     unsigned long long *d_first_mask = nullptr;   // [n_elems] bit I*8+K: this element stores block (I,K) instead of adding
     unsigned int *d_first_res = nullptr;          // [n_elems] bit I: this element stores the residual of its local node I
-    int mode = 0;                                 // effective assembly mode (1 falls back to 0 for collapsed elements)
+    int mode = 0;                                 // effective assembly mode (1 and 2 fall back to 0 where they do not apply)
+    // fused mode (assembly_mode 2): per-node countdown of missing contributions + queue of completed nodes
+    int *d_cnt_init = nullptr;                    // [n_nodes] number of incident elements
+    int *d_cnt = nullptr;                         // [n_nodes] working copy, counted down by the element CTAs
+    int *d_queue_init = nullptr;                  // [n_nodes] nodes without elements first, then -1
+    int *d_queue = nullptr;                       // [n_nodes] working copy: node ids in order of completion
+    unsigned int *d_qctl = nullptr;               // [0] tail (tickets handed out), [1] head (entries claimed), [2..3] initial values
+    int n_isolated = 0;
     bool has_collapsed = false;                   // some element lists a node twice
     int n_colours = 0, colour_rounds = 0;
     long long colour_start[65] = {0};

@@ -155,6 +155,15 @@ __global__ void k_eslot(long long n_elems, const int *__restrict__ inc, int *esl
     if (j < 8 * n_elems) eslot[inc[j]] = (int)j;
 }
 
+// fused mode: countdown template and the queue template (nodes without elements are queued from the start)
+__global__ void k_cnt_init(long long n_nodes, const int *__restrict__ inc_ptr, int *cnt_init, int *queue_init, int *n_iso) {
+    long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (n >= n_nodes) return;
+    const int m = inc_ptr[n + 1] - inc_ptr[n];
+    cnt_init[n] = m;
+    if (m == 0) queue_init[atomicAdd(n_iso, 1)] = (int)n;
+}
+
 // kvec for the fast gather; flags |= 16 if some node has more than 8 incident elements
 __global__ void k_kvec(long long n_nodes, const int *__restrict__ inc_ptr, const int *__restrict__ inc,
                        const int *__restrict__ nb_ptr, const unsigned char *__restrict__ elem_pos, unsigned int *kvec, int *flags) {
@@ -216,7 +225,7 @@ extern "C" int fem_hill_from_lankford(double r0, double r45, double r90, double 
 static void ctx_free(fem_ctx *c) {
     if (!c) return;
     void *ptrs[] = {c->d_coords, c->d_conn, c->d_inc_ptr, c->d_inc, c->d_nb_ptr, c->d_nb, c->d_row_ptr, c->d_col_idx,
-                    c->d_eslot, c->d_elem_pos, c->d_elem_slot, c->d_kvec, c->d_elist, c->d_first_mask, c->d_first_res, c->d_Ke, c->d_Re, c->d_matd, c->d_stats, c->d_u, c->d_hin, c->d_hout,
+                    c->d_eslot, c->d_cnt_init, c->d_cnt, c->d_queue_init, c->d_queue, c->d_qctl, c->d_elem_pos, c->d_elem_slot, c->d_kvec, c->d_elist, c->d_first_mask, c->d_first_res, c->d_Ke, c->d_Re, c->d_matd, c->d_stats, c->d_u, c->d_hin, c->d_hout,
                     c->d_mat, c->d_res, c->d_vals};
     for (void *p : ptrs) if (p) cudaFree(p);
     for (int i = 0; i < 4; i++) if (c->ev[i]) cudaEventDestroy(c->ev[i]);
@@ -234,7 +243,7 @@ extern "C" int fem_setup(fem_ctx **out, long long n_nodes, const double *coords,
     fem_default_options(&o);
     if (opt) o = *opt;
     if (o.quad_order != 2) return FEM_ERR_QUAD;
-    if ((o.fbar != 0 && o.fbar != 1) || !(o.tol > 0) || o.kmax < 1 || (o.assembly_mode != 0 && o.assembly_mode != 1)) return FEM_ERR_ARG;
+    if ((o.fbar != 0 && o.fbar != 1) || !(o.tol > 0) || o.kmax < 1 || (o.assembly_mode < 0 || o.assembly_mode > 2)) return FEM_ERR_ARG;
     int ndev = 0;
     FEM_CUDA(cudaGetDeviceCount(&ndev));
     if (ndev < 1) { snprintf(g_fem_cuda_err, sizeof(g_fem_cuda_err), "no CUDA device"); return FEM_ERR_CUDA; }
@@ -256,7 +265,7 @@ extern "C" int fem_setup(fem_ctx **out, long long n_nodes, const double *coords,
         if (hflags & 1) { rc = FEM_ERR_CONN; break; }
         if (hflags & 2) { rc = FEM_ERR_INVERTED; break; }
         c->has_collapsed = (hflags & 8) != 0;
-        c->mode = (o.assembly_mode == 1 && !c->has_collapsed) ? 1 : 0;   // in-place scatter needs distinct nodes per element
+        c->mode = (o.assembly_mode != 0 && !c->has_collapsed) ? o.assembly_mode : 0;   // modes 1, 2 need distinct nodes per element
         TRY(cudaMalloc(&c->d_stats, sizeof(unsigned long long) * 72));
         for (int i = 0; i < 4; i++) TRY(cudaEventCreate(&c->ev[i]));
 #undef TRY
@@ -320,6 +329,20 @@ extern "C" int fem_build_csr_pattern(fem_ctx *c, long long *n_rows, long long *n
                 int kf = 0;
                 TRY(cudaMemcpy(&kf, dflags, sizeof(int), cudaMemcpyDeviceToHost));
                 if (kf & 16) { cudaFree(c->d_kvec); c->d_kvec = nullptr; }   // general gather kernel instead
+            }
+            if (c->mode == 2 && !c->d_kvec) c->mode = 0;   // the fused mode uses the fast gather tables
+            if (c->mode == 2) {
+                TRY(cudaMalloc(&c->d_cnt_init, sizeof(int) * nn));
+                TRY(cudaMalloc(&c->d_cnt, sizeof(int) * nn));
+                TRY(cudaMalloc(&c->d_queue_init, sizeof(int) * nn));
+                TRY(cudaMalloc(&c->d_queue, sizeof(int) * nn));
+                TRY(cudaMalloc(&c->d_qctl, sizeof(unsigned int) * 4));   // [0..1] live tail/head, [2..3] their initial values
+                TRY(cudaMemset(c->d_queue_init, 0xff, sizeof(int) * nn));
+                TRY(cudaMemset(dflags, 0, sizeof(int)));
+                k_cnt_init<<<nblk(nn, 256), 256>>>(nn, c->d_inc_ptr, c->d_cnt_init, c->d_queue_init, dflags);
+                TRY(cudaMemcpy(&c->n_isolated, dflags, sizeof(int), cudaMemcpyDeviceToHost));
+                const unsigned int ctl0[4] = {0u, 0u, (unsigned)c->n_isolated, 0u};
+                TRY(cudaMemcpy(c->d_qctl, ctl0, sizeof(ctl0), cudaMemcpyHostToDevice));
             }
             TRY(cudaDeviceSynchronize());
             if (c->mode == 1) {

@@ -214,3 +214,43 @@ def test_collapsed_hex_wedge_elements():
     g = run_gpu(cfg, 0, want_elem_slot=True, assembly_mode=1)     # asks for mode 1, library must fall back to the gather mode
     assert g["ctx"].launches_per_assemble() == 3
     compare(g, run_oracle(cfg, 0, with_slots=True), "wedge")
+
+
+@pytest.mark.parametrize("fbar", [0, 1])
+@pytest.mark.parametrize("cfgid,n", [(1, None), (3, 22), (4, 18)])
+def test_fused_queue_assembly_mode(cfgid, n, fbar):
+    """assembly_mode 2 (element CTAs count nodes down and queue completed ones; gather CTAs of the same launch and a drain
+    kernel assemble them) matches the oracle, is bit-identical to mode 0 (same summation order) and to itself."""
+    cfg = synth.make_config(cfgid) if n is None else synth.make_config(cfgid, n=n)
+    g = run_gpu(cfg, fbar, assembly_mode=2)
+    compare(g, run_oracle(cfg, fbar), "fused cfg%d" % cfgid)
+    g0 = run_gpu(cfg, fbar, assembly_mode=0)
+    assert np.array_equal(g["csr_vals"], g0["csr_vals"]) and np.array_equal(g["residual"], g0["residual"])
+    g2 = run_gpu(cfg, fbar, assembly_mode=2)
+    assert np.array_equal(g["csr_vals"], g2["csr_vals"]) and np.array_equal(g["residual"], g2["residual"])
+
+
+def test_fused_mode_repeated_calls_and_isolated_node():
+    """Mode 2 resets its countdown / queue on every call; a node that belongs to no element gets a zero residual."""
+    import torch
+    import paper_2606_17390_b200 as fem
+    cfg = synth.make_config(3, n=12)
+    coords = np.vstack([cfg["coords"], [[5.0, 5.0, 5.0]]])          # one extra, unreferenced node
+    u = np.vstack([cfg["u"], [[0.0, 0.0, 0.0]]])
+    cfg2 = dict(cfg, coords=coords, u=u)
+    o = run_oracle(cfg2)
+    dev = torch.device("cuda:0")
+    ne = cfg2["conn"].shape[0]
+    ctx = fem.FemContext(torch.from_numpy(coords).to(dev), torch.from_numpy(cfg2["conn"]).to(dev), assembly_mode=2)
+    ctx.build_csr_pattern()
+    mat = torch.from_numpy(fem.mat_from_desc(cfg2["matdesc"], ne).ravel()).to(dev)
+    ud, hd = torch.from_numpy(u.ravel()).to(dev), torch.from_numpy(cfg2["hist_in"].ravel()).to(dev)
+    prev = None
+    for _ in range(3):
+        res, vals, hout, _ = ctx.assemble(ud, hd, mat, want_stats=True)
+        torch.cuda.synchronize()
+        assert rel_l2(res.cpu().numpy(), o["residual"]) <= 1e-11 and rel_l2(vals.cpu().numpy(), o["csr_vals"]) <= 1e-10
+        assert np.all(res.cpu().numpy()[-3:] == 0.0)
+        if prev is not None:
+            assert torch.equal(prev, vals)
+        prev = vals.clone()
