@@ -91,8 +91,9 @@ __device__ __forceinline__ void jacobi_rot(double &app, double &aqq, double &apq
     // cos^2 = (1 + |d|/r)/2 with r = hypot(d, 2 a_pq); sin = sgn(d) a_pq / (r cos); tan = sin / cos.  Two rsqrt, no division.
     const double d = aqq - app;
     const double r2 = fma(d, d, 4.0 * apq * apq);
-    const double ir = (r2 > 1e-280) ? frsqrt(r2) : 0.0;
-    const double c2 = fma(0.5 * fabs(d), ir, 0.5);
+    const bool ok = r2 > 1e-280;                     // d = a_pq = 0 (e.g. C = I exactly): identity rotation
+    const double ir = frsqrt(ok ? r2 : 1.0);         // branch-free: the rotations of a sweep stay in one basic block
+    const double c2 = ok ? fma(0.5 * fabs(d), ir, 0.5) : 1.0;
     const double ic = frsqrt(c2);
     const double c = c2 * ic;
     const double s = ((d < 0.0) ? -apq : apq) * ir * ic;   // sgn(d) a_pq / (r c); d = 0 counts as positive
@@ -107,15 +108,15 @@ __device__ __forceinline__ void jacobi_rot(double &app, double &aqq, double &apq
 
 // atanh(w)/w : first divided difference kernel of ln,  ln(b/a) = 2 atanh((b-a)/(b+a)).
 __device__ __forceinline__ double atanhc(double w, double dlog /* = ln b - ln a */) {
-    double w2 = w * w;
-    if (w2 < 0.0225) {  // |w| < 0.15 : series 1 + w^2/3 + w^4/5 + ...  (11 terms, remainder < 1e-19)
-        double s = 1.0 / 21.0;
-        s = fma(s, w2, 1.0 / 19.0); s = fma(s, w2, 1.0 / 17.0); s = fma(s, w2, 1.0 / 15.0); s = fma(s, w2, 1.0 / 13.0);
-        s = fma(s, w2, 1.0 / 11.0); s = fma(s, w2, 1.0 / 9.0);  s = fma(s, w2, 1.0 / 7.0);  s = fma(s, w2, 1.0 / 5.0);
-        s = fma(s, w2, 1.0 / 3.0);  s = fma(s, w2, 1.0);
-        return s;
-    }
-    return 0.5 * dlog * frcp(w);
+    // branch-free (both forms are evaluated, one is selected) so that the calls of a thread interleave:
+    // |w| < 0.15 : series 1 + w^2/3 + w^4/5 + ...  (11 terms, remainder < 1e-19), else ln(b/a) / (2 w)
+    const double w2 = w * w;
+    double s = 1.0 / 21.0;
+    s = fma(s, w2, 1.0 / 19.0); s = fma(s, w2, 1.0 / 17.0); s = fma(s, w2, 1.0 / 15.0); s = fma(s, w2, 1.0 / 13.0);
+    s = fma(s, w2, 1.0 / 11.0); s = fma(s, w2, 1.0 / 9.0);  s = fma(s, w2, 1.0 / 7.0);  s = fma(s, w2, 1.0 / 5.0);
+    s = fma(s, w2, 1.0 / 3.0);  s = fma(s, w2, 1.0);
+    const double big = 0.5 * dlog * frcp(w);   // NaN for w = 0, never selected then
+    return (w2 < 0.0225) ? s : big;
 }
 
 // Second divided difference g[a,b,c] of g = 1/2 ln for three eigenvalues within 1e-4 (relative) of each other:
@@ -507,10 +508,12 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
 
     // ---- S5 Hencky strain eps = sum_a 1/2 ln(lam_a) n_a (x) n_a (Eq.(5) :96 with the 1/2 restored, G1), material frame
     double lg[3];   // ln(lam_a): for stretches within ~15 % of 1, ln l = 2 w atanh(w)/w with w = (l-1)/(l+1) (same series as atanhc)
+    {
+        double w[3];
 #pragma unroll
-    for (int a = 0; a < 3; a++) {
-        const double w = (lam[a] - 1.0) * frcp(lam[a] + 1.0);
-        lg[a] = (w * w < 0.0225) ? 2.0 * w * atanhc(w, 0.0) : log(lam[a]);
+        for (int a = 0; a < 3; a++) { w[a] = (lam[a] - 1.0) * frcp(lam[a] + 1.0); lg[a] = 2.0 * w[a] * atanhc(w[a], 0.0); }
+#pragma unroll
+        for (int a = 0; a < 3; a++) if (w[a] * w[a] >= 0.0225) lg[a] = log(lam[a]);
     }
     double ee[6];  // elastic trial strain eps - eps_p_n, tensor components (11,22,33,12,23,13), material frame
     {
@@ -579,11 +582,19 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
         double lo = 0.0, hi = INFINITY;
         const double atol = 4.0e-16 * phitr / mu2;  // round-off floor of dgam (a strain): eps * |T| / 2mu
         bool conv = false;
-        double prev_step = INFINITY;
+        double prev_step = INFINITY, al_eval = alphan;
 #pragma unroll 1
         for (int pass = 0;; pass++) {
             const double al = fma(W23, dg, alphan);
-            flow_stress(law, hh0, hh1, hh2, al, sf, dsf);
+            if (conv && law != 0.0) {
+                // state at the solution: the last Newton step moved alpha by delta with |delta| <= 1e-3 (eps0 + alpha), so the
+                // Swift law is continued by its 4-term binomial series (remainder < 1e-16 relative) instead of a second pow
+                const double bp = hh1 + al_eval, rho = (al - al_eval) * frcp(bp), n = hh2;
+                const double c2 = 0.5 * n * (n - 1.0), c3 = c2 * (n - 2.0) * (1.0 / 3.0), c4 = c3 * (n - 3.0) * 0.25;
+                sf *= fma(rho, fma(rho, fma(rho, fma(rho, c4, c3), c2), n), 1.0);
+                dsf = n * sf * frcp(hh1 + al);
+            } else flow_stress(law, hh0, hh1, hh2, al, sf, dsf);
+            al_eval = al;
             const double sy = W23 * sf, dsy = W23 * dsf;
             const double isy = frcp(sy);
             const double x = mu2 * dg * isy;
@@ -1014,14 +1025,14 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
             const int w_el0 = (tid >> 5) * 4;
             const long long e0 = chunk * EL_PER_CTA + w_el0;
 #pragma unroll
-            for (int el = 0; el < 4; el++) {
-                const double2 *src = reinterpret_cast<const double2 *>(sm + (w_el0 + el) * ES + SM_KS);
-                const bool el_ok = e0 + el < n_elems;
+            for (int it = 0; it < 9; it++) {
+                const int g = it * 32 + lane, rec = g / 36, off = g - rec * 36;
 #pragma unroll
-                for (int it = 0; it < 9; it++) {
-                    const int g = it * 32 + lane, rec = g / 36, off = g - rec * 36;
+                for (int el = 0; el < 4; el++) {
                     const int slot = __shfl_sync(0xffffffffu, my_slot, el * 8 + rec);
-                    if (el_ok) reinterpret_cast<double2 *>(Ke + (long long)slot * 72)[off] = src[g];
+                    if (e0 + el < n_elems)
+                        reinterpret_cast<double2 *>(Ke + (long long)slot * 72)[off] =
+                            reinterpret_cast<const double2 *>(sm + (w_el0 + el) * ES + SM_KS)[g];
                 }
             }
         }

@@ -254,3 +254,17 @@ def test_fused_mode_repeated_calls_and_isolated_node():
         if prev is not None:
             assert torch.equal(prev, vals)
         prev = vals.clone()
+
+
+@pytest.mark.parametrize("fbar", [0, 1])
+def test_zero_and_rigid_displacement(fbar):
+    """u = 0 (C = I exactly: every Jacobi rotation is the degenerate d = a_pq = 0 case) gives the linear-elastic stiffness
+    and a zero residual; a rigid translation gives the same matrix."""
+    cfg = synth.make_config(3, n=7)
+    cfg0 = dict(cfg, u=np.zeros_like(cfg["u"]))
+    g, o = run_gpu(cfg0, fbar), run_oracle(cfg0, fbar)
+    compare(g, o, "u=0")
+    assert np.abs(g["residual"]).max() <= 1e-9 and g["stats"]["n_plastic"] == 0
+    cfg1 = dict(cfg, u=np.tile(np.array([0.3, -0.2, 0.1]), (cfg["u"].shape[0], 1)))
+    g1 = run_gpu(cfg1, fbar)
+    assert rel_l2(g1["csr_vals"], o["csr_vals"]) <= 1e-10 and np.abs(g1["residual"]).max() <= 1e-6
