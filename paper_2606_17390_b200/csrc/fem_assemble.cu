@@ -148,20 +148,24 @@ __host__ __device__ constexpr int sidx9(int r, int c) {  // packed upper triangl
 #define SM_XE 200   // [24] element coordinates   (overlay: dead before AA is written)
 #define SM_UE 224   // [24] element displacements (overlay)
 #define SM_KS 0     // K^e staging, 8 block-row records of 72 doubles (scratch record layout), overlays GG/AA after phase 2
-// component c of block (I,K) inside block row I: pairs of components interleaved by K so that the gather kernel reads
-// (c, c+1) of one block with one 16-byte load and its 8 lanes of an incident element touch 128 contiguous bytes
-#define KSX(I, K, c) (SM_KS + (I) * 72 + (((c) < 8) ? (((c) >> 1) * 16 + (K) * 2 + ((c) & 1)) : (64 + (K))))
+// component c of block (I,K) inside block row I: component-major [c][K], so that the two accumulators of a DMMA lane
+// (columns K = 2 tig, 2 tig + 1) are one 16-byte store and the 8 lanes of a transposed store fill 64 contiguous bytes
+#define KSX(I, K, c) (SM_KS + (I) * 72 + (c) * 8 + (K))
 #define SM_GQ 576   // [24][8]  (F-bar) g^q_Kk = G_KL F^-1_Lk
 #define SM_YY 768   // [9][8]   (F-bar) w/3 (A^:F^)_ia
 #define SM_GB 840   // [24]     (F-bar) gbar
 #define SM_WQ 864   // [8]      (F-bar) w_q J_q / (Jbar V)
-#define ES_STD 580   // >= 576, = 4 mod 16: the 4 elements of a warp start in 4 different bank groups
+#define ES_STD 564   // >= 560, = 4 mod 16: the 4 elements of a warp start in 4 different bank groups
+#define ES_STAGE 580 // >= 576, = 4 mod 16: variants that stage the whole K^e (coloured mode) or lend their buffer to gather CTAs (fused mode)
 #define ES_FBAR 884  // >= 872, = 4 mod 16
 #ifndef EL_PER_CTA
 #define EL_PER_CTA 16
 #endif
 #define CTA_THREADS (8 * EL_PER_CTA)
-#define CTAS_STD (384 / CTA_THREADS)   // 12 warps per SM: limited by 168 registers and ~4.5 KB shared memory per element
+#ifndef THREADS_PER_SM
+#define THREADS_PER_SM 384
+#endif
+#define CTAS_STD (THREADS_PER_SM / CTA_THREADS)   // 12 warps per SM: limited by 168 registers and ~4.5 KB shared memory per element
 #define CTAS_FBAR (256 / CTA_THREADS)
 
 __device__ __forceinline__ void flow_stress(double law, double h0, double h1, double h2, double alpha, double &sf,
@@ -181,7 +185,7 @@ __device__ __forceinline__ void flow_stress(double law, double h0, double h1, do
 // by the stand-alone gather kernels and by the gather CTAs of the fused mode.
 // The scratch is destination-major: node n's contributions are the records inc_ptr[n] .. inc_ptr[n+1]-1 (72 doubles each:
 // block row I of K^e of incident entry s = (e,I), ascending element id), one contiguous run.
-__device__ __forceinline__ int ksoff(int K, int c) { return (c < 8) ? ((c >> 1) * 16 + K * 2 + (c & 1)) : (64 + K); }
+__device__ __forceinline__ int ksoff(int K, int c) { return c * 8 + K; }
 __device__ __forceinline__ void cp_async16(void *smem_dst, const void *gsrc) {
     const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_dst);
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sa), "l"(gsrc) : "memory");
@@ -189,7 +193,7 @@ __device__ __forceinline__ void cp_async16(void *smem_dst, const void *gsrc) {
 // K = A K^e, R = A R^e (Eq.(34) :253, Eq.(38) :274) for one node whose run of records sits in shared memory (buf).
 // kvec[block] (built at setup) holds, for each incident entry s, the local node K of the block's column node (nibble s;
 // 0xF = that element does not contain it), so lane = neighbour position adds <= 8 blocks in ascending s (fixed order, no
-// atomics) with four 16-byte and one 8-byte conflict-free shared loads per block.
+// atomics) with nine conflict-free shared loads per block.
 __device__ __forceinline__ void gather_reduce_write(long long n, int b, int m, const double *buf, int lane,
                                                     const int *__restrict__ nb_ptr, const unsigned int *__restrict__ kvec,
                                                     const double *Re, double *__restrict__ csr_vals, double *__restrict__ residual) {
@@ -205,12 +209,9 @@ __device__ __forceinline__ void gather_reduce_write(long long n, int b, int m, c
             if (s < m) {   // warp-uniform
                 const unsigned K = (kv >> (4 * s)) & 15u;
                 if (K != 15u) {
-                    const double *rec = buf + s * 72 + 2 * K;
-                    const double2 p0 = *reinterpret_cast<const double2 *>(rec), p1 = *reinterpret_cast<const double2 *>(rec + 16),
-                                  p2 = *reinterpret_cast<const double2 *>(rec + 32), p3 = *reinterpret_cast<const double2 *>(rec + 48);
-                    const double p4 = buf[s * 72 + 64 + K];
-                    acc[0] += p0.x; acc[1] += p0.y; acc[2] += p1.x; acc[3] += p1.y; acc[4] += p2.x; acc[5] += p2.y;
-                    acc[6] += p3.x; acc[7] += p3.y; acc[8] += p4;
+                    const double *rec = buf + s * 72 + K;   // [c][K]: the lanes of one incident entry read 8 adjacent doubles
+#pragma unroll
+                    for (int j = 0; j < 9; j++) acc[j] += rec[8 * j];
                 }
             }
         }
@@ -316,7 +317,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
     extern __shared__ __align__(16) double sm[];
     __shared__ unsigned int s_hist[64];
     __shared__ unsigned int s_done;
-    constexpr int ES = FBAR ? ES_FBAR : ES_STD;
+    constexpr int ES = FBAR ? ES_FBAR : (MODE == 0 ? ES_STD : ES_STAGE);
     const int tid = threadIdx.x, lane = tid & 31, q = lane & 7;
     const int el_cta = tid >> 3;
     long long chunk = blockIdx.x;
@@ -329,7 +330,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
             if (tid == 0) { unsigned h; s_qn = queue_claim(sa.qctl, GATHER_POP, h); s_qh = h; }
             __syncthreads();
             const unsigned qh = s_qh, qn = s_qn;
-            double *wbuf = sm + (tid >> 5) * 4 * (FBAR ? ES_FBAR : ES_STD);
+            double *wbuf = sm + (tid >> 5) * 4 * (FBAR ? ES_FBAR : ES_STAGE);
             for (unsigned base = 4u * (tid >> 5); base < qn; base += 4u * (CTA_THREADS / 32)) {
                 const int cnt = (int)min(4u, qn - base);
                 int nd = 0;
@@ -968,10 +969,32 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
                                          : "+d"(C[p][0]), "+d"(C[p][1]) : "d"(g[h][a_]), "d"(hv));
                         }
                 }
-            __syncwarp();   // every lane has read this element's G^ and A^: the staging below overlays them
-            // ---- phase 3: stage the full K^e (8 block-row records [I][72], scratch record layout); lane holds
-            //      K^{ik}[gid][2 tig + j] = component (i,k) of block (gid, 2 tig + j) = component (k,i) of the transposed block
-            {
+            if (!FBAR && MODE != 1) {
+                // ---- phase 3 (standard element, scratch modes): the accumulators go straight to the destination-major scratch.
+                //      Lane holds K^{ik}[gid][2 tig + j] = component (i,k) of block (gid, 2 tig + j): one 16-byte store into block
+                //      row gid; for i != k it is also component (k,i) of block (2 tig + j, gid): two 8-byte stores (the 8
+                //      lanes of equal tig fill 64 contiguous bytes).  Every 32-byte sector is written whole.
+                const int w_el = (tid >> 5) * 4 + el;
+                const bool el_ok = chunk * EL_PER_CTA + w_el < n_elems;
+                const long long sd = __shfl_sync(0xffffffffu, my_slot, el * 8 + gid);
+                const long long st0 = __shfl_sync(0xffffffffu, my_slot, el * 8 + 2 * tig);
+                const long long st1 = __shfl_sync(0xffffffffu, my_slot, el * 8 + 2 * tig + 1);
+                if (el_ok) {
+                    int p = 0;
+#pragma unroll
+                    for (int i = 0; i < 3; i++)
+#pragma unroll
+                        for (int k = i; k < 3; k++, p++) {
+                            *reinterpret_cast<double2 *>(Ke + sd * 72 + (3 * i + k) * 8 + 2 * tig) = make_double2(C[p][0], C[p][1]);
+                            if (i != k) {
+                                Ke[st0 * 72 + (3 * k + i) * 8 + gid] = C[p][0];
+                                Ke[st1 * 72 + (3 * k + i) * 8 + gid] = C[p][1];
+                            }
+                        }
+                }
+            } else {
+                __syncwarp();   // every lane has read this element's G^ and A^: the staging below overlays them
+                // ---- phase 3 (F-bar, coloured mode): stage the full K^e (8 block-row records [I][72], scratch record layout)
                 int p = 0;
 #pragma unroll
                 for (int i = 0; i < 3; i++)
@@ -1020,8 +1043,8 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
             ro[0] = rI[0]; ro[1] = rI[1]; ro[2] = rI[2];
         }
         __syncwarp();
-        // copy-out of the warp's 4 elements x 8 records of 576 bytes, 16 bytes per lane per step (9 steps per element)
-        {
+        // F-bar: copy-out of the warp's 4 elements x 8 staged records of 576 bytes, 16 bytes per lane per step
+        if (FBAR) {
             const int w_el0 = (tid >> 5) * 4;
             const long long e0 = chunk * EL_PER_CTA + w_el0;
 #pragma unroll
@@ -1228,10 +1251,11 @@ int fem_launch_assemble(fem_ctx *c, const double *u, const double *hist_in, cons
         c->n_matd_cap = n_mat;
     }
     static bool attr_set = false;
-    const size_t sm_std = EL_PER_CTA * ES_STD * sizeof(double), sm_fbar = EL_PER_CTA * ES_FBAR * sizeof(double);
+    const size_t sm_std = EL_PER_CTA * ES_STD * sizeof(double), sm_stage = EL_PER_CTA * ES_STAGE * sizeof(double),
+                 sm_fbar = EL_PER_CTA * ES_FBAR * sizeof(double);
     if (!attr_set) {
         FEM_CUDA(cudaFuncSetAttribute(k_element<0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_std));
-        FEM_CUDA(cudaFuncSetAttribute(k_element<0, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_std));
+        FEM_CUDA(cudaFuncSetAttribute(k_element<0, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_stage));
         FEM_CUDA(cudaFuncSetAttribute(k_element<1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_fbar));
         FEM_CUDA(cudaFuncSetAttribute(k_element<1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_fbar));
         attr_set = true;
@@ -1248,7 +1272,7 @@ int fem_launch_assemble(fem_ctx *c, const double *u, const double *hist_in, cons
         // kernel assemble them.  Per call: reset the countdown, the queue (nodes without elements are pre-queued) and its counters.
         static bool attr2 = false;
         if (!attr2) {
-            FEM_CUDA(cudaFuncSetAttribute(k_element<0, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_std));
+            FEM_CUDA(cudaFuncSetAttribute(k_element<0, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_stage));
             FEM_CUDA(cudaFuncSetAttribute(k_element<1, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_fbar));
             FEM_CUDA(cudaFuncSetAttribute(k_gather_drain, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * 2304 * 8));
             attr2 = true;
@@ -1262,7 +1286,7 @@ int fem_launch_assemble(fem_ctx *c, const double *u, const double *hist_in, cons
             k_element<1, 2><<<grid, CTA_THREADS, sm_fbar, st>>>(c->n_elems, c->d_coords, c->d_conn, u, hist_in, c->d_matd, mstride,
                                                         c->opt.tol, c->opt.kmax, c->d_Ke, c->d_Re, hist_out, c->d_stats, sa);
         else
-            k_element<0, 2><<<grid, CTA_THREADS, sm_std, st>>>(c->n_elems, c->d_coords, c->d_conn, u, hist_in, c->d_matd, mstride,
+            k_element<0, 2><<<grid, CTA_THREADS, sm_stage, st>>>(c->n_elems, c->d_coords, c->d_conn, u, hist_in, c->d_matd, mstride,
                                                        c->opt.tol, c->opt.kmax, c->d_Ke, c->d_Re, hist_out, c->d_stats, sa);
         FEM_CUDA(cudaEventRecord(c->ev[2], st));
         int dev = 0, nsm = 148;
@@ -1281,7 +1305,7 @@ int fem_launch_assemble(fem_ctx *c, const double *u, const double *hist_in, cons
                 k_element<1, 1><<<grid, CTA_THREADS, sm_fbar, st>>>(cnt, c->d_coords, c->d_conn, u, hist_in, c->d_matd, mstride, c->opt.tol,
                                                             c->opt.kmax, nullptr, nullptr, hist_out, c->d_stats, sa);
             else
-                k_element<0, 1><<<grid, CTA_THREADS, sm_std, st>>>(cnt, c->d_coords, c->d_conn, u, hist_in, c->d_matd, mstride, c->opt.tol,
+                k_element<0, 1><<<grid, CTA_THREADS, sm_stage, st>>>(cnt, c->d_coords, c->d_conn, u, hist_in, c->d_matd, mstride, c->opt.tol,
                                                            c->opt.kmax, nullptr, nullptr, hist_out, c->d_stats, sa);
         }
         FEM_CUDA(cudaEventRecord(c->ev[2], st));
