@@ -308,6 +308,9 @@ struct scatter_args {
     const int *inc_ptr;
     const unsigned int *kvec;
 };
+#ifndef EL_PERSIST
+#define EL_PERSIST 0   // persistent CTAs with input prefetch measured slower (3.31 vs 3.13 ms): the CTAs of an SM stay in phase
+#endif
 template <int FBAR, int MODE>
 __global__ void __launch_bounds__(CTA_THREADS, FBAR ? CTAS_FBAR : CTAS_STD)
 k_element(long long n_elems, const double *__restrict__ coords, const int *__restrict__ conn,
@@ -342,33 +345,49 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
         }
         chunk = bx - grp;
     }
+    // MODE 0 is persistent: a CTA walks over the chunks blockIdx.x, blockIdx.x + gridDim.x, ... and loads the inputs of its
+    // next chunk while it works on the current one (connectivity at the top of the iteration, nodal data and history just
+    // before the tensor-core phase, where few registers are live), so no warp waits for the conn -> coords/u chain.
+    constexpr bool PERSIST = (MODE == 0) && EL_PERSIST;
+    const long long n_chunks = (n_elems + EL_PER_CTA - 1) / EL_PER_CTA;
+    double *se = sm + el_cta * ES;
+    int nd_n, slot_n = 0;
+    double xn[3], un[3], hn[7];
+    {
+        const long long er = chunk * EL_PER_CTA + el_cta, es = (er < n_elems) ? er : n_elems - 1;
+        const long long e0 = (MODE == 1 && sa.elist) ? (long long)sa.elist[es] : es;
+        nd_n = conn[e0 * 8 + q];
+        if (MODE != 1) slot_n = __ldg(sa.eslot + e0 * 8 + q);
+        const double *hin = hist_in + (e0 * 8 + q) * 7;
+#pragma unroll
+        for (int i = 0; i < 7; i++) hn[i] = __ldg(hin + i);
+#pragma unroll
+        for (int i = 0; i < 3; i++) { xn[i] = coords[3 * (long long)nd_n + i]; un[i] = u[3 * (long long)nd_n + i]; }
+    }
+    for (int j = tid; j < 64; j += CTA_THREADS) s_hist[j] = 0;
+    if (tid == 0) s_done = 0;
+    __syncthreads();
+  for (;;) {
     const long long e_raw = chunk * EL_PER_CTA + el_cta;
     const bool valid = e_raw < n_elems;
     const long long e_slot = valid ? e_raw : n_elems - 1;
     const long long e = (MODE == 1 && sa.elist) ? (long long)sa.elist[e_slot] : e_slot;
-    double *se = sm + el_cta * ES;
-    for (int j = tid; j < 64; j += CTA_THREADS) s_hist[j] = 0;
-    if (tid == 0) s_done = 0;
-    __syncthreads();
-
-    // history loads are issued first: their latency overlaps the geometry and the Jacobi sweeps
+    // ---- S2 gather: thread q holds node q of its element (prefetched), history of its Gauss point
     double epn[6];
-    double alphan;
-    {
-        const double *hin = hist_in + (e * 8 + q) * 7;
 #pragma unroll
-        for (int i = 0; i < 6; i++) epn[i] = __ldg(hin + i);
-        alphan = __ldg(hin + 6);
-    }
-    // ---- S2 gather: thread q loads node q of its element
-    int my_node, my_slot = 0;
-    if (MODE != 1) my_slot = __ldg(sa.eslot + e * 8 + q);
-    {
-        const long long nd = conn[e * 8 + q];
-        my_node = (int)nd;
-        se[SM_XE + 3 * q + 0] = coords[3 * nd + 0]; se[SM_XE + 3 * q + 1] = coords[3 * nd + 1];
-        se[SM_XE + 3 * q + 2] = coords[3 * nd + 2];
-        se[SM_UE + 3 * q + 0] = u[3 * nd + 0]; se[SM_UE + 3 * q + 1] = u[3 * nd + 1]; se[SM_UE + 3 * q + 2] = u[3 * nd + 2];
+    for (int i = 0; i < 6; i++) epn[i] = hn[i];
+    const double alphan = hn[6];
+    const int my_node = nd_n, my_slot = slot_n;
+#pragma unroll
+    for (int i = 0; i < 3; i++) { se[SM_XE + 3 * q + i] = xn[i]; se[SM_UE + 3 * q + i] = un[i]; }
+    const long long chunk_next = chunk + gridDim.x;
+    const bool has_next = PERSIST && chunk_next < n_chunks;
+    long long e_next = 0;
+    if (has_next) {
+        const long long er = chunk_next * EL_PER_CTA + el_cta;
+        e_next = (er < n_elems) ? er : n_elems - 1;
+        nd_n = conn[e_next * 8 + q];
+        slot_n = __ldg(sa.eslot + e_next * 8 + q);
     }
     __syncwarp();
 
@@ -751,21 +770,30 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
     double g_aaa[3], g_aab[3][3], g012;
 #pragma unroll
     for (int a = 0; a < 3; a++) g_aaa[a] = -d1[a] * d1[a];  // -1/(4 lam^2)
-#pragma unroll
-    for (int a = 0; a < 3; a++)
-#pragma unroll
-        for (int b = 0; b < 3; b++) {
-            if (a == b) { g_aab[a][b] = 0.0; continue; }
-            const double gap = lam[a] - lam[b];
-            g_aab[a][b] = (fabs(gap) >= thr) ? (d1[a] - d1[VG[a][b]]) * frcp(gap) : dd2_series(lam[a], lam[a], lam[b]);
-        }
     {
-        const double g01 = fabs(lam[0] - lam[1]), g12 = fabs(lam[1] - lam[2]), g02 = fabs(lam[0] - lam[2]);
+        // recursion on the gaps with one reciprocal per eigenvalue pair (branch-free; a zero gap gives an unselected NaN),
+        // series only where some point of the warp has a gap below the threshold (the nearly undeformed part of the mesh)
+        const double gp01 = lam[0] - lam[1], gp12 = lam[1] - lam[2], gp02 = lam[0] - lam[2];
+        const double i01 = frcp(gp01), i12 = frcp(gp12), i02 = frcp(gp02);
+        g_aab[0][0] = g_aab[1][1] = g_aab[2][2] = 0.0;
+        g_aab[0][1] = (d1[0] - d1[3]) * i01; g_aab[1][0] = (d1[3] - d1[1]) * i01;
+        g_aab[1][2] = (d1[1] - d1[4]) * i12; g_aab[2][1] = (d1[4] - d1[2]) * i12;
+        g_aab[0][2] = (d1[0] - d1[5]) * i02; g_aab[2][0] = (d1[5] - d1[2]) * i02;
+        const double g01 = fabs(gp01), g12 = fabs(gp12), g02 = fabs(gp02);
         const double gmax = fmax(g01, fmax(g12, g02));
-        if (gmax < thr) g012 = dd2_series(lam[0], lam[1], lam[2]);
-        else if (gmax == g01) g012 = (d1[VG[0][2]] - d1[VG[2][1]]) * frcp(lam[0] - lam[1]);   // (g[0,2]-g[2,1])/(l0-l1)
-        else if (gmax == g12) g012 = (d1[VG[1][0]] - d1[VG[0][2]]) * frcp(lam[1] - lam[2]);   // (g[1,0]-g[0,2])/(l1-l2)
-        else                  g012 = (d1[VG[0][1]] - d1[VG[1][2]]) * frcp(lam[0] - lam[2]);   // (g[0,1]-g[1,2])/(l0-l2)
+        // g[0,1,2] by recursion on the widest gap: (g[0,2]-g[2,1])/(l0-l1), (g[1,0]-g[0,2])/(l1-l2), (g[0,1]-g[1,2])/(l0-l2)
+        g012 = (gmax == g01) ? (d1[5] - d1[4]) * i01 : ((gmax == g12) ? (d1[3] - d1[5]) * i12 : (d1[3] - d1[4]) * i02);
+        const bool s01 = g01 < thr, s12 = g12 < thr, s02 = g02 < thr;
+        if (__any_sync(0xffffffffu, s01 || s12 || s02)) {
+            const double t01 = dd2_series(lam[0], lam[0], lam[1]), t10 = dd2_series(lam[1], lam[1], lam[0]);
+            const double t12 = dd2_series(lam[1], lam[1], lam[2]), t21 = dd2_series(lam[2], lam[2], lam[1]);
+            const double t02 = dd2_series(lam[0], lam[0], lam[2]), t20 = dd2_series(lam[2], lam[2], lam[0]);
+            const double t012 = dd2_series(lam[0], lam[1], lam[2]);
+            if (s01) { g_aab[0][1] = t01; g_aab[1][0] = t10; }
+            if (s12) { g_aab[1][2] = t12; g_aab[2][1] = t21; }
+            if (s02) { g_aab[0][2] = t02; g_aab[2][0] = t20; }
+            if (gmax < thr) g012 = t012;
+        }
     }
     // C_L^ = 4 g1_A g1_B C^_AB + Gamma_AB (T:L_L), weighted by the integration weight
     double CL[6][6];
@@ -903,6 +931,13 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
     }
     __syncwarp();
 
+    if (has_next) {   // inputs of the next chunk: in flight during the tensor-core phase
+        const double *hin = hist_in + (e_next * 8 + q) * 7;
+#pragma unroll
+        for (int i = 0; i < 7; i++) hn[i] = __ldg(hin + i);
+#pragma unroll
+        for (int i = 0; i < 3; i++) { xn[i] = coords[3 * (long long)nd_n + i]; un[i] = u[3 * (long long)nd_n + i]; }
+    }
     PHASE_SYNC_N(8);
     // ---- S12 phase 2: K^e_(Ii)(Kk) = sum_q G^_Ia A^_(ia)(kb) G^_Kb (Eq.(37) :267) on the FP64 tensor-core path.
     //      For each component pair (i,k), i <= k, the 8x8 node matrix K^{ik}[I][K] = sum_{(q,a)} G^q_Ia H^{ik}_{(q,a),K} with
@@ -1128,6 +1163,12 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
             if (mf) atomicAdd(&stats[3], (unsigned long long)__popc(mf));
         }
         if (valid && plastic) atomicAdd(&s_hist[iters < 63 ? iters : 63], 1u);
+    }
+    if (!has_next) break;
+    chunk = chunk_next;
+    __syncwarp();   // the next iteration overwrites this warp's shared-memory regions
+  }
+    {
         __syncwarp();
         unsigned done = 0;
         if (lane == 0) { __threadfence_block(); done = atomicAdd(&s_done, 1u); }
@@ -1310,7 +1351,19 @@ int fem_launch_assemble(fem_ctx *c, const double *u, const double *hist_in, cons
         }
         FEM_CUDA(cudaEventRecord(c->ev[2], st));
     } else {
-        const unsigned grid = nblk2(c->n_elems, EL_PER_CTA);
+        // persistent CTAs: one wave (resident CTAs per SM x SMs), each walks over its chunks
+        static int wave[2] = {0, 0};
+        if (!wave[0]) {
+            int dev = 0, nsm = 148, per = 1;
+            cudaGetDevice(&dev);
+            cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+            FEM_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, k_element<0, 0>, CTA_THREADS, sm_std));
+            wave[0] = (per > 0 ? per : 1) * nsm;
+            FEM_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, k_element<1, 0>, CTA_THREADS, sm_fbar));
+            wave[1] = (per > 0 ? per : 1) * nsm;
+        }
+        const unsigned n_chunks = nblk2(c->n_elems, EL_PER_CTA);
+        const unsigned grid = (!EL_PERSIST || n_chunks < (unsigned)wave[c->opt.fbar ? 1 : 0]) ? n_chunks : (unsigned)wave[c->opt.fbar ? 1 : 0];
         if (c->opt.fbar)
             k_element<1, 0><<<grid, CTA_THREADS, sm_fbar, st>>>(c->n_elems, c->d_coords, c->d_conn, u, hist_in, c->d_matd, mstride,
                                                         c->opt.tol, c->opt.kmax, c->d_Ke, c->d_Re, hist_out, c->d_stats, sa);
