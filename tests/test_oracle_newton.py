@@ -1,0 +1,125 @@
+"""Pins of oracle/newton.py against what mechanics and linear algebra fix, not against itself:
+dense brute force for the Dirichlet rows and y = K x, the homogeneous-deformation patch solution, the Hencky uniaxial
+closed form, the Lankford ratio of the plastic lateral strains, and quadratic convergence of the global Newton loop."""
+import numpy as np
+import pytest
+
+import oracle
+import oracle.newton as onw
+import synth
+from synth import mesh
+
+
+def _problem(nx, ny, nz, L=(1.0, 1.0, 1.0), desc=None):
+    coords, conn = mesh.structured_hex_mesh(nx, ny, nz, *L)
+    ne = conn.shape[0]
+    mat = oracle.mat_from_desc(dict(synth.configs.SWIFT) if desc is None else desc, ne)
+    row_ptr, col_idx, _ = oracle.pattern(coords.shape[0], conn, with_slots=False)
+    return coords, conn, mat, row_ptr, col_idx, np.zeros((ne, 8, 7))
+
+
+def _dense(row_ptr, col_idx, vals):
+    n = len(row_ptr) - 1
+    K = np.zeros((n, n))
+    for r in range(n):
+        for j in range(row_ptr[r], row_ptr[r + 1]):
+            K[r, col_idx[j]] += vals[j]
+    return K
+
+
+def test_spmv_and_dirichlet_against_dense_brute_force():
+    coords, conn, mat, rp, ci, h0 = _problem(2, 2, 1)
+    rng = np.random.default_rng(3)
+    u = 1e-3 * rng.normal(size=coords.shape)
+    out = oracle.assemble(coords, conn, u, h0, mat, rp, ci)
+    K = _dense(rp, ci, out["csr_vals"])
+    x = rng.normal(size=K.shape[0])
+    assert np.allclose(onw.spmv(rp, ci, out["csr_vals"], x), K @ x, rtol=1e-13, atol=1e-9)
+    bc = np.array([0, 4, 5, 17, 26])
+    g = rng.normal(size=bc.size)
+    vals, rhs = onw.dirichlet(rp, ci, out["csr_vals"], -out["residual"], bc, g)
+    Kd = K.copy()
+    Kd[bc, :] = 0.0
+    Kd[bc, bc] = 1.0
+    assert np.array_equal(_dense(rp, ci, vals), Kd)           # rows replaced, columns untouched
+    r2 = -out["residual"].copy(); r2[bc] = g
+    assert np.array_equal(rhs, r2)
+    xs = onw.linear_solve(rp, ci, vals, rhs)
+    assert np.allclose(xs, np.linalg.solve(Kd, r2), rtol=1e-9, atol=1e-14)
+    assert np.allclose(xs[bc], g, rtol=1e-12, atol=0)            # identity rows pin the constrained values
+
+
+def test_patch_solution_homogeneous_deformation():
+    """All boundary nodes follow u = A X; the homogeneous field is the exact discrete solution for a homogeneous material,
+    elastic or plastic, so Newton from a zero interior guess must return A X at the interior nodes."""
+    coords, conn, mat, rp, ci, h0 = _problem(3, 3, 3)
+    A = np.array([[0.02, 0.01, -0.004], [0.003, -0.012, 0.006], [-0.005, 0.002, 0.015]])
+    exact = coords @ A.T
+    on_b = np.any((np.abs(coords) < 1e-12) | (np.abs(coords - 1.0) < 1e-12), axis=1)
+    bc = (3 * np.flatnonzero(on_b)[:, None] + np.arange(3)).ravel()
+    res = onw.newton_solve(coords, conn, np.zeros_like(coords), h0, mat, rp, ci, bc, exact.ravel()[bc])
+    assert res["converged"] and res["stats"]["n_plastic"] == 8 * conn.shape[0]
+    assert np.abs(res["u"] - exact).max() < 1e-10
+
+
+def _uniaxial(delta, desc=None):
+    coords, conn, mat, rp, ci, h0 = _problem(2, 2, 2, desc=desc)
+    nid = np.arange(coords.shape[0])
+    bc, val = [], []
+    for sel, comp, v in ((np.abs(coords[:, 0]) < 1e-12, 0, 0.0), (np.abs(coords[:, 0] - 1) < 1e-12, 0, delta),
+                         (np.abs(coords[:, 1]) < 1e-12, 1, 0.0), (np.abs(coords[:, 2]) < 1e-12, 2, 0.0)):
+        bc += list(3 * nid[sel] + comp); val += [v] * int(sel.sum())
+    res = onw.newton_solve(coords, conn, np.zeros_like(coords), h0, mat, rp, ci, np.array(bc), np.array(val))
+    assert res["converged"]
+    u = res["u"]
+    top_y, top_z = np.abs(coords[:, 1] - 1) < 1e-12, np.abs(coords[:, 2] - 1) < 1e-12
+    return res, np.log1p(delta), np.log1p(u[top_y, 1]), np.log1p(u[top_z, 2])
+
+
+def test_hencky_uniaxial_elastic_closed_form():
+    """Below yield T = E : ln U, so free lateral faces give ln(lambda_lat) = -nu ln(lambda_ax) exactly (Eq.(7)-(8) :108-113)."""
+    res, e_ax, e_y, e_z = _uniaxial(5e-4)
+    assert res["stats"]["n_plastic"] == 0
+    assert np.allclose(e_y, -0.33 * e_ax, rtol=1e-9) and np.allclose(e_z, -0.33 * e_ax, rtol=1e-9)
+
+
+def test_plastic_uniaxial_lateral_strains_follow_lankford_r0():
+    """Uniaxial tension along material axis 1 beyond yield: the plastic width / thickness strain ratio is the Lankford
+    value r0 that produced the Hill ratios (associative flow Eq.(13) :141 + the Lankford conversion, D2)."""
+    res, e_ax, e_y, e_z = _uniaxial(0.03)
+    assert res["stats"]["n_plastic"] == 64
+    h = res["hist_out"].reshape(-1, 7)
+    ep = h.mean(axis=0)
+    assert np.ptp(h[:, 0]) < 1e-10                                   # homogeneous state
+    assert abs(ep[1] / ep[2] - 0.7) < 1e-9                           # eps_p22 / eps_p33 = r0
+    sig = 70000.0 * (e_ax - ep[0])                                   # uniaxial stress from the elastic axial log strain
+    assert np.allclose(e_y, -0.33 * sig / 70000.0 + ep[1], rtol=1e-8)
+    assert np.allclose(e_z, -0.33 * sig / 70000.0 + ep[2], rtol=1e-8)
+    # Swift flow stress reached: sigma11 = r11 * sigma_flow(alpha) with r11 = 1 (G2)
+    assert abs(sig - 500.0 * (0.01 + h[0, 6]) ** 0.2) < 1e-6 * sig
+
+
+def clamped_shear_problem():
+    """3^3 cube, face x = 0 clamped, face x = 1 displaced by (0.02, 0.01, 0): the paper's benchmark loading (PAPER.md:485,
+    left face fixed, right face moved in x and y), inhomogeneous and fully plastic."""
+    coords, conn, mat, rp, ci, h0 = _problem(3, 3, 3)
+    nid = np.arange(coords.shape[0])
+    lf, rt = np.abs(coords[:, 0]) < 1e-12, np.abs(coords[:, 0] - 1) < 1e-12
+    bc = np.concatenate([(3 * nid[lf][:, None] + np.arange(3)).ravel(), (3 * nid[rt][:, None] + np.arange(3)).ravel()])
+    val = np.concatenate([np.zeros(3 * lf.sum()), np.tile([0.02, 0.01, 0.0], rt.sum())])
+    return coords, conn, mat, rp, ci, h0, bc, val
+
+
+def test_global_newton_converges_quadratically():
+    """With the consistent tangent (Eq.(40) :294) the residual norm squares from one iteration to the next once it is small."""
+    coords, conn, mat, rp, ci, h0, bc, val = clamped_shear_problem()
+    res = onw.newton_solve(coords, conn, np.zeros_like(coords), h0, mat, rp, ci, bc, val)
+    n = res["norms"]
+    assert res["converged"] and res["stats"]["n_plastic"] > 0.9 * 8 * conn.shape[0]
+    k = next(i for i in range(1, len(n)) if n[i] < 1e-2)
+    assert n[k + 1] < 1e-4 * n[k], n
+    # equilibrium: the internal force of the returned state vanishes on the free DOFs
+    out = oracle.assemble(coords, conn, res["u"], h0, mat, rp, ci)
+    free = np.setdiff1d(np.arange(3 * coords.shape[0]), bc)
+    assert np.abs(out["residual"][free]).max() < 1e-9 * np.abs(out["residual"][bc]).max()
+    assert np.allclose(res["u"].ravel()[bc], val, rtol=0, atol=1e-15)
