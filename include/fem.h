@@ -37,7 +37,8 @@ enum {
     FEM_ERR_NO_PATTERN = -7,  /* fem_assemble before fem_build_csr_pattern */
     FEM_ERR_DEGREE = -8,      /* a node belongs to more than FEM_MAX_NODE_ELEMS elements */
     FEM_ERR_ALIAS = -9,       /* hist_out aliases hist_in */
-    FEM_ERR_MAT = -10         /* n_mat is neither 1 nor n_elems */
+    FEM_ERR_MAT = -10,        /* n_mat is neither 1 nor n_elems */
+    FEM_ERR_NOCONV = -11      /* iterative solve (fem_bicgstab, fem_newton_solve) did not converge */
 };
 #define FEM_MAX_NODE_ELEMS 32
 
@@ -136,6 +137,68 @@ const char *fem_last_cuda_error(void);
 /* Host helper: Lankford r0, r45, r90 -> the paper's yield-stress ratios (r11,r22,r33,r12,r23,r13) of Eq.(A3)-(A5)
  * (textbook Hill-1948 plane-stress relations, axis 1 = rolling direction, sigma11^y = sigma0; reading D2). */
 int fem_hill_from_lankford(double r0, double r45, double r90, double r_out[6] /*host*/);
+
+/* ------------------------------------------------------------------------------------------------------------------
+ * the steps on either side of fem_assemble in one global Newton iteration
+ * K dd = -R (Eq.(39)): Dirichlet rows (Alg. E1 steps 6-11 :1048-1053), a linear solve on
+ * the library's own CSR (the paper's default Krylov method is BiCGSTAB, :304; AMGX / cuDSS themselves are out of scope)
+ * and the Newton loop of one load increment.  All arrays are dev pointers on the pattern of fem_build_csr_pattern.
+ * ------------------------------------------------------------------------------------------------------------------ */
+
+/* y = K x with K = (pattern of this context, csr_vals).  x, y dev [n_rows], must not alias.  Deterministic
+ * (fixed reduction order).  Uses the block structure of the pattern (one warp per node, three rows at a time). */
+int fem_spmv(fem_ctx *c, const double *csr_vals /*dev [nnz]*/, const double *x, double *y, void *cuda_stream);
+
+/* Dirichlet rows, Alg. E1 steps 6-11 ("zero off-diagonal entries and reset the diagonal to unity",
+ * :298): for every listed DOF d the row d of K becomes the identity row and rhs[d] = bc_rhs[i] (0 when bc_rhs is NULL).
+ * Columns are left alone, as in the paper (K becomes unsymmetric).  One thread per constrained row.
+ *   bc_dofs dev [n_bc] int32, each in [0, n_rows), no duplicates required (duplicates write the same values)
+ *   bc_rhs  dev [n_bc] or NULL        csr_vals dev [nnz] in/out        rhs dev [n_rows] in/out, may be NULL */
+int fem_apply_dirichlet(fem_ctx *c, long long n_bc, const int *bc_dofs, const double *bc_rhs, double *csr_vals,
+                        double *rhs, void *cuda_stream);
+
+/* Jacobi-preconditioned BiCGSTAB (van der Vorst 1992; right preconditioning with M = diag K) for K x = b.
+ *   x dev [n_rows]: initial guess on entry, solution on exit        b dev [n_rows]
+ *   stops when ||b - K x||_2 <= rtol * ||b||_2 (recurrence residual, confirmed by one explicit residual at the end)
+ *   or after max_iter iterations.  On breakdown ((rhat, r), (rhat, v) or omega collapses) the iteration restarts from the
+ *   explicit residual of the current x (at most 50 times).
+ *   *iters (host, may be NULL) = iterations used; *relres (host, may be NULL) = explicit ||b - K x|| / ||b|| at exit.
+ * Returns FEM_OK when converged, FEM_ERR_NOCONV otherwise (x holds the last iterate).  Dot products are reduced in a
+ * fixed order: two calls with equal inputs give bit-identical results.  Synchronises the stream (scalars go through the host). */
+int fem_bicgstab(fem_ctx *c, const double *csr_vals, const double *b, double *x, double rtol, int max_iter, int *iters,
+                 double *relres, void *cuda_stream);
+
+typedef struct {
+    double rtol;      /* Newton stops when ||rhs||_2 <= rtol * ||rhs of iteration 0||_2 ... */
+    double atol;      /* ... or <= atol (rhs = -R on free DOFs, prescribed - current on constrained DOFs); defaults 1e-9, 1e-10 */
+    int max_newton;   /* default 25 */
+    double lin_rtol;  /* BiCGSTAB tolerance per Newton iteration, default 1e-10 */
+    int lin_max_iter; /* default 10000 */
+} fem_newton_options;
+
+typedef struct {
+    int newton_iters;        /* assemble + solve + update cycles performed */
+    int converged;           /* 1 when a residual test passed */
+    int lin_iters_total;     /* BiCGSTAB iterations over all Newton iterations */
+    int lin_failures;        /* linear solves that returned FEM_ERR_NOCONV (the update is applied anyway) */
+    double rhs_norm0, rhs_norm; /* first and last ||rhs||_2 */
+    fem_stats last_stats;    /* statistics of the last fem_assemble */
+} fem_newton_report;
+
+void fem_default_newton_options(fem_newton_options *o /*host*/);
+
+/* One load increment: global Newton-Raphson K dd = -R, d <- d + dd (Eq.(39)) with Dirichlet data.
+ *   u        dev [n_rows] in/out: initial guess (e.g. the last converged state) -> converged displacement
+ *   hist_in  dev [n_elems*56] history at the start of the increment (unchanged)
+ *   hist_out dev [n_elems*56] history at the returned u (from the last fem_assemble)
+ *   bc_dofs  dev [n_bc] constrained DOFs, bc_vals dev [n_bc] their prescribed TOTAL displacement
+ * Each iteration: fem_assemble(u) -> rhs = -R -> constrained rows: identity, rhs = bc_vals - u (so the update lands on
+ * the prescribed value) -> test ||rhs|| -> fem_bicgstab from a zero guess -> u += dd.  The stiffness matrix, residual and
+ * Krylov vectors live in library-owned workspace (allocated on first use).  Returns FEM_OK when converged,
+ * FEM_ERR_NOCONV when max_newton is reached; *rep (host, may be NULL) is always filled.  Synchronises the stream. */
+int fem_newton_solve(fem_ctx *c, double *u, const double *hist_in, const double *mat, long long n_mat, long long n_bc,
+                     const int *bc_dofs, const double *bc_vals, double *hist_out, const fem_newton_options *opt,
+                     fem_newton_report *rep, void *cuda_stream);
 
 #ifdef __cplusplus
 }

@@ -4,5 +4,5 @@ Every step of the path runs in the CUDA kernels of csrc/; this module only marsh
 (torch tensors -> device pointers, the current torch stream -> cuda_stream).  There is no CPU fallback:
 if the shared library is missing, or no CUDA device is visible, calls raise.
 """
-from .binding import (FemContext, FemError, FemOptions, FemStats, NPAR, hill_from_lankford, lib, lib_path,  # noqa: F401
+from .binding import (FemContext, FemError, FemOptions, FemStats, FemNewtonOptions, FemNewtonReport, NPAR, hill_from_lankford, lib, lib_path,  # noqa: F401
                       mat_from_desc, mat_record, probe_fp64_peak, ABI_SYMBOLS)

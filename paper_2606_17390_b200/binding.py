@@ -9,7 +9,8 @@ NPAR = 16
 
 ABI_SYMBOLS = ["fem_default_options", "fem_setup", "fem_build_csr_pattern", "fem_assemble", "fem_assemble_host",
                "fem_last_kernel_ms", "fem_launches_per_assemble", "fem_probe_fp64_peak", "fem_destroy", "fem_strerror",
-               "fem_last_cuda_error", "fem_hill_from_lankford"]
+               "fem_last_cuda_error", "fem_hill_from_lankford", "fem_spmv", "fem_apply_dirichlet", "fem_bicgstab",
+               "fem_default_newton_options", "fem_newton_solve"]
 
 
 class FemOptions(C.Structure):
@@ -24,6 +25,21 @@ class FemStats(C.Structure):
     def as_dict(self):
         return dict(n_plastic=self.n_plastic, n_nonconverged=self.n_nonconverged, n_detF_nonpos=self.n_detF_nonpos,
                     n_nonfinite=self.n_nonfinite, max_local_iters=self.max_local_iters, iter_hist=list(self.iter_hist))
+
+
+class FemNewtonOptions(C.Structure):
+    _fields_ = [("rtol", C.c_double), ("atol", C.c_double), ("max_newton", C.c_int), ("lin_rtol", C.c_double),
+                ("lin_max_iter", C.c_int)]
+
+
+class FemNewtonReport(C.Structure):
+    _fields_ = [("newton_iters", C.c_int), ("converged", C.c_int), ("lin_iters_total", C.c_int), ("lin_failures", C.c_int),
+                ("rhs_norm0", C.c_double), ("rhs_norm", C.c_double), ("last_stats", FemStats)]
+
+    def as_dict(self):
+        return dict(newton_iters=self.newton_iters, converged=bool(self.converged), lin_iters_total=self.lin_iters_total,
+                    lin_failures=self.lin_failures, rhs_norm0=self.rhs_norm0, rhs_norm=self.rhs_norm,
+                    last_stats=self.last_stats.as_dict())
 
 
 class FemError(RuntimeError):
@@ -73,6 +89,13 @@ def lib():
         L.fem_strerror.restype = C.c_char_p
         L.fem_last_cuda_error.restype = C.c_char_p
         L.fem_hill_from_lankford.argtypes = [C.c_double] * 3 + [dp]
+        L.fem_spmv.argtypes = [vp, vp, vp, vp, vp]
+        L.fem_apply_dirichlet.argtypes = [vp, ll, vp, vp, vp, vp, vp]
+        L.fem_bicgstab.argtypes = [vp, vp, vp, vp, C.c_double, C.c_int, C.POINTER(C.c_int), dp, vp]
+        L.fem_default_newton_options.argtypes = [C.POINTER(FemNewtonOptions)]
+        L.fem_default_newton_options.restype = None
+        L.fem_newton_solve.argtypes = [vp, vp, vp, vp, ll, ll, vp, vp, vp, C.POINTER(FemNewtonOptions),
+                                       C.POINTER(FemNewtonReport), vp]
         _lib = L
     return _lib
 
@@ -208,6 +231,60 @@ class FemContext:
                                        hp(csr_vals, self.nnz, "csr_vals"), hp(hist_out, 56 * self.n_elems, "hist_out"),
                                        C.byref(st) if want_stats else None), "fem_assemble_host")
         return st.as_dict() if want_stats else None
+
+    def spmv(self, csr_vals, x, y=None):
+        """fem_spmv: y = K x on the context's pattern."""
+        torch = _torch()
+        if y is None:
+            y = torch.empty(self.n_rows, dtype=torch.float64, device=self.device)
+        _check(lib().fem_spmv(self._h, _ptr(csr_vals, torch.float64, self.nnz, "csr_vals"), _ptr(x, torch.float64, self.n_rows, "x"),
+                              _ptr(y, torch.float64, self.n_rows, "y"), _stream_ptr()), "fem_spmv")
+        return y
+
+    def apply_dirichlet(self, bc_dofs, csr_vals, rhs=None, bc_rhs=None):
+        """fem_apply_dirichlet: identity rows for bc_dofs (int32 CUDA tensor), rhs[d] = bc_rhs (0 if None).  In place."""
+        torch = _torch()
+        nbc = bc_dofs.numel()
+        _check(lib().fem_apply_dirichlet(self._h, nbc, _ptr(bc_dofs, torch.int32, None, "bc_dofs"),
+                                         None if bc_rhs is None else _ptr(bc_rhs, torch.float64, nbc, "bc_rhs"),
+                                         _ptr(csr_vals, torch.float64, self.nnz, "csr_vals"),
+                                         None if rhs is None else _ptr(rhs, torch.float64, self.n_rows, "rhs"), _stream_ptr()),
+               "fem_apply_dirichlet")
+
+    def bicgstab(self, csr_vals, b, x=None, rtol=1e-10, max_iter=10000):
+        """fem_bicgstab: returns (x, iters, relres, converged)."""
+        torch = _torch()
+        if x is None:
+            x = torch.zeros(self.n_rows, dtype=torch.float64, device=self.device)
+        it, rr = C.c_int(0), C.c_double(0.0)
+        rc = lib().fem_bicgstab(self._h, _ptr(csr_vals, torch.float64, self.nnz, "csr_vals"), _ptr(b, torch.float64, self.n_rows, "b"),
+                                _ptr(x, torch.float64, self.n_rows, "x"), float(rtol), int(max_iter), C.byref(it), C.byref(rr),
+                                _stream_ptr())
+        if rc not in (0, -11):
+            _check(rc, "fem_bicgstab")
+        return x, it.value, rr.value, rc == 0
+
+    def newton_solve(self, u, hist_in, mat, bc_dofs, bc_vals, hist_out=None, rtol=None, atol=None, max_newton=None,
+                     lin_rtol=None, lin_max_iter=None):
+        """fem_newton_solve: one load increment; u is updated in place.  Returns (u, hist_out, report dict)."""
+        torch = _torch()
+        f64 = torch.float64
+        if hist_out is None:
+            hist_out = torch.empty(self.n_elems * 56, dtype=f64, device=self.device)
+        opt = FemNewtonOptions()
+        lib().fem_default_newton_options(C.byref(opt))
+        for k, v in (("rtol", rtol), ("atol", atol), ("max_newton", max_newton), ("lin_rtol", lin_rtol), ("lin_max_iter", lin_max_iter)):
+            if v is not None:
+                setattr(opt, k, v)
+        rep = FemNewtonReport()
+        nbc = bc_dofs.numel()
+        rc = lib().fem_newton_solve(self._h, _ptr(u, f64, self.n_rows, "u"), _ptr(hist_in, f64, 56 * self.n_elems, "hist_in"),
+                                    _ptr(mat, f64, None, "mat"), mat.numel() // NPAR, nbc, _ptr(bc_dofs, torch.int32, None, "bc_dofs"),
+                                    _ptr(bc_vals, f64, nbc, "bc_vals"), _ptr(hist_out, f64, 56 * self.n_elems, "hist_out"),
+                                    C.byref(opt), C.byref(rep), _stream_ptr())
+        if rc not in (0, -11):
+            _check(rc, "fem_newton_solve")
+        return u, hist_out, rep.as_dict()
 
     def last_kernel_ms(self):
         ms = (C.c_double * 3)()

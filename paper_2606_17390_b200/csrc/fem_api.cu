@@ -2,7 +2,7 @@
 #include "fem_internal.h"
 #include <string.h>
 
-static int read_stats(fem_ctx *c, fem_stats *stats, cudaStream_t st) {
+int fem_read_stats(fem_ctx *c, fem_stats *stats, cudaStream_t st) {
     unsigned long long h[72];
     FEM_CUDA(cudaMemcpyAsync(h, c->d_stats, sizeof(h), cudaMemcpyDeviceToHost, st));
     FEM_CUDA(cudaStreamSynchronize(st));
@@ -31,7 +31,7 @@ extern "C" int fem_assemble(fem_ctx *c, const double *u, const double *hist_in, 
     cudaStream_t st = (cudaStream_t)cuda_stream;
     int rc = fem_launch_assemble(c, u, hist_in, mat, n_mat, residual, csr_vals, hist_out, st);
     if (rc != FEM_OK) return rc;
-    if (stats) return read_stats(c, stats, st);
+    if (stats) return fem_read_stats(c, stats, st);
     return FEM_OK;
 }
 
@@ -63,7 +63,7 @@ extern "C" int fem_assemble_host(fem_ctx *c, const double *u, const double *hist
     FEM_CUDA(cudaMemcpyAsync(residual, c->d_res, sizeof(double) * nr, cudaMemcpyDeviceToHost, st));
     FEM_CUDA(cudaMemcpyAsync(csr_vals, c->d_vals, sizeof(double) * nz, cudaMemcpyDeviceToHost, st));
     FEM_CUDA(cudaMemcpyAsync(hist_out, c->d_hout, sizeof(double) * nh, cudaMemcpyDeviceToHost, st));
-    if (stats) return read_stats(c, stats, st);
+    if (stats) return fem_read_stats(c, stats, st);
     FEM_CUDA(cudaStreamSynchronize(st));
     return FEM_OK;
 }

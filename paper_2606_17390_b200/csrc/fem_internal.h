@@ -46,6 +46,14 @@ struct fem_ctx {
     double *d_matd = nullptr;    // [n_mat_cap*FEM_MATD]
     long long n_matd_cap = 0;
     unsigned long long *d_stats = nullptr;  // [4 + 1 + 64] counters
+    // NEXT-1 (fem_solve.cu): Dirichlet rows, SpMV, BiCGSTAB, Newton loop -- workspace allocated on first use
+    int *d_diagpos = nullptr;      // [n_nodes] position of node n in its own neighbour list (diagonal block)
+    double *d_sw = nullptr;        // [9*n_rows] Krylov vectors r, rhat, p, v, s, t, y, z and the inverse diagonal
+    double *d_part = nullptr;      // partial sums of the deterministic reductions
+    double *d_scal = nullptr;      // [8] reduced scalars
+    double *d_nw = nullptr;        // [3*n_rows] Newton workspace: residual, rhs, dd
+    double *d_nw_vals = nullptr;   // [nnz] Newton workspace: stiffness values
+    long long n_part = 0;
     // host-buffer path
     double *d_u = nullptr, *d_hin = nullptr, *d_hout = nullptr, *d_mat = nullptr, *d_res = nullptr, *d_vals = nullptr;
     long long n_mat_host_cap = 0;
@@ -61,6 +69,8 @@ int fem_cuda_fail(cudaError_t e, const char *where);
         if (_e != cudaSuccess) return fem_cuda_fail(_e, #call);          \
     } while (0)
 
+// fem_api.cu
+int fem_read_stats(fem_ctx *c, fem_stats *stats, cudaStream_t st);
 // fem_colour.cu
 int fem_build_colouring(fem_ctx *c);
 // fem_assemble.cu

@@ -1,0 +1,434 @@
+// the steps on either side of fem_assemble in one global Newton iteration K dd = -R
+// (Eq.(39)): Dirichlet rows (Alg. E1 steps 6-11 :1048-1053), y = K x on the library's
+// own block-structured CSR, Jacobi-preconditioned BiCGSTAB (the paper's default Krylov method, :304) and the Newton loop
+// of one load increment.  Every reduction has a fixed order (per-CTA partial sums, one final CTA): results are
+// bit-identical run to run.  Nothing here is shared with oracle/.
+#include "fem_internal.h"
+#include <math.h>
+#include <string.h>
+
+#define RED_CTAS 1184      // 148 SMs x 8 CTAs of 256 threads for the vector kernels (fixed: part of the reduction order)
+#define RED_THREADS 256
+
+static inline unsigned nblk3(long long n, int bs) { return (unsigned)((n + bs - 1) / bs); }
+
+// ------------------------------------------------------------------------------------------------ small kernels
+__global__ void k_diagpos(long long n_nodes, const int *__restrict__ nb_ptr, const int *__restrict__ nb, int *diagpos) {
+    long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (n >= n_nodes) return;
+    const int o = nb_ptr[n], len = nb_ptr[n + 1] - o;
+    int lo = 0, hi = len - 1;
+    while (lo < hi) { int mid = (lo + hi) >> 1; if (nb[o + mid] < (int)n) lo = mid + 1; else hi = mid; }
+    diagpos[n] = (len > 0 && nb[o + lo] == (int)n) ? lo : -1;   // -1: node without elements (empty rows)
+}
+
+// Alg. E1 step 10: "Enforce identity rows with one CUDA thread per row".  rhs[d] = bc_rhs[i], or
+// bc_vals[i] - u[d] inside the Newton loop (the update then lands on the prescribed value).
+__global__ void k_dirichlet(long long n_bc, const int *__restrict__ bc_dofs, const double *__restrict__ bc_rhs,
+                            const double *__restrict__ bc_vals, const double *__restrict__ u, const int *__restrict__ nb_ptr,
+                            const int *__restrict__ diagpos, double *__restrict__ vals, double *__restrict__ rhs) {
+    long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (t >= n_bc) return;
+    const int d = bc_dofs[t], n = d / 3, i = d - 3 * n;
+    const int o = nb_ptr[n], len = nb_ptr[n + 1] - o, dp = diagpos[n];
+    double *row = vals + 9LL * o + (long long)i * 3 * len;
+    for (int j = 0; j < 3 * len; j++) row[j] = 0.0;
+    if (dp >= 0) row[3 * dp + i] = 1.0;
+    if (rhs) rhs[d] = bc_vals ? bc_vals[t] - u[d] : (bc_rhs ? bc_rhs[t] : 0.0);
+}
+
+__global__ void k_check_dofs(long long n_bc, const int *__restrict__ bc_dofs, long long n_rows, int *flag) {
+    long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (t < n_bc && (bc_dofs[t] < 0 || bc_dofs[t] >= n_rows)) atomicOr(flag, 1);
+}
+
+// inverse diagonal of K (Jacobi preconditioner); a zero or missing diagonal entry counts as 1
+__global__ void k_dinv(long long n_nodes, const int *__restrict__ nb_ptr, const int *__restrict__ diagpos,
+                       const double *__restrict__ vals, double *__restrict__ dinv) {
+    long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (t >= 3 * n_nodes) return;
+    const long long n = t / 3;
+    const int i = (int)(t - 3 * n), o = nb_ptr[n], len = nb_ptr[n + 1] - o, dp = diagpos[n];
+    double dgl = (dp >= 0) ? vals[9LL * o + (long long)i * 3 * len + 3 * dp + i] : 1.0;
+    dinv[t] = (dgl != 0.0 && isfinite(dgl)) ? 1.0 / dgl : 1.0;
+}
+
+// ------------------------------------------------------------------------------------------------ reductions
+// CTA-wide sum of NV values per thread in a fixed order (warp xor-tree, then warps in ascending order); thread 0 returns it.
+template <int NV>
+__device__ __forceinline__ void cta_reduce(double (&v)[NV], double *smem /*[NV*32]*/) {
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = blockDim.x >> 5;
+#pragma unroll
+    for (int k = 0; k < NV; k++)
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v[k] += __shfl_xor_sync(0xffffffffu, v[k], o);
+    if (lane == 0)
+#pragma unroll
+        for (int k = 0; k < NV; k++) smem[k * 32 + w] = v[k];
+    __syncthreads();
+    if (threadIdx.x == 0)
+#pragma unroll
+        for (int k = 0; k < NV; k++) {
+            double s = 0.0;
+            for (int j = 0; j < nw; j++) s += smem[k * 32 + j];
+            v[k] = s;
+        }
+}
+// final stage: one CTA sums `count` partial records of NV values each (record-major) into out[0..NV)
+template <int NV>
+__global__ void __launch_bounds__(1024) k_reduce_final(const double *__restrict__ part, long long count, double *out) {
+    __shared__ double smem[NV * 32];
+    double v[NV];
+#pragma unroll
+    for (int k = 0; k < NV; k++) v[k] = 0.0;
+    for (long long j = threadIdx.x; j < count; j += blockDim.x)
+#pragma unroll
+        for (int k = 0; k < NV; k++) v[k] += part[j * NV + k];
+    cta_reduce<NV>(v, smem);
+    if (threadIdx.x == 0)
+#pragma unroll
+        for (int k = 0; k < NV; k++) out[k] = v[k];
+}
+
+// ------------------------------------------------------------------------------------------------ SpMV
+// y = K x on the block structure of the pattern: one warp per node n, lane = neighbour position; row 3n+i holds the
+// entries [pos][k] contiguously, so a lane reads 3 x 24 bytes of values, one block-column index (nb, 4 bytes per 3x3
+// block instead of col_idx's 36) and 3 entries of x.  DOT = 1: partial sums of (w, y); DOT = 2: of (y, w) and (y, y).
+template <int DOT>
+__global__ void __launch_bounds__(256)
+k_spmv(long long n_nodes, const int *__restrict__ nb_ptr, const int *__restrict__ nb, const double *__restrict__ vals,
+       const double *__restrict__ x, double *__restrict__ y, const double *__restrict__ w, double *__restrict__ part) {
+    __shared__ double smem[2 * 32];
+    const long long n = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    double a0 = 0.0, a1 = 0.0, a2 = 0.0;
+    if (n < n_nodes) {
+        const int o = nb_ptr[n], len = nb_ptr[n + 1] - o;
+        const double *base = vals + 9LL * o;
+        for (int pos = lane; pos < len; pos += 32) {
+            const long long m = nb[o + pos];
+            const double x0 = x[3 * m], x1 = x[3 * m + 1], x2 = x[3 * m + 2];
+            const double *r0 = base + 3 * pos, *r1 = r0 + 3 * len, *r2 = r1 + 3 * len;
+            a0 = fma(r0[2], x2, fma(r0[1], x1, fma(r0[0], x0, a0)));
+            a1 = fma(r1[2], x2, fma(r1[1], x1, fma(r1[0], x0, a1)));
+            a2 = fma(r2[2], x2, fma(r2[1], x1, fma(r2[0], x0, a2)));
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        a0 += __shfl_xor_sync(0xffffffffu, a0, o); a1 += __shfl_xor_sync(0xffffffffu, a1, o); a2 += __shfl_xor_sync(0xffffffffu, a2, o);
+    }
+    double d[2] = {0.0, 0.0};
+    if (n < n_nodes && lane == 0) {
+        y[3 * n] = a0; y[3 * n + 1] = a1; y[3 * n + 2] = a2;
+        if (DOT) {
+            const double w0 = w[3 * n], w1 = w[3 * n + 1], w2 = w[3 * n + 2];
+            d[0] = a0 * w0 + a1 * w1 + a2 * w2;
+            d[1] = a0 * a0 + a1 * a1 + a2 * a2;
+        }
+    }
+    if (DOT) {   // lane 0 of each warp holds the node's contribution; warps summed in ascending order
+        const int wi = threadIdx.x >> 5;
+        if (lane == 0) { smem[wi] = d[0]; smem[32 + wi] = d[1]; }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            double s0 = 0.0, s1 = 0.0;
+            for (int j = 0; j < (int)(blockDim.x >> 5); j++) { s0 += smem[j]; s1 += smem[32 + j]; }
+            part[2LL * blockIdx.x] = s0; part[2LL * blockIdx.x + 1] = s1;
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ BiCGSTAB vector kernels
+// r = b - r (r holds K x on entry), rhat = r, p = v = 0 ; partials: (r, r), (b, b)
+__global__ void __launch_bounds__(RED_THREADS)
+k_bicg_init(long long n, const double *__restrict__ b, double *__restrict__ r, double *__restrict__ rhat, double *__restrict__ p,
+            double *__restrict__ v, double *__restrict__ part) {
+    __shared__ double smem[2 * 32];
+    double s[2] = {0.0, 0.0};
+    for (long long j = blockIdx.x * (long long)blockDim.x + threadIdx.x; j < n; j += (long long)gridDim.x * blockDim.x) {
+        const double bj = b[j], rj = bj - r[j];
+        r[j] = rj; rhat[j] = rj; p[j] = 0.0; v[j] = 0.0;
+        s[0] = fma(rj, rj, s[0]); s[1] = fma(bj, bj, s[1]);
+    }
+    cta_reduce<2>(s, smem);
+    if (threadIdx.x == 0) { part[2LL * blockIdx.x] = s[0]; part[2LL * blockIdx.x + 1] = s[1]; }
+}
+// p = r + beta (p - omega v) ; y = M^-1 p
+__global__ void __launch_bounds__(RED_THREADS)
+k_bicg_p(long long n, double beta, double omega, const double *__restrict__ r, const double *__restrict__ v,
+         const double *__restrict__ dinv, double *__restrict__ p, double *__restrict__ y) {
+    for (long long j = blockIdx.x * (long long)blockDim.x + threadIdx.x; j < n; j += (long long)gridDim.x * blockDim.x) {
+        const double pj = fma(beta, fma(-omega, v[j], p[j]), r[j]);
+        p[j] = pj; y[j] = dinv[j] * pj;
+    }
+}
+// s = r - alpha v ; z = M^-1 s ; partial (s, s)
+__global__ void __launch_bounds__(RED_THREADS)
+k_bicg_s(long long n, double alpha, const double *__restrict__ r, const double *__restrict__ v, const double *__restrict__ dinv,
+         double *__restrict__ s, double *__restrict__ z, double *__restrict__ part) {
+    __shared__ double smem[32];
+    double a[1] = {0.0};
+    for (long long j = blockIdx.x * (long long)blockDim.x + threadIdx.x; j < n; j += (long long)gridDim.x * blockDim.x) {
+        const double sj = fma(-alpha, v[j], r[j]);
+        s[j] = sj; z[j] = dinv[j] * sj;
+        a[0] = fma(sj, sj, a[0]);
+    }
+    cta_reduce<1>(a, smem);
+    if (threadIdx.x == 0) part[blockIdx.x] = a[0];
+}
+// x += alpha y + omega z ; r = s - omega t ; partials (rhat, r), (r, r)
+__global__ void __launch_bounds__(RED_THREADS)
+k_bicg_xr(long long n, double alpha, double omega, const double *__restrict__ y, const double *__restrict__ z,
+          const double *__restrict__ s, const double *__restrict__ t, const double *__restrict__ rhat, double *__restrict__ x,
+          double *__restrict__ r, double *__restrict__ part) {
+    __shared__ double smem[2 * 32];
+    double a[2] = {0.0, 0.0};
+    for (long long j = blockIdx.x * (long long)blockDim.x + threadIdx.x; j < n; j += (long long)gridDim.x * blockDim.x) {
+        x[j] = fma(omega, z[j], fma(alpha, y[j], x[j]));
+        const double rj = fma(-omega, t[j], s[j]);
+        r[j] = rj;
+        a[0] = fma(rhat[j], rj, a[0]); a[1] = fma(rj, rj, a[1]);
+    }
+    cta_reduce<2>(a, smem);
+    if (threadIdx.x == 0) { part[2LL * blockIdx.x] = a[0]; part[2LL * blockIdx.x + 1] = a[1]; }
+}
+// x += alpha y (early exit after the first half step)
+__global__ void k_axpy(long long n, double alpha, const double *__restrict__ y, double *__restrict__ x) {
+    for (long long j = blockIdx.x * (long long)blockDim.x + threadIdx.x; j < n; j += (long long)gridDim.x * blockDim.x)
+        x[j] = fma(alpha, y[j], x[j]);
+}
+// rhs = -R ; partial (rhs, rhs) is taken later, after the Dirichlet rows
+__global__ void k_neg(long long n, const double *__restrict__ a, double *__restrict__ out) {
+    for (long long j = blockIdx.x * (long long)blockDim.x + threadIdx.x; j < n; j += (long long)gridDim.x * blockDim.x) out[j] = -a[j];
+}
+__global__ void __launch_bounds__(RED_THREADS) k_norm2(long long n, const double *__restrict__ a, double *__restrict__ part) {
+    __shared__ double smem[32];
+    double s[1] = {0.0};
+    for (long long j = blockIdx.x * (long long)blockDim.x + threadIdx.x; j < n; j += (long long)gridDim.x * blockDim.x) s[0] = fma(a[j], a[j], s[0]);
+    cta_reduce<1>(s, smem);
+    if (threadIdx.x == 0) part[blockIdx.x] = s[0];
+}
+
+// ------------------------------------------------------------------------------------------------ host side
+static int ensure_solver_ws(fem_ctx *c, bool newton) {
+    const long long n = c->n_rows;
+    if (!c->d_diagpos) {
+        FEM_CUDA(cudaMalloc(&c->d_diagpos, sizeof(int) * c->n_nodes));
+        k_diagpos<<<nblk3(c->n_nodes, 256), 256>>>(c->n_nodes, c->d_nb_ptr, c->d_nb, c->d_diagpos);
+        FEM_CUDA(cudaGetLastError());
+        FEM_CUDA(cudaDeviceSynchronize());
+    }
+    if (!c->d_sw) {
+        const long long spmv_ctas = (c->n_nodes + 7) / 8;
+        c->n_part = 2 * (spmv_ctas > RED_CTAS ? spmv_ctas : RED_CTAS);
+        FEM_CUDA(cudaMalloc(&c->d_sw, sizeof(double) * 9 * n));
+        FEM_CUDA(cudaMalloc(&c->d_part, sizeof(double) * c->n_part));
+        FEM_CUDA(cudaMalloc(&c->d_scal, sizeof(double) * 8));
+    }
+    if (newton && !c->d_nw) {
+        FEM_CUDA(cudaMalloc(&c->d_nw, sizeof(double) * 3 * n));
+        FEM_CUDA(cudaMalloc(&c->d_nw_vals, sizeof(double) * (size_t)c->nnz));
+    }
+    return FEM_OK;
+}
+
+// reduces `count` partial records of NV values and brings them to the host (synchronises the stream)
+template <int NV>
+static int fetch_sums(fem_ctx *c, long long count, double *host, cudaStream_t st) {
+    k_reduce_final<NV><<<1, 1024, 0, st>>>(c->d_part, count, c->d_scal);
+    FEM_CUDA(cudaMemcpyAsync(host, c->d_scal, sizeof(double) * NV, cudaMemcpyDeviceToHost, st));
+    FEM_CUDA(cudaStreamSynchronize(st));
+    return FEM_OK;
+}
+
+template <int DOT>
+static void launch_spmv(fem_ctx *c, const double *vals, const double *x, double *y, const double *w, cudaStream_t st) {
+    k_spmv<DOT><<<nblk3(c->n_nodes, 8), 256, 0, st>>>(c->n_nodes, c->d_nb_ptr, c->d_nb, vals, x, y, w, c->d_part);
+}
+
+extern "C" int fem_spmv(fem_ctx *c, const double *csr_vals, const double *x, double *y, void *cuda_stream) {
+    if (!c || !csr_vals || !x || !y) return FEM_ERR_NULL;
+    if (!c->has_pattern) return FEM_ERR_NO_PATTERN;
+    if (x == y) return FEM_ERR_ALIAS;
+    launch_spmv<0>(c, csr_vals, x, y, nullptr, (cudaStream_t)cuda_stream);
+    FEM_CUDA(cudaGetLastError());
+    return FEM_OK;
+}
+
+static int apply_dirichlet(fem_ctx *c, long long n_bc, const int *bc_dofs, const double *bc_rhs, const double *bc_vals,
+                           const double *u, double *vals, double *rhs, cudaStream_t st) {
+    if (n_bc == 0) return FEM_OK;
+    k_dirichlet<<<nblk3(n_bc, 128), 128, 0, st>>>(n_bc, bc_dofs, bc_rhs, bc_vals, u, c->d_nb_ptr, c->d_diagpos, vals, rhs);
+    FEM_CUDA(cudaGetLastError());
+    return FEM_OK;
+}
+
+static int check_dofs(fem_ctx *c, long long n_bc, const int *bc_dofs, cudaStream_t st) {
+    if (n_bc == 0) return FEM_OK;
+    int h = 0;
+    FEM_CUDA(cudaMemsetAsync(c->d_scal, 0, sizeof(int), st));
+    k_check_dofs<<<nblk3(n_bc, 256), 256, 0, st>>>(n_bc, bc_dofs, c->n_rows, reinterpret_cast<int *>(c->d_scal));
+    FEM_CUDA(cudaMemcpyAsync(&h, c->d_scal, sizeof(int), cudaMemcpyDeviceToHost, st));
+    FEM_CUDA(cudaStreamSynchronize(st));
+    return h ? FEM_ERR_ARG : FEM_OK;
+}
+
+extern "C" int fem_apply_dirichlet(fem_ctx *c, long long n_bc, const int *bc_dofs, const double *bc_rhs, double *csr_vals,
+                                   double *rhs, void *cuda_stream) {
+    if (!c || !csr_vals || (n_bc > 0 && !bc_dofs)) return FEM_ERR_NULL;
+    if (!c->has_pattern) return FEM_ERR_NO_PATTERN;
+    if (n_bc < 0) return FEM_ERR_ARG;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int rc = ensure_solver_ws(c, false);
+    if (rc != FEM_OK) return rc;
+    rc = check_dofs(c, n_bc, bc_dofs, st);
+    if (rc != FEM_OK) return rc;
+    return apply_dirichlet(c, n_bc, bc_dofs, bc_rhs, nullptr, nullptr, csr_vals, rhs, st);
+}
+
+// Jacobi-preconditioned BiCGSTAB, right preconditioning (van der Vorst 1992; the paper's default Krylov method):
+//   rho = (rhat, r); beta = (rho/rho_old)(alpha/omega); p = r + beta (p - omega v); y = M^-1 p; v = K y;
+//   alpha = rho / (rhat, v); s = r - alpha v; z = M^-1 s; t = K z; omega = (t, s)/(t, t);
+//   x += alpha y + omega z; r = s - omega t.
+static int bicgstab(fem_ctx *c, const double *vals, const double *b, double *x, double rtol, int max_iter, int *iters,
+                    double *relres, cudaStream_t st) {
+    const long long n = c->n_rows;
+    double *r = c->d_sw, *rhat = r + n, *p = rhat + n, *v = p + n, *s = v + n, *t = s + n, *y = t + n, *z = y + n, *dinv = z + n;
+    const long long spmv_ctas = (c->n_nodes + 7) / 8;
+    double h[2];
+    k_dinv<<<nblk3(n, 256), 256, 0, st>>>(c->n_nodes, c->d_nb_ptr, c->d_diagpos, vals, dinv);
+    launch_spmv<0>(c, vals, x, r, nullptr, st);
+    k_bicg_init<<<RED_CTAS, RED_THREADS, 0, st>>>(n, b, r, rhat, p, v, c->d_part);
+    int rc = fetch_sums<2>(c, RED_CTAS, h, st);
+    if (rc != FEM_OK) return rc;
+    double rr = h[0];
+    const double bb = h[1];
+    int it = 0;
+    bool conv = false;
+    if (bb == 0.0) {   // b = 0: the solution is x = 0
+        FEM_CUDA(cudaMemsetAsync(x, 0, sizeof(double) * n, st));
+        if (iters) *iters = 0;
+        if (relres) *relres = 0.0;
+        return FEM_OK;
+    }
+    const double tol2 = rtol * rtol * bb;
+    double rhat_norm = sqrt(rr);
+    double rho = rr, rho_old = 1.0, alpha = 1.0, omega = 1.0;
+    conv = rr <= tol2;
+    int restarts = 0;
+    while (!conv && it < max_iter) {
+        it++;
+        // breakdown guard: (rhat, r) has collapsed relative to |rhat||r| (rhat = the residual of the last restart), or a
+        // scalar is zero / not finite -> restart from the true residual of the current x (rhat = r = b - K x, p = v = 0)
+        bool restart = !(fabs(rho) > 1e-12 * sqrt(rr) * rhat_norm) || !isfinite(rho) || omega == 0.0 || !isfinite(omega);
+        double rv = 0.0;
+        if (!restart) {
+            const double beta = (rho / rho_old) * (alpha / omega);
+            k_bicg_p<<<RED_CTAS, RED_THREADS, 0, st>>>(n, beta, omega, r, v, dinv, p, y);
+            launch_spmv<1>(c, vals, y, v, rhat, st);
+            if ((rc = fetch_sums<2>(c, spmv_ctas, h, st)) != FEM_OK) return rc;
+            rv = h[0];
+            restart = (rv == 0.0 || !isfinite(rv));
+        }
+        if (restart) {
+            if (++restarts > 50) break;
+            launch_spmv<0>(c, vals, x, r, nullptr, st);
+            k_bicg_init<<<RED_CTAS, RED_THREADS, 0, st>>>(n, b, r, rhat, p, v, c->d_part);
+            if ((rc = fetch_sums<2>(c, RED_CTAS, h, st)) != FEM_OK) return rc;
+            rr = h[0]; rho = rr; rho_old = alpha = omega = 1.0; rhat_norm = sqrt(rr);
+            if (rr <= tol2) { conv = true; break; }
+            if (!isfinite(rr)) break;
+            continue;
+        }
+        alpha = rho / rv;
+        k_bicg_s<<<RED_CTAS, RED_THREADS, 0, st>>>(n, alpha, r, v, dinv, s, z, c->d_part);
+        if ((rc = fetch_sums<1>(c, RED_CTAS, h, st)) != FEM_OK) return rc;
+        if (h[0] <= tol2) {   // first half step already meets the tolerance
+            k_axpy<<<RED_CTAS, RED_THREADS, 0, st>>>(n, alpha, y, x);
+            conv = true;
+            break;
+        }
+        launch_spmv<2>(c, vals, z, t, s, st);
+        if ((rc = fetch_sums<2>(c, spmv_ctas, h, st)) != FEM_OK) return rc;
+        const double ts = h[0], tt = h[1];
+        omega = (tt > 0.0 && isfinite(tt)) ? ts / tt : 0.0;
+        k_bicg_xr<<<RED_CTAS, RED_THREADS, 0, st>>>(n, alpha, omega, y, z, s, t, rhat, x, r, c->d_part);
+        if ((rc = fetch_sums<2>(c, RED_CTAS, h, st)) != FEM_OK) return rc;
+        rho_old = rho; rho = h[0]; rr = h[1];
+        if (rr <= tol2) { conv = true; break; }
+    }
+    // explicit residual of the returned x (the recurrence residual can drift)
+    launch_spmv<0>(c, vals, x, r, nullptr, st);
+    k_bicg_init<<<RED_CTAS, RED_THREADS, 0, st>>>(n, b, r, rhat, p, v, c->d_part);
+    if ((rc = fetch_sums<2>(c, RED_CTAS, h, st)) != FEM_OK) return rc;
+    const double rel = sqrt(h[0] / bb);
+    if (iters) *iters = it;
+    if (relres) *relres = rel;
+    FEM_CUDA(cudaGetLastError());
+    return (conv && rel <= 100.0 * rtol) ? FEM_OK : FEM_ERR_NOCONV;
+}
+
+extern "C" int fem_bicgstab(fem_ctx *c, const double *csr_vals, const double *b, double *x, double rtol, int max_iter, int *iters,
+                            double *relres, void *cuda_stream) {
+    if (!c || !csr_vals || !b || !x) return FEM_ERR_NULL;
+    if (!c->has_pattern) return FEM_ERR_NO_PATTERN;
+    if (!(rtol > 0.0) || max_iter < 0 || b == x) return FEM_ERR_ARG;
+    int rc = ensure_solver_ws(c, false);
+    if (rc != FEM_OK) return rc;
+    return bicgstab(c, csr_vals, b, x, rtol, max_iter, iters, relres, (cudaStream_t)cuda_stream);
+}
+
+extern "C" void fem_default_newton_options(fem_newton_options *o) {
+    if (!o) return;
+    o->rtol = 1e-9; o->atol = 1e-10; o->max_newton = 25; o->lin_rtol = 1e-10; o->lin_max_iter = 10000;
+}
+
+// One load increment: K dd = -R, d <- d + dd (Eq.(39)) with identity rows for the constrained DOFs.
+extern "C" int fem_newton_solve(fem_ctx *c, double *u, const double *hist_in, const double *mat, long long n_mat, long long n_bc,
+                                const int *bc_dofs, const double *bc_vals, double *hist_out, const fem_newton_options *opt,
+                                fem_newton_report *rep, void *cuda_stream) {
+    if (!c || !u || !hist_in || !mat || !hist_out || (n_bc > 0 && (!bc_dofs || !bc_vals))) return FEM_ERR_NULL;
+    if (!c->has_pattern) return FEM_ERR_NO_PATTERN;
+    if (n_mat != 1 && n_mat != c->n_elems) return FEM_ERR_MAT;
+    if (n_bc < 0) return FEM_ERR_ARG;
+    fem_newton_options o;
+    fem_default_newton_options(&o);
+    if (opt) o = *opt;
+    if (!(o.rtol >= 0.0) || !(o.atol >= 0.0) || o.max_newton < 1 || !(o.lin_rtol > 0.0) || o.lin_max_iter < 1) return FEM_ERR_ARG;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int rc = ensure_solver_ws(c, true);
+    if (rc != FEM_OK) return rc;
+    if ((rc = check_dofs(c, n_bc, bc_dofs, st)) != FEM_OK) return rc;
+    const long long n = c->n_rows;
+    double *R = c->d_nw, *rhs = R + n, *dd = rhs + n, *vals = c->d_nw_vals;
+    fem_newton_report rp;
+    memset(&rp, 0, sizeof(rp));
+    int result = FEM_ERR_NOCONV;
+    for (int k = 0;; k++) {
+        if ((rc = fem_launch_assemble(c, u, hist_in, mat, n_mat, R, vals, hist_out, st)) != FEM_OK) return rc;
+        if ((rc = fem_read_stats(c, &rp.last_stats, st)) != FEM_OK) return rc;
+        k_neg<<<RED_CTAS, RED_THREADS, 0, st>>>(n, R, rhs);
+        if ((rc = apply_dirichlet(c, n_bc, bc_dofs, nullptr, bc_vals, u, vals, rhs, st)) != FEM_OK) return rc;
+        k_norm2<<<RED_CTAS, RED_THREADS, 0, st>>>(n, rhs, c->d_part);
+        double h[1];
+        if ((rc = fetch_sums<1>(c, RED_CTAS, h, st)) != FEM_OK) return rc;
+        rp.rhs_norm = sqrt(h[0]);
+        if (k == 0) rp.rhs_norm0 = rp.rhs_norm;
+        if (!isfinite(rp.rhs_norm)) break;
+        if (rp.rhs_norm <= o.atol || rp.rhs_norm <= o.rtol * rp.rhs_norm0) { rp.converged = 1; result = FEM_OK; break; }
+        if (k >= o.max_newton) break;
+        FEM_CUDA(cudaMemsetAsync(dd, 0, sizeof(double) * n, st));
+        int its = 0;
+        rc = bicgstab(c, vals, rhs, dd, o.lin_rtol, o.lin_max_iter, &its, nullptr, st);
+        rp.lin_iters_total += its;
+        if (rc == FEM_ERR_NOCONV) rp.lin_failures++;
+        else if (rc != FEM_OK) return rc;
+        k_axpy<<<RED_CTAS, RED_THREADS, 0, st>>>(n, 1.0, dd, u);
+        rp.newton_iters++;
+    }
+    FEM_CUDA(cudaGetLastError());
+    FEM_CUDA(cudaStreamSynchronize(st));
+    if (rep) *rep = rp;
+    return result;
+}

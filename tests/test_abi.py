@@ -30,7 +30,7 @@ def test_strerror_and_defaults():
     import paper_2606_17390_b200 as fem
     L = fem.lib()
     assert L.fem_strerror(0) == b"ok"
-    for code in range(-10, 0):
+    for code in range(-11, 0):
         assert L.fem_strerror(code) not in (b"ok", b"unknown error code")
     opt = fem.FemOptions()
     L.fem_default_options(C.byref(opt))
@@ -47,6 +47,13 @@ def test_null_and_argument_errors_without_device_work():
     assert L.fem_build_csr_pattern(None, None, None, None, None, None) == -1
     assert L.fem_assemble(None, None, None, None, 1, None, None, None, None, None) == -1
     assert L.fem_launches_per_assemble(None) == 0
+    assert L.fem_spmv(None, None, None, None, None) == -1
+    assert L.fem_apply_dirichlet(None, 0, None, None, None, None, None) == -1
+    assert L.fem_bicgstab(None, None, None, None, 1e-8, 10, None, None, None) == -1
+    assert L.fem_newton_solve(None, None, None, None, 1, 0, None, None, None, None, None, None) == -1
+    no = fem.FemNewtonOptions()
+    L.fem_default_newton_options(C.byref(no))
+    assert (no.rtol, no.atol, no.max_newton, no.lin_rtol, no.lin_max_iter) == (1e-9, 1e-10, 25, 1e-10, 10000)
 
 
 def test_lankford_helper_matches_closed_form():
