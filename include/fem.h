@@ -188,7 +188,9 @@ typedef struct {
 void fem_default_newton_options(fem_newton_options *o /*host*/);
 
 /* One load increment: global Newton-Raphson K dd = -R, d <- d + dd (Eq.(39)) with Dirichlet data.
- *   u        dev [n_rows] in/out: initial guess (e.g. the last converged state) -> converged displacement
+ *   u        dev [n_rows] in/out: initial guess (e.g. the last converged state) -> converged displacement; when the
+ *            increment fails (FEM_ERR_NOCONV) u is restored to its entry value, so the caller can cut the step back
+ *            (the paper's adaptive stepping, is host control flow and stays with the caller)
  *   hist_in  dev [n_elems*56] history at the start of the increment (unchanged)
  *   hist_out dev [n_elems*56] history at the returned u (from the last fem_assemble)
  *   bc_dofs  dev [n_bc] constrained DOFs, bc_vals dev [n_bc] their prescribed TOTAL displacement

@@ -1,0 +1,101 @@
+"""Measurements of SURVEY.md §8(f) NEXT-1 on the paper's unit-cube benchmark (Table 3 :493-495,
+Table F1 :1064-1073), 100^3 hex8 = 3,090,903 DOF, one B200:
+
+    python -m paper_2606_17390_b200.bench_solve [--n 100] [--lin-rtol 1e-8]
+
+  1. fem_spmv: ms and achieved GB/s (algorithmic bytes: 8 nnz values + 4 bytes per 3x3 block index + x read + y written).
+  2. fem_bicgstab on the linear-elastic stiffness (Table F1's workload: "linear elastic problem on a unit-cube domain";
+     left face fixed, right face displaced): iterations, seconds, ms per iteration.  Paper, H100: JAX-BiCGSTAB 11.21 s,
+     AMGX-BiCGSTAB 1.96 s at 3,090,903 DOF (tolerance not stated; context, other hardware).
+  3. fem_newton_solve: one load increment of the elastoplastic benchmark (Hill-48 + Voce, Table 3; right face moved by
+     dt * (0.2, 0.1, 0) mm, dt = 0.05 = the paper's largest step): Newton iterations, BiCGSTAB iterations, seconds.
+     Paper, H100: 31 load steps / 111 Newton iterations in 2030 s = 18.3 s per Newton iteration (context).
+Prints markdown; kept in profiles/.  Inputs are synthetic (structured unit cube, seeded nothing: the problem is fully
+specified by the paper's text).
+"""
+import argparse
+import os
+import sys
+import time
+
+import numpy as np
+
+sys.path.insert(0, os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
+
+
+def main():
+    import torch
+    import paper_2606_17390_b200 as fem
+    from synth import mesh
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--n", type=int, default=100)
+    ap.add_argument("--lin-rtol", type=float, default=1e-8)
+    ap.add_argument("--dt", default="0.002,0.005,0.01", help="load fractions of the Newton runs, each from the undeformed state")
+    args = ap.parse_args()
+    n = args.n
+    dev = torch.device("cuda:0")
+    coords, conn = mesh.structured_hex_mesh(n, n, n)
+    nn, ne = coords.shape[0], conn.shape[0]
+    ctx = fem.FemContext(torch.from_numpy(coords).to(dev), torch.from_numpy(conn).to(dev))
+    ctx.build_csr_pattern()
+    nnz, nr = ctx.nnz, 3 * nn
+    # Table 3: E = 219 GPa, Voce sigma0 = 138, Q = 410, b = 3.8, ratios r11..r23; nu is not printed: 0.3
+    rec = fem.mat_record(219000.0, 0.3, [1.5449, 1.0666, 1.0, 1.0307, 1.0, 1.0], 0.0, 138.0, 410.0, 3.8)
+    mat = torch.from_numpy(rec).to(dev)
+    nid = np.arange(nn)
+    lf, rt = np.abs(coords[:, 0]) < 1e-12, np.abs(coords[:, 0] - 1.0) < 1e-12
+    bc = np.concatenate([(3 * nid[lf][:, None] + np.arange(3)).ravel(), (3 * nid[rt][:, None] + np.arange(3)).ravel()]).astype(np.int32)
+    full = np.concatenate([np.zeros(3 * int(lf.sum())), np.tile([0.2, 0.1, 0.0], int(rt.sum()))])
+    bc_d = torch.from_numpy(bc).to(dev)
+    hin = torch.zeros(56 * ne, dtype=torch.float64, device=dev)
+    u0 = torch.zeros(nr, dtype=torch.float64, device=dev)
+    print("# NEXT-1 on the unit-cube benchmark, %d^3 elements, %d DOF, nnz %d\n" % (n, nr, nnz))
+
+    # ---- 1. SpMV
+    res, vals, _, _ = ctx.assemble(u0, hin, mat)
+    x = torch.from_numpy(np.random.default_rng(1).normal(size=nr)).to(dev)
+    y = torch.empty_like(x)
+    for _ in range(3):
+        ctx.spmv(vals, x, y)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    reps = 20
+    e0.record()
+    for _ in range(reps):
+        ctx.spmv(vals, x, y)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / reps
+    byts = 8.0 * nnz + 4.0 * nnz / 9 + 16.0 * nr
+    print("| fem_spmv | %.3f ms | %.0f GB/s algorithmic (values + block indices + x + y = %.2f GB) |" % (ms, byts / ms / 1e6, byts / 1e9))
+
+    # ---- 2. BiCGSTAB on the linear-elastic stiffness (Table F1 workload)
+    rhs = torch.zeros(nr, dtype=torch.float64, device=dev)
+    ctx.apply_dirichlet(bc_d, vals, rhs, torch.from_numpy(full * 0.05).to(dev))
+    torch.cuda.synchronize()
+    for rtol in (1e-6, args.lin_rtol):
+        t0 = time.perf_counter()
+        xs, its, rr, ok = ctx.bicgstab(vals, rhs, rtol=rtol, max_iter=20000)
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        print("| fem_bicgstab, linear elastic, rtol %.0e | %d iterations | %.3f s | %.3f ms/iteration | explicit relres %.2e | converged %s |"
+              % (rtol, its, dt, 1e3 * dt / max(its, 1), rr, ok))
+
+    # ---- 3. one elastoplastic load increment from the undeformed state, for several increment sizes
+    for dts in args.dt.split(","):
+        dtf = float(dts)
+        u = torch.zeros(nr, dtype=torch.float64, device=dev)
+        t0 = time.perf_counter()
+        u, hout, rep = ctx.newton_solve(u, hin, mat, bc_d, torch.from_numpy(full * dtf).to(dev), lin_rtol=args.lin_rtol,
+                                        lin_max_iter=5000, rtol=1e-8, max_newton=12)
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        st = rep["last_stats"]
+        print("| fem_newton_solve, load fraction %.3g (right face %.3g, %.3g mm), Table 3 material | %d Newton iterations | %d BiCGSTAB "
+              "iterations | %.2f s total = %.2f s per Newton iteration | plastic fraction %.3f | rhs norm %.2e -> %.2e | converged %s, "
+              "linear failures %d |" % (dtf, 0.2 * dtf, 0.1 * dtf, rep["newton_iters"], rep["lin_iters_total"], dt,
+                                        dt / max(rep["newton_iters"], 1), st["n_plastic"] / (8.0 * ne), rep["rhs_norm0"], rep["rhs_norm"],
+                                        rep["converged"], rep["lin_failures"]), flush=True)
+
+
+if __name__ == "__main__":
+    main()

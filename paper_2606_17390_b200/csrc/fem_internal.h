@@ -51,7 +51,7 @@ struct fem_ctx {
     double *d_sw = nullptr;        // [9*n_rows] Krylov vectors r, rhat, p, v, s, t, y, z and the inverse diagonal
     double *d_part = nullptr;      // partial sums of the deterministic reductions
     double *d_scal = nullptr;      // [8] reduced scalars
-    double *d_nw = nullptr;        // [3*n_rows] Newton workspace: residual, rhs, dd
+    double *d_nw = nullptr;        // [4*n_rows] Newton workspace: residual, rhs, dd, u at entry
     double *d_nw_vals = nullptr;   // [nnz] Newton workspace: stiffness values
     long long n_part = 0;
     // host-buffer path

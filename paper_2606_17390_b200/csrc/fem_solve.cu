@@ -227,7 +227,7 @@ static int ensure_solver_ws(fem_ctx *c, bool newton) {
         FEM_CUDA(cudaMalloc(&c->d_scal, sizeof(double) * 8));
     }
     if (newton && !c->d_nw) {
-        FEM_CUDA(cudaMalloc(&c->d_nw, sizeof(double) * 3 * n));
+        FEM_CUDA(cudaMalloc(&c->d_nw, sizeof(double) * 4 * n));
         FEM_CUDA(cudaMalloc(&c->d_nw_vals, sizeof(double) * (size_t)c->nnz));
     }
     return FEM_OK;
@@ -401,7 +401,8 @@ extern "C" int fem_newton_solve(fem_ctx *c, double *u, const double *hist_in, co
     if (rc != FEM_OK) return rc;
     if ((rc = check_dofs(c, n_bc, bc_dofs, st)) != FEM_OK) return rc;
     const long long n = c->n_rows;
-    double *R = c->d_nw, *rhs = R + n, *dd = rhs + n, *vals = c->d_nw_vals;
+    double *R = c->d_nw, *rhs = R + n, *dd = rhs + n, *u_entry = dd + n, *vals = c->d_nw_vals;
+    FEM_CUDA(cudaMemcpyAsync(u_entry, u, sizeof(double) * n, cudaMemcpyDeviceToDevice, st));
     fem_newton_report rp;
     memset(&rp, 0, sizeof(rp));
     int result = FEM_ERR_NOCONV;
@@ -427,6 +428,8 @@ extern "C" int fem_newton_solve(fem_ctx *c, double *u, const double *hist_in, co
         k_axpy<<<RED_CTAS, RED_THREADS, 0, st>>>(n, 1.0, dd, u);
         rp.newton_iters++;
     }
+    if (result != FEM_OK)   // failed increment: u goes back to its entry value, so the caller can cut the step back
+        FEM_CUDA(cudaMemcpyAsync(u, u_entry, sizeof(double) * n, cudaMemcpyDeviceToDevice, st));
     FEM_CUDA(cudaGetLastError());
     FEM_CUDA(cudaStreamSynchronize(st));
     if (rep) *rep = rp;

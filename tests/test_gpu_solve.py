@@ -127,6 +127,11 @@ def test_newton_patch_solution_and_error_paths():
     u = torch.zeros(coords.size, dtype=torch.float64, device=dev)
     u, _, rep = ctx.newton_solve(u, hin, mat, torch.from_numpy(bc).to(dev), torch.from_numpy(exact.ravel()[bc]).to(dev))
     assert rep["converged"] and np.abs(u.cpu().numpy() - exact.ravel()).max() < 1e-9   # homogeneous-deformation patch solution
+    # a failed increment (iteration cap) leaves u at its entry value
+    u_in = torch.from_numpy(1e-3 * np.random.default_rng(2).normal(size=coords.size)).to(dev)
+    u2, _, rep2 = ctx.newton_solve(u_in.clone(), hin, mat, torch.from_numpy(bc).to(dev), torch.from_numpy(exact.ravel()[bc]).to(dev),
+                                   max_newton=1)
+    assert not rep2["converged"] and rep2["newton_iters"] == 1 and torch.equal(u2, u_in)
     bad = torch.tensor([0, 3 * coords.shape[0]], dtype=torch.int32, device=dev)      # DOF out of range
     with pytest.raises(fem.FemError):
         ctx.newton_solve(u, hin, mat, bad, torch.zeros(2, dtype=torch.float64, device=dev))
