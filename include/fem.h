@@ -168,12 +168,22 @@ int fem_apply_dirichlet(fem_ctx *c, long long n_bc, const int *bc_dofs, const do
 int fem_bicgstab(fem_ctx *c, const double *csr_vals, const double *b, double *x, double rtol, int max_iter, int *iters,
                  double *relres, void *cuda_stream);
 
+/* Jacobi-preconditioned conjugate gradients for symmetric positive definite K; same arguments, stopping rule, determinism
+ * and return codes as fem_bicgstab.  After fem_apply_dirichlet K as a whole is not symmetric (rows only, as in the paper),
+ * but if the initial guess x already holds b[d] on every constrained DOF d, all Krylov vectors vanish there and the
+ * iteration is CG on the symmetric reduced system; fem_newton_solve calls it that way.  Also returns FEM_ERR_NOCONV when
+ * (p, K p) <= 0 is met (K not positive definite). */
+int fem_pcg(fem_ctx *c, const double *csr_vals, const double *b, double *x, double rtol, int max_iter, int *iters,
+            double *relres, void *cuda_stream);
+
 typedef struct {
     double rtol;      /* Newton stops when ||rhs||_2 <= rtol * ||rhs of iteration 0||_2 ... */
     double atol;      /* ... or <= atol (rhs = -R on free DOFs, prescribed - current on constrained DOFs); defaults 1e-9, 1e-10 */
     int max_newton;   /* default 25 */
     double lin_rtol;  /* BiCGSTAB tolerance per Newton iteration, default 1e-10 */
     int lin_max_iter; /* default 10000 */
+    int linear_solver; /* 0 (default) = fem_pcg for the standard element (K_ff symmetric), falling back to fem_bicgstab when CG
+                         gives up; F-bar (unsymmetric K) always uses fem_bicgstab.  1 = fem_bicgstab only, 2 = fem_pcg only */
 } fem_newton_options;
 
 typedef struct {
@@ -195,7 +205,7 @@ void fem_default_newton_options(fem_newton_options *o /*host*/);
  *   hist_out dev [n_elems*56] history at the returned u (from the last fem_assemble)
  *   bc_dofs  dev [n_bc] constrained DOFs, bc_vals dev [n_bc] their prescribed TOTAL displacement
  * Each iteration: fem_assemble(u) -> rhs = -R -> constrained rows: identity, rhs = bc_vals - u (so the update lands on
- * the prescribed value) -> test ||rhs|| -> fem_bicgstab from a zero guess -> u += dd.  The stiffness matrix, residual and
+ * the prescribed value) -> test ||rhs|| -> linear solve (fem_newton_options.linear_solver) -> u += dd.  The stiffness matrix, residual and
  * Krylov vectors live in library-owned workspace (allocated on first use).  Returns FEM_OK when converged,
  * FEM_ERR_NOCONV when max_newton is reached; *rep (host, may be NULL) is always filled.  Synchronises the stream. */
 int fem_newton_solve(fem_ctx *c, double *u, const double *hist_in, const double *mat, long long n_mat, long long n_bc,

@@ -30,7 +30,8 @@ def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--n", type=int, default=100)
     ap.add_argument("--lin-rtol", type=float, default=1e-8)
-    ap.add_argument("--dt", default="0.002,0.005,0.01", help="load fractions of the Newton runs, each from the undeformed state")
+    ap.add_argument("--dt", default="0.002,0.005", help="load fractions of the Newton runs, each from the undeformed state")
+    ap.add_argument("--path", default="0.002x8", help="load path: step size x number of steps, history and displacement carried over")
     args = ap.parse_args()
     n = args.n
     dev = torch.device("cuda:0")
@@ -90,11 +91,39 @@ def main():
         torch.cuda.synchronize()
         dt = time.perf_counter() - t0
         st = rep["last_stats"]
-        print("| fem_newton_solve, load fraction %.3g (right face %.3g, %.3g mm), Table 3 material | %d Newton iterations | %d BiCGSTAB "
+        print("| fem_newton_solve, load fraction %.3g (right face %.3g, %.3g mm), Table 3 material | %d Newton iterations | %d linear "
               "iterations | %.2f s total = %.2f s per Newton iteration | plastic fraction %.3f | rhs norm %.2e -> %.2e | converged %s, "
               "linear failures %d |" % (dtf, 0.2 * dtf, 0.1 * dtf, rep["newton_iters"], rep["lin_iters_total"], dt,
                                         dt / max(rep["newton_iters"], 1), st["n_plastic"] / (8.0 * ne), rep["rhs_norm0"], rep["rhs_norm"],
                                         rep["converged"], rep["lin_failures"]), flush=True)
+
+    # ---- 4. a load path: equal steps, converged state and history carried from step to step (the paper's protocol, :485-487,
+    #         without its adaptive step control; initial guess = last converged displacement)
+    step, nsteps = args.path.split("x")
+    step, nsteps = float(step), int(nsteps)
+    u = torch.zeros(nr, dtype=torch.float64, device=dev)
+    h_a = torch.zeros(56 * ne, dtype=torch.float64, device=dev)
+    h_b = torch.empty_like(h_a)
+    tot_newton = tot_lin = 0
+    t_path = time.perf_counter()
+    for k in range(1, nsteps + 1):
+        t0 = time.perf_counter()
+        u, h_b, rep = ctx.newton_solve(u, h_a, mat, bc_d, torch.from_numpy(full * (step * k)).to(dev), hist_out=h_b,
+                                       lin_rtol=args.lin_rtol, lin_max_iter=10000, rtol=1e-8, max_newton=12)
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        st = rep["last_stats"]
+        print("| path step %d, load fraction %.4g | %d Newton iterations | %d linear iterations | %.2f s | plastic fraction %.3f | "
+              "rhs norm %.2e -> %.2e | converged %s, linear failures %d |" % (k, step * k, rep["newton_iters"], rep["lin_iters_total"], dt,
+                                                                            st["n_plastic"] / (8.0 * ne), rep["rhs_norm0"], rep["rhs_norm"],
+                                                                            rep["converged"], rep["lin_failures"]), flush=True)
+        if not rep["converged"]:
+            break
+        tot_newton += rep["newton_iters"]; tot_lin += rep["lin_iters_total"]
+        h_a, h_b = h_b, h_a
+    dt = time.perf_counter() - t_path
+    print("| path total | %d Newton iterations | %d linear iterations | %.2f s = %.2f s per Newton iteration |"
+          % (tot_newton, tot_lin, dt, dt / max(tot_newton, 1)))
 
 
 if __name__ == "__main__":

@@ -9,7 +9,7 @@ NPAR = 16
 
 ABI_SYMBOLS = ["fem_default_options", "fem_setup", "fem_build_csr_pattern", "fem_assemble", "fem_assemble_host",
                "fem_last_kernel_ms", "fem_launches_per_assemble", "fem_probe_fp64_peak", "fem_destroy", "fem_strerror",
-               "fem_last_cuda_error", "fem_hill_from_lankford", "fem_spmv", "fem_apply_dirichlet", "fem_bicgstab",
+               "fem_last_cuda_error", "fem_hill_from_lankford", "fem_spmv", "fem_apply_dirichlet", "fem_bicgstab", "fem_pcg",
                "fem_default_newton_options", "fem_newton_solve"]
 
 
@@ -29,7 +29,7 @@ class FemStats(C.Structure):
 
 class FemNewtonOptions(C.Structure):
     _fields_ = [("rtol", C.c_double), ("atol", C.c_double), ("max_newton", C.c_int), ("lin_rtol", C.c_double),
-                ("lin_max_iter", C.c_int)]
+                ("lin_max_iter", C.c_int), ("linear_solver", C.c_int)]
 
 
 class FemNewtonReport(C.Structure):
@@ -92,6 +92,7 @@ def lib():
         L.fem_spmv.argtypes = [vp, vp, vp, vp, vp]
         L.fem_apply_dirichlet.argtypes = [vp, ll, vp, vp, vp, vp, vp]
         L.fem_bicgstab.argtypes = [vp, vp, vp, vp, C.c_double, C.c_int, C.POINTER(C.c_int), dp, vp]
+        L.fem_pcg.argtypes = [vp, vp, vp, vp, C.c_double, C.c_int, C.POINTER(C.c_int), dp, vp]
         L.fem_default_newton_options.argtypes = [C.POINTER(FemNewtonOptions)]
         L.fem_default_newton_options.restype = None
         L.fem_newton_solve.argtypes = [vp, vp, vp, vp, ll, ll, vp, vp, vp, C.POINTER(FemNewtonOptions),
@@ -264,8 +265,20 @@ class FemContext:
             _check(rc, "fem_bicgstab")
         return x, it.value, rr.value, rc == 0
 
+    def pcg(self, csr_vals, b, x=None, rtol=1e-10, max_iter=10000):
+        """fem_pcg: returns (x, iters, relres, converged).  x must hold b[d] on Dirichlet DOFs d (see include/fem.h)."""
+        torch = _torch()
+        if x is None:
+            x = torch.zeros(self.n_rows, dtype=torch.float64, device=self.device)
+        it, rr = C.c_int(0), C.c_double(0.0)
+        rc = lib().fem_pcg(self._h, _ptr(csr_vals, torch.float64, self.nnz, "csr_vals"), _ptr(b, torch.float64, self.n_rows, "b"),
+                           _ptr(x, torch.float64, self.n_rows, "x"), float(rtol), int(max_iter), C.byref(it), C.byref(rr), _stream_ptr())
+        if rc not in (0, -11):
+            _check(rc, "fem_pcg")
+        return x, it.value, rr.value, rc == 0
+
     def newton_solve(self, u, hist_in, mat, bc_dofs, bc_vals, hist_out=None, rtol=None, atol=None, max_newton=None,
-                     lin_rtol=None, lin_max_iter=None):
+                     lin_rtol=None, lin_max_iter=None, linear_solver=None):
         """fem_newton_solve: one load increment; u is updated in place.  Returns (u, hist_out, report dict)."""
         torch = _torch()
         f64 = torch.float64
@@ -273,7 +286,8 @@ class FemContext:
             hist_out = torch.empty(self.n_elems * 56, dtype=f64, device=self.device)
         opt = FemNewtonOptions()
         lib().fem_default_newton_options(C.byref(opt))
-        for k, v in (("rtol", rtol), ("atol", atol), ("max_newton", max_newton), ("lin_rtol", lin_rtol), ("lin_max_iter", lin_max_iter)):
+        for k, v in (("rtol", rtol), ("atol", atol), ("max_newton", max_newton), ("lin_rtol", lin_rtol), ("lin_max_iter", lin_max_iter),
+                     ("linear_solver", linear_solver)):
             if v is not None:
                 setattr(opt, k, v)
         rep = FemNewtonReport()

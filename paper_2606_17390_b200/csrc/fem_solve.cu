@@ -37,6 +37,10 @@ __global__ void k_dirichlet(long long n_bc, const int *__restrict__ bc_dofs, con
     if (rhs) rhs[d] = bc_vals ? bc_vals[t] - u[d] : (bc_rhs ? bc_rhs[t] : 0.0);
 }
 
+__global__ void k_scatter_bc(long long n_bc, const int *__restrict__ bc_dofs, const double *__restrict__ rhs, double *__restrict__ x) {
+    long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (t < n_bc) x[bc_dofs[t]] = rhs[bc_dofs[t]];
+}
 __global__ void k_check_dofs(long long n_bc, const int *__restrict__ bc_dofs, long long n_rows, int *flag) {
     long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (t < n_bc && (bc_dofs[t] < 0 || bc_dofs[t] >= n_rows)) atomicOr(flag, 1);
@@ -192,6 +196,27 @@ k_bicg_xr(long long n, double alpha, double omega, const double *__restrict__ y,
     }
     cta_reduce<2>(a, smem);
     if (threadIdx.x == 0) { part[2LL * blockIdx.x] = a[0]; part[2LL * blockIdx.x + 1] = a[1]; }
+}
+// ---- preconditioned CG vector kernels
+// x += alpha p ; r -= alpha q ; z = M^-1 r ; partials (r, z), (r, r)
+__global__ void __launch_bounds__(RED_THREADS)
+k_cg_update(long long n, double alpha, const double *__restrict__ p, const double *__restrict__ q, const double *__restrict__ dinv,
+            double *__restrict__ x, double *__restrict__ r, double *__restrict__ z, double *__restrict__ part) {
+    __shared__ double smem[2 * 32];
+    double a[2] = {0.0, 0.0};
+    for (long long j = blockIdx.x * (long long)blockDim.x + threadIdx.x; j < n; j += (long long)gridDim.x * blockDim.x) {
+        x[j] = fma(alpha, p[j], x[j]);
+        const double rj = fma(-alpha, q[j], r[j]), zj = dinv[j] * rj;
+        r[j] = rj; z[j] = zj;
+        a[0] = fma(rj, zj, a[0]); a[1] = fma(rj, rj, a[1]);
+    }
+    cta_reduce<2>(a, smem);
+    if (threadIdx.x == 0) { part[2LL * blockIdx.x] = a[0]; part[2LL * blockIdx.x + 1] = a[1]; }
+}
+// p = z + beta p
+__global__ void k_cg_p(long long n, double beta, const double *__restrict__ z, double *__restrict__ p) {
+    for (long long j = blockIdx.x * (long long)blockDim.x + threadIdx.x; j < n; j += (long long)gridDim.x * blockDim.x)
+        p[j] = fma(beta, p[j], z[j]);
 }
 // x += alpha y (early exit after the first half step)
 __global__ void k_axpy(long long n, double alpha, const double *__restrict__ y, double *__restrict__ x) {
@@ -369,6 +394,72 @@ static int bicgstab(fem_ctx *c, const double *vals, const double *b, double *x, 
     return (conv && rel <= 100.0 * rtol) ? FEM_OK : FEM_ERR_NOCONV;
 }
 
+// Jacobi-preconditioned conjugate gradients (Hestenes-Stiefel) for a symmetric positive definite K.  With identity rows for
+// the constrained DOFs and an initial guess that already carries the prescribed values there, every Krylov vector is zero
+// on the constrained DOFs and the iteration is CG on the symmetric reduced system K_ff (the row-eliminated K of Alg. E1 is
+// not symmetric as a whole).  Returns FEM_ERR_NOCONV also when (p, K p) <= 0 (K not positive definite).
+static int pcg(fem_ctx *c, const double *vals, const double *b, double *x, double rtol, int max_iter, int *iters, double *relres,
+               cudaStream_t st) {
+    const long long n = c->n_rows;
+    double *r = c->d_sw, *z = r + n, *p = z + n, *q = p + n, *scratch = q + n, *dinv = c->d_sw + 8 * n;
+    const long long spmv_ctas = (c->n_nodes + 7) / 8;
+    double h[2];
+    int rc;
+    k_dinv<<<nblk3(n, 256), 256, 0, st>>>(c->n_nodes, c->d_nb_ptr, c->d_diagpos, vals, dinv);
+    launch_spmv<0>(c, vals, x, r, nullptr, st);
+    k_bicg_init<<<RED_CTAS, RED_THREADS, 0, st>>>(n, b, r, scratch, p, q, c->d_part);   // r = b - K x, p = q = 0
+    if ((rc = fetch_sums<2>(c, RED_CTAS, h, st)) != FEM_OK) return rc;
+    const double bb = h[1];
+    if (bb == 0.0) {
+        FEM_CUDA(cudaMemsetAsync(x, 0, sizeof(double) * n, st));
+        if (iters) *iters = 0;
+        if (relres) *relres = 0.0;
+        return FEM_OK;
+    }
+    const double tol2 = rtol * rtol * bb;
+    double rr = h[0];
+    bool conv = rr <= tol2, bad = false;
+    int it = 0;
+    // z = M^-1 r and (r, z): one k_cg_update with alpha = 0
+    k_cg_update<<<RED_CTAS, RED_THREADS, 0, st>>>(n, 0.0, p, q, dinv, x, r, z, c->d_part);
+    if ((rc = fetch_sums<2>(c, RED_CTAS, h, st)) != FEM_OK) return rc;
+    double rz = h[0], beta = 0.0;
+    while (!conv && it < max_iter) {
+        it++;
+        k_cg_p<<<RED_CTAS, RED_THREADS, 0, st>>>(n, beta, z, p);
+        launch_spmv<1>(c, vals, p, q, p, st);                       // q = K p, partial (p, q)
+        if ((rc = fetch_sums<2>(c, spmv_ctas, h, st)) != FEM_OK) return rc;
+        const double pq = h[0];
+        if (!(pq > 0.0) || !isfinite(pq)) { bad = true; break; }
+        const double alpha = rz / pq;
+        k_cg_update<<<RED_CTAS, RED_THREADS, 0, st>>>(n, alpha, p, q, dinv, x, r, z, c->d_part);
+        if ((rc = fetch_sums<2>(c, RED_CTAS, h, st)) != FEM_OK) return rc;
+        const double rz_new = h[0];
+        rr = h[1];
+        if (rr <= tol2) { conv = true; break; }
+        if (!(rz_new > 0.0) || !isfinite(rz_new)) { bad = true; break; }
+        beta = rz_new / rz; rz = rz_new;
+    }
+    launch_spmv<0>(c, vals, x, r, nullptr, st);
+    k_bicg_init<<<RED_CTAS, RED_THREADS, 0, st>>>(n, b, r, scratch, p, q, c->d_part);
+    if ((rc = fetch_sums<2>(c, RED_CTAS, h, st)) != FEM_OK) return rc;
+    const double rel = sqrt(h[0] / bb);
+    if (iters) *iters = it;
+    if (relres) *relres = rel;
+    FEM_CUDA(cudaGetLastError());
+    return (conv && !bad && rel <= 100.0 * rtol) ? FEM_OK : FEM_ERR_NOCONV;
+}
+
+extern "C" int fem_pcg(fem_ctx *c, const double *csr_vals, const double *b, double *x, double rtol, int max_iter, int *iters,
+                       double *relres, void *cuda_stream) {
+    if (!c || !csr_vals || !b || !x) return FEM_ERR_NULL;
+    if (!c->has_pattern) return FEM_ERR_NO_PATTERN;
+    if (!(rtol > 0.0) || max_iter < 0 || b == x) return FEM_ERR_ARG;
+    int rc = ensure_solver_ws(c, false);
+    if (rc != FEM_OK) return rc;
+    return pcg(c, csr_vals, b, x, rtol, max_iter, iters, relres, (cudaStream_t)cuda_stream);
+}
+
 extern "C" int fem_bicgstab(fem_ctx *c, const double *csr_vals, const double *b, double *x, double rtol, int max_iter, int *iters,
                             double *relres, void *cuda_stream) {
     if (!c || !csr_vals || !b || !x) return FEM_ERR_NULL;
@@ -381,7 +472,7 @@ extern "C" int fem_bicgstab(fem_ctx *c, const double *csr_vals, const double *b,
 
 extern "C" void fem_default_newton_options(fem_newton_options *o) {
     if (!o) return;
-    o->rtol = 1e-9; o->atol = 1e-10; o->max_newton = 25; o->lin_rtol = 1e-10; o->lin_max_iter = 10000;
+    o->rtol = 1e-9; o->atol = 1e-10; o->max_newton = 25; o->lin_rtol = 1e-10; o->lin_max_iter = 10000; o->linear_solver = 0;
 }
 
 // One load increment: K dd = -R, d <- d + dd (Eq.(39)) with identity rows for the constrained DOFs.
@@ -395,7 +486,7 @@ extern "C" int fem_newton_solve(fem_ctx *c, double *u, const double *hist_in, co
     fem_newton_options o;
     fem_default_newton_options(&o);
     if (opt) o = *opt;
-    if (!(o.rtol >= 0.0) || !(o.atol >= 0.0) || o.max_newton < 1 || !(o.lin_rtol > 0.0) || o.lin_max_iter < 1) return FEM_ERR_ARG;
+    if (!(o.rtol >= 0.0) || !(o.atol >= 0.0) || o.max_newton < 1 || !(o.lin_rtol > 0.0) || o.lin_max_iter < 1 || o.linear_solver < 0 || o.linear_solver > 2) return FEM_ERR_ARG;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     int rc = ensure_solver_ws(c, true);
     if (rc != FEM_OK) return rc;
@@ -419,10 +510,20 @@ extern "C" int fem_newton_solve(fem_ctx *c, double *u, const double *hist_in, co
         if (!isfinite(rp.rhs_norm)) break;
         if (rp.rhs_norm <= o.atol || rp.rhs_norm <= o.rtol * rp.rhs_norm0) { rp.converged = 1; result = FEM_OK; break; }
         if (k >= o.max_newton) break;
-        FEM_CUDA(cudaMemsetAsync(dd, 0, sizeof(double) * n, st));
         int its = 0;
-        rc = bicgstab(c, vals, rhs, dd, o.lin_rtol, o.lin_max_iter, &its, nullptr, st);
-        rp.lin_iters_total += its;
+        rc = FEM_ERR_NOCONV;
+        if (o.linear_solver != 1 && !c->opt.fbar) {
+            // standard element: K_ff is symmetric -> CG from the guess dd = rhs on the constrained DOFs, 0 elsewhere
+            FEM_CUDA(cudaMemsetAsync(dd, 0, sizeof(double) * n, st));
+            if (n_bc > 0) k_scatter_bc<<<nblk3(n_bc, 256), 256, 0, st>>>(n_bc, bc_dofs, rhs, dd);
+            rc = pcg(c, vals, rhs, dd, o.lin_rtol, o.lin_max_iter, &its, nullptr, st);
+            rp.lin_iters_total += its;
+        }
+        if (rc == FEM_ERR_NOCONV && (o.linear_solver != 2 || c->opt.fbar)) {   // unsymmetric (F-bar), or CG gave up: BiCGSTAB from zero
+            FEM_CUDA(cudaMemsetAsync(dd, 0, sizeof(double) * n, st));
+            rc = bicgstab(c, vals, rhs, dd, o.lin_rtol, o.lin_max_iter, &its, nullptr, st);
+            rp.lin_iters_total += its;
+        }
         if (rc == FEM_ERR_NOCONV) rp.lin_failures++;
         else if (rc != FEM_OK) return rc;
         k_axpy<<<RED_CTAS, RED_THREADS, 0, st>>>(n, 1.0, dd, u);

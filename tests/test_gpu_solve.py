@@ -84,6 +84,14 @@ def test_bicgstab_against_direct_solve(case):
     assert rel_l2(x.cpu().numpy(), xo) <= 1e-7, (iters, relres)
     x2, it2, _, _ = ctx.bicgstab(vals, rhs, rtol=1e-12, max_iter=20000)
     assert it2 == iters and torch.equal(x, x2)                       # fixed reduction order: bit-identical
+    if not case.endswith("fbar"):
+        # CG on the symmetric reduced system: the guess carries the prescribed values on the constrained DOFs
+        xg = torch.zeros_like(rhs)
+        xg[torch.from_numpy(bc.astype(np.int64)).to(dev)] = rhs[torch.from_numpy(bc.astype(np.int64)).to(dev)]
+        xc, itc, rrc, okc = ctx.pcg(vals, rhs, x=xg.clone(), rtol=1e-12, max_iter=20000)
+        assert okc and rrc <= 1e-10 and rel_l2(xc.cpu().numpy(), xo) <= 1e-7, (itc, rrc)
+        xc2, itc2, _, _ = ctx.pcg(vals, rhs, x=xg.clone(), rtol=1e-12, max_iter=20000)
+        assert itc2 == itc and torch.equal(xc, xc2)
     # zero right-hand side and iteration cap
     x0, it0, rr0, ok0 = ctx.bicgstab(vals, torch.zeros_like(rhs), x=torch.ones_like(rhs))
     assert ok0 and it0 == 0 and float(x0.abs().max()) == 0.0
@@ -91,8 +99,8 @@ def test_bicgstab_against_direct_solve(case):
     assert (not ok1) and it1 == 3
 
 
-@pytest.mark.parametrize("fbar", [0, 1])
-def test_newton_solve_matches_oracle(fbar):
+@pytest.mark.parametrize("fbar,solver", [(0, 0), (0, 1), (1, 0)])
+def test_newton_solve_matches_oracle(fbar, solver):
     import torch
     import paper_2606_17390_b200 as fem
     import oracle.newton as onw
@@ -102,7 +110,7 @@ def test_newton_solve_matches_oracle(fbar):
     mat = torch.from_numpy(fem.mat_from_desc(dict(synth.configs.SWIFT), ne).ravel()).to(dev)
     u = torch.zeros(coords.size, dtype=torch.float64, device=dev)
     u, hout, rep = ctx.newton_solve(u, torch.from_numpy(h0.ravel()).to(dev), mat, torch.from_numpy(bc.astype(np.int32)).to(dev),
-                                    torch.from_numpy(val).to(dev), lin_rtol=1e-12)
+                                    torch.from_numpy(val).to(dev), lin_rtol=1e-12, linear_solver=solver)
     o = onw.newton_solve(coords, conn, np.zeros_like(coords), h0, omat, rp, ci, bc, val, fbar=fbar)
     assert rep["converged"] and o["converged"] and rep["lin_failures"] == 0
     assert rep["newton_iters"] == o["newton_iters"], (rep, o["norms"])
