@@ -61,7 +61,7 @@ def main():
     import synth
     ap = argparse.ArgumentParser()
     ap.add_argument("--steps", type=int, default=10)
-    ap.add_argument("--only", default="1,2,3,3fbar,4,5f,5s")
+    ap.add_argument("--only", default="1,2,3,3fbar,4,5f,5s,e4")
     args = ap.parse_args()
     only = set(args.only.split(","))
     print("| case | elements | DOF | nnz | plastic fraction | local iterations (count per iteration number) | non-converged | "
@@ -77,6 +77,15 @@ def main():
         run_case("config 3, fbar=1", synth.make_config(3), args.steps, fbar=1)
     if "4" in only:
         run_case("config 4 (100^3 void mask, shuffled, per-element material)", synth.make_config(4), args.steps)
+    if "e4" in only:
+        # the paper's largest case: 250 x 150 x 120 elements (13,758,063 DOF by its mesh; "~11.2 M" in the text),
+        # config-3 recipe (same field, peak strain 0.1, x_c = 0.62) on the unit cube
+        from synth import mesh, fields
+        from synth.configs import BASE_SEED, SWIFT, XC
+        coords, conn = mesh.structured_hex_mesh(250, 150, 120)
+        u = fields.scaled_smooth_displacement(BASE_SEED + 3, coords, conn, np.ones(3), 0.1, xc=XC[3])
+        run_case("E4 size (250x150x120), config-3 recipe", dict(coords=np.ascontiguousarray(coords), conn=np.ascontiguousarray(conn), u=u,
+                                                                hist_in=np.zeros((conn.shape[0], 8, 7)), matdesc=dict(SWIFT)), max(2, args.steps // 2))
     if "5f" in only:
         for lv in range(5):
             run_case("config 5 fraction level %d (64^3)" % lv, synth.make_config(5, level=lv, sweep="fraction"), args.steps)

@@ -40,13 +40,13 @@ def test_full_pattern_closed_form(full3):
     assert (d[mask] > 0).all()
 
 
-def test_full_sampled_rows_against_oracle(full3):
+def _compare_sampled_rows(full, n_samples=48):
     import oracle
-    cfg = full3["cfg"]
+    cfg = full["cfg"]
     conn = cfg["conn"]
     nn, ne = cfg["coords"].shape[0], conn.shape[0]
-    nodes = synth.configs.sample_indices(cfg["seed"], nn, 48)
-    rp = full3["row_ptr"].cpu().numpy(); ci = full3["col_idx"].cpu().numpy()
+    nodes = synth.configs.sample_indices(cfg["seed"], nn, n_samples)
+    rp = full["row_ptr"].cpu().numpy(); ci = full["col_idx"].cpu().numpy()
     mask = np.isin(conn, nodes)
     node_elems = {int(n): [] for n in nodes}
     for e in np.nonzero(mask.any(axis=1))[0]:
@@ -55,8 +55,8 @@ def test_full_sampled_rows_against_oracle(full3):
                 node_elems[int(conn[e, a])].append(int(e))
     mat = oracle.mat_from_desc(cfg["matdesc"], ne)
     rows, hist = oracle.assemble_rows(cfg["coords"], conn, cfg["u"], cfg["hist_in"], mat, rp, ci, [int(n) for n in nodes], node_elems)
-    vals = full3["vals"].cpu().numpy(); res = full3["res"].cpu().numpy()
-    hout = full3["hout"].cpu().numpy().reshape(ne, 8, 7)
+    vals = full["vals"].cpu().numpy(); res = full["res"].cpu().numpy()
+    hout = full["hout"].cpu().numpy().reshape(ne, 8, 7)
     g_rows, o_rows, g_res, o_res = [], [], [], []
     for n, (r3, rws) in rows.items():
         for i in range(3):
@@ -67,6 +67,35 @@ def test_full_sampled_rows_against_oracle(full3):
     assert np.abs(np.concatenate(g_res) - np.concatenate(o_res)).max() <= TOL_RES * max(np.abs(np.concatenate(o_res)).max(), scale)
     es = sorted(hist)
     assert rel_l2(np.stack([hout[e] for e in es]), np.stack([hist[e] for e in es])) <= TOL_HIST
+
+
+def test_full_sampled_rows_against_oracle(full3):
+    _compare_sampled_rows(full3)
+
+
+def test_largest_paper_mesh_sampled_rows_against_oracle():
+    """Maximum size: the paper's largest mesh, 250 x 150 x 120 hex8 (13,758,063 DOF, nnz 1,100,439,549 - more
+    than half of the int32 range the pattern uses), config-3 recipe; sampled rows and history against the oracle."""
+    import torch
+    import paper_2606_17390_b200 as fem
+    from synth import mesh, fields
+    coords, conn = mesh.structured_hex_mesh(250, 150, 120)
+    seed = synth.configs.BASE_SEED + 3
+    u = fields.scaled_smooth_displacement(seed, coords, conn, np.ones(3), 0.1, xc=synth.configs.XC[3])
+    cfg = dict(coords=np.ascontiguousarray(coords), conn=np.ascontiguousarray(conn), u=u, hist_in=np.zeros((conn.shape[0], 8, 7)),
+               matdesc=dict(synth.configs.SWIFT), seed=seed)
+    dev = torch.device("cuda:0")
+    ne = conn.shape[0]
+    ctx = fem.FemContext(torch.from_numpy(cfg["coords"]).to(dev), torch.from_numpy(cfg["conn"]).to(dev))
+    row_ptr, col_idx, _ = ctx.build_csr_pattern()
+    assert ctx.nnz == 9 * 751 * 451 * 361 == 1_100_439_549
+    mat = fem.mat_from_desc(cfg["matdesc"], ne)
+    res, vals, hout, stats = ctx.assemble(torch.from_numpy(u.ravel()).to(dev), torch.from_numpy(cfg["hist_in"].ravel()).to(dev),
+                                          torch.from_numpy(mat.ravel()).to(dev), want_stats=True)
+    torch.cuda.synchronize()
+    assert stats["n_nonconverged"] == 0 and stats["n_nonfinite"] == 0 and stats["n_detF_nonpos"] == 0
+    _compare_sampled_rows(dict(cfg=cfg, row_ptr=row_ptr, col_idx=col_idx, res=res, vals=vals, hout=hout), n_samples=32)
+    ctx.close()
 
 
 def test_full_properties(full3):
