@@ -294,7 +294,8 @@ __device__ __forceinline__ int queue_read(const int *queue, unsigned idx) {
 // MODE 0: K^e, R^e go to an HBM scratch (k_gather sums them).  MODE 1: launched once per colour (elist = the colour's
 // elements); K^e, R^e are added in place into csr_vals / residual (no two elements of a launch share a node).
 struct scatter_args {
-    const int *elist;                       // element ids of this launch (MODE 1), nullptr = identity
+    const int *elist;                       // element ids in processing order: a colour's elements (MODE 1), the locality order
+                                            // built at setup for shuffled meshes (MODE 0); nullptr = identity
     const int *eslot;                       // (MODE 0) [e*8+I] -> scratch record of block row I (node-sorted incidence index)
     const int *nb_ptr;                      // node -> first neighbour block; CSR rows of node n start at 9*nb_ptr[n]
     const unsigned char *elem_pos;          // [e][I][K] rank of node K in the neighbour list of node I
@@ -358,7 +359,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
     double xn[3], un[3], hn[7];
     {
         const long long er = chunk * EL_PER_CTA + el_cta, es = (er < n_elems) ? er : n_elems - 1;
-        const long long e0 = (MODE == 1 && sa.elist) ? (long long)sa.elist[es] : es;
+        const long long e0 = (MODE != 2 && sa.elist) ? (long long)sa.elist[es] : es;
         nd_n = conn[e0 * 8 + q];
         if (MODE != 1) slot_n = __ldg(sa.eslot + e0 * 8 + q);
         const double *hin = hist_in + (e0 * 8 + q) * 7;
@@ -370,7 +371,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
 #if EL_PF_DIST > 0
     if (MODE == 0) {   // streaming inputs of the chunk EL_PF_DIST launches ahead -> L2 (they are read exactly once)
         const long long ep = (chunk + EL_PF_DIST) * EL_PER_CTA + el_cta;
-        if (ep < n_elems) {
+        if (ep < n_elems && !sa.elist) {
             asm volatile("prefetch.global.L2 [%0];" ::"l"(conn + ep * 8 + q));
             asm volatile("prefetch.global.L2 [%0];" ::"l"(sa.eslot + ep * 8 + q));
             asm volatile("prefetch.global.L2 [%0];" ::"l"(hist_in + (ep * 8 + q) * 7));
@@ -385,7 +386,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
     const long long e_raw = chunk * EL_PER_CTA + el_cta;
     const bool valid = e_raw < n_elems;
     const long long e_slot = valid ? e_raw : n_elems - 1;
-    const long long e = (MODE == 1 && sa.elist) ? (long long)sa.elist[e_slot] : e_slot;
+    const long long e = (MODE != 2 && sa.elist) ? (long long)sa.elist[e_slot] : e_slot;
     // ---- S2 gather: thread q holds node q of its element (prefetched), history of its Gauss point
     double epn[6];
 #pragma unroll
@@ -1320,7 +1321,7 @@ int fem_launch_assemble(fem_ctx *c, const double *u, const double *hist_in, cons
     k_mat_prep<<<nblk2(n_mat, 128), 128, 0, st>>>(n_mat, mat, c->d_matd);
     FEM_CUDA(cudaEventRecord(c->ev[1], st));
     const int mstride = (n_mat == 1) ? 0 : FEM_MATD;
-    scatter_args sa = {nullptr, c->d_eslot, c->d_nb_ptr, c->d_elem_pos, c->d_first_mask, c->d_first_res, csr_vals, residual,
+    scatter_args sa = {c->mode == 0 ? c->d_eorder : nullptr, c->d_eslot, c->d_nb_ptr, c->d_elem_pos, c->d_first_mask, c->d_first_res, csr_vals, residual,
                        c->d_cnt, c->d_queue, c->d_qctl, c->d_inc_ptr, c->d_kvec};
     if (c->mode == 2) {
         // fused mode: element CTAs count the nodes down and queue completed ones; interleaved gather CTAs and the drain

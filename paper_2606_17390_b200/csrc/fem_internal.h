@@ -16,6 +16,8 @@ struct fem_ctx {
     bool has_pattern = false;
     int *d_inc_ptr = nullptr;    // [n_nodes+1]   node -> incident (element,local node) list
     int *d_inc = nullptr;        // [8*n_elems]   e*8+I, ascending within a node
+    int *d_eorder = nullptr;     // [n_elems] processing order of the elements (ascending smallest node id) when the input order
+                                 //   is not local (shuffled meshes); null = input order
     int *d_eslot = nullptr;      // [8*n_elems]   inverse of d_inc: index j of (e,I) in the node-sorted incidence list
     int *d_nb_ptr = nullptr;     // [n_nodes+1]   node -> sorted neighbour-node list
     int *d_nb = nullptr;         // [nnz/9]

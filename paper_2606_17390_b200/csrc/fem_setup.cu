@@ -4,6 +4,7 @@
 // neighbour node m (ascending) and k = 0..2.  The whole build runs on the device; integer atomics are used only for
 // counting / unordered filling, and every list is sorted afterwards, so the result is deterministic.
 #include "fem_internal.h"
+#include <cub/device/device_radix_sort.cuh>
 #include <cub/device/device_scan.cuh>
 #include <math.h>
 #include <new>
@@ -149,6 +150,20 @@ __global__ void k_elem_slot(long long n_elems, const int *__restrict__ conn, con
     }
 }
 
+// locality key of an element = its smallest node id; counts the descents of the key along the input order
+__global__ void k_elem_key(long long n_elems, const int *__restrict__ conn, int *key, int *ids, unsigned long long *descents) {
+    long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (e >= n_elems) return;
+    int k = conn[e * 8];
+    for (int a = 1; a < 8; a++) k = min(k, conn[e * 8 + a]);
+    key[e] = k; ids[e] = (int)e;
+    if (e > 0) {
+        int kp = conn[(e - 1) * 8];
+        for (int a = 1; a < 8; a++) kp = min(kp, conn[(e - 1) * 8 + a]);
+        if (kp > k) atomicAdd(descents, 1ull);
+    }
+}
+
 // inverse of the node-sorted incidence list: eslot[e*8+I] = j with inc[j] = e*8+I
 __global__ void k_eslot(long long n_elems, const int *__restrict__ inc, int *eslot) {
     long long j = blockIdx.x * (long long)blockDim.x + threadIdx.x;
@@ -226,7 +241,7 @@ extern "C" int fem_hill_from_lankford(double r0, double r45, double r90, double 
 static void ctx_free(fem_ctx *c) {
     if (!c) return;
     void *ptrs[] = {c->d_coords, c->d_conn, c->d_inc_ptr, c->d_inc, c->d_nb_ptr, c->d_nb, c->d_row_ptr, c->d_col_idx,
-                    c->d_eslot, c->d_diagpos, c->d_sw, c->d_part, c->d_scal, c->d_nw, c->d_nw_vals, c->d_cnt_init, c->d_cnt, c->d_queue_init, c->d_queue, c->d_qctl, c->d_elem_pos, c->d_elem_slot, c->d_kvec, c->d_elist, c->d_first_mask, c->d_first_res, c->d_Ke, c->d_Re, c->d_matd, c->d_stats, c->d_u, c->d_hin, c->d_hout,
+                    c->d_eslot, c->d_eorder, c->d_diagpos, c->d_sw, c->d_part, c->d_scal, c->d_nw, c->d_nw_vals, c->d_cnt_init, c->d_cnt, c->d_queue_init, c->d_queue, c->d_qctl, c->d_elem_pos, c->d_elem_slot, c->d_kvec, c->d_elist, c->d_first_mask, c->d_first_res, c->d_Ke, c->d_Re, c->d_matd, c->d_stats, c->d_u, c->d_hin, c->d_hout,
                     c->d_mat, c->d_res, c->d_vals};
     for (void *p : ptrs) if (p) cudaFree(p);
     for (int i = 0; i < 4; i++) if (c->ev[i]) cudaEventDestroy(c->ev[i]);
@@ -350,6 +365,27 @@ extern "C" int fem_build_csr_pattern(fem_ctx *c, long long *n_rows, long long *n
                 rc = fem_build_colouring(c);
                 if (rc != FEM_OK) break;
             } else {   // scratch for the two-kernel mode (destination-major: one 72-double record per incidence entry)
+                {   // processing order: when more than 5 % of the elements step back in node numbering (shuffled input), the element
+                    // kernel walks the elements by ascending smallest node id (neighbouring CTAs then share nodes in L2 and
+                    // write neighbouring scratch records); results do not depend on it
+                    int *key = nullptr, *key2 = nullptr, *ids = nullptr;
+                    unsigned long long *dsc = nullptr, hd = 0;
+                    TRY(cudaMalloc(&key, sizeof(int) * ne)); TRY(cudaMalloc(&key2, sizeof(int) * ne)); TRY(cudaMalloc(&ids, sizeof(int) * ne));
+                    TRY(cudaMalloc(&dsc, sizeof(unsigned long long)));
+                    TRY(cudaMemset(dsc, 0, sizeof(unsigned long long)));
+                    k_elem_key<<<nblk(ne, 256), 256>>>(ne, c->d_conn, key, ids, dsc);
+                    TRY(cudaMemcpy(&hd, dsc, sizeof(hd), cudaMemcpyDeviceToHost));
+                    if (hd * 20 > (unsigned long long)ne) {
+                        void *t2 = nullptr; size_t t2b = 0;
+                        TRY(cudaMalloc(&c->d_eorder, sizeof(int) * ne));
+                        TRY(cub::DeviceRadixSort::SortPairs(nullptr, t2b, key, key2, ids, c->d_eorder, (int)ne));
+                        TRY(cudaMalloc(&t2, t2b));
+                        TRY(cub::DeviceRadixSort::SortPairs(t2, t2b, key, key2, ids, c->d_eorder, (int)ne));
+                        TRY(cudaDeviceSynchronize());
+                        cudaFree(t2);
+                    }
+                    cudaFree(key); cudaFree(key2); cudaFree(ids); cudaFree(dsc);
+                }
                 TRY(cudaMalloc(&c->d_eslot, sizeof(int) * 8 * ne));
                 k_eslot<<<nblk(8 * ne, 256), 256>>>(ne, c->d_inc, c->d_eslot);
                 TRY(cudaGetLastError());
