@@ -963,15 +963,15 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
     //      sm_100a, but one issue keeps the pipe busy for 16 cycles, so the contraction no longer stalls on
     //      dependent-issue latency, and the accumulators shrink from 45 to 12 doubles per thread.
     const int I = q;
-    double rq[FBAR ? 8 : 1][3];
+    double rq[(FBAR && MODE == 1) ? 8 : 1][3];
     if (FBAR) {
 #pragma unroll
-        for (int qq = 0; qq < 8; qq++) {
+        for (int qq = 0; qq < ((MODE == 1) ? 8 : 0); qq++) {
             const double *sq = se + qq;
             const double gI[3] = {sq[GGX(I, 0)], sq[GGX(I, 1)], sq[GGX(I, 2)]};
 #pragma unroll
             for (int i = 0; i < 3; i++)
-                rq[FBAR ? qq : 0][i] = sq[SM_YY + (3 * i + 0) * 8] * gI[0] + sq[SM_YY + (3 * i + 1) * 8] * gI[1] +
+                rq[(FBAR && MODE == 1) ? qq : 0][i] = sq[SM_YY + (3 * i + 0) * 8] * gI[0] + sq[SM_YY + (3 * i + 1) * 8] * gI[1] +
                                        sq[SM_YY + (3 * i + 2) * 8] * gI[2];
         }
         // gbar_Kk = sum_q (w_q J_q / (Jbar V)) g^q_Kk for node K = I
@@ -1019,28 +1019,80 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
                                          : "+d"(C[p][0]), "+d"(C[p][1]) : "d"(g[h][a_]), "d"(hv));
                         }
                 }
-            if (!FBAR && MODE != 1) {
-                // ---- phase 3 (standard element, scratch modes): the accumulators go straight to the destination-major scratch.
+            if (MODE != 1) {
+                // ---- phase 3 (scratch modes): the accumulators go straight to the destination-major scratch.
                 //      Lane holds K^{ik}[gid][2 tig + j] = component (i,k) of block (gid, 2 tig + j): one 16-byte store into block
-                //      row gid; for i != k it is also component (k,i) of block (2 tig + j, gid): two 8-byte stores (the 8
-                //      lanes of equal tig fill 64 contiguous bytes).  Every 32-byte sector is written whole.
+                //      row gid.  Standard element: for i != k it is also component (k,i) of block (2 tig + j, gid): two 8-byte
+                //      stores (the 8 lanes of equal tig fill 64 contiguous bytes).  Every 32-byte sector is written whole.
                 const int w_el = (tid >> 5) * 4 + el;
                 const bool el_ok = chunk * EL_PER_CTA + w_el < n_elems;
                 const long long sd = __shfl_sync(0xffffffffu, my_slot, el * 8 + gid);
-                const long long st0 = __shfl_sync(0xffffffffu, my_slot, el * 8 + 2 * tig);
-                const long long st1 = __shfl_sync(0xffffffffu, my_slot, el * 8 + 2 * tig + 1);
-                if (el_ok) {
-                    int p = 0;
+                if (!FBAR) {
+                    const long long st0 = __shfl_sync(0xffffffffu, my_slot, el * 8 + 2 * tig);
+                    const long long st1 = __shfl_sync(0xffffffffu, my_slot, el * 8 + 2 * tig + 1);
+                    if (el_ok) {
+                        int p = 0;
+#pragma unroll
+                        for (int i = 0; i < 3; i++)
+#pragma unroll
+                            for (int k = i; k < 3; k++, p++) {
+                                *reinterpret_cast<double2 *>(Ke + sd * 72 + (3 * i + k) * 8 + 2 * tig) = make_double2(C[p][0], C[p][1]);
+                                if (i != k) {
+                                    Ke[st0 * 72 + (3 * k + i) * 8 + gid] = C[p][0];
+                                    Ke[st1 * 72 + (3 * k + i) * 8 + gid] = C[p][1];
+                                }
+                            }
+                    }
+                } else {
+                    // F-bar: K^e_(Ii)(Kk) += sum_q r^q_Ii (gbar_Kk - g^q_Kk), r^q_Ii = sum_a Y^q_ia G^q_Ia
+                    // (Y carries w_q/3): for each (i,k) an 8 x 8 x 8 product over q, two more DMMA steps per pair of the nine
+                    // (the term is not symmetric).  A fragment: r^q_{gid,i}; B fragment: gbar_{gid,k} - g^q_{gid,k}; q = 4 h + tig.
+                    double ra[2][3], hb[2][3];
+#pragma unroll
+                    for (int h = 0; h < 2; h++)
+#pragma unroll
+                        for (int i = 0; i < 3; i++) {
+                            const double *yy = sx + SM_YY + 4 * h + tig;
+                            ra[h][i] = fma(yy[(3 * i + 2) * 8], g[h][2], fma(yy[(3 * i + 1) * 8], g[h][1], yy[(3 * i) * 8] * g[h][0]));
+                            hb[h][i] = sx[SM_GB + 3 * gid + i] - sx[SM_GQ + (3 * gid + i) * 8 + 4 * h + tig];
+                        }
+                    double D[3][3][2];
 #pragma unroll
                     for (int i = 0; i < 3; i++)
 #pragma unroll
-                        for (int k = i; k < 3; k++, p++) {
-                            *reinterpret_cast<double2 *>(Ke + sd * 72 + (3 * i + k) * 8 + 2 * tig) = make_double2(C[p][0], C[p][1]);
-                            if (i != k) {
-                                Ke[st0 * 72 + (3 * k + i) * 8 + gid] = C[p][0];
-                                Ke[st1 * 72 + (3 * k + i) * 8 + gid] = C[p][1];
-                            }
+                        for (int k = 0; k < 3; k++) {
+                            D[i][k][0] = D[i][k][1] = 0.0;
+#pragma unroll
+                            for (int h = 0; h < 2; h++)
+                                asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                                             : "+d"(D[i][k][0]), "+d"(D[i][k][1]) : "d"(ra[h][i]), "d"(hb[h][k]));
                         }
+                    // symmetric part: pair (i,k), i <= k, is held as is; for i > k it is the transpose of pair (k,i), i.e. the
+                    // accumulator of the lane that holds row 2 tig + j, column gid
+                    {
+                        int p = 0;
+#pragma unroll
+                        for (int i = 0; i < 3; i++)
+#pragma unroll
+                            for (int k = i; k < 3; k++, p++) {
+                                D[i][k][0] += C[p][0]; D[i][k][1] += C[p][1];
+                                if (i != k) {
+#pragma unroll
+                                    for (int j = 0; j < 2; j++) {
+                                        const int src = (2 * tig + j) * 4 + (gid >> 1);
+                                        const double c0 = __shfl_sync(0xffffffffu, C[p][0], src), c1 = __shfl_sync(0xffffffffu, C[p][1], src);
+                                        D[k][i][j] += (gid & 1) ? c1 : c0;
+                                    }
+                                }
+                            }
+                    }
+                    if (el_ok) {
+#pragma unroll
+                        for (int i = 0; i < 3; i++)
+#pragma unroll
+                            for (int k = 0; k < 3; k++)
+                                *reinterpret_cast<double2 *>(Ke + sd * 72 + (3 * i + k) * 8 + 2 * tig) = make_double2(D[i][k][0], D[i][k][1]);
+                    }
                 }
             } else {
                 __syncwarp();   // every lane has read this element's G^ and A^: the staging below overlays them
@@ -1061,13 +1113,13 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
         __syncwarp();
     }
     PHASE_SYNC_N(9);
-    if (FBAR) {
+    if (FBAR && MODE == 1) {
         // K^e_(Ii)(Kk) += sum_q w_q/3 r^q_Ii (gbar_Kk - g^q_Kk)   (unsymmetric rank-1 terms)
         double rs[3] = {0, 0, 0};
 #pragma unroll
         for (int qq = 0; qq < 8; qq++)
 #pragma unroll
-            for (int i = 0; i < 3; i++) rs[i] += rq[FBAR ? qq : 0][i];
+            for (int i = 0; i < 3; i++) rs[i] += rq[(FBAR && MODE == 1) ? qq : 0][i];
 #pragma unroll 1
         for (int K = 0; K < 8; K++)
 #pragma unroll
@@ -1077,8 +1129,8 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
 #pragma unroll
                 for (int qq = 0; qq < 8; qq++) {
                     const double g = se[SM_GQ + (3 * K + k) * 8 + qq];
-                    t0 = fma(-rq[FBAR ? qq : 0][0], g, t0); t1 = fma(-rq[FBAR ? qq : 0][1], g, t1);
-                    t2 = fma(-rq[FBAR ? qq : 0][2], g, t2);
+                    t0 = fma(-rq[(FBAR && MODE == 1) ? qq : 0][0], g, t0); t1 = fma(-rq[(FBAR && MODE == 1) ? qq : 0][1], g, t1);
+                    t2 = fma(-rq[(FBAR && MODE == 1) ? qq : 0][2], g, t2);
                 }
                 se[KSX(I, K, 0 + k)] += t0;
                 se[KSX(I, K, 3 + k)] += t1;
@@ -1093,22 +1145,6 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
             ro[0] = rI[0]; ro[1] = rI[1]; ro[2] = rI[2];
         }
         __syncwarp();
-        // F-bar: copy-out of the warp's 4 elements x 8 staged records of 576 bytes, 16 bytes per lane per step
-        if (FBAR) {
-            const int w_el0 = (tid >> 5) * 4;
-            const long long e0 = chunk * EL_PER_CTA + w_el0;
-#pragma unroll
-            for (int it = 0; it < 9; it++) {
-                const int g = it * 32 + lane, rec = g / 36, off = g - rec * 36;
-#pragma unroll
-                for (int el = 0; el < 4; el++) {
-                    const int slot = __shfl_sync(0xffffffffu, my_slot, el * 8 + rec);
-                    if (e0 + el < n_elems)
-                        reinterpret_cast<double2 *>(Ke + (long long)slot * 72)[off] =
-                            reinterpret_cast<const double2 *>(sm + (w_el0 + el) * ES + SM_KS)[g];
-                }
-            }
-        }
         if (MODE == 2) {
             // publish: the records above become visible (fence), then each (element, node) counts its node down; whoever
             // brings a node to zero queues it for the gather CTAs (one ticket request per warp)
