@@ -32,6 +32,8 @@ def main():
     ap.add_argument("--lin-rtol", type=float, default=1e-8)
     ap.add_argument("--dt", default="0.002,0.005", help="load fractions of the Newton runs, each from the undeformed state")
     ap.add_argument("--path", default="0.002x8", help="load path: step size x number of steps, history and displacement carried over")
+    ap.add_argument("--full", type=float, default=0.0, help="if > 0: run the whole benchmark loading (right face to 0.2, 0.1 mm) with "
+                    "adaptive stepping (the paper's dt_initial 1e-3, dt_max 5e-2, cut-back on failure, :485) for at most this many seconds")
     args = ap.parse_args()
     n = args.n
     dev = torch.device("cuda:0")
@@ -124,6 +126,42 @@ def main():
     dt = time.perf_counter() - t_path
     print("| path total | %d Newton iterations | %d linear iterations | %.2f s = %.2f s per Newton iteration |"
           % (tot_newton, tot_lin, dt, dt / max(tot_newton, 1)))
+
+    # ---- 5. the whole benchmark loading with the paper's adaptive stepping parameters (host control flow)
+    if args.full > 0:
+        t, dt, dt_max, dt_min = 0.0, 1e-3, 5e-2, 1e-5
+        u = torch.zeros(nr, dtype=torch.float64, device=dev)
+        h_a = torch.zeros(56 * ne, dtype=torch.float64, device=dev)
+        h_b = torch.empty_like(h_a)
+        steps = newton = lin = rejected = 0
+        t_start = time.perf_counter()
+        print("\n| step | load fraction | dt | Newton iterations | linear iterations | s | plastic fraction | result |")
+        print("|---|---|---|---|---|---|---|---|")
+        while t < 1.0 - 1e-12 and time.perf_counter() - t_start < args.full:
+            dt = min(dt, 1.0 - t)
+            t0 = time.perf_counter()
+            u, h_b, rep = ctx.newton_solve(u, h_a, mat, bc_d, torch.from_numpy(full * (t + dt)).to(dev), hist_out=h_b,
+                                           lin_rtol=args.lin_rtol, lin_max_iter=20000, rtol=1e-8, max_newton=12)
+            torch.cuda.synchronize()
+            el = time.perf_counter() - t0
+            st = rep["last_stats"]
+            ok = rep["converged"] and rep["lin_failures"] == 0
+            print("| %d | %.5f | %.2e | %d | %d | %.2f | %.3f | %s |" % (steps + 1, t + dt, dt, rep["newton_iters"], rep["lin_iters_total"], el,
+                                                                  st["n_plastic"] / (8.0 * ne), "ok" if ok else "rejected"), flush=True)
+            newton += rep["newton_iters"]; lin += rep["lin_iters_total"]
+            if ok:
+                t += dt; steps += 1
+                h_a, h_b = h_b, h_a
+                if rep["newton_iters"] <= 6:
+                    dt = min(dt * 1.5, dt_max)
+            else:
+                rejected += 1
+                dt *= 0.5
+                if dt < dt_min:
+                    break
+        tot = time.perf_counter() - t_start
+        print("| total | reached %.4f of the load | | %d (incl. rejected steps) | %d | %.1f | | %d steps accepted, %d rejected |"
+              % (t, newton, lin, tot, steps, rejected))
 
 
 if __name__ == "__main__":

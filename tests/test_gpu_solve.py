@@ -145,3 +145,28 @@ def test_newton_patch_solution_and_error_paths():
         ctx.newton_solve(u, hin, mat, bad, torch.zeros(2, dtype=torch.float64, device=dev))
     with pytest.raises(fem.FemError):
         ctx.apply_dirichlet(bad, torch.zeros(ctx.nnz, dtype=torch.float64, device=dev))
+
+
+def test_load_path_with_history_matches_oracle():
+    """Three load steps on the clamped cube, converged state and history carried from step to step (the protocol of the
+    paper's benchmark): displacement and history after the last step against the oracle's own path."""
+    import torch
+    import paper_2606_17390_b200 as fem
+    import oracle.newton as onw
+    coords, conn, omat, rp, ci, h0, bc, val = clamped_shear_problem()
+    ctx, dev = _ctx(coords, conn)
+    ne = conn.shape[0]
+    mat = torch.from_numpy(fem.mat_from_desc(dict(synth.configs.SWIFT), ne).ravel()).to(dev)
+    bc_d = torch.from_numpy(bc.astype(np.int32)).to(dev)
+    u = torch.zeros(coords.size, dtype=torch.float64, device=dev)
+    h_a = torch.zeros(56 * ne, dtype=torch.float64, device=dev)
+    uo, ho = np.zeros_like(coords), h0.copy()
+    for frac in (0.3, 0.7, 1.0):
+        u, h_b, rep = ctx.newton_solve(u, h_a, mat, bc_d, torch.from_numpy(val * frac).to(dev), lin_rtol=1e-12)
+        assert rep["converged"]
+        h_a = h_b
+        o = onw.newton_solve(coords, conn, uo, ho, omat, rp, ci, bc, val * frac)
+        assert o["converged"]
+        uo, ho = o["u"], o["hist_out"]
+    assert rel_l2(u.cpu().numpy(), uo) <= 1e-8 and rel_l2(h_a.cpu().numpy(), ho) <= 1e-7
+    assert float(h_a.view(-1, 7)[:, 6].max()) > 0.01          # the path is well into the plastic range
