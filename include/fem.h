@@ -176,6 +176,10 @@ int fem_bicgstab(fem_ctx *c, const double *csr_vals, const double *b, double *x,
 int fem_pcg(fem_ctx *c, const double *csr_vals, const double *b, double *x, double rtol, int max_iter, int *iters,
             double *relres, void *cuda_stream);
 
+/* out = a x + b y on DOF vectors (dev [n_rows]; out may alias x or y).  For the caller's load-step control, e.g. the
+ * extrapolated initial guess u + (u - u_prev) dt/dt_prev of the paper's time stepping. */
+int fem_lincomb(fem_ctx *c, double a, const double *x, double b, const double *y, double *out, void *cuda_stream);
+
 typedef struct {
     double rtol;      /* Newton stops when ||rhs||_2 <= rtol * ||rhs of iteration 0||_2 ... */
     double atol;      /* ... or <= atol (rhs = -R on free DOFs, prescribed - current on constrained DOFs); defaults 1e-9, 1e-10 */

@@ -9,7 +9,7 @@ NPAR = 16
 
 ABI_SYMBOLS = ["fem_default_options", "fem_setup", "fem_build_csr_pattern", "fem_assemble", "fem_assemble_host",
                "fem_last_kernel_ms", "fem_launches_per_assemble", "fem_probe_fp64_peak", "fem_destroy", "fem_strerror",
-               "fem_last_cuda_error", "fem_hill_from_lankford", "fem_spmv", "fem_apply_dirichlet", "fem_bicgstab", "fem_pcg",
+               "fem_last_cuda_error", "fem_hill_from_lankford", "fem_spmv", "fem_apply_dirichlet", "fem_bicgstab", "fem_pcg", "fem_lincomb",
                "fem_default_newton_options", "fem_newton_solve"]
 
 
@@ -93,6 +93,7 @@ def lib():
         L.fem_apply_dirichlet.argtypes = [vp, ll, vp, vp, vp, vp, vp]
         L.fem_bicgstab.argtypes = [vp, vp, vp, vp, C.c_double, C.c_int, C.POINTER(C.c_int), dp, vp]
         L.fem_pcg.argtypes = [vp, vp, vp, vp, C.c_double, C.c_int, C.POINTER(C.c_int), dp, vp]
+        L.fem_lincomb.argtypes = [vp, C.c_double, vp, C.c_double, vp, vp, vp]
         L.fem_default_newton_options.argtypes = [C.POINTER(FemNewtonOptions)]
         L.fem_default_newton_options.restype = None
         L.fem_newton_solve.argtypes = [vp, vp, vp, vp, ll, ll, vp, vp, vp, C.POINTER(FemNewtonOptions),
@@ -264,6 +265,15 @@ class FemContext:
         if rc not in (0, -11):
             _check(rc, "fem_bicgstab")
         return x, it.value, rr.value, rc == 0
+
+    def lincomb(self, a, x, b, y, out=None):
+        """fem_lincomb: out = a x + b y on DOF vectors."""
+        torch = _torch()
+        if out is None:
+            out = torch.empty(self.n_rows, dtype=torch.float64, device=self.device)
+        _check(lib().fem_lincomb(self._h, float(a), _ptr(x, torch.float64, self.n_rows, "x"), float(b), _ptr(y, torch.float64, self.n_rows, "y"),
+                                 _ptr(out, torch.float64, self.n_rows, "out"), _stream_ptr()), "fem_lincomb")
+        return out
 
     def pcg(self, csr_vals, b, x=None, rtol=1e-10, max_iter=10000):
         """fem_pcg: returns (x, iters, relres, converged).  x must hold b[d] on Dirichlet DOFs d (see include/fem.h)."""

@@ -470,6 +470,17 @@ extern "C" int fem_bicgstab(fem_ctx *c, const double *csr_vals, const double *b,
     return bicgstab(c, csr_vals, b, x, rtol, max_iter, iters, relres, (cudaStream_t)cuda_stream);
 }
 
+__global__ void k_lincomb(long long n, double a, const double *__restrict__ x, double b, const double *__restrict__ y, double *out) {
+    for (long long j = blockIdx.x * (long long)blockDim.x + threadIdx.x; j < n; j += (long long)gridDim.x * blockDim.x)
+        out[j] = fma(a, x[j], b * y[j]);
+}
+extern "C" int fem_lincomb(fem_ctx *c, double a, const double *x, double b, const double *y, double *out, void *cuda_stream) {
+    if (!c || !x || !y || !out) return FEM_ERR_NULL;
+    k_lincomb<<<RED_CTAS, RED_THREADS, 0, (cudaStream_t)cuda_stream>>>(c->n_rows, a, x, b, y, out);
+    FEM_CUDA(cudaGetLastError());
+    return FEM_OK;
+}
+
 extern "C" void fem_default_newton_options(fem_newton_options *o) {
     if (!o) return;
     o->rtol = 1e-9; o->atol = 1e-10; o->max_newton = 25; o->lin_rtol = 1e-10; o->lin_max_iter = 10000; o->linear_solver = 0;

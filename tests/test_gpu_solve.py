@@ -140,6 +140,8 @@ def test_newton_patch_solution_and_error_paths():
     u2, _, rep2 = ctx.newton_solve(u_in.clone(), hin, mat, torch.from_numpy(bc).to(dev), torch.from_numpy(exact.ravel()[bc]).to(dev),
                                    max_newton=1)
     assert not rep2["converged"] and rep2["newton_iters"] == 1 and torch.equal(u2, u_in)
+    w = ctx.lincomb(2.0, u_in, -0.5, u)
+    assert torch.equal(w, torch.addcmul(-0.5 * u, u_in, torch.full_like(u_in, 2.0))) or rel_l2(w.cpu().numpy(), (2.0 * u_in - 0.5 * u).cpu().numpy()) <= 1e-16
     bad = torch.tensor([0, 3 * coords.shape[0]], dtype=torch.int32, device=dev)      # DOF out of range
     with pytest.raises(fem.FemError):
         ctx.newton_solve(u, hin, mat, bad, torch.zeros(2, dtype=torch.float64, device=dev))
