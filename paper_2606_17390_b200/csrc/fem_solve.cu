@@ -9,7 +9,12 @@
 
 #define RED_CTAS 1184      // 148 SMs x 8 CTAs of 256 threads for the vector kernels (fixed: part of the reduction order)
 #define RED_THREADS 256
+#define SPMV_CTAS 4736     // 148 SMs x 32 CTAs of 8 warps: grid-stride over the nodes, so the dot partials stay few
 
+static inline unsigned spmv_grid(const fem_ctx *c) {
+    const long long need = (c->n_nodes + 7) / 8;
+    return (unsigned)(need < SPMV_CTAS ? need : SPMV_CTAS);
+}
 static inline unsigned nblk3(long long n, int bs) { return (unsigned)((n + bs - 1) / bs); }
 
 // ------------------------------------------------------------------------------------------------ small kernels
@@ -103,10 +108,11 @@ __global__ void __launch_bounds__(256)
 k_spmv(long long n_nodes, const int *__restrict__ nb_ptr, const int *__restrict__ nb, const double *__restrict__ vals,
        const double *__restrict__ x, double *__restrict__ y, const double *__restrict__ w, double *__restrict__ part) {
     __shared__ double smem[2 * 32];
-    const long long n = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const int lane = threadIdx.x & 31;
-    double a0 = 0.0, a1 = 0.0, a2 = 0.0;
-    if (n < n_nodes) {
+    const long long warps = ((long long)gridDim.x * blockDim.x) >> 5;
+    double d[2] = {0.0, 0.0};   // lane 0: this warp's share of the dot products (fixed node order => fixed summation order)
+    for (long long n = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5; n < n_nodes; n += warps) {
+        double a0 = 0.0, a1 = 0.0, a2 = 0.0;
         const int o = nb_ptr[n], len = nb_ptr[n + 1] - o;
         const double *base = vals + 9LL * o;
         for (int pos = lane; pos < len; pos += 32) {
@@ -117,21 +123,20 @@ k_spmv(long long n_nodes, const int *__restrict__ nb_ptr, const int *__restrict_
             a1 = fma(r1[2], x2, fma(r1[1], x1, fma(r1[0], x0, a1)));
             a2 = fma(r2[2], x2, fma(r2[1], x1, fma(r2[0], x0, a2)));
         }
-    }
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-        a0 += __shfl_xor_sync(0xffffffffu, a0, o); a1 += __shfl_xor_sync(0xffffffffu, a1, o); a2 += __shfl_xor_sync(0xffffffffu, a2, o);
-    }
-    double d[2] = {0.0, 0.0};
-    if (n < n_nodes && lane == 0) {
-        y[3 * n] = a0; y[3 * n + 1] = a1; y[3 * n + 2] = a2;
-        if (DOT) {
-            const double w0 = w[3 * n], w1 = w[3 * n + 1], w2 = w[3 * n + 2];
-            d[0] = a0 * w0 + a1 * w1 + a2 * w2;
-            d[1] = a0 * a0 + a1 * a1 + a2 * a2;
+        for (int o2 = 16; o2 > 0; o2 >>= 1) {
+            a0 += __shfl_xor_sync(0xffffffffu, a0, o2); a1 += __shfl_xor_sync(0xffffffffu, a1, o2); a2 += __shfl_xor_sync(0xffffffffu, a2, o2);
+        }
+        if (lane == 0) {
+            y[3 * n] = a0; y[3 * n + 1] = a1; y[3 * n + 2] = a2;
+            if (DOT) {
+                const double w0 = w[3 * n], w1 = w[3 * n + 1], w2 = w[3 * n + 2];
+                d[0] += a0 * w0 + a1 * w1 + a2 * w2;
+                d[1] += a0 * a0 + a1 * a1 + a2 * a2;
+            }
         }
     }
-    if (DOT) {   // lane 0 of each warp holds the node's contribution; warps summed in ascending order
+    if (DOT) {   // lane 0 of each warp holds its share; warps summed in ascending order
         const int wi = threadIdx.x >> 5;
         if (lane == 0) { smem[wi] = d[0]; smem[32 + wi] = d[1]; }
         __syncthreads();
@@ -197,13 +202,45 @@ k_bicg_xr(long long n, double alpha, double omega, const double *__restrict__ y,
     cta_reduce<2>(a, smem);
     if (threadIdx.x == 0) { part[2LL * blockIdx.x] = a[0]; part[2LL * blockIdx.x + 1] = a[1]; }
 }
+// ---- CG scalars stay on the device (no host round trip per iteration).  sc[0] = (r,z), sc[1] = alpha, sc[2] = beta,
+//      sc[3] = (r,r), sc[4] = tol^2 (b,b), sc[5] = done flag (1 converged, 2 breakdown), sc[6] = iterations performed.
+// after q = K p: alpha = (r,z) / (p,q); a solve that is done keeps alpha = 0, so later iterations of the batch change nothing
+__global__ void __launch_bounds__(1024) k_cg_alpha(const double *__restrict__ part, long long count, double *sc) {
+    __shared__ double smem[2 * 32];
+    double v[2] = {0.0, 0.0};
+    for (long long j = threadIdx.x; j < count; j += blockDim.x) { v[0] += part[2 * j]; v[1] += part[2 * j + 1]; }
+    cta_reduce<2>(v, smem);
+    if (threadIdx.x == 0) {
+        const double pq = v[0];
+        if (sc[5] == 0.0 && (!(pq > 0.0) || !isfinite(pq))) sc[5] = 2.0;
+        sc[1] = (sc[5] == 0.0) ? sc[0] / pq : 0.0;
+        if (sc[5] == 0.0) sc[6] += 1.0;
+    }
+}
+// after the update: beta = (r,z)_new / (r,z); convergence and breakdown tests
+__global__ void __launch_bounds__(1024) k_cg_beta(const double *__restrict__ part, long long count, double *sc) {
+    __shared__ double smem[2 * 32];
+    double v[2] = {0.0, 0.0};
+    for (long long j = threadIdx.x; j < count; j += blockDim.x) { v[0] += part[2 * j]; v[1] += part[2 * j + 1]; }
+    cta_reduce<2>(v, smem);
+    if (threadIdx.x == 0 && sc[5] == 0.0) {
+        const double rz_new = v[0], rr = v[1];
+        sc[3] = rr;
+        if (rr <= sc[4]) sc[5] = 1.0;
+        else if (!(rz_new > 0.0) || !isfinite(rz_new)) sc[5] = 2.0;
+        sc[2] = rz_new / sc[0];
+        sc[0] = rz_new;
+    }
+}
 // ---- preconditioned CG vector kernels
 // x += alpha p ; r -= alpha q ; z = M^-1 r ; partials (r, z), (r, r)
 __global__ void __launch_bounds__(RED_THREADS)
-k_cg_update(long long n, double alpha, const double *__restrict__ p, const double *__restrict__ q, const double *__restrict__ dinv,
-            double *__restrict__ x, double *__restrict__ r, double *__restrict__ z, double *__restrict__ part) {
+k_cg_update(long long n, double alpha_h, const double *__restrict__ sc, const double *__restrict__ p, const double *__restrict__ q,
+            const double *__restrict__ dinv, double *__restrict__ x, double *__restrict__ r, double *__restrict__ z,
+            double *__restrict__ part) {
     __shared__ double smem[2 * 32];
     double a[2] = {0.0, 0.0};
+    const double alpha = sc ? sc[1] : alpha_h;
     for (long long j = blockIdx.x * (long long)blockDim.x + threadIdx.x; j < n; j += (long long)gridDim.x * blockDim.x) {
         x[j] = fma(alpha, p[j], x[j]);
         const double rj = fma(-alpha, q[j], r[j]), zj = dinv[j] * rj;
@@ -214,7 +251,8 @@ k_cg_update(long long n, double alpha, const double *__restrict__ p, const doubl
     if (threadIdx.x == 0) { part[2LL * blockIdx.x] = a[0]; part[2LL * blockIdx.x + 1] = a[1]; }
 }
 // p = z + beta p
-__global__ void k_cg_p(long long n, double beta, const double *__restrict__ z, double *__restrict__ p) {
+__global__ void k_cg_p(long long n, double beta_h, const double *__restrict__ sc, const double *__restrict__ z, double *__restrict__ p) {
+    const double beta = sc ? sc[2] : beta_h;
     for (long long j = blockIdx.x * (long long)blockDim.x + threadIdx.x; j < n; j += (long long)gridDim.x * blockDim.x)
         p[j] = fma(beta, p[j], z[j]);
 }
@@ -245,7 +283,7 @@ static int ensure_solver_ws(fem_ctx *c, bool newton) {
         FEM_CUDA(cudaDeviceSynchronize());
     }
     if (!c->d_sw) {
-        const long long spmv_ctas = (c->n_nodes + 7) / 8;
+        const long long spmv_ctas = spmv_grid(c);
         c->n_part = 2 * (spmv_ctas > RED_CTAS ? spmv_ctas : RED_CTAS);
         FEM_CUDA(cudaMalloc(&c->d_sw, sizeof(double) * 9 * n));
         FEM_CUDA(cudaMalloc(&c->d_part, sizeof(double) * c->n_part));
@@ -269,7 +307,7 @@ static int fetch_sums(fem_ctx *c, long long count, double *host, cudaStream_t st
 
 template <int DOT>
 static void launch_spmv(fem_ctx *c, const double *vals, const double *x, double *y, const double *w, cudaStream_t st) {
-    k_spmv<DOT><<<nblk3(c->n_nodes, 8), 256, 0, st>>>(c->n_nodes, c->d_nb_ptr, c->d_nb, vals, x, y, w, c->d_part);
+    k_spmv<DOT><<<spmv_grid(c), 256, 0, st>>>(c->n_nodes, c->d_nb_ptr, c->d_nb, vals, x, y, w, c->d_part);
 }
 
 extern "C" int fem_spmv(fem_ctx *c, const double *csr_vals, const double *x, double *y, void *cuda_stream) {
@@ -320,7 +358,7 @@ static int bicgstab(fem_ctx *c, const double *vals, const double *b, double *x, 
                     double *relres, cudaStream_t st) {
     const long long n = c->n_rows;
     double *r = c->d_sw, *rhat = r + n, *p = rhat + n, *v = p + n, *s = v + n, *t = s + n, *y = t + n, *z = y + n, *dinv = z + n;
-    const long long spmv_ctas = (c->n_nodes + 7) / 8;
+    const long long spmv_ctas = spmv_grid(c);
     double h[2];
     k_dinv<<<nblk3(n, 256), 256, 0, st>>>(c->n_nodes, c->d_nb_ptr, c->d_diagpos, vals, dinv);
     launch_spmv<0>(c, vals, x, r, nullptr, st);
@@ -402,7 +440,7 @@ static int pcg(fem_ctx *c, const double *vals, const double *b, double *x, doubl
                cudaStream_t st) {
     const long long n = c->n_rows;
     double *r = c->d_sw, *z = r + n, *p = z + n, *q = p + n, *scratch = q + n, *dinv = c->d_sw + 8 * n;
-    const long long spmv_ctas = (c->n_nodes + 7) / 8;
+    const long long spmv_ctas = spmv_grid(c);
     double h[2];
     int rc;
     k_dinv<<<nblk3(n, 256), 256, 0, st>>>(c->n_nodes, c->d_nb_ptr, c->d_diagpos, vals, dinv);
@@ -421,24 +459,31 @@ static int pcg(fem_ctx *c, const double *vals, const double *b, double *x, doubl
     bool conv = rr <= tol2, bad = false;
     int it = 0;
     // z = M^-1 r and (r, z): one k_cg_update with alpha = 0
-    k_cg_update<<<RED_CTAS, RED_THREADS, 0, st>>>(n, 0.0, p, q, dinv, x, r, z, c->d_part);
+    k_cg_update<<<RED_CTAS, RED_THREADS, 0, st>>>(n, 0.0, nullptr, p, q, dinv, x, r, z, c->d_part);
     if ((rc = fetch_sums<2>(c, RED_CTAS, h, st)) != FEM_OK) return rc;
-    double rz = h[0], beta = 0.0;
-    while (!conv && it < max_iter) {
-        it++;
-        k_cg_p<<<RED_CTAS, RED_THREADS, 0, st>>>(n, beta, z, p);
-        launch_spmv<1>(c, vals, p, q, p, st);                       // q = K p, partial (p, q)
-        if ((rc = fetch_sums<2>(c, spmv_ctas, h, st)) != FEM_OK) return rc;
-        const double pq = h[0];
-        if (!(pq > 0.0) || !isfinite(pq)) { bad = true; break; }
-        const double alpha = rz / pq;
-        k_cg_update<<<RED_CTAS, RED_THREADS, 0, st>>>(n, alpha, p, q, dinv, x, r, z, c->d_part);
-        if ((rc = fetch_sums<2>(c, RED_CTAS, h, st)) != FEM_OK) return rc;
-        const double rz_new = h[0];
-        rr = h[1];
-        if (rr <= tol2) { conv = true; break; }
-        if (!(rz_new > 0.0) || !isfinite(rz_new)) { bad = true; break; }
-        beta = rz_new / rz; rz = rz_new;
+    if (!conv && max_iter > 0) {
+        // iterations run in batches without a host round trip; the scalars live in d_scal, a finished solve freezes itself
+        double sc0[8] = {h[0], 0.0, 0.0, rr, tol2, 0.0, 0.0, 0.0};
+        double *sc = c->d_scal;
+        FEM_CUDA(cudaMemcpyAsync(sc, sc0, sizeof(sc0), cudaMemcpyHostToDevice, st));
+        FEM_CUDA(cudaStreamSynchronize(st));   // sc0 is on the stack
+        const int batch = 16;
+        while (it < max_iter) {
+            const int nb = (max_iter - it < batch) ? max_iter - it : batch;
+            for (int j = 0; j < nb; j++) {
+                k_cg_p<<<RED_CTAS, RED_THREADS, 0, st>>>(n, 0.0, sc, z, p);              // p = z + beta p (beta = 0 at first)
+                launch_spmv<1>(c, vals, p, q, p, st);                                   // q = K p, partial (p, q)
+                k_cg_alpha<<<1, 1024, 0, st>>>(c->d_part, spmv_ctas, sc);
+                k_cg_update<<<RED_CTAS, RED_THREADS, 0, st>>>(n, 0.0, sc, p, q, dinv, x, r, z, c->d_part);
+                k_cg_beta<<<1, 1024, 0, st>>>(c->d_part, RED_CTAS, sc);
+            }
+            double hs[8];
+            FEM_CUDA(cudaMemcpyAsync(hs, sc, sizeof(hs), cudaMemcpyDeviceToHost, st));
+            FEM_CUDA(cudaStreamSynchronize(st));
+            it = (int)hs[6];
+            if (hs[5] == 1.0) { conv = true; break; }
+            if (hs[5] == 2.0) { bad = true; break; }
+        }
     }
     launch_spmv<0>(c, vals, x, r, nullptr, st);
     k_bicg_init<<<RED_CTAS, RED_THREADS, 0, st>>>(n, b, r, scratch, p, q, c->d_part);
