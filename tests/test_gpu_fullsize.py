@@ -128,3 +128,16 @@ def test_full_properties(full3):
         lo = torch.where(go, mid + 1, lo); hi = torch.where(go, hi, mid)
     assert bool((ci[lo].long() == r).all())
     assert float((vals[idx] - vals[lo]).abs().max()) <= 1e-10 * float(vals.abs().max())
+
+
+def test_full_size_repeat_is_bit_identical(full3):
+    """Determinism at full size (fixed summation order, no floating-point atomics): a second call gives the same bits."""
+    import torch
+    import paper_2606_17390_b200 as fem
+    cfg, ctx = full3["cfg"], full3["ctx"]
+    dev = full3["vals"].device
+    ne = cfg["conn"].shape[0]
+    mat = torch.from_numpy(fem.mat_from_desc(cfg["matdesc"], ne).ravel()).to(dev)
+    res, vals, hout, _ = ctx.assemble(torch.from_numpy(cfg["u"].ravel()).to(dev), torch.from_numpy(cfg["hist_in"].ravel()).to(dev), mat)
+    torch.cuda.synchronize()
+    assert torch.equal(vals, full3["vals"]) and torch.equal(res, full3["res"]) and torch.equal(hout, full3["hout"])
