@@ -34,7 +34,7 @@ def main():
     ap.add_argument("--path", default="0.002x8", help="load path: step size x number of steps, history and displacement carried over")
     ap.add_argument("--full", type=float, default=0.0, help="if > 0: run the whole benchmark loading (right face to 0.2, 0.1 mm) with "
                     "adaptive stepping (the paper's dt_initial 1e-3, dt_max 5e-2, cut-back on failure, :485) for at most this many seconds")
-    ap.add_argument("--extrapolate", type=int, default=1)
+    ap.add_argument("--extrapolate", type=int, default=1, help="initial guess of a step: 0 last state, 1 linear, 2 quadratic extrapolation")
     ap.add_argument("--grow-below", type=int, default=6, help="grow the step after a step with at most this many Newton iterations")
     args = ap.parse_args()
     n = args.n
@@ -137,16 +137,25 @@ def main():
         h_b = torch.empty_like(h_a)
         steps = newton = lin = rejected = 0
         u_try = torch.empty_like(u)
-        u_prev = torch.zeros_like(u)          # converged state one step back (linear extrapolation of the guess)
-        dt_prev = 0.0
+        u_prev = torch.zeros_like(u)          # converged states one and two steps back ("linear or quadratic extrapolation")
+        u_pp = torch.zeros_like(u)
+        dt_prev = dt_pp = 0.0
         t_start = time.perf_counter()
         print("\n| step | load fraction | dt | Newton iterations | linear iterations | s | plastic fraction | result |")
         print("|---|---|---|---|---|---|---|---|")
         while t < 1.0 - 1e-12 and time.perf_counter() - t_start < args.full:
             dt = min(dt, 1.0 - t)
             t0 = time.perf_counter()
-            r = dt / dt_prev if (dt_prev > 0 and args.extrapolate) else 0.0
-            ctx.lincomb(1.0 + r, u, -r, u_prev, u_try)                      # u + (u - u_prev) dt / dt_prev
+            if args.extrapolate == 2 and dt_pp > 0:      # quadratic (Lagrange) through the last three converged states
+                t0_, t1_, t2_, t3_ = -(dt_prev + dt_pp), -dt_prev, 0.0, dt
+                l0 = (t3_ - t1_) * (t3_ - t2_) / ((t0_ - t1_) * (t0_ - t2_))
+                l1 = (t3_ - t0_) * (t3_ - t2_) / ((t1_ - t0_) * (t1_ - t2_))
+                l2 = (t3_ - t0_) * (t3_ - t1_) / ((t2_ - t0_) * (t2_ - t1_))
+                ctx.lincomb(l2, u, l1, u_prev, u_try)
+                ctx.lincomb(1.0, u_try, l0, u_pp, u_try)
+            else:
+                r = dt / dt_prev if (dt_prev > 0 and args.extrapolate) else 0.0
+                ctx.lincomb(1.0 + r, u, -r, u_prev, u_try)                  # u + (u - u_prev) dt / dt_prev
             u_try, h_b, rep = ctx.newton_solve(u_try, h_a, mat, bc_d, torch.from_numpy(full * (t + dt)).to(dev), hist_out=h_b,
                                                lin_rtol=args.lin_rtol, lin_max_iter=20000, rtol=1e-8, max_newton=12)
             torch.cuda.synchronize()
@@ -159,8 +168,8 @@ def main():
             if ok:
                 t += dt; steps += 1
                 h_a, h_b = h_b, h_a
-                u_prev, u, u_try = u, u_try, u_prev
-                dt_prev = dt
+                u_pp, u_prev, u, u_try = u_prev, u, u_try, u_pp
+                dt_pp, dt_prev = dt_prev, dt
                 if rep["newton_iters"] <= args.grow_below:
                     dt = min(dt * 1.5, dt_max)
             else:
