@@ -29,6 +29,7 @@ def main():
     from synth import mesh
     ap = argparse.ArgumentParser()
     ap.add_argument("--n", type=int, default=100)
+    ap.add_argument("--mesh", default="", help="nx x ny x nz elements on the unit cube, e.g. 250x150x120 (the paper's largest case, :489); overrides --n")
     ap.add_argument("--lin-rtol", type=float, default=1e-8)
     ap.add_argument("--dt", default="0.002,0.005", help="load fractions of the Newton runs, each from the undeformed state")
     ap.add_argument("--path", default="0.002x8", help="load path: step size x number of steps, history and displacement carried over")
@@ -39,7 +40,8 @@ def main():
     args = ap.parse_args()
     n = args.n
     dev = torch.device("cuda:0")
-    coords, conn = mesh.structured_hex_mesh(n, n, n)
+    nx, ny, nz = (int(v) for v in args.mesh.split("x")) if args.mesh else (n, n, n)
+    coords, conn = mesh.structured_hex_mesh(nx, ny, nz)
     nn, ne = coords.shape[0], conn.shape[0]
     ctx = fem.FemContext(torch.from_numpy(coords).to(dev), torch.from_numpy(conn).to(dev))
     ctx.build_csr_pattern()
@@ -54,7 +56,7 @@ def main():
     bc_d = torch.from_numpy(bc).to(dev)
     hin = torch.zeros(56 * ne, dtype=torch.float64, device=dev)
     u0 = torch.zeros(nr, dtype=torch.float64, device=dev)
-    print("# NEXT-1 on the unit-cube benchmark, %d^3 elements, %d DOF, nnz %d\n" % (n, nr, nnz))
+    print("# NEXT-1 on the unit-cube benchmark, %d x %d x %d elements, %d DOF, nnz %d\n" % (nx, ny, nz, nr, nnz))
 
     # ---- 1. SpMV
     res, vals, _, _ = ctx.assemble(u0, hin, mat)
@@ -86,7 +88,7 @@ def main():
               % (rtol, its, dt, 1e3 * dt / max(its, 1), rr, ok))
 
     # ---- 3. one elastoplastic load increment from the undeformed state, for several increment sizes
-    for dts in args.dt.split(","):
+    for dts in [d for d in args.dt.split(",") if d]:
         dtf = float(dts)
         u = torch.zeros(nr, dtype=torch.float64, device=dev)
         t0 = time.perf_counter()

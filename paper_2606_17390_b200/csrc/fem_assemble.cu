@@ -1,13 +1,18 @@
 // fem_assemble: the hot path as three kernels on one stream
 //   k_mat_prep  : per material record -> derived record (Lame constants, Hill eigen-system, orientation)
-//   k_element   : 8 threads per element (one per Gauss point), 4 elements per warp.
+//   k_element   : 8 threads per element (one per Gauss point), 4 elements per warp, 16 per CTA.
 //                 phase 1 (per point): shape gradients, F, C = F^T F, spectral decomposition, Hencky strain,
 //                   Hill-48 return map as ONE scalar equation, algorithmic tangent as diagonal + rank-1,
-//                   geometric post-processor in the eigenbasis of C, A^ = dP/dF in mixed axes -> shared memory
-//                 phase 2 (per element node): K^e block rows and R^e from the 8 points' A^, G^ in shared memory
-//                 phase 3: K^e staged in shared memory, written block-major with coalesced 16-byte stores
-//   k_gather    : one warp per node: sums the <= 8 incident element contributions of each 3x3 node-pair block in
-//                 ascending element id (fixed order, no atomics) into the CSR values and the residual.
+//                   geometric post-processor in the eigenbasis of C, A^ = dP/dF in mixed axes -> shared memory;
+//                   R^e by a shuffle butterfly over the element's 8 lanes
+//                 phase 2 (whole warp per element): K^e = sum_q G^ A^ G^ on the FP64 tensor-core path
+//                   (mma.sync.m8n8k4.f64, one 8x8 node matrix per component pair), F-bar rank-1 terms likewise
+//                 phase 3: the accumulators go straight to the destination-major scratch (one 72-double record per
+//                   (element, local node) in the node-sorted incidence order); only the coloured mode stages K^e
+//   k_gather_fast / k_gather : one warp per node: copies the node's contiguous run of records to shared memory and sums the
+//                 <= 8 contributions of each 3x3 node-pair block in ascending element id (fixed order, no atomics)
+//                 into the CSR values and the residual.
+// assembly_mode 1 (coloured in-place) and 2 (fused queue) are alternatives kept as tested, slower options.
 // All formulas are derived by hand from PAPER.md (equation numbers at each step); nothing here is shared with oracle/.
 #include "fem_internal.h"
 #include <math.h>
