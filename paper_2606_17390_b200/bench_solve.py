@@ -29,6 +29,7 @@ def main():
     from synth import mesh
     ap = argparse.ArgumentParser()
     ap.add_argument("--n", type=int, default=100)
+    ap.add_argument("--fbar", type=int, default=0, help="1: F-bar element (unsymmetric tangent, BiCGSTAB)")
     ap.add_argument("--mesh", default="", help="nx x ny x nz elements on the unit cube, e.g. 250x150x120 (the paper's largest case, :489); overrides --n")
     ap.add_argument("--lin-rtol", type=float, default=1e-8)
     ap.add_argument("--dt", default="0.002,0.005", help="load fractions of the Newton runs, each from the undeformed state")
@@ -43,7 +44,7 @@ def main():
     nx, ny, nz = (int(v) for v in args.mesh.split("x")) if args.mesh else (n, n, n)
     coords, conn = mesh.structured_hex_mesh(nx, ny, nz)
     nn, ne = coords.shape[0], conn.shape[0]
-    ctx = fem.FemContext(torch.from_numpy(coords).to(dev), torch.from_numpy(conn).to(dev))
+    ctx = fem.FemContext(torch.from_numpy(coords).to(dev), torch.from_numpy(conn).to(dev), fbar=args.fbar)
     ctx.build_csr_pattern()
     nnz, nr = ctx.nnz, 3 * nn
     # Table 3: E = 219 GPa, Voce sigma0 = 138, Q = 410, b = 3.8, ratios r11..r23; nu is not printed: 0.3
