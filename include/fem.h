@@ -63,7 +63,8 @@ typedef struct {
                           launch (plus a drain kernel) assemble them while other elements are still being evaluated.
                           Modes 1 and 2 are measured slower than mode 0 at config 3 and are kept as
                           tested options; they fall back to mode 0 for meshes with collapsed elements (1, 2) or a node with
-                          more than 8 elements (2). */
+                          more than 8 elements (2).  In mode 0 such nodes are gathered by a general path, all others by the
+                          table-driven fast path of the same kernel. */
 } fem_options;
 
 typedef struct {

@@ -1240,16 +1240,13 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
 }
 
 // ------------------------------------------------------------------------------------------------ gather kernels (S14)
-// General kernel (a node with more than 8 incident elements, or collapsed elements): one warp per node, lane <-> neighbour
-// position pos; the elem_pos bytes of each incident entry give the local nodes K whose column node sits at pos.
-__global__ void __launch_bounds__(256)
-k_gather(long long n_nodes, const int *__restrict__ inc_ptr, const int *__restrict__ inc, const int *__restrict__ nb_ptr,
-         const unsigned char *__restrict__ elem_pos, const double *__restrict__ Ke, const double *__restrict__ Re,
-         double *__restrict__ csr_vals, double *__restrict__ residual) {
-    const long long n = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-    const int lane = threadIdx.x & 31;
-    if (n >= n_nodes) return;
-    const int b = inc_ptr[n], m = inc_ptr[n + 1] - b;
+// General node gather (a node with more than 8 incident elements, or collapsed elements): lane <-> neighbour position pos;
+// the elem_pos bytes of each incident entry give the local nodes K whose column node sits at pos.  Reads the records from
+// global memory directly.
+__device__ __forceinline__ void gather_general_node(long long n, int b, int m, int lane, const int *__restrict__ inc,
+                                                    const int *__restrict__ nb_ptr, const unsigned char *__restrict__ elem_pos,
+                                                    const double *__restrict__ Ke, const double *__restrict__ Re,
+                                                    double *__restrict__ csr_vals, double *__restrict__ residual) {
     const int o = nb_ptr[n], len = nb_ptr[n + 1] - o;
     const uint2 *pos8 = reinterpret_cast<const uint2 *>(elem_pos);
     for (int pos = lane; pos < len; pos += 32) {
@@ -1281,23 +1278,39 @@ k_gather(long long n_nodes, const int *__restrict__ inc_ptr, const int *__restri
         residual[3 * n + lane] = r;
     }
 }
+// General kernel: every node through gather_general_node (meshes with collapsed elements).
+__global__ void __launch_bounds__(256)
+k_gather(long long n_nodes, const int *__restrict__ inc_ptr, const int *__restrict__ inc, const int *__restrict__ nb_ptr,
+         const unsigned char *__restrict__ elem_pos, const double *__restrict__ Ke, const double *__restrict__ Re,
+         double *__restrict__ csr_vals, double *__restrict__ residual) {
+    const long long n = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    if (n >= n_nodes) return;
+    const int b = inc_ptr[n], m = inc_ptr[n + 1] - b;
+    gather_general_node(n, b, m, lane, inc, nb_ptr, elem_pos, Ke, Re, csr_vals, residual);
+}
 
-// Fast gather for meshes where every node has <= 8 incident elements and no element lists a node twice (all hex meshes
-// of the configs): one warp per node copies the node's run of records (<= 4608 bytes) into shared memory with coalesced
-// 16-byte loads and reduces it with gather_reduce_write.
+// Fast gather for meshes where no element lists a node twice: one warp per node copies the node's run of records
+// (<= 4608 bytes) into shared memory with coalesced 16-byte loads and reduces it with gather_reduce_write; the few nodes
+// of an unstructured hex mesh that belong to more than 8 elements take gather_general_node.
 #define GW 8   // warps (nodes) per CTA
 #ifndef GMINB
 #define GMINB 5
 #endif
+template <int HV>   // HV = 1: the mesh has nodes with more than 8 elements (they take the general path)
 __global__ void __launch_bounds__(GW * 32, GMINB)
-k_gather_fast(long long n_nodes, const int *__restrict__ inc_ptr, const int *__restrict__ nb_ptr,
-              const unsigned int *__restrict__ kvec, const double *__restrict__ Ke, const double *__restrict__ Re,
-              double *__restrict__ csr_vals, double *__restrict__ residual) {
+k_gather_fast(long long n_nodes, const int *__restrict__ inc_ptr, const int *__restrict__ inc, const int *__restrict__ nb_ptr,
+              const unsigned int *__restrict__ kvec, const unsigned char *__restrict__ elem_pos, const double *__restrict__ Ke,
+              const double *__restrict__ Re, double *__restrict__ csr_vals, double *__restrict__ residual) {
     __shared__ __align__(16) double buf[GW][576];
     const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const long long n = (long long)blockIdx.x * GW + w;
     if (n >= n_nodes) return;
     const int b = inc_ptr[n], m = inc_ptr[n + 1] - b;
+    if (HV && m > 8) {   // warp-uniform
+        gather_general_node(n, b, m, lane, inc, nb_ptr, elem_pos, Ke, Re, csr_vals, residual);
+        return;
+    }
     {
         const double2 *src = reinterpret_cast<const double2 *>(Ke + (long long)b * 72);
         double2 *dst = reinterpret_cast<double2 *>(buf[w]);
@@ -1428,8 +1441,12 @@ int fem_launch_assemble(fem_ctx *c, const double *u, const double *hist_in, cons
                                                        c->opt.tol, c->opt.kmax, c->d_Ke, c->d_Re, hist_out, c->d_stats, sa);
         FEM_CUDA(cudaEventRecord(c->ev[2], st));
         if (c->d_kvec)   // every node has <= 8 incident elements, no collapsed element
-            k_gather_fast<<<nblk2(c->n_nodes, GW), GW * 32, 0, st>>>(c->n_nodes, c->d_inc_ptr, c->d_nb_ptr, c->d_kvec, c->d_Ke, c->d_Re,
-                                                                  csr_vals, residual);
+            if (c->has_high_valence)
+                k_gather_fast<1><<<nblk2(c->n_nodes, GW), GW * 32, 0, st>>>(c->n_nodes, c->d_inc_ptr, c->d_inc, c->d_nb_ptr, c->d_kvec,
+                                                                         c->d_elem_pos, c->d_Ke, c->d_Re, csr_vals, residual);
+            else
+                k_gather_fast<0><<<nblk2(c->n_nodes, GW), GW * 32, 0, st>>>(c->n_nodes, c->d_inc_ptr, c->d_inc, c->d_nb_ptr, c->d_kvec,
+                                                                         c->d_elem_pos, c->d_Ke, c->d_Re, csr_vals, residual);
         else
             k_gather<<<nblk2(c->n_nodes * 32, 256), 256, 0, st>>>(c->n_nodes, c->d_inc_ptr, c->d_inc, c->d_nb_ptr, c->d_elem_pos, c->d_Ke,
                                                                  c->d_Re, csr_vals, residual);

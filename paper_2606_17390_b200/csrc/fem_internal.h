@@ -38,6 +38,7 @@ struct fem_ctx {
     int *d_queue = nullptr;                       // [n_nodes] working copy: node ids in order of completion
     unsigned int *d_qctl = nullptr;               // [0] tail (tickets handed out), [1] head (entries claimed), [2..3] initial values
     int n_isolated = 0;
+    bool has_high_valence = false;                // some node belongs to more than 8 elements
     bool has_collapsed = false;                   // some element lists a node twice
     int n_colours = 0, colour_rounds = 0;
     long long colour_start[65] = {0};

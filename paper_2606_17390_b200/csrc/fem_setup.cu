@@ -185,7 +185,7 @@ __global__ void k_kvec(long long n_nodes, const int *__restrict__ inc_ptr, const
     long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (n >= n_nodes) return;
     const int b = inc_ptr[n], m = inc_ptr[n + 1] - b, o = nb_ptr[n], len = nb_ptr[n + 1] - o;
-    if (m > 8) { atomicOr(flags, 16); return; }
+    if (m > 8) { atomicOr(flags, 16); return; }   // this node takes the general path of the gather kernel (kvec unused)
     for (int p = 0; p < len; p++) kvec[o + p] = 0xffffffffu;
     for (int s = 0; s < m; s++) {
         const long long t = inc[b + s];
@@ -344,9 +344,9 @@ extern "C" int fem_build_csr_pattern(fem_ctx *c, long long *n_rows, long long *n
                 k_kvec<<<nblk(nn, 128), 128>>>(nn, c->d_inc_ptr, c->d_inc, c->d_nb_ptr, c->d_elem_pos, c->d_kvec, dflags);
                 int kf = 0;
                 TRY(cudaMemcpy(&kf, dflags, sizeof(int), cudaMemcpyDeviceToHost));
-                if (kf & 16) { cudaFree(c->d_kvec); c->d_kvec = nullptr; }   // general gather kernel instead
+                c->has_high_valence = (kf & 16) != 0;   // some node has more than 8 elements: it is gathered by the general path
             }
-            if (c->mode == 2 && !c->d_kvec) c->mode = 0;   // the fused mode uses the fast gather tables
+            if (c->mode == 2 && (!c->d_kvec || c->has_high_valence)) c->mode = 0;   // the fused mode buffers at most 8 records per node
             if (c->mode == 2) {
                 TRY(cudaMalloc(&c->d_cnt_init, sizeof(int) * nn));
                 TRY(cudaMalloc(&c->d_cnt, sizeof(int) * nn));

@@ -163,8 +163,8 @@ def test_coloured_in_place_assembly_mode(fbar):
 
 
 def _pinwheel_mesh(nsec=12, layers=2):
-    """nsec hexes around the z-axis share the axis edge: axis nodes belong to nsec (> 8) elements per layer pair, which
-    disables the fast gather table and exercises the general gather kernel."""
+    """nsec hexes around the z-axis share the axis edge: axis nodes belong to nsec (> 8) elements per layer pair; they take
+    the general path of the gather kernel, all other nodes of the same mesh the fast table path."""
     nodes, idx = [], {}
 
     def nid(key, xyz):
