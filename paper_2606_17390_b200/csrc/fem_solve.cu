@@ -165,8 +165,9 @@ k_bicg_init(long long n, const double *__restrict__ b, double *__restrict__ r, d
 }
 // p = r + beta (p - omega v) ; y = M^-1 p
 __global__ void __launch_bounds__(RED_THREADS)
-k_bicg_p(long long n, double beta, double omega, const double *__restrict__ r, const double *__restrict__ v,
+k_bicg_p(long long n, const double *__restrict__ sc, const double *__restrict__ r, const double *__restrict__ v,
          const double *__restrict__ dinv, double *__restrict__ p, double *__restrict__ y) {
+    const double beta = sc[4], omega = sc[3];   // omega of the previous iteration
     for (long long j = blockIdx.x * (long long)blockDim.x + threadIdx.x; j < n; j += (long long)gridDim.x * blockDim.x) {
         const double pj = fma(beta, fma(-omega, v[j], p[j]), r[j]);
         p[j] = pj; y[j] = dinv[j] * pj;
@@ -174,10 +175,11 @@ k_bicg_p(long long n, double beta, double omega, const double *__restrict__ r, c
 }
 // s = r - alpha v ; z = M^-1 s ; partial (s, s)
 __global__ void __launch_bounds__(RED_THREADS)
-k_bicg_s(long long n, double alpha, const double *__restrict__ r, const double *__restrict__ v, const double *__restrict__ dinv,
-         double *__restrict__ s, double *__restrict__ z, double *__restrict__ part) {
+k_bicg_s(long long n, const double *__restrict__ sc, const double *__restrict__ r, const double *__restrict__ v,
+         const double *__restrict__ dinv, double *__restrict__ s, double *__restrict__ z, double *__restrict__ part) {
     __shared__ double smem[32];
     double a[1] = {0.0};
+    const double alpha = sc[2];
     for (long long j = blockIdx.x * (long long)blockDim.x + threadIdx.x; j < n; j += (long long)gridDim.x * blockDim.x) {
         const double sj = fma(-alpha, v[j], r[j]);
         s[j] = sj; z[j] = dinv[j] * sj;
@@ -188,11 +190,12 @@ k_bicg_s(long long n, double alpha, const double *__restrict__ r, const double *
 }
 // x += alpha y + omega z ; r = s - omega t ; partials (rhat, r), (r, r)
 __global__ void __launch_bounds__(RED_THREADS)
-k_bicg_xr(long long n, double alpha, double omega, const double *__restrict__ y, const double *__restrict__ z,
+k_bicg_xr(long long n, const double *__restrict__ sc, const double *__restrict__ y, const double *__restrict__ z,
           const double *__restrict__ s, const double *__restrict__ t, const double *__restrict__ rhat, double *__restrict__ x,
           double *__restrict__ r, double *__restrict__ part) {
     __shared__ double smem[2 * 32];
     double a[2] = {0.0, 0.0};
+    const double alpha = sc[2], omega = sc[3];
     for (long long j = blockIdx.x * (long long)blockDim.x + threadIdx.x; j < n; j += (long long)gridDim.x * blockDim.x) {
         x[j] = fma(omega, z[j], fma(alpha, y[j], x[j]));
         const double rj = fma(-omega, t[j], s[j]);
@@ -201,6 +204,60 @@ k_bicg_xr(long long n, double alpha, double omega, const double *__restrict__ y,
     }
     cta_reduce<2>(a, smem);
     if (threadIdx.x == 0) { part[2LL * blockIdx.x] = a[0]; part[2LL * blockIdx.x + 1] = a[1]; }
+}
+// ---- BiCGSTAB scalars on the device: sc[0] rho, [1] rho_old, [2] alpha, [3] omega, [4] beta, [5] (r,r), [6] tol^2 (b,b),
+//      [7] flag (0 running, 1 converged, 2 breakdown: the host restarts), [8] iterations, [9] |rhat|.  A solve whose flag is
+//      set keeps alpha = omega = beta = 0, so the remaining iterations of a batch change neither x nor r.
+template <int NV>
+__device__ __forceinline__ void sum_partials(const double *__restrict__ part, long long count, double (&v)[NV], double *smem) {
+#pragma unroll
+    for (int k = 0; k < NV; k++) v[k] = 0.0;
+    for (long long j = threadIdx.x; j < count; j += blockDim.x)
+#pragma unroll
+        for (int k = 0; k < NV; k++) v[k] += part[j * NV + k];
+    cta_reduce<NV>(v, smem);
+}
+__device__ __forceinline__ void bi_next_beta(double *sc) {   // breakdown guard + beta of the next iteration
+    const double rho = sc[0], omega = sc[3];
+    if (!(fabs(rho) > 1e-12 * sqrt(sc[5]) * sc[9]) || !isfinite(rho) || omega == 0.0 || !isfinite(omega)) { sc[7] = 2.0; sc[4] = 0.0; }
+    else sc[4] = (rho / sc[1]) * (sc[2] / omega);
+}
+__global__ void __launch_bounds__(1024) k_bi_alpha(const double *__restrict__ part, long long count, double *sc) {   // after v = K y
+    __shared__ double smem[2 * 32];
+    double v[2];
+    sum_partials<2>(part, count, v, smem);
+    if (threadIdx.x == 0) {
+        if (sc[7] == 0.0) {
+            sc[8] += 1.0;
+            if (v[0] == 0.0 || !isfinite(v[0])) sc[7] = 2.0;
+        }
+        sc[2] = (sc[7] == 0.0) ? sc[0] / v[0] : 0.0;
+    }
+}
+__global__ void __launch_bounds__(1024) k_bi_half(const double *__restrict__ part, long long count, double *sc) {    // after s = r - alpha v
+    __shared__ double smem[32];
+    double v[1];
+    sum_partials<1>(part, count, v, smem);
+    if (threadIdx.x == 0 && sc[7] == 0.0 && v[0] <= sc[6]) { sc[7] = 1.0; sc[5] = v[0]; }   // the half step suffices: omega = 0 below, x += alpha y, r = s
+}
+__global__ void __launch_bounds__(1024) k_bi_omega(const double *__restrict__ part, long long count, double *sc) {   // after t = K z
+    __shared__ double smem[2 * 32];
+    double v[2];
+    sum_partials<2>(part, count, v, smem);
+    if (threadIdx.x == 0) sc[3] = (sc[7] == 0.0 && v[1] > 0.0 && isfinite(v[1])) ? v[0] / v[1] : 0.0;
+}
+__global__ void __launch_bounds__(1024) k_bi_rho(const double *__restrict__ part, long long count, double *sc) {     // after the x, r update
+    __shared__ double smem[2 * 32];
+    double v[2];
+    sum_partials<2>(part, count, v, smem);
+    if (threadIdx.x == 0) {
+        if (sc[7] == 0.0) {
+            sc[1] = sc[0]; sc[0] = v[0]; sc[5] = v[1];
+            if (v[1] <= sc[6]) sc[7] = 1.0;
+            else bi_next_beta(sc);
+        }
+        if (sc[7] != 0.0) sc[4] = 0.0;
+    }
 }
 // ---- CG scalars stay on the device (no host round trip per iteration).  sc[0] = (r,z), sc[1] = alpha, sc[2] = beta,
 //      sc[3] = (r,r), sc[4] = tol^2 (b,b), sc[5] = done flag (1 converged, 2 breakdown), sc[6] = iterations performed.
@@ -287,7 +344,7 @@ static int ensure_solver_ws(fem_ctx *c, bool newton) {
         c->n_part = 2 * (spmv_ctas > RED_CTAS ? spmv_ctas : RED_CTAS);
         FEM_CUDA(cudaMalloc(&c->d_sw, sizeof(double) * 9 * n));
         FEM_CUDA(cudaMalloc(&c->d_part, sizeof(double) * c->n_part));
-        FEM_CUDA(cudaMalloc(&c->d_scal, sizeof(double) * 8));
+        FEM_CUDA(cudaMalloc(&c->d_scal, sizeof(double) * 64));   // [0..8) reduction results, [16..48) solver scalars
     }
     if (newton && !c->d_nw) {
         FEM_CUDA(cudaMalloc(&c->d_nw, sizeof(double) * 4 * n));
@@ -376,50 +433,49 @@ static int bicgstab(fem_ctx *c, const double *vals, const double *b, double *x, 
         return FEM_OK;
     }
     const double tol2 = rtol * rtol * bb;
-    double rhat_norm = sqrt(rr);
-    double rho = rr, rho_old = 1.0, alpha = 1.0, omega = 1.0;
     conv = rr <= tol2;
+    // iterations run in batches without a host round trip (scalars in d_scal); the host looks at the flag after each batch
+    // and restarts from the true residual of the current x (rhat = r = b - K x, p = v = 0) when the recurrence broke down
+    double *sc = c->d_scal + 16;
     int restarts = 0;
+    const int batch = 8;
+    bool fresh = true;   // r, rhat, p, v and rr describe a fresh start
     while (!conv && it < max_iter) {
-        it++;
-        // breakdown guard: (rhat, r) has collapsed relative to |rhat||r| (rhat = the residual of the last restart), or a
-        // scalar is zero / not finite -> restart from the true residual of the current x (rhat = r = b - K x, p = v = 0)
-        bool restart = !(fabs(rho) > 1e-12 * sqrt(rr) * rhat_norm) || !isfinite(rho) || omega == 0.0 || !isfinite(omega);
-        double rv = 0.0;
-        if (!restart) {
-            const double beta = (rho / rho_old) * (alpha / omega);
-            k_bicg_p<<<RED_CTAS, RED_THREADS, 0, st>>>(n, beta, omega, r, v, dinv, p, y);
-            launch_spmv<1>(c, vals, y, v, rhat, st);
-            if ((rc = fetch_sums<2>(c, spmv_ctas, h, st)) != FEM_OK) return rc;
-            rv = h[0];
-            restart = (rv == 0.0 || !isfinite(rv));
-        }
-        if (restart) {
+        if (!fresh) {
             if (++restarts > 50) break;
             launch_spmv<0>(c, vals, x, r, nullptr, st);
             k_bicg_init<<<RED_CTAS, RED_THREADS, 0, st>>>(n, b, r, rhat, p, v, c->d_part);
             if ((rc = fetch_sums<2>(c, RED_CTAS, h, st)) != FEM_OK) return rc;
-            rr = h[0]; rho = rr; rho_old = alpha = omega = 1.0; rhat_norm = sqrt(rr);
+            rr = h[0];
             if (rr <= tol2) { conv = true; break; }
             if (!isfinite(rr)) break;
-            continue;
         }
-        alpha = rho / rv;
-        k_bicg_s<<<RED_CTAS, RED_THREADS, 0, st>>>(n, alpha, r, v, dinv, s, z, c->d_part);
-        if ((rc = fetch_sums<1>(c, RED_CTAS, h, st)) != FEM_OK) return rc;
-        if (h[0] <= tol2) {   // first half step already meets the tolerance
-            k_axpy<<<RED_CTAS, RED_THREADS, 0, st>>>(n, alpha, y, x);
-            conv = true;
-            break;
+        // rho = (rhat, r) = rr, rho_old = alpha = omega = 1, beta irrelevant (p = v = 0)
+        const double sc0[16] = {rr, 1.0, 1.0, 1.0, rr, rr, tol2, 0.0, (double)it, sqrt(rr), 0, 0, 0, 0, 0, 0};
+        FEM_CUDA(cudaMemcpyAsync(sc, sc0, sizeof(sc0), cudaMemcpyHostToDevice, st));
+        FEM_CUDA(cudaStreamSynchronize(st));   // sc0 is on the stack
+        fresh = false;
+        double hs[16];
+        hs[7] = 0.0;
+        while (it < max_iter && hs[7] == 0.0) {
+            const int nb = (max_iter - it < batch) ? max_iter - it : batch;
+            for (int j = 0; j < nb; j++) {
+                k_bicg_p<<<RED_CTAS, RED_THREADS, 0, st>>>(n, sc, r, v, dinv, p, y);
+                launch_spmv<1>(c, vals, y, v, rhat, st);
+                k_bi_alpha<<<1, 1024, 0, st>>>(c->d_part, spmv_ctas, sc);
+                k_bicg_s<<<RED_CTAS, RED_THREADS, 0, st>>>(n, sc, r, v, dinv, s, z, c->d_part);
+                k_bi_half<<<1, 1024, 0, st>>>(c->d_part, RED_CTAS, sc);
+                launch_spmv<2>(c, vals, z, t, s, st);
+                k_bi_omega<<<1, 1024, 0, st>>>(c->d_part, spmv_ctas, sc);
+                k_bicg_xr<<<RED_CTAS, RED_THREADS, 0, st>>>(n, sc, y, z, s, t, rhat, x, r, c->d_part);
+                k_bi_rho<<<1, 1024, 0, st>>>(c->d_part, RED_CTAS, sc);
+            }
+            FEM_CUDA(cudaMemcpyAsync(hs, sc, sizeof(hs), cudaMemcpyDeviceToHost, st));
+            FEM_CUDA(cudaStreamSynchronize(st));
+            it = (int)hs[8];
         }
-        launch_spmv<2>(c, vals, z, t, s, st);
-        if ((rc = fetch_sums<2>(c, spmv_ctas, h, st)) != FEM_OK) return rc;
-        const double ts = h[0], tt = h[1];
-        omega = (tt > 0.0 && isfinite(tt)) ? ts / tt : 0.0;
-        k_bicg_xr<<<RED_CTAS, RED_THREADS, 0, st>>>(n, alpha, omega, y, z, s, t, rhat, x, r, c->d_part);
-        if ((rc = fetch_sums<2>(c, RED_CTAS, h, st)) != FEM_OK) return rc;
-        rho_old = rho; rho = h[0]; rr = h[1];
-        if (rr <= tol2) { conv = true; break; }
+        if (hs[7] == 1.0) conv = true;
+        // hs[7] == 2: breakdown -> the outer loop restarts; 0: iteration cap
     }
     // explicit residual of the returned x (the recurrence residual can drift)
     launch_spmv<0>(c, vals, x, r, nullptr, st);
@@ -464,7 +520,7 @@ static int pcg(fem_ctx *c, const double *vals, const double *b, double *x, doubl
     if (!conv && max_iter > 0) {
         // iterations run in batches without a host round trip; the scalars live in d_scal, a finished solve freezes itself
         double sc0[8] = {h[0], 0.0, 0.0, rr, tol2, 0.0, 0.0, 0.0};
-        double *sc = c->d_scal;
+        double *sc = c->d_scal + 16;
         FEM_CUDA(cudaMemcpyAsync(sc, sc0, sizeof(sc0), cudaMemcpyHostToDevice, st));
         FEM_CUDA(cudaStreamSynchronize(st));   // sc0 is on the stack
         const int batch = 16;
