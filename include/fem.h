@@ -168,7 +168,8 @@ int fem_apply_dirichlet(fem_ctx *c, long long n_bc, const int *bc_dofs, const do
  *   explicit residual of the current x (at most 50 times).
  *   *iters (host, may be NULL) = iterations used; *relres (host, may be NULL) = explicit ||b - K x|| / ||b|| at exit.
  * Returns FEM_OK when converged, FEM_ERR_NOCONV otherwise (x holds the last iterate).  Dot products are reduced in a
- * fixed order: two calls with equal inputs give bit-identical results.  Synchronises the stream (scalars go through the host). */
+ * fixed order: two calls with equal inputs give bit-identical results.  Synchronises the stream (the iteration scalars stay on the device; the host
+ * checks the convergence flag after every batch of 8 iterations and restarts the recurrence on breakdown). */
 int fem_bicgstab(fem_ctx *c, const double *csr_vals, const double *b, double *x, double rtol, int max_iter, int *iters,
                  double *relres, void *cuda_stream);
 
