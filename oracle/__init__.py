@@ -62,6 +62,20 @@ def lib():
         L.orc_assemble.argtypes = [C.c_longlong, _dp, C.c_longlong, _ip, C.c_int, _dp, _dp, _dp, C.c_longlong, _ip, _ip,
                                    _dp, _dp, _dp, _lp]
         L.orc_num_threads.restype = C.c_int
+        L.orc_barlat_phi_eig.restype = C.c_double
+        L.orc_barlat_phi_eig.argtypes = [_dp, _dp]
+        L.orc_barlat_derivs.argtypes = [_dp] * 5
+        L.orc_yield_eval.argtypes = [_dp] * 6
+        L.orc_return_map_gen.restype = C.c_int
+        L.orc_return_map_gen.argtypes = [_dp, _dp, _dp, _dp, C.c_double, C.c_double, C.c_int, C.c_int, C.c_double, C.c_double,
+                                         _dp, _dp, _dp, _dp, _dp, _ip, _ip, _dp]
+        L.orc_point_yld.restype = C.c_int
+        L.orc_point_yld.argtypes = [_dp] * 10 + [_ip]
+        L.orc_element_yld.restype = C.c_int
+        L.orc_element_yld.argtypes = [_dp, _dp, _dp, _dp, _dp, C.c_int, _dp, _dp, _dp, _lp]
+        L.orc_assemble_yld.restype = C.c_int
+        L.orc_assemble_yld.argtypes = [C.c_longlong, _dp, C.c_longlong, _ip, C.c_int, _dp, _dp, _dp, C.c_longlong, _dp, _ip,
+                                       _ip, _dp, _dp, _dp, _lp]
         L.orc_hill_from_lankford.argtypes = [C.c_double] * 3 + [_dp]
         _lib = L
     return _lib
@@ -156,19 +170,68 @@ def postprocess(lam, R, T, Cep):
     return S, CL
 
 
-def point(mat, F, hin):
-    mat, F, hin = _f(mat), _f(F), _f(hin)
+def _bar(bar):
+    return None if bar is None else _f(bar)
+
+
+def point(mat, F, hin, bar=None):
+    mat, F, hin, bar = _f(mat), _f(F), _f(hin), _bar(bar)
     P = np.empty((3, 3)); A = np.empty((3, 3, 3, 3)); hout = np.empty(7); S = np.empty(6); T = np.empty(6); CL = np.empty((6, 6))
     it = C.c_int()
-    fl = lib().orc_point(_d(mat), _d(F), _d(hin), _d(P), _d(A), _d(hout), _d(S), _d(T), _d(CL), C.byref(it))
+    fl = lib().orc_point_yld(_d(mat), None if bar is None else _d(bar), _d(F), _d(hin), _d(P), _d(A), _d(hout), _d(S), _d(T),
+                             _d(CL), C.byref(it))
     return dict(flags=fl, P=P, A=A, hist=hout, S=S, T=T, CL=CL, iters=it.value)
 
 
-def element(X, u, hin, mat, fbar=0):
-    X, u, hin, mat = _f(X), _f(u), _f(hin), _f(mat)
+def element(X, u, hin, mat, fbar=0, bar=None):
+    X, u, hin, mat, bar = _f(X), _f(u), _f(hin), _f(mat), _bar(bar)
     Re = np.empty(24); Ke = np.empty((24, 24)); hout = np.empty((8, 7)); st = np.zeros(4, dtype=np.int64)
-    lib().orc_element(_d(X), _d(u), _d(hin), _d(mat), int(fbar), _d(Re), _d(Ke), _d(hout), st.ctypes.data_as(_lp))
+    lib().orc_element_yld(_d(X), _d(u), _d(hin), _d(mat), None if bar is None else _d(bar), int(fbar), _d(Re), _d(Ke), _d(hout),
+                          st.ctypes.data_as(_lp))
     return Re, Ke, hout, st
+
+
+# ---------------------------------------------------------------- Yld2004-18p
+NBAR = 20
+# PAPER.md:471-477 Table 2: c'12,c'13,c'21,c'23,c'31,c'32,c'44,c'55,c'66 ; the same nine for C'' ; m
+TABLE2_CP = (-0.069888, 0.936408, 0.079143, 1.003060, 0.524741, 1.363180, 1.023770, 1.069060, 0.954322)
+TABLE2_CPP = (0.981171, 0.476741, 0.575316, 0.866827, 1.145010, -0.079294, 1.051660, 1.147100, 1.404620)
+
+
+def barlat_record(cp=TABLE2_CP, cpp=TABLE2_CPP, m=8):
+    """One 20-double record: c' (9), c'' (9), m, 0."""
+    return np.array([*cp, *cpp, float(m), 0.0], dtype=np.float64)
+
+
+def barlat_phi_eig(bar, Tm):
+    """Eq.(12) by its definition (eigenvalues); Tm = material-frame stress, Mandel 6-vector."""
+    bar, Tm = _f(bar), _f(Tm)
+    return lib().orc_barlat_phi_eig(_d(bar), _d(Tm))
+
+
+def barlat_derivs(bar, Tm, hess=True):
+    bar, Tm = _f(bar), _f(Tm)
+    phi = C.c_double(); N = np.empty(6); H = np.empty((6, 6))
+    lib().orc_barlat_derivs(_d(bar), _d(Tm), C.byref(phi), _d(N), _d(H) if hess else None)
+    return phi.value, N, (H if hess else None)
+
+
+def yield_eval(mat, bar, T6):
+    """Global frame, T6 tensor components -> phi, N (Mandel), dN/dT (6x6 Mandel); bar None = Hill-48."""
+    mat, T6, bar = _f(mat), _f(T6), _bar(bar)
+    phi = C.c_double(); N = np.empty(6); H = np.empty((6, 6))
+    lib().orc_yield_eval(_d(mat), None if bar is None else _d(bar), _d(T6), C.byref(phi), _d(N), _d(H))
+    return phi.value, N, H
+
+
+def return_map_gen(mat, bar, eps, epn, alphan, tol=1e-14, kmax=100, jmax=20, beta=1e-4, eta=0.1):
+    """Alg. C1/C2 step by step (8 unknowns, line search of App. B) for either yield function."""
+    mat, eps, epn, bar = _f(mat), _f(eps), _f(epn), _bar(bar)
+    T = np.empty(6); ep = np.empty(6); Cep = np.empty((6, 6)); tr = np.empty((kmax + 1, 3))
+    a = C.c_double(); dg = C.c_double(); it = C.c_int(); nc = C.c_int()
+    pl = lib().orc_return_map_gen(_d(mat), None if bar is None else _d(bar), _d(eps), _d(epn), float(alphan), tol, kmax, jmax,
+                                  beta, eta, _d(T), _d(ep), C.byref(a), C.byref(dg), _d(Cep), C.byref(it), C.byref(nc), _d(tr))
+    return dict(plastic=bool(pl), T=T, ep=ep, alpha=a.value, dgam=dg.value, Cep=Cep, iters=it.value, nonconv=nc.value, trace=tr)
 
 
 # ---------------------------------------------------------------- mesh-level
@@ -183,13 +246,17 @@ def pattern(n_nodes, conn, with_slots=True):
     return row_ptr, col_idx, slots
 
 
-def assemble(coords, conn, u, hist_in, mat, row_ptr, col_idx, fbar=0):
+def assemble(coords, conn, u, hist_in, mat, row_ptr, col_idx, fbar=0, bar=None):
     coords, u, hist_in, mat = _f(coords), _f(u), _f(hist_in), _f(mat).reshape(-1, NPAR)
+    if bar is not None:
+        bar = _f(bar).reshape(-1, NBAR)
+        assert bar.shape[0] == mat.shape[0]
     conn = np.ascontiguousarray(conn, dtype=np.int32)
     nn, ne = coords.shape[0], conn.shape[0]
     res = np.empty(3 * nn); vals = np.empty(col_idx.shape[0]); hout = np.empty((ne, 8, 7)); st = np.zeros(4, dtype=np.int64)
-    rc = lib().orc_assemble(nn, _d(coords), ne, _i(conn), int(fbar), _d(u), _d(hist_in), _d(mat), mat.shape[0], _i(row_ptr),
-                            _i(col_idx), _d(res), _d(vals), _d(hout), st.ctypes.data_as(_lp))
+    rc = lib().orc_assemble_yld(nn, _d(coords), ne, _i(conn), int(fbar), _d(u), _d(hist_in), _d(mat), mat.shape[0],
+                                None if bar is None else _d(bar), _i(row_ptr), _i(col_idx), _d(res), _d(vals), _d(hout),
+                                st.ctypes.data_as(_lp))
     if rc != 0:
         raise MemoryError("orc_assemble")
     return dict(residual=res, csr_vals=vals, hist_out=hout,

@@ -16,6 +16,11 @@
  * (-m "not gpu").  The fbar=1 reading (literal Eq.(35)) is pinned
  * by internal consistency only (finite differences, affine fields) — the paper
  * prints no value that would distinguish it: "parity unpinned (reading G12)".
+ *
+ * SURVEY.md 8(f) NEXT-2 (Barlat Yld2004-18p, Eq.(12), App. A.2 :808-830): section "Yld2004-18p" below.
+ * Pins: tests/test_oracle_barlat.py (von Mises / Hill-48 reductions of :828, Hershey closed forms, the eigenvalue
+ * definition against the power-sum form, finite differences, App. D against differences of the return map, and the
+ * printed line-search example of App. B :871-877, zeta = 0.363 at the third iteration).
  */
 #include <math.h>
 #include <stdlib.h>
@@ -474,6 +479,276 @@ void orc_cep_implicit(const double *mat, const double *T6, double alpha, double 
     memcpy(Cep36, B, 36 * sizeof(double));
 }
 
+/* ------------------------------------------------- Yld2004-18p
+ * Barlat record bar[20]: c'12,c'13,c'21,c'23,c'31,c'32,c'44,c'55,c'66, the same nine for C'', m, 0.
+ * Eq.(A7)-(A9) PAPER.md:812-824: s = P:T (deviator), s' = C':s, s'' = C'':s in the material frame;
+ * reading B1: the shear rows follow the component order of App. A.1 (c44 <-> 12, c55 <-> 23, c66 <-> 13), and the
+ * fourth row of [C''] that the print drops (:822) is c''44;
+ * Eq.(12) :133 read as phi = [1/4 sum_{i,j=1..3} |s'_i - s''_j|^m]^(1/m) (reading B2: the print repeats |s'3-s''3|
+ * and omits |s'3-s''1|); yield function f = phi - sigma_flow(alpha), W = 1 (:145) — with all c = 1 phi is the
+ * uniaxial-equivalent stress, so no sqrt(2/3) appears here (the Hill reading G2 makes the two models agree, :828).
+ * Material orientation as for Hill: T_mat = Theta^T T Theta (:826, Eq.(A1) :774).
+ * Derivatives are taken for EVEN INTEGER m (2..16; the paper uses 8, and 2, 4 for its reductions), where
+ * |x|^m = x^m and Phi = sum_ij (a_i - b_j)^m = sum_k binom(m,k) (-1)^k tr(A^(m-k)) tr(B^k) is a polynomial of the
+ * two transformed tensors A = s', B = s'' (power sums of the eigenvalues are traces of powers): its first and
+ * second derivatives are written out with plain index loops, no eigenvectors, no repeated-eigenvalue cases. */
+#define NBAR 20
+static void barlat_maps(const double *bar, double LA[6][6], double LB[6][6]) {
+    /* L' = C'.P and L'' = C''.P as 6x6 Mandel matrices (the shear blocks are diagonal, so Voigt = Mandel there) */
+    double Pd[6][6];
+    memset(Pd, 0, sizeof(Pd));
+    for (int i = 0; i < 3; i++) for (int j = 0; j < 3; j++) Pd[i][j] = ((i == j) ? 2.0 : -1.0) / 3.0;   /* Eq.(A8) :816 */
+    for (int i = 3; i < 6; i++) Pd[i][i] = 1.0;
+    for (int t = 0; t < 2; t++) {
+        const double *c = bar + 9 * t;
+        double Cm[6][6];
+        memset(Cm, 0, sizeof(Cm));
+        Cm[0][1] = -c[0]; Cm[0][2] = -c[1]; Cm[1][0] = -c[2]; Cm[1][2] = -c[3]; Cm[2][0] = -c[4]; Cm[2][1] = -c[5];  /* Eq.(A9) */
+        Cm[3][3] = c[6]; Cm[4][4] = c[7]; Cm[5][5] = c[8];
+        double (*L)[6] = t ? LB : LA;
+        for (int a = 0; a < 6; a++) for (int b = 0; b < 6; b++) { double s = 0; for (int k = 0; k < 6; k++) s += Cm[a][k] * Pd[k][b]; L[a][b] = s; }
+    }
+}
+static void mandel_to_mat(const double m[6], double A[3][3]) { double v[6]; from_mandel6(m, v); sym6_to_mat(v, A); }
+static void matmul3(const double A[3][3], const double B[3][3], double C[3][3]) {
+    for (int i = 0; i < 3; i++) for (int j = 0; j < 3; j++) { double s = 0; for (int k = 0; k < 3; k++) s += A[i][k] * B[k][j]; C[i][j] = s; }
+}
+static double trace3(const double A[3][3]) { return A[0][0] + A[1][1] + A[2][2]; }
+static double binom(int n, int k) { double b = 1; for (int i = 1; i <= k; i++) b = b * (n - k + i) / i; return b; }
+
+/* phi by the DEFINITION: eigenvalues of s', s'' (any real m >= 1).  Tm = stress in the material frame, Mandel. */
+double orc_barlat_phi_eig(const double *bar, const double *Tm) {
+    double LA[6][6], LB[6][6], a6[6], b6[6], A[3][3], B[3][3], a[3], b[3], V[3][3], m = bar[18], s = 0;
+    barlat_maps(bar, LA, LB);
+    mv6(LA, Tm, a6); mv6(LB, Tm, b6);
+    mandel_to_mat(a6, A); mandel_to_mat(b6, B);
+    jacobi3(A, a, V); jacobi3(B, b, V);
+    for (int i = 0; i < 3; i++) for (int j = 0; j < 3; j++) s += pow(fabs(a[i] - b[j]), m);
+    return pow(0.25 * s, 1.0 / m);
+}
+/* phi, N = dphi/dT (Mandel), Hm = d2phi/dT2 (6x6 Mandel, may be NULL) in the material frame, even integer m. */
+void orc_barlat_derivs(const double *bar, const double *Tm, double *phi_out, double *Nm, double *Hm) {
+    int m = (int)bar[18];
+    double LA[6][6], LB[6][6], a6[6], b6[6];
+    double PA[17][3][3], PB[17][3][3], tA[17], tB[17];
+    barlat_maps(bar, LA, LB);
+    mv6(LA, Tm, a6); mv6(LB, Tm, b6);
+    memset(PA, 0, sizeof(PA)); memset(PB, 0, sizeof(PB));
+    for (int i = 0; i < 3; i++) PA[0][i][i] = PB[0][i][i] = 1.0;
+    mandel_to_mat(a6, PA[1]); mandel_to_mat(b6, PB[1]);
+    for (int n = 2; n <= m; n++) { matmul3(PA[n - 1], PA[1], PA[n]); matmul3(PB[n - 1], PB[1], PB[n]); }
+    for (int n = 0; n <= m; n++) { tA[n] = trace3(PA[n]); tB[n] = trace3(PB[n]); }
+    double Phi = 0, GA[3][3], GB[3][3];
+    memset(GA, 0, sizeof(GA)); memset(GB, 0, sizeof(GB));
+    for (int k = 0; k <= m; k++) {
+        double c = binom(m, k) * ((k & 1) ? -1.0 : 1.0);
+        Phi += c * tA[m - k] * tB[k];
+        for (int i = 0; i < 3; i++) for (int j = 0; j < 3; j++) {
+            if (k < m) GA[i][j] += c * (m - k) * tB[k] * PA[m - k - 1][i][j];    /* d tr(A^n)/dA = n A^(n-1) */
+            if (k > 0) GB[i][j] += c * k * tA[m - k] * PB[k - 1][i][j];
+        }
+    }
+    double phi = pow(0.25 * Phi, 1.0 / m);
+    double ga[6], gb[6], gam[6], gbm[6], dPhi[6];
+    mat_to_sym6(GA, ga); mat_to_sym6(GB, gb); to_mandel6(ga, gam); to_mandel6(gb, gbm);
+    for (int a = 0; a < 6; a++) { double s = 0; for (int b = 0; b < 6; b++) s += LA[b][a] * gam[b] + LB[b][a] * gbm[b]; dPhi[a] = s; }
+    double cf = pow(phi, 1.0 - m) / (4.0 * m);      /* phi^m = Phi/4  =>  dphi = phi^(1-m)/(4m) dPhi */
+    for (int a = 0; a < 6; a++) Nm[a] = cf * dPhi[a];
+    *phi_out = phi;
+    if (!Hm) return;
+    /* second derivatives of Phi with respect to (A,A), (A,B), (B,B) as 4-tensors, then Mandel and the chain rule */
+    double HAA[3][3][3][3], HBB[3][3][3][3], HAB[3][3][3][3];
+    memset(HAA, 0, sizeof(HAA)); memset(HBB, 0, sizeof(HBB)); memset(HAB, 0, sizeof(HAB));
+    for (int k = 0; k <= m; k++) {
+        double c = binom(m, k) * ((k & 1) ? -1.0 : 1.0);
+        int n = m - k - 1;                            /* GA term: c (m-k) tB[k] A^n ; d(A^n) = sum_r A^r dA A^(n-1-r) */
+        for (int r = 0; n >= 1 && r < n; r++)
+            for (int i = 0; i < 3; i++) for (int j = 0; j < 3; j++) for (int p = 0; p < 3; p++) for (int q = 0; q < 3; q++)
+                HAA[i][j][p][q] += c * (m - k) * tB[k] * 0.5 * (PA[r][i][p] * PA[n - 1 - r][q][j] + PA[r][i][q] * PA[n - 1 - r][p][j]);
+        int nb = k - 1;                               /* GB term: c k tA[m-k] B^nb */
+        for (int r = 0; nb >= 1 && r < nb; r++)
+            for (int i = 0; i < 3; i++) for (int j = 0; j < 3; j++) for (int p = 0; p < 3; p++) for (int q = 0; q < 3; q++)
+                HBB[i][j][p][q] += c * k * tA[m - k] * 0.5 * (PB[r][i][p] * PB[nb - 1 - r][q][j] + PB[r][i][q] * PB[nb - 1 - r][p][j]);
+        if (k >= 1 && k < m)                          /* d/dB of tB[k] = k B^(k-1) */
+            for (int i = 0; i < 3; i++) for (int j = 0; j < 3; j++) for (int p = 0; p < 3; p++) for (int q = 0; q < 3; q++)
+                HAB[i][j][p][q] += c * (m - k) * k * PA[m - k - 1][i][j] * PB[k - 1][p][q];
+    }
+    double MAA[6][6], MBB[6][6], MAB[6][6], d2Phi[6][6];
+    t4_to_mandel(HAA, MAA); t4_to_mandel(HBB, MBB); t4_to_mandel(HAB, MAB);
+    for (int a = 0; a < 6; a++) for (int b = 0; b < 6; b++) {
+        double s = 0;
+        for (int c = 0; c < 6; c++) for (int d = 0; d < 6; d++)
+            s += LA[c][a] * MAA[c][d] * LA[d][b] + LB[c][a] * MBB[c][d] * LB[d][b] + LA[c][a] * MAB[c][d] * LB[d][b] +
+                 LB[c][a] * MAB[d][c] * LA[d][b];
+        d2Phi[a][b] = s;
+    }
+    for (int a = 0; a < 6; a++) for (int b = 0; b < 6; b++)
+        Hm[a * 6 + b] = cf * d2Phi[a][b] - (m - 1.0) / phi * Nm[a] * Nm[b];
+}
+/* 6x6 Mandel matrix Q of the frame change X_mat = Theta^T X Theta (X_mat = Q X_glob); Q is orthogonal */
+static void mandel_rot(const double Th[3][3], double Q[6][6]) {
+    double R4[3][3][3][3];
+    for (int a = 0; a < 3; a++) for (int b = 0; b < 3; b++) for (int i = 0; i < 3; i++) for (int j = 0; j < 3; j++)
+        R4[a][b][i][j] = 0.5 * (Th[i][a] * Th[j][b] + Th[j][a] * Th[i][b]);
+    t4_to_mandel(R4, Q);
+}
+/* Yield function of either model in the GLOBAL frame: T6 tensor components -> phi, N (Mandel), H = dN/dT (6x6 Mandel
+ * or NULL).  bar == NULL: Hill-48 (phi = sqrt(T:H:T), Eq.(11) :127). */
+void orc_yield_eval(const double *mat, const double *bar, const double *T6, double *phi, double *N, double *H) {
+    double Tg[6];
+    to_mandel6(T6, Tg);
+    if (!bar) {
+        double H6[6][6], HT[6];
+        orc_hill_mandel(mat, &H6[0][0]);
+        mv6(H6, Tg, HT);
+        *phi = sqrt(dot6(Tg, HT));
+        for (int a = 0; a < 6; a++) N[a] = HT[a] / *phi;
+        if (H) for (int a = 0; a < 6; a++) for (int b = 0; b < 6; b++) H[a * 6 + b] = (H6[a][b] - N[a] * N[b]) / *phi;
+        return;
+    }
+    double Th[3][3], Q[6][6], Tm[6], Nm[6], Hm[36];
+    quat_to_rot(mat + 12, Th);
+    mandel_rot(Th, Q);
+    mv6(Q, Tg, Tm);
+    orc_barlat_derivs(bar, Tm, phi, Nm, H ? Hm : NULL);
+    for (int a = 0; a < 6; a++) { double s = 0; for (int b = 0; b < 6; b++) s += Q[b][a] * Nm[b]; N[a] = s; }
+    if (H) for (int a = 0; a < 6; a++) for (int b = 0; b < 6; b++) {
+        double s = 0;
+        for (int c = 0; c < 6; c++) for (int d = 0; d < 6; d++) s += Q[c][a] * Hm[c * 6 + d] * Q[d][b];
+        H[a * 6 + b] = s;
+    }
+}
+/* sigma_y(alpha) and W of Eq.(14)/(20): Hill sqrt(2/3) sigma_flow, W = sqrt(2/3); Barlat sigma_flow, W = 1 (:145) */
+static double yld_W(const double *bar) { return bar ? 1.0 : WHILL; }
+static void yld_sy(const double *mat, const double *bar, double alpha, double *sy, double *dsy) {
+    double s, d;
+    orc_flow(mat, alpha, &s, &d);
+    *sy = yld_W(bar) * s; *dsy = yld_W(bar) * d;
+}
+/* G(y) of Eq.(23), y = [T (Mandel), alpha, dgam]; T rows and f row divided by s0 = sigma_y(alpha_n) (G7) */
+static void gen_G(const double E6[6][6], const double *mat, const double *bar, const double em[6], const double epn[6],
+                  double alphan, double s0, const double y[8], double G[8]) {
+    double T6[6], N[6], ee[6], ET[6], phi, sy, dsy;
+    from_mandel6(y, T6);
+    orc_yield_eval(mat, bar, T6, &phi, N, NULL);
+    for (int a = 0; a < 6; a++) ee[a] = em[a] - epn[a] - y[7] * N[a];
+    mv6(E6, ee, ET);
+    for (int a = 0; a < 6; a++) G[a] = (y[a] - ET[a]) / s0;
+    G[6] = y[6] - alphan - yld_W(bar) * y[7];
+    yld_sy(mat, bar, y[6], &sy, &dsy);
+    G[7] = (phi - sy) / s0;
+}
+/* J^G = dG/dy (paper: by AD, :200; here from the hand-written second derivative), same row scaling as gen_G */
+static void gen_J(const double E6[6][6], const double *mat, const double *bar, double s0, const double y[8], double J[64]) {
+    double T6[6], N[6], H[36], phi, sy, dsy;
+    from_mandel6(y, T6);
+    orc_yield_eval(mat, bar, T6, &phi, N, H);
+    yld_sy(mat, bar, y[6], &sy, &dsy);
+    memset(J, 0, 64 * sizeof(double));
+    for (int a = 0; a < 6; a++) {
+        double EN = 0;
+        for (int b = 0; b < 6; b++) {
+            double s = 0;
+            for (int c = 0; c < 6; c++) s += E6[a][c] * H[c * 6 + b];
+            J[a * 8 + b] = ((a == b) + y[7] * s) / s0;
+            EN += E6[a][b] * N[b];
+        }
+        J[a * 8 + 7] = EN / s0;
+    }
+    J[6 * 8 + 6] = 1.0; J[6 * 8 + 7] = -yld_W(bar);
+    for (int b = 0; b < 6; b++) J[7 * 8 + b] = N[b] / s0;
+    J[7 * 8 + 6] = -dsy / s0;
+}
+/* Alg. C1 steps 2-8 with Alg. C2 step by step for either yield function: elastic predictor, yield
+ * test, Newton on the eight unknowns with the Goldstein line search of App. B Eq.(B1)-(B7) as printed (beta, eta of
+ * :871), recovery (step 27), then C_ep by the implicit differentiation of App. D Eq.(D4)-(D6) :1002-1019.
+ * Iterations run to the round-off floor: stop when |G| <= tol, or when |G| no longer halves after it fell below 1e-9.
+ * trace (may be NULL) [kmax+1][3] = psi(0), psi(1), accepted zeta of every iteration (NaN-filled beyond the last).
+ * Returns 1 if plastic. */
+int orc_return_map_gen(const double *mat, const double *bar, const double *eps6, const double *epn6, double alphan,
+                       double tol, int kmax, int jmax, double beta, double eta, double *T6, double *epnew6,
+                       double *alphanew, double *dgam_out, double *Cep36, int *iters, int *nonconv, double *trace) {
+    double E6[6][6], em[6], epn[6], ee[6], y[8], G[8], s0, d0, phitr, Ntr[6], Ttr6[6];
+    elast_mandel(mat, E6);
+    to_mandel6(eps6, em); to_mandel6(epn6, epn);
+    for (int a = 0; a < 6; a++) ee[a] = em[a] - epn[a];
+    mv6(E6, ee, y); y[6] = alphan; y[7] = 0.0;                       /* Eq.(16) :160; Alg. C2 steps 1-2 */
+    from_mandel6(y, Ttr6);
+    *iters = 0; *nonconv = 0;
+    if (trace) for (int k = 0; k < 3 * (kmax + 1); k++) trace[k] = NAN;
+    yld_sy(mat, bar, alphan, &s0, &d0);
+    {
+        double nrm2 = dot6(y, y);
+        if (nrm2 == 0.0) phitr = 0.0; else orc_yield_eval(mat, bar, Ttr6, &phitr, Ntr, NULL);
+    }
+    if (phitr - s0 <= 0.0) {                                         /* Eq.(17)-(18) :165-172, tie -> elastic (G10) */
+        memcpy(T6, Ttr6, sizeof(Ttr6));
+        for (int a = 0; a < 6; a++) epnew6[a] = epn6[a];
+        *alphanew = alphan; *dgam_out = 0.0;
+        memcpy(Cep36, E6, sizeof(E6));
+        return 0;
+    }
+    double prev = INFINITY;
+    int conv = 0;
+    for (int k = 0; k <= kmax; k++) {
+        gen_G(E6, mat, bar, em, epn, alphan, s0, y, G);
+        double nrm = 0; for (int a = 0; a < 8; a++) nrm += G[a] * G[a]; nrm = sqrt(nrm);
+        *iters = k;
+        if (nrm <= tol || (prev <= 1e-9 && nrm >= 0.5 * prev)) { conv = 1; break; }
+        if (k == kmax) break;
+        prev = nrm;
+        double J[64], rhs[8];
+        gen_J(E6, mat, bar, s0, y, J);
+        for (int a = 0; a < 8; a++) rhs[a] = -G[a];
+        if (solve_dense(8, J, rhs, 1)) break;                        /* Eq.(24) :196 */
+        double psi0 = 0.5 * nrm * nrm, yt[8], Gt[8], zeta = 1.0;
+        for (int a = 0; a < 8; a++) yt[a] = y[a] + rhs[a];
+        gen_G(E6, mat, bar, em, epn, alphan, s0, yt, Gt);
+        double psi1 = 0; for (int a = 0; a < 8; a++) psi1 += Gt[a] * Gt[a]; psi1 *= 0.5;
+        if (!(psi1 < (1 - 2 * beta) * psi0)) {                       /* Eq.(B3) :852 */
+            double zj = psi0 / (psi0 + psi1);                        /* Eq.(B5) :858 */
+            zeta = zj;
+            for (int j = 0; j <= jmax; j++) {
+                for (int a = 0; a < 8; a++) yt[a] = y[a] + zj * rhs[a];
+                gen_G(E6, mat, bar, em, epn, alphan, s0, yt, Gt);
+                double psij = 0; for (int a = 0; a < 8; a++) psij += Gt[a] * Gt[a]; psij *= 0.5;
+                if (j == 0 && psij < (1 - 2 * beta * zj) * psi0) break;   /* the first trial already passes Eq.(B3) */
+                double zn = psi0 / (psi0 + psij);                    /* Eq.(B6) :862 */
+                zn = fmax(eta * zj, zn);                             /* Eq.(B7) :866 */
+                for (int a = 0; a < 8; a++) yt[a] = y[a] + zn * rhs[a];
+                gen_G(E6, mat, bar, em, epn, alphan, s0, yt, Gt);
+                double psin = 0; for (int a = 0; a < 8; a++) psin += Gt[a] * Gt[a]; psin *= 0.5;
+                zeta = zn;
+                if (psin < (1 - 2 * beta * zn) * psi0) break;
+                zj = zn;
+            }
+        }
+        if (trace) { trace[3 * k] = psi0; trace[3 * k + 1] = psi1; trace[3 * k + 2] = zeta; }
+        for (int a = 0; a < 8; a++) y[a] += zeta * rhs[a];
+    }
+    if (!conv) *nonconv = 1;
+    /* Alg. C2 step 27 :979: eps_p = eps_p_n + dgam N, T = E:(eps - eps_p) */
+    double Tc6[6], N[6], phi, epm[6], Tm[6];
+    from_mandel6(y, Tc6);
+    orc_yield_eval(mat, bar, Tc6, &phi, N, NULL);
+    for (int a = 0; a < 6; a++) epm[a] = epn[a] + y[7] * N[a];
+    for (int a = 0; a < 6; a++) ee[a] = em[a] - epm[a];
+    mv6(E6, ee, Tm);
+    from_mandel6(Tm, T6);
+    from_mandel6(epm, epnew6);
+    *alphanew = y[6]; *dgam_out = y[7];
+    /* App. D: J_y ydot = -dG/deps edot, unscaled rows; the T rows of the solution are C_ep (6x6 Mandel) */
+    double yc[8], J[64], B[48];
+    for (int a = 0; a < 6; a++) yc[a] = Tm[a];
+    yc[6] = y[6]; yc[7] = y[7];
+    gen_J(E6, mat, bar, 1.0, yc, J);
+    memset(B, 0, sizeof(B));
+    for (int a = 0; a < 6; a++) for (int b = 0; b < 6; b++) B[a * 6 + b] = E6[a][b];
+    solve_dense(8, J, B, 6);
+    memcpy(Cep36, B, 36 * sizeof(double));
+    return 1;
+}
+
 /* ------------------------------------------------- O9: divided differences of g(lam) = 1/2 ln(lam)
  * first:  g[a,b] = 1/2 log1p((lb-la)/la)/(lb-la),  g[a,a] = 1/(2 la)
  * second: recursive formula on the widest gap; series about the mean when the spread is small:
@@ -559,15 +834,25 @@ void orc_postprocess(const double *lam, const double *Rm /*[3][3]*/, const doubl
 /* ------------------------------------------------- Alg. C1 at one point + O10
  * in: F (row-major F_iJ), hist_in (ep6, alpha), mat.  out: P[3][3], A[3][3][3][3] = dP_iJ/dF_kL, hist_out[7].
  * flags: bit0 plastic, bit1 local solve not converged, bit2 det F <= 0. */
+static const double *g_dummy_bar = 0;
+int orc_point_yld(const double *mat, const double *bar, const double *F, const double *hin, double *P, double *A, double *hout,
+                  double *S6out, double *T6out, double *CL36out, int *iters);
 int orc_point(const double *mat, const double *F, const double *hin, double *P, double *A, double *hout, double *S6out,
               double *T6out, double *CL36out, int *iters) {
+    return orc_point_yld(mat, g_dummy_bar, F, hin, P, A, hout, S6out, T6out, CL36out, iters);
+}
+/* bar == NULL: Hill-48 (bracketed scalar solver); else Yld2004-18p through Alg. C2 (orc_return_map_gen) */
+int orc_point_yld(const double *mat, const double *bar, const double *F, const double *hin, double *P, double *A, double *hout,
+                  double *S6out, double *T6out, double *CL36out, int *iters) {
     double eps[6], lam[3], R[9], T6[6], Cep[36], S6[6], CL[36], dg, an;
     int nonconv, flags = 0;
     double Fm[3][3];
     memcpy(Fm, F, sizeof(Fm));
     if (det3(Fm) <= 0.0) flags |= 4;
     orc_logstrain(F, eps, lam, R);
-    int pl = orc_return_map(mat, eps, hin, hin[6], T6, hout, &an, &dg, Cep, iters, &nonconv);
+    int pl = bar ? orc_return_map_gen(mat, bar, eps, hin, hin[6], 1e-14, 100, 20, 1e-4, 0.1, T6, hout, &an, &dg, Cep, iters,
+                                      &nonconv, NULL)
+                 : orc_return_map(mat, eps, hin, hin[6], T6, hout, &an, &dg, Cep, iters, &nonconv);
     hout[6] = an;
     if (pl) flags |= 1;
     if (nonconv) flags |= 2;
@@ -596,8 +881,14 @@ int orc_point(const double *mat, const double *F, const double *hin, double *P, 
  * X[8][3], u[8][3], hin[8][7] -> Re[24], Ke[24][24] (a = 3*I+i), hout[8][7].
  * fbar=1: Eq.(31)-(32) :237-243, residual contracts P(Fbar) directly with grad N (reading G12).
  * stats[0..3] += plastic, nonconverged, detF<=0, (unused); returns max local iterations. */
+int orc_element_yld(const double *X, const double *u, const double *hin, const double *mat, const double *bar, int fbar,
+                    double *Re, double *Ke, double *hout, long long *stats);
 int orc_element(const double *X, const double *u, const double *hin, const double *mat, int fbar, double *Re, double *Ke,
                 double *hout, long long *stats) {
+    return orc_element_yld(X, u, hin, mat, g_dummy_bar, fbar, Re, Ke, hout, stats);
+}
+int orc_element_yld(const double *X, const double *u, const double *hin, const double *mat, const double *bar, int fbar,
+                    double *Re, double *Ke, double *hout, long long *stats) {
     double G[8][24], w[8], F[8][9], Jq[8], V = 0, Jbar = 0;
     int maxit = 0;
     memset(Re, 0, 24 * sizeof(double));
@@ -631,7 +922,7 @@ int orc_element(const double *X, const double *u, const double *hin, const doubl
         int it;
         if (fbar) c = cbrt(Jbar / Jq[q]);
         for (int m = 0; m < 9; m++) Fb[m] = c * F[q][m];
-        int fl = orc_point(mat, Fb, hin + q * 7, P, A, hout + q * 7, 0, 0, 0, &it);
+        int fl = orc_point_yld(mat, bar, Fb, hin + q * 7, P, A, hout + q * 7, 0, 0, 0, &it);
         if (it > maxit) maxit = it;
         if (stats) { stats[0] += fl & 1; stats[1] += (fl >> 1) & 1; stats[2] += (Jq[q] <= 0.0); }
         for (int I = 0; I < 8; I++) for (int i = 0; i < 3; i++) {
@@ -712,9 +1003,19 @@ long long orc_pattern(long long n_nodes, long long n_elems, const int *conn, int
  * Elements evaluated in parallel chunks; contributions added in ascending element id in long double,
  * rounded once; outputs overwritten.  mat: n_mat == 1 (uniform) or n_elems records.
  * stats[0..3] = plastic, nonconverged, detF<=0, max local iterations. */
+int orc_assemble_yld(long long n_nodes, const double *coords, long long n_elems, const int *conn, int fbar, const double *u,
+                     const double *hist_in, const double *mat, long long n_mat, const double *bar, const int *row_ptr,
+                     const int *col_idx, double *residual, double *csr_vals, double *hist_out, long long *stats);
 int orc_assemble(long long n_nodes, const double *coords, long long n_elems, const int *conn, int fbar, const double *u,
                  const double *hist_in, const double *mat, long long n_mat, const int *row_ptr, const int *col_idx,
                  double *residual, double *csr_vals, double *hist_out, long long *stats) {
+    return orc_assemble_yld(n_nodes, coords, n_elems, conn, fbar, u, hist_in, mat, n_mat, g_dummy_bar, row_ptr, col_idx, residual,
+                            csr_vals, hist_out, stats);
+}
+/* bar: NULL (Hill-48) or n_mat records of NBAR doubles (Yld2004-18p) */
+int orc_assemble_yld(long long n_nodes, const double *coords, long long n_elems, const int *conn, int fbar, const double *u,
+                     const double *hist_in, const double *mat, long long n_mat, const double *bar, const int *row_ptr,
+                     const int *col_idx, double *residual, double *csr_vals, double *hist_out, long long *stats) {
     long long nnz = row_ptr[3 * n_nodes], CH = 8192;
     long double *acc = calloc(nnz, sizeof(long double)), *racc = calloc(3 * n_nodes, sizeof(long double));
     double *Kc = malloc(CH * 576 * sizeof(double)), *Rc = malloc(CH * 24 * sizeof(double));
@@ -732,8 +1033,9 @@ int orc_assemble(long long n_nodes, const double *coords, long long n_elems, con
                     X[a * 3 + i] = coords[3 * (long long)conn[e * 8 + a] + i];
                     ue[a * 3 + i] = u[3 * (long long)conn[e * 8 + a] + i];
                 }
-                int it = orc_element(X, ue, hist_in + e * 56, mat + (n_mat == 1 ? 0 : e * NPAR), fbar, Rc + (e - e0) * 24,
-                                     Kc + (e - e0) * 576, hist_out + e * 56, ls);
+                int it = orc_element_yld(X, ue, hist_in + e * 56, mat + (n_mat == 1 ? 0 : e * NPAR),
+                                         bar ? bar + (n_mat == 1 ? 0 : e * NBAR) : bar, fbar, Rc + (e - e0) * 24,
+                                         Kc + (e - e0) * 576, hist_out + e * 56, ls);
                 if (it > ls[3]) ls[3] = it;
             }
             #pragma omp critical
