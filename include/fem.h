@@ -25,6 +25,7 @@ extern "C" {
 #endif
 
 #define FEM_NPAR 16 /* doubles per material record, see fem_assemble */
+#define FEM_NBARLAT 20 /* doubles per Yld2004-18p record, see fem_assemble_barlat */
 
 enum {
     FEM_OK = 0,
@@ -117,6 +118,21 @@ int fem_build_csr_pattern(fem_ctx *c, long long *n_rows, long long *nnz, const i
  * Physics trouble (local non-convergence, det F <= 0, non-finite) is counted in stats, never an error return. */
 int fem_assemble(fem_ctx *c, const double *u, const double *hist_in, const double *mat, long long n_mat,
                  double *residual, double *csr_vals, double *hist_out, fem_stats *stats, void *cuda_stream);
+
+/* fem_assemble_barlat — SURVEY.md section 8(f) NEXT-2: the same pass with the Barlat Yld2004-18p yield function
+ * (Eq.(12); App. A.2 :808-830 Eq.(A7)-(A9)) in place of Hill-48: phi = [1/4 sum_{i,j} |s'_i - s''_j|^m]^(1/m)
+ * over the eigenvalues of s' = C':P:T and s'' = C'':P:T, f = phi - sigma_flow(alpha), W = 1 (:145), return map of
+ * Eq.(19)-(24) :176-196 by Newton iterations with the Goldstein line search of App. B :836-869 (beta = 1e-4, eta = 0.1).
+ *   barlat    dev [n_mat*20]  c'12,c'13,c'21,c'23,c'31,c'32,c'44,c'55,c'66, the same nine of C'', m, 0
+ *                             (Table 2 :471-477 order; shear rows in the component order 12,23,13; m an even integer 2..16 —
+ *                             the paper uses 8, and 2, 4 for its reductions — other values give undefined results)
+ *   mat       as in fem_assemble; r11..r13 are ignored, E, nu, the hardening law and the orientation quaternion apply
+ * All other arguments, the outputs, determinism and error behaviour are those of fem_assemble.  Requires assembly_mode 0
+ * (FEM_ERR_ARG otherwise); opt.kmax caps the Newton iterations, opt.tol is unused (the iteration stops at the round-off
+ * floor of the residual).  Launches one more (tiny) kernel than fem_assemble. */
+int fem_assemble_barlat(fem_ctx *c, const double *u, const double *hist_in, const double *mat, const double *barlat,
+                        long long n_mat, double *residual, double *csr_vals, double *hist_out, fem_stats *stats,
+                        void *cuda_stream);
 
 /* Same call with HOST buffers for every array: copies in, assembles, copies out, synchronises (used for end-to-end timing). */
 int fem_assemble_host(fem_ctx *c, const double *u, const double *hist_in, const double *mat, long long n_mat,

@@ -5,4 +5,4 @@ Every step of the path runs in the CUDA kernels of csrc/; this module only marsh
 if the shared library is missing, or no CUDA device is visible, calls raise.
 """
 from .binding import (FemContext, FemError, FemOptions, FemStats, FemNewtonOptions, FemNewtonReport, NPAR, hill_from_lankford, lib, lib_path,  # noqa: F401
-                      mat_from_desc, mat_record, probe_fp64_peak, ABI_SYMBOLS)
+                      mat_from_desc, mat_record, barlat_record, NBARLAT, probe_fp64_peak, ABI_SYMBOLS)

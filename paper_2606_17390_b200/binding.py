@@ -6,8 +6,9 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 NPAR = 16
+NBARLAT = 20
 
-ABI_SYMBOLS = ["fem_default_options", "fem_setup", "fem_build_csr_pattern", "fem_assemble", "fem_assemble_host",
+ABI_SYMBOLS = ["fem_default_options", "fem_setup", "fem_build_csr_pattern", "fem_assemble", "fem_assemble_barlat", "fem_assemble_host",
                "fem_last_kernel_ms", "fem_launches_per_assemble", "fem_probe_fp64_peak", "fem_destroy", "fem_strerror",
                "fem_last_cuda_error", "fem_hill_from_lankford", "fem_spmv", "fem_apply_dirichlet", "fem_bicgstab", "fem_pcg", "fem_lincomb",
                "fem_default_newton_options", "fem_newton_solve"]
@@ -79,6 +80,7 @@ def lib():
         L.fem_setup.argtypes = [C.POINTER(vp), ll, vp, ll, vp, C.POINTER(FemOptions)]
         L.fem_build_csr_pattern.argtypes = [vp, C.POINTER(ll), C.POINTER(ll), C.POINTER(vp), C.POINTER(vp), C.POINTER(vp)]
         L.fem_assemble.argtypes = [vp, vp, vp, vp, ll, vp, vp, vp, C.POINTER(FemStats), vp]
+        L.fem_assemble_barlat.argtypes = [vp, vp, vp, vp, vp, ll, vp, vp, vp, C.POINTER(FemStats), vp]
         L.fem_assemble_host.argtypes = [vp, vp, vp, vp, ll, vp, vp, vp, C.POINTER(FemStats)]
         L.fem_last_kernel_ms.argtypes = [vp, dp]
         L.fem_launches_per_assemble.argtypes = [vp]
@@ -116,6 +118,11 @@ def hill_from_lankford(r0, r45, r90):
 def mat_record(E, nu, r, law, h0, h1, h2, quat=(1.0, 0.0, 0.0, 0.0)):
     """One FEM_NPAR record: E,nu,r11,r22,r33,r12,r23,r13,law(0 Voce,1 Swift),h0,h1,h2,q0..q3."""
     return np.array([E, nu, *r, law, h0, h1, h2, *quat], dtype=np.float64)
+
+
+def barlat_record(cp, cpp, m):
+    """One FEM_NBARLAT record: c'12,c'13,c'21,c'23,c'31,c'32,c'44,c'55,c'66, the same nine of C'', m, 0 (PAPER.md:471-477 order)."""
+    return np.array([*cp, *cpp, float(m), 0.0], dtype=np.float64)
 
 
 def mat_from_desc(desc, n_elems):
@@ -196,8 +203,9 @@ class FemContext:
         elem_slot = copy(es, 576 * self.n_elems).view(self.n_elems, 576) if want_elem_slot else None
         return row_ptr, col_idx, elem_slot
 
-    def assemble(self, u, hist_in, mat, residual=None, csr_vals=None, hist_out=None, want_stats=False):
-        """One fem_assemble call on the current torch stream.  Returns (residual, csr_vals, hist_out, stats|None)."""
+    def assemble(self, u, hist_in, mat, residual=None, csr_vals=None, hist_out=None, want_stats=False, barlat=None):
+        """One fem_assemble call (fem_assemble_barlat when `barlat` records are given) on the current torch stream.
+        Returns (residual, csr_vals, hist_out, stats|None)."""
         torch = _torch()
         if self.nnz is None:
             raise FemError(-7, "fem_assemble")
@@ -210,6 +218,13 @@ class FemContext:
         if hist_out is None:
             hist_out = torch.empty(self.n_elems * 56, dtype=f64, device=self.device)
         st = FemStats() if want_stats else None
+        if barlat is not None:
+            _check(lib().fem_assemble_barlat(self._h, _ptr(u, f64, self.n_rows, "u"), _ptr(hist_in, f64, 56 * self.n_elems, "hist_in"),
+                                             _ptr(mat, f64, None, "mat"), _ptr(barlat, f64, NBARLAT * n_mat, "barlat"), n_mat,
+                                             _ptr(residual, f64, self.n_rows, "residual"), _ptr(csr_vals, f64, self.nnz, "csr_vals"),
+                                             _ptr(hist_out, f64, 56 * self.n_elems, "hist_out"),
+                                             C.byref(st) if want_stats else None, _stream_ptr()), "fem_assemble_barlat")
+            return residual, csr_vals, hist_out, (st.as_dict() if want_stats else None)
         _check(lib().fem_assemble(self._h, _ptr(u, f64, self.n_rows, "u"), _ptr(hist_in, f64, 56 * self.n_elems, "hist_in"),
                                   _ptr(mat, f64, None, "mat"), n_mat, _ptr(residual, f64, self.n_rows, "residual"),
                                   _ptr(csr_vals, f64, self.nnz, "csr_vals"), _ptr(hist_out, f64, 56 * self.n_elems, "hist_out"),

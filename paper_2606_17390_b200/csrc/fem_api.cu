@@ -35,6 +35,25 @@ extern "C" int fem_assemble(fem_ctx *c, const double *u, const double *hist_in, 
     return FEM_OK;
 }
 
+extern "C" int fem_assemble_barlat(fem_ctx *c, const double *u, const double *hist_in, const double *mat, const double *barlat,
+                                   long long n_mat, double *residual, double *csr_vals, double *hist_out, fem_stats *stats,
+                                   void *cuda_stream) {
+    if (!c || !u || !hist_in || !mat || !barlat || !residual || !csr_vals || !hist_out) return FEM_ERR_NULL;
+    if (!c->has_pattern) return FEM_ERR_NO_PATTERN;
+    if (n_mat != 1 && n_mat != c->n_elems) return FEM_ERR_MAT;
+    if (c->mode != 0) return FEM_ERR_ARG;
+    {
+        const char *a = (const char *)hist_in, *b = (const char *)hist_out;
+        const size_t bytes = sizeof(double) * 56 * (size_t)c->n_elems;
+        if (a < b + bytes && b < a + bytes) return FEM_ERR_ALIAS;
+    }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int rc = fem_launch_assemble(c, u, hist_in, mat, n_mat, residual, csr_vals, hist_out, st, barlat);
+    if (rc != FEM_OK) return rc;
+    if (stats) return fem_read_stats(c, stats, st);
+    return FEM_OK;
+}
+
 extern "C" int fem_assemble_host(fem_ctx *c, const double *u, const double *hist_in, const double *mat, long long n_mat,
                                  double *residual, double *csr_vals, double *hist_out, fem_stats *stats) {
     if (!c || !u || !hist_in || !mat || !residual || !csr_vals || !hist_out) return FEM_ERR_NULL;
@@ -82,7 +101,7 @@ extern "C" int fem_last_kernel_ms(fem_ctx *c, double ms[3]) {
 
 extern "C" int fem_launches_per_assemble(const fem_ctx *c) {
     if (!c) return 0;
-    return c->mode == 1 ? 1 + c->n_colours : 3;   // mat_prep + one element launch per colour | mat_prep + element (+ fused gather) + gather / drain
+    return c->mode == 1 ? 1 + c->n_colours : 3;   // (+1 for fem_assemble_barlat: its coefficient pre-pass)   // mat_prep + one element launch per colour | mat_prep + element (+ fused gather) + gather / drain
 }
 
 // ------------------------------------------------------------------------------------------------ FP64 peak probe

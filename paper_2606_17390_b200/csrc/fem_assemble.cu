@@ -186,6 +186,8 @@ __device__ __forceinline__ void flow_stress(double law, double h0, double h1, do
     }
 }
 
+#include "fem_barlat.cuh"
+
 // ------------------------------------------------------------------------------------------------ node gather (S14), shared
 // by the stand-alone gather kernels and by the gather CTAs of the fused mode.
 // The scratch is destination-major: node n's contributions are the records inc_ptr[n] .. inc_ptr[n+1]-1 (72 doubles each:
@@ -320,12 +322,14 @@ struct scatter_args {
 #ifndef EL_PERSIST
 #define EL_PERSIST 0   // persistent CTAs with input prefetch measured slower (3.31 vs 3.13 ms): the CTAs of an SM stay in phase
 #endif
-template <int FBAR, int MODE>
-__global__ void __launch_bounds__(CTA_THREADS, FBAR ? CTAS_FBAR : CTAS_STD)
+// YLD 0: Hill-48 (scalar return map); YLD 1: Barlat Yld2004-18p (fem_barlat.cuh), bard = derived Barlat records
+template <int FBAR, int MODE, int YLD = 0>
+__global__ void __launch_bounds__(CTA_THREADS, (FBAR || YLD) ? CTAS_FBAR : CTAS_STD)
 k_element(long long n_elems, const double *__restrict__ coords, const int *__restrict__ conn,
           const double *__restrict__ u, const double *__restrict__ hist_in, const double *__restrict__ matd,
           int mat_stride, double tol, int kmax, double *__restrict__ Ke, double *__restrict__ Re,
-          double *__restrict__ hist_out, unsigned long long *__restrict__ stats, const scatter_args sa) {
+          double *__restrict__ hist_out, unsigned long long *__restrict__ stats, const scatter_args sa,
+          const double *__restrict__ bard = nullptr, int bar_stride = 0) {
     extern __shared__ __align__(16) double sm[];
     __shared__ unsigned int s_hist[64];
     __shared__ unsigned int s_done;
@@ -588,6 +592,79 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
     for (int i = 0; i < 6; i++) ee[i] -= epm[i];
 
     PHASE_SYNC_N(2);
+    double Ch[6][6];   // C_ep in the eigenbasis of C, tensor components, upper triangle used
+    double Tt[6];      // T in the eigenbasis of C
+    int iters = 0;
+    bool plastic = false, nonconv = false;
+    if (YLD == 1) {
+        // ---- S6-S8, S10 for Yld2004-18p: general return map in the material frame (fem_barlat.cuh), then C_ep and T are
+        //      taken to the eigenbasis of C with the 6x6 matrix Q[A][I]: X^_A (tensor components) = sum_I Q[A][I] X_I (Mandel)
+        const double law = __ldg(md + 3), hh0 = __ldg(md + 4), hh1 = __ldg(md + 5), hh2 = __ldg(md + 6);
+        double Tm[6], dep[6], Cm[6][6], dg;
+        bar_return_map(bard + (long long)bar_stride * e, mu2, kb, law, hh0, hh1, hh2, ee, alphan, kmax, Tm, dep, Cm, dg, iters,
+                       plastic, nonconv);
+        if (valid) {
+            double *ho = hist_out + (e * 8 + q) * 7;
+            double ep1[6];
+#pragma unroll
+            for (int i = 0; i < 6; i++) ep1[i] = epm[i] + dep[i];
+            if (rot && plastic) {
+                const double A[3][3] = {{ep1[0], ep1[3], ep1[5]}, {ep1[3], ep1[1], ep1[4]}, {ep1[5], ep1[4], ep1[2]}};
+                double B[3][3];  // B = A Theta^T ; out = Theta B
+#pragma unroll
+                for (int i = 0; i < 3; i++)
+#pragma unroll
+                    for (int j = 0; j < 3; j++) B[i][j] = A[i][0] * Th[j][0] + A[i][1] * Th[j][1] + A[i][2] * Th[j][2];
+                ep1[0] = Th[0][0] * B[0][0] + Th[0][1] * B[1][0] + Th[0][2] * B[2][0];
+                ep1[1] = Th[1][0] * B[0][1] + Th[1][1] * B[1][1] + Th[1][2] * B[2][1];
+                ep1[2] = Th[2][0] * B[0][2] + Th[2][1] * B[1][2] + Th[2][2] * B[2][2];
+                ep1[3] = Th[0][0] * B[0][1] + Th[0][1] * B[1][1] + Th[0][2] * B[2][1];
+                ep1[4] = Th[1][0] * B[0][2] + Th[1][1] * B[1][2] + Th[1][2] * B[2][2];
+                ep1[5] = Th[0][0] * B[0][2] + Th[0][1] * B[1][2] + Th[0][2] * B[2][2];
+            }
+            if (!plastic) {
+#pragma unroll
+                for (int i = 0; i < 6; i++) ep1[i] = epn[i];  // elastic step: history copied unchanged (Eq.(18) :172)
+            }
+#pragma unroll
+            for (int i = 0; i < 6; i++) ho[i] = ep1[i];
+            ho[6] = alphan + dg;                              // Eq.(20) :178 with W = 1 (:145)
+        }
+        double Q[6][6];
+#pragma unroll
+        for (int A = 0; A < 6; A++) {
+            const int a = (A < 3) ? A : (A == 3 ? 0 : (A == 4 ? 1 : 0)), b = (A < 3) ? A : (A == 3 ? 1 : 2);
+#pragma unroll
+            for (int I = 0; I < 6; I++) {
+                const int i = (I < 3) ? I : (I == 3 ? 0 : (I == 4 ? 1 : 0)), j = (I < 3) ? I : (I == 3 ? 1 : 2);
+                Q[A][I] = (I < 3) ? Rm[i][a] * Rm[i][b] : RSQRT2 * (Rm[i][a] * Rm[j][b] + Rm[j][a] * Rm[i][b]);
+            }
+        }
+        double QC[6][6];
+#pragma unroll
+        for (int A = 0; A < 6; A++) {
+            double t = 0.0;
+#pragma unroll
+            for (int I = 0; I < 6; I++) t = fma(Q[A][I], Tm[I], t);
+            Tt[A] = t;
+#pragma unroll
+            for (int J = 0; J < 6; J++) {
+                double s = 0.0;
+#pragma unroll
+                for (int I = 0; I < 6; I++) s = fma(Q[A][I], (I <= J) ? Cm[I][J] : Cm[J][I], s);
+                QC[A][J] = s;
+            }
+        }
+#pragma unroll
+        for (int A = 0; A < 6; A++)
+#pragma unroll
+            for (int B = A; B < 6; B++) {
+                double s = 0.0;
+#pragma unroll
+                for (int J = 0; J < 6; J++) s = fma(QC[A][J], Q[B][J], s);
+                Ch[A][B] = s;
+            }
+    } else {
     // ---- S6 elastic predictor in the Hill eigenbasis: T_tr = p I + s, s = 2mu dev(ee) = sum_k c_k v_k (Eq.(16) :160)
     const double tre = ee[0] + ee[1] + ee[2];
     const double pres = kb * tre;
@@ -616,8 +693,6 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
     double dg = 0.0, sf = 0.0, dsf = 0.0;
     double rk[5] = {1.0, 1.0, 1.0, 1.0, 1.0};   // 1/(1 + x h_k)
     double phi2 = phitr2;
-    int iters = 0;
-    bool plastic = false, nonconv = false;
     {
         double lo = 0.0, hi = INFINITY;
         const double atol = 4.0e-16 * phitr / mu2;  // round-off floor of dgam (a strain): eps * |T| / 2mu
@@ -732,8 +807,9 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
     PHASE_SYNC_N(4);
     // ---- S8 algorithmic tangent in the eigenbasis of C (App. D :1002-1019 in closed form):
     //      C_ep = kb I(x)I + sum_k theta_k V^_k (x) V^_k + beta m^ (x) m^ ,  V^_k = Rm^T V_k Rm ; T^ = p I + sum c'_k V^_k
-    double Ch[6][6];   // tensor components, upper triangle used
-    double Tt[6] = {pres, pres, pres, 0.0, 0.0, 0.0}, mh[6] = {0, 0, 0, 0, 0, 0};
+    double mh[6] = {0, 0, 0, 0, 0, 0};
+#pragma unroll
+    for (int A = 0; A < 6; A++) Tt[A] = (A < 3) ? pres : 0.0;
 #pragma unroll
     for (int A = 0; A < 6; A++)
 #pragma unroll
@@ -771,6 +847,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
 #pragma unroll
         for (int B = A; B < 6; B++) Ch[A][B] = fma(bm, mh[B], Ch[A][B]);
     }
+    }   // YLD == 0
 
     PHASE_SYNC_N(5);
     // ---- S9 geometric post-processor (Eq.(25) :204, analytic route of :288): with g = 1/2 ln,
@@ -1353,7 +1430,14 @@ k_gather_drain(unsigned int n_nodes, const int *__restrict__ queue, unsigned int
 static inline unsigned nblk2(long long n, int bs) { return (unsigned)((n + bs - 1) / bs); }
 
 int fem_launch_assemble(fem_ctx *c, const double *u, const double *hist_in, const double *mat, long long n_mat,
-                        double *residual, double *csr_vals, double *hist_out, cudaStream_t st) {
+                        double *residual, double *csr_vals, double *hist_out, cudaStream_t st, const double *bar) {
+    if (bar && c->mode != 0) return FEM_ERR_ARG;   // Yld2004-18p runs in assembly mode 0 only
+    if (bar && n_mat > c->n_bard_cap) {
+        if (c->d_bard) cudaFree(c->d_bard);
+        c->d_bard = nullptr; c->n_bard_cap = 0;
+        FEM_CUDA(cudaMalloc(&c->d_bard, sizeof(double) * FEM_BARD * n_mat));
+        c->n_bard_cap = n_mat;
+    }
     if (n_mat > c->n_matd_cap) {
         if (c->d_matd) cudaFree(c->d_matd);
         c->d_matd = nullptr; c->n_matd_cap = 0;
@@ -1373,6 +1457,7 @@ int fem_launch_assemble(fem_ctx *c, const double *u, const double *hist_in, cons
     FEM_CUDA(cudaMemsetAsync(c->d_stats, 0, sizeof(unsigned long long) * 72, st));
     FEM_CUDA(cudaEventRecord(c->ev[0], st));
     k_mat_prep<<<nblk2(n_mat, 128), 128, 0, st>>>(n_mat, mat, c->d_matd);
+    if (bar) k_bar_prep<<<nblk2(n_mat, 128), 128, 0, st>>>(n_mat, bar, c->d_bard);
     FEM_CUDA(cudaEventRecord(c->ev[1], st));
     const int mstride = (n_mat == 1) ? 0 : FEM_MATD;
     scatter_args sa = {c->mode == 0 ? c->d_eorder : nullptr, c->d_eslot, c->d_nb_ptr, c->d_elem_pos, c->d_first_mask, c->d_first_res, csr_vals, residual,
@@ -1433,6 +1518,23 @@ int fem_launch_assemble(fem_ctx *c, const double *u, const double *hist_in, cons
         }
         const unsigned n_chunks = nblk2(c->n_elems, EL_PER_CTA);
         const unsigned grid = (!EL_PERSIST || n_chunks < (unsigned)wave[c->opt.fbar ? 1 : 0]) ? n_chunks : (unsigned)wave[c->opt.fbar ? 1 : 0];
+        if (bar) {
+            static bool attr3 = false;
+            if (!attr3) {
+                FEM_CUDA(cudaFuncSetAttribute(k_element<0, 0, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_std));
+                FEM_CUDA(cudaFuncSetAttribute(k_element<1, 0, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_fbar));
+                attr3 = true;
+            }
+            const int bstride = (n_mat == 1) ? 0 : FEM_BARD;
+            if (c->opt.fbar)
+                k_element<1, 0, 1><<<n_chunks, CTA_THREADS, sm_fbar, st>>>(c->n_elems, c->d_coords, c->d_conn, u, hist_in, c->d_matd, mstride,
+                                                                   c->opt.tol, c->opt.kmax, c->d_Ke, c->d_Re, hist_out, c->d_stats, sa,
+                                                                   c->d_bard, bstride);
+            else
+                k_element<0, 0, 1><<<n_chunks, CTA_THREADS, sm_std, st>>>(c->n_elems, c->d_coords, c->d_conn, u, hist_in, c->d_matd, mstride,
+                                                                  c->opt.tol, c->opt.kmax, c->d_Ke, c->d_Re, hist_out, c->d_stats, sa,
+                                                                  c->d_bard, bstride);
+        } else
         if (c->opt.fbar)
             k_element<1, 0><<<grid, CTA_THREADS, sm_fbar, st>>>(c->n_elems, c->d_coords, c->d_conn, u, hist_in, c->d_matd, mstride,
                                                         c->opt.tol, c->opt.kmax, c->d_Ke, c->d_Re, hist_out, c->d_stats, sa);

@@ -48,6 +48,8 @@ struct fem_ctx {
     double *d_Re = nullptr;      // [8*n_elems][3]  R^e_I of incidence entry j
     double *d_matd = nullptr;    // [n_mat_cap*FEM_MATD]
     long long n_matd_cap = 0;
+    double *d_bard = nullptr;    // [n_bard_cap*FEM_BARD] derived Yld2004-18p records (fem_barlat.cuh)
+    long long n_bard_cap = 0;
     unsigned long long *d_stats = nullptr;  // [4 + 1 + 64] counters
     // NEXT-1 (fem_solve.cu): Dirichlet rows, SpMV, BiCGSTAB, Newton loop -- workspace allocated on first use
     int *d_diagpos = nullptr;      // [n_nodes] position of node n in its own neighbour list (diagonal block)
@@ -78,4 +80,4 @@ int fem_read_stats(fem_ctx *c, fem_stats *stats, cudaStream_t st);
 int fem_build_colouring(fem_ctx *c);
 // fem_assemble.cu
 int fem_launch_assemble(fem_ctx *c, const double *u, const double *hist_in, const double *mat, long long n_mat,
-                        double *residual, double *csr_vals, double *hist_out, cudaStream_t st);
+                        double *residual, double *csr_vals, double *hist_out, cudaStream_t st, const double *bar = nullptr);

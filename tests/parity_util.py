@@ -11,7 +11,7 @@ def rel_l2(a, b):
     return np.linalg.norm(a - b) / nb if nb > 0 else np.linalg.norm(a)
 
 
-def run_gpu(cfg, fbar=0, want_elem_slot=False, mat=None, assembly_mode=None):
+def run_gpu(cfg, fbar=0, want_elem_slot=False, mat=None, assembly_mode=None, barlat=None):
     import torch
     import paper_2606_17390_b200 as fem
     dev = torch.device("cuda:0")
@@ -22,7 +22,8 @@ def run_gpu(cfg, fbar=0, want_elem_slot=False, mat=None, assembly_mode=None):
                          assembly_mode=assembly_mode)
     row_ptr, col_idx, slots = ctx.build_csr_pattern(want_elem_slot=want_elem_slot)
     res, vals, hout, stats = ctx.assemble(torch.from_numpy(cfg["u"].ravel()).to(dev), torch.from_numpy(cfg["hist_in"].ravel()).to(dev),
-                                          torch.from_numpy(np.ascontiguousarray(mat).ravel()).to(dev), want_stats=True)
+                                          torch.from_numpy(np.ascontiguousarray(mat).ravel()).to(dev), want_stats=True,
+                                          barlat=None if barlat is None else torch.from_numpy(np.ascontiguousarray(barlat).ravel()).to(dev))
     torch.cuda.synchronize()
     out = dict(row_ptr=row_ptr.cpu().numpy(), col_idx=col_idx.cpu().numpy(),
                elem_slot=None if slots is None else slots.cpu().numpy(), residual=res.cpu().numpy(), csr_vals=vals.cpu().numpy(),
@@ -30,13 +31,13 @@ def run_gpu(cfg, fbar=0, want_elem_slot=False, mat=None, assembly_mode=None):
     return out
 
 
-def run_oracle(cfg, fbar=0, with_slots=False, mat=None):
+def run_oracle(cfg, fbar=0, with_slots=False, mat=None, barlat=None):
     import oracle
     ne = cfg["conn"].shape[0]
     if mat is None:
         mat = oracle.mat_from_desc(cfg["matdesc"], ne)
     row_ptr, col_idx, slots = oracle.pattern(cfg["coords"].shape[0], cfg["conn"], with_slots=with_slots)
-    out = oracle.assemble(cfg["coords"], cfg["conn"], cfg["u"], cfg["hist_in"], mat, row_ptr, col_idx, fbar=fbar)
+    out = oracle.assemble(cfg["coords"], cfg["conn"], cfg["u"], cfg["hist_in"], mat, row_ptr, col_idx, fbar=fbar, bar=barlat)
     out.update(row_ptr=row_ptr, col_idx=col_idx, elem_slot=slots)
     return out
 
