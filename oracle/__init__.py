@@ -263,11 +263,13 @@ def assemble(coords, conn, u, hist_in, mat, row_ptr, col_idx, fbar=0, bar=None):
                 stats=dict(n_plastic=int(st[0]), n_nonconverged=int(st[1]), n_detF_nonpos=int(st[2]), max_local_iters=int(st[3])))
 
 
-def assemble_rows(coords, conn, u, hist_in, mat, row_ptr, col_idx, nodes, node_elems, fbar=0):
+def assemble_rows(coords, conn, u, hist_in, mat, row_ptr, col_idx, nodes, node_elems, fbar=0, bar=None):
     """Sampled check at full size: rows 3n..3n+2 of K and R for each node n in `nodes`, summing the incident
     elements (node_elems[n], ascending) one by one.  Returns {node: (res[3], rows list of 3 arrays)} and the
     hist_out of every touched element."""
     mat = _f(mat).reshape(-1, NPAR)
+    if bar is not None:
+        bar = _f(bar).reshape(-1, NBAR)
     out, hist = {}, {}
     cache = {}
     for n in nodes:
@@ -276,7 +278,8 @@ def assemble_rows(coords, conn, u, hist_in, mat, row_ptr, col_idx, nodes, node_e
         for e in sorted(node_elems[n]):
             if e not in cache:
                 c = conn[e].astype(np.int64)
-                cache[e] = element(coords[c], u[c], hist_in[e], mat[0 if mat.shape[0] == 1 else e], fbar)
+                cache[e] = element(coords[c], u[c], hist_in[e], mat[0 if mat.shape[0] == 1 else e], fbar,
+                                   bar=None if bar is None else bar[0 if bar.shape[0] == 1 else e])
             Re, Ke, ho, _ = cache[e]
             hist[e] = ho
             I = int(np.where(conn[e] == n)[0][0])

@@ -15,7 +15,12 @@ import numpy as np
 sys.path.insert(0, os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
 
 
-def run_case(label, cfg, steps, fbar=0, mode=None):
+# PAPER.md:471-477 Table 2 (c' , c'' , m = 8): the paper's Yld2004-18p coefficients
+TABLE2 = [-0.069888, 0.936408, 0.079143, 1.003060, 0.524741, 1.363180, 1.023770, 1.069060, 0.954322,
+          0.981171, 0.476741, 0.575316, 0.866827, 1.145010, -0.079294, 1.051660, 1.147100, 1.404620, 8.0, 0.0]
+
+
+def run_case(label, cfg, steps, fbar=0, mode=None, barlat=None):
     import torch
     import paper_2606_17390_b200 as fem
     dev = torch.device("cuda:0")
@@ -27,23 +32,25 @@ def run_case(label, cfg, steps, fbar=0, mode=None):
     u = torch.from_numpy(cfg["u"].ravel()).to(dev)
     hin = torch.from_numpy(cfg["hist_in"].ravel()).to(dev)
     mat = torch.from_numpy(np.ascontiguousarray(mat_np).ravel()).to(dev)
+    if barlat is not None:   # fem_assemble_barlat: same elastic constants and hardening, r-values ignored
+        barlat = torch.from_numpy(np.tile(np.asarray(barlat, dtype=np.float64), (mat_np.shape[0], 1)).ravel()).to(dev)
     res = torch.empty(3 * nn, dtype=torch.float64, device=dev)
     vals = torch.empty(ctx.nnz, dtype=torch.float64, device=dev)
     hout = torch.empty(56 * ne, dtype=torch.float64, device=dev)
     for _ in range(3):
-        ctx.assemble(u, hin, mat, res, vals, hout)
-    _, _, _, st = ctx.assemble(u, hin, mat, res, vals, hout, want_stats=True)
+        ctx.assemble(u, hin, mat, res, vals, hout, barlat=barlat)
+    _, _, _, st = ctx.assemble(u, hin, mat, res, vals, hout, want_stats=True, barlat=barlat)
     torch.cuda.synchronize()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
     for _ in range(steps):
-        ctx.assemble(u, hin, mat, res, vals, hout)
+        ctx.assemble(u, hin, mat, res, vals, hout, barlat=barlat)
     e1.record()
     torch.cuda.synchronize()
     ms = e0.elapsed_time(e1) / steps
     k = dict(element=0.0, gather=0.0)
     for _ in range(steps):
-        ctx.assemble(u, hin, mat, res, vals, hout)
+        ctx.assemble(u, hin, mat, res, vals, hout, barlat=barlat)
         km = ctx.last_kernel_ms()
         for key in k:
             k[key] += km[key] / steps
@@ -75,6 +82,14 @@ def main():
         run_case("config 3 (100^3)", synth.make_config(3), args.steps)
     if "3fbar" in only:
         run_case("config 3, fbar=1", synth.make_config(3), args.steps, fbar=1)
+    if "3b" in only:
+        run_case("config 3, Yld2004-18p (Table 2, m=8)", synth.make_config(3), args.steps, barlat=TABLE2)
+    if "3bfbar" in only:
+        run_case("config 3, Yld2004-18p, fbar=1", synth.make_config(3), args.steps, fbar=1, barlat=TABLE2)
+    if "5sb" in only:
+        for lv in range(4):
+            run_case("config 5 strain level %d (64^3), Yld2004-18p" % lv, synth.make_config(5, level=lv, sweep="strain"), args.steps,
+                     barlat=TABLE2)
     if "4" in only:
         run_case("config 4 (100^3 void mask, shuffled, per-element material)", synth.make_config(4), args.steps)
     if "e4" in only:

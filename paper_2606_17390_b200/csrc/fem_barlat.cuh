@@ -58,6 +58,7 @@ __device__ __forceinline__ void bar_apply_t(const double *__restrict__ L, const 
     for (int i = 0; i < 3; i++) y[3 + i] += L[9 + i] * g[3 + i] * SQRT2;
 }
 // X^2 of a symmetric 3x3 in tensor components, and the Cayley-Hamilton data: c[n] = (alpha,beta,gamma) of X^n, t[n] = tr X^n
+template <int M>
 __device__ __forceinline__ void bar_powers(const double a[6], int m, double a2[6], double (*c)[3], double *t) {
     a2[0] = a[0] * a[0] + a[3] * a[3] + a[5] * a[5];
     a2[1] = a[3] * a[3] + a[1] * a[1] + a[4] * a[4];
@@ -70,11 +71,13 @@ __device__ __forceinline__ void bar_powers(const double a[6], int m, double a2[6
     c[0][0] = 1.0; c[0][1] = 0.0; c[0][2] = 0.0;
     c[1][0] = 0.0; c[1][1] = 1.0; c[1][2] = 0.0;
     c[2][0] = 0.0; c[2][1] = 0.0; c[2][2] = 1.0;
-    for (int n = 2; n < m; n++) {   // X^(n+1) = X X^n with X^3 = I1 X^2 - I2 X + I3 I
+#pragma unroll
+    for (int n = 2; n < (M ? M : m); n++) {   // X^(n+1) = X X^n with X^3 = I1 X^2 - I2 X + I3 I
         const double al = c[n][0], be = c[n][1], ga = c[n][2];
         c[n + 1][0] = ga * I3; c[n + 1][1] = fma(-ga, I2, al); c[n + 1][2] = fma(ga, I1, be);
     }
-    for (int n = 0; n <= m; n++) t[n] = 3.0 * c[n][0] + c[n][1] * I1 + c[n][2] * tr2;
+#pragma unroll
+    for (int n = 0; n <= (M ? M : m); n++) t[n] = 3.0 * c[n][0] + c[n][1] * I1 + c[n][2] * tr2;
 }
 // H (6x6 Mandel, full) += fully symmetrised "box" product 1/4 (X_ik Y_jl + X_il Y_jk + Y_ik X_jl + Y_il X_jk)
 __device__ __forceinline__ void bar_box_acc(const double X[6], const double Y[6], double H[6][6]) {
@@ -117,17 +120,21 @@ __device__ __forceinline__ void bar_congr_acc(const double *__restrict__ L, cons
 }
 
 // phi (Eq.(12) :133), N = dphi/dT and (want_H) H = d2phi/dT2 (upper triangle) at the Mandel stress T, material frame.
-__device__ __noinline__ void bar_eval(const double *__restrict__ bd, const double T[6], bool want_H, double &phi_out, double N[6],
-                                      double H[6][6]) {
-    const int m = (int)bd[24];
+// M > 0: exponent known at compile time (every loop unrolls, the Cayley-Hamilton tables live in registers and the
+// binomial weights are immediates); M = 0: any even exponent up to BAR_MMAX with rolled loops and tables in local memory.
+template <int M>
+__device__ __noinline__ void bar_eval_t(const double *__restrict__ bd, const double T[6], bool want_H, double &phi_out, double N[6],
+                                        double H[6][6]) {
+    const int m = M ? M : (int)bd[24];
     const double *LA = bd, *LB = bd + 12;
     double a[6], b[6], a2[6], b2[6];
     double cA[BAR_MMAX + 1][3], cB[BAR_MMAX + 1][3], tA[BAR_MMAX + 1], tB[BAR_MMAX + 1];
     bar_apply(LA, T, a); bar_apply(LB, T, b);
-    bar_powers(a, m, a2, cA, tA); bar_powers(b, m, b2, cB, tB);
+    bar_powers<M>(a, m, a2, cA, tA); bar_powers<M>(b, m, b2, cB, tB);
     double Phi = 0.0, gA[3] = {0, 0, 0}, gB[3] = {0, 0, 0};
     {
         double sb = 1.0;   // (-1)^k binom(m,k)
+#pragma unroll
         for (int k = 0; k <= m; k++) {
             Phi = fma(sb * tA[m - k], tB[k], Phi);
             if (k < m) { const double w = sb * (m - k) * tB[k];
@@ -162,24 +169,27 @@ __device__ __noinline__ void bar_eval(const double *__restrict__ bd, const doubl
         for (int q = 0; q < 3; q++) { WA[p][q] = 0.0; WB[p][q] = 0.0; V[p][q] = 0.0; }
     {
         double sb = 1.0;
+#pragma unroll
         for (int k = 0; k <= m; k++) {
             if (k <= m - 2) {   // d/dA of (m-k) tB[k] A^n, n = m-k-1 >= 1: sum_{r=0}^{n-1} A^r (.) A^(n-1-r)
                 const double w = sb * (m - k) * tB[k];
                 const int j = m - k - 2;
+#pragma unroll
                 for (int r = 0; r <= j; r++)
 #pragma unroll
                     for (int p = 0; p < 3; p++)
 #pragma unroll
-                        for (int q = 0; q < 3; q++) WA[p][q] = fma(w * cA[r][p], cA[j - r][q], WA[p][q]);
+                        for (int q = p; q < 3; q++) WA[p][q] = fma(w * cA[r][p], cA[j - r][q], WA[p][q]);
             }
             if (k >= 2) {
                 const double w = sb * k * tA[m - k];
                 const int j = k - 2;
+#pragma unroll
                 for (int r = 0; r <= j; r++)
 #pragma unroll
                     for (int p = 0; p < 3; p++)
 #pragma unroll
-                        for (int q = 0; q < 3; q++) WB[p][q] = fma(w * cB[r][p], cB[j - r][q], WB[p][q]);
+                        for (int q = p; q < 3; q++) WB[p][q] = fma(w * cB[r][p], cB[j - r][q], WB[p][q]);
             }
             if (k >= 1 && k <= m - 1) {
                 const double w = sb * (m - k) * k;
@@ -191,6 +201,8 @@ __device__ __noinline__ void bar_eval(const double *__restrict__ bd, const doubl
             sb = -sb * (double)(m - k) / (double)(k + 1);
         }
     }
+    WA[1][0] = WA[0][1]; WA[2][0] = WA[0][2]; WA[2][1] = WA[1][2];   // sum_r c[r][p] c[j-r][q] is symmetric in (p,q)
+    WB[1][0] = WB[0][1]; WB[2][0] = WB[0][2]; WB[2][1] = WB[1][2];
     const double id6[6] = {1.0, 1.0, 1.0, 0.0, 0.0, 0.0};
     double d2[6][6];
 #pragma unroll
@@ -199,6 +211,7 @@ __device__ __noinline__ void bar_eval(const double *__restrict__ bd, const doubl
         for (int B = 0; B < 6; B++) d2[A][B] = 0.0;
     {
         double HX[6][6], Y[6];
+#pragma unroll
         for (int side = 0; side < 2; side++) {
             const double (*W)[3] = side ? WB : WA;
             const double *x = side ? b : a, *x2 = side ? b2 : a2;
@@ -238,6 +251,14 @@ __device__ __noinline__ void bar_eval(const double *__restrict__ bd, const doubl
     for (int A = 0; A < 6; A++)
 #pragma unroll
         for (int B = A; B < 6; B++) H[A][B] = fma(cf, d2[A][B], -cn * N[A] * N[B]);
+}
+
+__device__ __forceinline__ void bar_eval(const double *__restrict__ bd, const double T[6], bool want_H, double &phi_out, double N[6],
+                                         double H[6][6]) {
+    const int m = (int)bd[24];
+    if (m == 8) bar_eval_t<8>(bd, T, want_H, phi_out, N, H);        // aluminium alloys, the paper's Table 2
+    else if (m == 6) bar_eval_t<6>(bd, T, want_H, phi_out, N, H);   // steels
+    else bar_eval_t<0>(bd, T, want_H, phi_out, N, H);
 }
 
 // In-place Cholesky M = L L^T of a symmetric positive definite 6x6 (lower triangle of M on entry, L on exit).

@@ -40,7 +40,7 @@ def test_full_pattern_closed_form(full3):
     assert (d[mask] > 0).all()
 
 
-def _compare_sampled_rows(full, n_samples=48):
+def _compare_sampled_rows(full, n_samples=48, mat=None, bar=None):
     import oracle
     cfg = full["cfg"]
     conn = cfg["conn"]
@@ -53,8 +53,10 @@ def _compare_sampled_rows(full, n_samples=48):
         for a in range(8):
             if mask[e, a]:
                 node_elems[int(conn[e, a])].append(int(e))
-    mat = oracle.mat_from_desc(cfg["matdesc"], ne)
-    rows, hist = oracle.assemble_rows(cfg["coords"], conn, cfg["u"], cfg["hist_in"], mat, rp, ci, [int(n) for n in nodes], node_elems)
+    if mat is None:
+        mat = oracle.mat_from_desc(cfg["matdesc"], ne)
+    rows, hist = oracle.assemble_rows(cfg["coords"], conn, cfg["u"], cfg["hist_in"], mat, rp, ci, [int(n) for n in nodes], node_elems,
+                                      bar=bar)
     vals = full["vals"].cpu().numpy(); res = full["res"].cpu().numpy()
     hout = full["hout"].cpu().numpy().reshape(ne, 8, 7)
     g_rows, o_rows, g_res, o_res = [], [], [], []
@@ -71,6 +73,22 @@ def _compare_sampled_rows(full, n_samples=48):
 
 def test_full_sampled_rows_against_oracle(full3):
     _compare_sampled_rows(full3)
+
+
+def test_full_barlat_sampled_rows_against_oracle(full3):
+    """fem_assemble_barlat at full config-3 size, Table 2 coefficients, m = 8."""
+    import torch
+    cfg, ctx = full3["cfg"], full3["ctx"]
+    dev = full3["vals"].device
+    mat = np.array([[70000.0, 0.33, 1, 1, 1, 1, 1, 1, 1.0, 500.0, 0.01, 0.2, 1.0, 0.0, 0.0, 0.0]])
+    bar = np.array([[-0.069888, 0.936408, 0.079143, 1.003060, 0.524741, 1.363180, 1.023770, 1.069060, 0.954322,
+                     0.981171, 0.476741, 0.575316, 0.866827, 1.145010, -0.079294, 1.051660, 1.147100, 1.404620, 8.0, 0.0]])
+    res, vals, hout, stats = ctx.assemble(torch.from_numpy(cfg["u"].ravel()).to(dev), torch.from_numpy(cfg["hist_in"].ravel()).to(dev),
+                                          torch.from_numpy(mat.ravel()).to(dev), want_stats=True, barlat=torch.from_numpy(bar.ravel()).to(dev))
+    torch.cuda.synchronize()
+    assert stats["n_nonconverged"] == 0 and stats["n_nonfinite"] == 0 and stats["n_plastic"] > 4_000_000
+    _compare_sampled_rows(dict(cfg=cfg, row_ptr=full3["row_ptr"], col_idx=full3["col_idx"], res=res, vals=vals, hout=hout),
+                          n_samples=32, mat=mat, bar=bar)
 
 
 def test_largest_paper_mesh_sampled_rows_against_oracle():
