@@ -16,6 +16,9 @@
 
 #define FEM_BARD 32   // derived Barlat record: [0..8] N' = C'n.Pn (row-major), [9..11] c'44,c'55,c'66, [12..23] the same for C'', [24] m
 #define BAR_MMAX 16
+#ifndef BAR_START
+#define BAR_START 1
+#endif
 
 __global__ void k_bar_prep(long long n_mat, const double *__restrict__ bar, double *__restrict__ bd) {
     long long r = blockIdx.x * (long long)blockDim.x + threadIdx.x;
@@ -328,6 +331,32 @@ __device__ __noinline__ void bar_return_map(const double *__restrict__ bd, doubl
     const double is0 = 1.0 / s0;
     const double tolG = 1e-13 * fmax(1.0, sqrt(tn2) * is0);
     double dg = 0.0, sy = s0, dsy = ds0, prev = INFINITY;
+#if BAR_START
+    // Starting point (the root is unique, so any start reaches the state Alg. C2 reaches from T^tr): the trial deviator scaled
+    // back onto the yield surface, T0 = p 1 + c s^tr, with dgam from the N-component of Eq.(19): phi^tr - 2mu dgam N.N -
+    // sigma_y(alpha_n + dgam) = 0 (exact radial return for von Mises).  phi is homogeneous of degree one, so phi, N and H at
+    // T0 follow from the trial evaluation without another one: phi0 = c phi^tr, N0 = N, H0 = H / c.
+    {
+        double nn = 0.0;
+#pragma unroll
+        for (int i = 0; i < 6; i++) nn = fma(N[i], N[i], nn);
+        const double a = mu2 * nn;
+        for (int it = 0; it < 6; it++) {   // convex, decreasing: Newton from dgam = 0 approaches the root from the left
+            const double g = phi - a * dg - sy, d = g / (a + dsy);
+            dg += d;
+            flow_stress(law, hh0, hh1, hh2, alphan + dg, sy, dsy);
+            if (d <= 1e-3 * dg) break;
+        }
+        const double c = sy / phi, ic = phi / sy;
+#pragma unroll
+        for (int i = 0; i < 6; i++) T[i] = (i < 3) ? fma(c, Ttr[i] - pres, pres) : c * Ttr[i];
+        phi = sy;
+#pragma unroll
+        for (int A = 0; A < 6; A++)
+#pragma unroll
+            for (int B = A; B < 6; B++) H[A][B] *= ic;
+    }
+#endif
     double GT[6], fv, psi0;
     // merit of Eq.(B2) :846 with the rows of G scaled by sigma_y(alpha_n) (T rows and f row are stresses)
 #define BAR_RESID(Tc, dgc, Nc, phic, syc, GTo, fo, psio)                                              \
@@ -368,13 +397,15 @@ __device__ __noinline__ void bar_return_map(const double *__restrict__ bd, doubl
         // line search, App. B Eq.(B1)-(B7) :838-867, beta = 1e-4, eta = 0.1 (:871)
         double zeta = 1.0, Tt[6], Nt[6], GTt[6], phit, syt, dsyt, ft, psit, dgt;
         double zj = 1.0;
+        bool accepted0 = true;
         for (int j = 0;; j++) {
             dgt = fma(zeta, ddg, dg);
 #pragma unroll
             for (int i = 0; i < 6; i++) Tt[i] = fma(zeta, dT[i], T[i]);
-            bar_eval(bd, Tt, false, phit, Nt, H);
+            bar_eval(bd, Tt, j == 0, phit, Nt, H);   // the full step is accepted almost always: take H along with it
             flow_stress(law, hh0, hh1, hh2, alphan + dgt, syt, dsyt);
             BAR_RESID(Tt, dgt, Nt, phit, syt, GTt, ft, psit);
+            accepted0 = (j == 0);
             if (psit < (1.0 - 2.0e-4 * zeta) * psi0 || j >= 12) break;          // Eq.(B3)
             const double zn = psi0 / (psi0 + psit);                                // Eq.(B5)/(B6)
             zeta = (j == 0) ? zn : fmax(0.1 * zj, zn);                             // Eq.(B7)
@@ -383,7 +414,11 @@ __device__ __noinline__ void bar_return_map(const double *__restrict__ bd, doubl
         dg = dgt;
 #pragma unroll
         for (int i = 0; i < 6; i++) T[i] = Tt[i];
-        bar_eval(bd, T, true, phi, N, H);
+        if (accepted0) {
+            phi = phit;
+#pragma unroll
+            for (int i = 0; i < 6; i++) N[i] = Nt[i];
+        } else bar_eval(bd, T, true, phi, N, H);
         sy = syt; dsy = dsyt;
         BAR_RESID(T, dg, N, phi, sy, GT, fv, psi0);
     }
