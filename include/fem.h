@@ -237,6 +237,26 @@ int fem_newton_solve(fem_ctx *c, double *u, const double *hist_in, const double 
                      const int *bc_dofs, const double *bc_vals, double *hist_out, const fem_newton_options *opt,
                      fem_newton_report *rep, void *cuda_stream);
 
+/* fem_assemble_vjp — SURVEY.md section 8(f) NEXT-3: vector-Jacobian products of one fem_assemble pass, i.e. of the map
+ * (u, hist_in, mat) -> (residual, hist_out), for the discrete adjoint of Alg. 1 (Eq.(49)-(51) :355-366).
+ * With lam an adjoint vector on the residual and mu a cotangent on hist_out (either may be NULL = zero):
+ *   g_u       dev [n_rows]       = (dR/du)^T lam + (dhist_out/du)^T mu.  With lam = NULL this is the history leg of
+ *                                  (dR^{n+1}/du^n)^T lam^{n+1} on the right-hand side of Eq.(51); with mu = NULL it is K^T lam
+ *                                  (K = dR/du is symmetric for the standard element, so fem_pcg solves the adjoint system).
+ *   g_hist_in dev [n_elems*8*7]  = (dR/dhist_in)^T lam + (dhist_out/dhist_in)^T mu, in the stored components of hist
+ *                                  (it is the cotangent mu of the previous load step: the internal variables the paper
+ *                                  calls "implicitly accounted for", carried backwards; reading G17)
+ *   g_mat     dev [n_mat*16]     = (dR/dmat)^T lam + (dhist_out/dmat)^T mu (Eq.(49) :355) for E, nu, r11..r13, h0, h1, h2
+ *                                  (record positions 0-7 and 9-11); the law switch and the quaternion get 0.  n_mat = 1: the
+ *                                  sum over all elements; n_mat = n_elems: one record per element.
+ * Any of the three outputs may be NULL (not computed).  u, hist_in, mat, n_mat as in fem_assemble; the state is
+ * re-evaluated inside the call (nothing is kept from fem_assemble), the return map is differentiated implicitly at its
+ * root (App. D Eq.(D4)-(D7) :1002-1019, transposed).  Hill-48 and the standard element only: FEM_ERR_ARG for fbar = 1 or
+ * assembly_mode 1.  Sums run in a fixed order, no atomics: equal inputs give bit-identical outputs.  Uses the library's
+ * R^e scratch: do not run concurrently with fem_assemble on another stream.  Asynchronous on `cuda_stream`. */
+int fem_assemble_vjp(fem_ctx *c, const double *u, const double *hist_in, const double *mat, long long n_mat,
+                     const double *lam, const double *mu, double *g_u, double *g_hist_in, double *g_mat, void *cuda_stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -11,7 +11,7 @@ NBARLAT = 20
 ABI_SYMBOLS = ["fem_default_options", "fem_setup", "fem_build_csr_pattern", "fem_assemble", "fem_assemble_barlat", "fem_assemble_host",
                "fem_last_kernel_ms", "fem_launches_per_assemble", "fem_probe_fp64_peak", "fem_destroy", "fem_strerror",
                "fem_last_cuda_error", "fem_hill_from_lankford", "fem_spmv", "fem_apply_dirichlet", "fem_bicgstab", "fem_pcg", "fem_lincomb",
-               "fem_default_newton_options", "fem_newton_solve"]
+               "fem_default_newton_options", "fem_newton_solve", "fem_assemble_vjp"]
 
 
 class FemOptions(C.Structure):
@@ -100,6 +100,7 @@ def lib():
         L.fem_default_newton_options.restype = None
         L.fem_newton_solve.argtypes = [vp, vp, vp, vp, ll, ll, vp, vp, vp, C.POINTER(FemNewtonOptions),
                                        C.POINTER(FemNewtonReport), vp]
+        L.fem_assemble_vjp.argtypes = [vp, vp, vp, vp, ll, vp, vp, vp, vp, vp, vp]
         _lib = L
     return _lib
 
@@ -324,6 +325,22 @@ class FemContext:
         if rc not in (0, -11):
             _check(rc, "fem_newton_solve")
         return u, hist_out, rep.as_dict()
+
+    def assemble_vjp(self, u, hist_in, mat, lam=None, mu=None, want_u=True, want_hist=True, want_mat=True):
+        """fem_assemble_vjp: (g_u, g_hist_in, g_mat) for the cotangents lam on the residual and mu on hist_out (None = zero);
+        outputs not wanted are None."""
+        torch = _torch()
+        f64 = torch.float64
+        n_mat = mat.numel() // NPAR
+        g_u = torch.empty(self.n_rows, dtype=f64, device=self.device) if want_u else None
+        g_h = torch.empty(self.n_elems * 56, dtype=f64, device=self.device) if want_hist else None
+        g_m = torch.empty(n_mat * NPAR, dtype=f64, device=self.device) if want_mat else None
+        opt = lambda t, n, name: None if t is None else _ptr(t, f64, n, name)
+        _check(lib().fem_assemble_vjp(self._h, _ptr(u, f64, self.n_rows, "u"), _ptr(hist_in, f64, 56 * self.n_elems, "hist_in"),
+                                      _ptr(mat, f64, None, "mat"), n_mat, opt(lam, self.n_rows, "lam"), opt(mu, 56 * self.n_elems, "mu"),
+                                      opt(g_u, self.n_rows, "g_u"), opt(g_h, 56 * self.n_elems, "g_hist_in"),
+                                      opt(g_m, n_mat * NPAR, "g_mat"), _stream_ptr()), "fem_assemble_vjp")
+        return g_u, g_h, (g_m.view(n_mat, NPAR) if g_m is not None else None)
 
     def last_kernel_ms(self):
         ms = (C.c_double * 3)()

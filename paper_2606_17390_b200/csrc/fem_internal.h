@@ -59,6 +59,9 @@ struct fem_ctx {
     double *d_nw = nullptr;        // [4*n_rows] Newton workspace: residual, rhs, dd, u at entry
     double *d_nw_vals = nullptr;   // [nnz] Newton workspace: stiffness values
     long long n_part = 0;
+    // NEXT-3 (fem_sens.cu): per-CTA partial sums of the material gradient (uniform material)
+    double *d_sens_part = nullptr;
+    long long n_sens_part = 0;
     // host-buffer path
     double *d_u = nullptr, *d_hin = nullptr, *d_hout = nullptr, *d_mat = nullptr, *d_res = nullptr, *d_vals = nullptr;
     long long n_mat_host_cap = 0;
