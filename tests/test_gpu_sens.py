@@ -234,3 +234,80 @@ def test_vjp_full_size_properties_and_samples():
     gu = c_u.cpu().numpy().reshape(nn, 3)[nodes]
     assert rel_l2(gu, o2["g_u_full"][nodes]) <= TOL
     ctx.close()
+
+
+def test_adjoint_gradient_of_load_path_matches_oracle():
+    """Alg. 1 end to end on the GPU: two load increments with fem_newton_solve, then backwards per step
+    Eq.(51) K^T lam = -(dJ/du)^T - (dh/du)^T mu by fem_pcg on the row-eliminated tangent, Eq.(49) by fem_assemble_vjp with the
+    history cotangent carried from step to step (reading G17), J = sum_n |u^n - u_gt^n|^2.  Expected values: the same loop
+    written with oracle/ functions only (oracle.newton + oracle.sens, itself pinned to central differences of J)."""
+    import torch
+    import oracle
+    import oracle.sens as osn
+    import oracle.newton as onw
+    from synth import mesh
+    p = _small_problem(seed=4, n=(2, 2, 2), hist=False)
+    coords, conn, mat = p["coords"], p["conn"], p["mat"]
+    nn, ne = coords.shape[0], conn.shape[0]
+    X0 = mesh.structured_hex_mesh(2, 2, 2)[0]
+    x0, x1 = np.isclose(X0[:, 0], 0.0), np.isclose(X0[:, 0], 1.0)
+    bn = np.flatnonzero(x0 | x1)
+    bc = (3 * bn[:, None] + np.arange(3)).ravel()
+    free = np.setdiff1d(np.arange(3 * nn), bc)
+
+    def target(s):
+        t = np.zeros((nn, 3)); t[x1, 0] = 0.012 * s; t[x1, 1] = 0.006 * s
+        return t.ravel()[bc]
+    targets = [target(0.5), target(1.0)]
+    rng = np.random.default_rng(0)
+    ugt = [0.01 * rng.normal(size=(nn, 3)) for _ in targets]
+    # ---- oracle side
+    rp, ci, _ = oracle.pattern(nn, conn, with_slots=False)
+    uo, ho, states = np.zeros_like(coords), np.zeros((ne, 8, 7)), []
+    for t in targets:
+        r = onw.newton_solve(coords, conn, uo, ho, mat, rp, ci, bc, t, rtol=1e-13, atol=1e-9)
+        assert r["converged"]
+        states.append((r["u"].copy(), ho.copy()))
+        uo, ho = r["u"], r["hist_out"]
+    grad_o, mu_o = np.zeros(16), None
+    for (u, h), g in zip(reversed(states), reversed(ugt)):
+        out = oracle.assemble(coords, conn, u, h, mat, rp, ci)
+        rhs = -2.0 * (u - g).ravel()
+        if mu_o is not None:
+            rhs -= osn.assemble_vjp(coords, conn, u, h, mat, None, mu_o)["g_u"].ravel()
+        K = onw.csr(rp, ci, out["csr_vals"]).toarray()
+        lam = np.zeros(3 * nn)
+        lam[free] = np.linalg.solve(K[np.ix_(free, free)].T, rhs[free])
+        v = osn.assemble_vjp(coords, conn, u, h, mat, lam, mu_o)
+        grad_o += v["g_mat"][0]
+        mu_o = v["g_hist_in"]
+    # ---- GPU side
+    ctx = _ctx(coords, conn)
+    dev = ctx.device
+    t64 = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64).ravel()).to(dev)
+    mat_d, bc_d = t64(mat), torch.from_numpy(bc.astype(np.int32)).to(dev)
+    u_d = torch.zeros(3 * nn, dtype=torch.float64, device=dev)
+    h_d = torch.zeros(56 * ne, dtype=torch.float64, device=dev)
+    gstates = []
+    for t in targets:
+        u_d, h_new, rep = ctx.newton_solve(u_d, h_d, mat_d, bc_d, t64(t), rtol=1e-13, atol=1e-9, lin_rtol=1e-13)
+        assert rep["converged"]
+        gstates.append((u_d.clone(), h_d))
+        h_d = h_new
+    grad_g, mu_d = torch.zeros(16, dtype=torch.float64, device=dev), None
+    for (u, h), g in zip(reversed(gstates), reversed(ugt)):
+        _, vals, _, _ = ctx.assemble(u, h, mat_d)
+        rhs = -2.0 * (u - t64(g))
+        if mu_d is not None:
+            rhs = rhs - ctx.assemble_vjp(u, h, mat_d, None, mu_d, want_hist=False, want_mat=False)[0]
+        ctx.apply_dirichlet(bc_d, vals, rhs)                         # identity rows, lam = 0 on the constrained DOFs
+        lam, _, _, ok = ctx.pcg(vals, rhs, rtol=1e-13, max_iter=5000)
+        assert ok
+        _, mu_new, g_m = ctx.assemble_vjp(u, h, mat_d, lam, mu_d, want_u=False)
+        grad_g += g_m[0]
+        mu_d = mu_new
+    gg = grad_g.cpu().numpy()
+    idx = list(osn.THETA_IDX)
+    assert np.max(np.abs(gg[idx] - grad_o[idx]) / np.maximum(np.abs(grad_o[idx]), 1e-6 * np.abs(grad_o[idx]).max())) <= 1e-6
+    assert rel_l2(mu_d.cpu().numpy(), mu_o) <= 1e-6
+    ctx.close()
