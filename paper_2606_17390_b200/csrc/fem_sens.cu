@@ -21,12 +21,16 @@
 // Sums are taken in a fixed order (per node: ascending element id; uniform material: fixed two-level tree), no atomics.
 // Nothing here is shared with oracle/.
 #include "fem_internal.h"
+#include "fem_device.cuh"
 #include <math.h>
 
 #define SW23 0.81649658092772603273   // W = sqrt(2/3)
 #define SEL 16                        // elements per CTA
 #define STHREADS (8 * SEL)
 #define NTHETA 11
+#ifndef SENS_CTAS
+#define SENS_CTAS 3                   // CTAs per SM the register allocation aims at
+#endif
 
 __device__ constexpr int S_THETA_IDX[NTHETA] = {0, 1, 2, 3, 4, 5, 6, 7, 9, 10, 11};
 __device__ constexpr double S_XI[8][3] = {{-1, -1, -1}, {1, -1, -1}, {1, 1, -1}, {-1, 1, -1},
@@ -40,33 +44,30 @@ __device__ __forceinline__ void to33(const double a[6], double A[3][3]) {
     A[0][0] = a[0]; A[1][1] = a[1]; A[2][2] = a[2];
     A[0][1] = A[1][0] = a[3]; A[1][2] = A[2][1] = a[4]; A[0][2] = A[2][0] = a[5];
 }
-__device__ __forceinline__ void to6(const double A[3][3], double a[6]) {
-    a[0] = A[0][0]; a[1] = A[1][1]; a[2] = A[2][2];
-    a[3] = 0.5 * (A[0][1] + A[1][0]); a[4] = 0.5 * (A[1][2] + A[2][1]); a[5] = 0.5 * (A[0][2] + A[2][0]);
-}
-// B = Q^T A Q (tr = 0) or Q A Q^T (tr = 1) for symmetric A given as 6 components
-__device__ __forceinline__ void rot6(const double Q[3][3], const double a[6], double b[6], int tr) {
-    double A[3][3], T[3][3], B[3][3];
+// B = Q^T A Q (TR = 0) or Q A Q^T (TR = 1) for symmetric A, both as 6 components
+template <int TR>
+__device__ __forceinline__ void rot6(const double Q[3][3], const double a[6], double b[6]) {
+    double A[3][3], T[3][3];
     to33(a, A);
+#pragma unroll
     for (int i = 0; i < 3; i++)
+#pragma unroll
         for (int j = 0; j < 3; j++) {
-            double s = 0.0;
-            for (int k = 0; k < 3; k++) s += A[i][k] * (tr ? Q[j][k] : Q[k][j]);
-            T[i][j] = s;
+            const double q0 = TR ? Q[j][0] : Q[0][j], q1 = TR ? Q[j][1] : Q[1][j], q2 = TR ? Q[j][2] : Q[2][j];
+            T[i][j] = A[i][0] * q0 + A[i][1] * q1 + A[i][2] * q2;
         }
-    for (int i = 0; i < 3; i++)
-        for (int j = 0; j < 3; j++) {
-            double s = 0.0;
-            for (int k = 0; k < 3; k++) s += (tr ? Q[i][k] : Q[k][i]) * T[k][j];
-            B[i][j] = s;
-        }
-    to6(B, b);
+    constexpr int PI[6] = {0, 1, 2, 0, 1, 0}, PJ[6] = {0, 1, 2, 1, 2, 2};
+#pragma unroll
+    for (int k = 0; k < 6; k++) {
+        const int i = PI[k], j = PJ[k];
+        const double q0 = TR ? Q[i][0] : Q[0][i], q1 = TR ? Q[i][1] : Q[1][i], q2 = TR ? Q[i][2] : Q[2][i];
+        b[k] = q0 * T[0][j] + q1 * T[1][j] + q2 * T[2][j];
+    }
 }
 
 struct SMat {
-    double E, nu, mu2, lam, law, h0, h1, h2;
+    double E, iE, nu, mu2, imu2, lam, law, h0, h1, h2;
     double p[9];        // Hill coefficients p1..p9 of Eq.(A3)-(A5) :784-801 in the local (material) frame
-    double r[6];
 };
 
 // H : a  (Eq.(A2) :779 in tensor components: H1212 = p7/2, so (H:a)_12 = p7 a_12)
@@ -79,25 +80,30 @@ __device__ __forceinline__ void applyH(const SMat &m, const double a[6], double 
 // E : a  (Eq.(8) :110, isotropic)
 __device__ __forceinline__ void applyE(const SMat &m, const double a[6], double b[6]) {
     const double tr = m.lam * (a[0] + a[1] + a[2]);
+#pragma unroll
     for (int i = 0; i < 3; i++) b[i] = m.mu2 * a[i] + tr;
+#pragma unroll
     for (int i = 3; i < 6; i++) b[i] = m.mu2 * a[i];
 }
 __device__ __forceinline__ void applyEinv(const SMat &m, const double a[6], double b[6]) {
     const double s = m.nu * (a[0] + a[1] + a[2]);
-    for (int i = 0; i < 3; i++) b[i] = ((1.0 + m.nu) * a[i] - s) / m.E;
-    for (int i = 3; i < 6; i++) b[i] = a[i] / m.mu2;
+#pragma unroll
+    for (int i = 0; i < 3; i++) b[i] = ((1.0 + m.nu) * a[i] - s) * m.iE;
+#pragma unroll
+    for (int i = 3; i < 6; i++) b[i] = a[i] * m.imu2;
 }
 // D = E^-1 + kappa H : normal block 3x3 (symmetric, inverted once per kappa) + three shear scalars
 struct SDinv { double n[6]; double s[3]; };   // inverse normal block as (11,22,33,12,23,13), inverse shear scalars
 __device__ __forceinline__ void makeDinv(const SMat &m, double kap, SDinv &D) {
-    const double ie = 1.0 / m.E, o = -m.nu * ie;
+    const double ie = m.iE, o = -m.nu * ie;
     const double a = ie + kap * m.p[0], b = ie + kap * m.p[1], c = ie + kap * m.p[2];
     const double d = o + kap * m.p[3], e = o + kap * m.p[4], f = o + kap * m.p[5];   // 12, 23, 13
     const double c00 = b * c - e * e, c01 = f * e - d * c, c02 = d * e - f * b;
-    const double idet = 1.0 / (a * c00 + d * c01 + f * c02);
+    const double idet = frcp(a * c00 + d * c01 + f * c02);
     D.n[0] = c00 * idet; D.n[3] = c01 * idet; D.n[5] = c02 * idet;
     D.n[1] = (a * c - f * f) * idet; D.n[4] = (d * f - a * e) * idet; D.n[2] = (a * b - d * d) * idet;
-    for (int k = 0; k < 3; k++) D.s[k] = 1.0 / (1.0 / m.mu2 + kap * m.p[6 + k]);
+#pragma unroll
+    for (int k = 0; k < 3; k++) D.s[k] = frcp(m.imu2 + kap * m.p[6 + k]);
 }
 __device__ __forceinline__ void applyDinv(const SDinv &D, const double a[6], double b[6]) {
     b[0] = D.n[0] * a[0] + D.n[3] * a[1] + D.n[5] * a[2];
@@ -106,16 +112,24 @@ __device__ __forceinline__ void applyDinv(const SDinv &D, const double a[6], dou
     b[3] = D.s[0] * a[3]; b[4] = D.s[1] * a[4]; b[5] = D.s[2] * a[5];
 }
 
-// sigma_flow, d sigma_flow/d alpha and d sigma_flow/d(h0,h1,h2): Voce Eq.(10) :121, Swift (BASELINE configs)
-__device__ __forceinline__ void flow_all(const SMat &m, double alpha, double &sf, double &dsf, double dh[3]) {
+// sigma_flow and d sigma_flow/d alpha: Voce Eq.(10) :121, Swift (BASELINE configs)
+__device__ __forceinline__ void flow2(const SMat &m, double alpha, double &sf, double &dsf) {
     if (m.law == 0.0) {
         const double e = exp(-m.h2 * alpha);
         sf = m.h0 + m.h1 * (1.0 - e); dsf = m.h1 * m.h2 * e;
+    } else {
+        const double b = m.h1 + alpha, pw = exp(m.h2 * log(b));
+        sf = m.h0 * pw; dsf = m.h0 * m.h2 * pw * frcp(b);
+    }
+}
+// d sigma_flow/d(h0,h1,h2)
+__device__ __forceinline__ void flow_dh(const SMat &m, double alpha, double dh[3]) {
+    if (m.law == 0.0) {
+        const double e = exp(-m.h2 * alpha);
         dh[0] = 1.0; dh[1] = 1.0 - e; dh[2] = m.h1 * alpha * e;
     } else {
         const double b = m.h1 + alpha, lb = log(b), pw = exp(m.h2 * lb);
-        sf = m.h0 * pw; dsf = m.h0 * m.h2 * pw / b;
-        dh[0] = pw; dh[1] = m.h0 * m.h2 * pw / b; dh[2] = m.h0 * pw * lb;
+        dh[0] = pw; dh[1] = m.h0 * m.h2 * pw * frcp(b); dh[2] = m.h0 * pw * lb;
     }
 }
 
@@ -128,73 +142,35 @@ __device__ __forceinline__ void hill_bilinear_ds(const double x[6], const double
     B[3] = 2.0 * x[3] * t[3]; B[4] = 2.0 * x[4] * t[4]; B[5] = 2.0 * x[5] * t[5];
 }
 
-// atanh(w)/w
-__device__ __forceinline__ double s_atanhc(double w) {
-    const double w2 = w * w;
-    if (w2 < 0.01) {
-        double s = 1.0 / 19.0;
-        for (int k = 17; k >= 1; k -= 2) s = s * w2 + 1.0 / k;
-        return s;
-    }
-    return 0.5 * log((1.0 + w) / (1.0 - w)) / w;
+// First divided difference of g = 1/2 ln between eigenvalues a, b with ga = g(a), gb = g(b):
+// atanh(w)/w / (a+b), w = (a-b)/(a+b), by its series for |w| < 0.15 (remainder < 1e-19), else (ga - gb)/(a - b)
+__device__ __forceinline__ double g_dd1(double a, double b, double ga, double gb) {
+    const double is = frcp(a + b), w = (a - b) * is, w2 = w * w;
+    double s = 1.0 / 21.0;
+    s = fma(s, w2, 1.0 / 19.0); s = fma(s, w2, 1.0 / 17.0); s = fma(s, w2, 1.0 / 15.0); s = fma(s, w2, 1.0 / 13.0);
+    s = fma(s, w2, 1.0 / 11.0); s = fma(s, w2, 1.0 / 9.0);  s = fma(s, w2, 1.0 / 7.0);  s = fma(s, w2, 1.0 / 5.0);
+    s = fma(s, w2, 1.0 / 3.0);  s = fma(s, w2, 1.0);
+    const double big = (ga - gb) * frcp((w2 < 0.0225) ? 1.0 : a - b);
+    return (w2 < 0.0225) ? s * is : big;
 }
-// first divided difference of ln:  ln[a,b] = 2 atanhc(w) / (a + b), w = (a-b)/(a+b)
-__device__ __forceinline__ double ln_dd1(double a, double b) {
-    const double s = a + b;
-    return 2.0 * s_atanhc((a - b) / s) / s;
-}
-// second divided difference of ln over three (possibly coincident) nodes: series in the complete homogeneous polynomials of
-// the centred nodes when they are close, else the recursion over the widest gap
-__device__ double ln_dd2(double x0, double x1, double x2) {
-    const double m = (x0 + x1 + x2) * (1.0 / 3.0);
-    const double d0 = (x0 - m) / m, d1 = (x1 - m) / m, d2 = (x2 - m) / m;
+// Second divided difference of g = 1/2 ln over the nodes (x0, x1, x2) (coincident nodes allowed).  d02 = g[x0,x1], d12 =
+// g[x1,x2] are the first divided differences on either side of the middle node x1, x0 and x2 the two nodes farthest apart.
+// Nodes within 2e-3 (relative) of each other: series about the mean in the complete homogeneous polynomials h_k of the
+// centred nodes, g[x0,x1,x2] = 1/(2 m^2) sum_{n>=2} (-1)^(n-1)/n h_{n-2}, h_k = -e2 h_{k-2} + e3 h_{k-3} (e1 = 0), through h_5
+// (remainder < 1e-17); farther apart the recursion (g[x0,x1] - g[x1,x2])/(x0 - x2), whose cancellation costs 2 eps m/gap <= 1e-13.
+__device__ __forceinline__ double g_dd2(double x0, double x1, double x2, double g01, double g12) {
+    const double m = (x0 + x1 + x2) * (1.0 / 3.0), im = frcp(m);
+    const double d0 = (x0 - m) * im, d1 = (x1 - m) * im, d2 = (x2 - m) * im;
     const double sp = fmax(fabs(d0), fmax(fabs(d1), fabs(d2)));
-    if (sp < 0.08) {
-        // ln[x0,x1,x2] = 1/m^2 sum_{n>=2} (-1)^(n-1)/n h_{n-2}(d);  h_k = -e2 h_{k-2} + e3 h_{k-3}  (e1 = 0)
-        const double e2 = d0 * d1 + d1 * d2 + d0 * d2, e3 = d0 * d1 * d2;
-        double hm2 = 0.0, hm1 = 0.0, h = 1.0, s = 0.0, sg = -1.0;
-        for (int n = 2; n <= 22; n++) {
-            s += sg * h / n;
-            sg = -sg;
-            const double hn = -e2 * hm1 + e3 * hm2;
-            hm2 = hm1; hm1 = h; h = hn;
-        }
-        return s / (m * m);
-    }
-    // order so that lo <= mid <= hi
-    double lo = fmin(x0, fmin(x1, x2)), hi = fmax(x0, fmax(x1, x2)), mid = x0 + x1 + x2 - lo - hi;
-    const double f_hm = (hi == mid) ? 1.0 / hi : ln_dd1(hi, mid);
-    const double f_ml = (mid == lo) ? 1.0 / lo : ln_dd1(mid, lo);
-    return (f_hm - f_ml) / (hi - lo);
+    const double e2 = d0 * d1 + d1 * d2 + d0 * d2, e3 = d0 * d1 * d2;
+    // h0 = 1, h1 = 0, h2 = -e2, h3 = e3, h4 = e2^2, h5 = -2 e2 e3
+    const double ser = -0.5 + e2 * 0.25 + e3 * 0.2 - e2 * e2 * (1.0 / 6.0) - 2.0 * e2 * e3 * (1.0 / 7.0);
+    const bool close = sp < 2e-3;
+    const double rec = (g01 - g12) * frcp(close ? 1.0 : x0 - x2);
+    return close ? 0.5 * im * im * ser : rec;
 }
 
-// cyclic Jacobi on a symmetric 3x3: A = V diag(lam) V^T, columns of V the eigenvectors
-__device__ __forceinline__ void jacobi3(double A[3][3], double V[3][3], double lam[3]) {
-    for (int i = 0; i < 3; i++)
-        for (int j = 0; j < 3; j++) V[i][j] = (i == j) ? 1.0 : 0.0;
-    for (int sweep = 0; sweep < 6; sweep++) {
-        for (int pq = 0; pq < 3; pq++) {
-            const int p = (pq == 2) ? 1 : 0, q = (pq == 0) ? 1 : 2;
-            const double apq = A[p][q];
-            if (fabs(apq) < 1e-300) continue;
-            const double th = (A[q][q] - A[p][p]) / (2.0 * apq);
-            const double t = copysign(1.0, th) / (fabs(th) + sqrt(th * th + 1.0));
-            const double c = 1.0 / sqrt(t * t + 1.0), s = t * c;
-            const int r = 3 - p - q;
-            const double arp = A[r][p], arq = A[r][q];
-            A[p][p] -= t * apq; A[q][q] += t * apq; A[p][q] = A[q][p] = 0.0;
-            A[r][p] = A[p][r] = c * arp - s * arq;
-            A[r][q] = A[q][r] = s * arp + c * arq;
-            for (int k = 0; k < 3; k++) {
-                const double vp = V[k][p], vq = V[k][q];
-                V[k][p] = c * vp - s * vq; V[k][q] = s * vp + c * vq;
-            }
-        }
-    }
-    lam[0] = A[0][0]; lam[1] = A[1][1]; lam[2] = A[2][2];
-}
-
-__global__ void __launch_bounds__(STHREADS)
+__global__ void __launch_bounds__(STHREADS, SENS_CTAS)
 k_sens_point(long long n_elems, const double *__restrict__ coords, const int *__restrict__ conn, const int *__restrict__ eslot,
              const double *__restrict__ u, const double *__restrict__ hist_in, const double *__restrict__ mat, long long n_mat,
              const double *__restrict__ lamv, const double *__restrict__ muv,
@@ -202,15 +178,17 @@ k_sens_point(long long n_elems, const double *__restrict__ coords, const int *__
              double *__restrict__ g_hist /*may be null*/, double *__restrict__ g_mat /*per element, may be null*/,
              double *__restrict__ part /*[gridDim.x][NTHETA] uniform material, may be null*/) {
     __shared__ double sX[SEL][8][3], sU[SEL][8][3], sL[SEL][8][3];
-    __shared__ double sGu[SEL][8][25];      // [element][point][24 (+1 pad)]
+    __shared__ double sGu[SEL][8][25];      // per thread: G' (24 doubles, odd stride) during the pass, then its ubar contributions
     __shared__ double sTh[STHREADS][NTHETA];
     const int tid = threadIdx.x, el = tid >> 3, q = tid & 7;
     const long long e = (long long)blockIdx.x * SEL + el;
     const bool live = e < n_elems;
     double gth[NTHETA];
+#pragma unroll
     for (int k = 0; k < NTHETA; k++) gth[k] = 0.0;
     if (live) {
         const int nd = conn[e * 8 + q];
+#pragma unroll
         for (int i = 0; i < 3; i++) {
             sX[el][q][i] = coords[3LL * nd + i];
             sU[el][q][i] = u[3LL * nd + i];
@@ -219,207 +197,292 @@ k_sens_point(long long n_elems, const double *__restrict__ coords, const int *__
     }
     __syncthreads();
     if (live) {
+        double *Gs = &sGu[el][q][0];
         // ---- material record
         const double *mp = mat + (n_mat == 1 ? 0 : e) * FEM_NPAR;
         SMat m;
-        m.E = mp[0]; m.nu = mp[1]; m.mu2 = m.E / (1.0 + m.nu); m.lam = m.E * m.nu / ((1.0 + m.nu) * (1.0 - 2.0 * m.nu));
+        m.E = mp[0]; m.nu = mp[1]; m.iE = 1.0 / m.E; m.mu2 = m.E / (1.0 + m.nu); m.imu2 = (1.0 + m.nu) * m.iE;
+        m.lam = m.E * m.nu / ((1.0 + m.nu) * (1.0 - 2.0 * m.nu));
         m.law = mp[8]; m.h0 = mp[9]; m.h1 = mp[10]; m.h2 = mp[11];
-        for (int k = 0; k < 6; k++) m.r[k] = mp[2 + k];
-        m.p[0] = 2.0 / (3.0 * m.r[0] * m.r[0]); m.p[1] = 2.0 / (3.0 * m.r[1] * m.r[1]); m.p[2] = 2.0 / (3.0 * m.r[2] * m.r[2]);
-        m.p[6] = 1.0 / (m.r[3] * m.r[3]); m.p[7] = 1.0 / (m.r[4] * m.r[4]); m.p[8] = 1.0 / (m.r[5] * m.r[5]);
-        m.p[3] = 0.5 * (m.p[2] - m.p[0] - m.p[1]); m.p[4] = 0.5 * (m.p[0] - m.p[1] - m.p[2]); m.p[5] = 0.5 * (m.p[1] - m.p[0] - m.p[2]);
+        {
+            const double s0 = 1.0 / (mp[2] * mp[2]), s1 = 1.0 / (mp[3] * mp[3]), s2 = 1.0 / (mp[4] * mp[4]);
+            m.p[0] = (2.0 / 3.0) * s0; m.p[1] = (2.0 / 3.0) * s1; m.p[2] = (2.0 / 3.0) * s2;
+            m.p[6] = 1.0 / (mp[5] * mp[5]); m.p[7] = 1.0 / (mp[6] * mp[6]); m.p[8] = 1.0 / (mp[7] * mp[7]);
+            m.p[3] = 0.5 * (m.p[2] - m.p[0] - m.p[1]); m.p[4] = 0.5 * (m.p[0] - m.p[1] - m.p[2]); m.p[5] = 0.5 * (m.p[1] - m.p[0] - m.p[2]);
+        }
         double Th[3][3];
         {
-            const double qn = sqrt(mp[12] * mp[12] + mp[13] * mp[13] + mp[14] * mp[14] + mp[15] * mp[15]);
-            const double w = mp[12] / qn, x = mp[13] / qn, y = mp[14] / qn, z = mp[15] / qn;
+            const double qn = 1.0 / sqrt(mp[12] * mp[12] + mp[13] * mp[13] + mp[14] * mp[14] + mp[15] * mp[15]);
+            const double w = mp[12] * qn, x = mp[13] * qn, y = mp[14] * qn, z = mp[15] * qn;
             Th[0][0] = 1 - 2 * (y * y + z * z); Th[0][1] = 2 * (x * y - w * z);     Th[0][2] = 2 * (x * z + w * y);
             Th[1][0] = 2 * (x * y + w * z);     Th[1][1] = 1 - 2 * (x * x + z * z); Th[1][2] = 2 * (y * z - w * x);
             Th[2][0] = 2 * (x * z - w * y);     Th[2][1] = 2 * (y * z + w * x);     Th[2][2] = 1 - 2 * (x * x + y * y);
         }
-        // ---- shape gradients at Gauss point q (Eq.(28) :220), rotated: G'_IJ = G_IK Theta_KJ
+        // ---- shape gradients at Gauss point q (Eq.(28) :220), rotated: G'_IJ = G_IK Theta_KJ, kept in shared memory
         const double gp = 0.57735026918962576451;
-        const double xi[3] = {(q & 1) ? gp : -gp, (q & 2) ? gp : -gp, (q & 4) ? gp : -gp};
-        double dN[8][3], Jr[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}};
+        const double xi0 = (q & 1) ? gp : -gp, xi1 = (q & 2) ? gp : -gp, xi2 = (q & 4) ? gp : -gp;
+        double Jr[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}};
+#pragma unroll
         for (int I = 0; I < 8; I++) {
-            const double a = 1.0 + xi[0] * S_XI[I][0], b = 1.0 + xi[1] * S_XI[I][1], c = 1.0 + xi[2] * S_XI[I][2];
-            dN[I][0] = 0.125 * S_XI[I][0] * b * c; dN[I][1] = 0.125 * a * S_XI[I][1] * c; dN[I][2] = 0.125 * a * b * S_XI[I][2];
-            for (int i = 0; i < 3; i++)
-                for (int j = 0; j < 3; j++) Jr[i][j] += sX[el][I][i] * dN[I][j];
-        }
-        double Ji[3][3];
-        Ji[0][0] = Jr[1][1] * Jr[2][2] - Jr[1][2] * Jr[2][1]; Ji[0][1] = Jr[0][2] * Jr[2][1] - Jr[0][1] * Jr[2][2]; Ji[0][2] = Jr[0][1] * Jr[1][2] - Jr[0][2] * Jr[1][1];
-        Ji[1][0] = Jr[1][2] * Jr[2][0] - Jr[1][0] * Jr[2][2]; Ji[1][1] = Jr[0][0] * Jr[2][2] - Jr[0][2] * Jr[2][0]; Ji[1][2] = Jr[0][2] * Jr[1][0] - Jr[0][0] * Jr[1][2];
-        Ji[2][0] = Jr[1][0] * Jr[2][1] - Jr[1][1] * Jr[2][0]; Ji[2][1] = Jr[0][1] * Jr[2][0] - Jr[0][0] * Jr[2][1]; Ji[2][2] = Jr[0][0] * Jr[1][1] - Jr[0][1] * Jr[1][0];
-        const double wq = Jr[0][0] * Ji[0][0] + Jr[0][1] * Ji[1][0] + Jr[0][2] * Ji[2][0];   // det J_ref, weights 1
-        double JT[3][3];   // J_ref^-1 Theta
-        for (int i = 0; i < 3; i++)
-            for (int j = 0; j < 3; j++) JT[i][j] = (Ji[i][0] * Th[0][j] + Ji[i][1] * Th[1][j] + Ji[i][2] * Th[2][j]) / wq;
-        double G[8][3];
-        for (int I = 0; I < 8; I++)
-            for (int j = 0; j < 3; j++) G[I][j] = dN[I][0] * JT[0][j] + dN[I][1] * JT[1][j] + dN[I][2] * JT[2][j];
-        // ---- F' = F Theta = Theta + u^T G'  (Eq.(30) :228), C' = F'^T F'
-        double F[3][3];
-        for (int i = 0; i < 3; i++)
-            for (int j = 0; j < 3; j++) {
-                double s = Th[i][j];
-                for (int I = 0; I < 8; I++) s += sU[el][I][i] * G[I][j];
-                F[i][j] = s;
+            const double a = 1.0 + xi0 * S_XI[I][0], b = 1.0 + xi1 * S_XI[I][1], c = 1.0 + xi2 * S_XI[I][2];
+            const double dn0 = 0.125 * S_XI[I][0] * b * c, dn1 = 0.125 * a * S_XI[I][1] * c, dn2 = 0.125 * a * b * S_XI[I][2];
+#pragma unroll
+            for (int i = 0; i < 3; i++) {
+                const double x = sX[el][I][i];
+                Jr[i][0] = fma(x, dn0, Jr[i][0]); Jr[i][1] = fma(x, dn1, Jr[i][1]); Jr[i][2] = fma(x, dn2, Jr[i][2]);
             }
-        double Cw[3][3], R[3][3], lm[3];
-        for (int i = 0; i < 3; i++)
-            for (int j = 0; j < 3; j++) Cw[i][j] = F[0][i] * F[0][j] + F[1][i] * F[1][j] + F[2][i] * F[2][j];
-        jacobi3(Cw, R, lm);
-        // ---- Hencky strain in the material frame (Eq.(4)-(5) :92-96, reading G1: the factor 1/2)
-        double eh[6] = {0.5 * log(lm[0]), 0.5 * log(lm[1]), 0.5 * log(lm[2]), 0, 0, 0}, eps[6];
-        rot6(R, eh, eps, 1);
-        // ---- history in, rotated into the material frame
+        }
+        double wq;
+        double F[3][3];
+        {
+            double Ji[3][3];
+            Ji[0][0] = Jr[1][1] * Jr[2][2] - Jr[1][2] * Jr[2][1]; Ji[0][1] = Jr[0][2] * Jr[2][1] - Jr[0][1] * Jr[2][2]; Ji[0][2] = Jr[0][1] * Jr[1][2] - Jr[0][2] * Jr[1][1];
+            Ji[1][0] = Jr[1][2] * Jr[2][0] - Jr[1][0] * Jr[2][2]; Ji[1][1] = Jr[0][0] * Jr[2][2] - Jr[0][2] * Jr[2][0]; Ji[1][2] = Jr[0][2] * Jr[1][0] - Jr[0][0] * Jr[1][2];
+            Ji[2][0] = Jr[1][0] * Jr[2][1] - Jr[1][1] * Jr[2][0]; Ji[2][1] = Jr[0][1] * Jr[2][0] - Jr[0][0] * Jr[2][1]; Ji[2][2] = Jr[0][0] * Jr[1][1] - Jr[0][1] * Jr[1][0];
+            wq = Jr[0][0] * Ji[0][0] + Jr[0][1] * Ji[1][0] + Jr[0][2] * Ji[2][0];   // det J_ref, weights 1
+            const double iw = 1.0 / wq;
+            double JT[3][3];   // J_ref^-1 Theta
+#pragma unroll
+            for (int i = 0; i < 3; i++)
+#pragma unroll
+                for (int j = 0; j < 3; j++) JT[i][j] = (Ji[i][0] * Th[0][j] + Ji[i][1] * Th[1][j] + Ji[i][2] * Th[2][j]) * iw;
+            // F' = F Theta = Theta + u^T G'  (Eq.(30) :228)
+#pragma unroll
+            for (int i = 0; i < 3; i++)
+#pragma unroll
+                for (int j = 0; j < 3; j++) F[i][j] = Th[i][j];
+#pragma unroll
+            for (int I = 0; I < 8; I++) {
+                const double a = 1.0 + xi0 * S_XI[I][0], b = 1.0 + xi1 * S_XI[I][1], c = 1.0 + xi2 * S_XI[I][2];
+                const double dn0 = 0.125 * S_XI[I][0] * b * c, dn1 = 0.125 * a * S_XI[I][1] * c, dn2 = 0.125 * a * b * S_XI[I][2];
+                double g[3];
+#pragma unroll
+                for (int j = 0; j < 3; j++) { g[j] = dn0 * JT[0][j] + dn1 * JT[1][j] + dn2 * JT[2][j]; Gs[3 * I + j] = g[j]; }
+#pragma unroll
+                for (int i = 0; i < 3; i++) {
+                    const double ui = sU[el][I][i];
+                    F[i][0] = fma(ui, g[0], F[i][0]); F[i][1] = fma(ui, g[1], F[i][1]); F[i][2] = fma(ui, g[2], F[i][2]);
+                }
+            }
+        }
+        // ---- C' = F'^T F', cyclic Jacobi (5 sweeps), Hencky strain in the material frame (Eq.(4)-(5) :92-96, reading G1)
+        double R[3][3] = {{1, 0, 0}, {0, 1, 0}, {0, 0, 1}}, lm[3], gl[3];
+        {
+            double c00 = F[0][0] * F[0][0] + F[1][0] * F[1][0] + F[2][0] * F[2][0], c11 = F[0][1] * F[0][1] + F[1][1] * F[1][1] + F[2][1] * F[2][1];
+            double c22 = F[0][2] * F[0][2] + F[1][2] * F[1][2] + F[2][2] * F[2][2], c01 = F[0][0] * F[0][1] + F[1][0] * F[1][1] + F[2][0] * F[2][1];
+            double c12 = F[0][1] * F[0][2] + F[1][1] * F[1][2] + F[2][1] * F[2][2], c02 = F[0][0] * F[0][2] + F[1][0] * F[1][2] + F[2][0] * F[2][2];
+#pragma unroll 1
+            for (int sweep = 0; sweep < 5; sweep++) {
+                jacobi_rot(c00, c11, c01, c02, c12, R[0][0], R[0][1], R[1][0], R[1][1], R[2][0], R[2][1]);
+                jacobi_rot(c00, c22, c02, c01, c12, R[0][0], R[0][2], R[1][0], R[1][2], R[2][0], R[2][2]);
+                jacobi_rot(c11, c22, c12, c01, c02, R[0][1], R[0][2], R[1][1], R[1][2], R[2][1], R[2][2]);
+            }
+            lm[0] = c00; lm[1] = c11; lm[2] = c22;
+        }
+#pragma unroll
+        for (int a = 0; a < 3; a++) gl[a] = 0.5 * log(lm[a]);
+        double ee[6];
+        {
+            const double eh[6] = {gl[0], gl[1], gl[2], 0, 0, 0};
+            rot6<1>(R, eh, ee);
+        }
+        // ---- history in, rotated into the material frame; elastic trial strain
         const double *hp = hist_in + (e * 8 + q) * 7;
-        double epn_g[6] = {hp[0], hp[1], hp[2], hp[3], hp[4], hp[5]}, epn[6];
-        rot6(Th, epn_g, epn, 0);
         const double alpha_n = hp[6];
-        // ---- cotangent on hist_out: stored components -> tensor (shear / 2), rotated
-        double eb[6] = {0, 0, 0, 0, 0, 0}, ab = 0.0;
-        if (muv) {
-            const double *mq = muv + (e * 8 + q) * 7;
-            double t[6] = {mq[0], mq[1], mq[2], 0.5 * mq[3], 0.5 * mq[4], 0.5 * mq[5]};
-            rot6(Th, t, eb, 0);
-            ab = mq[6];
+        {
+            const double epn_g[6] = {hp[0], hp[1], hp[2], hp[3], hp[4], hp[5]};
+            double epn[6];
+            rot6<0>(Th, epn_g, epn);
+#pragma unroll
+            for (int k = 0; k < 6; k++) ee[k] -= epn[k];
         }
         // ---- trial state (Eq.(16)-(17) :160-165)
-        double ee[6], T[6], HT[6], N[6];
-        for (int k = 0; k < 6; k++) ee[k] = eps[k] - epn[k];
+        double T[6], HT[6], N[6];
         applyE(m, ee, T);
         applyH(m, T, HT);
         double phi = sqrt(fmax(dot6(T, HT), 0.0));
-        double sf, dsf, dh[3];
-        flow_all(m, alpha_n, sf, dsf, dh);
+        double sf, dsf;
+        flow2(m, alpha_n, sf, dsf);
         double dgam = 0.0, alpha = alpha_n, kap = 0.0;
         const bool plastic = phi - SW23 * sf > 0.0;
         SDinv D;
         if (plastic) {
             // ---- return map: f(dgam) = sigma_y(alpha)/phi(kappa) - 1 = 0, monotone increasing, f(0) < 0
             double lo = 0.0, hi = -1.0;
+#pragma unroll 1
             for (int it = 0; it < 60; it++) {
                 alpha = alpha_n + SW23 * dgam;
-                flow_all(m, alpha, sf, dsf, dh);
-                const double sy = SW23 * sf, dsy = (2.0 / 3.0) * dsf;   // d sigma_y / d dgam = W * W sigma_flow'
-                kap = dgam / sy;
+                flow2(m, alpha, sf, dsf);
+                const double sy = SW23 * sf, dsy = (2.0 / 3.0) * dsf, isy = frcp(sy);   // d sigma_y / d dgam = W^2 sigma_flow'
+                kap = dgam * isy;
                 makeDinv(m, kap, D);
                 applyDinv(D, ee, T);
                 applyH(m, T, HT);
-                phi = sqrt(dot6(T, HT));
-                for (int k = 0; k < 6; k++) N[k] = HT[k] / phi;
+                const double ph2 = dot6(T, HT), iphi = frsqrt(ph2);
+                phi = ph2 * iphi;
                 double mN[6];
-                applyDinv(D, N, mN);
-                const double a_ = dot6(N, mN);
-                const double f = sy / phi - 1.0;
-                const double dk = (sy - dgam * dsy) / (sy * sy);
-                const double df = dsy / phi + (sy / phi) * a_ * dk;
+                applyDinv(D, HT, mN);
+                const double a_ = dot6(HT, mN) * iphi * iphi;   // N : D^-1 : N
+                const double f = sy * iphi - 1.0;
+                const double dk = (sy - dgam * dsy) * isy * isy;
+                const double df = dsy * iphi + (sy * iphi) * a_ * dk;
                 if (f < 0.0) lo = dgam; else hi = dgam;
-                double nx = dgam - f / df;
+                double nx = dgam - f * frcp(df);
                 if (!(nx > lo) || (hi > 0.0 && !(nx < hi))) nx = (hi > 0.0) ? 0.5 * (lo + hi) : 2.0 * dgam + 1e-6;
-                const double step = fabs(nx - dgam);
-                const bool done = (fabs(f) <= 1e-15) || (step <= 4e-16 * nx);
-                if (done) break;
+                if (fabs(f) <= 1e-15 || fabs(nx - dgam) <= 4e-16 * nx) break;
                 dgam = nx;
             }
-        } else {
-            makeDinv(m, 0.0, D);
-        }
-        // ---- state at the solution
-        if (plastic) {
+            // state at the solution
             alpha = alpha_n + SW23 * dgam;
-            flow_all(m, alpha, sf, dsf, dh);
-            makeDinv(m, dgam / (SW23 * sf), D);
+            flow2(m, alpha, sf, dsf);
+            makeDinv(m, dgam * frcp(SW23 * sf), D);
             applyDinv(D, ee, T);
             applyH(m, T, HT);
-            phi = sqrt(dot6(T, HT));
-            for (int k = 0; k < 6; k++) N[k] = HT[k] / phi;
-            kap = dgam / phi;
+            const double ph2 = dot6(T, HT), iphi = frsqrt(ph2);
+            phi = ph2 * iphi;
+#pragma unroll
+            for (int k = 0; k < 6; k++) N[k] = HT[k] * iphi;
+            kap = dgam * iphi;
             makeDinv(m, kap, D);
         } else {
+#pragma unroll
             for (int k = 0; k < 6; k++) N[k] = 0.0;
         }
-        // ---- S^ = 2 g[a,b] T^_ab in the eigenbasis of C (PAPER.md:150), S' = R S^ R^T
+        // ---- divided differences of g = 1/2 ln at the eigenvalues of C
         double g1[3][3], g2[3][3][3];
-        for (int a = 0; a < 3; a++)
-            for (int b = a; b < 3; b++) g1[a][b] = g1[b][a] = (a == b) ? 0.5 / lm[a] : 0.5 * ln_dd1(lm[a], lm[b]);
-        for (int a = 0; a < 3; a++)
-            for (int b = a; b < 3; b++)
-                for (int c = b; c < 3; c++) {
-                    const double v = 0.5 * ln_dd2(lm[a], lm[b], lm[c]);
-                    g2[a][b][c] = g2[a][c][b] = g2[b][a][c] = g2[b][c][a] = g2[c][a][b] = g2[c][b][a] = v;
-                }
-        double Tq[6], Tq33[3][3], Sq[6], S6[6], S[3][3];
-        rot6(R, T, Tq, 0);
+        {
+            const double il0 = frcp(lm[0]), il1 = frcp(lm[1]), il2 = frcp(lm[2]);
+            g1[0][0] = 0.5 * il0; g1[1][1] = 0.5 * il1; g1[2][2] = 0.5 * il2;
+            g1[0][1] = g1[1][0] = g_dd1(lm[0], lm[1], gl[0], gl[1]);
+            g1[1][2] = g1[2][1] = g_dd1(lm[1], lm[2], gl[1], gl[2]);
+            g1[0][2] = g1[2][0] = g_dd1(lm[0], lm[2], gl[0], gl[2]);
+            g2[0][0][0] = -0.25 * il0 * il0; g2[1][1][1] = -0.25 * il1 * il1; g2[2][2][2] = -0.25 * il2 * il2;
+#pragma unroll
+            for (int a = 0; a < 3; a++)
+#pragma unroll
+                for (int b = 0; b < 3; b++)
+                    if (a != b) {   // g[a,a,b]: nodes (a, a, b), middle node a
+                        const double v = g_dd2(lm[a], lm[a], lm[b], g1[a][a], g1[a][b]);
+                        g2[a][a][b] = g2[a][b][a] = g2[b][a][a] = v;
+                    }
+            // g[0,1,2]: the middle node is the one opposite the widest gap
+            const double w01 = fabs(lm[0] - lm[1]), w12 = fabs(lm[1] - lm[2]), w02 = fabs(lm[0] - lm[2]);
+            const int mid = (w02 >= w01 && w02 >= w12) ? 1 : ((w01 >= w12) ? 2 : 0);
+            const int i0 = (mid == 0) ? 1 : 0, i2 = (mid == 2) ? 1 : 2;
+            const double x0 = (i0 == 0) ? lm[0] : lm[1], x2 = (i2 == 2) ? lm[2] : lm[1], x1 = (mid == 0) ? lm[0] : ((mid == 1) ? lm[1] : lm[2]);
+            const double ga = (mid == 0) ? g1[1][0] : ((mid == 1) ? g1[0][1] : g1[0][2]);   // g[x0, x1]
+            const double gb = (mid == 0) ? g1[0][2] : ((mid == 1) ? g1[1][2] : g1[2][1]);   // g[x1, x2]
+            const double v = g_dd2(x0, x1, x2, ga, gb);
+            g2[0][1][2] = g2[0][2][1] = g2[1][0][2] = g2[1][2][0] = g2[2][0][1] = g2[2][1][0] = v;
+        }
+        // ---- S^ = 2 g[a,b] T^_ab in the eigenbasis of C (PAPER.md:150), S' = R S^ R^T
+        double Tq[6], Tq33[3][3], S[3][3];
+        rot6<0>(R, T, Tq);
         to33(Tq, Tq33);
         {
-            double Sq33[3][3];
-            for (int a = 0; a < 3; a++)
-                for (int b = 0; b < 3; b++) Sq33[a][b] = 2.0 * g1[a][b] * Tq33[a][b];
-            to6(Sq33, Sq);
+            const double Sq[6] = {2.0 * g1[0][0] * Tq[0], 2.0 * g1[1][1] * Tq[1], 2.0 * g1[2][2] * Tq[2],
+                                  2.0 * g1[0][1] * Tq[3], 2.0 * g1[1][2] * Tq[4], 2.0 * g1[0][2] * Tq[5]};
+            double S6[6];
+            rot6<1>(R, Sq, S6);
+            to33(S6, S);
         }
-        rot6(R, Sq, S6, 1);
-        to33(S6, S);
         // ---- reverse: Pbar'_iK = w sum_I lam_Ii G'_IK (Eq.(35) :257);  P' = F' S'  (Eq.(26) :208)
-        double Pb[3][3], Fb[3][3], Sb33[3][3], Sb[6], Sbq[6], Sbq33[3][3];
-        for (int i = 0; i < 3; i++)
-            for (int j = 0; j < 3; j++) {
-                double s = 0.0;
-                for (int I = 0; I < 8; I++) s += sL[el][I][i] * G[I][j];
-                Pb[i][j] = wq * s;
+        double Fb[3][3], Sbq33[3][3];
+        {
+            double Pb[3][3] = {{0, 0, 0}, {0, 0, 0}, {0, 0, 0}};
+#pragma unroll
+            for (int I = 0; I < 8; I++) {
+                const double g0 = Gs[3 * I], g1_ = Gs[3 * I + 1], g2_ = Gs[3 * I + 2];
+#pragma unroll
+                for (int i = 0; i < 3; i++) {
+                    const double l = sL[el][I][i];
+                    Pb[i][0] = fma(l, g0, Pb[i][0]); Pb[i][1] = fma(l, g1_, Pb[i][1]); Pb[i][2] = fma(l, g2_, Pb[i][2]);
+                }
             }
-        for (int i = 0; i < 3; i++)
-            for (int j = 0; j < 3; j++) {
-                Fb[i][j] = Pb[i][0] * S[0][j] + Pb[i][1] * S[1][j] + Pb[i][2] * S[2][j];
-                Sb33[i][j] = F[0][i] * Pb[0][j] + F[1][i] * Pb[1][j] + F[2][i] * Pb[2][j];
+            double Sb[6], Sbq[6];
+            constexpr int PI[6] = {0, 1, 2, 0, 1, 0}, PJ[6] = {0, 1, 2, 1, 2, 2};
+#pragma unroll
+            for (int i = 0; i < 3; i++)
+#pragma unroll
+                for (int j = 0; j < 3; j++) {
+                    Pb[i][j] *= wq;
+                }
+#pragma unroll
+            for (int i = 0; i < 3; i++)
+#pragma unroll
+                for (int j = 0; j < 3; j++) Fb[i][j] = Pb[i][0] * S[0][j] + Pb[i][1] * S[1][j] + Pb[i][2] * S[2][j];
+#pragma unroll
+            for (int k = 0; k < 6; k++) {   // sym(F^T Pbar)
+                const int i = PI[k], j = PJ[k];
+                Sb[k] = 0.5 * (F[0][i] * Pb[0][j] + F[1][i] * Pb[1][j] + F[2][i] * Pb[2][j] + F[0][j] * Pb[0][i] + F[1][j] * Pb[1][i] + F[2][j] * Pb[2][i]);
             }
-        to6(Sb33, Sb);
-        rot6(R, Sb, Sbq, 0);
-        to33(Sbq, Sbq33);
+            rot6<0>(R, Sb, Sbq);
+            to33(Sbq, Sbq33);
+        }
         // dS = P_L:dT + (T:L_L):dC/2  (Eq.(25) :204):  Tbar^_ab = 2 g[a,b] Sbar^_ab,
         // Cbar^_ac = 2 sum_b g[a,b,c] (T^_ab Sbar^_bc + Sbar^_ab T^_bc)
-        double Tbq33[3][3], Cbq33[3][3], Tbq[6], Tb[6];
-        for (int a = 0; a < 3; a++)
-            for (int c = 0; c < 3; c++) {
-                Tbq33[a][c] = 2.0 * g1[a][c] * Sbq33[a][c];
+        double Cbq[6], Tb[6];
+        {
+            constexpr int PI[6] = {0, 1, 2, 0, 1, 0}, PJ[6] = {0, 1, 2, 1, 2, 2};
+            double Tbq[6];
+#pragma unroll
+            for (int k = 0; k < 6; k++) {
+                const int a = PI[k], c = PJ[k];
+                Tbq[k] = 2.0 * g1[a][c] * Sbq33[a][c];
                 double s = 0.0;
+#pragma unroll
                 for (int b = 0; b < 3; b++) s += g2[a][b][c] * (Tq33[a][b] * Sbq33[b][c] + Sbq33[a][b] * Tq33[b][c]);
-                Cbq33[a][c] = 2.0 * s;
+                Cbq[k] = 2.0 * s;
             }
-        to6(Tbq33, Tbq);
-        rot6(R, Tbq, Tb, 1);
+            rot6<1>(R, Tbq, Tb);
+        }
+        // ---- cotangent on hist_out: stored components -> tensor (shear / 2), rotated into the material frame
+        double eb[6] = {0, 0, 0, 0, 0, 0}, ab = 0.0;
+        if (muv) {
+            const double *mq = muv + (e * 8 + q) * 7;
+            const double t[6] = {mq[0], mq[1], mq[2], 0.5 * mq[3], 0.5 * mq[4], 0.5 * mq[5]};
+            rot6<0>(Th, t, eb);
+            ab = mq[6];
+        }
         // ---- transposed App. D solve (Eq.(D4)-(D7) :1002-1019)
-        double v[6], wT[6], epb[6], alb;
+        double v[6], wT[6], alb;
         if (plastic) {
-            flow_all(m, alpha, sf, dsf, dh);
             double Heb[6], yT[6], mN[6], b[6];
             applyH(m, eb, Heb);
             const double Neb = dot6(N, eb);
+#pragma unroll
             for (int k = 0; k < 6; k++) yT[k] = Tb[k] + kap * (Heb[k] - N[k] * Neb);
             applyDinv(D, N, mN);
             applyDinv(D, yT, b);
-            const double a_ = dot6(N, mN), om = 1.0 - kap * a_, myT = dot6(mN, yT);
+            const double a_ = dot6(N, mN), iom = frcp(1.0 - kap * a_), myT = dot6(mN, yT);
             const double Hp = (2.0 / 3.0) * dsf;                       // W sigma_y' = 2/3 sigma_flow'
-            const double wf = (myT / om - SW23 * ab - Neb) / (a_ / om + Hp);
-            for (int k = 0; k < 6; k++) v[k] = b[k] + ((kap * myT - wf) / om) * mN[k];
+            const double wf = (myT * iom - SW23 * ab - Neb) * frcp(a_ * iom + Hp);
+            const double cm = (kap * myT - wf) * iom;
+#pragma unroll
+            for (int k = 0; k < 6; k++) v[k] = b[k] + cm * mN[k];
             alb = ab + SW23 * dsf * wf;
             applyEinv(m, v, wT);
             // theta: r_k and hardening constants
-            double x[6], B1[6], B2[6];
+            double x[6], B1[6], B2[6], dh[3];
+#pragma unroll
             for (int k = 0; k < 6; k++) x[k] = dgam * (eb[k] - v[k]);
             hill_bilinear_ds(x, T, B1);
             hill_bilinear_ds(T, T, B2);
-            const double xN = dot6(x, N);
-            for (int k = 0; k < 6; k++)
-                gth[2 + k] = (-2.0 / (m.r[k] * m.r[k] * m.r[k])) * (B1[k] / phi - (xN / (2.0 * phi * phi) + wf / (2.0 * phi)) * B2[k]);
+            const double iphi = frcp(phi), c2 = (0.5 * dot6(x, N) * iphi + 0.5 * wf) * iphi;
+#pragma unroll
+            for (int k = 0; k < 6; k++) {
+                const double rk = mp[2 + k];
+                gth[2 + k] = -2.0 * (B1[k] * iphi - c2 * B2[k]) / (rk * rk * rk);
+            }
+            flow_dh(m, alpha, dh);
+#pragma unroll
             for (int k = 0; k < 3; k++) gth[8 + k] = SW23 * wf * dh[k];
         } else {
+#pragma unroll
             for (int k = 0; k < 6; k++) wT[k] = Tb[k];
             applyE(m, Tb, v);
             alb = ab;
         }
-        for (int k = 0; k < 6; k++) epb[k] = eb[k] - v[k];
         {
             // E and nu: dG_T/dE = -T/E, dG_T/dnu = -(dE/dnu):ee_el with ee_el = E^-1 T
             double eel[6], dEnu[6];
@@ -427,57 +490,69 @@ k_sens_point(long long n_elems, const double *__restrict__ coords, const int *__
             const double op = 1.0 + m.nu, om2 = 1.0 - 2.0 * m.nu;
             const double dmu2 = -m.E / (op * op), dlam = m.E * (1.0 + 2.0 * m.nu * m.nu) / (op * op * om2 * om2);
             const double tr = dlam * (eel[0] + eel[1] + eel[2]);
+#pragma unroll
             for (int k = 0; k < 3; k++) dEnu[k] = dmu2 * eel[k] + tr;
+#pragma unroll
             for (int k = 3; k < 6; k++) dEnu[k] = dmu2 * eel[k];
-            gth[0] = dot6(wT, T) / m.E;
+            gth[0] = dot6(wT, T) * m.iE;
             gth[1] = dot6(wT, dEnu);
         }
         // ---- history-in cotangent back in the global frame, stored components (shear x 2)
         if (g_hist) {
-            double o6[6];
-            rot6(Th, epb, o6, 1);
+            double epb[6], o6[6];
+#pragma unroll
+            for (int k = 0; k < 6; k++) epb[k] = eb[k] - v[k];
+            rot6<1>(Th, epb, o6);
             double *go = g_hist + (e * 8 + q) * 7;
             go[0] = o6[0]; go[1] = o6[1]; go[2] = o6[2]; go[3] = 2.0 * o6[3]; go[4] = 2.0 * o6[4]; go[5] = 2.0 * o6[5];
             go[6] = alb;
         }
         // ---- d eps = P_L : dC / 2:  Cbar^_ab += g[a,b] epsbar^_ab;  C = F^T F: Fbar += 2 F Cbar;  ubar_Ii = Fbar_iJ G_IJ
-        double vq[6], vq33[3][3], Cb6[6], Cb[6], Cb33[3][3];
-        rot6(R, v, vq, 0);
-        to33(vq, vq33);
-        for (int a = 0; a < 3; a++)
-            for (int b = 0; b < 3; b++) Cbq33[a][b] += g1[a][b] * vq33[a][b];
-        to6(Cbq33, Cb6);
-        rot6(R, Cb6, Cb, 1);
-        to33(Cb, Cb33);
-        for (int i = 0; i < 3; i++)
-            for (int j = 0; j < 3; j++) Fb[i][j] += 2.0 * (F[i][0] * Cb33[0][j] + F[i][1] * Cb33[1][j] + F[i][2] * Cb33[2][j]);
-        for (int I = 0; I < 8; I++)
-            for (int i = 0; i < 3; i++) sGu[el][q][3 * I + i] = Fb[i][0] * G[I][0] + Fb[i][1] * G[I][1] + Fb[i][2] * G[I][2];
+        if (gu_scr) {
+            double vq[6], Cb[6], Cb33[3][3];
+            rot6<0>(R, v, vq);
+            Cbq[0] += g1[0][0] * vq[0]; Cbq[1] += g1[1][1] * vq[1]; Cbq[2] += g1[2][2] * vq[2];
+            Cbq[3] += g1[0][1] * vq[3]; Cbq[4] += g1[1][2] * vq[4]; Cbq[5] += g1[0][2] * vq[5];
+            rot6<1>(R, Cbq, Cb);
+            to33(Cb, Cb33);
+#pragma unroll
+            for (int i = 0; i < 3; i++)
+#pragma unroll
+                for (int j = 0; j < 3; j++) Fb[i][j] += 2.0 * (F[i][0] * Cb33[0][j] + F[i][1] * Cb33[1][j] + F[i][2] * Cb33[2][j]);
+#pragma unroll
+            for (int I = 0; I < 8; I++) {
+                const double g0 = Gs[3 * I], g1_ = Gs[3 * I + 1], g2_ = Gs[3 * I + 2];
+#pragma unroll
+                for (int i = 0; i < 3; i++) Gs[3 * I + i] = Fb[i][0] * g0 + Fb[i][1] * g1_ + Fb[i][2] * g2_;
+            }
+        }
     }
+#pragma unroll
     for (int k = 0; k < NTHETA; k++) sTh[tid][k] = gth[k];
     __syncthreads();
     if (live) {
         // lane q sums local node q over the 8 Gauss points, ascending
         if (gu_scr) {
             const long long j = eslot[e * 8 + q];
+#pragma unroll
             for (int i = 0; i < 3; i++) {
                 double s = 0.0;
+#pragma unroll
                 for (int p = 0; p < 8; p++) s += sGu[el][p][3 * q + i];
                 gu_scr[3 * j + i] = s;
             }
         }
-        if (g_mat) {   // per-element records: points summed ascending
-            for (int k = q; k < FEM_NPAR; k += 8) g_mat[e * FEM_NPAR + k] = 0.0;
-        }
-    }
-    if (g_mat) {
-        __syncthreads();
-        if (live)
-            for (int k = q; k < NTHETA; k += 8) {
+        if (g_mat) {   // per-element records: points summed ascending; the entries that are not differentiated are 0
+            for (int k = q; k < FEM_NPAR; k += 8) {
+                int t = -1;
+#pragma unroll
+                for (int j = 0; j < NTHETA; j++) t = (S_THETA_IDX[j] == k) ? j : t;
                 double s = 0.0;
-                for (int p = 0; p < 8; p++) s += sTh[el * 8 + p][k];
-                g_mat[e * FEM_NPAR + S_THETA_IDX[k]] = s;
+                if (t >= 0)
+                    for (int p = 0; p < 8; p++) s += sTh[el * 8 + p][t];
+                g_mat[e * FEM_NPAR + k] = s;
             }
+        }
     }
     if (part && tid < NTHETA) {
         double s = 0.0;
