@@ -311,3 +311,43 @@ def test_adjoint_gradient_of_load_path_matches_oracle():
     assert np.max(np.abs(gg[idx] - grad_o[idx]) / np.maximum(np.abs(grad_o[idx]), 1e-6 * np.abs(grad_o[idx]).max())) <= 1e-6
     assert rel_l2(mu_d.cpu().numpy(), mu_o) <= 1e-6
     ctx.close()
+
+
+def test_vjp_config4_and_config5_samples():
+    """Config 4 (void-mask mesh, shuffled element order, per-element Hill ratios and Swift K: irregular gather, nodes with fewer
+    than 8 elements, n_mat = n_elems) and the top strain level of config 5 (peak strain 0.3): sampled elements (g_hist_in,
+    per-element g_mat) and sampled nodes (g_u) against the oracle; K lam against the library's own tangent."""
+    import torch
+    import oracle
+    import oracle.sens as osn
+    import synth
+    import paper_2606_17390_b200 as fem
+    dev = torch.device("cuda:0")
+    for label, cfg in (("config4", synth.make_config(4)), ("config5s3", synth.make_config(5, sweep="strain", level=3))):
+        ne, nn = cfg["conn"].shape[0], cfg["coords"].shape[0]
+        mat_np = np.ascontiguousarray(fem.mat_from_desc(cfg["matdesc"], ne))
+        omat = np.ascontiguousarray(oracle.mat_from_desc(cfg["matdesc"], ne))
+        ctx = _ctx(cfg["coords"], cfg["conn"])
+        g = torch.Generator(device="cpu"); g.manual_seed(11)
+        lam = torch.randn(3 * nn, dtype=torch.float64, generator=g).to(dev)
+        mu = (torch.randn(ne, 8, 7, dtype=torch.float64, generator=g) * torch.tensor([1e3] * 6 + [1e2], dtype=torch.float64)).reshape(-1).to(dev)
+        u = torch.from_numpy(cfg["u"].ravel()).to(dev); h = torch.from_numpy(cfg["hist_in"].ravel()).to(dev)
+        mat = torch.from_numpy(mat_np.ravel()).to(dev)
+        _, vals, _, _ = ctx.assemble(u, h, mat)
+        a_u, _, _ = ctx.assemble_vjp(u, h, mat, lam, None, want_hist=False, want_mat=False)
+        Kl = ctx.spmv(vals, lam)
+        assert float(torch.linalg.norm(a_u - Kl) / torch.linalg.norm(Kl)) <= 1e-10, label
+        c_u, c_h, c_m = ctx.assemble_vjp(u, h, mat, lam, mu)
+        lam_n, mu_n = lam.cpu().numpy().reshape(nn, 3), mu.cpu().numpy().reshape(ne, 8, 7)
+        rng = np.random.default_rng(12)
+        el = np.sort(rng.choice(ne, 40, replace=False))
+        o = osn.assemble_vjp(cfg["coords"], cfg["conn"], cfg["u"], cfg["hist_in"], omat, lam_n, mu_n, elems=el)
+        assert rel_l2(c_h.cpu().numpy().reshape(ne, 8, 7)[el], o["g_hist_in"][el]) <= TOL, label
+        if omat.shape[0] == ne:
+            gm = c_m.cpu().numpy()[el]
+            assert np.max(np.abs(gm - o["g_mat"][el]) / np.maximum(o["g_mat_abs"][el].max(axis=0), 1e-300)) <= TOL, label
+        nodes = rng.choice(nn, 10, replace=False)
+        els = np.unique(np.flatnonzero(np.isin(cfg["conn"], nodes).any(axis=1)))
+        o2 = osn.assemble_vjp(cfg["coords"], cfg["conn"], cfg["u"], cfg["hist_in"], omat, lam_n, mu_n, elems=els)
+        assert rel_l2(c_u.cpu().numpy().reshape(nn, 3)[nodes], o2["g_u_full"][nodes]) <= TOL, label
+        ctx.close()
