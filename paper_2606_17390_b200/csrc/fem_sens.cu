@@ -28,6 +28,12 @@
 #define SEL 16                        // elements per CTA
 #define STHREADS (8 * SEL)
 #define NTHETA 11
+// Phase barriers keep the warps of a CTA in the same code region so that they share instruction-cache lines (the pass is
+// ~7,000 straight-line instructions per warp; instruction fetch was the top stall without them).
+#ifndef SENS_PS_MASK
+#define SENS_PS_MASK 0x1f
+#endif
+#define SENS_SYNC(n) do { if ((SENS_PS_MASK >> (n)) & 1) __syncthreads(); } while (0)
 #ifndef SENS_CTAS
 #define SENS_CTAS 3                   // CTAs per SM the register allocation aims at
 #endif
@@ -181,12 +187,14 @@ k_sens_point(long long n_elems, const double *__restrict__ coords, const int *__
     __shared__ double sGu[SEL][8][25];      // per thread: G' (24 doubles, odd stride) during the pass, then its ubar contributions
     __shared__ double sTh[STHREADS][NTHETA];
     const int tid = threadIdx.x, el = tid >> 3, q = tid & 7;
-    const long long e = (long long)blockIdx.x * SEL + el;
-    const bool live = e < n_elems;
+    const long long e_raw = (long long)blockIdx.x * SEL + el;
+    const bool live = e_raw < n_elems;
+    const long long e = live ? e_raw : n_elems - 1;   // threads past the end redo the last element (no output): every thread
+                                                      // reaches the phase barriers below
     double gth[NTHETA];
 #pragma unroll
     for (int k = 0; k < NTHETA; k++) gth[k] = 0.0;
-    if (live) {
+    {
         const int nd = conn[e * 8 + q];
 #pragma unroll
         for (int i = 0; i < 3; i++) {
@@ -196,7 +204,7 @@ k_sens_point(long long n_elems, const double *__restrict__ coords, const int *__
         }
     }
     __syncthreads();
-    if (live) {
+    {
         double *Gs = &sGu[el][q][0];
         // ---- material record
         const double *mp = mat + (n_mat == 1 ? 0 : e) * FEM_NPAR;
@@ -265,6 +273,7 @@ k_sens_point(long long n_elems, const double *__restrict__ coords, const int *__
                 }
             }
         }
+        SENS_SYNC(5);
         // ---- C' = F'^T F', cyclic Jacobi (5 sweeps), Hencky strain in the material frame (Eq.(4)-(5) :92-96, reading G1)
         double R[3][3] = {{1, 0, 0}, {0, 1, 0}, {0, 0, 1}}, lm[3], gl[3];
         {
@@ -296,6 +305,7 @@ k_sens_point(long long n_elems, const double *__restrict__ coords, const int *__
 #pragma unroll
             for (int k = 0; k < 6; k++) ee[k] -= epn[k];
         }
+        SENS_SYNC(0);
         // ---- trial state (Eq.(16)-(17) :160-165)
         double T[6], HT[6], N[6];
         applyE(m, ee, T);
@@ -348,6 +358,7 @@ k_sens_point(long long n_elems, const double *__restrict__ coords, const int *__
 #pragma unroll
             for (int k = 0; k < 6; k++) N[k] = 0.0;
         }
+        SENS_SYNC(1);
         // ---- divided differences of g = 1/2 ln at the eigenvalues of C
         double g1[3][3], g2[3][3][3];
         {
@@ -375,6 +386,7 @@ k_sens_point(long long n_elems, const double *__restrict__ coords, const int *__
             const double v = g_dd2(x0, x1, x2, ga, gb);
             g2[0][1][2] = g2[0][2][1] = g2[1][0][2] = g2[1][2][0] = g2[2][0][1] = g2[2][1][0] = v;
         }
+        SENS_SYNC(6);
         // ---- S^ = 2 g[a,b] T^_ab in the eigenbasis of C, S' = R S^ R^T
         double Tq[6], Tq33[3][3], S[3][3];
         rot6<0>(R, T, Tq);
@@ -386,6 +398,7 @@ k_sens_point(long long n_elems, const double *__restrict__ coords, const int *__
             rot6<1>(R, Sq, S6);
             to33(S6, S);
         }
+        SENS_SYNC(2);
         // ---- reverse: Pbar'_iK = w sum_I lam_Ii G'_IK (Eq.(35) :257);  P' = F' S'  (Eq.(26) :208)
         double Fb[3][3], Sbq33[3][3];
         {
@@ -444,6 +457,7 @@ k_sens_point(long long n_elems, const double *__restrict__ coords, const int *__
             rot6<0>(Th, t, eb);
             ab = mq[6];
         }
+        SENS_SYNC(3);
         // ---- transposed App. D solve (Eq.(D4)-(D7) :1002-1019)
         double v[6], wT[6], alb;
         if (plastic) {
@@ -497,8 +511,9 @@ k_sens_point(long long n_elems, const double *__restrict__ coords, const int *__
             gth[0] = dot6(wT, T) * m.iE;
             gth[1] = dot6(wT, dEnu);
         }
+        SENS_SYNC(4);
         // ---- history-in cotangent back in the global frame, stored components (shear x 2)
-        if (g_hist) {
+        if (g_hist && live) {
             double epb[6], o6[6];
 #pragma unroll
             for (int k = 0; k < 6; k++) epb[k] = eb[k] - v[k];
@@ -507,6 +522,7 @@ k_sens_point(long long n_elems, const double *__restrict__ coords, const int *__
             go[0] = o6[0]; go[1] = o6[1]; go[2] = o6[2]; go[3] = 2.0 * o6[3]; go[4] = 2.0 * o6[4]; go[5] = 2.0 * o6[5];
             go[6] = alb;
         }
+        SENS_SYNC(7);
         // ---- d eps = P_L : dC / 2:  Cbar^_ab += g[a,b] epsbar^_ab;  C = F^T F: Fbar += 2 F Cbar;  ubar_Ii = Fbar_iJ G_IJ
         if (gu_scr) {
             double vq[6], Cb[6], Cb33[3][3];
@@ -528,7 +544,7 @@ k_sens_point(long long n_elems, const double *__restrict__ coords, const int *__
         }
     }
 #pragma unroll
-    for (int k = 0; k < NTHETA; k++) sTh[tid][k] = gth[k];
+    for (int k = 0; k < NTHETA; k++) sTh[tid][k] = live ? gth[k] : 0.0;
     __syncthreads();
     if (live) {
         // lane q sums local node q over the 8 Gauss points, ascending
