@@ -11,7 +11,7 @@ NBARLAT = 20
 ABI_SYMBOLS = ["fem_default_options", "fem_setup", "fem_build_csr_pattern", "fem_assemble", "fem_assemble_barlat", "fem_assemble_host",
                "fem_last_kernel_ms", "fem_launches_per_assemble", "fem_probe_fp64_peak", "fem_destroy", "fem_strerror",
                "fem_last_cuda_error", "fem_hill_from_lankford", "fem_spmv", "fem_apply_dirichlet", "fem_bicgstab", "fem_pcg", "fem_lincomb",
-               "fem_default_newton_options", "fem_newton_solve", "fem_assemble_vjp"]
+               "fem_default_newton_options", "fem_newton_solve", "fem_assemble_vjp", "fem_adjoint_step"]
 
 
 class FemOptions(C.Structure):
@@ -101,6 +101,7 @@ def lib():
         L.fem_newton_solve.argtypes = [vp, vp, vp, vp, ll, ll, vp, vp, vp, C.POINTER(FemNewtonOptions),
                                        C.POINTER(FemNewtonReport), vp]
         L.fem_assemble_vjp.argtypes = [vp, vp, vp, vp, ll, vp, vp, vp, vp, vp, vp]
+        L.fem_adjoint_step.argtypes = [vp, vp, vp, vp, ll, ll, vp, vp, vp, vp, vp, vp, C.c_double, C.c_int, C.POINTER(C.c_int), vp]
         _lib = L
     return _lib
 
@@ -341,6 +342,24 @@ class FemContext:
                                       opt(g_u, self.n_rows, "g_u"), opt(g_h, 56 * self.n_elems, "g_hist_in"),
                                       opt(g_m, n_mat * NPAR, "g_mat"), _stream_ptr()), "fem_assemble_vjp")
         return g_u, g_h, (g_m.view(n_mat, NPAR) if g_m is not None else None)
+
+    def adjoint_step(self, u, hist_in, mat, bc_dofs, dJdu=None, mu_in=None, lin_rtol=1e-10, lin_max_iter=10000):
+        """fem_adjoint_step: one step of the backward sweep of Alg. 1.  Returns (lam, mu_out, g_mat, lin_iters)."""
+        torch = _torch()
+        f64 = torch.float64
+        n_mat = mat.numel() // NPAR
+        lam = torch.empty(self.n_rows, dtype=f64, device=self.device)
+        mu_out = torch.empty(self.n_elems * 56, dtype=f64, device=self.device)
+        g_m = torch.empty(n_mat * NPAR, dtype=f64, device=self.device)
+        it = C.c_int(0)
+        opt = lambda t, n, name: None if t is None else _ptr(t, f64, n, name)
+        _check(lib().fem_adjoint_step(self._h, _ptr(u, f64, self.n_rows, "u"), _ptr(hist_in, f64, 56 * self.n_elems, "hist_in"),
+                                      _ptr(mat, f64, None, "mat"), n_mat, bc_dofs.numel(), _ptr(bc_dofs, torch.int32, None, "bc_dofs"),
+                                      opt(dJdu, self.n_rows, "dJdu"), opt(mu_in, 56 * self.n_elems, "mu_in"),
+                                      _ptr(lam, f64, self.n_rows, "lam"), _ptr(mu_out, f64, 56 * self.n_elems, "mu_out"),
+                                      _ptr(g_m, f64, n_mat * NPAR, "g_mat"), float(lin_rtol), int(lin_max_iter), C.byref(it),
+                                      _stream_ptr()), "fem_adjoint_step")
+        return lam, mu_out, g_m.view(n_mat, NPAR), it.value
 
     def last_kernel_ms(self):
         ms = (C.c_double * 3)()

@@ -648,3 +648,45 @@ extern "C" int fem_newton_solve(fem_ctx *c, double *u, const double *hist_in, co
     if (rep) *rep = rp;
     return result;
 }
+
+// One step of the backward sweep of Alg. 1: right-hand side of Eq.(51) :366, adjoint solve on the tangent
+// of the converged state (K_ff is symmetric for the standard element, so the row-eliminated K serves for K^T with lam = 0 on the
+// constrained DOFs), then the products of Eq.(49) :355 and the history cotangent for the step before (reading G17).
+__global__ void k_adj_rhs(long long n, const double *__restrict__ dJdu, const double *__restrict__ gu, double *__restrict__ rhs) {
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x)
+        rhs[i] = -((dJdu ? dJdu[i] : 0.0) + (gu ? gu[i] : 0.0));
+}
+
+extern "C" int fem_adjoint_step(fem_ctx *c, const double *u, const double *hist_in, const double *mat, long long n_mat,
+                                long long n_bc, const int *bc_dofs, const double *dJdu, const double *mu_in, double *lam,
+                                double *mu_out, double *g_mat, double lin_rtol, int lin_max_iter, int *lin_iters,
+                                void *cuda_stream) {
+    if (!c || !u || !hist_in || !mat || !lam || !mu_out || !g_mat || (n_bc > 0 && !bc_dofs)) return FEM_ERR_NULL;
+    if (!c->has_pattern) return FEM_ERR_NO_PATTERN;
+    if (n_mat != 1 && n_mat != c->n_elems) return FEM_ERR_MAT;
+    if (n_bc < 0 || c->opt.fbar != 0 || !(lin_rtol > 0.0) || lin_max_iter < 1) return FEM_ERR_ARG;
+    if (mu_out == hist_in || mu_out == mu_in) return FEM_ERR_ALIAS;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int rc = ensure_solver_ws(c, true);
+    if (rc != FEM_OK) return rc;
+    if ((rc = check_dofs(c, n_bc, bc_dofs, st)) != FEM_OK) return rc;
+    const long long n = c->n_rows;
+    double *R = c->d_nw, *rhs = R + n, *gu = rhs + n, *vals = c->d_nw_vals;
+    // tangent at the converged state; mu_out serves as the (unused) hist_out of this evaluation before it is overwritten below
+    if ((rc = fem_launch_assemble(c, u, hist_in, mat, n_mat, R, vals, mu_out, st)) != FEM_OK) return rc;
+    if (mu_in) {   // (dR^{n+1}/du^n)^T lam^{n+1} = (dhist_out/du)^T mu_in
+        if ((rc = fem_assemble_vjp(c, u, hist_in, mat, n_mat, nullptr, mu_in, gu, nullptr, nullptr, cuda_stream)) != FEM_OK) return rc;
+    }
+    k_adj_rhs<<<RED_CTAS, RED_THREADS, 0, st>>>(n, dJdu, mu_in ? gu : nullptr, rhs);
+    if ((rc = apply_dirichlet(c, n_bc, bc_dofs, nullptr, nullptr, nullptr, vals, rhs, st)) != FEM_OK) return rc;
+    FEM_CUDA(cudaMemsetAsync(lam, 0, sizeof(double) * n, st));
+    int its = 0, its2 = 0;
+    rc = pcg(c, vals, rhs, lam, lin_rtol, lin_max_iter, &its, nullptr, st);
+    if (rc == FEM_ERR_NOCONV) {   // K_ff not positive definite at this state: BiCGSTAB from zero (K_ff is still symmetric)
+        FEM_CUDA(cudaMemsetAsync(lam, 0, sizeof(double) * n, st));
+        rc = bicgstab(c, vals, rhs, lam, lin_rtol, lin_max_iter, &its2, nullptr, st);
+    }
+    if (lin_iters) *lin_iters = its + its2;
+    if (rc != FEM_OK) return rc;
+    return fem_assemble_vjp(c, u, hist_in, mat, n_mat, lam, mu_in, nullptr, mu_out, g_mat, cuda_stream);
+}

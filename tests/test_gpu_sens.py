@@ -245,6 +245,7 @@ def test_adjoint_gradient_of_load_path_matches_oracle():
     import oracle
     import oracle.sens as osn
     import oracle.newton as onw
+    import paper_2606_17390_b200 as fem
     from synth import mesh
     p = _small_problem(seed=4, n=(2, 2, 2), hist=False)
     coords, conn, mat = p["coords"], p["conn"], p["mat"]
@@ -310,6 +311,23 @@ def test_adjoint_gradient_of_load_path_matches_oracle():
     idx = list(osn.THETA_IDX)
     assert np.max(np.abs(gg[idx] - grad_o[idx]) / np.maximum(np.abs(grad_o[idx]), 1e-6 * np.abs(grad_o[idx]).max())) <= 1e-6
     assert rel_l2(mu_d.cpu().numpy(), mu_o) <= 1e-6
+    # the same backward sweep through fem_adjoint_step (one C-ABI call per load step)
+    grad_s, mu_s = torch.zeros(16, dtype=torch.float64, device=dev), None
+    for (u, h), g in zip(reversed(gstates), reversed(ugt)):
+        lam_s, mu_s, g_m, its = ctx.adjoint_step(u, h, mat_d, bc_d, dJdu=2.0 * (u - t64(g)), mu_in=mu_s, lin_rtol=1e-13)
+        assert its > 0 and float(torch.abs(lam_s[bc_d.long()]).max()) == 0.0
+        grad_s += g_m[0]
+    gs = grad_s.cpu().numpy()
+    assert np.max(np.abs(gs[idx] - gg[idx]) / np.maximum(np.abs(gg[idx]), 1e-6 * np.abs(gg[idx]).max())) <= 1e-9
+    assert np.max(np.abs(gs[idx] - grad_o[idx]) / np.maximum(np.abs(grad_o[idx]), 1e-6 * np.abs(grad_o[idx]).max())) <= 1e-6
+    assert rel_l2(mu_s.cpu().numpy(), mu_o) <= 1e-6
+    with pytest.raises(fem.FemError):      # mu_out must not alias hist_in: checked by the library
+        import ctypes as C
+        L = fem.lib()
+        rc = L.fem_adjoint_step(ctx._h, u.data_ptr(), h.data_ptr(), mat_d.data_ptr(), 1, bc_d.numel(), bc_d.data_ptr(), None, None,
+                                lam_s.data_ptr(), h.data_ptr(), g_m.data_ptr(), 1e-10, 100, None, None)
+        if rc != 0:
+            raise fem.FemError(rc, "fem_adjoint_step")
     ctx.close()
 
 
