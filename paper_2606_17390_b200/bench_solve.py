@@ -37,6 +37,8 @@ def main():
     ap.add_argument("--full", type=float, default=0.0, help="if > 0: run the whole benchmark loading (right face to 0.2, 0.1 mm) with "
                     "adaptive stepping (the paper's dt_initial 1e-3, dt_max 5e-2, cut-back on failure, :485) for at most this many seconds")
     ap.add_argument("--extrapolate", type=int, default=1, help="initial guess of a step: 0 last state, 1 linear, 2 quadratic extrapolation")
+    ap.add_argument("--adjoint", type=int, default=0, help="1: after the load path, run the backward sweep of Alg. 1 (fem_adjoint_step per step) "
+                    "for J = 1/2 sum_n |u^n|^2 on the free DOFs and check dJ/d(sigma0) against a central difference of two more forward paths")
     ap.add_argument("--grow-below", type=int, default=6, help="grow the step after a step with at most this many Newton iterations")
     args = ap.parse_args()
     n = args.n
@@ -131,6 +133,47 @@ def main():
     dt = time.perf_counter() - t_path
     print("| path total | %d Newton iterations | %d linear iterations | %.2f s = %.2f s per Newton iteration |"
           % (tot_newton, tot_lin, dt, dt / max(tot_newton, 1)))
+
+    # ---- 4b. NEXT-3: the discrete adjoint of that path (Alg. 1) and the paper's own check of it (Eq.(52) :412)
+    if args.adjoint:
+        free = torch.ones(nr, dtype=torch.float64, device=dev)
+        free[bc_d.long()] = 0.0
+
+        def forward(mat_t, keep):
+            u = torch.zeros(nr, dtype=torch.float64, device=dev)
+            h_a = torch.zeros(56 * ne, dtype=torch.float64, device=dev)
+            states, J = [], 0.0
+            for k in range(1, nsteps + 1):
+                u, h_b, rep = ctx.newton_solve(u, h_a, mat_t, bc_d, torch.from_numpy(full * (step * k)).to(dev),
+                                               lin_rtol=1e-10, lin_max_iter=20000, rtol=1e-9, atol=1e-8, max_newton=15)
+                assert rep["converged"], rep
+                J += 0.5 * float(((u * free) ** 2).sum())
+                if keep:
+                    states.append((u.clone(), h_a))
+                h_a = h_b
+            return J, states
+        torch.cuda.synchronize(); t0 = time.perf_counter()
+        J0, states = forward(mat, True)
+        torch.cuda.synchronize(); t_fwd = time.perf_counter() - t0
+        t0 = time.perf_counter()
+        grad = torch.zeros(16, dtype=torch.float64, device=dev)
+        mu, its_tot = None, 0
+        for (u_n, h_nm1) in reversed(states):
+            lam, mu, g_m, its = ctx.adjoint_step(u_n, h_nm1, mat, bc_d, dJdu=u_n * free, mu_in=mu, lin_rtol=1e-10, lin_max_iter=20000)
+            grad += g_m[0]; its_tot += its
+        torch.cuda.synchronize(); t_bwd = time.perf_counter() - t0
+        g = grad.cpu().numpy()
+        print("\n| adjoint of the %d-step path (J = 1/2 sum |u^n|^2 on the free DOFs = %.6e) | forward %.2f s (Newton rtol 1e-9, linear 1e-10) | backward sweep %.2f s "
+              "= %.2f s per step, %d CG iterations |" % (nsteps, J0, t_fwd, t_bwd, t_bwd / nsteps, its_tot))
+        names = ["E", "nu", "r11", "r22", "r33", "r12", "r23", "r13", "law", "sigma0", "Q", "b"]
+        print("| dJ/dtheta | " + " | ".join("%s %.6e" % (names[i], g[i]) for i in (0, 1, 2, 3, 4, 5, 6, 7, 9, 10, 11)) + " |")
+        for idx, rel in ((9, 1e-3), (3, 1e-3)):
+            mp, mm = mat.clone(), mat.clone()
+            hstep = rel * float(mat[idx])
+            mp[idx] += hstep; mm[idx] -= hstep
+            fd = (forward(mp, False)[0] - forward(mm, False)[0]) / (2 * hstep)
+            print("| central difference d J / d %s (Eq.(52), h = %.0e theta) | %.6e | adjoint %.6e | relative difference %.2e |"
+                  % (names[idx], rel, fd, g[idx], abs(fd - g[idx]) / abs(fd)), flush=True)
 
     # ---- 5. the whole benchmark loading with the paper's adaptive stepping parameters (host control flow)
     if args.full > 0:

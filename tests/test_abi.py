@@ -56,6 +56,8 @@ def test_null_and_argument_errors_without_device_work():
     assert (no.rtol, no.atol, no.max_newton, no.lin_rtol, no.lin_max_iter, no.linear_solver) == (1e-9, 1e-10, 25, 1e-10, 10000, 0)
     assert L.fem_pcg(None, None, None, None, 1e-8, 10, None, None, None) == -1
     assert L.fem_lincomb(None, 1.0, None, 1.0, None, None, None) == -1
+    assert L.fem_assemble_vjp(None, None, None, None, 1, None, None, None, None, None, None) == -1
+    assert L.fem_adjoint_step(None, None, None, None, 1, 0, None, None, None, None, None, None, 1e-8, 10, None, None) == -1
 
 
 def test_lankford_helper_matches_closed_form():
