@@ -20,7 +20,8 @@ dC/dF, d eps/dC = P_L/2, the return map by App. D (Eq.(D4)-(D7) :
 paper's 8 unknowns y = [T, alpha, dgam], G of Eq.(19)-(24) :176-196), dS = P_L:dT + (T:L_L):dC/2 (Eq.(25) :204), dP = dF S + F dS
 (Eq.(26) :208), and multiplies its transpose with the cotangent.  theta = (E, nu, r11, r22, r33, r12, r23, r13, h0, h1, h2)
 (Tables 3/5: the identified parameters are Hill ratios and hardening constants); the orientation quaternion and the
-law switch are not differentiated (their gradient entries are 0).  Standard element only (fbar = 0), Hill-48 only.
+law switch are not differentiated (their gradient entries are 0).  Hill-48 only; standard element and F-bar (fbar = 1: the
+relative-volume coupling of the 8 Gauss points, Eq.(31)-(32) :237-243, is differentiated at element level in `element_vjp`).
 
 Pins (tests/test_oracle_sens.py, -m "not gpu"): central differences of lambda.R + mu.hist_out computed with the C oracle's
 assemble (the paper's own check, Eq.(52)); g_u_full(lambda, 0) = K lambda with the oracle's assembled K; elastic closed
@@ -195,26 +196,49 @@ def point_jacobian(mat, F, hin):
     return J, rm
 
 
-def element_vjp(X, u, hin, mat, lam_e, mu_e):
+def element_vjp(X, u, hin, mat, lam_e, mu_e, fbar=0):
     """VJPs of one element: X[8,3], u[8,3], hin[8,7], lam_e[8,3], mu_e[8,7] ->
-    g_u[8,3] (history leg only), g_u_full[8,3], g_hist[8,7], g_theta[11]."""
+    g_u[8,3] (history leg only), g_u_full[8,3], g_hist[8,7], g_theta[11].
+    fbar = 1 (Eq.(31)-(32) PAPER.md:237-243, reading G12: R^e contracts P(Fbar) with grad_0 N): the point map is evaluated at
+    Fbar_q = c_q F_q, c_q = (Jbar/J_q)^(1/3), Jbar = sum_p w_p J_p / V, and the cotangent on Fbar_q is taken back to the F_p by
+    dFbar_q = c_q dF_q + F_q c_q/3 (dJbar/Jbar - dJ_q/J_q), dJ_p = J_p F_p^-T : dF_p."""
     X, u, hin = np.asarray(X, dtype=np.float64), np.asarray(u, dtype=np.float64), np.asarray(hin, dtype=np.float64)
     g_u, g_uf, g_h, g_t = np.zeros((8, 3)), np.zeros((8, 3)), np.zeros((8, 7)), np.zeros(NTH)
+    Gs, ws, Fs = [], [], []
     for q in range(8):
         G, w = shape_grad(X, q)
-        F = np.eye(3) + u.T @ G                                      # Eq.(30) :228
-        J, _ = point_jacobian(mat, F, hin[q])
-        Pbar = w * (lam_e.T @ G)                                     # R^e_Ii = sum_q w P_iJ G_IJ (Eq.(35) :257)
+        Gs.append(G); ws.append(w); Fs.append(np.eye(3) + u.T @ G)                # Eq.(30) :228
+    if fbar:
+        V = sum(ws)
+        Js = [np.linalg.det(F) for F in Fs]
+        Jbar = sum(w * J for w, J in zip(ws, Js)) / V                          # Eq.(31) :237
+        cs = [(Jbar / J) ** (1.0 / 3.0) for J in Js]                              # Eq.(32) :243
+    else:
+        cs = [1.0] * 8
+    gFb_full, gFb_hist = [], []
+    for q in range(8):
+        J, _ = point_jacobian(mat, cs[q] * Fs[q], hin[q])
+        Pbar = ws[q] * (lam_e.T @ Gs[q])                                          # R^e_Ii = sum_q w P_iJ G_IJ (Eq.(35) :257)
         cot = np.concatenate([Pbar.ravel(), mu_e[q]])
         g = J.T @ cot
-        g_uf += (g[0:9].reshape(3, 3) @ G.T).T
-        g_u += ((J[9:, 0:9].T @ mu_e[q]).reshape(3, 3) @ G.T).T
+        gFb_full.append(g[0:9].reshape(3, 3))
+        gFb_hist.append((J[9:, 0:9].T @ mu_e[q]).reshape(3, 3))
         g_h[q] = g[9:16]
         g_t += g[16:]
+    for gFb, out in ((gFb_full, g_uf), (gFb_hist, g_u)):
+        if fbar:
+            s = [cs[q] / 3.0 * float(np.sum(gFb[q] * Fs[q])) for q in range(8)]
+            S = sum(s)
+        for q in range(8):
+            gF = cs[q] * gFb[q]
+            if fbar:
+                FiT = np.linalg.inv(Fs[q]).T
+                gF = gF - s[q] * FiT + (S / Jbar) * (ws[q] * Js[q] / V) * FiT
+            out += (gF @ Gs[q].T).T
     return g_u, g_uf, g_h, g_t
 
 
-def assemble_vjp(coords, conn, u, hist_in, mat, lam, mu, elems=None):
+def assemble_vjp(coords, conn, u, hist_in, mat, lam, mu, elems=None, fbar=0):
     """Mesh level, elements in ascending id.  mat [n_mat,16] (n_mat = 1 or n_elems).  Returns dict with g_u, g_u_full [n_nodes,3],
     g_hist_in [n_elems,8,7], g_mat [n_mat,16] and g_mat_abs (sum of |element contributions|, the scale a tolerance refers to).
     `elems` restricts the work to a subset of elements (the other entries stay 0)."""
@@ -231,7 +255,7 @@ def assemble_vjp(coords, conn, u, hist_in, mat, lam, mu, elems=None):
     for e in (range(ne) if elems is None else elems):
         c = conn[e].astype(np.int64)
         m = 0 if mat.shape[0] == 1 else e
-        a, b, g_h[e], t = element_vjp(coords[c], u[c], hist_in[e], mat[m], lam[c], mu[e])
+        a, b, g_h[e], t = element_vjp(coords[c], u[c], hist_in[e], mat[m], lam[c], mu[e], fbar=fbar)
         for I in range(8):
             g_u[c[I]] += a[I]
             g_uf[c[I]] += b[I]

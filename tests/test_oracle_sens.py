@@ -163,3 +163,41 @@ def test_adjoint_gradient_against_central_differences():
     idx = list(osn.THETA_IDX)
     fd = _fd(J, mat, idx, lambda x: 1e-5 * abs(x))
     assert np.allclose(grad[idx], fd, rtol=2e-4, atol=1e-6 * np.abs(fd).max())
+
+
+def test_fbar_vjp_against_central_differences_and_transposed_tangent():
+    """F-bar element (Eq.(31)-(32) PAPER.md:237-243, reading G12): the element-level coupling through Jbar is part of the VJP.
+    Pins: central differences of the C oracle's F-bar assemble (Eq.(52) :412) in u, hist_in and theta, and g_u_full(lambda, 0) =
+    K^T lambda with the oracle's assembled F-bar tangent — which is unsymmetric, so K lambda must NOT match (a transposed
+    operand fails here)."""
+    p = _problem(seed=5)
+
+    def psi(u=None, h=None, mat=None):
+        out = oracle.assemble(p["coords"], p["conn"], p["u"] if u is None else u, p["h"] if h is None else h,
+                              p["mat"] if mat is None else mat, p["rp"], p["ci"], fbar=1)
+        return float(np.dot(out["residual"], p["lam"].ravel()) + np.dot(out["hist_out"].ravel(), p["mu"].ravel())), out
+    _, out = psi()
+    assert 8 < out["stats"]["n_plastic"] < 8 * p["conn"].shape[0] - 8
+    v = osn.assemble_vjp(p["coords"], p["conn"], p["u"], p["h"], p["mat"], p["lam"], p["mu"], fbar=1)
+    rng = np.random.default_rng(1)
+    idx = rng.choice(p["u"].size, 16, replace=False)
+    g = _fd(lambda x: psi(u=x)[0], p["u"], idx, lambda x: 1e-7)
+    assert np.allclose(v["g_u_full"].ravel()[idx], g, rtol=2e-6, atol=1e-6 * np.abs(g).max())
+    idx = rng.choice(p["h"].size, 24, replace=False)
+    g = _fd(lambda x: psi(h=x)[0], p["h"], idx, lambda x: 1e-7)
+    assert np.allclose(v["g_hist_in"].ravel()[idx], g, rtol=2e-6, atol=1e-6 * np.abs(g).max())
+    idx = list(osn.THETA_IDX)
+    g = _fd(lambda x: psi(mat=x)[0], p["mat"], idx, lambda x: 1e-6 * abs(x))
+    assert np.allclose(v["g_mat"].ravel()[idx], g, rtol=5e-6, atol=1e-7 * v["g_mat_abs"].ravel()[idx].max())
+    a = osn.assemble_vjp(p["coords"], p["conn"], p["u"], p["h"], p["mat"], p["lam"], None, fbar=1)
+    K = onw.csr(p["rp"], p["ci"], out["csr_vals"])
+    Ktl, Kl = K.T @ p["lam"].ravel(), K @ p["lam"].ravel()
+    assert np.allclose(a["g_u_full"].ravel(), Ktl, rtol=1e-10, atol=1e-10 * np.abs(Ktl).max())
+    assert np.abs(a["g_u_full"].ravel() - Kl).max() > 1e-5 * np.abs(Kl).max()
+    # the standard element is the fbar = 0 branch of the same function; on an affine field both coincide (J_q = Jbar)
+    A = np.array([[0.004, 0.001, 0.0], [0.0, -0.003, 0.002], [0.001, 0.0, 0.002]])
+    ua = p["coords"] @ A.T
+    s0 = osn.assemble_vjp(p["coords"], p["conn"], ua, p["h"] * 0, p["mat"], p["lam"], p["mu"], fbar=0)
+    s1 = osn.assemble_vjp(p["coords"], p["conn"], ua, p["h"] * 0, p["mat"], p["lam"], p["mu"], fbar=1)
+    assert np.allclose(s0["g_hist_in"], s1["g_hist_in"], rtol=1e-9, atol=1e-9 * np.abs(s0["g_hist_in"]).max())
+    assert np.allclose(s0["g_mat"], s1["g_mat"], rtol=1e-9, atol=1e-9 * np.abs(s0["g_mat_abs"]).max())
