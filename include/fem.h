@@ -251,8 +251,9 @@ int fem_newton_solve(fem_ctx *c, double *u, const double *hist_in, const double 
  *                                  sum over all elements; n_mat = n_elems: one record per element.
  * Any of the three outputs may be NULL (not computed).  u, hist_in, mat, n_mat as in fem_assemble; the state is
  * re-evaluated inside the call (nothing is kept from fem_assemble), the return map is differentiated implicitly at its
- * root (App. D Eq.(D4)-(D7) :1002-1019, transposed).  Hill-48 and the standard element only: FEM_ERR_ARG for fbar = 1 or
- * assembly_mode 1.  Sums run in a fixed order, no atomics: equal inputs give bit-identical outputs.  Uses the library's
+ * root (App. D Eq.(D4)-(D7) :1002-1019, transposed).  Hill-48 only; both element formulations: with fbar = 1 the
+ * coupling of an element's 8 Gauss points through Jbar (Eq.(31)-(32) :237-243) is part of the product, and K^T differs
+ * from K.  FEM_ERR_ARG when g_u is wanted in assembly_mode 1 (no scratch).  Sums run in a fixed order, no atomics: equal inputs give bit-identical outputs.  Uses the library's
  * R^e scratch: do not run concurrently with fem_assemble on another stream.  Asynchronous on `cuda_stream`. */
 int fem_assemble_vjp(fem_ctx *c, const double *u, const double *hist_in, const double *mat, long long n_mat,
                      const double *lam, const double *mu, double *g_u, double *g_hist_in, double *g_mat, void *cuda_stream);

@@ -176,6 +176,7 @@ __device__ __forceinline__ double g_dd2(double x0, double x1, double x2, double 
     return close ? 0.5 * im * im * ser : rec;
 }
 
+template <int FBAR>
 __global__ void __launch_bounds__(STHREADS, SENS_CTAS)
 k_sens_point(long long n_elems, const double *__restrict__ coords, const int *__restrict__ conn, const int *__restrict__ eslot,
              const double *__restrict__ u, const double *__restrict__ hist_in, const double *__restrict__ mat, long long n_mat,
@@ -272,6 +273,22 @@ k_sens_point(long long n_elems, const double *__restrict__ coords, const int *__
                     F[i][0] = fma(ui, g[0], F[i][0]); F[i][1] = fma(ui, g[1], F[i][1]); F[i][2] = fma(ui, g[2], F[i][2]);
                 }
             }
+        }
+        // ---- F-bar (Eq.(31)-(32) :237-243, reading G12): Fbar = (Jbar/J)^(1/3) F, Jbar = sum_q w_q J_q / V over the element's 8 lanes
+        double fb_c = 1.0, fb_J = 1.0, fb_Jbar = 1.0, fb_wJV = 0.0;
+        if (FBAR) {
+            fb_J = F[0][0] * (F[1][1] * F[2][2] - F[1][2] * F[2][1]) - F[0][1] * (F[1][0] * F[2][2] - F[1][2] * F[2][0]) +
+                   F[0][2] * (F[1][0] * F[2][1] - F[1][1] * F[2][0]);
+            double V = wq, SJ = wq * fb_J;
+#pragma unroll
+            for (int o = 1; o < 8; o <<= 1) { V += __shfl_xor_sync(0xffffffffu, V, o); SJ += __shfl_xor_sync(0xffffffffu, SJ, o); }
+            fb_Jbar = SJ / V;
+            fb_wJV = wq * fb_J / V;
+            fb_c = cbrt(fb_Jbar / fb_J);
+#pragma unroll
+            for (int i = 0; i < 3; i++)
+#pragma unroll
+                for (int j = 0; j < 3; j++) F[i][j] *= fb_c;
         }
         SENS_SYNC(5);
         // ---- C' = F'^T F', cyclic Jacobi (5 sweeps), Hencky strain in the material frame (Eq.(4)-(5) :92-96, reading G1)
@@ -535,6 +552,28 @@ k_sens_point(long long n_elems, const double *__restrict__ coords, const int *__
             for (int i = 0; i < 3; i++)
 #pragma unroll
                 for (int j = 0; j < 3; j++) Fb[i][j] += 2.0 * (F[i][0] * Cb33[0][j] + F[i][1] * Cb33[1][j] + F[i][2] * Cb33[2][j]);
+            if (FBAR) {
+                // dFbar_q = c_q dF_q + F_q c_q/3 (dJbar/Jbar - dJ_q/J_q), dJ_p = J_p F_p^-T : dF_p  =>
+                // Fb <- c_q Fb + F_q^-T ( (S/Jbar) w_q J_q / V - s_q ),  s_q = (Fb : Fbar_q)/3,  S = sum_q s_q,  F_q^-T = cof(Fbar_q)/(c_q^2 J_q)
+                double sq = 0.0;
+#pragma unroll
+                for (int i = 0; i < 3; i++)
+#pragma unroll
+                    for (int j = 0; j < 3; j++) sq += Fb[i][j] * F[i][j];
+                sq *= (1.0 / 3.0);
+                double S = sq;
+#pragma unroll
+                for (int o = 1; o < 8; o <<= 1) S += __shfl_xor_sync(0xffffffffu, S, o);
+                const double k = (S / fb_Jbar * fb_wJV - sq) / (fb_c * fb_c * fb_J);
+                double cof[3][3];
+                cof[0][0] = F[1][1] * F[2][2] - F[1][2] * F[2][1]; cof[0][1] = F[1][2] * F[2][0] - F[1][0] * F[2][2]; cof[0][2] = F[1][0] * F[2][1] - F[1][1] * F[2][0];
+                cof[1][0] = F[0][2] * F[2][1] - F[0][1] * F[2][2]; cof[1][1] = F[0][0] * F[2][2] - F[0][2] * F[2][0]; cof[1][2] = F[0][1] * F[2][0] - F[0][0] * F[2][1];
+                cof[2][0] = F[0][1] * F[1][2] - F[0][2] * F[1][1]; cof[2][1] = F[0][2] * F[1][0] - F[0][0] * F[1][2]; cof[2][2] = F[0][0] * F[1][1] - F[0][1] * F[1][0];
+#pragma unroll
+                for (int i = 0; i < 3; i++)
+#pragma unroll
+                    for (int j = 0; j < 3; j++) Fb[i][j] = fb_c * Fb[i][j] + k * cof[i][j];
+            }
 #pragma unroll
             for (int I = 0; I < 8; I++) {
                 const double g0 = Gs[3 * I], g1_ = Gs[3 * I + 1], g2_ = Gs[3 * I + 2];
@@ -612,7 +651,6 @@ extern "C" int fem_assemble_vjp(fem_ctx *c, const double *u, const double *hist_
     if (!c || !u || !hist_in || !mat) return FEM_ERR_NULL;
     if (!c->has_pattern) return FEM_ERR_NO_PATTERN;
     if (n_mat != 1 && n_mat != c->n_elems) return FEM_ERR_MAT;
-    if (c->opt.fbar != 0) return FEM_ERR_ARG;
     if (g_u && (!c->d_eslot || !c->d_Re)) return FEM_ERR_ARG;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const long long ne = c->n_elems;
@@ -632,7 +670,11 @@ extern "C" int fem_assemble_vjp(fem_ctx *c, const double *u, const double *hist_
         }
         part = c->d_sens_part;
     }
-    k_sens_point<<<(unsigned)nblk, STHREADS, 0, st>>>(ne, c->d_coords, c->d_conn, c->d_eslot, u, hist_in, mat, n_mat, lam, mu,
+    if (c->opt.fbar)
+        k_sens_point<1><<<(unsigned)nblk, STHREADS, 0, st>>>(ne, c->d_coords, c->d_conn, c->d_eslot, u, hist_in, mat, n_mat, lam, mu,
+                                                      g_u ? c->d_Re : nullptr, g_hist_in, (g_mat && n_mat != 1) ? g_mat : nullptr, part);
+    else
+        k_sens_point<0><<<(unsigned)nblk, STHREADS, 0, st>>>(ne, c->d_coords, c->d_conn, c->d_eslot, u, hist_in, mat, n_mat, lam, mu,
                                                       g_u ? c->d_Re : nullptr, g_hist_in, (g_mat && n_mat != 1) ? g_mat : nullptr, part);
     FEM_CUDA(cudaGetLastError());
     if (g_u) {

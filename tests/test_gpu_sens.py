@@ -163,8 +163,9 @@ def test_vjp_errors_and_edge_cases():
     ctx.close()
     ctx = fem.FemContext(torch.from_numpy(p["coords"]).to(dev), torch.from_numpy(p["conn"]).to(dev), fbar=1)
     ctx.build_csr_pattern()
-    with pytest.raises(fem.FemError):      # F-bar is not differentiated
-        _gpu_vjp(ctx, p)
+    with pytest.raises(fem.FemError):      # the adjoint step needs K^T products for the unsymmetric F-bar tangent: not built
+        t = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64).ravel()).to(dev)
+        ctx.adjoint_step(t(p["u"]), t(p["h"]), t(p["mat"]), torch.zeros(3, dtype=torch.int32, device=dev))
     ctx.close()
     # zero cotangents give zero gradients; zero displacement and virgin history (repeated eigenvalues of C, all elastic)
     ctx = _ctx(p["coords"], p["conn"])
@@ -369,3 +370,69 @@ def test_vjp_config4_and_config5_samples():
         o2 = osn.assemble_vjp(cfg["coords"], cfg["conn"], cfg["u"], cfg["hist_in"], omat, lam_n, mu_n, elems=els)
         assert rel_l2(c_u.cpu().numpy().reshape(nn, 3)[nodes], o2["g_u_full"][nodes]) <= TOL, label
         ctx.close()
+
+
+def _ctx_fbar(coords, conn):
+    import torch
+    import paper_2606_17390_b200 as fem
+    dev = torch.device("cuda:0")
+    ctx = fem.FemContext(torch.from_numpy(np.ascontiguousarray(coords)).to(dev), torch.from_numpy(np.ascontiguousarray(conn)).to(dev), fbar=1)
+    rp, ci, _ = ctx.build_csr_pattern()
+    return ctx, rp.cpu().numpy(), ci.cpu().numpy()
+
+
+@pytest.mark.parametrize("variant", ["uniform_swift", "per_elem_rotated_voce", "large_strain"])
+def test_vjp_fbar_small_meshes(variant):
+    """F-bar element (Eq.(31)-(32) PAPER.md:237-243): the 8 Gauss points of an element are coupled through Jbar."""
+    import oracle.sens as osn
+    p = _small_problem(per_elem=variant == "per_elem_rotated_voce", voce=variant == "per_elem_rotated_voce",
+                       amp=0.2 if variant == "large_strain" else 0.006, seed=31)
+    ctx, _, _ = _ctx_fbar(p["coords"], p["conn"])
+    o = osn.assemble_vjp(p["coords"], p["conn"], p["u"], p["h"], p["mat"], p["lam"], p["mu"], fbar=1)
+    g_u, g_h, g_m = _gpu_vjp(ctx, p)
+    assert rel_l2(g_u, o["g_u_full"]) <= TOL and rel_l2(g_h, o["g_hist_in"]) <= TOL
+    _check_mat(g_m, o)
+    g_u2, _, _ = _gpu_vjp(ctx, p, lam=False)
+    assert rel_l2(g_u2, o["g_u"]) <= TOL
+    # and it differs from the standard element (the coupling is not a no-op on this field)
+    o0 = osn.assemble_vjp(p["coords"], p["conn"], p["u"], p["h"], p["mat"], p["lam"], p["mu"], fbar=0)
+    assert rel_l2(g_u, o0["g_u_full"]) > 1e-6
+    ctx.close()
+
+
+def test_vjp_fbar_config2_transposed_tangent_and_samples():
+    """Config 2 with F-bar: g_u(lam, 0) = K^T lam with the library's own (unsymmetric) F-bar tangent — K lam must not match —
+    and sampled elements / nodes against the oracle."""
+    import torch
+    import scipy.sparse as sp
+    import oracle
+    import oracle.sens as osn
+    import synth
+    import paper_2606_17390_b200 as fem
+    cfg = synth.make_config(2)
+    ne, nn = cfg["conn"].shape[0], cfg["coords"].shape[0]
+    ctx, rp, ci = _ctx_fbar(cfg["coords"], cfg["conn"])
+    dev = ctx.device
+    rng = np.random.default_rng(41)
+    lam_n = rng.normal(size=(nn, 3)); mu_n = rng.normal(size=(ne, 8, 7)) * np.array([1e3] * 6 + [1e2])
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64).ravel()).to(dev)
+    u, h, lam, mu = t(cfg["u"]), t(cfg["hist_in"]), t(lam_n), t(mu_n)
+    mat = t(fem.mat_from_desc(cfg["matdesc"], ne))
+    _, vals, _, _ = ctx.assemble(u, h, mat)
+    a_u, _, _ = ctx.assemble_vjp(u, h, mat, lam, None, want_hist=False, want_mat=False)
+    K = sp.csr_matrix((vals.cpu().numpy(), ci, rp), shape=(3 * nn, 3 * nn))
+    Ktl, Kl = K.T @ lam_n.ravel(), K @ lam_n.ravel()
+    assert rel_l2(a_u.cpu().numpy(), Ktl) <= 1e-10
+    assert rel_l2(a_u.cpu().numpy(), Kl) > 1e-6
+    c_u, c_h, c_m = ctx.assemble_vjp(u, h, mat, lam, mu)
+    omat = oracle.mat_from_desc(cfg["matdesc"], ne)
+    el = np.sort(rng.choice(ne, 60, replace=False))
+    o = osn.assemble_vjp(cfg["coords"], cfg["conn"], cfg["u"], cfg["hist_in"], omat, lam_n, mu_n, elems=el, fbar=1)
+    assert rel_l2(c_h.cpu().numpy().reshape(ne, 8, 7)[el], o["g_hist_in"][el]) <= TOL
+    nodes = rng.choice(nn, 10, replace=False)
+    els = np.unique(np.flatnonzero(np.isin(cfg["conn"], nodes).any(axis=1)))
+    o2 = osn.assemble_vjp(cfg["coords"], cfg["conn"], cfg["u"], cfg["hist_in"], omat, lam_n, mu_n, elems=els, fbar=1)
+    assert rel_l2(c_u.cpu().numpy().reshape(nn, 3)[nodes], o2["g_u_full"][nodes]) <= TOL
+    d_u, d_h, d_m = ctx.assemble_vjp(u, h, mat, lam, mu)
+    assert torch.equal(c_u, d_u) and torch.equal(c_h, d_h) and torch.equal(c_m, d_m)
+    ctx.close()
