@@ -261,8 +261,9 @@ int fem_assemble_vjp(fem_ctx *c, const double *u, const double *hist_in, const d
 /* fem_adjoint_step — one step n of the backward sweep of Alg. 1, composed of the calls above:
  *   K = dR/du at (u^n, h^{n-1})                                   (fem_assemble; the tangent "assembled during the forward solve", :368)
  *   v = -[ dJdu + (dhist_out/du)^T mu_in ]                        (right-hand side of Eq.(51) :366; fem_assemble_vjp with lam = NULL)
- *   K^T lam = v on the free DOFs, lam = 0 on bc_dofs              (fem_pcg on the row-eliminated K — K_ff is symmetric for the
- *                                                                  standard element — falling back to fem_bicgstab)
+ *   K^T lam = v on the free DOFs, lam = 0 on bc_dofs              (standard element: K_ff is symmetric, fem_pcg on the row-eliminated K,
+ *                                                                  falling back to fem_bicgstab; F-bar: K^T is formed on the same
+ *                                                                  pattern (one more nnz-sized workspace) and solved by fem_bicgstab)
  *   mu_out = g_hist_in(lam, mu_in),  g_mat = (dR/dmat)^T lam + (dhist_out/dmat)^T mu_in      (Eq.(49) :355; fem_assemble_vjp)
  *   u        dev [n_rows]       converged displacement u^n of the step
  *   hist_in  dev [n_elems*56]   history h^{n-1} at the start of the step
@@ -271,7 +272,7 @@ int fem_assemble_vjp(fem_ctx *c, const double *u, const double *hist_in, const d
  *   lam      dev [n_rows] out   adjoint vector of the step
  *   mu_out   dev [n_elems*56] out  cotangent on h^{n-1} for step n-1 (must not alias hist_in or mu_in; also used as scratch)
  *   g_mat    dev [n_mat*16] out this step's term of dJ/dtheta (overwritten; the caller accumulates over the steps and adds dJ^n/dtheta)
- * Returns FEM_OK, FEM_ERR_NOCONV when the adjoint solve did not reach lin_rtol (outputs undefined), FEM_ERR_ARG for fbar = 1.
+ * Returns FEM_OK, or FEM_ERR_NOCONV when the adjoint solve did not reach lin_rtol (outputs undefined).
  * *lin_iters (host, may be NULL) = Krylov iterations used.  Synchronises the stream. */
 int fem_adjoint_step(fem_ctx *c, const double *u, const double *hist_in, const double *mat, long long n_mat, long long n_bc,
                      const int *bc_dofs, const double *dJdu, const double *mu_in, double *lam, double *mu_out, double *g_mat,

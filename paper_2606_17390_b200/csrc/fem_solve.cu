@@ -652,6 +652,26 @@ extern "C" int fem_newton_solve(fem_ctx *c, double *u, const double *hist_in, co
 // One step of the backward sweep of Alg. 1: right-hand side of Eq.(51) :366, adjoint solve on the tangent
 // of the converged state (K_ff is symmetric for the standard element, so the row-eliminated K serves for K^T with lam = 0 on the
 // constrained DOFs), then the products of Eq.(49) :355 and the history cotangent for the step before (reading G17).
+// K^T on the same (structurally symmetric) pattern: one thread per 3x3 node-pair block (n, m); the position of n in the sorted
+// neighbour list of m by binary search.  CSR row 3n+i starts at 9 nb_ptr[n] + 3 i len_n, block column pos at + 3 pos.
+__global__ void k_transpose_vals(long long n_nodes, const int *__restrict__ nb_ptr, const int *__restrict__ nb,
+                                 const double *__restrict__ vals, double *__restrict__ valsT) {
+    const long long n = blockIdx.x * (long long)(blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (n >= n_nodes) return;
+    const int lane = threadIdx.x & 31, o = nb_ptr[n], len = nb_ptr[n + 1] - o;
+    for (int pos = lane; pos < len; pos += 32) {
+        const int m = nb[o + pos], om = nb_ptr[m], lm = nb_ptr[m + 1] - om;
+        int lo = 0, hi = lm - 1;
+        while (lo < hi) { const int mid = (lo + hi) >> 1; if (nb[om + mid] < (int)n) lo = mid + 1; else hi = mid; }
+        const double *src = vals + 9LL * om + 3 * lo;     // block (m, n): entry (k, i) at src[k * 3 * lm + i]
+        double *dst = valsT + 9LL * o + 3 * pos;          // block (n, m) of K^T: entry (i, k) = K[(m,k)][(n,i)]
+#pragma unroll
+        for (int i = 0; i < 3; i++)
+#pragma unroll
+            for (int k = 0; k < 3; k++) dst[(long long)i * 3 * len + k] = src[(long long)k * 3 * lm + i];
+    }
+}
+
 __global__ void k_adj_rhs(long long n, const double *__restrict__ dJdu, const double *__restrict__ gu, double *__restrict__ rhs) {
     for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x)
         rhs[i] = -((dJdu ? dJdu[i] : 0.0) + (gu ? gu[i] : 0.0));
@@ -664,7 +684,7 @@ extern "C" int fem_adjoint_step(fem_ctx *c, const double *u, const double *hist_
     if (!c || !u || !hist_in || !mat || !lam || !mu_out || !g_mat || (n_bc > 0 && !bc_dofs)) return FEM_ERR_NULL;
     if (!c->has_pattern) return FEM_ERR_NO_PATTERN;
     if (n_mat != 1 && n_mat != c->n_elems) return FEM_ERR_MAT;
-    if (n_bc < 0 || c->opt.fbar != 0 || !(lin_rtol > 0.0) || lin_max_iter < 1) return FEM_ERR_ARG;
+    if (n_bc < 0 || !(lin_rtol > 0.0) || lin_max_iter < 1) return FEM_ERR_ARG;
     if (mu_out == hist_in || mu_out == mu_in) return FEM_ERR_ALIAS;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     int rc = ensure_solver_ws(c, true);
@@ -678,11 +698,17 @@ extern "C" int fem_adjoint_step(fem_ctx *c, const double *u, const double *hist_
         if ((rc = fem_assemble_vjp(c, u, hist_in, mat, n_mat, nullptr, mu_in, gu, nullptr, nullptr, cuda_stream)) != FEM_OK) return rc;
     }
     k_adj_rhs<<<RED_CTAS, RED_THREADS, 0, st>>>(n, dJdu, mu_in ? gu : nullptr, rhs);
+    if (c->opt.fbar) {   // unsymmetric tangent: the adjoint system needs K^T explicitly
+        if (!c->d_nw_valsT) FEM_CUDA(cudaMalloc(&c->d_nw_valsT, sizeof(double) * (size_t)c->nnz));
+        k_transpose_vals<<<nblk3(c->n_nodes, 8), 256, 0, st>>>(c->n_nodes, c->d_nb_ptr, c->d_nb, vals, c->d_nw_valsT);
+        FEM_CUDA(cudaGetLastError());
+        vals = c->d_nw_valsT;
+    }
     if ((rc = apply_dirichlet(c, n_bc, bc_dofs, nullptr, nullptr, nullptr, vals, rhs, st)) != FEM_OK) return rc;
     FEM_CUDA(cudaMemsetAsync(lam, 0, sizeof(double) * n, st));
     int its = 0, its2 = 0;
-    rc = pcg(c, vals, rhs, lam, lin_rtol, lin_max_iter, &its, nullptr, st);
-    if (rc == FEM_ERR_NOCONV) {   // K_ff not positive definite at this state: BiCGSTAB from zero (K_ff is still symmetric)
+    rc = c->opt.fbar ? FEM_ERR_NOCONV : pcg(c, vals, rhs, lam, lin_rtol, lin_max_iter, &its, nullptr, st);
+    if (rc == FEM_ERR_NOCONV) {   // F-bar, or K_ff not positive definite at this state: BiCGSTAB from zero
         FEM_CUDA(cudaMemsetAsync(lam, 0, sizeof(double) * n, st));
         rc = bicgstab(c, vals, rhs, lam, lin_rtol, lin_max_iter, &its2, nullptr, st);
     }

@@ -161,11 +161,10 @@ def test_vjp_errors_and_edge_cases():
     with pytest.raises(fem.FemError):      # no pattern yet
         _gpu_vjp(ctx, p)
     ctx.close()
-    ctx = fem.FemContext(torch.from_numpy(p["coords"]).to(dev), torch.from_numpy(p["conn"]).to(dev), fbar=1)
-    ctx.build_csr_pattern()
-    with pytest.raises(fem.FemError):      # the adjoint step needs K^T products for the unsymmetric F-bar tangent: not built
+    ctx = _ctx(p["coords"], p["conn"])
+    with pytest.raises(fem.FemError):      # constrained DOF out of range
         t = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64).ravel()).to(dev)
-        ctx.adjoint_step(t(p["u"]), t(p["h"]), t(p["mat"]), torch.zeros(3, dtype=torch.int32, device=dev))
+        ctx.adjoint_step(t(p["u"]), t(p["h"]), t(p["mat"]), torch.full((3,), 10 ** 6, dtype=torch.int32, device=dev))
     ctx.close()
     # zero cotangents give zero gradients; zero displacement and virgin history (repeated eigenvalues of C, all elastic)
     ctx = _ctx(p["coords"], p["conn"])
@@ -237,7 +236,8 @@ def test_vjp_full_size_properties_and_samples():
     ctx.close()
 
 
-def test_adjoint_gradient_of_load_path_matches_oracle():
+@pytest.mark.parametrize("fbar", [0, 1])
+def test_adjoint_gradient_of_load_path_matches_oracle(fbar):
     """Alg. 1 end to end on the GPU: two load increments with fem_newton_solve, then backwards per step
     Eq.(51) K^T lam = -(dJ/du)^T - (dh/du)^T mu by fem_pcg on the row-eliminated tangent, Eq.(49) by fem_assemble_vjp with the
     history cotangent carried from step to step (reading G17), J = sum_n |u^n - u_gt^n|^2.  Expected values: the same loop
@@ -267,24 +267,24 @@ def test_adjoint_gradient_of_load_path_matches_oracle():
     rp, ci, _ = oracle.pattern(nn, conn, with_slots=False)
     uo, ho, states = np.zeros_like(coords), np.zeros((ne, 8, 7)), []
     for t in targets:
-        r = onw.newton_solve(coords, conn, uo, ho, mat, rp, ci, bc, t, rtol=1e-13, atol=1e-9)
+        r = onw.newton_solve(coords, conn, uo, ho, mat, rp, ci, bc, t, rtol=1e-13, atol=1e-9, fbar=fbar)
         assert r["converged"]
         states.append((r["u"].copy(), ho.copy()))
         uo, ho = r["u"], r["hist_out"]
     grad_o, mu_o = np.zeros(16), None
     for (u, h), g in zip(reversed(states), reversed(ugt)):
-        out = oracle.assemble(coords, conn, u, h, mat, rp, ci)
+        out = oracle.assemble(coords, conn, u, h, mat, rp, ci, fbar=fbar)
         rhs = -2.0 * (u - g).ravel()
         if mu_o is not None:
-            rhs -= osn.assemble_vjp(coords, conn, u, h, mat, None, mu_o)["g_u"].ravel()
+            rhs -= osn.assemble_vjp(coords, conn, u, h, mat, None, mu_o, fbar=fbar)["g_u"].ravel()
         K = onw.csr(rp, ci, out["csr_vals"]).toarray()
         lam = np.zeros(3 * nn)
         lam[free] = np.linalg.solve(K[np.ix_(free, free)].T, rhs[free])
-        v = osn.assemble_vjp(coords, conn, u, h, mat, lam, mu_o)
+        v = osn.assemble_vjp(coords, conn, u, h, mat, lam, mu_o, fbar=fbar)
         grad_o += v["g_mat"][0]
         mu_o = v["g_hist_in"]
     # ---- GPU side
-    ctx = _ctx(coords, conn)
+    ctx = _ctx_fbar(coords, conn)[0] if fbar else _ctx(coords, conn)
     dev = ctx.device
     t64 = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64).ravel()).to(dev)
     mat_d, bc_d = t64(mat), torch.from_numpy(bc.astype(np.int32)).to(dev)
@@ -296,22 +296,24 @@ def test_adjoint_gradient_of_load_path_matches_oracle():
         assert rep["converged"]
         gstates.append((u_d.clone(), h_d))
         h_d = h_new
-    grad_g, mu_d = torch.zeros(16, dtype=torch.float64, device=dev), None
-    for (u, h), g in zip(reversed(gstates), reversed(ugt)):
-        _, vals, _, _ = ctx.assemble(u, h, mat_d)
-        rhs = -2.0 * (u - t64(g))
-        if mu_d is not None:
-            rhs = rhs - ctx.assemble_vjp(u, h, mat_d, None, mu_d, want_hist=False, want_mat=False)[0]
-        ctx.apply_dirichlet(bc_d, vals, rhs)                         # identity rows, lam = 0 on the constrained DOFs
-        lam, _, _, ok = ctx.pcg(vals, rhs, rtol=1e-13, max_iter=5000)
-        assert ok
-        _, mu_new, g_m = ctx.assemble_vjp(u, h, mat_d, lam, mu_d, want_u=False)
-        grad_g += g_m[0]
-        mu_d = mu_new
-    gg = grad_g.cpu().numpy()
     idx = list(osn.THETA_IDX)
-    assert np.max(np.abs(gg[idx] - grad_o[idx]) / np.maximum(np.abs(grad_o[idx]), 1e-6 * np.abs(grad_o[idx]).max())) <= 1e-6
-    assert rel_l2(mu_d.cpu().numpy(), mu_o) <= 1e-6
+    gg = None
+    if not fbar:      # composed from the single calls (CG on the symmetric reduced tangent)
+        grad_g, mu_d = torch.zeros(16, dtype=torch.float64, device=dev), None
+        for (u, h), g in zip(reversed(gstates), reversed(ugt)):
+            _, vals, _, _ = ctx.assemble(u, h, mat_d)
+            rhs = -2.0 * (u - t64(g))
+            if mu_d is not None:
+                rhs = rhs - ctx.assemble_vjp(u, h, mat_d, None, mu_d, want_hist=False, want_mat=False)[0]
+            ctx.apply_dirichlet(bc_d, vals, rhs)                         # identity rows, lam = 0 on the constrained DOFs
+            lam, _, _, ok = ctx.pcg(vals, rhs, rtol=1e-13, max_iter=5000)
+            assert ok
+            _, mu_new, g_m = ctx.assemble_vjp(u, h, mat_d, lam, mu_d, want_u=False)
+            grad_g += g_m[0]
+            mu_d = mu_new
+        gg = grad_g.cpu().numpy()
+        assert np.max(np.abs(gg[idx] - grad_o[idx]) / np.maximum(np.abs(grad_o[idx]), 1e-6 * np.abs(grad_o[idx]).max())) <= 1e-6
+        assert rel_l2(mu_d.cpu().numpy(), mu_o) <= 1e-6
     # the same backward sweep through fem_adjoint_step (one C-ABI call per load step)
     grad_s, mu_s = torch.zeros(16, dtype=torch.float64, device=dev), None
     for (u, h), g in zip(reversed(gstates), reversed(ugt)):
@@ -319,7 +321,8 @@ def test_adjoint_gradient_of_load_path_matches_oracle():
         assert its > 0 and float(torch.abs(lam_s[bc_d.long()]).max()) == 0.0
         grad_s += g_m[0]
     gs = grad_s.cpu().numpy()
-    assert np.max(np.abs(gs[idx] - gg[idx]) / np.maximum(np.abs(gg[idx]), 1e-6 * np.abs(gg[idx]).max())) <= 1e-9
+    if gg is not None:
+        assert np.max(np.abs(gs[idx] - gg[idx]) / np.maximum(np.abs(gg[idx]), 1e-6 * np.abs(gg[idx]).max())) <= 1e-9
     assert np.max(np.abs(gs[idx] - grad_o[idx]) / np.maximum(np.abs(grad_o[idx]), 1e-6 * np.abs(grad_o[idx]).max())) <= 1e-6
     assert rel_l2(mu_s.cpu().numpy(), mu_o) <= 1e-6
     with pytest.raises(fem.FemError):      # mu_out must not alias hist_in: checked by the library
