@@ -26,6 +26,9 @@ relative-volume coupling of the 8 Gauss points, Eq.(31)-(32) :237-243, is differ
 Pins (tests/test_oracle_sens.py, -m "not gpu"): central differences of lambda.R + mu.hist_out computed with the C oracle's
 assemble (the paper's own check, Eq.(52)); g_u_full(lambda, 0) = K lambda with the oracle's assembled K; elastic closed
 forms dT/dE = T/E; the adjoint gradient of a two-step load path against central differences of J.
+The fbar = 1 branch inherits reading G12 of the forward path (literal Eq.(35): no external value pins that reading, 'parity
+unpinned' there); its derivative is pinned by central differences of the F-bar assemble and by K^T lambda with the assembled
+unsymmetric tangent.
 Shares nothing with the CUDA path; imports nothing from paper_2606_17390_b200.
 """
 import numpy as np

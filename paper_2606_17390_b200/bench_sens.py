@@ -15,14 +15,14 @@ import numpy as np
 sys.path.insert(0, os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
 
 
-def run_case(k, steps):
+def run_case(k, steps, fbar=0):
     import torch
     import synth
     import paper_2606_17390_b200 as fem
     dev = torch.device("cuda:0")
     cfg = synth.make_config(k)
     ne, nn = cfg["conn"].shape[0], cfg["coords"].shape[0]
-    ctx = fem.FemContext(torch.from_numpy(cfg["coords"]).to(dev), torch.from_numpy(cfg["conn"]).to(dev))
+    ctx = fem.FemContext(torch.from_numpy(cfg["coords"]).to(dev), torch.from_numpy(cfg["conn"]).to(dev), fbar=fbar)
     ctx.build_csr_pattern()
     u = torch.from_numpy(cfg["u"].ravel()).to(dev)
     hin = torch.from_numpy(cfg["hist_in"].ravel()).to(dev)
@@ -48,8 +48,8 @@ def run_case(k, steps):
     ms_hm = timed(lambda: ctx.assemble_vjp(u, hin, mat, lam, mu, want_u=False))
     # algorithmic bytes per element of the full call: conn 32, coords+u+lam 3*24*nn/ne, hist_in+mu+g_hist 3*448, scratch 2*192, g_u 24*nn/ne
     b_alg = ne * (32 + 3 * 448 + 2 * 192) + nn * 24 * 4 + mat.numel() * 8 + (mat.numel() if mat.numel() > 16 else 0) * 8
-    print("| %d | %d | %d | %.3f | %.3f | %.3f | %.3f | %.1f | %.0f |" % (
-        k, ne, 3 * nn, ms_asm, ms_all, ms_u, ms_hm, ne / ms_all * 1e-3, b_alg / ms_all * 1e-6))
+    print("| %s | %d | %d | %.3f | %.3f | %.3f | %.3f | %.1f | %.0f |" % (
+        ("%d, fbar=1" % k) if fbar else str(k), ne, 3 * nn, ms_asm, ms_all, ms_u, ms_hm, ne / ms_all * 1e-3, b_alg / ms_all * 1e-6))
     ctx.close()
 
 
@@ -57,11 +57,14 @@ def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--configs", default="2,3,4")
+    ap.add_argument("--fbar", type=int, default=0, help="1: also time the F-bar element on every config")
     a = ap.parse_args()
     print("| config | elements | DOF | fem_assemble ms | fem_assemble_vjp ms (g_u, g_hist_in, g_mat) | g_u only (lam = NULL) ms | g_hist_in + g_mat ms | M element-VJPs/s | algorithmic GB/s |")
     print("|---|---|---|---|---|---|---|---|---|")
     for k in a.configs.split(","):
         run_case(int(k), a.steps)
+        if a.fbar:
+            run_case(int(k), a.steps, fbar=1)
 
 
 if __name__ == "__main__":

@@ -135,7 +135,7 @@ def main():
           % (tot_newton, tot_lin, dt, dt / max(tot_newton, 1)))
 
     # ---- 4b. NEXT-3: the discrete adjoint of that path (Alg. 1) and the paper's own check of it (Eq.(52) :412)
-    if args.adjoint:
+    if args.adjoint and nsteps > 0:
         free = torch.ones(nr, dtype=torch.float64, device=dev)
         free[bc_d.long()] = 0.0
 
@@ -182,6 +182,7 @@ def main():
         h_a = torch.zeros(56 * ne, dtype=torch.float64, device=dev)
         h_b = torch.empty_like(h_a)
         steps = newton = lin = rejected = 0
+        ts = []                               # accepted load fractions (the schedule the adjoint run below repeats)
         u_try = torch.empty_like(u)
         u_prev = torch.zeros_like(u)          # converged states one and two steps back ("linear or quadratic extrapolation")
         u_pp = torch.zeros_like(u)
@@ -212,7 +213,7 @@ def main():
                                                                   st["n_plastic"] / (8.0 * ne), "ok" if ok else "rejected"), flush=True)
             newton += rep["newton_iters"]; lin += rep["lin_iters_total"]
             if ok:
-                t += dt; steps += 1
+                t += dt; steps += 1; ts.append(t)
                 h_a, h_b = h_b, h_a
                 u_pp, u_prev, u, u_try = u_prev, u, u_try, u_pp
                 dt_pp, dt_prev = dt_prev, dt
@@ -226,6 +227,56 @@ def main():
         tot = time.perf_counter() - t_start
         print("| total | reached %.4f of the load | | %d (incl. rejected steps) | %d | %.1f | | %d steps accepted, %d rejected |"
               % (t, newton, lin, tot, steps, rejected))
+
+        # ---- 5b. NEXT-3 on the whole benchmark: forward over the accepted schedule with the states kept, backward sweep of Alg. 1,
+        #          and the paper's check (Eq.(52) :412) of dJ/d(sigma0) by two more forward runs over the same schedule
+        if args.adjoint and t >= 1.0 - 1e-12:
+            free = torch.ones(nr, dtype=torch.float64, device=dev)
+            free[bc_d.long()] = 0.0
+
+            def run_schedule(mat_t, keep):
+                u = torch.zeros(nr, dtype=torch.float64, device=dev)
+                u_prev = torch.zeros_like(u)
+                h_a = torch.zeros(56 * ne, dtype=torch.float64, device=dev)
+                states, J, t_prev, dt_prev, nwt = [], 0.0, 0.0, 0.0, 0
+                for tn in ts:
+                    r = (tn - t_prev) / dt_prev if dt_prev > 0 else 0.0
+                    u_try = ctx.lincomb(1.0 + r, u, -r, u_prev)
+                    u_try, h_b, rep = ctx.newton_solve(u_try, h_a, mat_t, bc_d, torch.from_numpy(full * tn).to(dev),
+                                                       lin_rtol=1e-10, lin_max_iter=40000, rtol=1e-9, atol=1e-8, max_newton=20)
+                    assert rep["converged"], (tn, rep)
+                    nwt += rep["newton_iters"]
+                    J += 0.5 * float(((u_try * free) ** 2).sum())
+                    if keep:
+                        states.append((u_try.clone(), h_a))
+                    u_prev, u = u, u_try
+                    dt_prev, t_prev = tn - t_prev, tn
+                    h_a = h_b
+                return J, states, nwt
+            torch.cuda.synchronize(); t0 = time.perf_counter()
+            J0, states, nwt = run_schedule(mat, True)
+            torch.cuda.synchronize(); t_fwd = time.perf_counter() - t0
+            t0 = time.perf_counter()
+            grad = torch.zeros(16, dtype=torch.float64, device=dev)
+            mu, its_tot = None, 0
+            for (u_n, h_nm1) in reversed(states):
+                lam, mu, g_m, its = ctx.adjoint_step(u_n, h_nm1, mat, bc_d, dJdu=u_n * free, mu_in=mu, lin_rtol=1e-10, lin_max_iter=40000)
+                grad += g_m[0]; its_tot += its
+            torch.cuda.synchronize(); t_bwd = time.perf_counter() - t0
+            g = grad.cpu().numpy()
+            print("\n| adjoint of the whole benchmark (%d steps, J = 1/2 sum |u^n|^2 on the free DOFs = %.6e) | forward %.1f s, %d Newton iterations "
+                  "(Newton rtol 1e-9, linear 1e-10) | backward sweep %.1f s = %.2f s per step, %d Krylov iterations |"
+                  % (len(ts), J0, t_fwd, nwt, t_bwd, t_bwd / len(ts), its_tot), flush=True)
+            names = ["E", "nu", "r11", "r22", "r33", "r12", "r23", "r13", "law", "sigma0", "Q", "b"]
+            print("| dJ/dtheta | " + " | ".join("%s %.6e" % (names[i], g[i]) for i in (0, 1, 2, 3, 4, 5, 6, 7, 9, 10, 11)) + " |", flush=True)
+            if args.adjoint > 1:
+                idx, rel = 9, 1e-3
+                mp, mm = mat.clone(), mat.clone()
+                hstep = rel * float(mat[idx])
+                mp[idx] += hstep; mm[idx] -= hstep
+                fd = (run_schedule(mp, False)[0] - run_schedule(mm, False)[0]) / (2 * hstep)
+                print("| central difference d J / d %s (Eq.(52), h = %.0e theta, same schedule) | %.6e | adjoint %.6e | relative difference %.2e |"
+                      % (names[idx], rel, fd, g[idx], abs(fd - g[idx]) / abs(fd)), flush=True)
 
 
 if __name__ == "__main__":
