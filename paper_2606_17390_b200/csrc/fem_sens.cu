@@ -17,7 +17,8 @@
 //              reduced by hand to Xi = (E^-1 + dgam dN/dT)^-1 (Sherman-Morrison on D - kappa N(x)N) and one scalar w_f,
 //              then zbar = -(dG/dz)^T w for z = (eps, eps_p_n, alpha_n, theta), d eps = P_L:dC/2, C = F^T F, F = I + u^T G.
 // theta = (E, nu, r11, r22, r33, r12, r23, r13, h0, h1, h2): positions 0-7 and 9-11 of the 16-double record; the law
-// switch and the orientation quaternion are not differentiated (their entries of g_mat are 0).  Hill-48, standard element.
+// switch and the orientation quaternion are not differentiated (their entries of g_mat are 0).  Hill-48; standard element and
+// F-bar (template FBAR = 1: Fbar = (Jbar/J)^(1/3) F, Eq.(31)-(32) :237-243, Jbar and the back-propagated sum by 8-lane butterflies).
 // Sums are taken in a fixed order (per node: ascending element id; uniform material: fixed two-level tree), no atomics.
 // Nothing here is shared with oracle/.
 #include "fem_internal.h"
