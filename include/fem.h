@@ -197,6 +197,14 @@ int fem_bicgstab(fem_ctx *c, const double *csr_vals, const double *b, double *x,
 int fem_pcg(fem_ctx *c, const double *csr_vals, const double *b, double *x, double rtol, int max_iter, int *iters,
             double *relres, void *cuda_stream);
 
+/* Mixed-precision CG (off by default).  on = 1: inside fem_pcg — and wherever the library calls it: fem_newton_solve,
+ * fem_adjoint_step — the SpMV of the iteration reads an fp32 copy of K (half the bytes of an HBM-bound kernel; one more
+ * nnz-sized float workspace, refreshed at every call), vectors and scalars stay fp64, and every residual that decides
+ * convergence is b - K x with the fp64 matrix: the iteration is restarted from it (iterative refinement, at most five
+ * orders of magnitude per round) until that residual meets rtol.  The returned x therefore satisfies the same test as with
+ * on = 0; iteration counts differ slightly, repeats are still bit-identical.  fem_bicgstab is not affected. */
+int fem_set_mixed_precision(fem_ctx *c, int on);
+
 /* out = a x + b y on DOF vectors (dev [n_rows]; out may alias x or y).  For the caller's load-step control, e.g. the
  * extrapolated initial guess u + (u - u_prev) dt/dt_prev of the paper's time stepping. */
 int fem_lincomb(fem_ctx *c, double a, const double *x, double b, const double *y, double *out, void *cuda_stream);

@@ -39,6 +39,7 @@ def main():
     ap.add_argument("--extrapolate", type=int, default=1, help="initial guess of a step: 0 last state, 1 linear, 2 quadratic extrapolation")
     ap.add_argument("--adjoint", type=int, default=0, help="1: after the load path, run the backward sweep of Alg. 1 (fem_adjoint_step per step) "
                     "for J = 1/2 sum_n |u^n|^2 on the free DOFs and check dJ/d(sigma0) against a central difference of two more forward paths")
+    ap.add_argument("--mixed", type=int, default=0, help="1: fem_set_mixed_precision (fp32 copy of K inside CG, fp64 residuals)")
     ap.add_argument("--grow-below", type=int, default=6, help="grow the step after a step with at most this many Newton iterations")
     args = ap.parse_args()
     n = args.n
@@ -48,6 +49,8 @@ def main():
     nn, ne = coords.shape[0], conn.shape[0]
     ctx = fem.FemContext(torch.from_numpy(coords).to(dev), torch.from_numpy(conn).to(dev), fbar=args.fbar)
     ctx.build_csr_pattern()
+    if args.mixed:
+        ctx.set_mixed_precision(True)
     nnz, nr = ctx.nnz, 3 * nn
     # Table 3: E = 219 GPa, Voce sigma0 = 138, Q = 410, b = 3.8, ratios r11..r23; nu is not printed: 0.3
     rec = fem.mat_record(219000.0, 0.3, [1.5449, 1.0666, 1.0, 1.0307, 1.0, 1.0], 0.0, 138.0, 410.0, 3.8)

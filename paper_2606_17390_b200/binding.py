@@ -11,7 +11,7 @@ NBARLAT = 20
 ABI_SYMBOLS = ["fem_default_options", "fem_setup", "fem_build_csr_pattern", "fem_assemble", "fem_assemble_barlat", "fem_assemble_host",
                "fem_last_kernel_ms", "fem_launches_per_assemble", "fem_probe_fp64_peak", "fem_destroy", "fem_strerror",
                "fem_last_cuda_error", "fem_hill_from_lankford", "fem_spmv", "fem_apply_dirichlet", "fem_bicgstab", "fem_pcg", "fem_lincomb",
-               "fem_default_newton_options", "fem_newton_solve", "fem_assemble_vjp", "fem_adjoint_step"]
+               "fem_default_newton_options", "fem_newton_solve", "fem_assemble_vjp", "fem_adjoint_step", "fem_set_mixed_precision"]
 
 
 class FemOptions(C.Structure):
@@ -101,6 +101,7 @@ def lib():
         L.fem_newton_solve.argtypes = [vp, vp, vp, vp, ll, ll, vp, vp, vp, C.POINTER(FemNewtonOptions),
                                        C.POINTER(FemNewtonReport), vp]
         L.fem_assemble_vjp.argtypes = [vp, vp, vp, vp, ll, vp, vp, vp, vp, vp, vp]
+        L.fem_set_mixed_precision.argtypes = [vp, C.c_int]
         L.fem_adjoint_step.argtypes = [vp, vp, vp, vp, ll, ll, vp, vp, vp, vp, vp, vp, C.c_double, C.c_int, C.POINTER(C.c_int), vp]
         _lib = L
     return _lib
@@ -360,6 +361,10 @@ class FemContext:
                                       _ptr(g_m, f64, n_mat * NPAR, "g_mat"), float(lin_rtol), int(lin_max_iter), C.byref(it),
                                       _stream_ptr()), "fem_adjoint_step")
         return lam, mu_out, g_m.view(n_mat, NPAR), it.value
+
+    def set_mixed_precision(self, on=True):
+        """fem_set_mixed_precision: fp32 copy of K inside the CG iteration, fp64 residuals and refinement."""
+        _check(lib().fem_set_mixed_precision(self._h, 1 if on else 0), "fem_set_mixed_precision")
 
     def last_kernel_ms(self):
         ms = (C.c_double * 3)()

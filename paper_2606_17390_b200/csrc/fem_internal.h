@@ -58,6 +58,8 @@ struct fem_ctx {
     double *d_scal = nullptr;      // [8] reduced scalars
     double *d_nw = nullptr;        // [4*n_rows] Newton workspace: residual, rhs, dd, u at entry
     double *d_nw_vals = nullptr;   // [nnz] Newton workspace: stiffness values
+    float *d_vals32 = nullptr;     // [nnz] fp32 copy of K for the SpMV inside mixed-precision CG (fem_set_mixed_precision)
+    int mixed_precision = 0;
     double *d_nw_valsT = nullptr;  // [nnz] transposed stiffness values (adjoint step of the F-bar element), allocated on first use
     long long n_part = 0;
     // NEXT-3 (fem_sens.cu): per-CTA partial sums of the material gradient (uniform material)

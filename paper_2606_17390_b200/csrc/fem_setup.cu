@@ -242,7 +242,7 @@ static void ctx_free(fem_ctx *c) {
     if (!c) return;
     void *ptrs[] = {c->d_coords, c->d_conn, c->d_inc_ptr, c->d_inc, c->d_nb_ptr, c->d_nb, c->d_row_ptr, c->d_col_idx,
                     c->d_eslot, c->d_eorder, c->d_diagpos, c->d_sw, c->d_part, c->d_scal, c->d_nw, c->d_nw_vals, c->d_cnt_init, c->d_cnt, c->d_queue_init, c->d_queue, c->d_qctl, c->d_elem_pos, c->d_elem_slot, c->d_kvec, c->d_elist, c->d_first_mask, c->d_first_res, c->d_Ke, c->d_Re, c->d_matd, c->d_bard, c->d_stats, c->d_u, c->d_hin, c->d_hout,
-                    c->d_mat, c->d_res, c->d_vals, c->d_sens_part, c->d_nw_valsT};
+                    c->d_mat, c->d_res, c->d_vals, c->d_sens_part, c->d_nw_valsT, c->d_vals32};
     for (void *p : ptrs) if (p) cudaFree(p);
     for (int i = 0; i < 4; i++) if (c->ev[i]) cudaEventDestroy(c->ev[i]);
     delete c;

@@ -103,9 +103,9 @@ __global__ void __launch_bounds__(1024) k_reduce_final(const double *__restrict_
 // y = K x on the block structure of the pattern: one warp per node n, lane = neighbour position; row 3n+i holds the
 // entries [pos][k] contiguously, so a lane reads 3 x 24 bytes of values, one block-column index (nb, 4 bytes per 3x3
 // block instead of col_idx's 36) and 3 entries of x.  DOT = 1: partial sums of (w, y); DOT = 2: of (y, w) and (y, y).
-template <int DOT>
+template <int DOT, typename VT = double>   // VT = float: the fp32 copy of K used inside mixed-precision CG (vectors stay fp64)
 __global__ void __launch_bounds__(256)
-k_spmv(long long n_nodes, const int *__restrict__ nb_ptr, const int *__restrict__ nb, const double *__restrict__ vals,
+k_spmv(long long n_nodes, const int *__restrict__ nb_ptr, const int *__restrict__ nb, const VT *__restrict__ vals,
        const double *__restrict__ x, double *__restrict__ y, const double *__restrict__ w, double *__restrict__ part) {
     __shared__ double smem[2 * 32];
     const int lane = threadIdx.x & 31;
@@ -114,14 +114,14 @@ k_spmv(long long n_nodes, const int *__restrict__ nb_ptr, const int *__restrict_
     for (long long n = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5; n < n_nodes; n += warps) {
         double a0 = 0.0, a1 = 0.0, a2 = 0.0;
         const int o = nb_ptr[n], len = nb_ptr[n + 1] - o;
-        const double *base = vals + 9LL * o;
+        const VT *base = vals + 9LL * o;
         for (int pos = lane; pos < len; pos += 32) {
             const long long m = nb[o + pos];
             const double x0 = x[3 * m], x1 = x[3 * m + 1], x2 = x[3 * m + 2];
-            const double *r0 = base + 3 * pos, *r1 = r0 + 3 * len, *r2 = r1 + 3 * len;
-            a0 = fma(r0[2], x2, fma(r0[1], x1, fma(r0[0], x0, a0)));
-            a1 = fma(r1[2], x2, fma(r1[1], x1, fma(r1[0], x0, a1)));
-            a2 = fma(r2[2], x2, fma(r2[1], x1, fma(r2[0], x0, a2)));
+            const VT *r0 = base + 3 * pos, *r1 = r0 + 3 * len, *r2 = r1 + 3 * len;
+            a0 = fma((double)r0[2], x2, fma((double)r0[1], x1, fma((double)r0[0], x0, a0)));
+            a1 = fma((double)r1[2], x2, fma((double)r1[1], x1, fma((double)r1[0], x0, a1)));
+            a2 = fma((double)r2[2], x2, fma((double)r2[1], x1, fma((double)r2[0], x0, a2)));
         }
 #pragma unroll
         for (int o2 = 16; o2 > 0; o2 >>= 1) {
@@ -367,6 +367,13 @@ static void launch_spmv(fem_ctx *c, const double *vals, const double *x, double 
     k_spmv<DOT><<<spmv_grid(c), 256, 0, st>>>(c->n_nodes, c->d_nb_ptr, c->d_nb, vals, x, y, w, c->d_part);
 }
 
+static void launch_spmv32_dot(fem_ctx *c, const float *vals, const double *x, double *y, const double *w, cudaStream_t st) {
+    k_spmv<1, float><<<spmv_grid(c), 256, 0, st>>>(c->n_nodes, c->d_nb_ptr, c->d_nb, vals, x, y, w, c->d_part);
+}
+__global__ void k_to_f32(long long n, const double *__restrict__ a, float *__restrict__ out) {
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) out[i] = (float)a[i];
+}
+
 extern "C" int fem_spmv(fem_ctx *c, const double *csr_vals, const double *x, double *y, void *cuda_stream) {
     if (!c || !csr_vals || !x || !y) return FEM_ERR_NULL;
     if (!c->has_pattern) return FEM_ERR_NO_PATTERN;
@@ -499,6 +506,15 @@ static int pcg(fem_ctx *c, const double *vals, const double *b, double *x, doubl
     const long long spmv_ctas = spmv_grid(c);
     double h[2];
     int rc;
+    // Mixed precision (fem_set_mixed_precision): the SpMV of the iteration reads an fp32 copy of K (half the bytes of an
+    // HBM-bound kernel); every residual that decides convergence is b - K x with the fp64 matrix, and the iteration is
+    // restarted from it (iterative refinement) until that residual meets rtol.  Vectors and scalars are fp64 throughout.
+    const float *v32 = nullptr;
+    if (c->mixed_precision) {
+        if (!c->d_vals32) FEM_CUDA(cudaMalloc(&c->d_vals32, sizeof(float) * (size_t)c->nnz));
+        k_to_f32<<<RED_CTAS * 8, RED_THREADS, 0, st>>>(c->nnz, vals, c->d_vals32);
+        v32 = c->d_vals32;
+    }
     k_dinv<<<nblk3(n, 256), 256, 0, st>>>(c->n_nodes, c->d_nb_ptr, c->d_diagpos, vals, dinv);
     launch_spmv<0>(c, vals, x, r, nullptr, st);
     k_bicg_init<<<RED_CTAS, RED_THREADS, 0, st>>>(n, b, r, scratch, p, q, c->d_part);   // r = b - K x, p = q = 0
@@ -511,24 +527,28 @@ static int pcg(fem_ctx *c, const double *vals, const double *b, double *x, doubl
         return FEM_OK;
     }
     const double tol2 = rtol * rtol * bb;
-    double rr = h[0];
-    bool conv = rr <= tol2, bad = false;
+    bool conv = h[0] <= tol2, bad = false;
     int it = 0;
-    // z = M^-1 r and (r, z): one k_cg_update with alpha = 0
-    k_cg_update<<<RED_CTAS, RED_THREADS, 0, st>>>(n, 0.0, nullptr, p, q, dinv, x, r, z, c->d_part);
-    if ((rc = fetch_sums<2>(c, RED_CTAS, h, st)) != FEM_OK) return rc;
-    if (!conv && max_iter > 0) {
+    for (int round = 0; !conv && !bad && it < max_iter && round < 10; round++) {
+        const double rr = h[0];
+        // a refinement round asks for at most five orders of magnitude: below that the fp32 matrix, not the iteration, sets the residual
+        const double tol2_round = (v32 && 1e-10 * rr > tol2) ? 1e-10 * rr : tol2;
+        // z = M^-1 r and (r, z): one k_cg_update with alpha = 0
+        k_cg_update<<<RED_CTAS, RED_THREADS, 0, st>>>(n, 0.0, nullptr, p, q, dinv, x, r, z, c->d_part);
+        if ((rc = fetch_sums<2>(c, RED_CTAS, h, st)) != FEM_OK) return rc;
         // iterations run in batches without a host round trip; the scalars live in d_scal, a finished solve freezes itself
-        double sc0[8] = {h[0], 0.0, 0.0, rr, tol2, 0.0, 0.0, 0.0};
+        double sc0[8] = {h[0], 0.0, 0.0, rr, tol2_round, 0.0, 0.0, 0.0};
         double *sc = c->d_scal + 16;
         FEM_CUDA(cudaMemcpyAsync(sc, sc0, sizeof(sc0), cudaMemcpyHostToDevice, st));
         FEM_CUDA(cudaStreamSynchronize(st));   // sc0 is on the stack
-        const int batch = 16;
+        const int batch = 16, it0 = it;
+        bool round_conv = false;
         while (it < max_iter) {
             const int nb = (max_iter - it < batch) ? max_iter - it : batch;
             for (int j = 0; j < nb; j++) {
                 k_cg_p<<<RED_CTAS, RED_THREADS, 0, st>>>(n, 0.0, sc, z, p);              // p = z + beta p (beta = 0 at first)
-                launch_spmv<1>(c, vals, p, q, p, st);                                   // q = K p, partial (p, q)
+                if (v32) launch_spmv32_dot(c, v32, p, q, p, st);                        // q = K p, partial (p, q)
+                else launch_spmv<1>(c, vals, p, q, p, st);
                 k_cg_alpha<<<1, 1024, 0, st>>>(c->d_part, spmv_ctas, sc);
                 k_cg_update<<<RED_CTAS, RED_THREADS, 0, st>>>(n, 0.0, sc, p, q, dinv, x, r, z, c->d_part);
                 k_cg_beta<<<1, 1024, 0, st>>>(c->d_part, RED_CTAS, sc);
@@ -536,19 +556,28 @@ static int pcg(fem_ctx *c, const double *vals, const double *b, double *x, doubl
             double hs[8];
             FEM_CUDA(cudaMemcpyAsync(hs, sc, sizeof(hs), cudaMemcpyDeviceToHost, st));
             FEM_CUDA(cudaStreamSynchronize(st));
-            it = (int)hs[6];
-            if (hs[5] == 1.0) { conv = true; break; }
+            it = it0 + (int)hs[6];
+            if (hs[5] == 1.0) { round_conv = true; break; }
             if (hs[5] == 2.0) { bad = true; break; }
         }
+        // the residual that counts: b - K x with the fp64 matrix (also the start of the next refinement round)
+        launch_spmv<0>(c, vals, x, r, nullptr, st);
+        k_bicg_init<<<RED_CTAS, RED_THREADS, 0, st>>>(n, b, r, scratch, p, q, c->d_part);
+        if ((rc = fetch_sums<2>(c, RED_CTAS, h, st)) != FEM_OK) return rc;
+        conv = v32 ? (h[0] <= tol2) : round_conv;
+        if (!v32 || !round_conv) break;
     }
-    launch_spmv<0>(c, vals, x, r, nullptr, st);
-    k_bicg_init<<<RED_CTAS, RED_THREADS, 0, st>>>(n, b, r, scratch, p, q, c->d_part);
-    if ((rc = fetch_sums<2>(c, RED_CTAS, h, st)) != FEM_OK) return rc;
     const double rel = sqrt(h[0] / bb);
     if (iters) *iters = it;
     if (relres) *relres = rel;
     FEM_CUDA(cudaGetLastError());
     return (conv && !bad && rel <= 100.0 * rtol) ? FEM_OK : FEM_ERR_NOCONV;
+}
+
+extern "C" int fem_set_mixed_precision(fem_ctx *c, int on) {
+    if (!c) return FEM_ERR_NULL;
+    c->mixed_precision = on ? 1 : 0;
+    return FEM_OK;
 }
 
 extern "C" int fem_pcg(fem_ctx *c, const double *csr_vals, const double *b, double *x, double rtol, int max_iter, int *iters,

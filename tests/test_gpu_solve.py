@@ -92,6 +92,16 @@ def test_bicgstab_against_direct_solve(case):
         assert okc and rrc <= 1e-10 and rel_l2(xc.cpu().numpy(), xo) <= 1e-7, (itc, rrc)
         xc2, itc2, _, _ = ctx.pcg(vals, rhs, x=xg.clone(), rtol=1e-12, max_iter=20000)
         assert itc2 == itc and torch.equal(xc, xc2)
+        # mixed precision: fp32 copy of K inside the iteration, fp64 residuals + refinement: same acceptance test, same solution
+        ctx.set_mixed_precision(True)
+        xm, itm, rrm, okm = ctx.pcg(vals, rhs, x=xg.clone(), rtol=1e-12, max_iter=20000)
+        assert okm and rrm <= 1e-12 and rel_l2(xm.cpu().numpy(), xo) <= 1e-7, (itm, rrm)
+        assert itm <= 2 * itc, (itm, itc)
+        xm2, itm2, _, _ = ctx.pcg(vals, rhs, x=xg.clone(), rtol=1e-12, max_iter=20000)
+        assert itm2 == itm and torch.equal(xm, xm2)
+        xl, itl, rrl, okl = ctx.pcg(vals, rhs, x=xg.clone(), rtol=1e-4, max_iter=20000)     # loose tolerance: one round
+        assert okl and rrl <= 1e-4 and itl < itm
+        ctx.set_mixed_precision(False)
     # zero right-hand side and iteration cap
     x0, it0, rr0, ok0 = ctx.bicgstab(vals, torch.zeros_like(rhs), x=torch.ones_like(rhs))
     assert ok0 and it0 == 0 and float(x0.abs().max()) == 0.0
