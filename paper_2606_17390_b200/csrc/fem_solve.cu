@@ -114,6 +114,8 @@ k_spmv(long long n_nodes, const int *__restrict__ nb_ptr, const int *__restrict_
     for (long long n = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5; n < n_nodes; n += warps) {
         double a0 = 0.0, a1 = 0.0, a2 = 0.0;
         const int o = nb_ptr[n], len = nb_ptr[n + 1] - o;
+        double w0 = 0.0, w1 = 0.0, w2 = 0.0;
+        if (DOT) { w0 = w[3 * n]; w1 = w[3 * n + 1]; w2 = w[3 * n + 2]; }   // issued with the row loads, not after the reduction
         const VT *base = vals + 9LL * o;
         for (int pos = lane; pos < len; pos += 32) {
             const long long m = nb[o + pos];
@@ -130,7 +132,6 @@ k_spmv(long long n_nodes, const int *__restrict__ nb_ptr, const int *__restrict_
         if (lane == 0) {
             y[3 * n] = a0; y[3 * n + 1] = a1; y[3 * n + 2] = a2;
             if (DOT) {
-                const double w0 = w[3 * n], w1 = w[3 * n + 1], w2 = w[3 * n + 2];
                 d[0] += a0 * w0 + a1 * w1 + a2 * w2;
                 d[1] += a0 * a0 + a1 * a1 + a2 * a2;
             }
