@@ -54,18 +54,19 @@ typedef struct {
     int jmax;          /* kept for ABI parity with Alg. C2's line search; the scalar solve
                           uses a bracket instead, so it is unused */
     double beta, eta;  /* Alg. C2 / App. B constants; unused by the scalar solve */
-    int assembly_mode; /* 0 (default) = element kernel writes K^e, R^e to a destination-major scratch, a node-row gather kernel
-                          sums them in ascending element id (deterministic, no atomics);
-                          1 = coloured in-place assembly: elements are coloured at pattern-build time so that no two elements
-                          of a colour share a node; one element-kernel launch per colour adds K^e, R^e into the outputs with
-                          plain read-modify-write in colour order (deterministic, no atomics, no scratch);
-                          2 = fused: same scratch and summation order as mode 0, but the element CTAs count every node's
-                          missing contributions down and queue completed nodes, and gather CTAs interleaved in the same
-                          launch (plus a drain kernel) assemble them while other elements are still being evaluated.
-                          Modes 1 and 2 are measured slower than mode 0 at config 3 and are kept as
-                          tested options; they fall back to mode 0 for meshes with collapsed elements (1, 2) or a node with
-                          more than 8 elements (2).  In mode 0 such nodes are gathered by a general path, all others by the
-                          table-driven fast path of the same kernel. */
+    int assembly_mode; /* How S14 (K = A K^e, R = A R^e, Eq.(34) :253, Eq.(38) :274) is scheduled; the result is bit-identical in both.
+                          The element kernel writes K^e, R^e to a destination-major scratch (one 72-double record per
+                          (element, local node), node-sorted), and every CSR entry is the sum of its records in ascending element
+                          id (deterministic, no atomics).
+                          0 (default) = fused, lagged gather: at pattern-build time the nodes are cut into quads of four and every
+                          quad is given to one warp of an element CTA that is launched at least one wave of resident CTAs after
+                          the last CTA that writes one of its records; that warp sums the quad's CSR rows at the start of its CTA,
+                          reading the records back from L2 while its own inputs are on their way.  Completion is tracked by one
+                          flag per CTA; a warp never waits: a quad that is not ready (or is scheduled past the last CTA) is
+                          finished by a short gather kernel after the element launch.  Meshes with collapsed elements or a node
+                          with more than 8 elements use mode 1.
+                          1 = the element kernel, then a stand-alone node-row gather kernel over all nodes (nodes with more than 8
+                          elements / collapsed elements take a general path in it). */
 } fem_options;
 
 typedef struct {
@@ -96,8 +97,8 @@ int fem_setup(fem_ctx **out, long long n_nodes, const double *coords, long long 
  *   a,b = 3*local_node + component.  Any out-pointer may be NULL; the 576-wide map is only materialised when
  *   elem_slot != NULL (fem_assemble uses the compressed per-node-pair form internally).
  * Built entirely on the device; synchronises once.  Must precede fem_assemble.
- * Library-owned device memory after this call (bytes per element, hex meshes): pattern and gather tables ~1.4 kB
- * (col_idx 0.98 kB of it), assembly scratch 4.8 kB (8 block-row records of 576 B + R^e; modes 0 and 2), i.e. ~6.2 GB at
+ * Library-owned device memory after this call (bytes per element, hex meshes): pattern and gather tables ~1.5 kB
+ * (col_idx 0.98 kB of it), assembly scratch 4.8 kB (8 block-row records of 576 B + R^e), i.e. ~6.3 GB at
  * 1M elements, plus 2.3 kB per element if elem_slot is requested.  A cudaMalloc failure returns FEM_ERR_CUDA. */
 int fem_build_csr_pattern(fem_ctx *c, long long *n_rows, long long *nnz, const int **row_ptr, const int **col_idx,
                           const int **elem_slot);
@@ -113,8 +114,9 @@ int fem_build_csr_pattern(fem_ctx *c, long long *n_rows, long long *nnz, const i
  *   residual  dev [n_rows]   csr_vals dev [nnz]   hist_out dev [n_elems*8*7] (must not alias hist_in)
  *   stats     host, may be NULL; when non-NULL the call synchronises `stream` and copies the counters back
  *   cuda_stream  a cudaStream_t (NULL = legacy default stream); all work is ordered on it
- * Sums are taken in a fixed order (mode 0: ascending element id per entry; mode 1: colour order): two calls with equal
- * inputs give bit-identical output.
+ * Sums are taken in a fixed order (ascending element id per entry, in either assembly mode): two calls with equal
+ * inputs give bit-identical output.  The call is ordered on `cuda_stream`; two fem_assemble calls on the SAME context must
+ * not run concurrently on different streams (they share the scratch and the completion flags).
  * Physics trouble (local non-convergence, det F <= 0, non-finite) is counted in stats, never an error return. */
 int fem_assemble(fem_ctx *c, const double *u, const double *hist_in, const double *mat, long long n_mat,
                  double *residual, double *csr_vals, double *hist_out, fem_stats *stats, void *cuda_stream);
@@ -125,10 +127,10 @@ int fem_assemble(fem_ctx *c, const double *u, const double *hist_in, const doubl
  * Eq.(19)-(24) :176-196 by Newton iterations with the Goldstein line search of App. B :836-869 (beta = 1e-4, eta = 0.1).
  *   barlat    dev [n_mat*20]  c'12,c'13,c'21,c'23,c'31,c'32,c'44,c'55,c'66, the same nine of C'', m, 0
  *                             (Table 2 :471-477 order; shear rows in the component order 12,23,13; m an even integer 2..16 —
- *                             the paper uses 8, and 2, 4 for its reductions — other values give undefined results)
+ *                             the paper uses 8, and 2, 4 for its reductions.  Any other value is replaced by the nearest
+ *                             supported exponent inside the call, and the call returns FEM_ERR_ARG when stats != NULL)
  *   mat       as in fem_assemble; r11..r13 are ignored, E, nu, the hardening law and the orientation quaternion apply
- * All other arguments, the outputs, determinism and error behaviour are those of fem_assemble.  Requires assembly_mode 0
- * (FEM_ERR_ARG otherwise); opt.kmax caps the Newton iterations, opt.tol is unused (the iteration stops at the round-off
+ * All other arguments, the outputs, determinism and error behaviour are those of fem_assemble; opt.kmax caps the Newton iterations, opt.tol is unused (the iteration stops at the round-off
  * floor of the residual).  Launches one more (tiny) kernel than fem_assemble. */
 int fem_assemble_barlat(fem_ctx *c, const double *u, const double *hist_in, const double *mat, const double *barlat,
                         long long n_mat, double *residual, double *csr_vals, double *hist_out, fem_stats *stats,
@@ -138,8 +140,9 @@ int fem_assemble_barlat(fem_ctx *c, const double *u, const double *hist_in, cons
 int fem_assemble_host(fem_ctx *c, const double *u, const double *hist_in, const double *mat, long long n_mat,
                       double *residual, double *csr_vals, double *hist_out, fem_stats *stats);
 
-/* Device time in milliseconds of the two kernels of the last fem_assemble on this context, measured with CUDA events
- * on the call's stream: ms[0] = element kernel (S2-S12), ms[1] = gather kernel (S14), ms[2] = material pre-pass.
+/* Device time in milliseconds of the kernels of the last fem_assemble on this context, measured with CUDA events
+ * on the call's stream: ms[0] = element kernel (S2-S12; in assembly_mode 0 it also gathers most node rows, S14),
+ * ms[1] = the gather kernel that follows it (mode 0: the quads left over; mode 1: all nodes), ms[2] = material pre-pass.
  * Synchronises on the recorded events. */
 int fem_last_kernel_ms(fem_ctx *c, double ms[3] /*host*/);
 
@@ -183,7 +186,9 @@ int fem_apply_dirichlet(fem_ctx *c, long long n_bc, const int *bc_dofs, const do
  *   or after max_iter iterations.  On breakdown ((rhat, r), (rhat, v) or omega collapses) the iteration restarts from the
  *   explicit residual of the current x (at most 50 times).
  *   *iters (host, may be NULL) = iterations used; *relres (host, may be NULL) = explicit ||b - K x|| / ||b|| at exit.
- * Returns FEM_OK when converged, FEM_ERR_NOCONV otherwise (x holds the last iterate).  Dot products are reduced in a
+ * Returns FEM_OK when the recurrence residual met rtol AND the explicit residual of the returned x is within 100 rtol (the
+ * two drift apart by round-off at tight tolerances; *relres reports the explicit one), FEM_ERR_NOCONV otherwise (x holds the
+ * last iterate).  Dot products are reduced in a
  * fixed order: two calls with equal inputs give bit-identical results.  Synchronises the stream (the iteration scalars stay on the device; the host
  * checks the convergence flag after every batch of 8 iterations and restarts the recurrence on breakdown). */
 int fem_bicgstab(fem_ctx *c, const double *csr_vals, const double *b, double *x, double rtol, int max_iter, int *iters,
@@ -226,6 +231,8 @@ typedef struct {
     int lin_failures;        /* linear solves that returned FEM_ERR_NOCONV (the update is applied anyway) */
     double rhs_norm0, rhs_norm; /* first and last ||rhs||_2 */
     fem_stats last_stats;    /* statistics of the last fem_assemble */
+    int physics_trouble;     /* 1 when the residual test passed but last_stats shows local solves that hit kmax, points with
+                                det F <= 0 or non-finite stresses: the increment is then NOT accepted (converged = 0, FEM_ERR_NOCONV) */
 } fem_newton_report;
 
 void fem_default_newton_options(fem_newton_options *o /*host*/);
@@ -238,12 +245,57 @@ void fem_default_newton_options(fem_newton_options *o /*host*/);
  *   hist_out dev [n_elems*56] history at the returned u (from the last fem_assemble)
  *   bc_dofs  dev [n_bc] constrained DOFs, bc_vals dev [n_bc] their prescribed TOTAL displacement
  * Each iteration: fem_assemble(u) -> rhs = -R -> constrained rows: identity, rhs = bc_vals - u (so the update lands on
- * the prescribed value) -> test ||rhs|| -> linear solve (fem_newton_options.linear_solver) -> u += dd.  The stiffness matrix, residual and
+ * the prescribed value) -> test ||rhs|| (relative to the ||rhs|| of iteration 0 of THIS call, which includes the boundary
+ * mismatch of the initial guess) -> linear solve (fem_newton_options.linear_solver) -> u += dd.  The stiffness matrix, residual and
  * Krylov vectors live in library-owned workspace (allocated on first use).  Returns FEM_OK when converged,
- * FEM_ERR_NOCONV when max_newton is reached; *rep (host, may be NULL) is always filled.  Synchronises the stream. */
+ * FEM_ERR_NOCONV when max_newton is reached or when the balanced state shows physics trouble (rep->physics_trouble);
+ * FEM_ERR_ALIAS when hist_out overlaps hist_in.  On every non-OK return u holds its entry value.  *rep (host, may be NULL) is
+ * always filled.  Synchronises the stream. */
 int fem_newton_solve(fem_ctx *c, double *u, const double *hist_in, const double *mat, long long n_mat, long long n_bc,
                      const int *bc_dofs, const double *bc_vals, double *hist_out, const fem_newton_options *opt,
                      fem_newton_report *rep, void *cuda_stream);
+
+typedef struct {
+    double dt0;        /* first load increment, as a fraction of the full load (default 1e-3) */
+    double dt_min;     /* the path is abandoned (FEM_ERR_NOCONV) when a cut-back goes below this (1e-5) */
+    double dt_max;     /* largest increment (5e-2) */
+    double grow;       /* factor applied to dt after an accepted step that needed <= grow_below Newton iterations (1.5) */
+    double cut;        /* factor applied to dt after a rejected step (0.5) */
+    int grow_below;    /* (5) */
+    int max_steps;     /* cap on accepted + rejected steps (10000) */
+    int extrapolate;   /* initial guess of a step: 0 = last converged state, 1 = linear, 2 = quadratic extrapolation of the
+                          converged states ("extrapolated initial guess") */
+    fem_newton_options newton; /* per-increment Newton options (defaults: rtol 1e-8, max_newton 12, lin_rtol 1e-6, lin_max_iter 20000) */
+} fem_path_options;
+
+typedef struct {
+    int steps;               /* accepted load steps */
+    int rejected;            /* rejected steps (each one cuts dt back) */
+    int rejected_physics;    /* of those: balanced states rejected for fem_stats trouble (fem_newton_report.physics_trouble) */
+    int newton_iters_total;  /* over accepted and rejected steps */
+    int lin_iters_total;
+    double t_reached;        /* load fraction of the last accepted state (1 when the path was completed) */
+    fem_newton_report last;  /* report of the last accepted step */
+} fem_path_report;
+
+void fem_default_path_options(fem_path_options *o /*host*/);
+
+/* fem_load_path — the adaptive load stepping of the paper around fem_newton_solve ("time step in
+ * [dt_min, dt_max], cut back on failure or non-finite values, extrapolated initial guess"; benchmark settings :485):
+ * the prescribed displacement bc_full is ramped from 0 to its full value, load fraction t in (0, 1].
+ *   u        dev [n_rows] in/out   converged state at t = 0 on entry (e.g. zeros) -> state at t_reached
+ *   hist     dev [n_elems*56] in/out   history at t = 0 -> history of the last accepted state
+ *   bc_dofs  dev [n_bc], bc_full dev [n_bc]: constrained DOFs and their prescribed displacement at t = 1
+ *   t_accepted host [n_t_cap] or NULL: load fractions of the accepted steps (the schedule an adjoint sweep repeats)
+ * A step is: guess = extrapolation of the last converged states (fem_lincomb arithmetic) -> fem_newton_solve at t + dt ->
+ * accepted when it converged with no failed linear solve and no physics trouble; then dt grows by `grow` if the step was
+ * easy.  Otherwise the state is left at the last accepted one and dt is cut by `cut`.
+ * Returns FEM_OK when t = 1 was reached, FEM_ERR_NOCONV when dt fell below dt_min or max_steps was used up (u, hist hold the
+ * last accepted state, rep->t_reached says where), other codes as fem_newton_solve.  Allocates one history-sized and four
+ * n_rows-sized workspace arrays on first use.  Synchronises the stream. */
+int fem_load_path(fem_ctx *c, double *u, double *hist, const double *mat, long long n_mat, long long n_bc, const int *bc_dofs,
+                  const double *bc_full, const fem_path_options *opt, fem_path_report *rep, double *t_accepted, int n_t_cap,
+                  void *cuda_stream);
 
 /* fem_assemble_vjp — SURVEY.md section 8(f) NEXT-3: vector-Jacobian products of one fem_assemble pass, i.e. of the map
  * (u, hist_in, mat) -> (residual, hist_out), for the discrete adjoint of Alg. 1 (Eq.(49)-(51) :355-366).
@@ -261,7 +313,7 @@ int fem_newton_solve(fem_ctx *c, double *u, const double *hist_in, const double 
  * re-evaluated inside the call (nothing is kept from fem_assemble), the return map is differentiated implicitly at its
  * root (App. D Eq.(D4)-(D7) :1002-1019, transposed).  Hill-48 only; both element formulations: with fbar = 1 the
  * coupling of an element's 8 Gauss points through Jbar (Eq.(31)-(32) :237-243) is part of the product, and K^T differs
- * from K.  FEM_ERR_ARG when g_u is wanted in assembly_mode 1 (no scratch).  Sums run in a fixed order, no atomics: equal inputs give bit-identical outputs.  Uses the library's
+ * from K.  Sums run in a fixed order, no atomics: equal inputs give bit-identical outputs.  Uses the library's
  * R^e scratch: do not run concurrently with fem_assemble on another stream.  Asynchronous on `cuda_stream`. */
 int fem_assemble_vjp(fem_ctx *c, const double *u, const double *hist_in, const double *mat, long long n_mat,
                      const double *lam, const double *mu, double *g_u, double *g_hist_in, double *g_mat, void *cuda_stream);

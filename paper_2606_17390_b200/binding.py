@@ -11,7 +11,8 @@ NBARLAT = 20
 ABI_SYMBOLS = ["fem_default_options", "fem_setup", "fem_build_csr_pattern", "fem_assemble", "fem_assemble_barlat", "fem_assemble_host",
                "fem_last_kernel_ms", "fem_launches_per_assemble", "fem_probe_fp64_peak", "fem_destroy", "fem_strerror",
                "fem_last_cuda_error", "fem_hill_from_lankford", "fem_spmv", "fem_apply_dirichlet", "fem_bicgstab", "fem_pcg", "fem_lincomb",
-               "fem_default_newton_options", "fem_newton_solve", "fem_assemble_vjp", "fem_adjoint_step", "fem_set_mixed_precision"]
+               "fem_default_newton_options", "fem_newton_solve", "fem_assemble_vjp", "fem_adjoint_step", "fem_set_mixed_precision",
+               "fem_default_path_options", "fem_load_path"]
 
 
 class FemOptions(C.Structure):
@@ -35,12 +36,27 @@ class FemNewtonOptions(C.Structure):
 
 class FemNewtonReport(C.Structure):
     _fields_ = [("newton_iters", C.c_int), ("converged", C.c_int), ("lin_iters_total", C.c_int), ("lin_failures", C.c_int),
-                ("rhs_norm0", C.c_double), ("rhs_norm", C.c_double), ("last_stats", FemStats)]
+                ("rhs_norm0", C.c_double), ("rhs_norm", C.c_double), ("last_stats", FemStats), ("physics_trouble", C.c_int)]
 
     def as_dict(self):
         return dict(newton_iters=self.newton_iters, converged=bool(self.converged), lin_iters_total=self.lin_iters_total,
                     lin_failures=self.lin_failures, rhs_norm0=self.rhs_norm0, rhs_norm=self.rhs_norm,
-                    last_stats=self.last_stats.as_dict())
+                    last_stats=self.last_stats.as_dict(), physics_trouble=bool(self.physics_trouble))
+
+
+class FemPathOptions(C.Structure):
+    _fields_ = [("dt0", C.c_double), ("dt_min", C.c_double), ("dt_max", C.c_double), ("grow", C.c_double), ("cut", C.c_double),
+                ("grow_below", C.c_int), ("max_steps", C.c_int), ("extrapolate", C.c_int), ("newton", FemNewtonOptions)]
+
+
+class FemPathReport(C.Structure):
+    _fields_ = [("steps", C.c_int), ("rejected", C.c_int), ("rejected_physics", C.c_int), ("newton_iters_total", C.c_int),
+                ("lin_iters_total", C.c_int), ("t_reached", C.c_double), ("last", FemNewtonReport)]
+
+    def as_dict(self):
+        return dict(steps=self.steps, rejected=self.rejected, rejected_physics=self.rejected_physics,
+                    newton_iters_total=self.newton_iters_total, lin_iters_total=self.lin_iters_total, t_reached=self.t_reached,
+                    last=self.last.as_dict())
 
 
 class FemError(RuntimeError):
@@ -100,6 +116,10 @@ def lib():
         L.fem_default_newton_options.restype = None
         L.fem_newton_solve.argtypes = [vp, vp, vp, vp, ll, ll, vp, vp, vp, C.POINTER(FemNewtonOptions),
                                        C.POINTER(FemNewtonReport), vp]
+        L.fem_default_path_options.argtypes = [C.POINTER(FemPathOptions)]
+        L.fem_default_path_options.restype = None
+        L.fem_load_path.argtypes = [vp, vp, vp, vp, ll, ll, vp, vp, C.POINTER(FemPathOptions), C.POINTER(FemPathReport),
+                                    C.POINTER(C.c_double), C.c_int, vp]
         L.fem_assemble_vjp.argtypes = [vp, vp, vp, vp, ll, vp, vp, vp, vp, vp, vp]
         L.fem_set_mixed_precision.argtypes = [vp, C.c_int]
         L.fem_adjoint_step.argtypes = [vp, vp, vp, vp, ll, ll, vp, vp, vp, vp, vp, vp, C.c_double, C.c_int, C.POINTER(C.c_int), vp]
@@ -327,6 +347,29 @@ class FemContext:
         if rc not in (0, -11):
             _check(rc, "fem_newton_solve")
         return u, hist_out, rep.as_dict()
+
+    def load_path(self, u, hist, mat, bc_dofs, bc_full, newton=None, **path):
+        """fem_load_path: adaptive load stepping from t = 0 to 1; u and hist are updated in place.
+        `path`: dt0, dt_min, dt_max, grow, cut, grow_below, max_steps, extrapolate; `newton`: dict of fem_newton_options fields.
+        Returns (return code, report dict, accepted load fractions)."""
+        torch = _torch()
+        f64 = torch.float64
+        opt = FemPathOptions()
+        lib().fem_default_path_options(C.byref(opt))
+        for k, v in path.items():
+            setattr(opt, k, v)
+        for k, v in (newton or {}).items():
+            setattr(opt.newton, k, v)
+        rep = FemPathReport()
+        cap = int(opt.max_steps)
+        ts = (C.c_double * cap)()
+        nbc = bc_dofs.numel()
+        rc = lib().fem_load_path(self._h, _ptr(u, f64, self.n_rows, "u"), _ptr(hist, f64, 56 * self.n_elems, "hist"),
+                                 _ptr(mat, f64, None, "mat"), mat.numel() // NPAR, nbc, _ptr(bc_dofs, torch.int32, None, "bc_dofs"),
+                                 _ptr(bc_full, f64, nbc, "bc_full"), C.byref(opt), C.byref(rep), ts, cap, _stream_ptr())
+        if rc not in (0, -11):
+            _check(rc, "fem_load_path")
+        return rc, rep.as_dict(), list(ts[:rep.steps])
 
     def assemble_vjp(self, u, hist_in, mat, lam=None, mu=None, want_u=True, want_hist=True, want_mat=True):
         """fem_assemble_vjp: (g_u, g_hist_in, g_mat) for the cotangents lam on the residual and mu on hist_out (None = zero);

@@ -5,7 +5,7 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libfem_b200.so")
-SOURCES = ["fem_setup.cu", "fem_colour.cu", "fem_assemble.cu", "fem_api.cu", "fem_solve.cu", "fem_sens.cu"]
+SOURCES = ["fem_setup.cu", "fem_assemble.cu", "fem_api.cu", "fem_solve.cu", "fem_sens.cu"]
 HEADERS = [os.path.join(CSRC, "fem_internal.h"), os.path.join(CSRC, "fem_barlat.cuh"), os.path.join(CSRC, "fem_device.cuh"), os.path.join(HERE, "..", "include", "fem.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "--use_fast_math=false",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"]

@@ -15,6 +15,7 @@ int fem_read_stats(fem_ctx *c, fem_stats *stats, cudaStream_t st) {
         stats->iter_hist[k] = (long long)h[5 + k];
         if (h[5 + k]) stats->max_local_iters = k;
     }
+    c->bad_barlat_m = h[69] != 0;
     return FEM_OK;
 }
 
@@ -23,11 +24,7 @@ extern "C" int fem_assemble(fem_ctx *c, const double *u, const double *hist_in, 
     if (!c || !u || !hist_in || !mat || !residual || !csr_vals || !hist_out) return FEM_ERR_NULL;
     if (!c->has_pattern) return FEM_ERR_NO_PATTERN;
     if (n_mat != 1 && n_mat != c->n_elems) return FEM_ERR_MAT;
-    {   // hist_out must not overlap hist_in
-        const char *a = (const char *)hist_in, *b = (const char *)hist_out;
-        const size_t bytes = sizeof(double) * 56 * (size_t)c->n_elems;
-        if (a < b + bytes && b < a + bytes) return FEM_ERR_ALIAS;
-    }
+    if (fem_ranges_overlap(hist_in, hist_out, sizeof(double) * 56 * (size_t)c->n_elems)) return FEM_ERR_ALIAS;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     int rc = fem_launch_assemble(c, u, hist_in, mat, n_mat, residual, csr_vals, hist_out, st);
     if (rc != FEM_OK) return rc;
@@ -41,16 +38,15 @@ extern "C" int fem_assemble_barlat(fem_ctx *c, const double *u, const double *hi
     if (!c || !u || !hist_in || !mat || !barlat || !residual || !csr_vals || !hist_out) return FEM_ERR_NULL;
     if (!c->has_pattern) return FEM_ERR_NO_PATTERN;
     if (n_mat != 1 && n_mat != c->n_elems) return FEM_ERR_MAT;
-    if (c->mode != 0) return FEM_ERR_ARG;
-    {
-        const char *a = (const char *)hist_in, *b = (const char *)hist_out;
-        const size_t bytes = sizeof(double) * 56 * (size_t)c->n_elems;
-        if (a < b + bytes && b < a + bytes) return FEM_ERR_ALIAS;
-    }
+    if (fem_ranges_overlap(hist_in, hist_out, sizeof(double) * 56 * (size_t)c->n_elems)) return FEM_ERR_ALIAS;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     int rc = fem_launch_assemble(c, u, hist_in, mat, n_mat, residual, csr_vals, hist_out, st, barlat);
     if (rc != FEM_OK) return rc;
-    if (stats) return fem_read_stats(c, stats, st);
+    if (stats) {
+        rc = fem_read_stats(c, stats, st);
+        if (rc == FEM_OK && c->bad_barlat_m) rc = FEM_ERR_ARG;   // an exponent outside the even integers 2..16 (it was clamped)
+        return rc;
+    }
     return FEM_OK;
 }
 
@@ -101,7 +97,8 @@ extern "C" int fem_last_kernel_ms(fem_ctx *c, double ms[3]) {
 
 extern "C" int fem_launches_per_assemble(const fem_ctx *c) {
     if (!c) return 0;
-    return c->mode == 1 ? 1 + c->n_colours : 3;   // (+1 for fem_assemble_barlat: its coefficient pre-pass)   // mat_prep + one element launch per colour | mat_prep + element (+ fused gather) + gather / drain
+    return 3;   // k_mat_prep, k_element (with the fused gather where the mesh allows it), k_gather_list / k_gather_fast / k_gather
+                // (+1 for fem_assemble_barlat: its coefficient pre-pass)
 }
 
 // ------------------------------------------------------------------------------------------------ FP64 peak probe

@@ -12,7 +12,6 @@
 //   k_gather_fast / k_gather : one warp per node: copies the node's contiguous run of records to shared memory and sums the
 //                 <= 8 contributions of each 3x3 node-pair block in ascending element id (fixed order, no atomics)
 //                 into the CSR values and the residual.
-// assembly_mode 1 (coloured in-place) and 2 (fused queue) are alternatives kept as tested, slower options.
 // All formulas are derived by hand from PAPER.md (equation numbers at each step); nothing here is shared with oracle/.
 #include "fem_internal.h"
 #include "fem_device.cuh"
@@ -112,16 +111,12 @@ __host__ __device__ constexpr int sidx9(int r, int c) {  // packed upper triangl
 #define SM_AA 200   // 45 entries w * A^_(ia)(kb), packed symmetric: entry s < 44 at (s/2)*16 + 2 q + (s&1), entry 44 at 352 + q
 #define SM_XE 200   // [24] element coordinates   (overlay: dead before AA is written)
 #define SM_UE 224   // [24] element displacements (overlay)
-#define SM_KS 0     // K^e staging, 8 block-row records of 72 doubles (scratch record layout), overlays GG/AA after phase 2
-// component c of block (I,K) inside block row I: component-major [c][K], so that the two accumulators of a DMMA lane
-// (columns K = 2 tig, 2 tig + 1) are one 16-byte store and the 8 lanes of a transposed store fill 64 contiguous bytes
-#define KSX(I, K, c) (SM_KS + (I) * 72 + (c) * 8 + (K))
 #define SM_GQ 576   // [24][8]  (F-bar) g^q_Kk = G_KL F^-1_Lk
 #define SM_YY 768   // [9][8]   (F-bar) w/3 (A^:F^)_ia
 #define SM_GB 840   // [24]     (F-bar) gbar
 #define SM_WQ 864   // [8]      (F-bar) w_q J_q / (Jbar V)
 #define ES_STD 564   // >= 560, = 4 mod 16: the 4 elements of a warp start in 4 different bank groups
-#define ES_STAGE 580 // >= 576, = 4 mod 16: variants that stage the whole K^e (coloured mode) or lend their buffer to gather CTAs (fused mode)
+#define ES_FUSE 580  // >= 576, = 4 mod 16: the warp's four slots double as the gather buffer of four nodes (4 x 576 doubles)
 #define ES_FBAR 884  // >= 872, = 4 mod 16
 #ifndef EL_PER_CTA
 #define EL_PER_CTA 16
@@ -225,65 +220,42 @@ __device__ __forceinline__ void gather_warp_nodes(int nd, int cnt, double *wbuf,
                             wbuf + j * 576, lane, nb_ptr, kvec, Re, csr_vals, residual);
     __syncwarp();
 }
-// Claims up to `want` completed nodes of the queue: returns the count and the first queue index in h.  Entries below the
-// tail have a ticket; their node id may still be on its way (the reader spins on -1).
-__device__ __forceinline__ unsigned queue_claim(unsigned int *qctl, unsigned want, unsigned &h) {
-    volatile unsigned int *q = qctl;
-    for (;;) {
-        h = q[1];
-        const unsigned t = q[0];
-        if (t <= h) return 0u;
-        const unsigned n = min(want, t - h);
-        if (atomicCAS(&qctl[1], h, h + n) == h) return n;
-    }
-}
-__device__ __forceinline__ int queue_read(const int *queue, unsigned idx) {
-    volatile const int *qp = queue + idx;
-    int v;
-    while ((v = *qp) < 0) { }
-    return v;
-}
-#ifndef GATHER_EVERY
-#define GATHER_EVERY 8
-#endif
-// GATHER_EVERY:   // fused mode: one gather CTA after every 8 element CTAs
-#ifndef GATHER_POP
-#define GATHER_POP 160
-#endif
-// GATHER_POP:   // nodes a gather CTA claims at most (8 element CTAs complete ~132 nodes)
-
 // Keeping the warps of a CTA in the same code region lets them share instruction-cache lines (the kernel is ~94 KB of
 // straight-line SASS); ncu showed instruction fetch as a top stall without it.
 #ifndef PS_MASK
 #define PS_MASK 0x094   // measured best subset of the ten phase boundaries (sweep in DESIGN.md): before the return map, the tangent, phase 2
 #endif
 #define PHASE_SYNC_N(n) do { if ((PS_MASK >> (n)) & 1) __syncthreads(); } while (0)
-// MODE 0: K^e, R^e go to an HBM scratch (k_gather sums them).  MODE 1: launched once per colour (elist = the colour's
-// elements); K^e, R^e are added in place into csr_vals / residual (no two elements of a launch share a node).
+// Launch-time arguments of the assembly side of k_element.
+// Fused, lagged gather (FUSE = 1): the scratch is consumed while it is still in L2.  The nodes are cut into quads of
+// four consecutive ids; at setup every quad is given to one warp of an element CTA that is launched at least FUSE_LAG
+// chunks after the last chunk that contributes to the quad's nodes.  CTAs are dispatched in index order, so by then those
+// chunks have normally retired; each chunk publishes a completion flag (threadfence + flag = epoch of this call), the
+// gathering warp checks the flags of its quad's chunks WITHOUT waiting, and a quad that is not ready (or is scheduled
+// past the last chunk) goes to a short list that k_gather_list finishes after the element kernel.  Which warp sums a
+// node never changes the order of the sum, so results are bit-identical to the unfused path.
+#define FUSE_DEPW 16    // ints per quad dependency record: [0] = number of chunks (<= 15), [1..] chunk ids
+#define FUSE_QPC 8      // quads a CTA can be given (two per warp)
 struct scatter_args {
-    const int *elist;                       // element ids in processing order: a colour's elements (MODE 1), the locality order
-                                            // built at setup for shuffled meshes (MODE 0); nullptr = identity
-    const int *eslot;                       // (MODE 0) [e*8+I] -> scratch record of block row I (node-sorted incidence index)
-    const int *nb_ptr;                      // node -> first neighbour block; CSR rows of node n start at 9*nb_ptr[n]
-    const unsigned char *elem_pos;          // [e][I][K] rank of node K in the neighbour list of node I
-    const unsigned long long *first_mask;   // bit I*8+K: store instead of add
-    const unsigned int *first_res;          // bit I: store the residual instead of add
-    double *csr_vals, *residual;
-    // MODE 2 (fused): countdown of missing contributions per node, queue of completed nodes, gather tables
-    int *cnt;
-    int *queue;
-    unsigned int *qctl;                     // [0] tail, [1] head
-    const int *inc_ptr;
+    const int *elist;   // element ids in processing order (the locality order built at setup for shuffled meshes); nullptr = identity
+    const int *eslot;   // [e*8+I] -> scratch record of block row I (node-sorted incidence index)
+    // fused gather
+    const int *cta_quads;          // [n_chunks*FUSE_QPC] quad ids given to the warps of chunk c (warp w: entries 2w, 2w+1), -1 = none
+    const int *quad_deps;          // [n_quads*FUSE_DEPW]
+    unsigned int *chunk_flag;      // [n_chunks] epoch of the last call in which the chunk's records were complete
+    unsigned int epoch;
+    int *left_list;                // quads that were not ready when their warp looked
+    unsigned int *left_count;
+    long long n_nodes;
+    const int *inc_ptr, *nb_ptr;
     const unsigned int *kvec;
+    double *csr_vals, *residual;
 };
 #ifndef EL_PF_DIST
 #define EL_PF_DIST 444   // L2 prefetch distance in chunks (one wave of CTAs): 3.135 -> 3.108 ms; 888 and 1776 gain nothing
 #endif
-#ifndef EL_PERSIST
-#define EL_PERSIST 0   // persistent CTAs with input prefetch measured slower (3.31 vs 3.13 ms): the CTAs of an SM stay in phase
-#endif
 // YLD 0: Hill-48 (scalar return map); YLD 1: Barlat Yld2004-18p (fem_barlat.cuh), bard = derived Barlat records
-template <int FBAR, int MODE, int YLD = 0>
+template <int FBAR, int FUSE, int YLD = 0>
 __global__ void __launch_bounds__(CTA_THREADS, (FBAR || YLD) ? CTAS_FBAR : CTAS_STD)
 k_element(long long n_elems, const double *__restrict__ coords, const int *__restrict__ conn,
           const double *__restrict__ u, const double *__restrict__ hist_in, const double *__restrict__ matd,
@@ -293,52 +265,29 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
     extern __shared__ __align__(16) double sm[];
     __shared__ unsigned int s_hist[64];
     __shared__ unsigned int s_done;
-    constexpr int ES = FBAR ? ES_FBAR : (MODE == 0 ? ES_STD : ES_STAGE);
+    constexpr int ES = FBAR ? ES_FBAR : (FUSE ? ES_FUSE : ES_STD);
     const int tid = threadIdx.x, lane = tid & 31, q = lane & 7;
     const int el_cta = tid >> 3;
-    long long chunk = blockIdx.x;
-    if (MODE == 2) {
-        // fused mode: every (GATHER_EVERY+1)-th CTA is a gather CTA: it claims nodes whose contributions are complete (queue
-        // filled by the element CTAs below) and assembles their CSR rows; it never waits for a node that is not in the queue
-        const unsigned bx = blockIdx.x, grp = bx / (GATHER_EVERY + 1);
-        if (bx - grp * (GATHER_EVERY + 1) == GATHER_EVERY) {
-            __shared__ unsigned s_qh, s_qn;
-            if (tid == 0) { unsigned h; s_qn = queue_claim(sa.qctl, GATHER_POP, h); s_qh = h; }
-            __syncthreads();
-            const unsigned qh = s_qh, qn = s_qn;
-            double *wbuf = sm + (tid >> 5) * 4 * (FBAR ? ES_FBAR : ES_STAGE);
-            for (unsigned base = 4u * (tid >> 5); base < qn; base += 4u * (CTA_THREADS / 32)) {
-                const int cnt = (int)min(4u, qn - base);
-                int nd = 0;
-                if (lane < cnt) nd = queue_read(sa.queue, qh + base + lane);
-                __threadfence();
-                gather_warp_nodes(nd, cnt, wbuf, lane, sa.inc_ptr, sa.nb_ptr, sa.kvec, Ke, Re, sa.csr_vals, sa.residual);
-            }
-            return;
-        }
-        chunk = bx - grp;
-    }
-    // MODE 0 is persistent: a CTA walks over the chunks blockIdx.x, blockIdx.x + gridDim.x, ... and loads the inputs of its
-    // next chunk while it works on the current one (connectivity at the top of the iteration, nodal data and history just
-    // before the tensor-core phase, where few registers are live), so no warp waits for the conn -> coords/u chain.
-    constexpr bool PERSIST = (MODE == 0) && EL_PERSIST;
-    const long long n_chunks = (n_elems + EL_PER_CTA - 1) / EL_PER_CTA;
+    const long long chunk = blockIdx.x;
     double *se = sm + el_cta * ES;
-    int nd_n, slot_n = 0;
-    double xn[3], un[3], hn[7];
+    const long long e_raw = chunk * EL_PER_CTA + el_cta;
+    const bool valid = e_raw < n_elems;
+    const long long e_slot = valid ? e_raw : n_elems - 1;
+    const long long e = sa.elist ? (long long)sa.elist[e_slot] : e_slot;
+    // ---- S2 gather: thread q loads node q of its element and the history of its Gauss point
+    const int my_node = conn[e * 8 + q];
+    const int my_slot = __ldg(sa.eslot + e * 8 + q);
+    double epn[6], xn[3], un[3];
     {
-        const long long er = chunk * EL_PER_CTA + el_cta, es = (er < n_elems) ? er : n_elems - 1;
-        const long long e0 = (MODE != 2 && sa.elist) ? (long long)sa.elist[es] : es;
-        nd_n = conn[e0 * 8 + q];
-        if (MODE != 1) slot_n = __ldg(sa.eslot + e0 * 8 + q);
-        const double *hin = hist_in + (e0 * 8 + q) * 7;
+        const double *hin = hist_in + (e * 8 + q) * 7;
 #pragma unroll
-        for (int i = 0; i < 7; i++) hn[i] = __ldg(hin + i);
-#pragma unroll
-        for (int i = 0; i < 3; i++) { xn[i] = coords[3 * (long long)nd_n + i]; un[i] = u[3 * (long long)nd_n + i]; }
+        for (int i = 0; i < 6; i++) epn[i] = __ldg(hin + i);
     }
+    const double alphan = __ldg(hist_in + (e * 8 + q) * 7 + 6);
+#pragma unroll
+    for (int i = 0; i < 3; i++) { xn[i] = coords[3 * (long long)my_node + i]; un[i] = u[3 * (long long)my_node + i]; }
 #if EL_PF_DIST > 0
-    if (MODE == 0) {   // streaming inputs of the chunk EL_PF_DIST launches ahead -> L2 (they are read exactly once)
+    {   // streaming inputs of the chunk EL_PF_DIST launches ahead -> L2 (they are read exactly once)
         const long long ep = (chunk + EL_PF_DIST) * EL_PER_CTA + el_cta;
         if (ep < n_elems && !sa.elist) {
             asm volatile("prefetch.global.L2 [%0];" ::"l"(conn + ep * 8 + q));
@@ -350,29 +299,32 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
 #endif
     for (int j = tid; j < 64; j += CTA_THREADS) s_hist[j] = 0;
     if (tid == 0) s_done = 0;
+    if (FUSE) {
+        // ---- S14 for the quads this warp was given at setup, while its own inputs are on their way: the records of those
+        //      nodes were written by chunks launched at least FUSE_LAG chunks ago and are read back from L2
+        double *wbuf = sm + (tid >> 5) * 4 * ES;     // the warp's four element slots (>= 4 x 576 doubles), not yet in use
+#pragma unroll 1
+        for (int k = 0; k < 2; k++) {
+            const int quad = __ldg(sa.cta_quads + chunk * FUSE_QPC + 2 * (tid >> 5) + k);
+            if (quad < 0) continue;                  // warp-uniform
+            const int *dep = sa.quad_deps + (long long)quad * FUSE_DEPW;
+            const int nd = __ldg(dep);
+            bool ok = true;
+            if (lane < nd) ok = (*reinterpret_cast<volatile unsigned int *>(sa.chunk_flag + __ldg(dep + 1 + lane)) == sa.epoch);
+            if (__all_sync(0xffffffffu, ok)) {
+                __threadfence();                     // the flags were read before any record is
+                const long long n0 = 4LL * quad;
+                const int cnt = (int)min(4LL, sa.n_nodes - n0);
+                gather_warp_nodes((int)n0 + lane, cnt, wbuf, lane, sa.inc_ptr, sa.nb_ptr, sa.kvec, Ke, Re, sa.csr_vals, sa.residual);
+            } else if (lane == 0) {
+                sa.left_list[atomicAdd(sa.left_count, 1u)] = quad;
+            }
+        }
+    }
     __syncthreads();
-  for (;;) {
-    const long long e_raw = chunk * EL_PER_CTA + el_cta;
-    const bool valid = e_raw < n_elems;
-    const long long e_slot = valid ? e_raw : n_elems - 1;
-    const long long e = (MODE != 2 && sa.elist) ? (long long)sa.elist[e_slot] : e_slot;
-    // ---- S2 gather: thread q holds node q of its element (prefetched), history of its Gauss point
-    double epn[6];
-#pragma unroll
-    for (int i = 0; i < 6; i++) epn[i] = hn[i];
-    const double alphan = hn[6];
-    const int my_node = nd_n, my_slot = slot_n;
+  {
 #pragma unroll
     for (int i = 0; i < 3; i++) { se[SM_XE + 3 * q + i] = xn[i]; se[SM_UE + 3 * q + i] = un[i]; }
-    const long long chunk_next = chunk + gridDim.x;
-    const bool has_next = PERSIST && chunk_next < n_chunks;
-    long long e_next = 0;
-    if (has_next) {
-        const long long er = chunk_next * EL_PER_CTA + el_cta;
-        e_next = (er < n_elems) ? er : n_elems - 1;
-        nd_n = conn[e_next * 8 + q];
-        slot_n = __ldg(sa.eslot + e_next * 8 + q);
-    }
     __syncwarp();
 
     // ---- S1 shape gradients at this Gauss point (O1): Jr = sum X_I (x) dN_I/dxi, G_I = dN_I/dxi Jr^-1, w = det Jr
@@ -988,13 +940,6 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
     }
     __syncwarp();
 
-    if (has_next) {   // inputs of the next chunk: in flight during the tensor-core phase
-        const double *hin = hist_in + (e_next * 8 + q) * 7;
-#pragma unroll
-        for (int i = 0; i < 7; i++) hn[i] = __ldg(hin + i);
-#pragma unroll
-        for (int i = 0; i < 3; i++) { xn[i] = coords[3 * (long long)nd_n + i]; un[i] = u[3 * (long long)nd_n + i]; }
-    }
     PHASE_SYNC_N(8);
     // ---- S12 phase 2: K^e_(Ii)(Kk) = sum_q G^_Ia A^_(ia)(kb) G^_Kb (Eq.(37) :267) on the FP64 tensor-core path.
     //      For each component pair (i,k), i <= k, the 8x8 node matrix K^{ik}[I][K] = sum_{(q,a)} G^q_Ia H^{ik}_{(q,a),K} with
@@ -1005,17 +950,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
     //      sm_100a, but one issue keeps the pipe busy for 16 cycles, so the contraction no longer stalls on
     //      dependent-issue latency, and the accumulators shrink from 45 to 12 doubles per thread.
     const int I = q;
-    double rq[(FBAR && MODE == 1) ? 8 : 1][3];
     if (FBAR) {
-#pragma unroll
-        for (int qq = 0; qq < ((MODE == 1) ? 8 : 0); qq++) {
-            const double *sq = se + qq;
-            const double gI[3] = {sq[GGX(I, 0)], sq[GGX(I, 1)], sq[GGX(I, 2)]};
-#pragma unroll
-            for (int i = 0; i < 3; i++)
-                rq[(FBAR && MODE == 1) ? qq : 0][i] = sq[SM_YY + (3 * i + 0) * 8] * gI[0] + sq[SM_YY + (3 * i + 1) * 8] * gI[1] +
-                                       sq[SM_YY + (3 * i + 2) * 8] * gI[2];
-        }
         // gbar_Kk = sum_q (w_q J_q / (Jbar V)) g^q_Kk for node K = I
 #pragma unroll
         for (int k = 0; k < 3; k++) {
@@ -1061,8 +996,8 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
                                          : "+d"(C[p][0]), "+d"(C[p][1]) : "d"(g[h][a_]), "d"(hv));
                         }
                 }
-            if (MODE != 1) {
-                // ---- phase 3 (scratch modes): the accumulators go straight to the destination-major scratch.
+            {
+                // ---- phase 3: the accumulators go straight to the destination-major scratch.
                 //      Lane holds K^{ik}[gid][2 tig + j] = component (i,k) of block (gid, 2 tig + j): one 16-byte store into block
                 //      row gid.  Standard element: for i != k it is also component (k,i) of block (2 tig + j, gid): two 8-byte
                 //      stores (the 8 lanes of equal tig fill 64 contiguous bytes).  Every 32-byte sector is written whole.
@@ -1136,110 +1071,17 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
                                 *reinterpret_cast<double2 *>(Ke + sd * 72 + (3 * i + k) * 8 + 2 * tig) = make_double2(D[i][k][0], D[i][k][1]);
                     }
                 }
-            } else {
-                __syncwarp();   // every lane has read this element's G^ and A^: the staging below overlays them
-                // ---- phase 3 (F-bar, coloured mode): stage the full K^e (8 block-row records [I][72], scratch record layout)
-                int p = 0;
-#pragma unroll
-                for (int i = 0; i < 3; i++)
-#pragma unroll
-                    for (int k = i; k < 3; k++, p++)
-#pragma unroll
-                        for (int j = 0; j < 2; j++) {
-                            const int K = 2 * tig + j;
-                            sx[KSX(gid, K, 3 * i + k)] = C[p][j];
-                            if (i != k) sx[KSX(K, gid, 3 * k + i)] = C[p][j];
-                        }
             }
         }
         __syncwarp();
     }
     PHASE_SYNC_N(9);
-    if (FBAR && MODE == 1) {
-        // K^e_(Ii)(Kk) += sum_q w_q/3 r^q_Ii (gbar_Kk - g^q_Kk)   (unsymmetric rank-1 terms)
-        double rs[3] = {0, 0, 0};
-#pragma unroll
-        for (int qq = 0; qq < 8; qq++)
-#pragma unroll
-            for (int i = 0; i < 3; i++) rs[i] += rq[(FBAR && MODE == 1) ? qq : 0][i];
-#pragma unroll 1
-        for (int K = 0; K < 8; K++)
-#pragma unroll
-            for (int k = 0; k < 3; k++) {
-                const double gb = se[SM_GB + 3 * K + k];
-                double t0 = rs[0] * gb, t1 = rs[1] * gb, t2 = rs[2] * gb;
-#pragma unroll
-                for (int qq = 0; qq < 8; qq++) {
-                    const double g = se[SM_GQ + (3 * K + k) * 8 + qq];
-                    t0 = fma(-rq[(FBAR && MODE == 1) ? qq : 0][0], g, t0); t1 = fma(-rq[(FBAR && MODE == 1) ? qq : 0][1], g, t1);
-                    t2 = fma(-rq[(FBAR && MODE == 1) ? qq : 0][2], g, t2);
-                }
-                se[KSX(I, K, 0 + k)] += t0;
-                se[KSX(I, K, 3 + k)] += t1;
-                se[KSX(I, K, 6 + k)] += t2;
-            }
-    }
-    if (MODE != 1) {
+    {
         // destination-major scratch: block row I of K^e and R^e_I go to the record of incidence entry (e,I) in the node-sorted
-        // list, so that the gather kernel reads every node's contributions as one contiguous run
+        // list, so that a gathering warp reads every node's contributions as one contiguous run
         if (valid) {
             double *ro = Re + (long long)my_slot * 3;
             ro[0] = rI[0]; ro[1] = rI[1]; ro[2] = rI[2];
-        }
-        __syncwarp();
-        if (MODE == 2) {
-            // publish: the records above become visible (fence), then each (element, node) counts its node down; whoever
-            // brings a node to zero queues it for the gather CTAs (one ticket request per warp)
-            __threadfence();
-            __syncwarp();
-            __threadfence();
-            const bool last = valid && (atomicSub(&sa.cnt[my_node], 1) == 1);
-            const unsigned mk = __ballot_sync(0xffffffffu, last);
-            if (mk) {
-                const int leader = __ffs(mk) - 1;
-                unsigned base = 0;
-                if (lane == leader) base = atomicAdd(&sa.qctl[0], (unsigned)__popc(mk));
-                base = __shfl_sync(0xffffffffu, base, leader);
-                if (last) {
-                    __threadfence();
-                    *reinterpret_cast<volatile int *>(sa.queue + base + __popc(mk & ((1u << lane) - 1u))) = my_node;
-                }
-            }
-        }
-    }
-    if (MODE == 1) {
-        // ---- S14 in-place assembly (Eq.(34) :253, Eq.(38) :274): no other element of this launch touches this element's
-        //      nodes, so plain read-modify-write is race-free; launches run in colour order => fixed summation order.
-        //      The first contributor of a block (marked at setup) stores, so the outputs need no zero-fill.
-        const int nbI = sa.nb_ptr[my_node], lenI = sa.nb_ptr[my_node + 1] - nbI;
-        const uint2 posI = reinterpret_cast<const uint2 *>(sa.elem_pos)[e * 8 + I];   // bytes pos(I,K), K = 0..7
-        const unsigned long long fm = sa.first_mask[e];
-        const unsigned fr = sa.first_res[e];
-        double *const rowsI = sa.csr_vals + 9LL * nbI;
-        {
-            __syncwarp();
-#pragma unroll 1
-            for (int K = 0; K < 8; K++) {
-                const int pIK = (int)(((K < 4) ? (posI.x >> (8 * K)) : (posI.y >> (8 * (K - 4)))) & 0xffu);
-                const bool first = (fm >> (I * 8 + K)) & 1ull;
-                if (valid) {
-#pragma unroll
-                    for (int i = 0; i < 3; i++) {
-                        double *a = rowsI + (long long)i * 3 * lenI + 3 * pIK;
-#pragma unroll
-                        for (int k = 0; k < 3; k++) {
-                            const double v = se[KSX(I, K, 3 * i + k)];
-                            a[k] = first ? v : a[k] + v;
-                        }
-                    }
-                }
-            }
-        }
-        if (valid) {
-            double *ro = sa.residual + 3LL * my_node;
-            const bool firstr = (fr >> I) & 1u;
-#pragma unroll
-            for (int i = 0; i < 3; i++) ro[i] = firstr ? rI[i] : ro[i] + rI[i];
         }
     }
 
@@ -1257,10 +1099,13 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
         }
         if (valid && plastic) atomicAdd(&s_hist[iters < 63 ? iters : 63], 1u);
     }
-    if (!has_next) break;
-    chunk = chunk_next;
-    __syncwarp();   // the next iteration overwrites this warp's shared-memory regions
   }
+    if (FUSE) {
+        // publish: every thread's records are visible device-wide (fence) before the chunk's flag takes this call's epoch
+        __threadfence();
+        __syncthreads();
+        if (tid == 0) *reinterpret_cast<volatile unsigned int *>(sa.chunk_flag + chunk) = sa.epoch;
+    }
     {
         __syncwarp();
         unsigned done = 0;
@@ -1362,36 +1207,48 @@ k_gather_fast(long long n_nodes, const int *__restrict__ inc_ptr, const int *__r
     gather_reduce_write(n, b, m, buf[w], lane, nb_ptr, kvec, Re, csr_vals, residual);
 }
 
-// Fused mode, after the element kernel: persistent CTAs drain what is left in the queue of completed nodes (every node is
-// in it by now).  4 warps x 4 nodes per batch.
-__global__ void __launch_bounds__(128)
-k_gather_drain(unsigned int n_nodes, const int *__restrict__ queue, unsigned int *qctl, const int *__restrict__ inc_ptr,
-               const int *__restrict__ nb_ptr, const unsigned int *__restrict__ kvec, const double *__restrict__ Ke,
-               const double *__restrict__ Re, double *__restrict__ csr_vals, double *__restrict__ residual) {
+// After a fused element launch: the quads that no element warp gathered (scheduled past the last chunk: `tail`, fixed at
+// setup; not ready when their warp looked: `left`, counted during the launch).  Every chunk has retired by now (stream
+// order), so no flag is read.  4 warps x 4 nodes per CTA, grid-stride.
+#define GL_WARPS 4
+__global__ void __launch_bounds__(GL_WARPS * 32)
+k_gather_list(long long n_nodes, const int *__restrict__ tail, int n_tail, const int *__restrict__ left,
+              const unsigned int *__restrict__ left_count, const int *__restrict__ inc_ptr, const int *__restrict__ nb_ptr,
+              const unsigned int *__restrict__ kvec, const double *__restrict__ Ke, const double *__restrict__ Re,
+              double *__restrict__ csr_vals, double *__restrict__ residual) {
     extern __shared__ __align__(16) double dbuf[];
-    __shared__ unsigned s_h;
     const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    for (;;) {
-        if (threadIdx.x == 0) s_h = atomicAdd(&qctl[1], 16u);
-        __syncthreads();
-        const unsigned h = s_h;
-        __syncthreads();
-        if (h >= n_nodes) return;
-        const unsigned base = h + 4u * w;
-        if (base >= n_nodes) continue;
-        const int cnt = (int)min(4u, n_nodes - base);
-        int nd = 0;
-        if (lane < cnt) nd = queue[base + lane];
-        gather_warp_nodes(nd, cnt, dbuf + w * 2304, lane, inc_ptr, nb_ptr, kvec, Ke, Re, csr_vals, residual);
+    const long long total = (long long)n_tail + (long long)*left_count;
+    for (long long it = (long long)blockIdx.x * GL_WARPS + w; it < total; it += (long long)gridDim.x * GL_WARPS) {
+        const int quad = (it < n_tail) ? tail[it] : left[it - n_tail];
+        const long long n0 = 4LL * quad;
+        const int cnt = (int)min(4LL, n_nodes - n0);
+        gather_warp_nodes((int)n0 + lane, cnt, dbuf + w * 2304, lane, inc_ptr, nb_ptr, kvec, Ke, Re, csr_vals, residual);
     }
 }
 
 // ------------------------------------------------------------------------------------------------ launch
 static inline unsigned nblk2(long long n, int bs) { return (unsigned)((n + bs - 1) / bs); }
 
+template <int FBAR, int FUSE, int YLD>
+static int launch_element(fem_ctx *c, const double *u, const double *hist_in, int mstride, double *hist_out, const scatter_args &sa,
+                          int bstride, cudaStream_t st) {
+    constexpr int ES = FBAR ? ES_FBAR : (FUSE ? ES_FUSE : ES_STD);
+    const size_t smem = (size_t)EL_PER_CTA * ES * sizeof(double);
+    // the opt-in for > 48 KB of dynamic shared memory is per device and per kernel: remembered per context (= per device)
+    const int slot = (FBAR ? 1 : 0) + 2 * (FUSE ? 1 : 0) + 4 * (YLD ? 1 : 0);
+    if (!(c->attr_mask & (1u << slot))) {
+        FEM_CUDA(cudaFuncSetAttribute(k_element<FBAR, FUSE, YLD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        c->attr_mask |= 1u << slot;
+    }
+    k_element<FBAR, FUSE, YLD><<<nblk2(c->n_elems, EL_PER_CTA), CTA_THREADS, smem, st>>>(
+        c->n_elems, c->d_coords, c->d_conn, u, hist_in, c->d_matd, mstride, c->opt.tol, c->opt.kmax, c->d_Ke, c->d_Re, hist_out,
+        c->d_stats, sa, YLD ? c->d_bard : nullptr, bstride);
+    return FEM_OK;
+}
+
 int fem_launch_assemble(fem_ctx *c, const double *u, const double *hist_in, const double *mat, long long n_mat,
                         double *residual, double *csr_vals, double *hist_out, cudaStream_t st, const double *bar) {
-    if (bar && c->mode != 0) return FEM_ERR_ARG;   // Yld2004-18p runs in assembly mode 0 only
     if (bar && n_mat > c->n_bard_cap) {
         if (c->d_bard) cudaFree(c->d_bard);
         c->d_bard = nullptr; c->n_bard_cap = 0;
@@ -1404,114 +1261,50 @@ int fem_launch_assemble(fem_ctx *c, const double *u, const double *hist_in, cons
         FEM_CUDA(cudaMalloc(&c->d_matd, sizeof(double) * FEM_MATD * n_mat));
         c->n_matd_cap = n_mat;
     }
-    static bool attr_set = false;
-    const size_t sm_std = EL_PER_CTA * ES_STD * sizeof(double), sm_stage = EL_PER_CTA * ES_STAGE * sizeof(double),
-                 sm_fbar = EL_PER_CTA * ES_FBAR * sizeof(double);
-    if (!attr_set) {
-        FEM_CUDA(cudaFuncSetAttribute(k_element<0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_std));
-        FEM_CUDA(cudaFuncSetAttribute(k_element<0, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_stage));
-        FEM_CUDA(cudaFuncSetAttribute(k_element<1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_fbar));
-        FEM_CUDA(cudaFuncSetAttribute(k_element<1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_fbar));
-        attr_set = true;
-    }
+    const bool fuse = c->fuse_ok && c->opt.assembly_mode == 0;
     FEM_CUDA(cudaMemsetAsync(c->d_stats, 0, sizeof(unsigned long long) * 72, st));
+    if (fuse) FEM_CUDA(cudaMemsetAsync(c->d_left_count, 0, sizeof(unsigned int), st));
     FEM_CUDA(cudaEventRecord(c->ev[0], st));
     k_mat_prep<<<nblk2(n_mat, 128), 128, 0, st>>>(n_mat, mat, c->d_matd);
-    if (bar) k_bar_prep<<<nblk2(n_mat, 128), 128, 0, st>>>(n_mat, bar, c->d_bard);
+    if (bar) {
+        k_bar_prep<<<nblk2(n_mat, 128), 128, 0, st>>>(n_mat, bar, c->d_bard, c->d_stats + 69);
+    }
     FEM_CUDA(cudaEventRecord(c->ev[1], st));
-    const int mstride = (n_mat == 1) ? 0 : FEM_MATD;
-    scatter_args sa = {c->mode == 0 ? c->d_eorder : nullptr, c->d_eslot, c->d_nb_ptr, c->d_elem_pos, c->d_first_mask, c->d_first_res, csr_vals, residual,
-                       c->d_cnt, c->d_queue, c->d_qctl, c->d_inc_ptr, c->d_kvec};
-    if (c->mode == 2) {
-        // fused mode: element CTAs count the nodes down and queue completed ones; interleaved gather CTAs and the drain
-        // kernel assemble them.  Per call: reset the countdown, the queue (nodes without elements are pre-queued) and its counters.
-        static bool attr2 = false;
-        if (!attr2) {
-            FEM_CUDA(cudaFuncSetAttribute(k_element<0, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_stage));
-            FEM_CUDA(cudaFuncSetAttribute(k_element<1, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_fbar));
-            FEM_CUDA(cudaFuncSetAttribute(k_gather_drain, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * 2304 * 8));
-            attr2 = true;
+    const int mstride = (n_mat == 1) ? 0 : FEM_MATD, bstride = (n_mat == 1) ? 0 : FEM_BARD;
+    c->epoch++;
+    if (c->epoch == 0) c->epoch = 1;   // the flags start at 0
+    scatter_args sa = {c->d_eorder, c->d_eslot, c->d_cta_quads, c->d_quad_deps, c->d_chunk_flag, c->epoch, c->d_left_list,
+                       c->d_left_count, c->n_nodes, c->d_inc_ptr, c->d_nb_ptr, c->d_kvec, csr_vals, residual};
+    int rc;
+    if (bar)       rc = c->opt.fbar ? (fuse ? launch_element<1, 1, 1>(c, u, hist_in, mstride, hist_out, sa, bstride, st)
+                                            : launch_element<1, 0, 1>(c, u, hist_in, mstride, hist_out, sa, bstride, st))
+                                    : (fuse ? launch_element<0, 1, 1>(c, u, hist_in, mstride, hist_out, sa, bstride, st)
+                                            : launch_element<0, 0, 1>(c, u, hist_in, mstride, hist_out, sa, bstride, st));
+    else           rc = c->opt.fbar ? (fuse ? launch_element<1, 1, 0>(c, u, hist_in, mstride, hist_out, sa, 0, st)
+                                            : launch_element<1, 0, 0>(c, u, hist_in, mstride, hist_out, sa, 0, st))
+                                    : (fuse ? launch_element<0, 1, 0>(c, u, hist_in, mstride, hist_out, sa, 0, st)
+                                            : launch_element<0, 0, 0>(c, u, hist_in, mstride, hist_out, sa, 0, st));
+    if (rc != FEM_OK) return rc;
+    FEM_CUDA(cudaEventRecord(c->ev[2], st));
+    if (fuse) {
+        if (!(c->attr_mask & (1u << 8))) {
+            FEM_CUDA(cudaFuncSetAttribute(k_gather_list, cudaFuncAttributeMaxDynamicSharedMemorySize, GL_WARPS * 2304 * 8));
+            c->attr_mask |= 1u << 8;
         }
-        FEM_CUDA(cudaMemcpyAsync(c->d_cnt, c->d_cnt_init, sizeof(int) * c->n_nodes, cudaMemcpyDeviceToDevice, st));
-        FEM_CUDA(cudaMemcpyAsync(c->d_queue, c->d_queue_init, sizeof(int) * c->n_nodes, cudaMemcpyDeviceToDevice, st));
-        FEM_CUDA(cudaMemcpyAsync(c->d_qctl, c->d_qctl + 2, sizeof(unsigned int) * 2, cudaMemcpyDeviceToDevice, st));   // tail = isolated nodes, head = 0
-        const long long nE = (c->n_elems + EL_PER_CTA - 1) / EL_PER_CTA;
-        const unsigned grid = (unsigned)(nE + (nE + GATHER_EVERY - 1) / GATHER_EVERY);   // element CTAs + one gather CTA per GATHER_EVERY
-        if (c->opt.fbar)
-            k_element<1, 2><<<grid, CTA_THREADS, sm_fbar, st>>>(c->n_elems, c->d_coords, c->d_conn, u, hist_in, c->d_matd, mstride,
-                                                        c->opt.tol, c->opt.kmax, c->d_Ke, c->d_Re, hist_out, c->d_stats, sa);
+        // the tail is known; what was left over is counted on the device: a fixed grid walks both lists
+        k_gather_list<<<2 * c->n_sm, GL_WARPS * 32, GL_WARPS * 2304 * 8, st>>>(c->n_nodes, c->d_tail_quads, c->n_tail_quads, c->d_left_list,
+                                                                          c->d_left_count, c->d_inc_ptr, c->d_nb_ptr, c->d_kvec, c->d_Ke,
+                                                                          c->d_Re, csr_vals, residual);
+    } else if (c->d_kvec) {   // no collapsed element: the table-driven gather (nodes with more than 8 elements take its general path)
+        if (c->has_high_valence)
+            k_gather_fast<1><<<nblk2(c->n_nodes, GW), GW * 32, 0, st>>>(c->n_nodes, c->d_inc_ptr, c->d_inc, c->d_nb_ptr, c->d_kvec,
+                                                                     c->d_elem_pos, c->d_Ke, c->d_Re, csr_vals, residual);
         else
-            k_element<0, 2><<<grid, CTA_THREADS, sm_stage, st>>>(c->n_elems, c->d_coords, c->d_conn, u, hist_in, c->d_matd, mstride,
-                                                       c->opt.tol, c->opt.kmax, c->d_Ke, c->d_Re, hist_out, c->d_stats, sa);
-        FEM_CUDA(cudaEventRecord(c->ev[2], st));
-        int dev = 0, nsm = 148;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
-        k_gather_drain<<<3 * nsm, 128, 4 * 2304 * 8, st>>>((unsigned)c->n_nodes, c->d_queue, c->d_qctl, c->d_inc_ptr, c->d_nb_ptr, c->d_kvec,
-                                                        c->d_Ke, c->d_Re, csr_vals, residual);
-    } else
-    if (c->mode == 1) {
-        // one launch per colour, in colour order (stream order = summation order)
-        for (int k = 0; k < c->n_colours; k++) {
-            const long long cnt = c->colour_start[k + 1] - c->colour_start[k];
-            sa.elist = c->d_elist + c->colour_start[k];
-            const unsigned grid = nblk2(cnt, EL_PER_CTA);
-            if (c->opt.fbar)
-                k_element<1, 1><<<grid, CTA_THREADS, sm_fbar, st>>>(cnt, c->d_coords, c->d_conn, u, hist_in, c->d_matd, mstride, c->opt.tol,
-                                                            c->opt.kmax, nullptr, nullptr, hist_out, c->d_stats, sa);
-            else
-                k_element<0, 1><<<grid, CTA_THREADS, sm_stage, st>>>(cnt, c->d_coords, c->d_conn, u, hist_in, c->d_matd, mstride, c->opt.tol,
-                                                           c->opt.kmax, nullptr, nullptr, hist_out, c->d_stats, sa);
-        }
-        FEM_CUDA(cudaEventRecord(c->ev[2], st));
+            k_gather_fast<0><<<nblk2(c->n_nodes, GW), GW * 32, 0, st>>>(c->n_nodes, c->d_inc_ptr, c->d_inc, c->d_nb_ptr, c->d_kvec,
+                                                                     c->d_elem_pos, c->d_Ke, c->d_Re, csr_vals, residual);
     } else {
-        // persistent CTAs: one wave (resident CTAs per SM x SMs), each walks over its chunks
-        static int wave[2] = {0, 0};
-        if (!wave[0]) {
-            int dev = 0, nsm = 148, per = 1;
-            cudaGetDevice(&dev);
-            cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
-            FEM_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, k_element<0, 0>, CTA_THREADS, sm_std));
-            wave[0] = (per > 0 ? per : 1) * nsm;
-            FEM_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, k_element<1, 0>, CTA_THREADS, sm_fbar));
-            wave[1] = (per > 0 ? per : 1) * nsm;
-        }
-        const unsigned n_chunks = nblk2(c->n_elems, EL_PER_CTA);
-        const unsigned grid = (!EL_PERSIST || n_chunks < (unsigned)wave[c->opt.fbar ? 1 : 0]) ? n_chunks : (unsigned)wave[c->opt.fbar ? 1 : 0];
-        if (bar) {
-            static bool attr3 = false;
-            if (!attr3) {
-                FEM_CUDA(cudaFuncSetAttribute(k_element<0, 0, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_std));
-                FEM_CUDA(cudaFuncSetAttribute(k_element<1, 0, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_fbar));
-                attr3 = true;
-            }
-            const int bstride = (n_mat == 1) ? 0 : FEM_BARD;
-            if (c->opt.fbar)
-                k_element<1, 0, 1><<<n_chunks, CTA_THREADS, sm_fbar, st>>>(c->n_elems, c->d_coords, c->d_conn, u, hist_in, c->d_matd, mstride,
-                                                                   c->opt.tol, c->opt.kmax, c->d_Ke, c->d_Re, hist_out, c->d_stats, sa,
-                                                                   c->d_bard, bstride);
-            else
-                k_element<0, 0, 1><<<n_chunks, CTA_THREADS, sm_std, st>>>(c->n_elems, c->d_coords, c->d_conn, u, hist_in, c->d_matd, mstride,
-                                                                  c->opt.tol, c->opt.kmax, c->d_Ke, c->d_Re, hist_out, c->d_stats, sa,
-                                                                  c->d_bard, bstride);
-        } else
-        if (c->opt.fbar)
-            k_element<1, 0><<<grid, CTA_THREADS, sm_fbar, st>>>(c->n_elems, c->d_coords, c->d_conn, u, hist_in, c->d_matd, mstride,
-                                                        c->opt.tol, c->opt.kmax, c->d_Ke, c->d_Re, hist_out, c->d_stats, sa);
-        else
-            k_element<0, 0><<<grid, CTA_THREADS, sm_std, st>>>(c->n_elems, c->d_coords, c->d_conn, u, hist_in, c->d_matd, mstride,
-                                                       c->opt.tol, c->opt.kmax, c->d_Ke, c->d_Re, hist_out, c->d_stats, sa);
-        FEM_CUDA(cudaEventRecord(c->ev[2], st));
-        if (c->d_kvec)   // every node has <= 8 incident elements, no collapsed element
-            if (c->has_high_valence)
-                k_gather_fast<1><<<nblk2(c->n_nodes, GW), GW * 32, 0, st>>>(c->n_nodes, c->d_inc_ptr, c->d_inc, c->d_nb_ptr, c->d_kvec,
-                                                                         c->d_elem_pos, c->d_Ke, c->d_Re, csr_vals, residual);
-            else
-                k_gather_fast<0><<<nblk2(c->n_nodes, GW), GW * 32, 0, st>>>(c->n_nodes, c->d_inc_ptr, c->d_inc, c->d_nb_ptr, c->d_kvec,
-                                                                         c->d_elem_pos, c->d_Ke, c->d_Re, csr_vals, residual);
-        else
-            k_gather<<<nblk2(c->n_nodes * 32, 256), 256, 0, st>>>(c->n_nodes, c->d_inc_ptr, c->d_inc, c->d_nb_ptr, c->d_elem_pos, c->d_Ke,
-                                                                 c->d_Re, csr_vals, residual);
+        k_gather<<<nblk2(c->n_nodes * 32, 256), 256, 0, st>>>(c->n_nodes, c->d_inc_ptr, c->d_inc, c->d_nb_ptr, c->d_elem_pos, c->d_Ke,
+                                                             c->d_Re, csr_vals, residual);
     }
     FEM_CUDA(cudaEventRecord(c->ev[3], st));
     FEM_CUDA(cudaGetLastError());

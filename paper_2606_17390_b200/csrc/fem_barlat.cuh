@@ -20,7 +20,10 @@
 #define BAR_START 1
 #endif
 
-__global__ void k_bar_prep(long long n_mat, const double *__restrict__ bar, double *__restrict__ bd) {
+// bad_m: counts records whose exponent is not an even integer in 2..BAR_MMAX; such an exponent is replaced by the nearest
+// supported one so that the tables indexed by m (BAR_MMAX + 1 entries) are never overrun; fem_assemble_barlat reports
+// FEM_ERR_ARG when the counter is non-zero and the caller asked for statistics.
+__global__ void k_bar_prep(long long n_mat, const double *__restrict__ bar, double *__restrict__ bd, unsigned long long *bad_m) {
     long long r = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (r >= n_mat) return;
     const double *p = bar + r * FEM_NBARLAT;
@@ -37,7 +40,16 @@ __global__ void k_bar_prep(long long n_mat, const double *__restrict__ bar, doub
             }
         o[12 * t + 9] = c[6]; o[12 * t + 10] = c[7]; o[12 * t + 11] = c[8];
     }
-    o[24] = p[18];
+    {
+        double m = p[18];
+        const bool ok = (m >= 2.0) && (m <= (double)BAR_MMAX) && (m == 2.0 * floor(0.5 * m));
+        if (!ok) {
+            atomicAdd(bad_m, 1ull);
+            m = 2.0 * rint(0.5 * (isfinite(m) ? m : 2.0));
+            m = fmin(fmax(m, 2.0), (double)BAR_MMAX);
+        }
+        o[24] = m;
+    }
     for (int i = 25; i < FEM_BARD; i++) o[i] = 0.0;
 }
 

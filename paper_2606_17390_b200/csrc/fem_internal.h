@@ -26,22 +26,21 @@ struct fem_ctx {
     unsigned char *d_elem_pos = nullptr;  // [n_elems*64]  pos(conn[e][I], conn[e][K]) = rank of node K in nb list of node I
     int *d_elem_slot = nullptr;  // [n_elems*576], built on request
     unsigned int *d_kvec = nullptr;  // [nnz/9] per node-pair block: nibble s = local node K of the column node in incident entry s (0xF none); null if some node has > 8 elements
-    // colouring (assembly_mode 1): elements grouped by colour, first-writer masks
-    int *d_elist = nullptr;                       // [n_elems] element ids sorted by (colour, id)
-    unsigned long long *d_first_mask = nullptr;   // [n_elems] bit I*8+K: this element stores block (I,K) instead of adding
-    unsigned int *d_first_res = nullptr;          // [n_elems] bit I: this element stores the residual of its local node I
-    int mode = 0;                                 // effective assembly mode (1 and 2 fall back to 0 where they do not apply)
-    // fused mode (assembly_mode 2): per-node countdown of missing contributions + queue of completed nodes
-    int *d_cnt_init = nullptr;                    // [n_nodes] number of incident elements
-    int *d_cnt = nullptr;                         // [n_nodes] working copy, counted down by the element CTAs
-    int *d_queue_init = nullptr;                  // [n_nodes] nodes without elements first, then -1
-    int *d_queue = nullptr;                       // [n_nodes] working copy: node ids in order of completion
-    unsigned int *d_qctl = nullptr;               // [0] tail (tickets handed out), [1] head (entries claimed), [2..3] initial values
-    int n_isolated = 0;
+    // fused, lagged gather (fem_assemble.cu): node quads given to element warps at setup, chunk completion flags
+    bool fuse_ok = false;                         // the mesh qualifies (no collapsed element, no node with more than 8 elements)
+    int *d_cta_quads = nullptr;                   // [n_chunks*8] quad ids per chunk (two per warp), -1 = none
+    int *d_quad_deps = nullptr;                   // [n_quads*16] [0] = number of chunks contributing to the quad's nodes, then their ids
+    int *d_tail_quads = nullptr;                  // quads no element warp was given: gathered by k_gather_list after the element kernel
+    int n_tail_quads = 0;
+    unsigned int *d_chunk_flag = nullptr;         // [n_chunks] epoch of the last call in which the chunk finished
+    int *d_left_list = nullptr;                   // [n_quads] quads whose chunks had not all finished when their warp looked
+    unsigned int *d_left_count = nullptr;
+    unsigned int epoch = 0;
+    unsigned int attr_mask = 0;                   // kernels whose dynamic shared-memory opt-in has been set on this context's device
+    int n_sm = 148;
+    bool bad_barlat_m = false;                    // last fem_assemble_barlat saw an exponent outside the even integers 2..16
     bool has_high_valence = false;                // some node belongs to more than 8 elements
     bool has_collapsed = false;                   // some element lists a node twice
-    int n_colours = 0, colour_rounds = 0;
-    long long colour_start[65] = {0};
     // assemble workspace
     double *d_Ke = nullptr;      // [8*n_elems][72] destination-major scratch: record j = block row I of K^e of incidence entry j
                                  //   (node-sorted), component c of block (I,K) at (c>>1)*16 + 2K + (c&1) for c < 8, 64 + K for c = 8
@@ -62,6 +61,8 @@ struct fem_ctx {
     int mixed_precision = 0;
     double *d_nw_valsT = nullptr;  // [nnz] transposed stiffness values (adjoint step of the F-bar element), allocated on first use
     long long n_part = 0;
+    double *d_path = nullptr;      // [4*n_rows] fem_load_path: trial state, two previous converged states, boundary values of the step
+    double *d_path_hist = nullptr; // [n_elems*56] fem_load_path: second history buffer
     // NEXT-3 (fem_sens.cu): per-CTA partial sums of the material gradient (uniform material)
     double *d_sens_part = nullptr;
     long long n_sens_part = 0;
@@ -74,6 +75,12 @@ struct fem_ctx {
 
 extern char g_fem_cuda_err[512];
 int fem_cuda_fail(cudaError_t e, const char *where);
+static inline int fem_cuda_rc(cudaError_t e, const char *where) { return e == cudaSuccess ? FEM_OK : fem_cuda_fail(e, where); }
+// true when the byte ranges [a, a+bytes) and [b, b+bytes) intersect (hist_in / hist_out style aliasing checks)
+static inline bool fem_ranges_overlap(const void *a, const void *b, size_t bytes) {
+    const char *p = (const char *)a, *q = (const char *)b;
+    return p < q + bytes && q < p + bytes;
+}
 #define FEM_CUDA(call)                                                   \
     do {                                                                 \
         cudaError_t _e = (call);                                         \
@@ -82,8 +89,6 @@ int fem_cuda_fail(cudaError_t e, const char *where);
 
 // fem_api.cu
 int fem_read_stats(fem_ctx *c, fem_stats *stats, cudaStream_t st);
-// fem_colour.cu
-int fem_build_colouring(fem_ctx *c);
 // fem_assemble.cu
 int fem_launch_assemble(fem_ctx *c, const double *u, const double *hist_in, const double *mat, long long n_mat,
                         double *residual, double *csr_vals, double *hist_out, cudaStream_t st, const double *bar = nullptr);

@@ -170,13 +170,31 @@ __global__ void k_eslot(long long n_elems, const int *__restrict__ inc, int *esl
     if (j < 8 * n_elems) eslot[inc[j]] = (int)j;
 }
 
-// fused mode: countdown template and the queue template (nodes without elements are queued from the start)
-__global__ void k_cnt_init(long long n_nodes, const int *__restrict__ inc_ptr, int *cnt_init, int *queue_init, int *n_iso) {
-    long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    if (n >= n_nodes) return;
-    const int m = inc_ptr[n + 1] - inc_ptr[n];
-    cnt_init[n] = m;
-    if (m == 0) queue_init[atomicAdd(n_iso, 1)] = (int)n;
+// ---- fused, lagged gather (fem_assemble.cu): which chunks of the element launch write the records of a node quad
+// epos[e] = position of element e in the processing order (only when a locality order exists)
+__global__ void k_epos(long long n_elems, const int *__restrict__ eorder, int *epos) {
+    long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (i < n_elems) epos[eorder[i]] = (int)i;
+}
+// quad = nodes 4q .. 4q+3: deps[q*16] = number of distinct chunks (of el_per_cta consecutive elements of the processing
+// order) that hold an element of one of these nodes (-1: more than 15), deps[q*16+1..] their ids; ready[q] = the largest.
+__global__ void k_quad_deps(long long n_nodes, long long n_quads, int el_per_cta, const int *__restrict__ inc_ptr,
+                            const int *__restrict__ inc, const int *__restrict__ epos, int *deps, int *ready) {
+    long long qd = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (qd >= n_quads) return;
+    int list[15], cnt = 0, mx = -1;
+    bool over = false;
+    for (long long n = 4 * qd; n < 4 * qd + 4 && n < n_nodes; n++)
+        for (int s = inc_ptr[n]; s < inc_ptr[n + 1]; s++) {
+            const int e = inc[s] >> 3, ch = (epos ? epos[e] : e) / el_per_cta;
+            mx = max(mx, ch);
+            bool found = false;
+            for (int j = 0; j < cnt; j++) found |= (list[j] == ch);
+            if (!found) { if (cnt < 15) list[cnt++] = ch; else over = true; }
+        }
+    deps[qd * 16] = over ? -1 : cnt;
+    for (int j = 0; j < 15; j++) deps[qd * 16 + 1 + j] = (j < cnt) ? list[j] : 0;
+    ready[qd] = over ? 0x7fffffff : mx;
 }
 
 // kvec for the fast gather; flags |= 16 if some node has more than 8 incident elements
@@ -241,8 +259,8 @@ extern "C" int fem_hill_from_lankford(double r0, double r45, double r90, double 
 static void ctx_free(fem_ctx *c) {
     if (!c) return;
     void *ptrs[] = {c->d_coords, c->d_conn, c->d_inc_ptr, c->d_inc, c->d_nb_ptr, c->d_nb, c->d_row_ptr, c->d_col_idx,
-                    c->d_eslot, c->d_eorder, c->d_diagpos, c->d_sw, c->d_part, c->d_scal, c->d_nw, c->d_nw_vals, c->d_cnt_init, c->d_cnt, c->d_queue_init, c->d_queue, c->d_qctl, c->d_elem_pos, c->d_elem_slot, c->d_kvec, c->d_elist, c->d_first_mask, c->d_first_res, c->d_Ke, c->d_Re, c->d_matd, c->d_bard, c->d_stats, c->d_u, c->d_hin, c->d_hout,
-                    c->d_mat, c->d_res, c->d_vals, c->d_sens_part, c->d_nw_valsT, c->d_vals32};
+                    c->d_eslot, c->d_eorder, c->d_diagpos, c->d_sw, c->d_part, c->d_scal, c->d_nw, c->d_nw_vals, c->d_cta_quads, c->d_quad_deps, c->d_tail_quads, c->d_chunk_flag, c->d_left_list, c->d_left_count, c->d_elem_pos, c->d_elem_slot, c->d_kvec, c->d_Ke, c->d_Re, c->d_matd, c->d_bard, c->d_stats, c->d_u, c->d_hin, c->d_hout,
+                    c->d_mat, c->d_res, c->d_vals, c->d_sens_part, c->d_nw_valsT, c->d_vals32, c->d_path, c->d_path_hist};
     for (void *p : ptrs) if (p) cudaFree(p);
     for (int i = 0; i < 4; i++) if (c->ev[i]) cudaEventDestroy(c->ev[i]);
     delete c;
@@ -259,7 +277,7 @@ extern "C" int fem_setup(fem_ctx **out, long long n_nodes, const double *coords,
     fem_default_options(&o);
     if (opt) o = *opt;
     if (o.quad_order != 2) return FEM_ERR_QUAD;
-    if ((o.fbar != 0 && o.fbar != 1) || !(o.tol > 0) || o.kmax < 1 || (o.assembly_mode < 0 || o.assembly_mode > 2)) return FEM_ERR_ARG;
+    if ((o.fbar != 0 && o.fbar != 1) || !(o.tol > 0) || o.kmax < 1 || (o.assembly_mode < 0 || o.assembly_mode > 1)) return FEM_ERR_ARG;
     int ndev = 0;
     FEM_CUDA(cudaGetDeviceCount(&ndev));
     if (ndev < 1) { snprintf(g_fem_cuda_err, sizeof(g_fem_cuda_err), "no CUDA device"); return FEM_ERR_CUDA; }
@@ -281,7 +299,11 @@ extern "C" int fem_setup(fem_ctx **out, long long n_nodes, const double *coords,
         if (hflags & 1) { rc = FEM_ERR_CONN; break; }
         if (hflags & 2) { rc = FEM_ERR_INVERTED; break; }
         c->has_collapsed = (hflags & 8) != 0;
-        c->mode = (o.assembly_mode != 0 && !c->has_collapsed) ? o.assembly_mode : 0;   // modes 1, 2 need distinct nodes per element
+        {
+            int dev = 0;
+            TRY(cudaGetDevice(&dev));
+            TRY(cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, dev));
+        }
         TRY(cudaMalloc(&c->d_stats, sizeof(unsigned long long) * 72));
         for (int i = 0; i < 4; i++) TRY(cudaEventCreate(&c->ev[i]));
 #undef TRY
@@ -346,25 +368,8 @@ extern "C" int fem_build_csr_pattern(fem_ctx *c, long long *n_rows, long long *n
                 TRY(cudaMemcpy(&kf, dflags, sizeof(int), cudaMemcpyDeviceToHost));
                 c->has_high_valence = (kf & 16) != 0;   // some node has more than 8 elements: it is gathered by the general path
             }
-            if (c->mode == 2 && (!c->d_kvec || c->has_high_valence)) c->mode = 0;   // the fused mode buffers at most 8 records per node
-            if (c->mode == 2) {
-                TRY(cudaMalloc(&c->d_cnt_init, sizeof(int) * nn));
-                TRY(cudaMalloc(&c->d_cnt, sizeof(int) * nn));
-                TRY(cudaMalloc(&c->d_queue_init, sizeof(int) * nn));
-                TRY(cudaMalloc(&c->d_queue, sizeof(int) * nn));
-                TRY(cudaMalloc(&c->d_qctl, sizeof(unsigned int) * 4));   // [0..1] live tail/head, [2..3] their initial values
-                TRY(cudaMemset(c->d_queue_init, 0xff, sizeof(int) * nn));
-                TRY(cudaMemset(dflags, 0, sizeof(int)));
-                k_cnt_init<<<nblk(nn, 256), 256>>>(nn, c->d_inc_ptr, c->d_cnt_init, c->d_queue_init, dflags);
-                TRY(cudaMemcpy(&c->n_isolated, dflags, sizeof(int), cudaMemcpyDeviceToHost));
-                const unsigned int ctl0[4] = {0u, 0u, (unsigned)c->n_isolated, 0u};
-                TRY(cudaMemcpy(c->d_qctl, ctl0, sizeof(ctl0), cudaMemcpyHostToDevice));
-            }
             TRY(cudaDeviceSynchronize());
-            if (c->mode == 1) {
-                rc = fem_build_colouring(c);
-                if (rc != FEM_OK) break;
-            } else {   // scratch for the two-kernel mode (destination-major: one 72-double record per incidence entry)
+            {   // scratch (destination-major: one 72-double record per incidence entry)
                 {   // processing order: when more than 5 % of the elements step back in node numbering (shuffled input), the element
                     // kernel walks the elements by ascending smallest node id (neighbouring CTAs then share nodes in L2 and
                     // write neighbouring scratch records); results do not depend on it
@@ -392,6 +397,61 @@ extern "C" int fem_build_csr_pattern(fem_ctx *c, long long *n_rows, long long *n
                 TRY(cudaMalloc(&c->d_Ke, sizeof(double) * 576 * ne));
                 TRY(cudaMalloc(&c->d_Re, sizeof(double) * 24 * ne));
                 TRY(cudaDeviceSynchronize());
+            }
+            if (c->d_kvec && !c->has_high_valence) {
+                // fused, lagged gather: give every node quad to a warp of a chunk launched FUSE lag chunks after the last
+                // chunk that writes one of its records (one wave of resident CTAs + a margin), at most two quads per warp
+                const int EPC = 16, QPC = 8;                      // elements per CTA (fem_assemble.cu EL_PER_CTA), quads per chunk
+                const long long n_chunks = (ne + EPC - 1) / EPC, n_quads = (nn + 3) / 4;
+                const long long lag = 3LL * c->n_sm + 64;
+                int *epos = nullptr, *d_ready = nullptr;
+                if (c->d_eorder) {
+                    TRY(cudaMalloc(&epos, sizeof(int) * ne));
+                    k_epos<<<nblk(ne, 256), 256>>>(ne, c->d_eorder, epos);
+                }
+                TRY(cudaMalloc(&d_ready, sizeof(int) * n_quads));
+                TRY(cudaMalloc(&c->d_quad_deps, sizeof(int) * 16 * n_quads));
+                k_quad_deps<<<nblk(n_quads, 128), 128>>>(nn, n_quads, EPC, c->d_inc_ptr, c->d_inc, epos, c->d_quad_deps, d_ready);
+                TRY(cudaGetLastError());
+                int *ready = new (std::nothrow) int[n_quads], *cq = new (std::nothrow) int[n_chunks * QPC];
+                int *nxt = new (std::nothrow) int[n_chunks + 1], *fill = new (std::nothrow) int[n_chunks], *tail = new (std::nothrow) int[n_quads];
+                bool ok = ready && cq && nxt && fill && tail;
+                cudaError_t ce = ok ? cudaMemcpy(ready, d_ready, sizeof(int) * n_quads, cudaMemcpyDeviceToHost) : cudaSuccess;
+                int n_tail = 0;
+                if (ok && ce == cudaSuccess) {
+                    for (long long i = 0; i < n_chunks * QPC; i++) cq[i] = -1;
+                    for (long long i = 0; i <= n_chunks; i++) nxt[i] = (int)i;       // next chunk >= i with a free slot (path-compressed)
+                    for (long long i = 0; i < n_chunks; i++) fill[i] = 0;
+                    static const int order[8] = {0, 2, 4, 6, 1, 3, 5, 7};             // one quad per warp first, then the second
+                    for (long long qd = 0; qd < n_quads; qd++) {
+                        long long want = (ready[qd] == 0x7fffffff) ? n_chunks : (long long)ready[qd] + lag;
+                        if (want < 0) want = 0;
+                        if (want >= n_chunks) { tail[n_tail++] = (int)qd; continue; }
+                        long long r = want;
+                        while (nxt[r] != r) r = nxt[r];
+                        for (long long i = want; nxt[i] != r;) { const long long j = nxt[i]; nxt[i] = (int)r; i = j; }
+                        if (r >= n_chunks) { tail[n_tail++] = (int)qd; continue; }
+                        cq[r * QPC + order[fill[r]++]] = (int)qd;
+                        if (fill[r] == QPC) nxt[r] = (int)(r + 1);
+                    }
+                }
+                if (ok && ce == cudaSuccess) ce = cudaMalloc(&c->d_cta_quads, sizeof(int) * n_chunks * QPC);
+                if (ok && ce == cudaSuccess) ce = cudaMemcpy(c->d_cta_quads, cq, sizeof(int) * n_chunks * QPC, cudaMemcpyHostToDevice);
+                if (ok && ce == cudaSuccess) ce = cudaMalloc(&c->d_tail_quads, sizeof(int) * (n_tail > 0 ? n_tail : 1));
+                if (ok && ce == cudaSuccess && n_tail) ce = cudaMemcpy(c->d_tail_quads, tail, sizeof(int) * n_tail, cudaMemcpyHostToDevice);
+                delete[] ready; delete[] cq; delete[] nxt; delete[] fill; delete[] tail;
+                if (epos) cudaFree(epos);
+                cudaFree(d_ready);
+                if (!ok) { rc = FEM_ERR_ARG; break; }
+                TRY(ce);
+                c->n_tail_quads = n_tail;
+                TRY(cudaMalloc(&c->d_chunk_flag, sizeof(unsigned int) * n_chunks));
+                TRY(cudaMemset(c->d_chunk_flag, 0, sizeof(unsigned int) * n_chunks));
+                TRY(cudaMalloc(&c->d_left_list, sizeof(int) * n_quads));
+                TRY(cudaMalloc(&c->d_left_count, sizeof(unsigned int)));
+                TRY(cudaMemset(c->d_left_count, 0, sizeof(unsigned int)));
+                TRY(cudaDeviceSynchronize());
+                c->fuse_ok = true;
             }
 #undef TRY
         } while (0);

@@ -7,9 +7,10 @@
 #include <math.h>
 #include <string.h>
 
-#define RED_CTAS 1184      // 148 SMs x 8 CTAs of 256 threads for the vector kernels (fixed: part of the reduction order)
+#define RED_CTAS 1184      // grid-stride vector kernels: a FIXED number of CTAs on every device (the per-CTA partial sums
+                           // are part of the reduction order, so results do not depend on the SM count)
 #define RED_THREADS 256
-#define SPMV_CTAS 4736     // 148 SMs x 32 CTAs of 8 warps: grid-stride over the nodes, so the dot partials stay few
+#define SPMV_CTAS 4736     // likewise fixed: grid-stride over the nodes, 8 warps per CTA, so the dot partials stay few
 
 static inline unsigned spmv_grid(const fem_ctx *c) {
     const long long need = (c->n_nodes + 7) / 8;
@@ -343,13 +344,29 @@ static int ensure_solver_ws(fem_ctx *c, bool newton) {
     if (!c->d_sw) {
         const long long spmv_ctas = spmv_grid(c);
         c->n_part = 2 * (spmv_ctas > RED_CTAS ? spmv_ctas : RED_CTAS);
-        FEM_CUDA(cudaMalloc(&c->d_sw, sizeof(double) * 9 * n));
-        FEM_CUDA(cudaMalloc(&c->d_part, sizeof(double) * c->n_part));
-        FEM_CUDA(cudaMalloc(&c->d_scal, sizeof(double) * 64));   // [0..8) reduction results, [16..48) solver scalars
+        // all or nothing: a failed allocation leaves no half-built workspace behind for the next call to trip over
+        double *sw = nullptr, *part = nullptr, *scal = nullptr;
+        cudaError_t e = cudaMalloc(&sw, sizeof(double) * 9 * n);
+        if (e == cudaSuccess) e = cudaMalloc(&part, sizeof(double) * c->n_part);
+        if (e == cudaSuccess) e = cudaMalloc(&scal, sizeof(double) * 64);   // [0..8) reduction results, [16..48) solver scalars
+        if (e != cudaSuccess) {
+            if (sw) cudaFree(sw);
+            if (part) cudaFree(part);
+            if (scal) cudaFree(scal);
+            return fem_cuda_fail(e, "cudaMalloc(solver workspace)");
+        }
+        c->d_sw = sw; c->d_part = part; c->d_scal = scal;
     }
     if (newton && !c->d_nw) {
-        FEM_CUDA(cudaMalloc(&c->d_nw, sizeof(double) * 4 * n));
-        FEM_CUDA(cudaMalloc(&c->d_nw_vals, sizeof(double) * (size_t)c->nnz));
+        double *nw = nullptr, *nv = nullptr;
+        cudaError_t e = cudaMalloc(&nw, sizeof(double) * 4 * n);
+        if (e == cudaSuccess) e = cudaMalloc(&nv, sizeof(double) * (size_t)c->nnz);
+        if (e != cudaSuccess) {
+            if (nw) cudaFree(nw);
+            if (nv) cudaFree(nv);
+            return fem_cuda_fail(e, "cudaMalloc(Newton workspace)");
+        }
+        c->d_nw = nw; c->d_nw_vals = nv;
     }
     return FEM_OK;
 }
@@ -629,6 +646,7 @@ extern "C" int fem_newton_solve(fem_ctx *c, double *u, const double *hist_in, co
     fem_default_newton_options(&o);
     if (opt) o = *opt;
     if (!(o.rtol >= 0.0) || !(o.atol >= 0.0) || o.max_newton < 1 || !(o.lin_rtol > 0.0) || o.lin_max_iter < 1 || o.linear_solver < 0 || o.linear_solver > 2) return FEM_ERR_ARG;
+    if (fem_ranges_overlap(hist_in, hist_out, sizeof(double) * 56 * (size_t)c->n_elems)) return FEM_ERR_ALIAS;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     int rc = ensure_solver_ws(c, true);
     if (rc != FEM_OK) return rc;
@@ -639,44 +657,147 @@ extern "C" int fem_newton_solve(fem_ctx *c, double *u, const double *hist_in, co
     fem_newton_report rp;
     memset(&rp, 0, sizeof(rp));
     int result = FEM_ERR_NOCONV;
+    int err = FEM_OK;   // a hard error (CUDA, allocation) inside the loop: u is restored before it is returned
     for (int k = 0;; k++) {
-        if ((rc = fem_launch_assemble(c, u, hist_in, mat, n_mat, R, vals, hist_out, st)) != FEM_OK) return rc;
-        if ((rc = fem_read_stats(c, &rp.last_stats, st)) != FEM_OK) return rc;
+        if ((err = fem_launch_assemble(c, u, hist_in, mat, n_mat, R, vals, hist_out, st)) != FEM_OK) break;
+        if ((err = fem_read_stats(c, &rp.last_stats, st)) != FEM_OK) break;
         k_neg<<<RED_CTAS, RED_THREADS, 0, st>>>(n, R, rhs);
-        if ((rc = apply_dirichlet(c, n_bc, bc_dofs, nullptr, bc_vals, u, vals, rhs, st)) != FEM_OK) return rc;
+        if ((err = apply_dirichlet(c, n_bc, bc_dofs, nullptr, bc_vals, u, vals, rhs, st)) != FEM_OK) break;
         k_norm2<<<RED_CTAS, RED_THREADS, 0, st>>>(n, rhs, c->d_part);
         double h[1];
-        if ((rc = fetch_sums<1>(c, RED_CTAS, h, st)) != FEM_OK) return rc;
+        if ((err = fetch_sums<1>(c, RED_CTAS, h, st)) != FEM_OK) break;
         rp.rhs_norm = sqrt(h[0]);
         if (k == 0) rp.rhs_norm0 = rp.rhs_norm;
         if (!isfinite(rp.rhs_norm)) break;
-        if (rp.rhs_norm <= o.atol || rp.rhs_norm <= o.rtol * rp.rhs_norm0) { rp.converged = 1; result = FEM_OK; break; }
+        if (rp.rhs_norm <= o.atol || rp.rhs_norm <= o.rtol * rp.rhs_norm0) {
+            // a state that balances but holds inverted points, local solves that hit kmax or non-finite stresses is no root of
+            // the discrete problem (hist_out is not the return-map solution there): the increment is rejected so that the
+            // caller cuts the step back, as the paper's step control does
+            const fem_stats &ls = rp.last_stats;
+            rp.physics_trouble = (ls.n_nonconverged > 0 || ls.n_detF_nonpos > 0 || ls.n_nonfinite > 0) ? 1 : 0;
+            if (!rp.physics_trouble) { rp.converged = 1; result = FEM_OK; }
+            break;
+        }
         if (k >= o.max_newton) break;
         int its = 0;
         rc = FEM_ERR_NOCONV;
         if (o.linear_solver != 1 && !c->opt.fbar) {
             // standard element: K_ff is symmetric -> CG from the guess dd = rhs on the constrained DOFs, 0 elsewhere
-            FEM_CUDA(cudaMemsetAsync(dd, 0, sizeof(double) * n, st));
+            if ((err = fem_cuda_rc(cudaMemsetAsync(dd, 0, sizeof(double) * n, st), "cudaMemsetAsync(dd)")) != FEM_OK) break;
             if (n_bc > 0) k_scatter_bc<<<nblk3(n_bc, 256), 256, 0, st>>>(n_bc, bc_dofs, rhs, dd);
             rc = pcg(c, vals, rhs, dd, o.lin_rtol, o.lin_max_iter, &its, nullptr, st);
             rp.lin_iters_total += its;
         }
         if (rc == FEM_ERR_NOCONV && (o.linear_solver != 2 || c->opt.fbar)) {   // unsymmetric (F-bar), or CG gave up: BiCGSTAB from zero
-            FEM_CUDA(cudaMemsetAsync(dd, 0, sizeof(double) * n, st));
+            if ((err = fem_cuda_rc(cudaMemsetAsync(dd, 0, sizeof(double) * n, st), "cudaMemsetAsync(dd)")) != FEM_OK) break;
             rc = bicgstab(c, vals, rhs, dd, o.lin_rtol, o.lin_max_iter, &its, nullptr, st);
             rp.lin_iters_total += its;
         }
         if (rc == FEM_ERR_NOCONV) rp.lin_failures++;
-        else if (rc != FEM_OK) return rc;
+        else if (rc != FEM_OK) { err = rc; break; }
         k_axpy<<<RED_CTAS, RED_THREADS, 0, st>>>(n, 1.0, dd, u);
         rp.newton_iters++;
     }
-    if (result != FEM_OK)   // failed increment: u goes back to its entry value, so the caller can cut the step back
-        FEM_CUDA(cudaMemcpyAsync(u, u_entry, sizeof(double) * n, cudaMemcpyDeviceToDevice, st));
+    if (result != FEM_OK || err != FEM_OK)   // failed increment or error: u goes back to its entry value, so the caller can cut the step back
+        cudaMemcpyAsync(u, u_entry, sizeof(double) * n, cudaMemcpyDeviceToDevice, st);
+    if (err != FEM_OK) { cudaStreamSynchronize(st); if (rep) *rep = rp; return err; }
     FEM_CUDA(cudaGetLastError());
     FEM_CUDA(cudaStreamSynchronize(st));
     if (rep) *rep = rp;
     return result;
+}
+
+// ---- load path: the paper's adaptive load stepping around the Newton increment (settings of the unit-cube
+// benchmark :485).  Host control flow only: every number is produced by the kernels behind fem_newton_solve / fem_lincomb.
+extern "C" void fem_default_path_options(fem_path_options *o) {
+    if (!o) return;
+    o->dt0 = 1e-3; o->dt_min = 1e-5; o->dt_max = 5e-2; o->grow = 1.5; o->cut = 0.5; o->grow_below = 5; o->max_steps = 10000;
+    o->extrapolate = 1;
+    fem_default_newton_options(&o->newton);
+    o->newton.rtol = 1e-8; o->newton.max_newton = 12; o->newton.lin_rtol = 1e-6; o->newton.lin_max_iter = 20000;
+}
+
+__global__ void k_scale(long long n, double a, const double *__restrict__ x, double *__restrict__ out) {
+    for (long long j = blockIdx.x * (long long)blockDim.x + threadIdx.x; j < n; j += (long long)gridDim.x * blockDim.x) out[j] = a * x[j];
+}
+
+extern "C" int fem_load_path(fem_ctx *c, double *u, double *hist, const double *mat, long long n_mat, long long n_bc,
+                             const int *bc_dofs, const double *bc_full, const fem_path_options *opt, fem_path_report *rep,
+                             double *t_accepted, int n_t_cap, void *cuda_stream) {
+    if (!c || !u || !hist || !mat || (n_bc > 0 && (!bc_dofs || !bc_full))) return FEM_ERR_NULL;
+    if (!c->has_pattern) return FEM_ERR_NO_PATTERN;
+    if (n_mat != 1 && n_mat != c->n_elems) return FEM_ERR_MAT;
+    fem_path_options o;
+    fem_default_path_options(&o);
+    if (opt) o = *opt;
+    if (!(o.dt0 > 0.0) || !(o.dt_min > 0.0) || !(o.dt_max >= o.dt_min) || !(o.grow >= 1.0) || !(o.cut > 0.0 && o.cut < 1.0) ||
+        o.max_steps < 1 || o.extrapolate < 0 || o.extrapolate > 2 || n_bc < 0 || (t_accepted && n_t_cap < 0))
+        return FEM_ERR_ARG;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const long long n = c->n_rows;
+    const size_t hb = sizeof(double) * 56 * (size_t)c->n_elems;
+    if (!c->d_path) {   // u_try, u_prev, u_pp, bc values of the step (n_rows each) and the second history buffer: all or nothing
+        double *pw = nullptr, *ph = nullptr;
+        cudaError_t e = cudaMalloc(&pw, sizeof(double) * 4 * n);
+        if (e == cudaSuccess) e = cudaMalloc(&ph, hb);
+        if (e != cudaSuccess) { if (pw) cudaFree(pw); if (ph) cudaFree(ph); return fem_cuda_fail(e, "cudaMalloc(load path workspace)"); }
+        c->d_path = pw; c->d_path_hist = ph;
+    }
+    double *u_try = c->d_path, *u_prev = u_try + n, *u_pp = u_prev + n, *bcv = u_pp + n;
+    double *h_a = hist, *h_b = c->d_path_hist;          // history at the start of the step / written by the step
+    FEM_CUDA(cudaMemcpyAsync(u_prev, u, sizeof(double) * n, cudaMemcpyDeviceToDevice, st));
+    FEM_CUDA(cudaMemcpyAsync(u_pp, u, sizeof(double) * n, cudaMemcpyDeviceToDevice, st));
+    fem_path_report rp;
+    memset(&rp, 0, sizeof(rp));
+    double t = 0.0, dt = o.dt0 < o.dt_max ? o.dt0 : o.dt_max, dt_prev = 0.0, dt_pp = 0.0;
+    int rc = FEM_OK;
+    while (t < 1.0 - 1e-12) {
+        if (rp.steps + rp.rejected >= o.max_steps) { rc = FEM_ERR_NOCONV; break; }
+        if (dt > 1.0 - t) dt = 1.0 - t;
+        // initial guess: extrapolation of the converged states ("linear or quadratic extrapolation")
+        if (o.extrapolate == 2 && dt_pp > 0.0) {   // Lagrange parabola through the last three converged states
+            const double t0 = -(dt_prev + dt_pp), t1 = -dt_prev, t2 = 0.0, t3 = dt;
+            const double l0 = (t3 - t1) * (t3 - t2) / ((t0 - t1) * (t0 - t2)), l1 = (t3 - t0) * (t3 - t2) / ((t1 - t0) * (t1 - t2)),
+                         l2 = (t3 - t0) * (t3 - t1) / ((t2 - t0) * (t2 - t1));
+            k_lincomb<<<RED_CTAS, RED_THREADS, 0, st>>>(n, l2, u, l1, u_prev, u_try);
+            k_lincomb<<<RED_CTAS, RED_THREADS, 0, st>>>(n, 1.0, u_try, l0, u_pp, u_try);
+        } else {
+            const double r = (o.extrapolate && dt_prev > 0.0) ? dt / dt_prev : 0.0;
+            k_lincomb<<<RED_CTAS, RED_THREADS, 0, st>>>(n, 1.0 + r, u, -r, u_prev, u_try);   // u + (u - u_prev) dt / dt_prev
+        }
+        if (n_bc > 0) k_scale<<<nblk3(n_bc, 256), 256, 0, st>>>(n_bc, t + dt, bc_full, bcv);
+        fem_newton_report nr;
+        rc = fem_newton_solve(c, u_try, h_a, mat, n_mat, n_bc, bc_dofs, bcv, h_b, &o.newton, &nr, cuda_stream);
+        rp.newton_iters_total += nr.newton_iters;
+        rp.lin_iters_total += nr.lin_iters_total;
+        if (rc != FEM_OK && rc != FEM_ERR_NOCONV) break;
+        const bool ok = (rc == FEM_OK) && nr.converged && nr.lin_failures == 0;
+        if (ok) {
+            t += dt;
+            if (t_accepted && rp.steps < n_t_cap) t_accepted[rp.steps] = t;
+            rp.steps++;
+            rp.last = nr;
+            // rotate: u_pp <- u_prev <- u <- u_try (u is the caller's buffer: copies, three n_rows vectors per accepted step)
+            FEM_CUDA(cudaMemcpyAsync(u_pp, u_prev, sizeof(double) * n, cudaMemcpyDeviceToDevice, st));
+            FEM_CUDA(cudaMemcpyAsync(u_prev, u, sizeof(double) * n, cudaMemcpyDeviceToDevice, st));
+            FEM_CUDA(cudaMemcpyAsync(u, u_try, sizeof(double) * n, cudaMemcpyDeviceToDevice, st));
+            double *tmp = h_a; h_a = h_b; h_b = tmp;
+            dt_pp = dt_prev; dt_prev = dt;
+            if (nr.newton_iters <= o.grow_below) { dt *= o.grow; if (dt > o.dt_max) dt = o.dt_max; }
+            rc = FEM_OK;
+        } else {   // failed increment, a linear solve that gave up, or physics trouble at the converged state: cut back
+            rp.rejected++;
+            if (nr.physics_trouble) rp.rejected_physics++;
+            dt *= o.cut;
+            if (dt < o.dt_min) { rc = FEM_ERR_NOCONV; break; }
+            rc = FEM_OK;
+        }
+    }
+    rp.t_reached = t;
+    if (h_a != hist) FEM_CUDA(cudaMemcpyAsync(hist, h_a, hb, cudaMemcpyDeviceToDevice, st));   // the history of the last accepted state
+    FEM_CUDA(cudaStreamSynchronize(st));
+    if (rep) *rep = rp;
+    return rc;
 }
 
 // One step of the backward sweep of Alg. 1: right-hand side of Eq.(51) :366, adjoint solve on the tangent
@@ -715,7 +836,10 @@ extern "C" int fem_adjoint_step(fem_ctx *c, const double *u, const double *hist_
     if (!c->has_pattern) return FEM_ERR_NO_PATTERN;
     if (n_mat != 1 && n_mat != c->n_elems) return FEM_ERR_MAT;
     if (n_bc < 0 || !(lin_rtol > 0.0) || lin_max_iter < 1) return FEM_ERR_ARG;
-    if (mu_out == hist_in || mu_out == mu_in) return FEM_ERR_ALIAS;
+    {
+        const size_t hb = sizeof(double) * 56 * (size_t)c->n_elems;
+        if (fem_ranges_overlap(mu_out, hist_in, hb) || (mu_in && fem_ranges_overlap(mu_out, mu_in, hb))) return FEM_ERR_ALIAS;
+    }
     cudaStream_t st = (cudaStream_t)cuda_stream;
     int rc = ensure_solver_ws(c, true);
     if (rc != FEM_OK) return rc;

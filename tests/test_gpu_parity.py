@@ -151,15 +151,52 @@ def test_error_codes_on_device():
 
 
 @pytest.mark.parametrize("fbar", [0, 1])
-def test_coloured_in_place_assembly_mode(fbar):
-    """assembly_mode 1 (one launch per colour, in-place read-modify-write) gives the same matrix as the oracle and is
-    bitwise reproducible; irregular mesh with shuffled element order."""
-    cfg = synth.make_config(4, n=14)
-    g = run_gpu(cfg, fbar, assembly_mode=1)
-    assert g["ctx"].launches_per_assemble() > 3          # mat_prep + one launch per colour (>= 8 colours for hex meshes)
-    compare(g, run_oracle(cfg, fbar), "coloured")
-    g2 = run_gpu(cfg, fbar, assembly_mode=1)
+@pytest.mark.parametrize("cfgid,n", [(3, 22), (4, 27)])
+def test_fused_gather_equals_separate_gather(cfgid, n, fbar):
+    """assembly_mode 0 gathers node quads inside the element launch (warps of chunks launched one wave later read the
+    records back from L2, completion flags, no waiting) and finishes the rest in k_gather_list; assembly_mode 1 runs the
+    element kernel and the stand-alone gather kernel one after the other.  Both sum in ascending element id: the two
+    must agree bit for bit, with the oracle within tolerance, and with themselves on a second call.  Sizes: more than
+    3*148+64 chunks of 16 elements, so that part of the quads really is gathered in-kernel."""
+    cfg = synth.make_config(cfgid, n=n)
+    assert cfg["conn"].shape[0] > 16 * (3 * 148 + 64)
+    g = run_gpu(cfg, fbar, assembly_mode=0)
+    compare(g, run_oracle(cfg, fbar), "fused cfg%d" % cfgid)
+    g1 = run_gpu(cfg, fbar, assembly_mode=1)
+    assert np.array_equal(g["csr_vals"], g1["csr_vals"]) and np.array_equal(g["residual"], g1["residual"])
+    assert np.array_equal(g["hist_out"], g1["hist_out"])
+    g2 = run_gpu(cfg, fbar, assembly_mode=0)
     assert np.array_equal(g["csr_vals"], g2["csr_vals"]) and np.array_equal(g["residual"], g2["residual"])
+
+
+def test_fused_gather_repeated_calls_and_isolated_node():
+    """The chunk flags carry the epoch of the call: repeated calls on one context stay correct; a node that belongs to no
+    element gets a zero residual."""
+    import torch
+    import paper_2606_17390_b200 as fem
+    cfg = synth.make_config(3, n=22)
+    coords = np.vstack([cfg["coords"], [[5.0, 5.0, 5.0]]])          # one extra, unreferenced node
+    u = np.vstack([cfg["u"], [[0.0, 0.0, 0.0]]])
+    cfg2 = dict(cfg, coords=coords, u=u)
+    o = run_oracle(cfg2)
+    dev = torch.device("cuda:0")
+    ne = cfg2["conn"].shape[0]
+    ctx = fem.FemContext(torch.from_numpy(coords).to(dev), torch.from_numpy(cfg2["conn"]).to(dev))
+    ctx.build_csr_pattern()
+    mat = torch.from_numpy(fem.mat_from_desc(cfg2["matdesc"], ne).ravel()).to(dev)
+    ud, hd = torch.from_numpy(u.ravel()).to(dev), torch.from_numpy(cfg2["hist_in"].ravel()).to(dev)
+    prev = None
+    for rep in range(4):
+        uu = ud if rep != 2 else 0.5 * ud                            # a different state in between: stale records must not leak
+        res, vals, hout, _ = ctx.assemble(uu, hd, mat, want_stats=True)
+        torch.cuda.synchronize()
+        if rep == 2:
+            continue
+        assert rel_l2(res.cpu().numpy(), o["residual"]) <= 1e-11 and rel_l2(vals.cpu().numpy(), o["csr_vals"]) <= 1e-10
+        assert np.all(res.cpu().numpy()[-3:] == 0.0)
+        if prev is not None:
+            assert torch.equal(prev, vals)
+        prev = vals.clone()
 
 
 def _pinwheel_mesh(nsec=12, layers=2):
@@ -193,11 +230,10 @@ def _mini_cfg(coords, conn, seed=5, amp=0.03):
     return dict(coords=coords, conn=conn, u=u, hist_in=np.zeros((conn.shape[0], 8, 7)), matdesc=dict(synth.configs.SWIFT))
 
 
-@pytest.mark.parametrize("mode", [0, 1])
-def test_high_valence_mesh_uses_general_gather(mode):
+def test_high_valence_mesh_uses_general_gather():
     coords, conn = _pinwheel_mesh()
     cfg = _mini_cfg(coords, conn)
-    g = run_gpu(cfg, 0, want_elem_slot=True, assembly_mode=mode)
+    g = run_gpu(cfg, 0, want_elem_slot=True)
     compare(g, run_oracle(cfg, 0, with_slots=True), "pinwheel")
     assert g["stats"]["n_plastic"] > 0
 
@@ -211,49 +247,9 @@ def test_collapsed_hex_wedge_elements():
         return [a + off, b + off, c + off, c + off, a + off + 4, b + off + 4, c + off + 4, c + off + 4]
     conn = np.array([wedge(0, 1, 2, 0), wedge(1, 3, 2, 0), wedge(0, 1, 2, 4), wedge(1, 3, 2, 4)], dtype=np.int32)
     cfg = _mini_cfg(coords, conn, seed=9)
-    g = run_gpu(cfg, 0, want_elem_slot=True, assembly_mode=1)     # asks for mode 1, library must fall back to the gather mode
+    g = run_gpu(cfg, 0, want_elem_slot=True)                      # collapsed elements: the general gather kernel
     assert g["ctx"].launches_per_assemble() == 3
     compare(g, run_oracle(cfg, 0, with_slots=True), "wedge")
-
-
-@pytest.mark.parametrize("fbar", [0, 1])
-@pytest.mark.parametrize("cfgid,n", [(1, None), (3, 22), (4, 18)])
-def test_fused_queue_assembly_mode(cfgid, n, fbar):
-    """assembly_mode 2 (element CTAs count nodes down and queue completed ones; gather CTAs of the same launch and a drain
-    kernel assemble them) matches the oracle, is bit-identical to mode 0 (same summation order) and to itself."""
-    cfg = synth.make_config(cfgid) if n is None else synth.make_config(cfgid, n=n)
-    g = run_gpu(cfg, fbar, assembly_mode=2)
-    compare(g, run_oracle(cfg, fbar), "fused cfg%d" % cfgid)
-    g0 = run_gpu(cfg, fbar, assembly_mode=0)
-    assert np.array_equal(g["csr_vals"], g0["csr_vals"]) and np.array_equal(g["residual"], g0["residual"])
-    g2 = run_gpu(cfg, fbar, assembly_mode=2)
-    assert np.array_equal(g["csr_vals"], g2["csr_vals"]) and np.array_equal(g["residual"], g2["residual"])
-
-
-def test_fused_mode_repeated_calls_and_isolated_node():
-    """Mode 2 resets its countdown / queue on every call; a node that belongs to no element gets a zero residual."""
-    import torch
-    import paper_2606_17390_b200 as fem
-    cfg = synth.make_config(3, n=12)
-    coords = np.vstack([cfg["coords"], [[5.0, 5.0, 5.0]]])          # one extra, unreferenced node
-    u = np.vstack([cfg["u"], [[0.0, 0.0, 0.0]]])
-    cfg2 = dict(cfg, coords=coords, u=u)
-    o = run_oracle(cfg2)
-    dev = torch.device("cuda:0")
-    ne = cfg2["conn"].shape[0]
-    ctx = fem.FemContext(torch.from_numpy(coords).to(dev), torch.from_numpy(cfg2["conn"]).to(dev), assembly_mode=2)
-    ctx.build_csr_pattern()
-    mat = torch.from_numpy(fem.mat_from_desc(cfg2["matdesc"], ne).ravel()).to(dev)
-    ud, hd = torch.from_numpy(u.ravel()).to(dev), torch.from_numpy(cfg2["hist_in"].ravel()).to(dev)
-    prev = None
-    for _ in range(3):
-        res, vals, hout, _ = ctx.assemble(ud, hd, mat, want_stats=True)
-        torch.cuda.synchronize()
-        assert rel_l2(res.cpu().numpy(), o["residual"]) <= 1e-11 and rel_l2(vals.cpu().numpy(), o["csr_vals"]) <= 1e-10
-        assert np.all(res.cpu().numpy()[-3:] == 0.0)
-        if prev is not None:
-            assert torch.equal(prev, vals)
-        prev = vals.clone()
 
 
 @pytest.mark.parametrize("fbar", [0, 1])

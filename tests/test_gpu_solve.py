@@ -182,3 +182,88 @@ def test_load_path_with_history_matches_oracle():
         uo, ho = o["u"], o["hist_out"]
     assert rel_l2(u.cpu().numpy(), uo) <= 1e-8 and rel_l2(h_a.cpu().numpy(), ho) <= 1e-7
     assert float(h_a.view(-1, 7)[:, 6].max()) > 0.01          # the path is well into the plastic range
+
+
+@pytest.mark.parametrize("fbar,extrapolate", [(0, 1), (0, 2), (1, 1)])
+def test_fem_load_path_matches_oracle_loop(fbar, extrapolate):
+    """fem_load_path (the adaptive load stepping of PAPER.md:306 behind one C-ABI call) against the same loop written with
+    oracle functions only (oracle.newton.load_path): a schedule that starts too ambitiously for the Newton cap, so it has
+    to cut back and grow again.  Same accepted load fractions, same number of rejected steps, same final state."""
+    import torch
+    import paper_2606_17390_b200 as fem
+    import oracle.newton as onw
+    coords, conn, omat, rp, ci, h0, bc, val = clamped_shear_problem()
+    ctx, dev = _ctx(coords, conn, fbar)
+    ne = conn.shape[0]
+    mat = torch.from_numpy(fem.mat_from_desc(dict(synth.configs.SWIFT), ne).ravel()).to(dev)
+    u = torch.zeros(coords.size, dtype=torch.float64, device=dev)
+    hist = torch.zeros(56 * ne, dtype=torch.float64, device=dev)
+    kw = dict(dt0=0.7, dt_min=1e-3, dt_max=0.5, grow=1.5, cut=0.5, grow_below=5, extrapolate=extrapolate)
+    rc, rep, ts = ctx.load_path(u, hist, mat, torch.from_numpy(bc.astype(np.int32)).to(dev), torch.from_numpy(val).to(dev),
+                                newton=dict(rtol=1e-8, atol=1e-10, max_newton=4, lin_rtol=1e-12, lin_max_iter=20000), **kw)
+    o = onw.load_path(coords, conn, h0, omat, rp, ci, bc, val, fbar=fbar, rtol=1e-8, atol=1e-10, max_newton=4, **kw)
+    assert rc == 0 and o["completed"] and rep["t_reached"] == 1.0
+    assert rep["rejected"] == o["rejected"] >= 1 and rep["steps"] == o["steps"] >= 3
+    assert np.allclose(ts, o["ts"], rtol=0, atol=1e-15)
+    assert rep["newton_iters_total"] == o["newton_iters_total"]
+    assert rel_l2(u.cpu().numpy(), o["u"]) <= 1e-8 and rel_l2(hist.cpu().numpy(), o["hist"]) <= 1e-7
+    assert float(hist.view(-1, 7)[:, 6].max()) > 0.01
+    # a second path on the same context (workspace reuse) from the same start gives the same bits
+    u2 = torch.zeros_like(u); hist2 = torch.zeros_like(hist)
+    rc2, rep2, ts2 = ctx.load_path(u2, hist2, mat, torch.from_numpy(bc.astype(np.int32)).to(dev), torch.from_numpy(val).to(dev),
+                                   newton=dict(rtol=1e-8, atol=1e-10, max_newton=4, lin_rtol=1e-12, lin_max_iter=20000), **kw)
+    assert rc2 == 0 and ts2 == ts and torch.equal(u2, u) and torch.equal(hist2, hist)
+
+
+def test_balanced_state_with_local_nonconvergence_is_rejected():
+    """an increment whose balanced state holds local solves that hit kmax is no root of the discrete problem.
+    With the local iteration cap at 2 the return map is cut short at every plastic point: fem_newton_solve must report
+    physics trouble, return FEM_ERR_NOCONV and restore u; fem_load_path must cut back and finally give up, leaving the
+    last accepted state.  Overlapping history buffers are refused."""
+    import torch
+    import paper_2606_17390_b200 as fem
+    coords, conn, omat, rp, ci, h0, bc, val = clamped_shear_problem()
+    dev = torch.device("cuda:0")
+    ne = conn.shape[0]
+    ctx = fem.FemContext(torch.from_numpy(coords).to(dev), torch.from_numpy(conn).to(dev), kmax=2)
+    ctx.build_csr_pattern()
+    mat = torch.from_numpy(fem.mat_from_desc(dict(synth.configs.SWIFT), ne).ravel()).to(dev)
+    bc_d, val_d = torch.from_numpy(bc.astype(np.int32)).to(dev), torch.from_numpy(val).to(dev)
+    hin = torch.zeros(56 * ne, dtype=torch.float64, device=dev)
+    u_in = torch.zeros(coords.size, dtype=torch.float64, device=dev)
+    u, _, rep = ctx.newton_solve(u_in.clone(), hin, mat, bc_d, val_d, lin_rtol=1e-12, rtol=1e-7, max_newton=40)
+    assert rep["last_stats"]["n_nonconverged"] > 0
+    assert rep["physics_trouble"] and not rep["converged"] and torch.equal(u, u_in)
+    rc, prep, ts = ctx.load_path(u_in.clone(), hin.clone(), mat, bc_d, val_d, dt0=0.5, dt_min=0.2, dt_max=0.5,
+                                 newton=dict(lin_rtol=1e-12, rtol=1e-7, max_newton=40))
+    assert rc == -11 and prep["rejected_physics"] >= 1 and prep["steps"] == 0 and prep["t_reached"] == 0.0
+    with pytest.raises(fem.FemError) as ei:            # hist_out overlapping hist_in (offset view of the same buffer)
+        big = torch.zeros(56 * ne + 8, dtype=torch.float64, device=dev)
+        ctx.newton_solve(u_in.clone(), big[:56 * ne], mat, bc_d, val_d, hist_out=big[8:])
+    assert ei.value.code == -9
+    ctx.close()
+
+
+def test_barlat_exponent_outside_the_supported_set_is_reported():
+    """an exponent m that is not an even integer in 2..16 must not index past the coefficient tables: it is clamped
+    inside the call and the call reports FEM_ERR_ARG when statistics are requested."""
+    import torch
+    import paper_2606_17390_b200 as fem
+    cfg = synth.make_config(1)
+    dev = torch.device("cuda:0")
+    ctx = fem.FemContext(torch.from_numpy(cfg["coords"]).to(dev), torch.from_numpy(cfg["conn"]).to(dev))
+    ctx.build_csr_pattern()
+    mat = torch.tensor([70000.0, 0.33, 1, 1, 1, 1, 1, 1, 1.0, 500.0, 0.01, 0.2, 1.0, 0.0, 0.0, 0.0], dtype=torch.float64, device=dev)
+    u = torch.from_numpy(cfg["u"].ravel()).to(dev); h = torch.from_numpy(cfg["hist_in"].ravel()).to(dev)
+    good = torch.tensor([1.0] * 18 + [8.0, 0.0], dtype=torch.float64, device=dev)
+    r8, v8, _, st = ctx.assemble(u, h, mat, want_stats=True, barlat=good)
+    assert st["n_nonfinite"] == 0
+    for m in (40.0, 7.0, 0.0, float("nan")):
+        bad = good.clone(); bad[18] = m
+        with pytest.raises(fem.FemError) as ei:
+            ctx.assemble(u, h, mat, want_stats=True, barlat=bad)
+        assert ei.value.code == -2
+        r, v, _, _ = ctx.assemble(u, h, mat, barlat=bad)         # without statistics: clamped, finite, no fault
+        torch.cuda.synchronize()
+        assert bool(torch.isfinite(v).all())
+    ctx.close()

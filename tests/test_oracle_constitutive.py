@@ -232,6 +232,115 @@ def test_return_map_invariants_and_c2(which, swift_mat, voce_mat3):
     assert n_c2 > 150     # Alg. C2 converges on most; where it does, same root
 
 
+def _mp_root_of_eq19_24(mat, eps, epn, an, start):
+    """The root of the paper's local system G(y) = 0, y = [T, alpha, dgam] (Eq.(19)-(24) PAPER.md:176-196), by plain
+    Newton on all 8 unknowns in 40-digit arithmetic (mpmath), started from `start`.  Written from the equations, not
+    from the oracle's scalar reduction; only the Hill matrix (pinned by P4/P5) is taken from the oracle."""
+    import mpmath as mp
+    mp.mp.dps = 40
+    E, nu = mp.mpf(float(mat[0])), mp.mpf(float(mat[1]))
+    mu, lam = E / (2 * (1 + nu)), E * nu / ((1 + nu) * (1 - 2 * nu))
+    EE = mp.zeros(6, 6)
+    for i in range(6):
+        EE[i, i] = 2 * mu
+    for i in range(3):
+        for j in range(3):
+            EE[i, j] += lam
+    H = mp.matrix(oracle.hill_mandel(mat).tolist())
+    mw = [1, 1, 1, mp.sqrt(2), mp.sqrt(2), mp.sqrt(2)]
+    Wm = mp.sqrt(mp.mpf(2) / 3)
+    e = mp.matrix([mw[a] * (mp.mpf(float(eps[a])) - mp.mpf(float(epn[a]))) for a in range(6)])
+    law = mat[8]
+    h0, h1, h2 = [mp.mpf(float(x)) for x in mat[9:12]]
+
+    def sy(a):      # sqrt(2/3) sigma_flow (reading G2), Voce Eq.(10) :121 / Swift (BASELINE configs)
+        if law == 0:
+            return Wm * (h0 + h1 * (1 - mp.exp(-h2 * a))), Wm * h1 * h2 * mp.exp(-h2 * a)
+        return Wm * h0 * (h1 + a) ** h2, Wm * h0 * h2 * (h1 + a) ** (h2 - 1)
+    T = mp.matrix([mw[a] * mp.mpf(float(start["T"][a])) for a in range(6)])
+    al, dg, aN = mp.mpf(float(start["alpha"])), mp.mpf(float(start["dgam"])), mp.mpf(float(an))
+    for _ in range(12):
+        HT = H * T
+        phi = mp.sqrt((T.T * HT)[0])
+        N = HT / phi
+        s, ds = sy(al)
+        G = mp.matrix(8, 1)
+        GT = T - EE * (e - dg * N)
+        for a in range(6):
+            G[a] = GT[a]
+        G[6] = al - aN - Wm * dg
+        G[7] = phi - s
+        J = mp.zeros(8, 8)
+        A = mp.eye(6) + dg * (EE * ((H - N * N.T) / phi))
+        EN = EE * N
+        for a in range(6):
+            for b in range(6):
+                J[a, b] = A[a, b]
+            J[a, 7] = EN[a]
+            J[7, a] = N[a]
+        J[6, 6] = 1; J[6, 7] = -Wm; J[7, 6] = -ds
+        dy = mp.lu_solve(J, -G)
+        for a in range(6):
+            T[a] += dy[a]
+        al += dy[6]; dg += dy[7]
+        if mp.norm(dy) < mp.mpf(10) ** -30 * mp.norm(T):
+            break
+    else:
+        raise AssertionError("40-digit Newton did not converge")
+    return np.array([float(T[a] / mw[a]) for a in range(6)]), float(al), float(dg)
+
+
+@pytest.mark.parametrize("which", ["swift", "voce3"])
+def test_return_map_termination_at_large_strain(which, swift_mat, voce_mat3):
+    """Pins the stop test of the oracle's primary solver (reading G7: stop at the round-off floor of the 6x6
+    solve, then one polish step): strain-driven trial states with |eps| up to 0.3 (config 5's largest level), non-zero
+    history and a large pressure part, where |T_tr| is hundreds of times the yield stress.  The solver must never
+    report `nonconv`, must finish in a bounded number of evaluations, and must land on the root of Eq.(19)-(24)
+    computed in 40-digit arithmetic to 5e-12 (the north_star bounds history and tangent at 1e-10); it must be the
+    root literal Alg. C2 finds wherever C2 converges.  Sampling after PAPER.md:879.
+    f = phi - sigma_y evaluated in double from the returned T cancels |T_tr| ~ 2mu |eps| down to sigma_y (and the 6x6
+    solve adds its condition number), so f <= 1e-12 sigma_y is asserted only where that cancellation is mild
+    (|eps| <= 0.01); beyond, the 40-digit root is the accuracy pin."""
+    mat = swift_mat if which == "swift" else voce_mat3
+    rng = np.random.default_rng(11)
+    H = oracle.hill_mandel(mat)
+    n_c2 = n = 0
+    max_iters = 0
+    for norm in (0.01, 0.03, 0.1, 0.2, 0.3):
+        for trial in range(40):
+            d = rng.normal(size=6)
+            d[:3] -= d[:3].mean()                                       # deviatoric direction ...
+            d /= np.sqrt((d * MW) @ (d * MW))
+            vol = rng.uniform(-1.0, 1.0) * (0.0 if trial % 3 == 0 else 0.5)   # ... plus a volumetric part (pressure ~ K tr eps)
+            eps = norm * (d + vol * np.array([1, 1, 1, 0, 0, 0]) / np.sqrt(3.0))
+            an = 0.2 * rng.random()
+            p = rng.normal(size=6); p[:3] -= p[:3].mean(); p /= np.sqrt((p * MW) @ (p * MW))
+            epn = 0.5 * an * p                                          # trace-free plastic strain of the size of alpha
+            r = oracle.return_map(mat, eps, epn, an)
+            if not r["plastic"]:
+                continue
+            n += 1
+            assert r["nonconv"] == 0 and r["dgam"] > 0
+            max_iters = max(max_iters, r["iters"])
+            Tx, ax, dgx = _mp_root_of_eq19_24(mat, eps, epn, an, r)
+            assert abs(r["dgam"] / dgx - 1) <= 5e-12, (norm, trial)
+            assert abs(r["alpha"] - ax) <= 5e-12 * ax
+            assert np.abs(r["T"] - Tx).max() <= 5e-12 * np.abs(Tx).max(), (norm, trial)
+            if norm <= 0.01:
+                t = r["T"] * MW
+                phi = np.sqrt(t @ H @ t)
+                sf, _ = oracle.flow(mat, r["alpha"])
+                assert abs(phi - W * sf) <= 1e-12 * W * sf, (norm, trial, phi, W * sf)
+            assert abs(r["ep"][:3].sum() - epn[:3].sum()) < 1e-14
+            c2 = oracle.return_map_c2(mat, eps, epn, an)
+            if c2["iters"] >= 0:
+                n_c2 += 1
+                assert abs(c2["dgam"] / r["dgam"] - 1) < 1e-9, (norm, trial)
+                assert np.allclose(c2["T"], r["T"], rtol=1e-9, atol=1e-9 * np.abs(r["T"]).max() + 1e-7)
+    assert n >= 150 and n_c2 >= 50, (n, n_c2)
+    assert max_iters <= 40          # bracket doubling + safeguarded Newton: far from the 200-evaluation caps
+
+
 def test_c2_quadratic_convergence(swift_mat):
     F = np.array(GOLD["F"])
     eps, _, _ = oracle.logstrain(F)

@@ -123,3 +123,36 @@ def test_global_newton_converges_quadratically():
     free = np.setdiff1d(np.arange(3 * coords.shape[0]), bc)
     assert np.abs(out["residual"][free]).max() < 1e-9 * np.abs(out["residual"][bc]).max()
     assert np.allclose(res["u"].ravel()[bc], val, rtol=0, atol=1e-15)
+
+
+def test_load_path_is_step_size_independent_for_proportional_loading():
+    """Pin of oracle.newton.load_path.  Isotropic material (all r = 1), homogeneous isochoric-free uniaxial
+    stretch of a patch with lateral faces free: the loading is proportional in fixed principal axes, N is constant along
+    the path, and backward Euler is then exact for any step size - so the adaptively stepped path, with whatever
+    schedule and cut-backs it takes, must end in the state of one single increment (displacement and history)."""
+    desc = dict(synth.configs.SWIFT, r0=1.0, r45=1.0, r90=1.0)
+    coords, conn, mat, rp, ci, h0 = _problem(2, 2, 2, desc=desc)
+    nid = np.arange(coords.shape[0])
+    x0, x1 = np.abs(coords[:, 0]) < 1e-12, np.abs(coords[:, 0] - 1) < 1e-12
+    bc = [3 * nid[x0], 3 * nid[x1]]                                   # u_x on both x faces
+    bc += [np.array([3 * n + 1]) for n in nid[np.abs(coords[:, 1]) < 1e-12]]   # symmetry planes y = 0, z = 0
+    bc += [np.array([3 * n + 2]) for n in nid[np.abs(coords[:, 2]) < 1e-12]]
+    bc = np.concatenate(bc)
+    full = np.zeros(bc.size)
+    full[x0.sum():x0.sum() + x1.sum()] = 0.04                          # 4 % stretch: well into the plastic range
+    one = onw.newton_solve(coords, conn, np.zeros_like(coords), h0, mat, rp, ci, bc, full, max_newton=30)
+    assert one["converged"] and one["stats"]["n_plastic"] == 8 * conn.shape[0]
+    # a schedule that starts too ambitiously for 3 Newton iterations: it must cut back, then grow again
+    path = onw.load_path(coords, conn, h0, mat, rp, ci, bc, full, dt0=1.0, dt_min=1e-3, dt_max=0.4, grow=1.5, cut=0.5, grow_below=4,
+                         max_newton=3, extrapolate=1)
+    assert path["completed"] and path["rejected"] >= 1 and path["steps"] >= 3
+    assert np.all(np.diff(path["ts"]) > 0) and abs(path["ts"][-1] - 1.0) < 1e-12
+    assert np.allclose(path["u"], one["u"], rtol=0, atol=1e-9 * np.abs(one["u"]).max())
+    assert np.allclose(path["hist"], one["hist_out"], rtol=0, atol=1e-9 * np.abs(one["hist_out"]).max())
+    # no extrapolation and quadratic extrapolation reach the same state
+    for ex in (0, 2):
+        p2 = onw.load_path(coords, conn, h0, mat, rp, ci, bc, full, dt0=0.2, dt_min=1e-3, dt_max=0.3, extrapolate=ex, max_newton=12)
+        assert p2["completed"] and np.allclose(p2["u"], one["u"], rtol=0, atol=1e-9 * np.abs(one["u"]).max())
+    # a path that cannot be completed reports where it stopped
+    p3 = onw.load_path(coords, conn, h0, mat, rp, ci, bc, full, dt0=1.0, dt_min=0.6, dt_max=1.0, max_newton=1)
+    assert not p3["completed"] and p3["t"] == 0.0 and p3["rejected"] == 1
