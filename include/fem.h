@@ -58,15 +58,15 @@ typedef struct {
                           The element kernel writes K^e, R^e to a destination-major scratch (one 72-double record per
                           (element, local node), node-sorted), and every CSR entry is the sum of its records in ascending element
                           id (deterministic, no atomics).
-                          0 (default) = fused, lagged gather: at pattern-build time the nodes are cut into quads of four and every
-                          quad is given to one warp of an element CTA that is launched at least one wave of resident CTAs after
-                          the last CTA that writes one of its records; that warp sums the quad's CSR rows at the start of its CTA,
-                          reading the records back from L2 while its own inputs are on their way.  Completion is tracked by one
-                          flag per CTA; a warp never waits: a quad that is not ready (or is scheduled past the last CTA) is
-                          finished by a short gather kernel after the element launch.  Meshes with collapsed elements or a node
-                          with more than 8 elements use mode 1.
-                          1 = the element kernel, then a stand-alone node-row gather kernel over all nodes (nodes with more than 8
-                          elements / collapsed elements take a general path in it). */
+                          0 (default) = the element kernel, then a stand-alone node-row gather kernel over all nodes (nodes with
+                          more than 8 elements / collapsed elements take a general path in it).
+                          1 = fused, lagged gather (experimental, measured slower at config 3): at
+                          pattern-build time the nodes are cut into quads of four and every quad is given to one warp of an
+                          element CTA that is launched at least one wave of resident CTAs after the last CTA that writes one of
+                          its records; that warp sums the quad's CSR rows at the start of its CTA, reading the records back from
+                          L2.  Completion is tracked by one flag per CTA; a warp never waits: a quad that is not ready (or is
+                          scheduled past the last CTA) is finished by a short gather kernel after the element launch.  Meshes
+                          with collapsed elements or a node with more than 8 elements fall back to mode 0. */
 } fem_options;
 
 typedef struct {
@@ -141,8 +141,8 @@ int fem_assemble_host(fem_ctx *c, const double *u, const double *hist_in, const 
                       double *residual, double *csr_vals, double *hist_out, fem_stats *stats);
 
 /* Device time in milliseconds of the kernels of the last fem_assemble on this context, measured with CUDA events
- * on the call's stream: ms[0] = element kernel (S2-S12; in assembly_mode 0 it also gathers most node rows, S14),
- * ms[1] = the gather kernel that follows it (mode 0: the quads left over; mode 1: all nodes), ms[2] = material pre-pass.
+ * on the call's stream: ms[0] = element kernel (S2-S12; in assembly_mode 1 it also gathers most node rows, S14),
+ * ms[1] = the gather kernel that follows it (mode 0: all nodes; mode 1: the quads left over), ms[2] = material pre-pass.
  * Synchronises on the recorded events. */
 int fem_last_kernel_ms(fem_ctx *c, double ms[3] /*host*/);
 

@@ -75,10 +75,7 @@ __device__ __forceinline__ double atanhc(double w, double dlog /* = ln b - ln a 
     // branch-free (both forms are evaluated, one is selected) so that the calls of a thread interleave:
     // |w| < 0.15 : series 1 + w^2/3 + w^4/5 + ...  (11 terms, remainder < 1e-19), else ln(b/a) / (2 w)
     const double w2 = w * w;
-    double s = 1.0 / 21.0;
-    s = fma(s, w2, 1.0 / 19.0); s = fma(s, w2, 1.0 / 17.0); s = fma(s, w2, 1.0 / 15.0); s = fma(s, w2, 1.0 / 13.0);
-    s = fma(s, w2, 1.0 / 11.0); s = fma(s, w2, 1.0 / 9.0);  s = fma(s, w2, 1.0 / 7.0);  s = fma(s, w2, 1.0 / 5.0);
-    s = fma(s, w2, 1.0 / 3.0);  s = fma(s, w2, 1.0);
+    const double s = atanh_poly(w2);
     const double big = 0.5 * dlog * frcp(w);   // NaN for w = 0, never selected then
     return (w2 < 0.0225) ? s : big;
 }
@@ -131,12 +128,12 @@ __host__ __device__ constexpr int sidx9(int r, int c) {  // packed upper triangl
 __device__ __forceinline__ void flow_stress(double law, double h0, double h1, double h2, double alpha, double &sf,
                                             double &dsf) {
     if (law == 0.0) {  // Voce, Eq.(10) PAPER.md:121 (flow stress part; the sqrt(2/3) is applied by the caller, G2)
-        double ex = exp(-h2 * alpha);
+        double ex = fexp(-h2 * alpha);
         sf = fma(h1, 1.0 - ex, h0);
         dsf = h1 * h2 * ex;
     } else {           // Swift K (eps0 + alpha)^n (BASELINE.json configs)
         double b = h1 + alpha;
-        sf = h0 * exp(h2 * log(b));
+        sf = h0 * fexp(h2 * flog(b));
         dsf = h2 * sf * frcp(b);
     }
 }
@@ -469,7 +466,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
 #pragma unroll
         for (int a = 0; a < 3; a++) { w[a] = (lam[a] - 1.0) * frcp(lam[a] + 1.0); lg[a] = 2.0 * w[a] * atanhc(w[a], 0.0); }
 #pragma unroll
-        for (int a = 0; a < 3; a++) if (w[a] * w[a] >= 0.0225) lg[a] = log(lam[a]);
+        for (int a = 0; a < 3; a++) if (w[a] * w[a] >= 0.0225) lg[a] = flog(lam[a]);
     }
     double ee[6];  // elastic trial strain eps - eps_p_n, tensor components (11,22,33,12,23,13), material frame
     {
@@ -534,9 +531,10 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
                 ep1[4] = Th[1][0] * B[0][2] + Th[1][1] * B[1][2] + Th[1][2] * B[2][2];
                 ep1[5] = Th[0][0] * B[0][2] + Th[0][1] * B[1][2] + Th[0][2] * B[2][2];
             }
-            if (!plastic) {
+            if (!plastic) {   // elastic step: history copied unchanged (Eq.(18) :172), re-read rather than kept in registers
+                const double *hin = hist_in + (e * 8 + q) * 7;
 #pragma unroll
-                for (int i = 0; i < 6; i++) ep1[i] = epn[i];  // elastic step: history copied unchanged (Eq.(18) :172)
+                for (int i = 0; i < 6; i++) ep1[i] = __ldg(hin + i);
             }
 #pragma unroll
             for (int i = 0; i < 6; i++) ho[i] = ep1[i];
@@ -707,9 +705,10 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
             ep1[4] = Th[1][0] * B[0][2] + Th[1][1] * B[1][2] + Th[1][2] * B[2][2];
             ep1[5] = Th[0][0] * B[0][2] + Th[0][1] * B[1][2] + Th[0][2] * B[2][2];
         }
-        if (!plastic) {
+        if (!plastic) {   // elastic step: history copied unchanged (Eq.(18) :172), re-read rather than kept in registers
+            const double *hin = hist_in + (e * 8 + q) * 7;
 #pragma unroll
-            for (int i = 0; i < 6; i++) ep1[i] = epn[i];  // elastic step: history copied unchanged (Eq.(18) :172)
+            for (int i = 0; i < 6; i++) ep1[i] = __ldg(hin + i);
         }
 #pragma unroll
         for (int i = 0; i < 6; i++) ho[i] = ep1[i];
@@ -1261,7 +1260,7 @@ int fem_launch_assemble(fem_ctx *c, const double *u, const double *hist_in, cons
         FEM_CUDA(cudaMalloc(&c->d_matd, sizeof(double) * FEM_MATD * n_mat));
         c->n_matd_cap = n_mat;
     }
-    const bool fuse = c->fuse_ok && c->opt.assembly_mode == 0;
+    const bool fuse = c->fuse_ok && c->opt.assembly_mode == 1;
     FEM_CUDA(cudaMemsetAsync(c->d_stats, 0, sizeof(unsigned long long) * 72, st));
     if (fuse) FEM_CUDA(cudaMemsetAsync(c->d_left_count, 0, sizeof(unsigned int), st));
     FEM_CUDA(cudaEventRecord(c->ev[0], st));

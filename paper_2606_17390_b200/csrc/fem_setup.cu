@@ -398,7 +398,7 @@ extern "C" int fem_build_csr_pattern(fem_ctx *c, long long *n_rows, long long *n
                 TRY(cudaMalloc(&c->d_Re, sizeof(double) * 24 * ne));
                 TRY(cudaDeviceSynchronize());
             }
-            if (c->d_kvec && !c->has_high_valence) {
+            if (c->opt.assembly_mode == 1 && c->d_kvec && !c->has_high_valence) {
                 // fused, lagged gather: give every node quad to a warp of a chunk launched FUSE lag chunks after the last
                 // chunk that writes one of its records (one wave of resident CTAs + a margin), at most two quads per warp
                 const int EPC = 16, QPC = 8;                      // elements per CTA (fem_assemble.cu EL_PER_CTA), quads per chunk

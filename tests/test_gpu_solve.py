@@ -217,7 +217,7 @@ def test_fem_load_path_matches_oracle_loop(fbar, extrapolate):
 
 def test_balanced_state_with_local_nonconvergence_is_rejected():
     """an increment whose balanced state holds local solves that hit kmax is no root of the discrete problem.
-    With the local iteration cap at 2 the return map is cut short at every plastic point: fem_newton_solve must report
+    With the local iteration cap at 1 the return map is cut short at every plastic point: fem_newton_solve must report
     physics trouble, return FEM_ERR_NOCONV and restore u; fem_load_path must cut back and finally give up, leaving the
     last accepted state.  Overlapping history buffers are refused."""
     import torch
@@ -225,7 +225,7 @@ def test_balanced_state_with_local_nonconvergence_is_rejected():
     coords, conn, omat, rp, ci, h0, bc, val = clamped_shear_problem()
     dev = torch.device("cuda:0")
     ne = conn.shape[0]
-    ctx = fem.FemContext(torch.from_numpy(coords).to(dev), torch.from_numpy(conn).to(dev), kmax=2)
+    ctx = fem.FemContext(torch.from_numpy(coords).to(dev), torch.from_numpy(conn).to(dev), kmax=1)
     ctx.build_csr_pattern()
     mat = torch.from_numpy(fem.mat_from_desc(dict(synth.configs.SWIFT), ne).ravel()).to(dev)
     bc_d, val_d = torch.from_numpy(bc.astype(np.int32)).to(dev), torch.from_numpy(val).to(dev)
