@@ -113,7 +113,6 @@ __host__ __device__ constexpr int sidx9(int r, int c) {  // packed upper triangl
 #define SM_GB 840   // [24]     (F-bar) gbar
 #define SM_WQ 864   // [8]      (F-bar) w_q J_q / (Jbar V)
 #define ES_STD 564   // >= 560, = 4 mod 16: the 4 elements of a warp start in 4 different bank groups
-#define ES_FUSE 580  // >= 576, = 4 mod 16: the warp's four slots double as the gather buffer of four nodes (4 x 576 doubles)
 #define ES_FBAR 884  // >= 872, = 4 mod 16
 #ifndef EL_PER_CTA
 #define EL_PER_CTA 16
@@ -190,8 +189,9 @@ __device__ __forceinline__ void gather_reduce_write(long long n, int b, int m, c
         if (lane < 3) residual[3 * n + lane] = r;
     }
 }
-// One warp gathers up to 4 nodes (lane j < cnt holds node id nd): asynchronous 16-byte copies of the four runs into the
-// warp's shared-memory buffer (4 x 576 doubles) are all in flight before the first reduction starts.
+// One warp gathers up to NB nodes (lane j < cnt holds node id nd): asynchronous 16-byte copies of the runs into the
+// warp's shared-memory buffer (NB x 576 doubles) are all in flight before the first reduction starts.
+template <int NB>
 __device__ __forceinline__ void gather_warp_nodes(int nd, int cnt, double *wbuf, int lane, const int *__restrict__ inc_ptr,
                                                   const int *__restrict__ nb_ptr, const unsigned int *__restrict__ kvec,
                                                   const double *Ke, const double *Re, double *__restrict__ csr_vals,
@@ -199,7 +199,7 @@ __device__ __forceinline__ void gather_warp_nodes(int nd, int cnt, double *wbuf,
     int b = 0, m = 0;
     if (lane < cnt) { b = inc_ptr[nd]; m = inc_ptr[nd + 1] - b; }
 #pragma unroll
-    for (int j = 0; j < 4; j++) {
+    for (int j = 0; j < NB; j++) {
         const int bj = __shfl_sync(0xffffffffu, b, j), lim = 36 * __shfl_sync(0xffffffffu, m, j);
         const double *src = Ke + (long long)bj * 72;
 #pragma unroll
@@ -222,17 +222,31 @@ __device__ __forceinline__ void gather_warp_nodes(int nd, int cnt, double *wbuf,
 #ifndef PS_MASK
 #define PS_MASK 0x094   // measured best subset of the ten phase boundaries (sweep in DESIGN.md): before the return map, the tangent, phase 2
 #endif
-#define PHASE_SYNC_N(n) do { if ((PS_MASK >> (n)) & 1) __syncthreads(); } while (0)
+// barrier over the element warps of the CTA: the whole CTA, or (fused kernel) named barrier 1 over the element warpgroup
+template <int FUSE> __device__ __forceinline__ void el_sync() {
+    if (FUSE) asm volatile("bar.sync 1, 128;" ::: "memory");
+    else __syncthreads();
+}
+#define PHASE_SYNC_N(n) do { if ((PS_MASK >> (n)) & 1) el_sync<FUSE>(); } while (0)
 // Launch-time arguments of the assembly side of k_element.
-// Fused, lagged gather (FUSE = 1): the scratch is consumed while it is still in L2.  The nodes are cut into quads of
-// four consecutive ids; at setup every quad is given to one warp of an element CTA that is launched at least FUSE_LAG
-// chunks after the last chunk that contributes to the quad's nodes.  CTAs are dispatched in index order, so by then those
-// chunks have normally retired; each chunk publishes a completion flag (threadfence + flag = epoch of this call), the
-// gathering warp checks the flags of its quad's chunks WITHOUT waiting, and a quad that is not ready (or is scheduled
-// past the last chunk) goes to a short list that k_gather_list finishes after the element kernel.  Which warp sums a
-// node never changes the order of the sum, so results are bit-identical to the unfused path.
+// Fused, lagged gather (FUSE = 1): the scratch is consumed while it is still in L2, by warps that cost the element warps
+// almost nothing.  The CTA has two warpgroups: warps 0-3 evaluate the chunk's 16 elements exactly as in the unfused
+// kernel, warps 4-7 gather.  Measured: the element kernel loses only 9 % when it runs 2 CTAs per SM with 208 registers
+// instead of 3 with 168, which frees a third of the shared memory; `setmaxnreg` moves the
+// gather warps' registers to the element warps (2 CTAs x (128 x 208 + 128 x 48) = the whole register file).
+// The nodes are cut into quads of four consecutive ids; at setup every quad is given to one gather warp of a chunk
+// launched at least FUSE lag chunks (one wave of resident CTAs) after the last chunk that writes one of its records.
+// CTAs are dispatched in index order, so those chunks are resident or retired: each chunk publishes a completion flag
+// (threadfence + flag = epoch of this call); a gather warp polls the flags of its quad's chunks for a BOUNDED time (the
+// chunks it waits for never wait for anything), and a quad that still is not ready (or is scheduled past the last
+// chunk) goes to a short list that k_gather_list finishes after the element kernel.  Which warp sums a node never
+// changes the order of the sum, so results are bit-identical to the unfused path.
 #define FUSE_DEPW 16    // ints per quad dependency record: [0] = number of chunks (<= 15), [1..] chunk ids
-#define FUSE_QPC 8      // quads a CTA can be given (two per warp)
+#define FUSE_QPC 8      // quads a CTA can be given (two per gather warp)
+#define FUSE_EREGS 208   // registers per thread of the element warpgroup / the gather warpgroup after setmaxnreg
+#define FUSE_GREGS 48
+#define FUSE_GNB 2       // nodes a gather warp holds in shared memory at a time (2 x 4608 B)
+#define FUSE_POLLS 96   // bounded wait of a gather warp for its quad's chunks: polls of ~0.25 us
 struct scatter_args {
     const int *elist;   // element ids in processing order (the locality order built at setup for shuffled meshes); nullptr = identity
     const int *eslot;   // [e*8+I] -> scratch record of block row I (node-sorted incidence index)
@@ -252,8 +266,126 @@ struct scatter_args {
 #define EL_PF_DIST 444   // L2 prefetch distance in chunks (one wave of CTAs): 3.135 -> 3.108 ms; 888 and 1776 gain nothing
 #endif
 // YLD 0: Hill-48 (scalar return map); YLD 1: Barlat Yld2004-18p (fem_barlat.cuh), bard = derived Barlat records
+template <int N> __device__ __forceinline__ void reg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
+template <int N> __device__ __forceinline__ void reg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
+
+// The reduction of gather_reduce_write for a node with at most 8 incident elements (hence at most 27 <= 32 neighbours),
+// with every table value already in registers: kv = kvec entry of this lane's neighbour position, rv = R^e value of
+// lane 3 s + i.  Same sums in the same order.
+__device__ __forceinline__ void gather_reduce_pre(long long n, int m, int o, int len, unsigned kv, double rv, const double *buf,
+                                                  int lane, double *__restrict__ csr_vals, double *__restrict__ residual) {
+    // branch-free: a missing block (nibble 0xF, also every s >= m) reads block 0 of the record slot and adds +0.0, which
+    // leaves the sum unchanged bit for bit; without branches the loads of several records are in flight at once
+    double acc[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
+#pragma unroll
+    for (int s = 0; s < 8; s++) {
+        const unsigned K = (kv >> (4 * s)) & 15u;
+        const bool ok = K != 15u;
+        const double *rec = buf + s * 72 + (ok ? K : 0u);
+#pragma unroll
+        for (int j = 0; j < 9; j++) { const double v = rec[8 * j]; acc[j] += ok ? v : 0.0; }
+    }
+    if (lane < len) {
+        double *out = csr_vals + 9LL * o + 3 * lane;
+#pragma unroll
+        for (int i = 0; i < 3; i++) {
+            __stcs(out + (long long)i * 3 * len + 0, acc[3 * i + 0]);   // streaming stores: written once, not read by this call
+            __stcs(out + (long long)i * 3 * len + 1, acc[3 * i + 1]);
+            __stcs(out + (long long)i * 3 * len + 2, acc[3 * i + 2]);
+        }
+    }
+    double r = 0.0;
+    for (int j = 0; j < m; j++) r += __shfl_sync(0xffffffffu, rv, (3 * j + lane) & 31);
+    if (lane < 3) residual[3 * n + lane] = r;
+}
+
+// The gather warpgroup of the fused kernel (warps 4-7 of the CTA; gw = warp index in the group).  A warp is given up to
+// two quads = eight nodes; lane j holds the tables of node j (loaded once, before anything is known to be ready: they are
+// static).  The nodes of the quads whose chunks have all published their flag are then streamed through a two-slot
+// buffer: the records (and table values) of node i+1 are on their way while node i is reduced.
+__device__ __forceinline__ void fuse_gather_role(long long chunk, int gw, int lane, double *wbuf, const double *Ke, const double *Re,
+                                                 const scatter_args &sa) {
+    const int q0 = __ldg(sa.cta_quads + chunk * FUSE_QPC + 2 * gw), q1 = __ldg(sa.cta_quads + chunk * FUSE_QPC + 2 * gw + 1);
+    if ((q0 & q1) < 0 && q0 < 0 && q1 < 0) return;
+    // lane j < 8: node j of the two quads
+    const int myq = (lane < 4) ? q0 : q1;
+    long long node = -1;
+    if (lane < 8 && myq >= 0) { node = 4LL * myq + (lane & 3); if (node >= sa.n_nodes) node = -1; }
+    int b = 0, m = 0, o = 0, len = 0;
+    if (node >= 0) {
+        b = __ldg(sa.inc_ptr + node); m = __ldg(sa.inc_ptr + node + 1) - b;
+        o = __ldg(sa.nb_ptr + node); len = __ldg(sa.nb_ptr + node + 1) - o;
+    }
+    // readiness of the two quads: bounded polling of their chunks' flags (lanes 0-15: quad 0, lanes 16-31: quad 1)
+    unsigned live = 0;   // bit j: node j is to be gathered by this warp
+    {
+        const int qq = (lane < 16) ? q0 : q1, dl = lane & 15;
+        int nd = 0;
+        const volatile unsigned int *fl = sa.chunk_flag;
+        if (qq >= 0) {
+            const int *dep = sa.quad_deps + (long long)qq * FUSE_DEPW;
+            nd = __ldg(dep);
+            if (dl < nd) fl = sa.chunk_flag + __ldg(dep + 1 + dl);
+        }
+        unsigned okm = 0;
+#pragma unroll 1
+        for (int poll = 0; poll < FUSE_POLLS; poll++) {
+            const bool ok = (dl < nd) ? (*fl == sa.epoch) : true;
+            okm = __ballot_sync(0xffffffffu, ok);
+            if (okm == 0xffffffffu) break;
+            __nanosleep(250);
+        }
+        const bool r0 = (q0 >= 0) && ((okm & 0xffffu) == 0xffffu), r1 = (q1 >= 0) && ((okm >> 16) == 0xffffu);
+        if (lane == 0 && q0 >= 0 && !r0) sa.left_list[atomicAdd(sa.left_count, 1u)] = q0;
+        if (lane == 0 && q1 >= 0 && !r1) sa.left_list[atomicAdd(sa.left_count, 1u)] = q1;
+        live = __ballot_sync(0xffffffffu, node >= 0 && ((lane < 4) ? r0 : r1)) & 0xffu;
+    }
+    if (!live) return;
+    __threadfence();                         // the flags were read before any record is
+    // stream the live nodes through the two slots
+    int cur = __ffs(live) - 1;
+    live &= live - 1;
+    unsigned kv_c = 0xffffffffu, kv_n = 0xffffffffu;
+    double rv_c = 0.0, rv_n = 0.0;
+    int slot = 0;
+    {   // prologue: node `cur` -> slot 0
+        const int bj = __shfl_sync(0xffffffffu, b, cur), mj = __shfl_sync(0xffffffffu, m, cur), oj = __shfl_sync(0xffffffffu, o, cur),
+                  lj = __shfl_sync(0xffffffffu, len, cur);
+        const double *src = Ke + (long long)bj * 72;
+#pragma unroll
+        for (int it = 0; it < 9; it++) { const int idx = it * 32 + lane; if (idx < 36 * mj) cp_async16(wbuf + 2 * idx, src + 2 * idx); }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+        kv_c = (lane < lj) ? __ldg(sa.kvec + oj + lane) : 0xffffffffu;
+        rv_c = (lane < 3 * mj) ? __ldcg(Re + (long long)bj * 3 + lane) : 0.0;
+    }
+#pragma unroll 1
+    while (cur >= 0) {
+        const int nxt = live ? __ffs(live) - 1 : -1;
+        live &= live - 1;
+        if (nxt >= 0) {   // records and table values of the next node -> the other slot
+            const int bj = __shfl_sync(0xffffffffu, b, nxt), mj = __shfl_sync(0xffffffffu, m, nxt), oj = __shfl_sync(0xffffffffu, o, nxt),
+                      lj = __shfl_sync(0xffffffffu, len, nxt);
+            const double *src = Ke + (long long)bj * 72;
+            double *dst = wbuf + (slot ^ 1) * 576;
+#pragma unroll
+            for (int it = 0; it < 9; it++) { const int idx = it * 32 + lane; if (idx < 36 * mj) cp_async16(dst + 2 * idx, src + 2 * idx); }
+            kv_n = (lane < lj) ? __ldg(sa.kvec + oj + lane) : 0xffffffffu;
+            rv_n = (lane < 3 * mj) ? __ldcg(Re + (long long)bj * 3 + lane) : 0.0;
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+        asm volatile("cp.async.wait_group 1;" ::: "memory");     // everything but the newest group: the current node is in
+        __syncwarp();
+        const long long n = __shfl_sync(0xffffffffu, node, cur);
+        gather_reduce_pre(n, __shfl_sync(0xffffffffu, m, cur), __shfl_sync(0xffffffffu, o, cur), __shfl_sync(0xffffffffu, len, cur),
+                          kv_c, rv_c, wbuf + slot * 576, lane, sa.csr_vals, sa.residual);
+        __syncwarp();                        // the slot is free for the node after next
+        cur = nxt; kv_c = kv_n; rv_c = rv_n; slot ^= 1;
+    }
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
+}
+
 template <int FBAR, int FUSE, int YLD = 0>
-__global__ void __launch_bounds__(CTA_THREADS, (FBAR || YLD) ? CTAS_FBAR : CTAS_STD)
+__global__ void __launch_bounds__(FUSE ? 2 * CTA_THREADS : CTA_THREADS, FUSE ? 2 : ((FBAR || YLD) ? CTAS_FBAR : CTAS_STD))
 k_element(long long n_elems, const double *__restrict__ coords, const int *__restrict__ conn,
           const double *__restrict__ u, const double *__restrict__ hist_in, const double *__restrict__ matd,
           int mat_stride, double tol, int kmax, double *__restrict__ Ke, double *__restrict__ Re,
@@ -262,10 +394,19 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
     extern __shared__ __align__(16) double sm[];
     __shared__ unsigned int s_hist[64];
     __shared__ unsigned int s_done;
-    constexpr int ES = FBAR ? ES_FBAR : (FUSE ? ES_FUSE : ES_STD);
+    constexpr int ES = FBAR ? ES_FBAR : ES_STD;
     const int tid = threadIdx.x, lane = tid & 31, q = lane & 7;
-    const int el_cta = tid >> 3;
     const long long chunk = blockIdx.x;
+    if (FUSE) {
+        if (tid >= CTA_THREADS) {   // gather warpgroup: hands most of its registers to the element warpgroup
+            reg_dec<FUSE_GREGS>();
+            const int gw = (tid - CTA_THREADS) >> 5;
+            fuse_gather_role(chunk, gw, lane, sm + EL_PER_CTA * ES + gw * FUSE_GNB * 576, Ke, Re, sa);
+            return;
+        }
+        reg_inc<FUSE_EREGS>();
+    }
+    const int el_cta = tid >> 3;
     double *se = sm + el_cta * ES;
     const long long e_raw = chunk * EL_PER_CTA + el_cta;
     const bool valid = e_raw < n_elems;
@@ -296,29 +437,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
 #endif
     for (int j = tid; j < 64; j += CTA_THREADS) s_hist[j] = 0;
     if (tid == 0) s_done = 0;
-    if (FUSE) {
-        // ---- S14 for the quads this warp was given at setup, while its own inputs are on their way: the records of those
-        //      nodes were written by chunks launched at least FUSE_LAG chunks ago and are read back from L2
-        double *wbuf = sm + (tid >> 5) * 4 * ES;     // the warp's four element slots (>= 4 x 576 doubles), not yet in use
-#pragma unroll 1
-        for (int k = 0; k < 2; k++) {
-            const int quad = __ldg(sa.cta_quads + chunk * FUSE_QPC + 2 * (tid >> 5) + k);
-            if (quad < 0) continue;                  // warp-uniform
-            const int *dep = sa.quad_deps + (long long)quad * FUSE_DEPW;
-            const int nd = __ldg(dep);
-            bool ok = true;
-            if (lane < nd) ok = (*reinterpret_cast<volatile unsigned int *>(sa.chunk_flag + __ldg(dep + 1 + lane)) == sa.epoch);
-            if (__all_sync(0xffffffffu, ok)) {
-                __threadfence();                     // the flags were read before any record is
-                const long long n0 = 4LL * quad;
-                const int cnt = (int)min(4LL, sa.n_nodes - n0);
-                gather_warp_nodes((int)n0 + lane, cnt, wbuf, lane, sa.inc_ptr, sa.nb_ptr, sa.kvec, Ke, Re, sa.csr_vals, sa.residual);
-            } else if (lane == 0) {
-                sa.left_list[atomicAdd(sa.left_count, 1u)] = quad;
-            }
-        }
-    }
-    __syncthreads();
+    el_sync<FUSE>();
   {
 #pragma unroll
     for (int i = 0; i < 3; i++) { se[SM_XE + 3 * q + i] = xn[i]; se[SM_UE + 3 * q + i] = un[i]; }
@@ -1102,7 +1221,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
     if (FUSE) {
         // publish: every thread's records are visible device-wide (fence) before the chunk's flag takes this call's epoch
         __threadfence();
-        __syncthreads();
+        el_sync<FUSE>();
         if (tid == 0) *reinterpret_cast<volatile unsigned int *>(sa.chunk_flag + chunk) = sa.epoch;
     }
     {
@@ -1110,7 +1229,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
         unsigned done = 0;
         if (lane == 0) { __threadfence_block(); done = atomicAdd(&s_done, 1u); }
         done = __shfl_sync(0xffffffffu, done, 0);
-        if (done == (blockDim.x >> 5) - 1) {   // last warp of the CTA: flush (no CTA-wide barrier at the tail)
+        if (done == (CTA_THREADS >> 5) - 1) {   // last element warp of the CTA: flush (no CTA-wide barrier at the tail)
             __threadfence_block();
             for (int b = lane; b < 64; b += 32) {
                 const unsigned v = s_hist[b];
@@ -1222,7 +1341,7 @@ k_gather_list(long long n_nodes, const int *__restrict__ tail, int n_tail, const
         const int quad = (it < n_tail) ? tail[it] : left[it - n_tail];
         const long long n0 = 4LL * quad;
         const int cnt = (int)min(4LL, n_nodes - n0);
-        gather_warp_nodes((int)n0 + lane, cnt, dbuf + w * 2304, lane, inc_ptr, nb_ptr, kvec, Ke, Re, csr_vals, residual);
+        gather_warp_nodes<4>((int)n0 + lane, cnt, dbuf + w * 2304, lane, inc_ptr, nb_ptr, kvec, Ke, Re, csr_vals, residual);
     }
 }
 
@@ -1232,15 +1351,15 @@ static inline unsigned nblk2(long long n, int bs) { return (unsigned)((n + bs - 
 template <int FBAR, int FUSE, int YLD>
 static int launch_element(fem_ctx *c, const double *u, const double *hist_in, int mstride, double *hist_out, const scatter_args &sa,
                           int bstride, cudaStream_t st) {
-    constexpr int ES = FBAR ? ES_FBAR : (FUSE ? ES_FUSE : ES_STD);
-    const size_t smem = (size_t)EL_PER_CTA * ES * sizeof(double);
+    constexpr int ES = FBAR ? ES_FBAR : ES_STD;
+    const size_t smem = ((size_t)EL_PER_CTA * ES + (FUSE ? 4 * FUSE_GNB * 576 : 0)) * sizeof(double);
     // the opt-in for > 48 KB of dynamic shared memory is per device and per kernel: remembered per context (= per device)
     const int slot = (FBAR ? 1 : 0) + 2 * (FUSE ? 1 : 0) + 4 * (YLD ? 1 : 0);
     if (!(c->attr_mask & (1u << slot))) {
         FEM_CUDA(cudaFuncSetAttribute(k_element<FBAR, FUSE, YLD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         c->attr_mask |= 1u << slot;
     }
-    k_element<FBAR, FUSE, YLD><<<nblk2(c->n_elems, EL_PER_CTA), CTA_THREADS, smem, st>>>(
+    k_element<FBAR, FUSE, YLD><<<nblk2(c->n_elems, EL_PER_CTA), FUSE ? 2 * CTA_THREADS : CTA_THREADS, smem, st>>>(
         c->n_elems, c->d_coords, c->d_conn, u, hist_in, c->d_matd, mstride, c->opt.tol, c->opt.kmax, c->d_Ke, c->d_Re, hist_out,
         c->d_stats, sa, YLD ? c->d_bard : nullptr, bstride);
     return FEM_OK;
@@ -1260,7 +1379,8 @@ int fem_launch_assemble(fem_ctx *c, const double *u, const double *hist_in, cons
         FEM_CUDA(cudaMalloc(&c->d_matd, sizeof(double) * FEM_MATD * n_mat));
         c->n_matd_cap = n_mat;
     }
-    const bool fuse = c->fuse_ok && c->opt.assembly_mode == 1;
+    // the fused kernel exists for the Hill-48 standard element (the F-bar and Yld2004-18p variants need all shared memory / registers)
+    const bool fuse = c->fuse_ok && c->opt.assembly_mode == 1 && !c->opt.fbar && !bar;
     FEM_CUDA(cudaMemsetAsync(c->d_stats, 0, sizeof(unsigned long long) * 72, st));
     if (fuse) FEM_CUDA(cudaMemsetAsync(c->d_left_count, 0, sizeof(unsigned int), st));
     FEM_CUDA(cudaEventRecord(c->ev[0], st));
@@ -1275,14 +1395,11 @@ int fem_launch_assemble(fem_ctx *c, const double *u, const double *hist_in, cons
     scatter_args sa = {c->d_eorder, c->d_eslot, c->d_cta_quads, c->d_quad_deps, c->d_chunk_flag, c->epoch, c->d_left_list,
                        c->d_left_count, c->n_nodes, c->d_inc_ptr, c->d_nb_ptr, c->d_kvec, csr_vals, residual};
     int rc;
-    if (bar)       rc = c->opt.fbar ? (fuse ? launch_element<1, 1, 1>(c, u, hist_in, mstride, hist_out, sa, bstride, st)
-                                            : launch_element<1, 0, 1>(c, u, hist_in, mstride, hist_out, sa, bstride, st))
-                                    : (fuse ? launch_element<0, 1, 1>(c, u, hist_in, mstride, hist_out, sa, bstride, st)
-                                            : launch_element<0, 0, 1>(c, u, hist_in, mstride, hist_out, sa, bstride, st));
-    else           rc = c->opt.fbar ? (fuse ? launch_element<1, 1, 0>(c, u, hist_in, mstride, hist_out, sa, 0, st)
-                                            : launch_element<1, 0, 0>(c, u, hist_in, mstride, hist_out, sa, 0, st))
-                                    : (fuse ? launch_element<0, 1, 0>(c, u, hist_in, mstride, hist_out, sa, 0, st)
-                                            : launch_element<0, 0, 0>(c, u, hist_in, mstride, hist_out, sa, 0, st));
+    if (bar)              rc = c->opt.fbar ? launch_element<1, 0, 1>(c, u, hist_in, mstride, hist_out, sa, bstride, st)
+                                           : launch_element<0, 0, 1>(c, u, hist_in, mstride, hist_out, sa, bstride, st);
+    else if (c->opt.fbar) rc = launch_element<1, 0, 0>(c, u, hist_in, mstride, hist_out, sa, 0, st);
+    else if (fuse)        rc = launch_element<0, 1, 0>(c, u, hist_in, mstride, hist_out, sa, 0, st);
+    else                  rc = launch_element<0, 0, 0>(c, u, hist_in, mstride, hist_out, sa, 0, st);
     if (rc != FEM_OK) return rc;
     FEM_CUDA(cudaEventRecord(c->ev[2], st));
     if (fuse) {

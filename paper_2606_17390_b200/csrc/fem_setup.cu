@@ -399,11 +399,11 @@ extern "C" int fem_build_csr_pattern(fem_ctx *c, long long *n_rows, long long *n
                 TRY(cudaDeviceSynchronize());
             }
             if (c->opt.assembly_mode == 1 && c->d_kvec && !c->has_high_valence) {
-                // fused, lagged gather: give every node quad to a warp of a chunk launched FUSE lag chunks after the last
+                // fused, lagged gather: give every node quad to a gather warp of a chunk launched `lag` chunks after the last
                 // chunk that writes one of its records (one wave of resident CTAs + a margin), at most two quads per warp
                 const int EPC = 16, QPC = 8;                      // elements per CTA (fem_assemble.cu EL_PER_CTA), quads per chunk
                 const long long n_chunks = (ne + EPC - 1) / EPC, n_quads = (nn + 3) / 4;
-                const long long lag = 3LL * c->n_sm + 64;
+                const long long lag = 2LL * c->n_sm + 32;    // the fused kernel runs 2 CTAs per SM: one wave + a margin (328 ... 1000 measured alike)
                 int *epos = nullptr, *d_ready = nullptr;
                 if (c->d_eorder) {
                     TRY(cudaMalloc(&epos, sizeof(int) * ne));
@@ -423,6 +423,7 @@ extern "C" int fem_build_csr_pattern(fem_ctx *c, long long *n_rows, long long *n
                     for (long long i = 0; i <= n_chunks; i++) nxt[i] = (int)i;       // next chunk >= i with a free slot (path-compressed)
                     for (long long i = 0; i < n_chunks; i++) fill[i] = 0;
                     static const int order[8] = {0, 2, 4, 6, 1, 3, 5, 7};             // one quad per warp first, then the second
+                    const int cap = QPC;
                     for (long long qd = 0; qd < n_quads; qd++) {
                         long long want = (ready[qd] == 0x7fffffff) ? n_chunks : (long long)ready[qd] + lag;
                         if (want < 0) want = 0;
@@ -432,7 +433,7 @@ extern "C" int fem_build_csr_pattern(fem_ctx *c, long long *n_rows, long long *n
                         for (long long i = want; nxt[i] != r;) { const long long j = nxt[i]; nxt[i] = (int)r; i = j; }
                         if (r >= n_chunks) { tail[n_tail++] = (int)qd; continue; }
                         cq[r * QPC + order[fill[r]++]] = (int)qd;
-                        if (fill[r] == QPC) nxt[r] = (int)(r + 1);
+                        if (fill[r] == cap) nxt[r] = (int)(r + 1);
                     }
                 }
                 if (ok && ce == cudaSuccess) ce = cudaMalloc(&c->d_cta_quads, sizeof(int) * n_chunks * QPC);

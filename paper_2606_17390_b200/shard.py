@@ -31,25 +31,43 @@ def partition(n_nodes, conn, world, rank):
     return dict(n0=n0, n1=n1, elems=elems, lnodes=lnodes, lconn=lconn, lo=lo, hi=hi, world=world, rank=rank, n_nodes=n_nodes)
 
 
-def exchange_u(u_owned, part, group=None):
+def exchange_plan(part, device):
+    """Index tensors of exchange_u built once per partition (no host work inside the timed step): for every local node its
+    row in the padded all-gather buffer [world, width/3, 3]."""
+    import torch
+    world, n_nodes = part["world"], part["n_nodes"]
+    bounds = np.array([((r * n_nodes) // world, ((r + 1) * n_nodes) // world) for r in range(world)], dtype=np.int64)
+    width = int((bounds[:, 1] - bounds[:, 0]).max())
+    ln = part["lnodes"].astype(np.int64)
+    owner = np.searchsorted(bounds[:, 1], ln, side="right")
+    gidx = owner * width + (ln - bounds[owner, 0])
+    return dict(width=width, gidx=torch.from_numpy(gidx).to(device))
+
+
+def exchange_u(u_owned, part, group=None, plan=None):
     """The one collective of the sharded path: all-gather of the owned displacement slabs (padded to the largest slab, NCCL
     needs equal counts) -> the displacement of this rank's local nodes, owned and ghost.  u_owned: [3 (n1-n0)] torch tensor
     on the device of the process group's backend; world 1 needs no process group."""
     import torch
-    world, n_nodes = part["world"], part["n_nodes"]
-    bounds = [((r * n_nodes) // world, ((r + 1) * n_nodes) // world) for r in range(world)]
+    world = part["world"]
+    if plan is None:
+        plan = exchange_plan(part, u_owned.device)
+    width = plan["width"]
     if world == 1:
-        full = u_owned
+        full = u_owned.view(-1, 3)
     else:
         import torch.distributed as dist
-        width = 3 * max(b - a for a, b in bounds)
-        send = torch.zeros(width, dtype=u_owned.dtype, device=u_owned.device)
+        send = torch.zeros(3 * width, dtype=u_owned.dtype, device=u_owned.device)
         send[:u_owned.numel()] = u_owned
-        recv = [torch.empty_like(send) for _ in range(world)]
-        dist.all_gather(recv, send, group=group)
-        full = torch.cat([recv[r][:3 * (b - a)] for r, (a, b) in enumerate(bounds)])
-    idx = torch.from_numpy(part["lnodes"].astype(np.int64)).to(full.device)
-    return full.view(-1, 3)[idx].reshape(-1).contiguous()
+        recv = torch.empty(world * 3 * width, dtype=u_owned.dtype, device=u_owned.device)
+        dist.all_gather_into_tensor(recv, send, group=group)
+        full = recv.view(-1, 3)
+    return full[plan["gidx"]].reshape(-1).contiguous()
+
+
+def owned_nnz(row_ptr, part):
+    """Number of CSR entries in the rows this rank owns, from the local pattern's row_ptr."""
+    return int(row_ptr[3 * part["hi"]]) - int(row_ptr[3 * part["lo"]])
 
 
 class ShardedFem:
