@@ -161,9 +161,12 @@ __device__ __noinline__ void bar_eval_t(const double *__restrict__ bd, const dou
             sb = -sb * (double)(m - k) / (double)(k + 1);
         }
     }
-    const double phi = exp(log(0.25 * Phi) / m);
+    // phi = (Phi/4)^(1/m): three nested square roots for m = 8 (the paper's exponent), exp(ln/m) otherwise
+    double phi;
+    if (M == 8) { double r = 0.25 * Phi; r = r * frsqrt(r); r = r * frsqrt(r); phi = r * frsqrt(r); }
+    else phi = fexp(flog(0.25 * Phi) / m);
     phi_out = phi;
-    const double cf = phi / (m * Phi);   // dphi = phi^(1-m)/(4m) dPhi, 4 phi^m = Phi
+    const double cf = phi * frcp(m * Phi);   // dphi = phi^(1-m)/(4m) dPhi, 4 phi^m = Phi
     double GA[6], GB[6];
 #pragma unroll
     for (int i = 0; i < 6; i++) {
@@ -261,7 +264,7 @@ __device__ __noinline__ void bar_eval_t(const double *__restrict__ bd, const dou
 #pragma unroll
             for (int B = A; B < 6; B++) d2[A][B] += lu[A] * lb[B] + lb[A] * lu[B];
     }
-    const double cn = (m - 1.0) / phi;
+    const double cn = (m - 1.0) * frcp(phi);
 #pragma unroll
     for (int A = 0; A < 6; A++)
 #pragma unroll
@@ -276,15 +279,16 @@ __device__ __forceinline__ void bar_eval(const double *__restrict__ bd, const do
     else bar_eval_t<0>(bd, T, want_H, phi_out, N, H);
 }
 
-// In-place Cholesky M = L L^T of a symmetric positive definite 6x6 (lower triangle of M on entry, L on exit).
+// In-place Cholesky M = L L^T of a symmetric positive definite 6x6 (lower triangle of M on entry; on exit the strict lower
+// triangle of L and, on the diagonal, the RECIPROCALS 1/L_jj, so that the solves multiply instead of dividing).
 __device__ __forceinline__ void chol6(double M[6][6]) {
 #pragma unroll
     for (int j = 0; j < 6; j++) {
         double d = M[j][j];
 #pragma unroll
         for (int k = 0; k < j; k++) d = fma(-M[j][k], M[j][k], d);
-        const double id = rsqrt(d);
-        M[j][j] = d * id;
+        const double id = frsqrt(d);
+        M[j][j] = id;
 #pragma unroll
         for (int i = j + 1; i < 6; i++) {
             double s = M[i][j];
@@ -301,14 +305,14 @@ __device__ __forceinline__ void chol6_solve(const double L[6][6], const double r
         double s = rhs[i];
 #pragma unroll
         for (int k = 0; k < i; k++) s = fma(-L[i][k], y[k], s);
-        y[i] = s / L[i][i];
+        y[i] = s * L[i][i];
     }
 #pragma unroll
     for (int i = 5; i >= 0; i--) {
         double s = y[i];
 #pragma unroll
         for (int k = i + 1; k < 6; k++) s = fma(-L[k][i], x[k], s);
-        x[i] = s / L[i][i];
+        x[i] = s * L[i][i];
     }
 }
 
@@ -340,7 +344,7 @@ __device__ __noinline__ void bar_return_map(const double *__restrict__ bd, doubl
 #pragma unroll
         for (int B = A; B < 6; B++) Cep[A][B] = ((A < 3 && B < 3) ? kb - mu2 * (1.0 / 3.0) : 0.0) + ((A == B) ? mu2 : 0.0);
     if (!plastic) return;
-    const double is0 = 1.0 / s0;
+    const double is0 = frcp(s0);
     const double tolG = 1e-13 * fmax(1.0, sqrt(tn2) * is0);
     double dg = 0.0, sy = s0, dsy = ds0, prev = INFINITY;
 #if BAR_START
@@ -354,12 +358,12 @@ __device__ __noinline__ void bar_return_map(const double *__restrict__ bd, doubl
         for (int i = 0; i < 6; i++) nn = fma(N[i], N[i], nn);
         const double a = mu2 * nn;
         for (int it = 0; it < 6; it++) {   // convex, decreasing: Newton from dgam = 0 approaches the root from the left
-            const double g = phi - a * dg - sy, d = g / (a + dsy);
+            const double g = phi - a * dg - sy, d = g * frcp(a + dsy);
             dg += d;
             flow_stress(law, hh0, hh1, hh2, alphan + dg, sy, dsy);
             if (d <= 1e-3 * dg) break;
         }
-        const double c = sy / phi, ic = phi / sy;
+        const double c = sy * frcp(phi), ic = phi * frcp(sy);
 #pragma unroll
         for (int i = 0; i < 6; i++) T[i] = (i < 3) ? fma(c, Ttr[i] - pres, pres) : c * Ttr[i];
         phi = sy;
@@ -402,7 +406,7 @@ __device__ __noinline__ void bar_return_map(const double *__restrict__ bd, doubl
         double nx1 = 0.0, nx2 = 0.0;
 #pragma unroll
         for (int i = 0; i < 6; i++) { nx1 = fma(N[i], x1[i], nx1); nx2 = fma(N[i], x2[i], nx2); }
-        const double ddg = (fv * s0 - nx1) / fma(mu2, nx2, dsy);
+        const double ddg = (fv * s0 - nx1) * frcp(fma(mu2, nx2, dsy));
         double dT[6];
 #pragma unroll
         for (int i = 0; i < 6; i++) dT[i] = -fma(mu2 * ddg, x2[i], x1[i]);
@@ -419,7 +423,7 @@ __device__ __noinline__ void bar_return_map(const double *__restrict__ bd, doubl
             BAR_RESID(Tt, dgt, Nt, phit, syt, GTt, ft, psit);
             accepted0 = (j == 0);
             if (psit < (1.0 - 2.0e-4 * zeta) * psi0 || j >= 12) break;          // Eq.(B3)
-            const double zn = psi0 / (psi0 + psit);                                // Eq.(B5)/(B6)
+            const double zn = psi0 * frcp(psi0 + psit);                                // Eq.(B5)/(B6)
             zeta = (j == 0) ? zn : fmax(0.1 * zj, zn);                             // Eq.(B7)
             zj = zeta;
         }
@@ -460,13 +464,13 @@ __device__ __noinline__ void bar_return_map(const double *__restrict__ bd, doubl
             double s = (i == j) ? 1.0 : 0.0;
 #pragma unroll
             for (int k = j; k < i; k++) s = fma(-M[i][k], Li[k][j], s);
-            Li[i][j] = s / M[i][i];
+            Li[i][j] = s * M[i][i];
         }
     }
     double nx2 = 0.0;
 #pragma unroll
     for (int i = 0; i < 6; i++) nx2 = fma(N[i], x2[i], nx2);
-    const double cden = mu2 * mu2 / fma(mu2, nx2, dsy);
+    const double cden = mu2 * mu2 * frcp(fma(mu2, nx2, dsy));
 #pragma unroll
     for (int A = 0; A < 6; A++)
 #pragma unroll

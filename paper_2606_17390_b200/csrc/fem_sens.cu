@@ -122,20 +122,20 @@ __device__ __forceinline__ void applyDinv(const SDinv &D, const double a[6], dou
 // sigma_flow and d sigma_flow/d alpha: Voce Eq.(10) :121, Swift (BASELINE configs)
 __device__ __forceinline__ void flow2(const SMat &m, double alpha, double &sf, double &dsf) {
     if (m.law == 0.0) {
-        const double e = exp(-m.h2 * alpha);
+        const double e = fexp(-m.h2 * alpha);
         sf = m.h0 + m.h1 * (1.0 - e); dsf = m.h1 * m.h2 * e;
     } else {
-        const double b = m.h1 + alpha, pw = exp(m.h2 * log(b));
+        const double b = m.h1 + alpha, pw = fexp(m.h2 * flog(b));
         sf = m.h0 * pw; dsf = m.h0 * m.h2 * pw * frcp(b);
     }
 }
 // d sigma_flow/d(h0,h1,h2)
 __device__ __forceinline__ void flow_dh(const SMat &m, double alpha, double dh[3]) {
     if (m.law == 0.0) {
-        const double e = exp(-m.h2 * alpha);
+        const double e = fexp(-m.h2 * alpha);
         dh[0] = 1.0; dh[1] = 1.0 - e; dh[2] = m.h1 * alpha * e;
     } else {
-        const double b = m.h1 + alpha, lb = log(b), pw = exp(m.h2 * lb);
+        const double b = m.h1 + alpha, lb = flog(b), pw = fexp(m.h2 * lb);
         dh[0] = pw; dh[1] = m.h0 * m.h2 * pw * frcp(b); dh[2] = m.h0 * pw * lb;
     }
 }
@@ -153,10 +153,7 @@ __device__ __forceinline__ void hill_bilinear_ds(const double x[6], const double
 // atanh(w)/w / (a+b), w = (a-b)/(a+b), by its series for |w| < 0.15 (remainder < 1e-19), else (ga - gb)/(a - b)
 __device__ __forceinline__ double g_dd1(double a, double b, double ga, double gb) {
     const double is = frcp(a + b), w = (a - b) * is, w2 = w * w;
-    double s = 1.0 / 21.0;
-    s = fma(s, w2, 1.0 / 19.0); s = fma(s, w2, 1.0 / 17.0); s = fma(s, w2, 1.0 / 15.0); s = fma(s, w2, 1.0 / 13.0);
-    s = fma(s, w2, 1.0 / 11.0); s = fma(s, w2, 1.0 / 9.0);  s = fma(s, w2, 1.0 / 7.0);  s = fma(s, w2, 1.0 / 5.0);
-    s = fma(s, w2, 1.0 / 3.0);  s = fma(s, w2, 1.0);
+    const double s = atanh_poly(w2);
     const double big = (ga - gb) * frcp((w2 < 0.0225) ? 1.0 : a - b);
     return (w2 < 0.0225) ? s * is : big;
 }
@@ -250,7 +247,7 @@ k_sens_point(long long n_elems, const double *__restrict__ coords, const int *__
             Ji[1][0] = Jr[1][2] * Jr[2][0] - Jr[1][0] * Jr[2][2]; Ji[1][1] = Jr[0][0] * Jr[2][2] - Jr[0][2] * Jr[2][0]; Ji[1][2] = Jr[0][2] * Jr[1][0] - Jr[0][0] * Jr[1][2];
             Ji[2][0] = Jr[1][0] * Jr[2][1] - Jr[1][1] * Jr[2][0]; Ji[2][1] = Jr[0][1] * Jr[2][0] - Jr[0][0] * Jr[2][1]; Ji[2][2] = Jr[0][0] * Jr[1][1] - Jr[0][1] * Jr[1][0];
             wq = Jr[0][0] * Ji[0][0] + Jr[0][1] * Ji[1][0] + Jr[0][2] * Ji[2][0];   // det J_ref, weights 1
-            const double iw = 1.0 / wq;
+            const double iw = frcp(wq);
             double JT[3][3];   // J_ref^-1 Theta
 #pragma unroll
             for (int i = 0; i < 3; i++)
@@ -307,7 +304,7 @@ k_sens_point(long long n_elems, const double *__restrict__ coords, const int *__
             lm[0] = c00; lm[1] = c11; lm[2] = c22;
         }
 #pragma unroll
-        for (int a = 0; a < 3; a++) gl[a] = 0.5 * log(lm[a]);
+        for (int a = 0; a < 3; a++) gl[a] = 0.5 * flog(lm[a]);
         double ee[6];
         {
             const double eh[6] = {gl[0], gl[1], gl[2], 0, 0, 0};
