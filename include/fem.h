@@ -54,19 +54,23 @@ typedef struct {
     int jmax;          /* kept for ABI parity with Alg. C2's line search; the scalar solve
                           uses a bracket instead, so it is unused */
     double beta, eta;  /* Alg. C2 / App. B constants; unused by the scalar solve */
-    int assembly_mode; /* How S14 (K = A K^e, R = A R^e, Eq.(34) :253, Eq.(38) :274) is scheduled; the result is bit-identical in both.
+    int assembly_mode; /* How S14 (K = A K^e, R = A R^e, Eq.(34) :253, Eq.(38) :274) is scheduled; the result is bit-identical in all modes.
                           The element kernel writes K^e, R^e to a destination-major scratch (one 72-double record per
                           (element, local node), node-sorted), and every CSR entry is the sum of its records in ascending element
                           id (deterministic, no atomics).
-                          0 (default) = the element kernel, then a stand-alone node-row gather kernel over all nodes (nodes with
+                          1 = two kernels: the element kernel, then a stand-alone node-row gather kernel over all nodes (nodes with
                           more than 8 elements / collapsed elements take a general path in it).
-                          1 = fused, lagged gather (experimental, measured slower at config 3): at
-                          pattern-build time the nodes are cut into quads of four and every quad is given to one warp of an
-                          element CTA that is launched at least one wave of resident CTAs after the last CTA that writes one of
-                          its records; that warp sums the quad's CSR rows at the start of its CTA, reading the records back from
-                          L2.  Completion is tracked by one flag per CTA; a warp never waits: a quad that is not ready (or is
-                          scheduled past the last CTA) is finished by a short gather kernel after the element launch.  Meshes
-                          with collapsed elements or a node with more than 8 elements fall back to mode 0. */
+                          2 = fused, lagged gather: the element kernel's CTAs carry a second warpgroup that gathers.  At
+                          pattern-build time the nodes are cut into quads of four and every quad is given to one gather warp of
+                          an element CTA that is launched at least one wave of resident CTAs after the last CTA that writes one
+                          of its records; that warp sums the quad's CSR rows while the CTA's element warps evaluate their own 16
+                          elements, reading the records back from L2 (they are then discarded there and never reach HBM).
+                          Completion is tracked by one flag per CTA; a gather warp polls for a bounded time only, and a quad
+                          that is not ready (or is scheduled past the last CTA) is finished by a short gather kernel after the
+                          element launch.  Hill-48 standard element only; F-bar, fem_assemble_barlat, meshes with collapsed
+                          elements or a node with more than 8 elements use mode 1.
+                          0 (default) = mode 2 where it is the faster one (standard element, at least 8 waves of element CTAs,
+                          about 42k elements on a B200), mode 1 otherwise. */
 } fem_options;
 
 typedef struct {
@@ -141,8 +145,8 @@ int fem_assemble_host(fem_ctx *c, const double *u, const double *hist_in, const 
                       double *residual, double *csr_vals, double *hist_out, fem_stats *stats);
 
 /* Device time in milliseconds of the kernels of the last fem_assemble on this context, measured with CUDA events
- * on the call's stream: ms[0] = element kernel (S2-S12; in assembly_mode 1 it also gathers most node rows, S14),
- * ms[1] = the gather kernel that follows it (mode 0: all nodes; mode 1: the quads left over), ms[2] = material pre-pass.
+ * on the call's stream: ms[0] = element kernel (S2-S12; in the fused mode it also gathers most node rows, S14),
+ * ms[1] = the gather kernel that follows it (two-kernel mode: all nodes; fused mode: the quads left over), ms[2] = material pre-pass.
  * Synchronises on the recorded events. */
 int fem_last_kernel_ms(fem_ctx *c, double ms[3] /*host*/);
 

@@ -148,6 +148,29 @@ __device__ __forceinline__ void cp_async16(void *smem_dst, const void *gsrc) {
     const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_dst);
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sa), "l"(gsrc) : "memory");
 }
+// L2 residency hints of the fused kernel: the scratch records are written once and read back once, ~one wave of CTAs
+// later, so they are stored with an evict-last policy and read with evict-first; everything that streams (history, CSR
+// values) is marked evict-first, so that it does not push the records out of the 126 MB L2 before they are consumed.
+__device__ __forceinline__ unsigned long long l2_policy_last() {
+    unsigned long long p;
+    asm("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ unsigned long long l2_policy_first() {
+    unsigned long long p;
+    asm("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ void st_hint(double *ptr, double a, unsigned long long pol) {
+    asm volatile("st.global.L2::cache_hint.f64 [%0], %1, %2;" ::"l"(ptr), "d"(a), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void st_hint2(double *ptr, double a, double b, unsigned long long pol) {
+    asm volatile("st.global.L2::cache_hint.v2.f64 [%0], {%1, %2}, %3;" ::"l"(ptr), "d"(a), "d"(b), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void cp_async16_hint(void *smem_dst, const void *gsrc, unsigned long long pol) {
+    const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2;" ::"r"(sa), "l"(gsrc), "l"(pol) : "memory");
+}
 // K = A K^e, R = A R^e (Eq.(34) :253, Eq.(38) :274) for one node whose run of records sits in shared memory (buf).
 // kvec[block] (built at setup) holds, for each incident entry s, the local node K of the block's column node (nibble s;
 // 0xF = that element does not contain it), so lane = neighbour position adds <= 8 blocks in ascending s (fixed order, no
@@ -220,7 +243,7 @@ __device__ __forceinline__ void gather_warp_nodes(int nd, int cnt, double *wbuf,
 // Keeping the warps of a CTA in the same code region lets them share instruction-cache lines (the kernel is ~94 KB of
 // straight-line SASS); ncu showed instruction fetch as a top stall without it.
 #ifndef PS_MASK
-#define PS_MASK 0x094   // measured best subset of the ten phase boundaries (sweep in DESIGN.md): before the return map, the tangent, phase 2
+#define PS_MASK 0x010   // measured best subset of the ten phase boundaries (sweeps in DESIGN.md): one barrier, before the tangent
 #endif
 // barrier over the element warps of the CTA: the whole CTA, or (fused kernel) named barrier 1 over the element warpgroup
 template <int FUSE> __device__ __forceinline__ void el_sync() {
@@ -246,6 +269,9 @@ template <int FUSE> __device__ __forceinline__ void el_sync() {
 #define FUSE_EREGS 208   // registers per thread of the element warpgroup / the gather warpgroup after setmaxnreg
 #define FUSE_GREGS 48
 #define FUSE_GNB 2       // nodes a gather warp holds in shared memory at a time (2 x 4608 B)
+#ifndef FUSE_DISCARD
+#define FUSE_DISCARD 1
+#endif
 #define FUSE_POLLS 96   // bounded wait of a gather warp for its quad's chunks: polls of ~0.25 us
 struct scatter_args {
     const int *elist;   // element ids in processing order (the locality order built at setup for shuffled meshes); nullptr = identity
@@ -273,17 +299,18 @@ template <int N> __device__ __forceinline__ void reg_dec() { asm volatile("setma
 // with every table value already in registers: kv = kvec entry of this lane's neighbour position, rv = R^e value of
 // lane 3 s + i.  Same sums in the same order.
 __device__ __forceinline__ void gather_reduce_pre(long long n, int m, int o, int len, unsigned kv, double rv, const double *buf,
-                                                  int lane, double *__restrict__ csr_vals, double *__restrict__ residual) {
-    // branch-free: a missing block (nibble 0xF, also every s >= m) reads block 0 of the record slot and adds +0.0, which
-    // leaves the sum unchanged bit for bit; without branches the loads of several records are in flight at once
+                                                  const double *zero, int lane, double *__restrict__ csr_vals,
+                                                  double *__restrict__ residual) {
+    // branch-free and select-free: a missing block (nibble 0xF, also every s >= m) is read from `zero`, 65 doubles of +0.0
+    // in shared memory; adding +0.0 leaves a sum that started at +0.0 unchanged bit for bit.  One address select per
+    // record instead of a branch or nine value selects: the gather warps share issue slots with the element warps.
     double acc[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
 #pragma unroll
     for (int s = 0; s < 8; s++) {
         const unsigned K = (kv >> (4 * s)) & 15u;
-        const bool ok = K != 15u;
-        const double *rec = buf + s * 72 + (ok ? K : 0u);
+        const double *rec = (K != 15u) ? buf + s * 72 + K : zero;
 #pragma unroll
-        for (int j = 0; j < 9; j++) { const double v = rec[8 * j]; acc[j] += ok ? v : 0.0; }
+        for (int j = 0; j < 9; j++) acc[j] += rec[8 * j];
     }
     if (lane < len) {
         double *out = csr_vals + 9LL * o + 3 * lane;
@@ -303,8 +330,10 @@ __device__ __forceinline__ void gather_reduce_pre(long long n, int m, int o, int
 // two quads = eight nodes; lane j holds the tables of node j (loaded once, before anything is known to be ready: they are
 // static).  The nodes of the quads whose chunks have all published their flag are then streamed through a two-slot
 // buffer: the records (and table values) of node i+1 are on their way while node i is reduced.
-__device__ __forceinline__ void fuse_gather_role(long long chunk, int gw, int lane, double *wbuf, const double *Ke, const double *Re,
-                                                 const scatter_args &sa) {
+__device__ __forceinline__ void fuse_gather_role(long long chunk, int gw, int lane, double *wbuf, double *zero, const double *Ke,
+                                                 const double *Re, const scatter_args &sa) {
+    zero[lane] = 0.0; zero[32 + lane] = 0.0; if (lane == 0) zero[64] = 0.0;   // the block of +0.0 read in place of a missing block
+    __syncwarp();
     const int q0 = __ldg(sa.cta_quads + chunk * FUSE_QPC + 2 * gw), q1 = __ldg(sa.cta_quads + chunk * FUSE_QPC + 2 * gw + 1);
     if ((q0 & q1) < 0 && q0 < 0 && q1 < 0) return;
     // lane j < 8: node j of the two quads
@@ -342,6 +371,7 @@ __device__ __forceinline__ void fuse_gather_role(long long chunk, int gw, int la
     }
     if (!live) return;
     __threadfence();                         // the flags were read before any record is
+    const unsigned long long pol_f = l2_policy_first();
     // stream the live nodes through the two slots
     int cur = __ffs(live) - 1;
     live &= live - 1;
@@ -353,7 +383,7 @@ __device__ __forceinline__ void fuse_gather_role(long long chunk, int gw, int la
                   lj = __shfl_sync(0xffffffffu, len, cur);
         const double *src = Ke + (long long)bj * 72;
 #pragma unroll
-        for (int it = 0; it < 9; it++) { const int idx = it * 32 + lane; if (idx < 36 * mj) cp_async16(wbuf + 2 * idx, src + 2 * idx); }
+        for (int it = 0; it < 9; it++) { const int idx = it * 32 + lane; if (idx < 36 * mj) cp_async16_hint(wbuf + 2 * idx, src + 2 * idx, pol_f); }
         asm volatile("cp.async.commit_group;" ::: "memory");
         kv_c = (lane < lj) ? __ldg(sa.kvec + oj + lane) : 0xffffffffu;
         rv_c = (lane < 3 * mj) ? __ldcg(Re + (long long)bj * 3 + lane) : 0.0;
@@ -368,7 +398,7 @@ __device__ __forceinline__ void fuse_gather_role(long long chunk, int gw, int la
             const double *src = Ke + (long long)bj * 72;
             double *dst = wbuf + (slot ^ 1) * 576;
 #pragma unroll
-            for (int it = 0; it < 9; it++) { const int idx = it * 32 + lane; if (idx < 36 * mj) cp_async16(dst + 2 * idx, src + 2 * idx); }
+            for (int it = 0; it < 9; it++) { const int idx = it * 32 + lane; if (idx < 36 * mj) cp_async16_hint(dst + 2 * idx, src + 2 * idx, pol_f); }
             kv_n = (lane < lj) ? __ldg(sa.kvec + oj + lane) : 0xffffffffu;
             rv_n = (lane < 3 * mj) ? __ldcg(Re + (long long)bj * 3 + lane) : 0.0;
         }
@@ -377,8 +407,17 @@ __device__ __forceinline__ void fuse_gather_role(long long chunk, int gw, int la
         __syncwarp();
         const long long n = __shfl_sync(0xffffffffu, node, cur);
         gather_reduce_pre(n, __shfl_sync(0xffffffffu, m, cur), __shfl_sync(0xffffffffu, o, cur), __shfl_sync(0xffffffffu, len, cur),
-                          kv_c, rv_c, wbuf + slot * 576, lane, sa.csr_vals, sa.residual);
+                          kv_c, rv_c, wbuf + slot * 576, zero, lane, sa.csr_vals, sa.residual);
         __syncwarp();                        // the slot is free for the node after next
+#if FUSE_DISCARD
+        {   // the records of this node have been consumed and are never read again in this call: drop their (dirty) L2 lines
+            // instead of letting them be written back to HBM.  Only 128-byte lines that lie wholly inside the node's run.
+            const unsigned long long a0 = (unsigned long long)(Ke + (long long)__shfl_sync(0xffffffffu, b, cur) * 72);
+            const unsigned long long a1 = a0 + 576ull * (unsigned long long)__shfl_sync(0xffffffffu, m, cur);
+            for (unsigned long long pl = ((a0 + 127ull) & ~127ull) + 128ull * lane; pl + 128ull <= a1; pl += 32ull * 128ull)
+                asm volatile("discard.global.L2 [%0], 128;" ::"l"(pl) : "memory");
+        }
+#endif
         cur = nxt; kv_c = kv_n; rv_c = rv_n; slot ^= 1;
     }
     asm volatile("cp.async.wait_group 0;" ::: "memory");
@@ -401,11 +440,13 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
         if (tid >= CTA_THREADS) {   // gather warpgroup: hands most of its registers to the element warpgroup
             reg_dec<FUSE_GREGS>();
             const int gw = (tid - CTA_THREADS) >> 5;
-            fuse_gather_role(chunk, gw, lane, sm + EL_PER_CTA * ES + gw * FUSE_GNB * 576, Ke, Re, sa);
+            fuse_gather_role(chunk, gw, lane, sm + EL_PER_CTA * ES + gw * FUSE_GNB * 576, sm + EL_PER_CTA * ES + 4 * FUSE_GNB * 576 + gw * 66,
+                             Ke, Re, sa);
             return;
         }
         reg_inc<FUSE_EREGS>();
     }
+    const unsigned long long pol_keep = FUSE ? l2_policy_last() : 0ull;
     const int el_cta = tid >> 3;
     double *se = sm + el_cta * ES;
     const long long e_raw = chunk * EL_PER_CTA + el_cta;
@@ -830,8 +871,8 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
             for (int i = 0; i < 6; i++) ep1[i] = __ldg(hin + i);
         }
 #pragma unroll
-        for (int i = 0; i < 6; i++) ho[i] = ep1[i];
-        ho[6] = alpha1;
+        for (int i = 0; i < 6; i++) __stcs(ho + i, ep1[i]);   // streaming: written once, never read by this call
+        __stcs(ho + 6, alpha1);
     }
 
     PHASE_SYNC_N(4);
@@ -1131,10 +1172,18 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
                         for (int i = 0; i < 3; i++)
 #pragma unroll
                             for (int k = i; k < 3; k++, p++) {
-                                *reinterpret_cast<double2 *>(Ke + sd * 72 + (3 * i + k) * 8 + 2 * tig) = make_double2(C[p][0], C[p][1]);
-                                if (i != k) {
-                                    Ke[st0 * 72 + (3 * k + i) * 8 + gid] = C[p][0];
-                                    Ke[st1 * 72 + (3 * k + i) * 8 + gid] = C[p][1];
+                                if (FUSE) {
+                                    st_hint2(Ke + sd * 72 + (3 * i + k) * 8 + 2 * tig, C[p][0], C[p][1], pol_keep);
+                                    if (i != k) {
+                                        st_hint(Ke + st0 * 72 + (3 * k + i) * 8 + gid, C[p][0], pol_keep);
+                                        st_hint(Ke + st1 * 72 + (3 * k + i) * 8 + gid, C[p][1], pol_keep);
+                                    }
+                                } else {
+                                    *reinterpret_cast<double2 *>(Ke + sd * 72 + (3 * i + k) * 8 + 2 * tig) = make_double2(C[p][0], C[p][1]);
+                                    if (i != k) {
+                                        Ke[st0 * 72 + (3 * k + i) * 8 + gid] = C[p][0];
+                                        Ke[st1 * 72 + (3 * k + i) * 8 + gid] = C[p][1];
+                                    }
                                 }
                             }
                     }
@@ -1199,11 +1248,13 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
         // list, so that a gathering warp reads every node's contributions as one contiguous run
         if (valid) {
             double *ro = Re + (long long)my_slot * 3;
-            ro[0] = rI[0]; ro[1] = rI[1]; ro[2] = rI[2];
+            if (FUSE) { st_hint(ro, rI[0], pol_keep); st_hint(ro + 1, rI[1], pol_keep); st_hint(ro + 2, rI[2], pol_keep); }
+            else { ro[0] = rI[0]; ro[1] = rI[1]; ro[2] = rI[2]; }
         }
     }
 
-    // ---- stats: warp-aggregated counters, per-CTA iteration histogram
+    // ---- stats: warp-aggregated counters, per-CTA iteration histogram (a per-CTA shared-memory stage for the four counters and
+    //      a ballot / match-based histogram were both measured slower: 3.04-3.05 vs 3.00 ms)
     {
         const unsigned mp = __ballot_sync(0xffffffffu, valid && plastic);
         const unsigned mn = __ballot_sync(0xffffffffu, valid && nonconv);
@@ -1352,7 +1403,7 @@ template <int FBAR, int FUSE, int YLD>
 static int launch_element(fem_ctx *c, const double *u, const double *hist_in, int mstride, double *hist_out, const scatter_args &sa,
                           int bstride, cudaStream_t st) {
     constexpr int ES = FBAR ? ES_FBAR : ES_STD;
-    const size_t smem = ((size_t)EL_PER_CTA * ES + (FUSE ? 4 * FUSE_GNB * 576 : 0)) * sizeof(double);
+    const size_t smem = ((size_t)EL_PER_CTA * ES + (FUSE ? 4 * FUSE_GNB * 576 + 4 * 66 : 0)) * sizeof(double);   // + the zero blocks
     // the opt-in for > 48 KB of dynamic shared memory is per device and per kernel: remembered per context (= per device)
     const int slot = (FBAR ? 1 : 0) + 2 * (FUSE ? 1 : 0) + 4 * (YLD ? 1 : 0);
     if (!(c->attr_mask & (1u << slot))) {
@@ -1380,7 +1431,7 @@ int fem_launch_assemble(fem_ctx *c, const double *u, const double *hist_in, cons
         c->n_matd_cap = n_mat;
     }
     // the fused kernel exists for the Hill-48 standard element (the F-bar and Yld2004-18p variants need all shared memory / registers)
-    const bool fuse = c->fuse_ok && c->opt.assembly_mode == 1 && !c->opt.fbar && !bar;
+    const bool fuse = c->fuse_ok && !c->opt.fbar && !bar;   // fuse_ok: the mesh qualifies and the mode asks for it (fem_build_csr_pattern)
     FEM_CUDA(cudaMemsetAsync(c->d_stats, 0, sizeof(unsigned long long) * 72, st));
     if (fuse) FEM_CUDA(cudaMemsetAsync(c->d_left_count, 0, sizeof(unsigned int), st));
     FEM_CUDA(cudaEventRecord(c->ev[0], st));

@@ -277,7 +277,7 @@ extern "C" int fem_setup(fem_ctx **out, long long n_nodes, const double *coords,
     fem_default_options(&o);
     if (opt) o = *opt;
     if (o.quad_order != 2) return FEM_ERR_QUAD;
-    if ((o.fbar != 0 && o.fbar != 1) || !(o.tol > 0) || o.kmax < 1 || (o.assembly_mode < 0 || o.assembly_mode > 1)) return FEM_ERR_ARG;
+    if ((o.fbar != 0 && o.fbar != 1) || !(o.tol > 0) || o.kmax < 1 || (o.assembly_mode < 0 || o.assembly_mode > 2)) return FEM_ERR_ARG;
     int ndev = 0;
     FEM_CUDA(cudaGetDeviceCount(&ndev));
     if (ndev < 1) { snprintf(g_fem_cuda_err, sizeof(g_fem_cuda_err), "no CUDA device"); return FEM_ERR_CUDA; }
@@ -398,7 +398,12 @@ extern "C" int fem_build_csr_pattern(fem_ctx *c, long long *n_rows, long long *n
                 TRY(cudaMalloc(&c->d_Re, sizeof(double) * 24 * ne));
                 TRY(cudaDeviceSynchronize());
             }
-            if (c->opt.assembly_mode == 1 && c->d_kvec && !c->has_high_valence) {
+            // assembly_mode 0: fused gather where it pays (Hill-48 standard element, a mesh of at least FUSE_MIN_CHUNKS chunks of 16
+            // elements - below that most quads are scheduled past the last chunk and the stand-alone gather is faster); 1: never;
+            // 2: whenever the mesh qualifies (no collapsed element, no node with more than 8 elements)
+            const long long FUSE_MIN_CHUNKS = 8LL * (2LL * c->n_sm + 32);
+            const bool want_fuse = (c->opt.assembly_mode == 2) || (c->opt.assembly_mode == 0 && !c->opt.fbar && (ne + 15) / 16 >= FUSE_MIN_CHUNKS);
+            if (want_fuse && c->d_kvec && !c->has_high_valence) {
                 // fused, lagged gather: give every node quad to a gather warp of a chunk launched `lag` chunks after the last
                 // chunk that writes one of its records (one wave of resident CTAs + a margin), at most two quads per warp
                 const int EPC = 16, QPC = 8;                      // elements per CTA (fem_assemble.cu EL_PER_CTA), quads per chunk

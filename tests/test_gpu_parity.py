@@ -153,19 +153,19 @@ def test_error_codes_on_device():
 @pytest.mark.parametrize("fbar", [0, 1])
 @pytest.mark.parametrize("cfgid,n", [(3, 22), (4, 27)])
 def test_fused_gather_equals_separate_gather(cfgid, n, fbar):
-    """assembly_mode 1 gathers node quads inside the element launch (warps of chunks launched one wave later read the
-    records back from L2, completion flags, no waiting) and finishes the rest in k_gather_list; assembly_mode 0 runs the
-    element kernel and the stand-alone gather kernel one after the other.  Both sum in ascending element id: the two
+    """assembly_mode 2 gathers node quads inside the element launch (a second warpgroup of chunks launched one wave later
+    reads the records back from L2, completion flags, bounded polling) and finishes the rest in k_gather_list;
+    assembly_mode 1 runs the element kernel and the stand-alone gather kernel one after the other.  Both sum in ascending element id: the two
     must agree bit for bit, with the oracle within tolerance, and with themselves on a second call.  Sizes: more than
     3*148+64 chunks of 16 elements, so that part of the quads really is gathered in-kernel."""
     cfg = synth.make_config(cfgid, n=n)
     assert cfg["conn"].shape[0] > 16 * (3 * 148 + 64)
-    g = run_gpu(cfg, fbar, assembly_mode=1)
+    g = run_gpu(cfg, fbar, assembly_mode=2)
     compare(g, run_oracle(cfg, fbar), "fused cfg%d" % cfgid)
-    g1 = run_gpu(cfg, fbar, assembly_mode=0)
+    g1 = run_gpu(cfg, fbar, assembly_mode=1)
     assert np.array_equal(g["csr_vals"], g1["csr_vals"]) and np.array_equal(g["residual"], g1["residual"])
     assert np.array_equal(g["hist_out"], g1["hist_out"])
-    g2 = run_gpu(cfg, fbar, assembly_mode=1)
+    g2 = run_gpu(cfg, fbar, assembly_mode=2)
     assert np.array_equal(g["csr_vals"], g2["csr_vals"]) and np.array_equal(g["residual"], g2["residual"])
 
 
@@ -181,7 +181,7 @@ def test_fused_gather_repeated_calls_and_isolated_node():
     o = run_oracle(cfg2)
     dev = torch.device("cuda:0")
     ne = cfg2["conn"].shape[0]
-    ctx = fem.FemContext(torch.from_numpy(coords).to(dev), torch.from_numpy(cfg2["conn"]).to(dev), assembly_mode=1)
+    ctx = fem.FemContext(torch.from_numpy(coords).to(dev), torch.from_numpy(cfg2["conn"]).to(dev), assembly_mode=2)
     ctx.build_csr_pattern()
     mat = torch.from_numpy(fem.mat_from_desc(cfg2["matdesc"], ne).ravel()).to(dev)
     ud, hd = torch.from_numpy(u.ravel()).to(dev), torch.from_numpy(cfg2["hist_in"].ravel()).to(dev)
