@@ -335,6 +335,7 @@ __device__ __noinline__ void bar_return_map(const double *__restrict__ bd, doubl
     for (int i = 0; i < 6; i++) { T[i] = Ttr[i]; dep[i] = 0.0; tn2 = fma(Ttr[i] - ((i < 3) ? pres : 0.0), Ttr[i] - ((i < 3) ? pres : 0.0), tn2); }
     iters = 0; nonconv = false; dg_out = 0.0;
     plastic = false;
+    __syncthreads();   // the trial evaluation too is walked by the four warps together
     if (tn2 > 0.0) {
         bar_eval(bd, Ttr, true, phi, N, H);
         plastic = (phi - s0) > 0.0;                     // Eq.(17)-(18) :165-172, tie -> elastic
@@ -343,11 +344,14 @@ __device__ __noinline__ void bar_return_map(const double *__restrict__ bd, doubl
     for (int A = 0; A < 6; A++)
 #pragma unroll
         for (int B = A; B < 6; B++) Cep[A][B] = ((A < 3 && B < 3) ? kb - mu2 * (1.0 / 3.0) : 0.0) + ((A == B) ? mu2 : 0.0);
-    if (!plastic) return;
+    // From here on the warps of the CTA walk the (large, unrolled) evaluation code together: every Newton iteration starts at
+    // a CTA-wide barrier and the loop runs until no thread of the CTA is active (elastic points and converged points idle).
+    // ncu showed instruction fetch as the top stall (2.5 per issue) with every warp at its own place in ~60 KB of SASS.
     const double is0 = frcp(s0);
     const double tolG = 1e-13 * fmax(1.0, sqrt(tn2) * is0);
     double dg = 0.0, sy = s0, dsy = ds0, prev = INFINITY;
 #if BAR_START
+    if (plastic)
     // Starting point (the root is unique, so any start reaches the state Alg. C2 reaches from T^tr): the trial deviator scaled
     // back onto the yield surface, T0 = p 1 + c s^tr, with dgam from the N-component of Eq.(19): phi^tr - 2mu dgam N.N -
     // sigma_y(alpha_n + dgam) = 0 (exact radial return for von Mises).  phi is homogeneous of degree one, so phi, N and H at
@@ -386,13 +390,17 @@ __device__ __noinline__ void bar_return_map(const double *__restrict__ bd, doubl
         psio = 0.5 * fma(fo, fo, psio);                                                                \
     } while (0)
     BAR_RESID(T, dg, N, phi, sy, GT, fv, psi0);
-    bool conv = false;
+    bool conv = false, active = plastic;
     for (int k = 0;; k++) {
-        const double nrm = sqrt(2.0 * psi0);
-        iters = k;
-        if (nrm <= tolG || (prev <= 1e-9 && nrm >= 0.5 * prev)) { conv = true; break; }
-        if (k >= kmax) break;
-        prev = nrm;
+        if (active) {
+            const double nrm = sqrt(2.0 * psi0);
+            iters = k;
+            if (nrm <= tolG || (prev <= 1e-9 && nrm >= 0.5 * prev)) { conv = true; active = false; }
+            else if (k >= kmax) active = false;
+            else prev = nrm;
+        }
+        if (!__syncthreads_or(active)) break;
+        if (!active) continue;
         // Newton direction of Eq.(24) :196 on (T, dgam): M dT + 2mu N ddg = -G_T s0 ; N.dT - sigma' ddg = -f s0
         double M[6][6], x1[6], x2[6], r1[6];
 #pragma unroll
@@ -439,6 +447,7 @@ __device__ __noinline__ void bar_return_map(const double *__restrict__ bd, doubl
         BAR_RESID(T, dg, N, phi, sy, GT, fv, psi0);
     }
 #undef BAR_RESID
+    if (!plastic) return;
     nonconv = !conv;
     dg_out = dg;
     // Alg. C2 step 27 :979: eps_p += dgam N, T = E:(eps - eps_p)
