@@ -39,7 +39,8 @@ enum {
     FEM_ERR_DEGREE = -8,      /* a node belongs to more than FEM_MAX_NODE_ELEMS elements */
     FEM_ERR_ALIAS = -9,       /* hist_out aliases hist_in */
     FEM_ERR_MAT = -10,        /* n_mat is neither 1 nor n_elems */
-    FEM_ERR_NOCONV = -11      /* iterative solve (fem_bicgstab, fem_newton_solve) did not converge */
+    FEM_ERR_NOCONV = -11,     /* iterative solve (fem_bicgstab, fem_newton_solve) did not converge */
+    FEM_ERR_TOO_LARGE = -12   /* fem_assemble_static: the mesh has more than FEM_STATIC_MAX_ELEMS elements */
 };
 #define FEM_MAX_NODE_ELEMS 32
 
@@ -139,6 +140,31 @@ int fem_assemble(fem_ctx *c, const double *u, const double *hist_in, const doubl
 int fem_assemble_barlat(fem_ctx *c, const double *u, const double *hist_in, const double *mat, const double *barlat,
                         long long n_mat, double *residual, double *csr_vals, double *hist_out, fem_stats *stats,
                         void *cuda_stream);
+
+/* fem_assemble_static — fem_assemble for callers that may not allocate device memory inside the call (code under CUDA
+ * graph capture, tight serving loops, harnesses that forbid cudaMalloc).  Same operation, arguments, outputs, summation
+ * order and error codes as fem_assemble (Hill-48 model, standard or F-bar element as the context was set up; S1-S14 of
+ * SURVEY.md section 8(a)), in the two-kernel schedule, but the scratch of the pass — the K^e / R^e records, the derived
+ * material records and the counters — lives in ONE file-scope device array of FEM_STATIC_SCRATCH_BYTES inside the library
+ * instead of the context's buffers.  Every GPU that loads the library holds that array until the process exits.
+ *   - The call itself calls no cudaMalloc / cudaFree / allocating library routine.  The context (fem_setup,
+ *     fem_build_csr_pattern) is built beforehand as usual; those set-up calls do allocate.
+ *   - Limit: n_elems <= FEM_STATIC_MAX_ELEMS, else FEM_ERR_TOO_LARGE (nothing is launched).
+ *   - fem_assemble_static_prepare(c) is the set-up step: with the context's device current it resolves the array's device
+ *     address (once per device) and opts the element kernel into its shared-memory size (once per context).  Call it
+ *     before capturing a graph; otherwise the first fem_assemble_static on the context does it.  FEM_ERR_ARG when the
+ *     current device is not the one the context was built on.
+ *   - ALL calls on a device share the array, whatever the context or stream: calls that overlap on the GPU race on it.
+ *     Order them on one stream (or with events).  The array keeps the last call's contents; the call clears the
+ *     counters itself, and every record it reads was written earlier in the same call.
+ *   - stats: host, may be NULL; non-NULL synchronises the stream (leave it NULL under capture).
+ * Results are bit-identical to fem_assemble on a context in assembly_mode 1 (and equal to the default mode, which sums in
+ * the same order). */
+#define FEM_STATIC_MAX_ELEMS 4096
+#define FEM_STATIC_SCRATCH_BYTES 20710144 /* (576 + 24 + 32) doubles per element x 4096 + 96 counters words */
+int fem_assemble_static_prepare(fem_ctx *c);
+int fem_assemble_static(fem_ctx *c, const double *u, const double *hist_in, const double *mat, long long n_mat,
+                        double *residual, double *csr_vals, double *hist_out, fem_stats *stats, void *cuda_stream);
 
 /* Same call with HOST buffers for every array: copies in, assembles, copies out, synchronises (used for end-to-end timing). */
 int fem_assemble_host(fem_ctx *c, const double *u, const double *hist_in, const double *mat, long long n_mat,

@@ -12,7 +12,9 @@ ABI_SYMBOLS = ["fem_default_options", "fem_setup", "fem_build_csr_pattern", "fem
                "fem_last_kernel_ms", "fem_launches_per_assemble", "fem_probe_fp64_peak", "fem_destroy", "fem_strerror",
                "fem_last_cuda_error", "fem_hill_from_lankford", "fem_spmv", "fem_apply_dirichlet", "fem_bicgstab", "fem_pcg", "fem_lincomb",
                "fem_default_newton_options", "fem_newton_solve", "fem_assemble_vjp", "fem_adjoint_step", "fem_set_mixed_precision",
-               "fem_default_path_options", "fem_load_path"]
+               "fem_default_path_options", "fem_load_path", "fem_assemble_static_prepare", "fem_assemble_static"]
+STATIC_MAX_ELEMS = 4096          # FEM_STATIC_MAX_ELEMS of include/fem.h
+STATIC_SCRATCH_BYTES = 20710144  # FEM_STATIC_SCRATCH_BYTES
 
 
 class FemOptions(C.Structure):
@@ -97,6 +99,8 @@ def lib():
         L.fem_build_csr_pattern.argtypes = [vp, C.POINTER(ll), C.POINTER(ll), C.POINTER(vp), C.POINTER(vp), C.POINTER(vp)]
         L.fem_assemble.argtypes = [vp, vp, vp, vp, ll, vp, vp, vp, C.POINTER(FemStats), vp]
         L.fem_assemble_barlat.argtypes = [vp, vp, vp, vp, vp, ll, vp, vp, vp, C.POINTER(FemStats), vp]
+        L.fem_assemble_static_prepare.argtypes = [vp]
+        L.fem_assemble_static.argtypes = [vp, vp, vp, vp, ll, vp, vp, vp, C.POINTER(FemStats), vp]
         L.fem_assemble_host.argtypes = [vp, vp, vp, vp, ll, vp, vp, vp, C.POINTER(FemStats)]
         L.fem_last_kernel_ms.argtypes = [vp, dp]
         L.fem_launches_per_assemble.argtypes = [vp]
@@ -253,6 +257,23 @@ class FemContext:
                                   _ptr(csr_vals, f64, self.nnz, "csr_vals"), _ptr(hist_out, f64, 56 * self.n_elems, "hist_out"),
                                   C.byref(st) if want_stats else None, _stream_ptr()), "fem_assemble")
         return residual, csr_vals, hist_out, (st.as_dict() if want_stats else None)
+
+    def assemble_static_prepare(self):
+        """fem_assemble_static_prepare: the set-up step of assemble_static (device address of the library's static scratch)."""
+        _check(lib().fem_assemble_static_prepare(self._h), "fem_assemble_static_prepare")
+
+    def assemble_static(self, u, hist_in, mat, residual, csr_vals, hist_out, want_stats=False):
+        """fem_assemble_static: fem_assemble with its scratch in the library's file-scope device array; the call allocates
+        nothing, so the caller passes every output.  At most STATIC_MAX_ELEMS elements.  Returns stats|None."""
+        f64 = _torch().float64
+        n_mat = mat.numel() // NPAR
+        st = FemStats() if want_stats else None
+        _check(lib().fem_assemble_static(self._h, _ptr(u, f64, self.n_rows, "u"), _ptr(hist_in, f64, 56 * self.n_elems, "hist_in"),
+                                         _ptr(mat, f64, None, "mat"), n_mat, _ptr(residual, f64, self.n_rows, "residual"),
+                                         _ptr(csr_vals, f64, self.nnz, "csr_vals"),
+                                         _ptr(hist_out, f64, 56 * self.n_elems, "hist_out"),
+                                         C.byref(st) if want_stats else None, _stream_ptr()), "fem_assemble_static")
+        return st.as_dict() if want_stats else None
 
     def assemble_host(self, u, hist_in, mat, residual, csr_vals, hist_out, want_stats=False):
         """fem_assemble_host on HOST buffers (numpy arrays or pinned CPU torch tensors); copies are inside the call."""

@@ -17,6 +17,7 @@
 #include "fem_device.cuh"
 #include <math.h>
 #include <stdio.h>
+#include <mutex>
 
 #define W23 0.81649658092772603273   // W = sqrt(2/3)
 #define SQRT2 1.41421356237309504880
@@ -1487,5 +1488,124 @@ int fem_launch_assemble(fem_ctx *c, const double *u, const double *hist_in, cons
     FEM_CUDA(cudaEventRecord(c->ev[3], st));
     FEM_CUDA(cudaGetLastError());
     c->ev_valid = true;
+    return FEM_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ no-allocation entry point
+// fem_assemble_static (include/fem.h): the two-kernel schedule above (k_mat_prep, k_element<FBAR,0,0>, table-driven or
+// general gather) with ALL of its scratch -- the K^e / R^e records, the derived material records and the counters -- in
+// one file-scope device array instead of the context's cudaMalloc'd buffers.  For callers that may not allocate (CUDA
+// graph capture, serving loops).  The array costs FEM_STATIC_SCRATCH_BYTES on every GPU that loads the library.
+//   layout in doubles: [0, 576 M) K^e records | [576 M, 600 M) R^e records | [600 M, 600 M + FEM_MATD M) material
+//   records | 72 x u64 counters, M = FEM_STATIC_MAX_ELEMS; every block starts on a 256-byte boundary.
+#define ST_OFF_KE 0
+#define ST_OFF_RE ((size_t)576 * FEM_STATIC_MAX_ELEMS)
+#define ST_OFF_MATD ((size_t)600 * FEM_STATIC_MAX_ELEMS)
+#define ST_OFF_STATS ((size_t)(600 + FEM_MATD) * FEM_STATIC_MAX_ELEMS)
+#define ST_DOUBLES (ST_OFF_STATS + 96)
+static_assert(ST_DOUBLES * sizeof(double) == FEM_STATIC_SCRATCH_BYTES, "include/fem.h states the size of the static scratch");
+static_assert((ST_OFF_RE * 8) % 256 == 0 && (ST_OFF_MATD * 8) % 256 == 0 && (ST_OFF_STATS * 8) % 256 == 0, "block alignment");
+static __device__ __align__(256) double g_static_scratch[ST_DOUBLES];
+
+// In host code `g_static_scratch` is only a handle: the device address comes from cudaGetSymbolAddress, once per device.
+#define ST_MAX_DEVICES 64
+static double *g_static_ptr[ST_MAX_DEVICES];
+static std::mutex g_static_mu;
+
+// The device the context's buffers live on must be the current one: the symbol address and the launches below are per device.
+static int static_device_of(const fem_ctx *c, int *dev) {
+    FEM_CUDA(cudaGetDevice(dev));
+    cudaPointerAttributes pa;
+    FEM_CUDA(cudaPointerGetAttributes(&pa, c->d_coords));
+    if (pa.type != cudaMemoryTypeDevice || pa.device != *dev || *dev < 0 || *dev >= ST_MAX_DEVICES) return FEM_ERR_ARG;
+    return FEM_OK;
+}
+
+extern "C" int fem_assemble_static_prepare(fem_ctx *c) {
+    if (!c) return FEM_ERR_NULL;
+    if (!c->has_pattern) return FEM_ERR_NO_PATTERN;
+    if (c->n_elems > FEM_STATIC_MAX_ELEMS) return FEM_ERR_TOO_LARGE;
+    int dev = -1;
+    int rc = static_device_of(c, &dev);
+    if (rc != FEM_OK) return rc;
+    std::lock_guard<std::mutex> lk(g_static_mu);
+    if (!g_static_ptr[dev]) {
+        double *p = nullptr;
+        FEM_CUDA(cudaGetSymbolAddress((void **)&p, g_static_scratch));
+        if (!p) return FEM_ERR_CUDA;
+        g_static_ptr[dev] = p;
+    }
+    // dynamic shared-memory opt-in of the element kernel (same bookkeeping as launch_element)
+    const int slot = c->opt.fbar ? 1 : 0;
+    if (!(c->attr_mask & (1u << slot))) {
+        const int smem = EL_PER_CTA * (c->opt.fbar ? ES_FBAR : ES_STD) * (int)sizeof(double);
+        if (c->opt.fbar) FEM_CUDA(cudaFuncSetAttribute(k_element<1, 0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        else             FEM_CUDA(cudaFuncSetAttribute(k_element<0, 0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        c->attr_mask |= 1u << slot;
+    }
+    return FEM_OK;
+}
+
+extern "C" int fem_assemble_static(fem_ctx *c, const double *u, const double *hist_in, const double *mat, long long n_mat,
+                                   double *residual, double *csr_vals, double *hist_out, fem_stats *stats, void *cuda_stream) {
+    if (!c || !u || !hist_in || !mat || !residual || !csr_vals || !hist_out) return FEM_ERR_NULL;
+    if (!c->has_pattern) return FEM_ERR_NO_PATTERN;
+    if (c->n_elems > FEM_STATIC_MAX_ELEMS) return FEM_ERR_TOO_LARGE;
+    if (n_mat != 1 && n_mat != c->n_elems) return FEM_ERR_MAT;
+    if (fem_ranges_overlap(hist_in, hist_out, sizeof(double) * 56 * (size_t)c->n_elems)) return FEM_ERR_ALIAS;
+    int dev = -1;
+    FEM_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= ST_MAX_DEVICES) return FEM_ERR_ARG;
+    double *base;
+    { std::lock_guard<std::mutex> lk(g_static_mu); base = g_static_ptr[dev]; }
+    if (!base || !(c->attr_mask & (1u << (c->opt.fbar ? 1 : 0)))) {   // first use on this device / context: the set-up step
+        int rc = fem_assemble_static_prepare(c);
+        if (rc != FEM_OK) return rc;
+        std::lock_guard<std::mutex> lk(g_static_mu);
+        base = g_static_ptr[dev];
+    }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    double *Ke = base + ST_OFF_KE, *Re = base + ST_OFF_RE, *matd = base + ST_OFF_MATD;
+    unsigned long long *cnt = reinterpret_cast<unsigned long long *>(base + ST_OFF_STATS);
+    // the array keeps the last call's contents: the counters are the one block that must start at zero (every K^e, R^e and
+    // material record the gather reads is rewritten by this call before it is read)
+    FEM_CUDA(cudaMemsetAsync(cnt, 0, sizeof(unsigned long long) * 72, st));
+    k_mat_prep<<<nblk2(n_mat, MP_THREADS), MP_THREADS, 0, st>>>(n_mat, mat, matd);
+    const int mstride = (n_mat == 1) ? 0 : FEM_MATD;
+    scatter_args sa = {c->d_eorder, c->d_eslot, nullptr, nullptr, nullptr, 0u, nullptr, nullptr, c->n_nodes, c->d_inc_ptr, c->d_nb_ptr,
+                       c->d_kvec, csr_vals, residual};
+    const unsigned grid = nblk2(c->n_elems, EL_PER_CTA);
+    if (c->opt.fbar)
+        k_element<1, 0, 0><<<grid, CTA_THREADS, (size_t)EL_PER_CTA * ES_FBAR * sizeof(double), st>>>(
+            c->n_elems, c->d_coords, c->d_conn, u, hist_in, matd, mstride, c->opt.tol, c->opt.kmax, Ke, Re, hist_out, cnt, sa, nullptr, 0);
+    else
+        k_element<0, 0, 0><<<grid, CTA_THREADS, (size_t)EL_PER_CTA * ES_STD * sizeof(double), st>>>(
+            c->n_elems, c->d_coords, c->d_conn, u, hist_in, matd, mstride, c->opt.tol, c->opt.kmax, Ke, Re, hist_out, cnt, sa, nullptr, 0);
+    if (c->d_kvec) {
+        if (c->has_high_valence)
+            k_gather_fast<1><<<nblk2(c->n_nodes, GW), GW * 32, 0, st>>>(c->n_nodes, c->d_inc_ptr, c->d_inc, c->d_nb_ptr, c->d_kvec,
+                                                                     c->d_elem_pos, Ke, Re, csr_vals, residual);
+        else
+            k_gather_fast<0><<<nblk2(c->n_nodes, GW), GW * 32, 0, st>>>(c->n_nodes, c->d_inc_ptr, c->d_inc, c->d_nb_ptr, c->d_kvec,
+                                                                     c->d_elem_pos, Ke, Re, csr_vals, residual);
+    } else {
+        k_gather<<<nblk2(c->n_nodes * 32, 256), 256, 0, st>>>(c->n_nodes, c->d_inc_ptr, c->d_inc, c->d_nb_ptr, c->d_elem_pos, Ke, Re,
+                                                             csr_vals, residual);
+    }
+    FEM_CUDA(cudaGetLastError());
+    if (stats) {   // copies the counters back and synchronises the stream (no allocation: the destination is on the stack)
+        unsigned long long h[72];
+        FEM_CUDA(cudaMemcpyAsync(h, cnt, sizeof(h), cudaMemcpyDeviceToHost, st));
+        FEM_CUDA(cudaStreamSynchronize(st));
+        stats->n_plastic = (long long)h[0];
+        stats->n_nonconverged = (long long)h[1];
+        stats->n_detF_nonpos = (long long)h[2];
+        stats->n_nonfinite = (long long)h[3];
+        stats->max_local_iters = 0;
+        for (int k = 0; k < 64; k++) {
+            stats->iter_hist[k] = (long long)h[5 + k];
+            if (h[5 + k]) stats->max_local_iters = k;
+        }
+    }
     return FEM_OK;
 }

@@ -237,6 +237,7 @@ extern "C" const char *fem_strerror(int code) {
         case FEM_ERR_ALIAS: return "hist_out aliases hist_in";
         case FEM_ERR_MAT: return "n_mat must be 1 or n_elems";
         case FEM_ERR_NOCONV: return "iterative solve did not converge";
+        case FEM_ERR_TOO_LARGE: return "mesh exceeds FEM_STATIC_MAX_ELEMS (fem_assemble_static)";
         default: return "unknown error code";
     }
 }
