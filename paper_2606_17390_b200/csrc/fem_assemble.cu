@@ -135,6 +135,9 @@ __host__ __device__ constexpr int sidx9(int r, int c) {  // packed upper triangl
 #endif
 #define CTAS_STD (THREADS_PER_SM / CTA_THREADS)   // 12 warps per SM: limited by 168 registers and ~4.5 KB shared memory per element
 #define CTAS_FBAR (256 / CTA_THREADS)
+#ifndef CTAS_YLD
+#define CTAS_YLD CTAS_FBAR
+#endif
 
 __device__ __forceinline__ void flow_stress(double law, double h0, double h1, double h2, double alpha, double &sf,
                                             double &dsf) {
@@ -149,6 +152,9 @@ __device__ __forceinline__ void flow_stress(double law, double h0, double h1, do
     }
 }
 
+#ifndef BAR_PARK
+#define BAR_PARK 1
+#endif
 #include "fem_barlat.cuh"
 
 // ------------------------------------------------------------------------------------------------ node gather (S14), shared
@@ -436,7 +442,7 @@ __device__ __forceinline__ void fuse_gather_role(long long chunk, int gw, int la
 }
 
 template <int FBAR, int FUSE, int YLD = 0>
-__global__ void __launch_bounds__(FUSE ? 2 * CTA_THREADS : CTA_THREADS, FUSE ? 2 : ((FBAR || YLD) ? CTAS_FBAR : CTAS_STD))
+__global__ void __launch_bounds__(FUSE ? 2 * CTA_THREADS : CTA_THREADS, FUSE ? 2 : (YLD ? CTAS_YLD : (FBAR ? CTAS_FBAR : CTAS_STD)))
 k_element(long long n_elems, const double *__restrict__ coords, const int *__restrict__ conn,
           const double *__restrict__ u, const double *__restrict__ hist_in, const double *__restrict__ matd,
           int mat_stride, double tol, int kmax, double *__restrict__ Ke, double *__restrict__ Re,
@@ -595,7 +601,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
         jacobi_rot(c00, c22, c02, c01, c12, R[0][0], R[0][2], R[1][0], R[1][2], R[2][0], R[2][2]);
         jacobi_rot(c11, c22, c12, c01, c02, R[0][1], R[0][2], R[1][1], R[1][2], R[2][1], R[2][2]);
     }
-    const double lam[3] = {c00, c11, c22};
+    double lam[3] = {c00, c11, c22};
 
     PHASE_SYNC_N(1);
     // ---- rotate F and G into the eigenbasis (Lagrangian principal axes): F^_ia = F_iJ R_Ja, G^_Ia = G_IJ R_Ja
@@ -682,8 +688,27 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
         //      taken to the eigenbasis of C with the 6x6 matrix Q[A][I]: X^_A (tensor components) = sum_I Q[A][I] X_I (Mandel)
         const double law = __ldg(md + 3), hh0 = __ldg(md + 4), hh1 = __ldg(md + 5), hh2 = __ldg(md + 6);
         double Tm[6], dep[6], Cm[6][6], dg;
+#if BAR_PARK
+        // What the rest of the kernel needs after the return map waits in the (still unused) A^ region of shared memory:
+        // the return map and the yield-function evaluation inside it want every register they can get.
+#define PARK_ALL(OP)                                                                                          \
+        _Pragma("unroll") for (int i_ = 0; i_ < 9; i_++) { OP(i_, Fh[i_ / 3][i_ % 3]); OP(9 + i_, Rm[i_ / 3][i_ % 3]); \
+                                                           OP(30 + i_, Th[i_ / 3][i_ % 3]); }                  \
+        _Pragma("unroll") for (int i_ = 0; i_ < 6; i_++) OP(18 + i_, epm[i_]);                                 \
+        _Pragma("unroll") for (int i_ = 0; i_ < 3; i_++) { OP(24 + i_, lam[i_]); OP(27 + i_, lg[i_]); }        \
+        OP(39, wq); OP(40, wgt); OP(41, detF);
+#define PARK_ST(i, v) se[SM_AA + 8 * (i) + q] = (v)
+#define PARK_LD(i, v) (v) = se[SM_AA + 8 * (i) + q]
+        PARK_ALL(PARK_ST)
+#endif
         bar_return_map(bard + (long long)bar_stride * e, mu2, kb, law, hh0, hh1, hh2, ee, alphan, kmax, Tm, dep, Cm, dg, iters,
                        plastic, nonconv);
+#if BAR_PARK
+        PARK_ALL(PARK_LD)
+#undef PARK_ALL
+#undef PARK_ST
+#undef PARK_LD
+#endif
         if (valid) {
             double *ho = hist_out + (e * 8 + q) * 7;
             double ep1[6];

@@ -16,6 +16,9 @@
 
 #define FEM_BARD 32   // derived Barlat record: [0..8] N' = C'n.Pn (row-major), [9..11] c'44,c'55,c'66, [12..23] the same for C'', [24] m
 #define BAR_MMAX 16
+#ifndef BAR_TOLG
+#define BAR_TOLG 1e-13
+#endif
 #ifndef BAR_START
 #define BAR_START 1
 #endif
@@ -72,6 +75,8 @@ __device__ __forceinline__ void bar_apply_t(const double *__restrict__ L, const 
 #pragma unroll
     for (int i = 0; i < 3; i++) y[3 + i] += L[9 + i] * g[3 + i] * SQRT2;
 }
+// c[n][p] of the Cayley-Hamilton table below is structurally zero for n < 3, p != n (X^n = unit vector n of {I, X, X^2})
+__device__ __forceinline__ constexpr bool bar_cnz(int n, int p) { return n >= 3 || n == p; }
 // X^2 of a symmetric 3x3 in tensor components, and the Cayley-Hamilton data: c[n] = (alpha,beta,gamma) of X^n, t[n] = tr X^n
 template <int M>
 __device__ __forceinline__ void bar_powers(const double a[6], int m, double a2[6], double (*c)[3], double *t) {
@@ -106,6 +111,23 @@ __device__ __forceinline__ void bar_box_acc(const double X[6], const double Y[6]
             H[A][B] = fma(w, v, H[A][B]);
         }
 }
+// the same with X = I: 1/4 (d_ik Y_jl + d_il Y_jk + Y_ik d_jl + Y_il d_jk), the Kronecker deltas resolved at compile time
+__device__ __forceinline__ void bar_box_id_acc(const double Y[6], double H[6][6]) {
+#pragma unroll
+    for (int A = 0; A < 6; A++)
+#pragma unroll
+        for (int B = A; B < 6; B++) {
+            const int i = BI[A], j = BJ[A], k = BI[B], l = BJ[B];
+            double v = 0.0;
+            bool any = false;
+            if (i == k) { v = Y[BV[j][l]]; any = true; }
+            if (i == l) { v = any ? v + Y[BV[j][k]] : Y[BV[j][k]]; any = true; }
+            if (j == l) { v = any ? v + Y[BV[i][k]] : Y[BV[i][k]]; any = true; }
+            if (j == k) { v = any ? v + Y[BV[i][l]] : Y[BV[i][l]]; any = true; }
+            const double w = ((A < 3) ? 1.0 : SQRT2) * ((B < 3) ? 1.0 : SQRT2) * 0.25;
+            if (any) H[A][B] = fma(w, v, H[A][B]);
+        }
+}
 // Out (upper triangle) += L^T H L for the block map L = (Nn 3x3, ds 3); H upper triangle (Mandel)
 __device__ __forceinline__ void bar_congr_acc(const double *__restrict__ L, const double H[6][6], double Out[6][6]) {
     double T1[6][6];   // H L
@@ -138,9 +160,9 @@ __device__ __forceinline__ void bar_congr_acc(const double *__restrict__ L, cons
 // M > 0: exponent known at compile time (every loop unrolls, the Cayley-Hamilton tables live in registers and the
 // binomial weights are immediates); M = 0: any even exponent up to BAR_MMAX with rolled loops and tables in local memory.
 template <int M>
-__device__ __noinline__ void bar_eval_t(const double *__restrict__ bd, const double T[6], bool want_H, double &phi_out, double N[6],
-                                        double H[6][6]) {
-    const int m = M ? M : (int)bd[24];
+__device__ __forceinline__ void bar_eval_t(const double *__restrict__ bd, int m_rt, const double T[6], bool want_H, double &phi_out,
+                                           double N[6], double H[6][6]) {
+    const int m = M ? M : m_rt;
     const double *LA = bd, *LB = bd + 12;
     double a[6], b[6], a2[6], b2[6];
     double cA[BAR_MMAX + 1][3], cB[BAR_MMAX + 1][3], tA[BAR_MMAX + 1], tB[BAR_MMAX + 1];
@@ -154,10 +176,10 @@ __device__ __noinline__ void bar_eval_t(const double *__restrict__ bd, const dou
             Phi = fma(sb * tA[m - k], tB[k], Phi);
             if (k < m) { const double w = sb * (m - k) * tB[k];
 #pragma unroll
-                for (int p = 0; p < 3; p++) gA[p] = fma(w, cA[m - k - 1][p], gA[p]); }
+                for (int p = 0; p < 3; p++) if (bar_cnz(m - k - 1, p)) gA[p] = fma(w, cA[m - k - 1][p], gA[p]); }
             if (k > 0) { const double w = sb * k * tA[m - k];
 #pragma unroll
-                for (int p = 0; p < 3; p++) gB[p] = fma(w, cB[k - 1][p], gB[p]); }
+                for (int p = 0; p < 3; p++) if (bar_cnz(k - 1, p)) gB[p] = fma(w, cB[k - 1][p], gB[p]); }
             sb = -sb * (double)(m - k) / (double)(k + 1);
         }
     }
@@ -186,37 +208,50 @@ __device__ __noinline__ void bar_eval_t(const double *__restrict__ bd, const dou
 #pragma unroll
         for (int q = 0; q < 3; q++) { WA[p][q] = 0.0; WB[p][q] = 0.0; V[p][q] = 0.0; }
     {
-        double sb = 1.0;
+        // d/dA of A^n is sum_{r=0}^{n-1} A^r (.) A^(n-1-r): with A^r = c[r][0] I + c[r][1] A + c[r][2] A^2 the coefficient
+        // matrix of order j = n-1 is the convolution S_j[p][q] = sum_{r=0}^{j} c[r][p] c[j-r][q] (symmetric in p,q), formed
+        // once per j for either side and weighted by the binomial term it belongs to
+        double sbk[BAR_MMAX + 1];   // (-1)^k binom(m,k)
+        {
+            double sb = 1.0;
 #pragma unroll
-        for (int k = 0; k <= m; k++) {
-            if (k <= m - 2) {   // d/dA of (m-k) tB[k] A^n, n = m-k-1 >= 1: sum_{r=0}^{n-1} A^r (.) A^(n-1-r)
-                const double w = sb * (m - k) * tB[k];
-                const int j = m - k - 2;
+            for (int k = 0; k <= m; k++) { sbk[k] = sb; sb = -sb * (double)(m - k) / (double)(k + 1); }
+        }
 #pragma unroll
-                for (int r = 0; r <= j; r++)
+        for (int j = 0; j <= m - 2; j++) {
+            double SA[3][3], SB[3][3];
 #pragma unroll
-                    for (int p = 0; p < 3; p++)
+            for (int p = 0; p < 3; p++)
 #pragma unroll
-                        for (int q = p; q < 3; q++) WA[p][q] = fma(w * cA[r][p], cA[j - r][q], WA[p][q]);
-            }
-            if (k >= 2) {
-                const double w = sb * k * tA[m - k];
-                const int j = k - 2;
+                for (int q = p; q < 3; q++) { SA[p][q] = 0.0; SB[p][q] = 0.0; }
 #pragma unroll
-                for (int r = 0; r <= j; r++)
-#pragma unroll
-                    for (int p = 0; p < 3; p++)
-#pragma unroll
-                        for (int q = p; q < 3; q++) WB[p][q] = fma(w * cB[r][p], cB[j - r][q], WB[p][q]);
-            }
-            if (k >= 1 && k <= m - 1) {
-                const double w = sb * (m - k) * k;
+            for (int r = 0; r <= j; r++)
 #pragma unroll
                 for (int p = 0; p < 3; p++)
 #pragma unroll
-                    for (int q = 0; q < 3; q++) V[p][q] = fma(w * cA[m - k - 1][p], cB[k - 1][q], V[p][q]);
-            }
-            sb = -sb * (double)(m - k) / (double)(k + 1);
+                    for (int q = p; q < 3; q++) {
+                        if (!bar_cnz(r, p) || !bar_cnz(j - r, q)) continue;   // c[n] = unit vector n for n < 3
+                        SA[p][q] = fma(cA[r][p], cA[j - r][q], SA[p][q]);
+                        SB[p][q] = fma(cB[r][p], cB[j - r][q], SB[p][q]);
+                    }
+            const int kA = m - 2 - j, kB = j + 2;
+            const double wA = sbk[kA] * (m - kA) * tB[kA];   // term k = kA of Phi: (m-k) tB[k] d(A^(m-k-1))
+            const double wB = sbk[kB] * kB * tA[m - kB];     // term k = kB:        k tA[m-k] d(B^(k-1))
+#pragma unroll
+            for (int p = 0; p < 3; p++)
+#pragma unroll
+                for (int q = p; q < 3; q++) { WA[p][q] = fma(wA, SA[p][q], WA[p][q]); WB[p][q] = fma(wB, SB[p][q], WB[p][q]); }
+        }
+#pragma unroll
+        for (int k = 1; k <= m - 1; k++) {
+            const double w = sbk[k] * (m - k) * k;
+#pragma unroll
+            for (int p = 0; p < 3; p++)
+#pragma unroll
+                for (int q = 0; q < 3; q++) {
+                    if (!bar_cnz(m - k - 1, p) || !bar_cnz(k - 1, q)) continue;
+                    V[p][q] = fma(w * cA[m - k - 1][p], cB[k - 1][q], V[p][q]);
+                }
         }
     }
     WA[1][0] = WA[0][1]; WA[2][0] = WA[0][2]; WA[2][1] = WA[1][2];   // sum_r c[r][p] c[j-r][q] is symmetric in (p,q)
@@ -238,13 +273,13 @@ __device__ __noinline__ void bar_eval_t(const double *__restrict__ bd, const dou
 #pragma unroll
                 for (int B = 0; B < 6; B++) HX[A][B] = 0.0;
 #pragma unroll
-            for (int i = 0; i < 6; i++) Y[i] = fma(W[0][2], x2[i], fma(W[0][1], x[i], W[0][0] * id6[i]));
-            bar_box_acc(id6, Y, HX);
+            for (int i = 0; i < 6; i++) Y[i] = fma(W[0][2], x2[i], (i < 3) ? fma(W[0][1], x[i], W[0][0]) : W[0][1] * x[i]);
+            bar_box_id_acc(Y, HX);
 #pragma unroll
-            for (int i = 0; i < 6; i++) Y[i] = fma(W[1][2], x2[i], fma(W[1][1], x[i], W[1][0] * id6[i]));
+            for (int i = 0; i < 6; i++) Y[i] = fma(W[1][2], x2[i], (i < 3) ? fma(W[1][1], x[i], W[1][0]) : W[1][1] * x[i]);
             bar_box_acc(x, Y, HX);
 #pragma unroll
-            for (int i = 0; i < 6; i++) Y[i] = fma(W[2][2], x2[i], fma(W[2][1], x[i], W[2][0] * id6[i]));
+            for (int i = 0; i < 6; i++) Y[i] = fma(W[2][2], x2[i], (i < 3) ? fma(W[2][1], x[i], W[2][0]) : W[2][1] * x[i]);
             bar_box_acc(x2, Y, HX);
             bar_congr_acc(side ? LB : LA, HX, d2);
         }
@@ -255,7 +290,7 @@ __device__ __noinline__ void bar_eval_t(const double *__restrict__ bd, const dou
         double uq[6], bq[6], lu[6] = {0, 0, 0, 0, 0, 0}, lb[6] = {0, 0, 0, 0, 0, 0};
 #pragma unroll
         for (int i = 0; i < 6; i++) {
-            uq[i] = fma(V[2][q], a2[i], fma(V[1][q], a[i], V[0][q] * id6[i]));
+            uq[i] = fma(V[2][q], a2[i], (i < 3) ? fma(V[1][q], a[i], V[0][q]) : V[1][q] * a[i]);
             bq[i] = (q == 0) ? id6[i] : ((q == 1) ? b[i] : b2[i]);
         }
         bar_apply_t(LA, uq, lu); bar_apply_t(LB, bq, lb);
@@ -271,12 +306,32 @@ __device__ __noinline__ void bar_eval_t(const double *__restrict__ bd, const dou
         for (int B = A; B < 6; B++) H[A][B] = fma(cf, d2[A][B], -cn * N[A] * N[B]);
 }
 
-__device__ __forceinline__ void bar_eval(const double *__restrict__ bd, const double T[6], bool want_H, double &phi_out, double N[6],
-                                         double H[6][6]) {
-    const int m = (int)bd[24];
-    if (m == 8) bar_eval_t<8>(bd, T, want_H, phi_out, N, H);        // aluminium alloys, the paper's Table 2
-    else if (m == 6) bar_eval_t<6>(bd, T, want_H, phi_out, N, H);   // steels
-    else bar_eval_t<0>(bd, T, want_H, phi_out, N, H);
+// The return map below has ONE evaluation site.  The paper's exponent (m = 8, Table 2) is inlined there, so that the
+// stress, the gradient and the Hessian stay in registers across the iteration; every other exponent goes through an
+// out-of-line copy whose arguments travel in a small block of local memory for the duration of the call only.
+struct bar_io { double T[6], N[6], H[6][6], phi; };
+__device__ __noinline__ void bar_eval_other(const double *__restrict__ bd, int m, bool want_H, bar_io &io) {
+    if (m == 6) bar_eval_t<6>(bd, m, io.T, want_H, io.phi, io.N, io.H);   // steels
+    else bar_eval_t<0>(bd, m, io.T, want_H, io.phi, io.N, io.H);
+}
+__device__ __forceinline__ void bar_eval(const double *__restrict__ bd, int m, const double T[6], bool want_H, double &phi_out,
+                                         double N[6], double H[6][6]) {
+    if (m == 8) bar_eval_t<8>(bd, m, T, want_H, phi_out, N, H);        // aluminium alloys, the paper's Table 2
+    else {
+        bar_io io;
+#pragma unroll
+        for (int i = 0; i < 6; i++) io.T[i] = T[i];
+        bar_eval_other(bd, m, want_H, io);
+        phi_out = io.phi;
+#pragma unroll
+        for (int i = 0; i < 6; i++) N[i] = io.N[i];
+        if (want_H) {
+#pragma unroll
+            for (int A = 0; A < 6; A++)
+#pragma unroll
+                for (int B = A; B < 6; B++) H[A][B] = io.H[A][B];
+        }
+    }
 }
 
 // In-place Cholesky M = L L^T of a symmetric positive definite 6x6 (lower triangle of M on entry; on exit the strict lower
@@ -319,10 +374,19 @@ __device__ __forceinline__ void chol6_solve(const double L[6][6], const double r
 // Alg. C1 steps 2-8 / Alg. C2 for Yld2004-18p at one Gauss point, material frame.
 //   ee   elastic trial strain eps - eps_p_n (tensor components)      out: T (Mandel stress), dep = dgam N (tensor components),
 //   Cep  (6x6 Mandel, upper triangle), dg, iteration count, flags
-__device__ __noinline__ void bar_return_map(const double *__restrict__ bd, double mu2, double kb, double law, double hh0,
+#ifndef BAR_RM_INLINE
+#define BAR_RM_INLINE 1
+#endif
+#if BAR_RM_INLINE
+__device__ __forceinline__
+#else
+__device__ __noinline__
+#endif
+void bar_return_map(const double *__restrict__ bd, double mu2, double kb, double law, double hh0,
                                             double hh1, double hh2, const double ee[6], double alphan, int kmax, double T[6],
                                             double dep[6], double Cep[6][6], double &dg_out, int &iters, bool &plastic,
                                             bool &nonconv) {
+    const int m_exp = (int)__ldg(bd + 24);
     const double tre = ee[0] + ee[1] + ee[2], pres = kb * tre, tm = tre * (1.0 / 3.0);
     double Ttr[6];   // Eq.(16) :160
 #pragma unroll
@@ -332,52 +396,21 @@ __device__ __noinline__ void bar_return_map(const double *__restrict__ bd, doubl
     double phi = 0.0, N[6], H[6][6];
     double tn2 = 0.0;
 #pragma unroll
-    for (int i = 0; i < 6; i++) { T[i] = Ttr[i]; dep[i] = 0.0; tn2 = fma(Ttr[i] - ((i < 3) ? pres : 0.0), Ttr[i] - ((i < 3) ? pres : 0.0), tn2); }
+    for (int i = 0; i < 6; i++) { T[i] = Ttr[i]; dep[i] = 0.0; N[i] = 0.0; tn2 = fma(Ttr[i] - ((i < 3) ? pres : 0.0), Ttr[i] - ((i < 3) ? pres : 0.0), tn2); }
+#pragma unroll
+    for (int A = 0; A < 6; A++)
+#pragma unroll
+        for (int B = 0; B < 6; B++) H[A][B] = 0.0;
     iters = 0; nonconv = false; dg_out = 0.0;
     plastic = false;
-    __syncthreads();   // the trial evaluation too is walked by the four warps together
-    if (tn2 > 0.0) {
-        bar_eval(bd, Ttr, true, phi, N, H);
-        plastic = (phi - s0) > 0.0;                     // Eq.(17)-(18) :165-172, tie -> elastic
-    }
 #pragma unroll
     for (int A = 0; A < 6; A++)
 #pragma unroll
         for (int B = A; B < 6; B++) Cep[A][B] = ((A < 3 && B < 3) ? kb - mu2 * (1.0 / 3.0) : 0.0) + ((A == B) ? mu2 : 0.0);
-    // From here on the warps of the CTA walk the (large, unrolled) evaluation code together: every Newton iteration starts at
-    // a CTA-wide barrier and the loop runs until no thread of the CTA is active (elastic points and converged points idle).
-    // ncu showed instruction fetch as the top stall (2.5 per issue) with every warp at its own place in ~60 KB of SASS.
     const double is0 = frcp(s0);
-    const double tolG = 1e-13 * fmax(1.0, sqrt(tn2) * is0);
+    const double tolG = BAR_TOLG * fmax(1.0, sqrt(tn2) * is0);
     double dg = 0.0, sy = s0, dsy = ds0, prev = INFINITY;
-#if BAR_START
-    if (plastic)
-    // Starting point (the root is unique, so any start reaches the state Alg. C2 reaches from T^tr): the trial deviator scaled
-    // back onto the yield surface, T0 = p 1 + c s^tr, with dgam from the N-component of Eq.(19): phi^tr - 2mu dgam N.N -
-    // sigma_y(alpha_n + dgam) = 0 (exact radial return for von Mises).  phi is homogeneous of degree one, so phi, N and H at
-    // T0 follow from the trial evaluation without another one: phi0 = c phi^tr, N0 = N, H0 = H / c.
-    {
-        double nn = 0.0;
-#pragma unroll
-        for (int i = 0; i < 6; i++) nn = fma(N[i], N[i], nn);
-        const double a = mu2 * nn;
-        for (int it = 0; it < 6; it++) {   // convex, decreasing: Newton from dgam = 0 approaches the root from the left
-            const double g = phi - a * dg - sy, d = g * frcp(a + dsy);
-            dg += d;
-            flow_stress(law, hh0, hh1, hh2, alphan + dg, sy, dsy);
-            if (d <= 1e-3 * dg) break;
-        }
-        const double c = sy * frcp(phi), ic = phi * frcp(sy);
-#pragma unroll
-        for (int i = 0; i < 6; i++) T[i] = (i < 3) ? fma(c, Ttr[i] - pres, pres) : c * Ttr[i];
-        phi = sy;
-#pragma unroll
-        for (int A = 0; A < 6; A++)
-#pragma unroll
-            for (int B = A; B < 6; B++) H[A][B] *= ic;
-    }
-#endif
-    double GT[6], fv, psi0;
+    double GT[6], fv = 0.0, psi0 = 0.0;
     // merit of Eq.(B2) :846 with the rows of G scaled by sigma_y(alpha_n) (T rows and f row are stresses)
 #define BAR_RESID(Tc, dgc, Nc, phic, syc, GTo, fo, psio)                                              \
     do {                                                                                               \
@@ -389,62 +422,107 @@ __device__ __noinline__ void bar_return_map(const double *__restrict__ bd, doubl
         fo = (phic - syc) * is0;                                                                       \
         psio = 0.5 * fma(fo, fo, psio);                                                                \
     } while (0)
-    BAR_RESID(T, dg, N, phi, sy, GT, fv, psi0);
-    bool conv = false, active = plastic;
-    for (int k = 0;; k++) {
-        if (active) {
-            const double nrm = sqrt(2.0 * psi0);
-            iters = k;
-            if (nrm <= tolG || (prev <= 1e-9 && nrm >= 0.5 * prev)) { conv = true; active = false; }
-            else if (k >= kmax) active = false;
-            else prev = nrm;
-        }
+    // ONE loop with ONE evaluation site of the (large, unrolled) yield function: every pass evaluates phi, N and H at the
+    // point Te and then does what its mode says -- 0: the trial state (yield test Eq.(17)-(18) :165-172, starting point);
+    // 1: a line-search point of the current Newton step (App. B Eq.(B1)-(B7) :838-867, beta = 1e-4, eta = 0.1, :871; the
+    // full step j = 0 is accepted almost always, so the Hessian is taken along with every point instead of being
+    // evaluated again at an accepted shortened step: H is then a pure output of the evaluation and nothing of it has to
+    // survive one).  A pass that leaves (T, dgam) updated ends in the Newton head: convergence test, then the direction of
+    // Eq.(24) :196.  The warps of the CTA walk the evaluation code together: every pass starts at a CTA-wide barrier and
+    // the loop runs until no thread of the CTA is active (elastic points and converged points idle); ncu showed
+    // instruction fetch as the top stall with every warp at its own place in ~60 KB of SASS.
+    double Te[6], dT[6], ddg = 0.0, dgt = 0.0, zeta = 1.0, zj = 1.0;
+#pragma unroll
+    for (int i = 0; i < 6; i++) { Te[i] = Ttr[i]; dT[i] = 0.0; GT[i] = 0.0; }
+    int mode = 0, j = 0, k = 0;
+    bool conv = false, active = tn2 > 0.0;
+    for (;;) {
         if (!__syncthreads_or(active)) break;
         if (!active) continue;
-        // Newton direction of Eq.(24) :196 on (T, dgam): M dT + 2mu N ddg = -G_T s0 ; N.dT - sigma' ddg = -f s0
-        double M[6][6], x1[6], x2[6], r1[6];
+        double phie, Ne[6];
+        bar_eval(bd, m_exp, Te, true, phie, Ne, H);
+        if (mode == 0) {
+            plastic = (phie - s0) > 0.0;                     // Eq.(17)-(18) :165-172, tie -> elastic
+            if (!plastic) { active = false; continue; }
+            phi = phie;
 #pragma unroll
-        for (int A = 0; A < 6; A++)
+            for (int i = 0; i < 6; i++) N[i] = Ne[i];
+#if BAR_START
+            // Starting point (the root is unique, so any start reaches the state Alg. C2 reaches from T^tr): the trial deviator
+            // scaled back onto the yield surface, T0 = p 1 + c s^tr, with dgam from the N-component of Eq.(19): phi^tr - 2mu dgam
+            // N.N - sigma_y(alpha_n + dgam) = 0 (exact radial return for von Mises).  phi is homogeneous of degree one, so phi, N
+            // and H at T0 follow from the trial evaluation without another one: phi0 = c phi^tr, N0 = N, H0 = H / c.
+            {
+                double nn = 0.0;
 #pragma unroll
-            for (int B = 0; B <= A; B++) M[A][B] = fma(mu2 * dg, H[B][A], (A == B) ? 1.0 : 0.0);
-        chol6(M);
+                for (int i = 0; i < 6; i++) nn = fma(N[i], N[i], nn);
+                const double a = mu2 * nn;
+                for (int it = 0; it < 6; it++) {   // convex, decreasing: Newton from dgam = 0 approaches the root from the left
+                    const double g = phi - a * dg - sy, d = g * frcp(a + dsy);
+                    dg += d;
+                    flow_stress(law, hh0, hh1, hh2, alphan + dg, sy, dsy);
+                    if (d <= 1e-3 * dg) break;
+                }
+                const double c = sy * frcp(phi), ic = phi * frcp(sy);
 #pragma unroll
-        for (int i = 0; i < 6; i++) r1[i] = GT[i] * s0;
-        chol6_solve(M, r1, x1); chol6_solve(M, N, x2);
-        double nx1 = 0.0, nx2 = 0.0;
+                for (int i = 0; i < 6; i++) T[i] = (i < 3) ? fma(c, Ttr[i] - pres, pres) : c * Ttr[i];
+                phi = sy;
 #pragma unroll
-        for (int i = 0; i < 6; i++) { nx1 = fma(N[i], x1[i], nx1); nx2 = fma(N[i], x2[i], nx2); }
-        const double ddg = (fv * s0 - nx1) * frcp(fma(mu2, nx2, dsy));
-        double dT[6];
+                for (int A = 0; A < 6; A++)
 #pragma unroll
-        for (int i = 0; i < 6; i++) dT[i] = -fma(mu2 * ddg, x2[i], x1[i]);
-        // line search, App. B Eq.(B1)-(B7) :838-867, beta = 1e-4, eta = 0.1 (:871)
-        double zeta = 1.0, Tt[6], Nt[6], GTt[6], phit, syt, dsyt, ft, psit, dgt;
-        double zj = 1.0;
-        bool accepted0 = true;
-        for (int j = 0;; j++) {
-            dgt = fma(zeta, ddg, dg);
-#pragma unroll
-            for (int i = 0; i < 6; i++) Tt[i] = fma(zeta, dT[i], T[i]);
-            bar_eval(bd, Tt, j == 0, phit, Nt, H);   // the full step is accepted almost always: take H along with it
+                    for (int B = A; B < 6; B++) H[A][B] *= ic;
+            }
+#endif
+            BAR_RESID(T, dg, N, phi, sy, GT, fv, psi0);
+        } else {
+            double syt, dsyt, GTt[6], ft, psit;
             flow_stress(law, hh0, hh1, hh2, alphan + dgt, syt, dsyt);
-            BAR_RESID(Tt, dgt, Nt, phit, syt, GTt, ft, psit);
-            accepted0 = (j == 0);
-            if (psit < (1.0 - 2.0e-4 * zeta) * psi0 || j >= 12) break;          // Eq.(B3)
-            const double zn = psi0 * frcp(psi0 + psit);                                // Eq.(B5)/(B6)
-            zeta = (j == 0) ? zn : fmax(0.1 * zj, zn);                             // Eq.(B7)
-            zj = zeta;
+            BAR_RESID(Te, dgt, Ne, phie, syt, GTt, ft, psit);
+            if (!(psit < (1.0 - 2.0e-4 * zeta) * psi0 || j >= 12)) {             // Eq.(B3) fails: shorten the step
+                const double zn = psi0 * frcp(psi0 + psit);                         // Eq.(B5)/(B6)
+                zeta = (j == 0) ? zn : fmax(0.1 * zj, zn);                          // Eq.(B7)
+                zj = zeta;
+                j++;
+                dgt = fma(zeta, ddg, dg);
+#pragma unroll
+                for (int i = 0; i < 6; i++) Te[i] = fma(zeta, dT[i], T[i]);
+                continue;
+            }
+            dg = dgt; sy = syt; dsy = dsyt; phi = phie; fv = ft; psi0 = psit;
+#pragma unroll
+            for (int i = 0; i < 6; i++) { T[i] = Te[i]; N[i] = Ne[i]; GT[i] = GTt[i]; }
         }
-        dg = dgt;
+        // ---- Newton head: (T, dgam, phi, N, H, sigma_y, G, psi) describe the current iterate k
+        {
+            const double nrm = sqrt(2.0 * psi0);
+            iters = k;
+            if (nrm <= tolG || (prev <= 1e-9 && nrm >= 0.5 * prev)) { conv = true; active = false; continue; }
+            if (k >= kmax) { active = false; continue; }
+            prev = nrm;
+        }
+        // Newton direction of Eq.(24) :196 on (T, dgam): M dT + 2mu N ddg = -G_T s0 ; N.dT - sigma' ddg = -f s0
+        {
+            double M[6][6], x1[6], x2[6], r1[6];
 #pragma unroll
-        for (int i = 0; i < 6; i++) T[i] = Tt[i];
-        if (accepted0) {
-            phi = phit;
+            for (int A = 0; A < 6; A++)
 #pragma unroll
-            for (int i = 0; i < 6; i++) N[i] = Nt[i];
-        } else bar_eval(bd, T, true, phi, N, H);
-        sy = syt; dsy = dsyt;
-        BAR_RESID(T, dg, N, phi, sy, GT, fv, psi0);
+                for (int B = 0; B <= A; B++) M[A][B] = fma(mu2 * dg, H[B][A], (A == B) ? 1.0 : 0.0);
+            chol6(M);
+#pragma unroll
+            for (int i = 0; i < 6; i++) r1[i] = GT[i] * s0;
+            chol6_solve(M, r1, x1); chol6_solve(M, N, x2);
+            double nx1 = 0.0, nx2 = 0.0;
+#pragma unroll
+            for (int i = 0; i < 6; i++) { nx1 = fma(N[i], x1[i], nx1); nx2 = fma(N[i], x2[i], nx2); }
+            ddg = (fv * s0 - nx1) * frcp(fma(mu2, nx2, dsy));
+#pragma unroll
+            for (int i = 0; i < 6; i++) dT[i] = -fma(mu2 * ddg, x2[i], x1[i]);
+        }
+        zeta = 1.0; zj = 1.0; j = 0; k++;
+        dgt = dg + ddg;
+#pragma unroll
+        for (int i = 0; i < 6; i++) Te[i] = T[i] + dT[i];
+        mode = 1;
     }
 #undef BAR_RESID
     if (!plastic) return;
