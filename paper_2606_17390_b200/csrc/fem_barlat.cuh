@@ -16,6 +16,9 @@
 
 #define FEM_BARD 32   // derived Barlat record: [0..8] N' = C'n.Pn (row-major), [9..11] c'44,c'55,c'66, [12..23] the same for C'', [24] m
 #define BAR_MMAX 16
+#ifndef BAR_LOCKSTEP
+#define BAR_LOCKSTEP 1
+#endif
 #ifndef BAR_TOLG
 #define BAR_TOLG 1e-13
 #endif
@@ -71,9 +74,9 @@ __device__ __forceinline__ void bar_apply(const double *__restrict__ L, const do
 // y (Mandel) += L^T g, g given in tensor components
 __device__ __forceinline__ void bar_apply_t(const double *__restrict__ L, const double g[6], double y[6]) {
 #pragma unroll
-    for (int j = 0; j < 3; j++) y[j] += L[j] * g[0] + L[3 + j] * g[1] + L[6 + j] * g[2];
+    for (int j = 0; j < 3; j++) y[j] = fma(L[6 + j], g[2], fma(L[3 + j], g[1], fma(L[j], g[0], y[j])));
 #pragma unroll
-    for (int i = 0; i < 3; i++) y[3 + i] += L[9 + i] * g[3 + i] * SQRT2;
+    for (int i = 0; i < 3; i++) y[3 + i] = fma(L[9 + i] * SQRT2, g[3 + i], y[3 + i]);
 }
 // c[n][p] of the Cayley-Hamilton table below is structurally zero for n < 3, p != n (X^n = unit vector n of {I, X, X^2})
 __device__ __forceinline__ constexpr bool bar_cnz(int n, int p) { return n >= 3 || n == p; }
@@ -148,10 +151,10 @@ __device__ __forceinline__ void bar_congr_acc(const double *__restrict__ L, cons
 #pragma unroll
         for (int b = a; b < 6; b++) {
             if (a < 3) {
-                double s = 0.0;
+                double s = Out[a][b];
 #pragma unroll
                 for (int c = 0; c < 3; c++) s = fma(L[3 * c + a], T1[c][b], s);
-                Out[a][b] += s;
+                Out[a][b] = s;
             } else Out[a][b] = fma(L[9 + a - 3], T1[a][b], Out[a][b]);
         }
 }
@@ -297,7 +300,7 @@ __device__ __forceinline__ void bar_eval_t(const double *__restrict__ bd, int m_
 #pragma unroll
         for (int A = 0; A < 6; A++)
 #pragma unroll
-            for (int B = A; B < 6; B++) d2[A][B] += lu[A] * lb[B] + lb[A] * lu[B];
+            for (int B = A; B < 6; B++) d2[A][B] = fma(lu[A], lb[B], fma(lb[A], lu[B], d2[A][B]));
     }
     const double cn = (m - 1.0) * frcp(phi);
 #pragma unroll
@@ -437,7 +440,11 @@ void bar_return_map(const double *__restrict__ bd, double mu2, double kb, double
     int mode = 0, j = 0, k = 0;
     bool conv = false, active = tn2 > 0.0;
     for (;;) {
+#if BAR_LOCKSTEP
         if (!__syncthreads_or(active)) break;
+#else
+        if (!__any_sync(0xffffffffu, active)) break;
+#endif
         if (!active) continue;
         double phie, Ne[6];
         bar_eval(bd, m_exp, Te, true, phie, Ne, H);
