@@ -46,6 +46,21 @@ def alg_flops_per_element(plastic_fraction):
     return 8.0 * (FLOPS_ELASTIC_POINT + FLOPS_PLASTIC_EXTRA * plastic_fraction) + FLOPS_ELEMENT_EXTRA
 
 
+# fem_assemble_barlat, frozen in round 2 (FMA = 2): elastic point 12,050 (trial evaluation of phi, N, H
+# included), plastic point 13,000 + 4,800 per Newton iteration of the return map (6x6 Cholesky, two solves, evaluation with
+# Hessian, hardening law, merit); the iteration count is the measured one (stats.iter_hist of the same call).
+FLOPS_BAR_ELASTIC_POINT = 12050.0
+FLOPS_BAR_PLASTIC_POINT = 13000.0
+FLOPS_BAR_ITERATION = 4800.0
+
+
+def alg_flops_per_element_barlat(plastic_fraction, iter_hist):
+    n_pl = float(sum(iter_hist))
+    mean_it = sum(k * v for k, v in enumerate(iter_hist)) / n_pl if n_pl > 0 else 0.0
+    return 8.0 * ((1.0 - plastic_fraction) * FLOPS_BAR_ELASTIC_POINT +
+                  plastic_fraction * (FLOPS_BAR_PLASTIC_POINT + FLOPS_BAR_ITERATION * mean_it)) + FLOPS_ELEMENT_EXTRA
+
+
 def alg_bytes_per_element(n_nodes, n_elems, nnz, per_elem_mat):
     # conn + coords,u (once per node) + hist in/out + csr values + residual + compressed slot map (+ material records)
     b = 32.0 + 2 * 24.0 * n_nodes / n_elems + 896.0 + 8.0 * nnz / n_elems + 24.0 * n_nodes / n_elems + 256.0
@@ -376,7 +391,7 @@ def run_gpu(args):
         return
 
     # ---- roofline of the dominant kernel (element kernel): FP64 ALU bound
-    fl_el = alg_flops_per_element(pfrac)
+    fl_el = alg_flops_per_element_barlat(pfrac, stats["iter_hist"]) if args.barlat else alg_flops_per_element(pfrac)
     by_el = alg_bytes_per_element(nn_g, ne_g, nnz_g, mat_np.shape[0] > 1)
     hbm_gbs, hbm_src = measured_peaks()
     dom = max(("element", "gather"), key=lambda k: kms[k])

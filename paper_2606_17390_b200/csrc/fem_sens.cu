@@ -190,7 +190,8 @@ k_sens_point(long long n_elems, const double *__restrict__ coords, const int *__
     const bool live = e_raw < n_elems;
     const long long e = live ? e_raw : n_elems - 1;   // threads past the end redo the last element (no output): every thread
                                                       // reaches the phase barriers below
-    double gth[NTHETA];
+    // the material gradient of this point goes straight to its row of sTh (it is only read after the pass)
+    double *const gth = &sTh[tid][0];
 #pragma unroll
     for (int k = 0; k < NTHETA; k++) gth[k] = 0.0;
     {
@@ -208,18 +209,18 @@ k_sens_point(long long n_elems, const double *__restrict__ coords, const int *__
         // ---- material record
         const double *mp = mat + (n_mat == 1 ? 0 : e) * FEM_NPAR;
         SMat m;
-        m.E = mp[0]; m.nu = mp[1]; m.iE = 1.0 / m.E; m.mu2 = m.E / (1.0 + m.nu); m.imu2 = (1.0 + m.nu) * m.iE;
-        m.lam = m.E * m.nu / ((1.0 + m.nu) * (1.0 - 2.0 * m.nu));
+        m.E = mp[0]; m.nu = mp[1]; m.iE = frcp(m.E); m.mu2 = m.E * frcp(1.0 + m.nu); m.imu2 = (1.0 + m.nu) * m.iE;
+        m.lam = m.E * m.nu * frcp((1.0 + m.nu) * (1.0 - 2.0 * m.nu));
         m.law = mp[8]; m.h0 = mp[9]; m.h1 = mp[10]; m.h2 = mp[11];
         {
-            const double s0 = 1.0 / (mp[2] * mp[2]), s1 = 1.0 / (mp[3] * mp[3]), s2 = 1.0 / (mp[4] * mp[4]);
+            const double s0 = frcp(mp[2] * mp[2]), s1 = frcp(mp[3] * mp[3]), s2 = frcp(mp[4] * mp[4]);
             m.p[0] = (2.0 / 3.0) * s0; m.p[1] = (2.0 / 3.0) * s1; m.p[2] = (2.0 / 3.0) * s2;
-            m.p[6] = 1.0 / (mp[5] * mp[5]); m.p[7] = 1.0 / (mp[6] * mp[6]); m.p[8] = 1.0 / (mp[7] * mp[7]);
+            m.p[6] = frcp(mp[5] * mp[5]); m.p[7] = frcp(mp[6] * mp[6]); m.p[8] = frcp(mp[7] * mp[7]);
             m.p[3] = 0.5 * (m.p[2] - m.p[0] - m.p[1]); m.p[4] = 0.5 * (m.p[0] - m.p[1] - m.p[2]); m.p[5] = 0.5 * (m.p[1] - m.p[0] - m.p[2]);
         }
         double Th[3][3];
         {
-            const double qn = 1.0 / sqrt(mp[12] * mp[12] + mp[13] * mp[13] + mp[14] * mp[14] + mp[15] * mp[15]);
+            const double qn = frsqrt(mp[12] * mp[12] + mp[13] * mp[13] + mp[14] * mp[14] + mp[15] * mp[15]);
             const double w = mp[12] * qn, x = mp[13] * qn, y = mp[14] * qn, z = mp[15] * qn;
             Th[0][0] = 1 - 2 * (y * y + z * z); Th[0][1] = 2 * (x * y - w * z);     Th[0][2] = 2 * (x * z + w * y);
             Th[1][0] = 2 * (x * y + w * z);     Th[1][1] = 1 - 2 * (x * x + z * z); Th[1][2] = 2 * (y * z - w * x);
@@ -325,7 +326,7 @@ k_sens_point(long long n_elems, const double *__restrict__ coords, const int *__
         double T[6], HT[6], N[6];
         applyE(m, ee, T);
         applyH(m, T, HT);
-        double phi = sqrt(fmax(dot6(T, HT), 0.0));
+        double phi; { const double p2 = fmax(dot6(T, HT), 0.0); phi = (p2 > 0.0) ? p2 * frsqrt(p2) : 0.0; }
         double sf, dsf;
         flow2(m, alpha_n, sf, dsf);
         double dgam = 0.0, alpha = alpha_n, kap = 0.0;
@@ -501,7 +502,7 @@ k_sens_point(long long n_elems, const double *__restrict__ coords, const int *__
 #pragma unroll
             for (int k = 0; k < 6; k++) {
                 const double rk = mp[2 + k];
-                gth[2 + k] = -2.0 * (B1[k] * iphi - c2 * B2[k]) / (rk * rk * rk);
+                gth[2 + k] = -2.0 * (B1[k] * iphi - c2 * B2[k]) * frcp(rk * rk * rk);
             }
             flow_dh(m, alpha, dh);
 #pragma unroll
@@ -517,7 +518,7 @@ k_sens_point(long long n_elems, const double *__restrict__ coords, const int *__
             double eel[6], dEnu[6];
             applyEinv(m, T, eel);
             const double op = 1.0 + m.nu, om2 = 1.0 - 2.0 * m.nu;
-            const double dmu2 = -m.E / (op * op), dlam = m.E * (1.0 + 2.0 * m.nu * m.nu) / (op * op * om2 * om2);
+            const double iop2 = frcp(op * op), dmu2 = -m.E * iop2, dlam = m.E * (1.0 + 2.0 * m.nu * m.nu) * iop2 * frcp(om2 * om2);
             const double tr = dlam * (eel[0] + eel[1] + eel[2]);
 #pragma unroll
             for (int k = 0; k < 3; k++) dEnu[k] = dmu2 * eel[k] + tr;
@@ -580,8 +581,10 @@ k_sens_point(long long n_elems, const double *__restrict__ coords, const int *__
             }
         }
     }
+    if (!live) {
 #pragma unroll
-    for (int k = 0; k < NTHETA; k++) sTh[tid][k] = live ? gth[k] : 0.0;
+        for (int k = 0; k < NTHETA; k++) gth[k] = 0.0;
+    }
     __syncthreads();
     if (live) {
         // lane q sums local node q over the 8 Gauss points, ascending
