@@ -119,24 +119,30 @@ __device__ __forceinline__ void applyDinv(const SDinv &D, const double a[6], dou
     b[3] = D.s[0] * a[3]; b[4] = D.s[1] * a[4]; b[5] = D.s[2] * a[5];
 }
 
-// sigma_flow and d sigma_flow/d alpha: Voce Eq.(10) :121, Swift (BASELINE configs)
-__device__ __forceinline__ void flow2(const SMat &m, double alpha, double &sf, double &dsf) {
+// sigma_flow and d sigma_flow/d alpha: Voce Eq.(10) :121, Swift (BASELINE configs).  aux = (exp(-h2 alpha), -) for Voce,
+// ((h1+alpha)^h2, ln(h1+alpha)) for Swift: what flow_dh needs at the same alpha.
+__device__ __forceinline__ void flow2x(const SMat &m, double alpha, double &sf, double &dsf, double aux[2]) {
     if (m.law == 0.0) {
         const double e = fexp(-m.h2 * alpha);
         sf = m.h0 + m.h1 * (1.0 - e); dsf = m.h1 * m.h2 * e;
-    } else {
-        const double b = m.h1 + alpha, pw = fexp(m.h2 * flog(b));
-        sf = m.h0 * pw; dsf = m.h0 * m.h2 * pw * frcp(b);
-    }
-}
-// d sigma_flow/d(h0,h1,h2)
-__device__ __forceinline__ void flow_dh(const SMat &m, double alpha, double dh[3]) {
-    if (m.law == 0.0) {
-        const double e = fexp(-m.h2 * alpha);
-        dh[0] = 1.0; dh[1] = 1.0 - e; dh[2] = m.h1 * alpha * e;
+        aux[0] = e; aux[1] = 0.0;
     } else {
         const double b = m.h1 + alpha, lb = flog(b), pw = fexp(m.h2 * lb);
-        dh[0] = pw; dh[1] = m.h0 * m.h2 * pw * frcp(b); dh[2] = m.h0 * pw * lb;
+        sf = m.h0 * pw; dsf = m.h0 * m.h2 * pw * frcp(b);
+        aux[0] = pw; aux[1] = lb;
+    }
+}
+__device__ __forceinline__ void flow2(const SMat &m, double alpha, double &sf, double &dsf) {
+    double aux[2];
+    flow2x(m, alpha, sf, dsf, aux);
+}
+// d sigma_flow/d(h0,h1,h2) at the alpha of the flow2x call that produced (dsf, aux)
+__device__ __forceinline__ void flow_dh(const SMat &m, double alpha, double dsf, const double aux[2], double dh[3]) {
+    if (m.law == 0.0) {
+        const double e = aux[0];
+        dh[0] = 1.0; dh[1] = 1.0 - e; dh[2] = m.h1 * alpha * e;
+    } else {
+        dh[0] = aux[0]; dh[1] = dsf; dh[2] = m.h0 * aux[0] * aux[1];   // d/dh1 of h0 (h1+alpha)^h2 equals d/dalpha
     }
 }
 
@@ -290,14 +296,14 @@ k_sens_point(long long n_elems, const double *__restrict__ coords, const int *__
                 for (int j = 0; j < 3; j++) F[i][j] *= fb_c;
         }
         SENS_SYNC(5);
-        // ---- C' = F'^T F', cyclic Jacobi (5 sweeps), Hencky strain in the material frame (Eq.(4)-(5) :92-96, reading G1)
+        // ---- C' = F'^T F', cyclic Jacobi (4 sweeps, as in k_element), Hencky strain in the material frame (Eq.(4)-(5) :92-96, reading G1)
         double R[3][3] = {{1, 0, 0}, {0, 1, 0}, {0, 0, 1}}, lm[3], gl[3];
         {
             double c00 = F[0][0] * F[0][0] + F[1][0] * F[1][0] + F[2][0] * F[2][0], c11 = F[0][1] * F[0][1] + F[1][1] * F[1][1] + F[2][1] * F[2][1];
             double c22 = F[0][2] * F[0][2] + F[1][2] * F[1][2] + F[2][2] * F[2][2], c01 = F[0][0] * F[0][1] + F[1][0] * F[1][1] + F[2][0] * F[2][1];
             double c12 = F[0][1] * F[0][2] + F[1][1] * F[1][2] + F[2][1] * F[2][2], c02 = F[0][0] * F[0][2] + F[1][0] * F[1][2] + F[2][0] * F[2][2];
 #pragma unroll 1
-            for (int sweep = 0; sweep < 5; sweep++) {
+            for (int sweep = 0; sweep < 4; sweep++) {
                 jacobi_rot(c00, c11, c01, c02, c12, R[0][0], R[0][1], R[1][0], R[1][1], R[2][0], R[2][1]);
                 jacobi_rot(c00, c22, c02, c01, c12, R[0][0], R[0][2], R[1][0], R[1][2], R[2][0], R[2][2]);
                 jacobi_rot(c11, c22, c12, c01, c02, R[0][1], R[0][2], R[1][1], R[1][2], R[2][1], R[2][2]);
@@ -327,7 +333,7 @@ k_sens_point(long long n_elems, const double *__restrict__ coords, const int *__
         applyE(m, ee, T);
         applyH(m, T, HT);
         double phi; { const double p2 = fmax(dot6(T, HT), 0.0); phi = (p2 > 0.0) ? p2 * frsqrt(p2) : 0.0; }
-        double sf, dsf;
+        double sf, dsf, faux[2] = {0.0, 0.0};
         flow2(m, alpha_n, sf, dsf);
         double dgam = 0.0, alpha = alpha_n, kap = 0.0;
         const bool plastic = phi - SW23 * sf > 0.0;
@@ -352,24 +358,29 @@ k_sens_point(long long n_elems, const double *__restrict__ coords, const int *__
                 const double f = sy * iphi - 1.0;
                 const double dk = (sy - dgam * dsy) * isy * isy;
                 const double df = dsy * iphi + (sy * iphi) * a_ * dk;
+                if (fabs(f) <= 1e-15) break;
                 if (f < 0.0) lo = dgam; else hi = dgam;
                 double nx = dgam - f * frcp(df);
-                if (!(nx > lo) || (hi > 0.0 && !(nx < hi))) nx = (hi > 0.0) ? 0.5 * (lo + hi) : 2.0 * dgam + 1e-6;
-                if (fabs(f) <= 1e-15 || fabs(nx - dgam) <= 4e-16 * nx) break;
+                const bool inside = (nx > lo) && !(hi > 0.0 && !(nx < hi));
+                if (!inside) nx = (hi > 0.0) ? 0.5 * (lo + hi) : 2.0 * dgam + 1e-6;
+                // f is smooth and monotone: once |f| <= 1e-9 the Newton step just computed lands on the root to round-off
+                // (error ~ f^2), so it is applied and the loop ends without a pass that only confirms it
+                const bool done = (inside && fabs(f) <= 1e-9) || fabs(nx - dgam) <= 4e-16 * nx;
                 dgam = nx;
+                if (done) break;
             }
             // state at the solution
             alpha = alpha_n + SW23 * dgam;
-            flow2(m, alpha, sf, dsf);
-            makeDinv(m, dgam * frcp(SW23 * sf), D);
+            flow2x(m, alpha, sf, dsf, faux);
+            kap = dgam * frcp(SW23 * sf);
+            makeDinv(m, kap, D);
             applyDinv(D, ee, T);
             applyH(m, T, HT);
             const double ph2 = dot6(T, HT), iphi = frsqrt(ph2);
             phi = ph2 * iphi;
 #pragma unroll
             for (int k = 0; k < 6; k++) N[k] = HT[k] * iphi;
-            kap = dgam * iphi;
-            makeDinv(m, kap, D);
+            // kappa = dgam / phi with phi = sigma_y at the root: D above is already E^-1 + kappa H
         } else {
 #pragma unroll
             for (int k = 0; k < 6; k++) N[k] = 0.0;
@@ -504,7 +515,7 @@ k_sens_point(long long n_elems, const double *__restrict__ coords, const int *__
                 const double rk = mp[2 + k];
                 gth[2 + k] = -2.0 * (B1[k] * iphi - c2 * B2[k]) * frcp(rk * rk * rk);
             }
-            flow_dh(m, alpha, dh);
+            flow_dh(m, alpha, dsf, faux, dh);
 #pragma unroll
             for (int k = 0; k < 3; k++) gth[8 + k] = SW23 * wf * dh[k];
         } else {
