@@ -126,6 +126,9 @@ __host__ __device__ constexpr int sidx9(int r, int c) {  // packed upper triangl
 #define SM_WQ 864   // [8]      (F-bar) w_q J_q / (Jbar V)
 #define ES_STD 564   // >= 560, = 4 mod 16: the 4 elements of a warp start in 4 different bank groups
 #define ES_FBAR 884  // >= 872, = 4 mod 16
+#ifndef JAC_SWEEPS
+#define JAC_SWEEPS 4
+#endif
 #ifndef EL_PER_CTA
 #define EL_PER_CTA 16
 #endif
@@ -576,9 +579,9 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
         double V = wq, WJ = wq * detF;
 #pragma unroll
         for (int o = 1; o < 8; o <<= 1) { V += __shfl_xor_sync(0xffffffffu, V, o); WJ += __shfl_xor_sync(0xffffffffu, WJ, o); }
-        double Jbar = WJ / V;
-        double cq = cbrt(Jbar / detF);
-        se[SM_WQ + q] = wq * detF / WJ;
+        double Jbar = WJ * frcp(V);
+        double cq = cbrt(Jbar * idt);
+        se[SM_WQ + q] = wq * detF * frcp(WJ);
 #pragma unroll
         for (int i = 0; i < 3; i++)
 #pragma unroll
@@ -596,7 +599,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
     double c02 = F[0][0] * F[0][2] + F[1][0] * F[1][2] + F[2][0] * F[2][2];
     double R[3][3] = {{1, 0, 0}, {0, 1, 0}, {0, 0, 1}};  // columns = eigenvectors n_a
 #pragma unroll 1
-    for (int sweep = 0; sweep < 4; sweep++) {
+    for (int sweep = 0; sweep < JAC_SWEEPS; sweep++) {
         jacobi_rot(c00, c11, c01, c02, c12, R[0][0], R[0][1], R[1][0], R[1][1], R[2][0], R[2][1]);
         jacobi_rot(c00, c22, c02, c01, c12, R[0][0], R[0][2], R[1][0], R[1][2], R[2][0], R[2][2]);
         jacobi_rot(c11, c22, c12, c01, c02, R[0][1], R[0][2], R[1][1], R[1][2], R[2][1], R[2][2]);
@@ -791,7 +794,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
     double phitr2 = 0.0;
 #pragma unroll
     for (int k = 0; k < 5; k++) { hc2[k] = hk[k] * ck[k] * ck[k]; phitr2 += hc2[k]; }
-    const double phitr = sqrt(phitr2);  // Eq.(11) :127
+    const double phitr = (phitr2 > 0.0) ? phitr2 * frsqrt(phitr2) : 0.0;  // Eq.(11) :127
     const double law = __ldg(md + 3), hh0 = __ldg(md + 4), hh1 = __ldg(md + 5), hh2 = __ldg(md + 6);
     // ---- S6/S7 yield test and return map in ONE loop with a single evaluation site (code size): pass 0 evaluates the
     //      trial state (dgam = 0): f_tr = phi(T_tr) - sqrt(2/3) sigma_flow(alpha_n) (Eq.(17) :165, tie -> elastic); later
@@ -802,7 +805,7 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
     double phi2 = phitr2;
     {
         double lo = 0.0, hi = INFINITY;
-        const double atol = 4.0e-16 * phitr / mu2;  // round-off floor of dgam (a strain): eps * |T| / 2mu
+        const double atol = 4.0e-16 * phitr * frcp(mu2);  // round-off floor of dgam (a strain): eps * |T| / 2mu
         bool conv = false;
         double prev_step = INFINITY, al_eval = alphan;
 #pragma unroll 1
@@ -853,8 +856,9 @@ k_element(long long n_elems, const double *__restrict__ coords, const int *__res
             const double step = fabs(dgn - dg), lim = fma(tol, dgn, atol);
             // third exit: in the quadratic regime the error left after this step is ~ (step_k / step_{k-1}^2) step_k^2;
             // when that is 100x below the step tolerance the verification pass is skipped
-            const double pred = step * step * step / (prev_step * prev_step);
-            conv = (step <= lim) || (fabs(Fv) <= 1e-12) || (step <= 1e-3 * dgn && pred <= 0.01 * lim);
+            // (pred = step^3 / prev_step^2 <= 0.01 lim, written without the division; prev_step = inf on the first pass)
+            conv = (step <= lim) || (fabs(Fv) <= 1e-12) ||
+                   (step <= 1e-3 * dgn && step * step * step <= 0.01 * lim * (prev_step * prev_step));
             prev_step = step;
             dg = dgn;
         }
