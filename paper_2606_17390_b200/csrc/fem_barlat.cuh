@@ -411,7 +411,8 @@ void bar_return_map(const double *__restrict__ bd, double mu2, double kb, double
 #pragma unroll
         for (int B = A; B < 6; B++) Cep[A][B] = ((A < 3 && B < 3) ? kb - mu2 * (1.0 / 3.0) : 0.0) + ((A == B) ? mu2 : 0.0);
     const double is0 = frcp(s0);
-    const double tolG = BAR_TOLG * fmax(1.0, sqrt(tn2) * is0);
+    // the stop test below works on squared norms (no square root in the loop): tolG2 = tolG^2, tolG = BAR_TOLG max(1, |s^tr| / sigma_0)
+    const double tolG2 = (BAR_TOLG * BAR_TOLG) * fmax(1.0, tn2 * is0 * is0);
     double dg = 0.0, sy = s0, dsy = ds0, prev = INFINITY;
     double GT[6], fv = 0.0, psi0 = 0.0;
     // merit of Eq.(B2) :846 with the rows of G scaled by sigma_y(alpha_n) (T rows and f row are stresses)
@@ -501,11 +502,11 @@ void bar_return_map(const double *__restrict__ bd, double mu2, double kb, double
         }
         // ---- Newton head: (T, dgam, phi, N, H, sigma_y, G, psi) describe the current iterate k
         {
-            const double nrm = sqrt(2.0 * psi0);
+            const double nrm2 = 2.0 * psi0;   // |G|^2; `prev` holds the previous iterate's
             iters = k;
-            if (nrm <= tolG || (prev <= 1e-9 && nrm >= 0.5 * prev)) { conv = true; active = false; continue; }
+            if (nrm2 <= tolG2 || (prev <= 1e-18 && nrm2 >= 0.25 * prev)) { conv = true; active = false; continue; }
             if (k >= kmax) { active = false; continue; }
-            prev = nrm;
+            prev = nrm2;
         }
         // Newton direction of Eq.(24) :196 on (T, dgam): M dT + 2mu N ddg = -G_T s0 ; N.dT - sigma' ddg = -f s0
         {
