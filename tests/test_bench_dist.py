@@ -54,3 +54,16 @@ def test_aggregate_single_rank():
     ms, val = bench.aggregate_over_ranks(4.0, 1_000_000, 1)
     assert ms == 4.0 and val == 2.5e8
     assert abs(bench.alg_flops_per_element(0.7) - (8 * (6850 + 1600 * 0.7) + 600)) < 1e-9
+
+
+def test_barlat_flop_model_is_the_frozen_one():
+    """DESIGN.md section 10 / profiles/r02_ncu_full.md: elastic point 12,050 flop, plastic point 13,000 + 4,800 per Newton
+    iteration; with the histogram measured at config 3 (Table 2 coefficients) that is 225.5 kflop per element."""
+    sys.path.insert(0, ROOT)
+    import bench
+    hist = [0, 1, 3160, 91383, 2699726, 2703180, 171352, 3646, 571, 54]
+    pf = sum(hist) / 8.0e6
+    assert abs(bench.alg_flops_per_element_barlat(pf, hist) - 225.5e3) < 0.2e3
+    assert bench.alg_flops_per_element_barlat(0.0, []) == 8 * 12050.0 + 600.0
+    one_it = bench.alg_flops_per_element_barlat(1.0, [0, 0, 0, 8]) - bench.alg_flops_per_element_barlat(1.0, [0, 0, 8])
+    assert abs(one_it - 8 * 4800.0) < 1e-6
