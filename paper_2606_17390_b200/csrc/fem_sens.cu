@@ -32,7 +32,7 @@
 // Phase barriers keep the warps of a CTA in the same code region so that they share instruction-cache lines (the pass is
 // ~7,000 straight-line instructions per warp; instruction fetch was the top stall without them).
 #ifndef SENS_PS_MASK
-#define SENS_PS_MASK 0x1f
+#define SENS_PS_MASK 0x0a   // re-swept after the round-2 rework: 0x0a 2.62, 0x1f 2.72, 0x0f 2.67, none 2.82 ms
 #endif
 #define SENS_SYNC(n) do { if ((SENS_PS_MASK >> (n)) & 1) __syncthreads(); } while (0)
 #ifndef SENS_CTAS
