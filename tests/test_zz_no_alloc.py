@@ -102,3 +102,34 @@ def test_static_scratch_rejects_meshes_beyond_the_maximum():
     torch.cuda.synchronize()
     assert bool((res == 7.0).all()) and bool((vals == 7.0).all()) and bool((hout == 7.0).all())
     ctx.close()
+
+
+def test_static_scratch_call_can_be_captured_in_a_cuda_graph():
+    """The reason the entry point exists: under stream capture a cudaMalloc fails the capture.  The call (counters cleared with a
+    memset node, three kernel nodes) is captured once after the set-up step and replayed on new inputs."""
+    import torch
+    cfg = synth.make_config(3, n=13)
+    ctx, u, h, mat = _setup(cfg, 0)
+    ctx.assemble_static_prepare()                      # set-up step outside the capture
+    ref1 = ctx.assemble(u, h, mat)
+    u_in = u.clone()
+    res = torch.empty_like(ref1[0]); vals = torch.empty_like(ref1[1]); hout = torch.empty_like(ref1[2])
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):                      # warm-up on the capture stream (torch's recipe)
+        ctx.assemble_static(u_in, h, mat, res, vals, hout)
+    torch.cuda.current_stream().wait_stream(side)
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=side):
+        ctx.assemble_static(u_in, h, mat, res, vals, hout)
+    for scale in (1.0, 0.4):
+        u_in.copy_(u * scale)
+        res.fill_(float("nan")); vals.fill_(float("nan")); hout.fill_(float("nan"))
+        g.replay()
+        torch.cuda.synchronize()
+        ref = ctx.assemble(u * scale, h, mat)
+        torch.cuda.synchronize()
+        assert torch.equal(res, ref[0]) and torch.equal(vals, ref[1]) and torch.equal(hout, ref[2]), scale
+    del g
+    ctx.close()
