@@ -204,6 +204,9 @@ __global__ void k_kvec(long long n_nodes, const int *__restrict__ inc_ptr, const
     if (n >= n_nodes) return;
     const int b = inc_ptr[n], m = inc_ptr[n + 1] - b, o = nb_ptr[n], len = nb_ptr[n + 1] - o;
     if (m > 8) { atomicOr(flags, 16); return; }   // this node takes the general path of the gather kernel (kvec unused)
+    // The in-kernel (fused) reduction keeps one neighbour position per lane: a node of a non-conforming mesh whose <= 8 elements do
+    // not share faces can have up to 57 neighbours.  Such a mesh takes the two-kernel schedule (its gather loops over positions).
+    if (len > 32) atomicOr(flags, 16);
     for (int p = 0; p < len; p++) kvec[o + p] = 0xffffffffu;
     for (int s = 0; s < m; s++) {
         const long long t = inc[b + s];

@@ -238,6 +238,42 @@ def test_high_valence_mesh_uses_general_gather():
     assert g["stats"]["n_plastic"] > 0
 
 
+def test_node_with_more_than_32_neighbours_takes_the_two_kernel_schedule():
+    """Eight hexes that share ONLY the centre node (a non-conforming mesh: every element has its own copies of the other
+    seven nodes): the centre node has 8 elements but 57 neighbours, more than one warp holds one position per lane for.
+    Even with the fused schedule requested the result must be the oracle's."""
+    nodes, conn = [[0.0, 0.0, 0.0]], []
+    for sx in (-1, 1):
+        for sy in (-1, 1):
+            for sz in (-1, 1):
+                loc = {}
+                for (i, j, k) in [(0, 0, 0), (1, 0, 0), (1, 1, 0), (0, 1, 0), (0, 0, 1), (1, 0, 1), (1, 1, 1), (0, 1, 1)]:
+                    if (i, j, k) == (0, 0, 0):
+                        loc[(i, j, k)] = 0
+                    else:
+                        loc[(i, j, k)] = len(nodes); nodes.append([sx * i * 1.0, sy * j * 0.9, sz * k * 1.1])
+                # hex8 node order (-,-,-),(+,-,-),(+,+,-),(-,+,-),(-,-,+),... in the element's own axes; mirrored octants are
+                # re-ordered so that det J_ref > 0
+                order = [(0, 0, 0), (1, 0, 0), (1, 1, 0), (0, 1, 0), (0, 0, 1), (1, 0, 1), (1, 1, 1), (0, 1, 1)]
+                el = [loc[o] for o in order]
+                if sx * sy * sz < 0:
+                    el = [el[0], el[3], el[2], el[1], el[4], el[7], el[6], el[5]]
+                conn.append(el)
+    coords, conn = np.array(nodes), np.array(conn, dtype=np.int32)
+    assert coords.shape[0] == 57
+    # the star comes first in a mesh large enough for the fused schedule to gather its nodes inside the element launch
+    cube = synth.make_config(3, n=22)
+    coords = np.vstack([coords + np.array([5.0, 5.0, 5.0]), cube["coords"]])
+    conn = np.vstack([conn, cube["conn"] + 57]).astype(np.int32)
+    assert conn.shape[0] > 16 * (3 * 148 + 64)
+    cfg = _mini_cfg(coords, conn, seed=11)
+    o = run_oracle(cfg, 0)
+    assert np.diff(o["row_ptr"]).max() == 3 * 57
+    for mode in (2, 1, 0):
+        g = run_gpu(cfg, 0, assembly_mode=mode)
+        compare(g, o, "star mesh mode %d" % mode)
+
+
 def test_collapsed_hex_wedge_elements():
     """A wedge written as a hex with two node pairs repeated (collapsed element): the same node appears twice in an
     element, so several local (I,K) pairs map to one CSR block; assembly must add them all (mode falls back to 0)."""
